@@ -1,0 +1,576 @@
+/*
+ * bzo.c -- CPU ORACLE (test infrastructure, see bzo.h).  Plain C, sequential fp64, one loop
+ * nest per equation.  Compile with  gcc -O2 -ffp-contract=off -fopenmp  (no FMA contraction:
+ * the sample generation must round every + - * / sqrt separately, S8c step 2).
+ *
+ * What is computed, and where it is defined:
+ *   - the 2->2 collision integral, Eq. 5, assembled per species with the 1/2
+ *     factors of Eq. 3-4;
+ *   - estimated by direct Monte Carlo, Eq. 20;
+ *   - with the symmetrical sampling of Eq. 22: one sample feeds four cells;
+ *   - |M|^2 from Table I, regulated by the gluon thermal mass of Eq. 8
+ *     evaluated with E_p = |p|;
+ *   - sampling parametrisation (p2 uniform in the box, isotropic CM direction), Philox
+ *     keying, Marsaglia unit vectors, upwind transport, massless kinematics: NS, as made
+ *     precise in SURVEY.md 8c (steps 0-7) and listed as readings in DESIGN.md.
+ *
+ * PARITY PINS (tests/test_oracle_*.py):  Philox known answers, kinematic invariants (P1),
+ * isotropy (P2), equilibrium bracket (P3), independent paper-parametrisation Monte Carlo of
+ * Eq. 17-21 (P4), labelled-vs-symmetric estimator (P5), exact number conservation (P6),
+ * Bose/Fermi closed forms for Eq. 8, 10, 11 (P7), upwind shift / Fourier factor (P8),
+ * direction of g -> q qbar conversion (P9), constant-|M|^2 closed form (P10), textbook
+ * colour/spin-averaged values and crossing relations for Table I.
+ * Per-cell values of C[f] are printed nowhere in the paper: they are pinned only through
+ * P4/P5/P10 (independent estimators agreeing), not by a published number.
+ */
+#include "bzo.h"
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define MAXS 7
+#define MAXCH 127
+#define HBARC 0.1973269804 /* GeV fm (S8c step 0) */
+#define MARSAGLIA_MAX 62   /* blk = 2 .. 63 (S8c step 1) */
+
+struct bzo_ctx {
+    bzo_grid g;
+    int S;
+    int species[MAXS];
+    double alpha_s, m_D;
+    uint32_t seed;
+    int Ns;
+    int nthreads;
+    unsigned step;
+    int Nx, Np;
+    double *f, *gross;
+    int nch;
+    bzo_channel ch[MAXCH];
+    double msq_override[BZO_N_KINDS];
+};
+
+/* ------------------------------------------------------------------ species facts */
+static int is_gluon(int id) { return id == 0; }
+static int flavour(int id) { return (id - 1) / 2; }                 /* 0 = u, 1 = d, 2 = s */
+static int antiparticle(int id) { return (id & 1) ? id + 1 : id - 1; }
+static double degeneracy(int id) { return is_gluon(id) ? 16.0 : 6.0; } /* N_g, N_q: P:78 */
+/* F = 1 + f for gluons, 1 - f for quarks and antiquarks */
+static double Fstat(int id, double f) { return is_gluon(id) ? 1.0 + f : 1.0 - f; }
+
+/* ------------------------------------------------------------------ S8c step 1: Philox4x32-10 */
+void bzo_philox4x32_10(const unsigned ctr[4], const unsigned key[2], unsigned out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += W0; k1 += W1; }
+        uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+        uint32_t h0 = (uint32_t)(p0 >> 32), l0 = (uint32_t)p0;
+        uint32_t h1 = (uint32_t)(p1 >> 32), l1 = (uint32_t)p1;
+        uint32_t n0 = h1 ^ c1 ^ k0, n1 = l1, n2 = h0 ^ c3 ^ k1, n3 = l0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* 52-bit integer plus one half, times 2^-52: in (0,1), exact (S8c step 1) */
+double bzo_uniform(unsigned a, unsigned b)
+{
+    uint64_t m = ((uint64_t)(a >> 6) << 26) | (uint64_t)(b >> 6);
+    return ((double)m + 0.5) * 2.220446049250313e-16; /* 2^-52 */
+}
+
+static void draw(const bzo_ctx* c, unsigned step, unsigned xcell, unsigned pcell, unsigned sample,
+                 unsigned blk, double* ua, double* ub)
+{
+    unsigned ctr[4] = { blk, sample, pcell, xcell }, key[2] = { c->seed, step }, w[4];
+    bzo_philox4x32_10(ctr, key, w);
+    *ua = bzo_uniform(w[0], w[1]);
+    *ub = bzo_uniform(w[2], w[3]);
+}
+
+/* ------------------------------------------------------------------ S8c step 0: grid constants */
+static double cell_width(const bzo_ctx* c) { return (c->g.pmax - c->g.pmin) / c->g.np; }
+static double cell_centre(const bzo_ctx* c, int i) { return c->g.pmin + (i + 0.5) * cell_width(c); }
+
+/* S8c step 3: cell of a momentum, -1 if any axis is outside [pmin, pmax) */
+static int bin_cell(const bzo_ctx* c, const double p[3])
+{
+    const int n = c->g.np;
+    const double dp = cell_width(c);
+    int idx[3];
+    for (int d = 0; d < 3; ++d) {
+        double q = (p[d] - c->g.pmin) / dp;
+        if (!(q >= 0.0 && q < (double)n)) return -1;
+        idx[d] = (int)floor(q);
+    }
+    return idx[0] + n * (idx[1] + n * idx[2]);
+}
+
+/* ------------------------------------------------------------------ S8c steps 1-3: one kinematic sample */
+static void gen_sample(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, bzo_sample* o)
+{
+    const int n = c->g.np;
+    const double pmin = c->g.pmin, L = c->g.pmax - c->g.pmin;
+    memset(o, 0, sizeof *o);
+    o->k = o->l = -1;
+
+    const int ipx = pcell % n, ipy = (pcell / n) % n, ipz = pcell / (n * n);
+    const double p1x = cell_centre(c, ipx), p1y = cell_centre(c, ipy), p1z = cell_centre(c, ipz);
+    const double E1 = sqrt((p1x * p1x + p1y * p1y) + p1z * p1z);
+
+    double u0, u1, u2, unused;
+    draw(c, step, xcell, pcell, sample, 0u, &u0, &u1);
+    draw(c, step, xcell, pcell, sample, 1u, &u2, &unused);
+    const double p2x = pmin + u0 * L, p2y = pmin + u1 * L, p2z = pmin + u2 * L;
+    const double E2 = sqrt((p2x * p2x + p2y * p2y) + p2z * p2z);
+    const double d12 = (p1x * p2x + p1y * p2y) + p1z * p2z;
+    const double s = 2.0 * (E1 * E2 - d12);
+
+    o->p1[0] = p1x; o->p1[1] = p1y; o->p1[2] = p1z;
+    o->p2[0] = p2x; o->p2[1] = p2y; o->p2[2] = p2z;
+    o->E1 = E1; o->E2 = E2;
+    {   /* p2 is inside by construction; clamp defensively (S8c step 3) */
+        const double dp = cell_width(c);
+        int idx[3];
+        for (int d = 0; d < 3; ++d) {
+            int q = (int)floor((o->p2[d] - pmin) / dp);
+            idx[d] = q < 0 ? 0 : (q > n - 1 ? n - 1 : q);
+        }
+        o->j = idx[0] + n * (idx[1] + n * idx[2]);
+    }
+    if (!(s > 0.0)) return; /* p1 = 0 cell, exact collinearity, rounding: contributes nothing */
+
+    /* Marsaglia (1972): uniform point on the sphere from a point in the unit disc */
+    double nx = 0.0, ny = 0.0, nz = 1.0;
+    int k;
+    for (k = 0; k < MARSAGLIA_MAX; ++k) {
+        double a, b;
+        draw(c, step, xcell, pcell, sample, 2u + (unsigned)k, &a, &b);
+        const double v1 = 2.0 * a - 1.0, v2 = 2.0 * b - 1.0;
+        const double q = v1 * v1 + v2 * v2;
+        if (q < 1.0) {
+            const double r = sqrt(1.0 - q);
+            nx = (2.0 * v1) * r; ny = (2.0 * v2) * r; nz = 1.0 - 2.0 * q;
+            break;
+        }
+    }
+    o->attempts = k + 1;
+
+    /* boost the CM pair (M/2)(1, n) back: E3 = (E + P.n)/2, p3 = [M n + P (1 + P.n/(E+M))]/2 */
+    const double Px = p1x + p2x, Py = p1y + p2y, Pz = p1z + p2z;
+    const double E = E1 + E2, M = sqrt(s);
+    const double cc = (Px * nx + Py * ny) + Pz * nz;
+    const double h = 1.0 + cc / (E + M);
+    const double p3x = 0.5 * (M * nx + Px * h), p3y = 0.5 * (M * ny + Py * h), p3z = 0.5 * (M * nz + Pz * h);
+    const double p4x = Px - p3x, p4y = Py - p3y, p4z = Pz - p3z;
+    const double E3 = 0.5 * (E + cc);
+    const double d13 = (p1x * p3x + p1y * p3y) + p1z * p3z;
+    const double t = -2.0 * (E1 * E3 - d13);
+    const double u = (-s) - t;
+
+    o->s = s; o->t = t; o->u = u; o->E3 = E3;
+    o->nhat[0] = nx; o->nhat[1] = ny; o->nhat[2] = nz;
+    o->p3[0] = p3x; o->p3[1] = p3y; o->p3[2] = p3z;
+    o->p4[0] = p4x; o->p4[1] = p4y; o->p4[2] = p4z;
+    o->k = bin_cell(c, o->p3);
+    o->l = bin_cell(c, o->p4);
+    o->flag = (o->k >= 0 && o->l >= 0); /* S9: any leg outside the box rejects the whole sample */
+}
+
+int bzo_sample_one(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, bzo_sample* out)
+{
+    if (!c || !out || xcell < 0 || xcell >= c->Nx || pcell < 0 || pcell >= c->Np || sample < 0) return -1;
+    gen_sample(c, step, xcell, pcell, sample, out);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S8c step 4: Table I */
+double bzo_msq(int kind, double s, double t, double u, double m2, double g4)
+{
+    /* SU(3): d_F = C_A = 3, C_F = 4/3, d_A = 8 */
+    const double dF = 3.0, CA = 3.0, CF = 4.0 / 3.0, dA = 8.0;
+    const double c1 = 8.0 * dF * dF * CF * CF / dA;        /* 16     */
+    const double c2 = 16.0 * dF * CF * (CF - CA / 2.0);    /* -32/3  */
+    const double c3 = 8.0 * dF * CF * CF;                  /* 128/3  */
+    const double c4 = 8.0 * dF * CF * CA;                  /* 96     */
+    const double c5 = 16.0 * dA * CA * CA;                 /* 1152   */
+    const double tt = t - m2, ut = u - m2;                 /* regulated propagators */
+    switch (kind) {
+    case BZO_M_A:    return c1 * g4 * (s * s + u * u) / (tt * tt);
+    case BZO_M_11:   return c1 * g4 * ((s * s + u * u) / (tt * tt) + (s * s + t * t) / (ut * ut))
+                          + c2 * g4 * (s * s) / (tt * ut);
+    case BZO_M_1B:   return c1 * g4 * ((s * s + u * u) / (tt * tt) + (u * u + t * t) / (s * s))
+                          + c2 * g4 * (u * u) / (tt * s);
+    case BZO_M_ANN:  return c1 * g4 * (t * t + u * u) / (s * s);
+    case BZO_M_QQGG: return c3 * g4 * (u / tt + t / ut) - c4 * g4 * (t * t + u * u) / (s * s);
+    case BZO_M_QG:   return -c3 * g4 * (u / s + s / ut) + c4 * g4 * (s * s + u * u) / (tt * tt);
+    case BZO_M_GG:   return c5 * g4 * (3.0 - s * u / (tt * tt) - s * t / (ut * ut) - t * u / (s * s));
+    }
+    return 0.0;
+}
+
+/* ------------------------------------------------------------------ S8c step 5: ordered channel table */
+static int slot_of(const bzo_ctx* c, int id)
+{
+    for (int a = 0; a < c->S; ++a) if (c->species[a] == id) return a;
+    return -1;
+}
+static void add_channel(bzo_ctx* c, int a, int b, int cc, int d, int kind, int crossed)
+{
+    bzo_channel* x = &c->ch[c->nch++];
+    x->a = a; x->b = b; x->c = cc; x->d = d; x->kind = kind; x->crossed = crossed;
+}
+static void build_channels(bzo_ctx* c)
+{
+    c->nch = 0;
+    const int g = slot_of(c, 0);
+    for (int a = 0; a < c->S; ++a) for (int b = 0; b < c->S; ++b) {
+        const int ia = c->species[a], ib = c->species[b];
+        if (is_gluon(ia) && is_gluon(ib)) {
+            add_channel(c, a, b, a, b, BZO_M_GG, 0);
+            for (int fl = 0; fl < 3; ++fl) {             /* g g -> q qbar and g g -> qbar q */
+                const int q = slot_of(c, 1 + 2 * fl), qb = slot_of(c, 2 + 2 * fl);
+                if (q < 0 || qb < 0) continue;
+                add_channel(c, a, b, q, qb, BZO_M_QQGG, 0);
+                add_channel(c, a, b, qb, q, BZO_M_QQGG, 0);
+            }
+        } else if (is_gluon(ia) || is_gluon(ib)) {
+            add_channel(c, a, b, a, b, BZO_M_QG, 0);
+            add_channel(c, a, b, b, a, BZO_M_QG, 1);
+        } else if (ia == ib) {
+            add_channel(c, a, a, a, a, BZO_M_11, 0);
+        } else if (ib == antiparticle(ia)) {
+            add_channel(c, a, b, a, b, BZO_M_1B, 0);
+            add_channel(c, a, b, b, a, BZO_M_1B, 1);
+            for (int fl = 0; fl < 3; ++fl) {             /* q qbar -> q' qbar', q' != q */
+                if (fl == flavour(ia)) continue;
+                const int q = slot_of(c, 1 + 2 * fl), qb = slot_of(c, 2 + 2 * fl);
+                if (q < 0 || qb < 0) continue;
+                add_channel(c, a, b, q, qb, BZO_M_ANN, 0);
+                add_channel(c, a, b, qb, q, BZO_M_ANN, 0);
+            }
+            if (g >= 0) add_channel(c, a, b, g, g, BZO_M_QQGG, 0);
+        } else {
+            add_channel(c, a, b, a, b, BZO_M_A, 0);
+            add_channel(c, a, b, b, a, BZO_M_A, 1);
+        }
+    }
+}
+
+int bzo_n_channels(const bzo_ctx* c) { return c ? c->nch : -1; }
+int bzo_get_channels(const bzo_ctx* c, bzo_channel* out)
+{
+    if (!c || !out) return -1;
+    memcpy(out, c->ch, (size_t)c->nch * sizeof(bzo_channel));
+    return 0;
+}
+int bzo_set_msq_override(bzo_ctx* c, int kind, double value)
+{
+    if (!c || kind < 0 || kind >= BZO_N_KINDS) return -1;
+    c->msq_override[kind] = value;
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S8c step 6: bracket and deposit */
+/* K = dtG Vp / (2048 pi^4 Ns): (1/8) symmetric reuse * 1/(2E1 2E2) [E's divided in w] *
+ * 1/(8 pi) two-body phase space * 1/(2 pi)^3 * Vp/Ns (Eq. 20) * dt/hbarc */
+static double deposit_constant(const bzo_ctx* c, double dt_fm)
+{
+    const double pi = 3.14159265358979323846;
+    const double L = c->g.pmax - c->g.pmin, Vp = (L * L) * L, dtG = dt_fm / HBARC;
+    return dtG * Vp / (2048.0 * (pi * pi * pi * pi) * c->Ns);
+}
+
+static void msq_table(const bzo_ctx* c, double s, double t, double u, double m2, double msqv[BZO_N_KINDS][2])
+{
+    const double pi = 3.14159265358979323846;
+    const double g2 = 4.0 * pi * c->alpha_s, g4 = g2 * g2;
+    for (int kind = 0; kind < BZO_N_KINDS; ++kind) {
+        if (c->msq_override[kind] >= 0.0) { msqv[kind][0] = msqv[kind][1] = c->msq_override[kind]; continue; }
+        msqv[kind][0] = bzo_msq(kind, s, t, u, m2, g4);   /* straight: M(s,t,u) */
+        msqv[kind][1] = bzo_msq(kind, s, u, t, m2, g4);   /* crossed:  M(s,u,t) */
+    }
+}
+
+double bzo_sample_channels(const bzo_ctx* c, const double* fv, double s, double t, double u,
+                           double E1, double E2, double m2, double dt_fm, double* dN, double* fwd_out)
+{
+    const int S = c->S;
+    const double w = deposit_constant(c, dt_fm) / (E1 * E2);
+    double msqv[BZO_N_KINDS][2], gross = 0.0;
+    msq_table(c, s, t, u, m2, msqv);
+    for (int x = 0; x < 4 * S; ++x) dN[x] = 0.0;
+    for (int q = 0; q < c->nch; ++q) {
+        const bzo_channel* ch = &c->ch[q];
+        const int ia = c->species[ch->a], ib = c->species[ch->b], ic = c->species[ch->c], id = c->species[ch->d];
+        const double fa = fv[0 * S + ch->a], fb = fv[1 * S + ch->b], fc = fv[2 * S + ch->c], fd = fv[3 * S + ch->d];
+        /* gain-loss bracket of Eq. 5, forward direction a b -> c d */
+        const double fwd = fa * fb * Fstat(ic, fc) * Fstat(id, fd) - Fstat(ia, fa) * Fstat(ib, fb) * fc * fd;
+        const double A = w * msqv[ch->kind][ch->crossed] * fwd;
+        dN[0 * S + ch->a] -= A; dN[1 * S + ch->b] -= A;   /* Eq. 22: -A, -A, +A, +A */
+        dN[2 * S + ch->c] += A; dN[3 * S + ch->d] += A;
+        gross += fabs(A);
+        if (fwd_out) fwd_out[q] = fwd;
+    }
+    return gross;
+}
+
+/* ------------------------------------------------------------------ Eq. 8 with E_p = |p| (S8a.1) */
+double bzo_regulator_m2(const bzo_ctx* c, const double* ft)
+{
+    const double pi = 3.14159265358979323846;
+    if (c->m_D > 0.0) return c->m_D * c->m_D;
+    const int n = c->g.np, Np = c->Np;
+    const double dp = cell_width(c), d3p = (dp * dp) * dp, g2 = 4.0 * pi * c->alpha_s;
+    const double twopi3 = (2.0 * pi) * (2.0 * pi) * (2.0 * pi);
+    double sum = 0.0;
+    for (int pc = 0; pc < Np; ++pc) {
+        const double px = cell_centre(c, pc % n), py = cell_centre(c, (pc / n) % n), pz = cell_centre(c, pc / (n * n));
+        const double E = sqrt((px * px + py * py) + pz * pz);
+        if (!(E > 0.0)) continue;                         /* S10: the p = 0 cell is skipped */
+        double bracket = 0.0;                              /* (2 g^2/d_A)(1/2)[N_g C_A f_g + N_q C_F sum f_q] / g^2 */
+        for (int a = 0; a < c->S; ++a)
+            bracket += (is_gluon(c->species[a]) ? 6.0 : 1.0) * ft[(size_t)a * Np + pc];
+        sum += d3p / (twopi3 * E) * bracket;
+    }
+    return g2 * sum;
+}
+
+/* ------------------------------------------------------------------ one spatial cell (S8c steps 1-6) */
+static void collide_tile(const bzo_ctx* c, double dt_fm, unsigned step, int xcell, const double* ft, double m2,
+                         int p_begin, int p_end, int mode, double* dN, double* gross)
+{
+    const int Np = c->Np;
+    const double K = deposit_constant(c, dt_fm);
+    bzo_sample sm;
+    double msqv[BZO_N_KINDS][2];
+    for (int i = p_begin; i < p_end; ++i) {
+        for (int smp = 0; smp < c->Ns; ++smp) {
+            gen_sample(c, step, xcell, i, smp, &sm);
+            if (!sm.flag) continue;
+            const int j = sm.j, k = sm.k, l = sm.l;
+            const double w = K / (sm.E1 * sm.E2);
+            msq_table(c, sm.s, sm.t, sm.u, m2, msqv);
+            for (int q = 0; q < c->nch; ++q) {
+                const bzo_channel* ch = &c->ch[q];
+                const int ia = c->species[ch->a], ib = c->species[ch->b], ic = c->species[ch->c], id = c->species[ch->d];
+                const size_t xa = (size_t)ch->a * Np + i, xb = (size_t)ch->b * Np + j;
+                const size_t xc = (size_t)ch->c * Np + k, xd = (size_t)ch->d * Np + l;
+                const double fa = ft[xa], fb = ft[xb], fc = ft[xc], fd = ft[xd];
+                const double fwd = fa * fb * Fstat(ic, fc) * Fstat(id, fd) - Fstat(ia, fa) * Fstat(ib, fb) * fc * fd;
+                const double A = w * msqv[ch->kind][ch->crossed] * fwd;
+                if (mode == 0) {            /* symmetric: Eq. 22 */
+                    dN[xa] -= A; dN[xb] -= A; dN[xc] += A; dN[xd] += A;
+                    if (gross) { const double g = fabs(A); gross[xa] += g; gross[xb] += g; gross[xc] += g; gross[xd] += g; }
+                } else {                    /* labelled: only the grid point itself, 1/2 instead of 1/8 */
+                    dN[xa] -= 4.0 * A;
+                    if (gross) gross[xa] += 4.0 * fabs(A);
+                }
+            }
+        }
+    }
+}
+
+int bzo_collision_tile(const bzo_ctx* c, double dt_fm, unsigned step, int xcell, const double* ft,
+                       int p_begin, int p_end, int mode, double* dN, double* gross, double* m2_out)
+{
+    if (!c || !ft || !dN || xcell < 0 || xcell >= c->Nx || p_begin < 0 || p_end > c->Np || p_begin > p_end) return -1;
+    const double m2 = bzo_regulator_m2(c, ft);
+    if (m2_out) *m2_out = m2;
+    collide_tile(c, dt_fm, step, xcell, ft, m2, p_begin, p_end, mode, dN, gross);
+    return 0;
+}
+
+int bzo_collision(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
+{
+    if (!c || !dF) return -1;
+    const int S = c->S, Np = c->Np, Nx = c->Nx;
+    const size_t tile = (size_t)S * Np, total = tile * Nx;
+    memset(dF, 0, total * sizeof(double));
+    memset(c->gross, 0, total * sizeof(double));
+    int nt = c->nthreads < 1 ? 1 : c->nthreads;
+
+    if (Nx > 1 || nt == 1) {
+        /* spatial cells are independent (Eq. 5 is local in x): same result for any thread count */
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
+        for (int x = 0; x < Nx; ++x) {
+            const double* ft = c->f + (size_t)x * tile;
+            collide_tile(c, dt_fm, step, x, ft, bzo_regulator_m2(c, ft), 0, Np, 0, dF + (size_t)x * tile, c->gross + (size_t)x * tile);
+        }
+    } else {
+        /* one spatial cell: strips of p1 cells with private sums, merged in strip order (timed run / long cases) */
+        double* priv = (double*)calloc((size_t)nt * 2 * tile, sizeof(double));
+        if (!priv) return -3;
+        const double m2 = bzo_regulator_m2(c, c->f);
+#pragma omp parallel for schedule(static, 1) num_threads(nt)
+        for (int th = 0; th < nt; ++th) {
+            const int b = (int)((long long)Np * th / nt), e = (int)((long long)Np * (th + 1) / nt);
+            collide_tile(c, dt_fm, step, 0, c->f, m2, b, e, 0, priv + (size_t)th * 2 * tile, priv + (size_t)th * 2 * tile + tile);
+        }
+        for (int th = 0; th < nt; ++th)
+            for (size_t q = 0; q < tile; ++q) {
+                dF[q] += priv[(size_t)th * 2 * tile + q];
+                c->gross[q] += priv[(size_t)th * 2 * tile + tile + q];
+            }
+        free(priv);
+    }
+    /* number units -> occupation: dF_a = dN_a / N_a */
+    for (int x = 0; x < Nx; ++x) for (int a = 0; a < S; ++a) {
+        const double Na = degeneracy(c->species[a]);
+        double* d = dF + ((size_t)x * S + a) * Np;
+        double* g = c->gross + ((size_t)x * S + a) * Np;
+        for (int pc = 0; pc < Np; ++pc) { d[pc] = d[pc] / Na; g[pc] = g[pc] / Na; }
+    }
+    return 0;
+}
+
+int bzo_get_gross(const bzo_ctx* c, double* gross)
+{
+    if (!c || !gross) return -1;
+    memcpy(gross, c->gross, (size_t)c->S * c->Np * c->Nx * sizeof(double));
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S8a.6: upwind free streaming, periodic */
+int bzo_stream(bzo_ctx* c, double dt_fm, double* dF)
+{
+    if (!c || !dF) return -1;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const int dims[3] = { c->g.nx, c->g.ny, c->g.nz };
+    const int strides[3] = { 1, c->g.nx, c->g.nx * c->g.ny };
+    const int nt = c->nthreads < 1 ? 1 : c->nthreads;
+    /* every output value is written by exactly one iteration: threads do not change the result */
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int x = 0; x < c->Nx; ++x) {
+        const int idx[3] = { x % dims[0], (x / dims[0]) % dims[1], x / (dims[0] * dims[1]) };
+        for (int a = 0; a < S; ++a) for (int pc = 0; pc < Np; ++pc) {
+            const double p[3] = { cell_centre(c, pc % n), cell_centre(c, (pc / n) % n), cell_centre(c, pc / (n * n)) };
+            const double E = sqrt((p[0] * p[0] + p[1] * p[1]) + p[2] * p[2]);
+            const double f0 = c->f[((size_t)x * S + a) * Np + pc];
+            double acc = 0.0;
+            for (int d = 0; d < 3; ++d) {
+                const double v = E > 0.0 ? p[d] / E : 0.0;      /* massless velocity p/|p| (S14); 0 at p = 0 (S10) */
+                const double cd = v * dt_fm / c->g.dx;           /* Courant number */
+                const int im = (idx[d] + dims[d] - 1) % dims[d], ip = (idx[d] + 1) % dims[d];
+                const int xm = x + (im - idx[d]) * strides[d], xp = x + (ip - idx[d]) * strides[d];
+                const double fm = c->f[((size_t)xm * S + a) * Np + pc], fp = c->f[((size_t)xp * S + a) * Np + pc];
+                acc += fmax(cd, 0.0) * (f0 - fm) + fmin(cd, 0.0) * (fp - f0);
+            }
+            dF[((size_t)x * S + a) * Np + pc] = -acc;
+        }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S8a.7: forward Euler, unsplit (Eq. 15) */
+int bzo_step(bzo_ctx* c, double dt_fm)
+{
+    if (!c) return -1;
+    const size_t total = (size_t)c->S * c->Np * c->Nx;
+    double* dFc = (double*)malloc(total * sizeof(double));
+    double* dFs = (double*)malloc(total * sizeof(double));
+    if (!dFc || !dFs) { free(dFc); free(dFs); return -3; }
+    bzo_collision(c, dt_fm, c->step, dFc);
+    bzo_stream(c, dt_fm, dFs);
+    for (size_t q = 0; q < total; ++q) c->f[q] = (c->f[q] + dFs[q]) + dFc[q];
+    c->step += 1;
+    free(dFc); free(dFs);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ S8a.8: Eq. 10 and T^00 of Eq. 11, massless */
+int bzo_moments(bzo_ctx* c, double* out)
+{
+    if (!c || !out) return -1;
+    const double pi = 3.14159265358979323846;
+    const int S = c->S, Np = c->Np, Nx = c->Nx, n = c->g.np;
+    const double dp = cell_width(c), d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * pi) * (2.0 * pi) * (2.0 * pi);
+    const double d3x = ((c->g.dx * c->g.dx) * c->g.dx) / ((HBARC * HBARC) * HBARC);   /* GeV^-3 */
+    double* tot = out + (size_t)Nx * S * 2;
+    double* m2 = tot + (size_t)S * 2;
+    for (int a = 0; a < 2 * S; ++a) tot[a] = 0.0;
+    for (int x = 0; x < Nx; ++x) {
+        for (int a = 0; a < S; ++a) {
+            const double Na = degeneracy(c->species[a]);
+            const double* fa = c->f + ((size_t)x * S + a) * Np;
+            double sn = 0.0, se = 0.0;
+            for (int pc = 0; pc < Np; ++pc) {
+                const double px = cell_centre(c, pc % n), py = cell_centre(c, (pc / n) % n), pz = cell_centre(c, pc / (n * n));
+                const double E = sqrt((px * px + py * py) + pz * pz);
+                sn += fa[pc];
+                se += E * fa[pc];
+            }
+            const double na = Na * sn * d3p / twopi3, ea = Na * se * d3p / twopi3;
+            out[((size_t)x * S + a) * 2 + 0] = na;
+            out[((size_t)x * S + a) * 2 + 1] = ea;
+            tot[2 * a + 0] += na * d3x;
+            tot[2 * a + 1] += ea * d3x;
+        }
+        m2[x] = bzo_regulator_m2(c, c->f + (size_t)x * S * Np);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ test export: sampled cells */
+int bzo_debug_samples(bzo_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int* cells, double* stu)
+{
+    if (!c || !cells || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np || pcell_begin > pcell_end) return -1;
+    bzo_sample sm;
+    size_t o = 0;
+    for (int i = pcell_begin; i < pcell_end; ++i) for (int smp = 0; smp < c->Ns; ++smp, ++o) {
+        gen_sample(c, step, xcell, i, smp, &sm);
+        cells[4 * o + 0] = sm.j; cells[4 * o + 1] = sm.k; cells[4 * o + 2] = sm.l; cells[4 * o + 3] = sm.flag;
+        if (stu) { stu[3 * o + 0] = sm.s; stu[3 * o + 1] = sm.t; stu[3 * o + 2] = sm.u; }
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ housekeeping */
+int bzo_create(const bzo_grid* g, const int* species, int n_species, double alpha_s, double m_D, bzo_ctx** out)
+{
+    if (!g || !species || !out || n_species < 1 || n_species > MAXS) return -1;
+    if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->np < 1 || !(g->pmax > g->pmin) || !(g->dx > 0.0) || !(alpha_s > 0.0)) return -1;
+    for (int a = 0; a < n_species; ++a) {
+        if (species[a] < 0 || species[a] >= MAXS) return -1;
+        if (a > 0 && species[a] <= species[a - 1]) return -1;      /* ascending, no repeats */
+    }
+    bzo_ctx* c = (bzo_ctx*)calloc(1, sizeof *c);
+    if (!c) return -3;
+    c->g = *g; c->S = n_species;
+    for (int a = 0; a < n_species; ++a) c->species[a] = species[a];
+    c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->Ns = 64; c->nthreads = 1; c->step = 0;
+    c->Nx = g->nx * g->ny * g->nz; c->Np = g->np * g->np * g->np;
+    for (int k = 0; k < BZO_N_KINDS; ++k) c->msq_override[k] = -1.0;
+    const size_t total = (size_t)c->S * c->Np * c->Nx;
+    c->f = (double*)calloc(total, sizeof(double));
+    c->gross = (double*)calloc(total, sizeof(double));
+    if (!c->f || !c->gross) { free(c->f); free(c->gross); free(c); return -3; }
+    build_channels(c);
+    *out = c;
+    return 0;
+}
+int bzo_destroy(bzo_ctx* c) { if (!c) return -1; free(c->f); free(c->gross); free(c); return 0; }
+int bzo_set_seed(bzo_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
+int bzo_set_samples(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->Ns = n; return 0; }
+int bzo_set_threads(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->nthreads = n; return 0; }
+int bzo_get_threads(const bzo_ctx* c) { return c ? c->nthreads : -1; }
+int bzo_set_step(bzo_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
+int bzo_set_f(bzo_ctx* c, const double* f)
+{
+    if (!c || !f) return -1;
+    memcpy(c->f, f, (size_t)c->S * c->Np * c->Nx * sizeof(double));
+    return 0;
+}
+int bzo_get_f(const bzo_ctx* c, double* f)
+{
+    if (!c || !f) return -1;
+    memcpy(f, c->f, (size_t)c->S * c->Np * c->Nx * sizeof(double));
+    return 0;
+}
