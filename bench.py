@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the whole hot path (bz_step + bz_moments: SURVEY.md 8a rows a1-a8) on synthetic input.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference]
+
+Default workload: BASELINE.json configs[4] (16^3 spatial x 24^3 momentum cells, 7 species, 64 samples per cell:
+3.6e9 kinematic samples and 3.96e8 phase-space values per step, 3.17 GB per copy of f) -- the largest config, the one
+north_star quotes the roofline target on; it fits one GPU.  One JSON line is printed by rank 0.
+
+  value            kinematic collision samples per second over the whole step, inputs resident in HBM
+  e2e              the same, but every step starts from HOST f (bz_set_f from pinned memory) and ends with f and the
+                   moments back on the host (bz_get_f, bz_moments)
+  roofline         the collision kernel alone (CUDA events inside libbz.so around every launch of the timed region):
+                   algorithmic gather/scatter bytes per sample x samples / duration vs measured HBM GB/s
+  cpu_baseline     the oracle as it stands, on this box's host cores, on a bounded sample of the same workload
+
+N > 1 (torchrun): the path is built for one GPU (north_star); ranks run independent replicas ("replicas only", weak
+scaling, no data-path collective) and the max over ranks of the device time is used.
+--impl reference: the oracle arm (rank 0 only), each step a bounded sample of the workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+METRIC = "collision_samples_per_sec"
+UNIT = "samples/s"
+
+
+def algorithmic_bytes_per_sample(cfg):
+    """3 random cells x S species x (8 B gather + 8 B scatter), plus the p1 cell once per N_s samples."""
+    return 48.0 * cfg.S + 16.0 * cfg.S / cfg.samples
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks and throttle reasons during the timed region (the recipe's clocks line)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt, self.proc = index, [], threading.Event(), None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([x.strip() for x in line.split(",")])
+                if self._stop_evt.is_set():
+                    break
+        except Exception:
+            pass
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.proc:
+            self.proc.terminate()
+        sm, mx, reasons = [], 0.0, set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(cfg, f0, cores, tiles_per_core=12):
+    """An oracle context holding M spatial cells of the workload (evenly spaced over the grid) as a bounded sample."""
+    from oracle import bzo
+    M = max(1, min(cfg.Nx, cores * tiles_per_core if cfg.Nx > 1 else 1))
+    xs = (np.arange(M) * (cfg.Nx // M)).astype(np.int64)
+    o = bzo.Oracle(nx=M, ny=1, nz=1, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species,
+                   alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples, threads=cores)
+    o.set_f(np.ascontiguousarray(f0[xs]))
+    desc = ("%s restricted to %d of %d spatial cells (every %d-th), all %d momentum cells x %d samples, %d species; "
+            "one full step (collision + stream + Euler + moments)" % (cfg.name, M, cfg.Nx, max(1, cfg.Nx // M), cfg.Np,
+                                                                      cfg.samples, cfg.S))
+    return o, M, desc
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    f0 = wl.initial_f(cfg)
+    o, M, desc = oracle_sample(cfg, f0, cores, tiles_per_core=6)
+    for _ in range(args.warmup):
+        o.step(cfg.dt)
+        o.moments()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(cfg.dt)
+        o.moments()
+    dt = time.perf_counter() - t0
+    samples = M * cfg.Np * cfg.samples * args.steps
+    v = samples / dt
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "note": "CPU oracle (oracle/bzo.c), each step a bounded sample: " + desc},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": o_threads(o), "kind": "oracle", "sample": desc},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "cell_updates_per_sec": M * cfg.S * cfg.Np * args.steps / dt,
+    }))
+
+
+def o_threads(o):
+    from oracle import bzo
+    return int(bzo.lib().bzo_get_threads(o._h))
+
+
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+
+    from paper_1912_04457_b200 import bz
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU path (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    g = bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
+                     species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples, device=dev)
+    f0 = wl.initial_f(cfg)
+    host_in = torch.from_numpy(f0).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    mom_host = torch.empty(2 * cfg.S * cfg.Nx + 2 * cfg.S + cfg.Nx, dtype=torch.float64).pin_memory()
+    g.set_f(host_in)
+    small = cfg.n_values * 8 * 3 < 256e6                    # footprint below ~2x L2: flush L2 between steps
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev) if small else None
+
+    def one_step():
+        g.step(cfg.dt)
+        g.moments(mom_host)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        one_step()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)
+    g.set_profile(True)
+    g.get_profile()
+    barrier()
+    ms = 0.0
+    if small:
+        for _ in range(args.steps):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            one_step()
+            e1.record()
+            torch.cuda.synchronize()
+            ms += e0.elapsed_time(e1)
+    else:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            one_step()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+    barrier()
+    coll_ms, coll_n = g.get_profile()
+    g.set_profile(False)
+    clocks = sampler.stop() if sampler else None
+    N1 = float(mom_host[2 * cfg.S * cfg.Nx:2 * cfg.S * cfg.Nx + 2 * cfg.S:2].sum())
+
+    # ---- end to end: host f in, host f and moments out, every step
+    e2e_steps = args.steps
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(e2e_steps):
+        g.set_f(host_in)
+        g.step(cfg.dt)
+        g.moments(mom_host)
+        g.get_f(host_out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_e2e = e0.elapsed_time(e1)
+    barrier()
+
+    t = torch.tensor([ms, ms_e2e, coll_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, ms_e2e, coll_ms = (float(x) for x in t.cpu())
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    samples_step = cfg.samples_per_step
+    value = world * samples_step * args.steps / (ms * 1e-3)
+    e2e_value = world * samples_step * e2e_steps / (ms_e2e * 1e-3)
+    peak, peak_src = measured_peaks()
+    bps = algorithmic_bytes_per_sample(cfg)
+    ach = bps * samples_step * coll_n / (coll_ms * 1e-3) / 1e9 if coll_ms > 0 else None
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "spatial_cells": cfg.Nx, "momentum_cells": cfg.Np, "species": cfg.S,
+                   "samples_per_cell": cfg.samples, "dt_fm": cfg.dt, "samples_per_step": samples_step,
+                   "phase_space_values": cfg.n_values, "step": "bz_step + bz_moments",
+                   "l2": "L2 flushed between steps (256 MB write)" if small else "inputs larger than L2 (3 x %.2f GB)" % (cfg.n_values * 8 / 1e9),
+                   "parallelism": "replicas only (1 GPU path)" if world > 1 else "1 GPU"},
+        "cell_updates_per_sec": world * cfg.n_values * args.steps / (ms * 1e-3),
+        "collision_kernel_samples_per_sec": samples_step * coll_n / (coll_ms * 1e-3) if coll_ms > 0 else None,
+        "collision_kernel_share_of_step": coll_ms / ms if ms > 0 else None,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": cfg.n_values * 8,
+                "d2h_bytes_per_step": cfg.n_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
+        "gpu_launches": 7 * args.steps,
+        "roofline": {"bound": "hbm", "kernel": "collide_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
+                     "frac": ach / peak if ach else None, "traffic": None, "peak_source": peak_src,
+                     "bytes_per_sample": bps, "samples_per_launch": samples_step,
+                     "ms_per_launch": coll_ms / coll_n if coll_n else None},
+        "clocks": clocks,
+        "total_particle_number": N1,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        o, M, desc = oracle_sample(cfg, f0, cores)
+        t0 = time.perf_counter()
+        o.step(cfg.dt)
+        o.moments()
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": M * cfg.Np * cfg.samples / dt, "unit": UNIT, "cores": o_threads(o), "kind": "oracle",
+                               "sample": desc, "seconds": dt}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    cfg = wl.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

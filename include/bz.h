@@ -1,0 +1,111 @@
+/*
+ * bz.h -- C ABI of the B200 (sm_100a) library for the Monte Carlo 2->2 collision term of the relativistic
+ * Boltzmann equation for gluons and 3-flavour quarks/antiquarks (arXiv:1912.04457), with upwind free
+ * streaming, a forward-Euler step and number/energy moments.
+ *
+ * Citations: "P:nnn" = line nnn of the paper text; "S8x" = SURVEY.md section 8x; "NS" = BASELINE.json
+ * north_star (which names these entry points: bz_create(grid, species, alpha_s, m_D), bz_set_f, bz_collision -> dF,
+ * bz_stream, bz_step, bz_moments).
+ *
+ * Conventions (S8b)
+ *   - every function returns int: 0 = OK, -1 bad argument, -2 CUDA error (text via bz_last_error), -3 out of
+ *     memory, -4 wrong state.  No exceptions, no aborts, nothing is printed.
+ *   - bz_ctx is opaque and OWNS its device buffers (f, f_new, the deposit scratch dN, m^2 per spatial cell,
+ *     moment partials).  The caller owns every pointer it passes in.
+ *   - pointers named *_dev are DEVICE pointers (e.g. torch tensor .data_ptr()); *_host are HOST pointers;
+ *     where a flag `on_device` is given the pointer is interpreted accordingly.
+ *   - work is enqueued on the CUDA stream given to bz_set_stream (default: the legacy default stream) and is
+ *     asynchronous unless the call says "synchronises".  A context is not thread safe.
+ *   - there is no CPU fallback: without a CUDA device bz_create fails with -2.
+ *
+ * Data layout (S8a), all fp64:
+ *   f[(xcell*S + a)*Np + pcell],  pcell = ipx + np*(ipy + np*ipz),  xcell = ix + nx*(iy + ny*iz),
+ *   a = index into the ascending list of active species ids (0 = g, 1 = u, 2 = ubar, 3 = d, 4 = dbar, 5 = s,
+ *   6 = sbar), Np = np^3, momentum cells contiguous per (spatial cell, species).
+ *   dF arrays have the same layout and size S*Nx*Np doubles.
+ */
+#ifndef BZ_H
+#define BZ_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bz_ctx bz_ctx;
+
+typedef struct {
+    int nx, ny, nz;      /* spatial cells (1,1,1 = homogeneous), periodic                      */
+    double dx;           /* spatial cell edge, fm                                               */
+    int np;              /* momentum cells per axis (2..1024)                                   */
+    double pmin, pmax;   /* momentum box edges, GeV, same on every axis; uniform cells  */
+} bz_grid;
+
+/* Create a context.  species: n_species ids in 0..6, strictly ascending.  alpha_s > 0.
+ * m_D > 0: fixed regulator mass (GeV) in the t/u propagators of Table I;
+ * m_D <= 0: regulator mass^2 = the gluon thermal mass of Eq. 8 evaluated from the current f with
+ * E_p = |p|, one value per spatial cell, recomputed at every bz_collision / bz_step (S8a.1, S7).
+ * f starts as 0, seed 0, 64 samples per cell, step counter 0. */
+int bz_create(const bz_grid* grid, const int* species, int n_species, double alpha_s, double m_D, bz_ctx** out);
+int bz_destroy(bz_ctx* ctx);
+
+int bz_set_stream(bz_ctx* ctx, void* cuda_stream);              /* cudaStream_t; NULL = default stream        */
+int bz_set_seed(bz_ctx* ctx, unsigned long long seed);          /* Philox key word 0 = low 32 bits (S8c step 1) */
+int bz_set_samples(bz_ctx* ctx, int samples_per_cell);          /* kinematic samples per (xcell, pcell) (S3)  */
+int bz_set_step(bz_ctx* ctx, unsigned step);                    /* step counter used by bz_step               */
+
+/* Copy S*Nx*Np doubles into / out of the context.  on_device != 0: f is a device pointer (async copy on the
+ * context's stream); on_device == 0: f is a host pointer and the call synchronises the stream. */
+int bz_set_f(bz_ctx* ctx, const double* f, int on_device);
+int bz_get_f(bz_ctx* ctx, double* f, int on_device);
+
+/* dF = dt * C_a[f]: Monte Carlo estimate (Eq. 20) of the 2->2 collision term (Eq. 3-5) with
+ * symmetrical sampling (Eq. 22): for every (xcell, p1 cell, sample) a Philox4x32-10 keyed (seed, step),
+ * counter (block, sample, pcell, xcell) draws p2 uniform in the box and an isotropic centre-of-mass direction
+ * (Marsaglia), p3 and p4 follow by the boost, all ordered LO QCD channels of Table I are evaluated with the
+ * Bose/Fermi gain-loss bracket of Eq. 5, and the same weight goes with - to the p1, p2 cells and with + to the
+ * p3, p4 cells (S8c steps 0-6).  dF_dev: device pointer, S*Nx*Np doubles, overwritten.  dt_fm in fm/c.
+ * Asynchronous. */
+int bz_collision(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
+
+/* dF = first-order upwind finite-volume free-streaming increment, periodic, velocity p/|p| at the momentum cell
+ * centre (flux form of the drift term of Eq. 13; S8a.6).  Asynchronous. */
+int bz_stream(bz_ctx* ctx, double dt_fm, double* dF_dev);
+
+/* One forward-Euler step (Eq. 15 unsplit; S8a.7): f <- (f + dF_stream) + dF_coll with both increments
+ * from the old f and the context's step counter as the Philox step; the counter is then incremented.
+ * Asynchronous. */
+int bz_step(bz_ctx* ctx, double dt_fm);
+
+/* Moments of the current f (Eq. 10; T^00 of Eq. 11, massless; S8a.8) written to HOST memory:
+ *   out_host[(xcell*S + a)*2 + {0,1}] = n_a(x) in GeV^3, e_a(x) in GeV^4;
+ *   then S pairs (N_a, E_a) = sum_x (n, e) dx^3/hbarc^3  (dimensionless, GeV);
+ *   then Nx values m^2(x) in GeV^2 (the regulator of S8a.1 for the current f, or m_D^2).
+ * Size 2*S*Nx + 2*S + Nx doubles.  Synchronises. */
+int bz_moments(bz_ctx* ctx, double* out_host);
+
+/* Text of the last CUDA error seen by this context ("" if none). */
+const char* bz_last_error(const bz_ctx* ctx);
+
+/* Kernel timing for the roofline report: while profiling is on (on != 0), every launch of the collision kernel is
+ * bracketed by CUDA events on the context's stream.  bz_get_profile synchronises the stream, writes the summed
+ * duration (milliseconds) and the number of launches since the last call, and clears the record. */
+int bz_set_profile(bz_ctx* ctx, int on);
+int bz_get_profile(bz_ctx* ctx, double* collide_ms_total, int* collide_launches);
+
+/* ---- test-only exports ---------------------------------------------------------------------------------- */
+/* Sampled cells of p1 cells [pcell_begin, pcell_end) of spatial cell xcell, needed for the "bit-exact sampled
+ * indices" target of NS: cells_dev[n][Ns][4] = (j, k, l, flag) int32, stu_dev[n][Ns][3] = (s, t, u) or NULL.
+ * k = l = -1 when !(s > 0); k or l = -1 when that leg leaves the box; flag = 1 iff the sample deposits. */
+int bz_debug_samples(bz_ctx* ctx, unsigned step, int xcell, int pcell_begin, int pcell_end,
+                     int* cells_dev, double* stu_dev);
+
+/* The per-sample channel algebra (S8c steps 4-6) run ON THE HOST through the same inline function the kernels
+ * use, so that its factorised form can be checked against the per-channel definition without a GPU.
+ * fv_host[slot*7 + id], slot 0..3 = cells i, j, k, l, id = species id (inactive ids ignored);
+ * out_host[slot*7 + id] = deposit in number units for weight w (= K/(E1 E2)).  Never used by the product path. */
+int bz_debug_deposit_host(const int* species, int n_species, double alpha_s, const double* fv_host,
+                          double s, double t, double u, double m2, double w, double* out_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,198 @@
+"""ctypes binding of libbz.so with the same names as include/bz.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/; there is no Python or CPU fallback: if the library
+cannot be loaded, or no CUDA device is present, the calls raise.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+LIB_PATH = _build.LIB
+_lib = None
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("dx", C.c_double),
+                ("np", C.c_int), ("pmin", C.c_double), ("pmax", C.c_double)]
+
+
+EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_f",
+           "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
+           "bz_get_profile", "bz_debug_samples",
+           "bz_debug_deposit_host")
+
+
+def lib():
+    """Load libbz.so (building it with nvcc first if it is missing or stale).  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(path)
+        vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+        L.bz_create.argtypes = [C.POINTER(Grid), ip, C.c_int, C.c_double, C.c_double, C.POINTER(vp)]
+        L.bz_destroy.argtypes = [vp]
+        L.bz_set_stream.argtypes = [vp, vp]
+        L.bz_set_seed.argtypes = [vp, C.c_ulonglong]
+        L.bz_set_samples.argtypes = [vp, C.c_int]
+        L.bz_set_step.argtypes = [vp, C.c_uint]
+        L.bz_set_f.argtypes = [vp, vp, C.c_int]
+        L.bz_get_f.argtypes = [vp, vp, C.c_int]
+        L.bz_collision.argtypes = [vp, C.c_double, C.c_uint, vp]
+        L.bz_stream.argtypes = [vp, C.c_double, vp]
+        L.bz_step.argtypes = [vp, C.c_double]
+        L.bz_moments.argtypes = [vp, vp]
+        L.bz_last_error.argtypes = [vp]
+        L.bz_last_error.restype = C.c_char_p
+        L.bz_set_profile.argtypes = [vp, C.c_int]
+        L.bz_get_profile.argtypes = [vp, dp, ip]
+        L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
+        L.bz_debug_deposit_host.argtypes = [ip, C.c_int, C.c_double, dp] + [C.c_double] * 5 + [dp]
+        _lib = L
+    return _lib
+
+
+class BzError(RuntimeError):
+    pass
+
+
+class Boltzmann:
+    """One bz_ctx.  Methods carry the names of the C entry points without the prefix."""
+
+    def __init__(self, nx=1, ny=1, nz=1, dx=1.0, np_=15, pmin=-3.0, pmax=3.0, species=(0,), alpha_s=0.3, m_D=0.0,
+                 seed=0, samples=64, device="cuda:0"):
+        self._h = None
+        self.device = torch.device(device)
+        self.species = tuple(species)
+        self.S, self.Nx, self.Np, self.Ns = len(self.species), nx * ny * nz, np_ ** 3, samples
+        self.shape = (self.Nx, self.S, self.Np)
+        self.n_values = self.Nx * self.S * self.Np
+        self._grid = Grid(nx, ny, nz, dx, np_, pmin, pmax)
+        L = lib()
+        if not torch.cuda.is_available():
+            raise BzError("no CUDA device: libbz.so has no CPU path")
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = L.bz_create(C.byref(self._grid), (C.c_int * self.S)(*self.species), self.S, alpha_s, m_D, C.byref(h))
+        if rc != 0:
+            msg = L.bz_last_error(h).decode() if h else "bad argument"
+            if h:
+                L.bz_destroy(h)
+            raise BzError("bz_create failed (%d): %s" % (rc, msg))
+        self._h = h
+        self._chk(L.bz_set_seed(h, seed), "bz_set_seed")
+        self._chk(L.bz_set_samples(h, samples), "bz_set_samples")
+        self.set_stream(torch.cuda.current_stream(self.device))
+
+    # ---- plumbing
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise BzError("%s failed (%d): %s" % (what, rc, lib().bz_last_error(self._h).decode()))
+
+    def close(self):
+        if self._h:
+            lib().bz_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev_ptr(self, t, n, dtype=torch.float64):
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.numel() == n):
+            raise ValueError("expected a contiguous CUDA %s tensor with %d elements" % (dtype, n))
+        return C.c_void_p(t.data_ptr())
+
+    def set_stream(self, stream):
+        self._chk(lib().bz_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "bz_set_stream")
+
+    def set_seed(self, seed):
+        self._chk(lib().bz_set_seed(self._h, seed), "bz_set_seed")
+
+    def set_samples(self, n):
+        self._chk(lib().bz_set_samples(self._h, n), "bz_set_samples")
+        self.Ns = n
+
+    def set_step(self, step):
+        self._chk(lib().bz_set_step(self._h, step), "bz_set_step")
+
+    # ---- state
+    def set_f(self, f):
+        """f: CUDA tensor (device copy) or CPU tensor / numpy array (host copy, synchronises)."""
+        if isinstance(f, torch.Tensor) and f.is_cuda:
+            self._chk(lib().bz_set_f(self._h, self._dev_ptr(f, self.n_values), 1), "bz_set_f")
+        else:
+            t = torch.as_tensor(f, dtype=torch.float64).contiguous()
+            if t.numel() != self.n_values:
+                raise ValueError("f has %d values, expected %d" % (t.numel(), self.n_values))
+            self._chk(lib().bz_set_f(self._h, C.c_void_p(t.data_ptr()), 0), "bz_set_f")
+
+    def get_f(self, out=None):
+        """Returns a CUDA tensor (device copy); pass a CPU tensor as `out` for a host copy (synchronises)."""
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        if out.is_cuda:
+            self._chk(lib().bz_get_f(self._h, self._dev_ptr(out, self.n_values), 1), "bz_get_f")
+        else:
+            if not (out.dtype == torch.float64 and out.is_contiguous() and out.numel() == self.n_values):
+                raise ValueError("bad host buffer")
+            self._chk(lib().bz_get_f(self._h, C.c_void_p(out.data_ptr()), 0), "bz_get_f")
+        return out
+
+    # ---- the path
+    def collision(self, dt, step, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_collision(self._h, dt, step, self._dev_ptr(out, self.n_values)), "bz_collision")
+        return out
+
+    def stream(self, dt, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_stream(self._h, dt, self._dev_ptr(out, self.n_values)), "bz_stream")
+        return out
+
+    def step(self, dt):
+        self._chk(lib().bz_step(self._h, dt), "bz_step")
+
+    def moments(self, out=None):
+        n = 2 * self.S * self.Nx + 2 * self.S + self.Nx
+        if out is None:
+            out = torch.empty(n, dtype=torch.float64)
+        self._chk(lib().bz_moments(self._h, C.c_void_p(out.data_ptr())), "bz_moments")
+        a = self.Nx * self.S * 2
+        return {"ne": out[:a].view(self.Nx, self.S, 2), "tot": out[a:a + 2 * self.S].view(self.S, 2),
+                "m2": out[a + 2 * self.S:]}
+
+    def set_profile(self, on):
+        self._chk(lib().bz_set_profile(self._h, int(bool(on))), "bz_set_profile")
+
+    def get_profile(self):
+        ms, n = C.c_double(), C.c_int()
+        self._chk(lib().bz_get_profile(self._h, C.byref(ms), C.byref(n)), "bz_get_profile")
+        return ms.value, n.value
+
+    def debug_samples(self, step, xcell, pbegin, pend, want_stu=True):
+        n = pend - pbegin
+        cells = torch.empty((n, self.Ns, 4), dtype=torch.int32, device=self.device)
+        stu = torch.empty((n, self.Ns, 3), dtype=torch.float64, device=self.device) if want_stu else None
+        self._chk(lib().bz_debug_samples(self._h, step, xcell, pbegin, pend, C.c_void_p(cells.data_ptr()),
+                                         C.c_void_p(stu.data_ptr()) if want_stu else None), "bz_debug_samples")
+        return cells, stu
+
+
+def debug_deposit_host(species, alpha_s, fv, s, t, u, m2, w):
+    """bz_debug_deposit_host: the kernels' channel algebra evaluated on the host (test aid, not a compute path)."""
+    import numpy as np
+    fv = np.ascontiguousarray(fv, dtype=np.float64).reshape(4, 7)
+    out = np.empty((4, 7), dtype=np.float64)
+    sp = (C.c_int * len(species))(*species)
+    rc = lib().bz_debug_deposit_host(sp, len(species), alpha_s, fv.ctypes.data_as(C.POINTER(C.c_double)), s, t, u, m2, w,
+                                     out.ctypes.data_as(C.POINTER(C.c_double)))
+    if rc != 0:
+        raise BzError("bz_debug_deposit_host failed (%d)" % rc)
+    return out

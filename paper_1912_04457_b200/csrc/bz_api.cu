@@ -1,0 +1,295 @@
+// bz_api.cu -- the C ABI of include/bz.h: context, argument checks, kernel sequencing.  No compute on the host
+// except the O(Np) cell-centre tables built once in bz_create.
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "bz_channels.cuh"
+#include "bz_internal.h"
+
+using namespace bz;
+
+struct bz_ctx : public bz_ctx_impl {};
+
+namespace {
+
+int fail_cuda(bz_ctx* c, cudaError_t e, const char* where)
+{
+    c->err = std::string(where) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? -3 : -2;
+}
+#define BZ_CUDA(call, where)                                  \
+    do {                                                      \
+        cudaError_t e_ = (call);                              \
+        if (e_ != cudaSuccess) return fail_cuda(c, e_, where); \
+    } while (0)
+
+double degeneracy(int id) { return id == 0 ? 16.0 : 6.0; }   // N_g = 2 x 8, N_q = 2 x 3
+
+void fill_deg(const bz_ctx* c, double (&deg)[7])
+{
+    for (int a = 0; a < 7; ++a) deg[a] = a < c->S ? degeneracy(c->species[a]) : 1.0;
+}
+
+GridConst grid_const(const bz_ctx* c)
+{
+    GridConst g;
+    g.n = c->grid.np;
+    g.pmin = c->grid.pmin;
+    g.L = c->grid.pmax - c->grid.pmin;
+    g.dp = g.L / g.n;
+    g.inv_dp = (double)g.n / g.L;
+    return g;
+}
+
+CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
+{
+    CollideParams P;
+    P.g = grid_const(c);
+    P.f = c->f; P.dN = c->dN; P.m2 = c->m2;
+    P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
+    P.seed = c->seed; P.step = step;
+    const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
+    P.K = dtG * Vp / (2048.0 * (kPi * kPi * kPi * kPi) * c->Ns);
+    const double g2 = 4.0 * kPi * c->alpha_s;
+    P.g4 = g2 * g2;
+    P.mask = c->mask;
+    for (int a = 0; a < 7; ++a) P.slot[a] = c->slot[a];
+    return P;
+}
+
+int run_collide(bz_ctx* c, double dt_fm, unsigned step)
+{
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c->profile) {
+        BZ_CUDA(cudaEventCreate(&e0), "event");
+        BZ_CUDA(cudaEventCreate(&e1), "event");
+        BZ_CUDA(cudaEventRecord(e0, c->stream), "event record");
+    }
+    BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->stream), "collide");
+    if (c->profile) {
+        BZ_CUDA(cudaEventRecord(e1, c->stream), "event record");
+        c->prof_events.push_back(e0);
+        c->prof_events.push_back(e1);
+    }
+    return 0;
+}
+
+// regulator mass^2 per spatial cell from the current f (S8a.1)
+int update_m2(bz_ctx* c)
+{
+    BZ_CUDA(launch_rowsums(c->f, c->absp, c->w_invE, c->rowsum, c->Nx * c->S, c->Np, c->stream), "rowsums");
+    const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;   // the gluon, if active, is layout index 0
+    BZ_CUDA(launch_m2(c->rowsum, c->m2, c->Nx, c->S, glue_slot_mask, 4.0 * kPi * c->alpha_s, c->m_D, c->stream), "m2");
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_s, double m_D, bz_ctx** out)
+{
+    if (!g || !species || !out || n_species < 1 || n_species > 7) return -1;
+    if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->np < 2 || g->np > 1024 || !(g->pmax > g->pmin) || !(g->dx > 0.0) ||
+        !(alpha_s > 0.0))
+        return -1;
+    if ((long long)g->nx * g->ny * g->nz > 65535) return -1;
+    for (int a = 0; a < n_species; ++a) {
+        if (species[a] < 0 || species[a] > 6) return -1;
+        if (a > 0 && species[a] <= species[a - 1]) return -1;
+    }
+    int ndev = 0;
+    bz_ctx* c = new (std::nothrow) bz_ctx();
+    if (!c) return -3;
+    *out = c;                                   // returned even on failure so that bz_last_error can be read
+    c->grid = *g; c->S = n_species; c->Nx = g->nx * g->ny * g->nz; c->Np = g->np * g->np * g->np; c->Ns = 64;
+    c->mask = 0;
+    for (int a = 0; a < 7; ++a) c->slot[a] = -1;
+    for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
+    c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
+    c->n_values = (size_t)c->Nx * c->S * c->Np;
+    c->f = c->f_new = c->dN = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = nullptr;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        c->err = "bz_create: no CUDA device (this library has no CPU path)";
+        return -2;
+    }
+    const size_t bytes = c->n_values * sizeof(double);
+    BZ_CUDA(cudaMalloc(&c->f, bytes), "cudaMalloc f");
+    BZ_CUDA(cudaMalloc(&c->f_new, bytes), "cudaMalloc f_new");
+    BZ_CUDA(cudaMalloc(&c->dN, bytes), "cudaMalloc dN");
+    BZ_CUDA(cudaMalloc(&c->m2, c->Nx * sizeof(double)), "cudaMalloc m2");
+    BZ_CUDA(cudaMalloc(&c->rowsum, (size_t)c->Nx * c->S * 3 * sizeof(double)), "cudaMalloc rowsum");
+    BZ_CUDA(cudaMalloc(&c->mom, ((size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx) * sizeof(double)), "cudaMalloc mom");
+    BZ_CUDA(cudaMalloc(&c->absp, 5 * (size_t)c->Np * sizeof(double)), "cudaMalloc tables");
+    c->w_invE = c->absp + c->Np; c->vx = c->w_invE + c->Np; c->vy = c->vx + c->Np; c->vz = c->vy + c->Np;
+    BZ_CUDA(cudaMemset(c->f, 0, bytes), "memset f");
+    BZ_CUDA(cudaMemset(c->f_new, 0, bytes), "memset f_new");
+    BZ_CUDA(cudaMemset(c->dN, 0, bytes), "memset dN");
+    // cell-centre tables: |p|, d3p/((2pi)^3 |p|) (0 at p = 0, S10), p/|p| (0 at p = 0)
+    {
+        const int n = g->np;
+        const double L = g->pmax - g->pmin, dp = L / n, d3p = (dp * dp) * dp;
+        const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
+        std::vector<double> tab(5 * (size_t)c->Np);
+        for (int pc = 0; pc < c->Np; ++pc) {
+            const double px = g->pmin + ((pc % n) + 0.5) * dp, py = g->pmin + (((pc / n) % n) + 0.5) * dp,
+                         pz = g->pmin + ((pc / (n * n)) + 0.5) * dp;
+            const double E = std::sqrt((px * px + py * py) + pz * pz);
+            tab[pc] = E;
+            tab[(size_t)c->Np + pc] = E > 0.0 ? d3p / (twopi3 * E) : 0.0;
+            tab[2 * (size_t)c->Np + pc] = E > 0.0 ? px / E : 0.0;
+            tab[3 * (size_t)c->Np + pc] = E > 0.0 ? py / E : 0.0;
+            tab[4 * (size_t)c->Np + pc] = E > 0.0 ? pz / E : 0.0;
+        }
+        BZ_CUDA(cudaMemcpy(c->absp, tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice), "upload tables");
+    }
+    return 0;
+}
+
+int bz_destroy(bz_ctx* c)
+{
+    if (!c) return -1;
+    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->dN); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
+    cudaFree(c->absp);
+    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    delete c;
+    return 0;
+}
+
+int bz_set_stream(bz_ctx* c, void* s) { if (!c) return -1; c->stream = (cudaStream_t)s; return 0; }
+int bz_set_seed(bz_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
+int bz_set_samples(bz_ctx* c, int n) { if (!c || n < 1) return -1; c->Ns = n; return 0; }
+int bz_set_step(bz_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
+const char* bz_last_error(const bz_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int bz_set_f(bz_ctx* c, const double* f, int on_device)
+{
+    if (!c || !f) return -1;
+    if (!c->f) return -4;
+    BZ_CUDA(cudaMemcpyAsync(c->f, f, c->n_values * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                            c->stream), "bz_set_f copy");
+    if (!on_device) BZ_CUDA(cudaStreamSynchronize(c->stream), "bz_set_f sync");
+    return 0;
+}
+
+int bz_get_f(bz_ctx* c, double* f, int on_device)
+{
+    if (!c || !f) return -1;
+    if (!c->f) return -4;
+    BZ_CUDA(cudaMemcpyAsync(f, c->f, c->n_values * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                            c->stream), "bz_get_f copy");
+    if (!on_device) BZ_CUDA(cudaStreamSynchronize(c->stream), "bz_get_f sync");
+    return 0;
+}
+
+int bz_collision(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
+{
+    if (!c || !dF_dev) return -1;
+    if (!c->f) return -4;
+    if (int rc = update_m2(c)) return rc;
+    if (int rc = run_collide(c, dt_fm, step)) return rc;
+    double deg[7];
+    fill_deg(c, deg);
+    BZ_CUDA(launch_finalize(c->dN, dF_dev, c->Nx, c->S, c->Np, deg, c->stream), "finalize");
+    return 0;
+}
+
+static TransportParams transport_params(const bz_ctx* c, double dt_fm, double* out)
+{
+    TransportParams T;
+    T.f = c->f; T.dN = c->dN; T.out = out; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
+    T.nx = c->grid.nx; T.ny = c->grid.ny; T.nz = c->grid.nz; T.S = c->S; T.Np = c->Np;
+    T.cfl = dt_fm / c->grid.dx;
+    fill_deg(c, T.inv_deg);
+    return T;
+}
+
+int bz_stream(bz_ctx* c, double dt_fm, double* dF_dev)
+{
+    if (!c || !dF_dev) return -1;
+    if (!c->f) return -4;
+    BZ_CUDA(launch_transport(transport_params(c, dt_fm, dF_dev), 0, c->stream), "stream");
+    return 0;
+}
+
+int bz_step(bz_ctx* c, double dt_fm)
+{
+    if (!c) return -1;
+    if (!c->f) return -4;
+    if (int rc = update_m2(c)) return rc;
+    if (int rc = run_collide(c, dt_fm, c->step)) return rc;
+    BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 1, c->stream), "stream+euler");
+    double* t = c->f; c->f = c->f_new; c->f_new = t;
+    c->step += 1;
+    return 0;
+}
+
+int bz_moments(bz_ctx* c, double* out_host)
+{
+    if (!c || !out_host) return -1;
+    if (!c->f) return -4;
+    if (int rc = update_m2(c)) return rc;
+    double deg[7];
+    fill_deg(c, deg);
+    const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
+    const double d3x = ((c->grid.dx * c->grid.dx) * c->grid.dx) / ((kHbarc * kHbarc) * kHbarc);
+    BZ_CUDA(launch_moments(c->rowsum, c->m2, c->mom, c->Nx, c->S, deg, d3p / twopi3, d3x, c->stream), "moments");
+    const size_t cnt = (size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx;
+    BZ_CUDA(cudaMemcpyAsync(out_host, c->mom, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "moments copy");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "moments sync");
+    return 0;
+}
+
+int bz_set_profile(bz_ctx* c, int on) { if (!c) return -1; c->profile = on != 0; return 0; }
+
+int bz_get_profile(bz_ctx* c, double* ms_total, int* launches)
+{
+    if (!c || !ms_total || !launches) return -1;
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "profile sync");
+    double tot = 0.0;
+    for (size_t q = 0; q + 1 < c->prof_events.size(); q += 2) {
+        float ms = 0.f;
+        BZ_CUDA(cudaEventElapsedTime(&ms, c->prof_events[q], c->prof_events[q + 1]), "event elapsed");
+        tot += ms;
+    }
+    *ms_total = tot;
+    *launches = (int)(c->prof_events.size() / 2);
+    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    c->prof_events.clear();
+    return 0;
+}
+
+int bz_debug_samples(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int* cells_dev, double* stu_dev)
+{
+    if (!c || !cells_dev || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np || pcell_begin > pcell_end)
+        return -1;
+    if (!c->f) return -4;
+    BZ_CUDA(launch_debug_samples(collide_params(c, 1.0, step), xcell, pcell_begin, pcell_end, cells_dev, stu_dev, c->stream),
+            "debug_samples");
+    return 0;
+}
+
+int bz_debug_deposit_host(const int* species, int n_species, double alpha_s, const double* fv, double s, double t, double u,
+                          double m2, double w, double* out)
+{
+    if (!species || !fv || !out || n_species < 1 || n_species > 7) return -1;
+    unsigned mask = 0;
+    for (int a = 0; a < n_species; ++a) {
+        if (species[a] < 0 || species[a] > 6) return -1;
+        mask |= 1u << species[a];
+    }
+    double f[4][7], d[4][7];
+    for (int sl = 0; sl < 4; ++sl)
+        for (int id = 0; id < 7; ++id) f[sl][id] = ((mask >> id) & 1u) ? fv[sl * 7 + id] : 0.0;
+    const double g2 = 4.0 * kPi * alpha_s;
+    const MsqSet M = msq_set<true, true>(s, t, u, m2, g2 * g2 * w);
+    deposit<-1>(mask, f[0], f[1], f[2], f[3], M, d[0], d[1], d[2], d[3]);
+    for (int sl = 0; sl < 4; ++sl)
+        for (int id = 0; id < 7; ++id) out[sl * 7 + id] = d[sl][id];
+    return 0;
+}
+
+}  // extern "C"

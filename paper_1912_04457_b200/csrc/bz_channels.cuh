@@ -1,0 +1,190 @@
+// bz_channels.cuh -- |M|^2 of Table I and the per-sample channel algebra (S8c steps 4-6).
+//
+// The 127 ordered channels of the 7-species mixture (S8c step 5) are not looped over.  Every channel's bracket
+// (Eq. 5) factorises into an "incoming" and an "outgoing" pair product, and the channels fall into three
+// families that share the cell routing of their species:
+//   t-family  a: i->k, b: j->l   (straight elastic, incl. gg->gg and q q->q q)      |M|^2(s,t,u)
+//   u-family  a: i->l, b: j->k   (crossed elastic)                                   |M|^2(s,u,t)
+//   s-family  (a,abar) or (g,g) at (i,j)  ->  (c,cbar) or (g,g) at (k,l)             annihilation / pair creation
+// Within a family the sum over the partner species is a short dot product with at most four distinct |M|^2
+// values, so one sample costs O(S) fused multiply-adds instead of 127 x 12.  The result differs from the
+// channel-by-channel sum only by fp64 rounding order (bounded by the gross sum of S16).
+//
+// Arrays are indexed by species id 0..6; entries of inactive species must hold f = 0 and are masked out where
+// a vanishing f alone does not switch a channel off (pair creation into an absent flavour).
+#pragma once
+
+#if defined(__CUDACC__)
+#define BZ_HD __host__ __device__ __forceinline__
+#else
+#define BZ_HD inline
+#endif
+
+namespace bz {
+
+constexpr int kMaxSpecies = 7;
+
+// the <= 10 distinct values one kinematic sample needs, each already multiplied by g^4 * w
+struct MsqSet {
+    double gg;            // gg -> gg
+    double qqgg;          // q qbar <-> g g            (t <-> u symmetric)
+    double qg_t, qg_u;    // q g -> q g, straight / crossed
+    double m11;           // q1 q1 -> q1 q1             (t <-> u symmetric)
+    double m1b_t, m1b_u;  // q1 q1bar -> q1 q1bar, straight / crossed
+    double ann;           // q1 q1bar -> q2 q2bar       (t <-> u symmetric)
+    double a_t, a_u;      // q1 q2 -> q1 q2 (different flavours), straight / crossed
+};
+
+// Table I with the regulated propagators tt = t - m^2, ut = u - m^2; SU(3): 8 dF^2 CF^2/dA = 16,
+// 16 dF CF (CF - CA/2) = -32/3, 8 dF CF^2 = 128/3, 8 dF CF CA = 96, 16 dA CA^2 = 1152.
+template <bool kGlue, bool kQuark>
+BZ_HD MsqSet msq_set(double s, double t, double u, double m2, double g4w)
+{
+    MsqSet M = {};
+    const double it = 1.0 / (t - m2), iu = 1.0 / (u - m2), is = 1.0 / s;
+    const double s2 = s * s, t2 = t * t, u2 = u * u;
+    const double it2 = it * it, iu2 = iu * iu, is2 = is * is;
+    const double c16 = 16.0 * g4w, c323 = (32.0 / 3.0) * g4w, c1283 = (128.0 / 3.0) * g4w;
+    const double at = c16 * (s2 + u2) * it2;       // M_A(s,t,u)
+    const double au = c16 * (s2 + t2) * iu2;       // M_A(s,u,t)
+    const double ann = c16 * (t2 + u2) * is2;      // M_ann
+    if (kQuark) {
+        M.a_t = at;
+        M.a_u = au;
+        M.ann = ann;
+        M.m11 = (at + au) - c323 * s2 * (it * iu);
+        M.m1b_t = (at + ann) - c323 * u2 * (it * is);
+        M.m1b_u = (au + ann) - c323 * t2 * (iu * is);
+    }
+    if (kGlue && kQuark) {
+        M.qqgg = c1283 * (u * it + t * iu) - 6.0 * ann;
+        M.qg_t = 6.0 * at - c1283 * (u * is + s * iu);
+        M.qg_u = 6.0 * au - c1283 * (t * is + s * it);
+    }
+    if (kGlue) M.gg = 1152.0 * g4w * (3.0 - s * u * it2 - s * t * iu2 - t * u * is2);
+    return M;
+}
+
+// Deposits of one sample in number units: dI, dJ, dK, dL for the cells of p1, p2, p3, p4 (Eq. 22, P:201:
+// every channel adds -A, -A, +A, +A).  kMask >= 0: compile-time species mask; kMask < 0: use rt_mask.
+template <int kMask>
+BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7], const double (&fk)[7],
+                   const double (&fl)[7], const MsqSet& M, double (&dI)[7], double (&dJ)[7], double (&dK)[7],
+                   double (&dL)[7])
+{
+    const unsigned mask = kMask >= 0 ? (unsigned)kMask : rt_mask;
+#define BZ_ON(a) (((mask) >> (a)) & 1u)
+    const bool glue = BZ_ON(0);
+    // F = 1 + f (gluon), 1 - f (quark, antiquark)
+    double Fi[7], Fj[7], Fk[7], Fl[7];
+    Fi[0] = 1.0 + fi[0]; Fj[0] = 1.0 + fj[0]; Fk[0] = 1.0 + fk[0]; Fl[0] = 1.0 + fl[0];
+#pragma unroll
+    for (int a = 1; a < 7; ++a) { Fi[a] = 1.0 - fi[a]; Fj[a] = 1.0 - fj[a]; Fk[a] = 1.0 - fk[a]; Fl[a] = 1.0 - fl[a]; }
+#pragma unroll
+    for (int a = 0; a < 7; ++a) dI[a] = dJ[a] = dK[a] = dL[a] = 0.0;
+
+    // ------------------------------------------------------------------ t-family: a i->k, b j->l
+    {
+        double X[7], Y[7], Z[7], W[7], Xf[3], Yf[3], Zf[3], Wf[3];
+#pragma unroll
+        for (int a = 0; a < 7; ++a) {
+            X[a] = fi[a] * Fk[a]; Y[a] = Fi[a] * fk[a];
+            Z[a] = fj[a] * Fl[a]; W[a] = Fj[a] * fl[a];
+        }
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            Xf[p] = X[1 + 2 * p] + X[2 + 2 * p]; Yf[p] = Y[1 + 2 * p] + Y[2 + 2 * p];
+            Zf[p] = Z[1 + 2 * p] + Z[2 + 2 * p]; Wf[p] = W[1 + 2 * p] + W[2 + 2 * p];
+        }
+        if (glue) {
+            const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
+            const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
+            const double T = X[0] * (M.gg * Z[0] + M.qg_t * Zq) - Y[0] * (M.gg * W[0] + M.qg_t * Wq);
+            const double U = Z[0] * (M.gg * X[0] + M.qg_t * Xq) - W[0] * (M.gg * Y[0] + M.qg_t * Yq);
+            dI[0] -= T; dK[0] += T; dJ[0] -= U; dL[0] += U;
+        }
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            if (!BZ_ON(a)) continue;
+            const int p = (a - 1) >> 1, ab = (a & 1) ? a + 1 : a - 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
+            const double ZM = ((M.qg_t * Z[0] + M.m11 * Z[a]) + M.m1b_t * Z[ab]) + M.a_t * (Zf[p1] + Zf[p2]);
+            const double WM = ((M.qg_t * W[0] + M.m11 * W[a]) + M.m1b_t * W[ab]) + M.a_t * (Wf[p1] + Wf[p2]);
+            const double XM = ((M.qg_t * X[0] + M.m11 * X[a]) + M.m1b_t * X[ab]) + M.a_t * (Xf[p1] + Xf[p2]);
+            const double YM = ((M.qg_t * Y[0] + M.m11 * Y[a]) + M.m1b_t * Y[ab]) + M.a_t * (Yf[p1] + Yf[p2]);
+            const double T = X[a] * ZM - Y[a] * WM;
+            const double U = Z[a] * XM - W[a] * YM;
+            dI[a] -= T; dK[a] += T; dJ[a] -= U; dL[a] += U;
+        }
+    }
+    // ------------------------------------------------------------------ u-family: a i->l, b j->k
+    {
+        double X[7], Y[7], Z[7], W[7], Xf[3], Yf[3], Zf[3], Wf[3];
+#pragma unroll
+        for (int a = 0; a < 7; ++a) {
+            X[a] = fi[a] * Fl[a]; Y[a] = Fi[a] * fl[a];
+            Z[a] = fj[a] * Fk[a]; W[a] = Fj[a] * fk[a];
+        }
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            Xf[p] = X[1 + 2 * p] + X[2 + 2 * p]; Yf[p] = Y[1 + 2 * p] + Y[2 + 2 * p];
+            Zf[p] = Z[1 + 2 * p] + Z[2 + 2 * p]; Wf[p] = W[1 + 2 * p] + W[2 + 2 * p];
+        }
+        if (glue) {
+            const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
+            const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
+            const double T = M.qg_u * (X[0] * Zq - Y[0] * Wq);
+            const double U = M.qg_u * (Z[0] * Xq - W[0] * Yq);
+            dI[0] -= T; dL[0] += T; dJ[0] -= U; dK[0] += U;
+        }
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            if (!BZ_ON(a)) continue;
+            const int p = (a - 1) >> 1, ab = (a & 1) ? a + 1 : a - 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
+            const double ZM = (M.qg_u * Z[0] + M.m1b_u * Z[ab]) + M.a_u * (Zf[p1] + Zf[p2]);
+            const double WM = (M.qg_u * W[0] + M.m1b_u * W[ab]) + M.a_u * (Wf[p1] + Wf[p2]);
+            const double XM = (M.qg_u * X[0] + M.m1b_u * X[ab]) + M.a_u * (Xf[p1] + Xf[p2]);
+            const double YM = (M.qg_u * Y[0] + M.m1b_u * Y[ab]) + M.a_u * (Yf[p1] + Yf[p2]);
+            const double T = X[a] * ZM - Y[a] * WM;
+            const double U = Z[a] * XM - W[a] * YM;
+            dI[a] -= T; dL[a] += T; dJ[a] -= U; dK[a] += U;
+        }
+    }
+    // ------------------------------------------------------------------ s-family: pairs at (i,j) -> pairs at (k,l)
+    {
+        // quark "state a": a at the first cell of the pair, abar at the second; valid only if both are active
+        double In[7], Ib[7], Out[7], Ob[7], Inf[3], Ibf[3], Outf[3], Obf[3];
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const bool ok = BZ_ON(a) && BZ_ON(ab);
+            In[a] = ok ? fi[a] * fj[ab] : 0.0;  Ib[a] = ok ? Fi[a] * Fj[ab] : 0.0;
+            Out[a] = ok ? Fk[a] * Fl[ab] : 0.0; Ob[a] = ok ? fk[a] * fl[ab] : 0.0;
+        }
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            Inf[p] = In[1 + 2 * p] + In[2 + 2 * p];    Ibf[p] = Ib[1 + 2 * p] + Ib[2 + 2 * p];
+            Outf[p] = Out[1 + 2 * p] + Out[2 + 2 * p]; Obf[p] = Ob[1 + 2 * p] + Ob[2 + 2 * p];
+        }
+        const double Ing = glue ? fi[0] * fj[0] : 0.0, Ibg = glue ? Fi[0] * Fj[0] : 0.0;
+        const double Outg = glue ? Fk[0] * Fl[0] : 0.0, Obg = glue ? fk[0] * fl[0] : 0.0;
+        if (glue) {
+            const double Sg = M.qqgg * (Ing * ((Outf[0] + Outf[1]) + Outf[2]) - Ibg * ((Obf[0] + Obf[1]) + Obf[2]));
+            const double Rg = M.qqgg * (Outg * ((Inf[0] + Inf[1]) + Inf[2]) - Obg * ((Ibf[0] + Ibf[1]) + Ibf[2]));
+            dI[0] -= Sg; dJ[0] -= Sg; dK[0] += Rg; dL[0] += Rg;
+        }
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            if (!(BZ_ON(a) && BZ_ON(ab))) continue;
+            const int p = (a - 1) >> 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
+            const double S = In[a] * (M.qqgg * Outg + M.ann * (Outf[p1] + Outf[p2]))
+                           - Ib[a] * (M.qqgg * Obg + M.ann * (Obf[p1] + Obf[p2]));
+            const double R = Out[a] * (M.qqgg * Ing + M.ann * (Inf[p1] + Inf[p2]))
+                           - Ob[a] * (M.qqgg * Ibg + M.ann * (Ibf[p1] + Ibf[p2]));
+            dI[a] -= S; dJ[ab] -= S; dK[a] += R; dL[ab] += R;
+        }
+    }
+#undef BZ_ON
+}
+
+}  // namespace bz

@@ -1,0 +1,77 @@
+// bz_internal.h -- context and kernel-launcher declarations shared by the translation units of libbz.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/bz.h"
+#include "bz_sample.cuh"
+
+namespace bz {
+
+constexpr double kHbarc = 0.1973269804;   // GeV fm (S8c step 0)
+constexpr double kPi = 3.14159265358979323846;
+
+struct CollideParams {
+    GridConst g;
+    const double* f;      // [Nx][S][Np]
+    double* dN;           // [Nx][S][Np] deposit scratch in number units, zero on entry
+    const double* m2;     // [Nx] regulator mass^2
+    int S, Np, Nx, Ns;
+    uint32_t seed, step;
+    double K;             // dtG Vp / (2048 pi^4 Ns)                       (S8c step 0)
+    double g4;            // (4 pi alpha_s)^2
+    unsigned mask;        // bit id set <=> species id active
+    int slot[7];          // species id -> index a in the layout (or -1)
+};
+
+struct TransportParams {
+    const double* f;      // old f
+    double* dN;           // collision deposits (number units), reset to 0 when consumed
+    double* out;          // f_new or dF
+    const double* vx; const double* vy; const double* vz;   // [Np] p/|p| at the cell centre (0 at p = 0)
+    int nx, ny, nz, S, Np;
+    double cfl;           // dt / dx
+    double inv_deg[7];    // per layout index a: 1/N_a is NOT used (division kept exact); holds N_a
+};
+
+struct bz_ctx_impl {
+    bz_grid grid;
+    int S, Nx, Np, Ns;
+    int species[7], slot[7];
+    unsigned mask;
+    double alpha_s, m_D;
+    uint32_t seed, step;
+    cudaStream_t stream;
+    size_t n_values;
+    double *f, *f_new, *dN;          // device, n_values each
+    double *m2;                      // device [Nx]
+    double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|)
+    double *mom;                     // device [2*S*Nx + 2*S + Nx]
+    double *absp, *w_invE, *vx, *vy, *vz;   // device [Np] tables
+    std::string err;
+    bool profile;
+    std::vector<cudaEvent_t> prof_events;   // start/stop pairs around collide launches
+};
+
+// launchers (each returns the cudaError_t of the launch)
+cudaError_t launch_collide(const CollideParams& P, cudaStream_t st);
+cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin, int p_end, int* cells, double* stu,
+                                 cudaStream_t st);
+// out = dN / N_a, dN = 0
+cudaError_t launch_finalize(double* dN, double* dF, int Nx, int S, int Np, const double* deg, cudaStream_t st);
+// mode 0: out = dF_stream;  mode 1: out = (f + dF_stream) + dN/N_a and dN = 0
+cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st);
+// rowsum[x][a][0..2]
+cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_invE, double* rowsum, int rows, int Np,
+                           cudaStream_t st);
+// m2[x] = g2 * sum_a c_a rowsum[x][a][2]  (or m_D^2)
+cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned glue_slot_mask, double g2, double m_D,
+                      cudaStream_t st);
+// mom = per-cell (n, e), totals, m2
+cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
+                           double d3p_over_2pi3, double d3x, cudaStream_t st);
+
+}  // namespace bz

@@ -1,0 +1,142 @@
+// bz_transport.cu -- upwind free streaming + forward Euler (S8a.6, S8a.7), row sums, regulator mass and moments
+// (S8a.1, S8a.8).  All HBM-bound: one coalesced pass over f, momentum index fastest.
+#include "bz_internal.h"
+
+namespace bz {
+
+namespace {
+
+// One thread per (xcell, a, pcell) value, pcell fastest.  Upwind flux form of the drift term of Eq. 13:
+// dF = - sum_d [ max(c_d,0) (f(x) - f(x - e_d)) + min(c_d,0) (f(x + e_d) - f(x)) ],  c_d = v_d dt/dx, periodic.
+template <int kMode>
+__global__ void __launch_bounds__(256) transport_kernel(const TransportParams P)
+{
+    const int xcell = blockIdx.y;
+    const int ix = xcell % P.nx, iy = (xcell / P.nx) % P.ny, iz = xcell / (P.nx * P.ny);
+    const size_t row = (size_t)P.S * P.Np;                    // doubles per spatial cell
+    const int xm = (ix + P.nx - 1) % P.nx - ix, xp = (ix + 1) % P.nx - ix;
+    const int ym = ((iy + P.ny - 1) % P.ny - iy) * P.nx, yp = ((iy + 1) % P.ny - iy) * P.nx;
+    const int zm = ((iz + P.nz - 1) % P.nz - iz) * P.nx * P.ny, zp = ((iz + 1) % P.nz - iz) * P.nx * P.ny;
+    const int per_cell = P.S * P.Np;
+    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < per_cell; q += gridDim.x * blockDim.x) {
+        const int pc = q % P.Np, a = q / P.Np;
+        const size_t idx = (size_t)xcell * row + q;
+        const double f0 = P.f[idx];
+        const double cx = P.vx[pc] * P.cfl, cy = P.vy[pc] * P.cfl, cz = P.vz[pc] * P.cfl;
+        // only the upwind neighbour of each axis is read
+        const double fx = P.f[idx + (ptrdiff_t)(cx > 0.0 ? xm : xp) * (ptrdiff_t)row];
+        const double fy = P.f[idx + (ptrdiff_t)(cy > 0.0 ? ym : yp) * (ptrdiff_t)row];
+        const double fz = P.f[idx + (ptrdiff_t)(cz > 0.0 ? zm : zp) * (ptrdiff_t)row];
+        // max(c,0)(f0 - f-) + min(c,0)(f+ - f0) = |c| (f0 - f_upwind)
+        double acc = fabs(cx) * (f0 - fx);
+        acc += fabs(cy) * (f0 - fy);
+        acc += fabs(cz) * (f0 - fz);
+        if (kMode == 0) {
+            P.out[idx] = -acc;
+        } else {
+            const double dFc = P.dN[idx] / P.inv_deg[a];
+            P.dN[idx] = 0.0;
+            P.out[idx] = (f0 - acc) + dFc;
+        }
+    }
+}
+
+// One CTA per (xcell, a) row: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|) over the Np momentum cells.
+__global__ void __launch_bounds__(256) rowsum_kernel(const double* __restrict__ f, const double* __restrict__ absp,
+                                                     const double* __restrict__ w_invE, double* __restrict__ rowsum, int Np)
+{
+    const double* fr = f + (size_t)blockIdx.x * Np;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int p = threadIdx.x; p < Np; p += blockDim.x) {
+        const double v = fr[p];
+        s0 += v; s1 += absp[p] * v; s2 += w_invE[p] * v;
+    }
+    __shared__ double sh[3][8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sh[0][warp] = s0; sh[1][warp] = s1; sh[2][warp] = s2; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += sh[threadIdx.x][w];
+        rowsum[(size_t)blockIdx.x * 3 + threadIdx.x] = t;
+    }
+}
+
+// m2[x] = g^2 sum_a c_a rowsum[x][a][2], c = 6 for the gluon row, 1 for quark rows (Eq. 8 with E_p = |p|, S8a.1)
+__global__ void m2_kernel(const double* __restrict__ rowsum, double* __restrict__ m2, int Nx, int S, unsigned glue_slot_mask,
+                          double g2, double m_D)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= Nx) return;
+    if (m_D > 0.0) { m2[x] = m_D * m_D; return; }
+    double acc = 0.0;
+    for (int a = 0; a < S; ++a) acc += (((glue_slot_mask >> a) & 1u) ? 6.0 : 1.0) * rowsum[((size_t)x * S + a) * 3 + 2];
+    m2[x] = g2 * acc;
+}
+
+// per-cell (n, e), totals over x in a fixed order (one thread per species), then m2 copied behind them
+__global__ void moments_kernel(const double* __restrict__ rowsum, const double* __restrict__ m2, double* __restrict__ mom,
+                               int Nx, int S, double d3p_over_2pi3, double d3x, const double d0, const double d1,
+                               const double d2, const double d3, const double d4, const double d5, const double d6)
+{
+    const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
+    const size_t rows = (size_t)Nx * S;
+    for (size_t r = blockIdx.x * (size_t)blockDim.x + threadIdx.x; r < rows; r += (size_t)gridDim.x * blockDim.x) {
+        const int a = (int)(r % S);
+        mom[2 * r + 0] = deg[a] * rowsum[3 * r + 0] * d3p_over_2pi3;
+        mom[2 * r + 1] = deg[a] * rowsum[3 * r + 1] * d3p_over_2pi3;
+    }
+    for (size_t x = blockIdx.x * (size_t)blockDim.x + threadIdx.x; x < (size_t)Nx; x += (size_t)gridDim.x * blockDim.x)
+        mom[2 * rows + 2 * S + x] = m2[x];
+    if (blockIdx.x == 0 && threadIdx.x < 2 * S) {
+        const int a = threadIdx.x >> 1, c = threadIdx.x & 1;
+        double t = 0.0;
+        for (int x = 0; x < Nx; ++x) t += (deg[a] * rowsum[3 * ((size_t)x * S + a) + c] * d3p_over_2pi3) * d3x;
+        mom[2 * rows + threadIdx.x] = t;
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st)
+{
+    const int per_cell = P.S * P.Np;
+    int bx = (per_cell + 255) / 256;
+    if (bx > 64) bx = 64;
+    dim3 grid(bx, P.nx * P.ny * P.nz);
+    if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
+    else transport_kernel<1><<<grid, 256, 0, st>>>(P);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_invE, double* rowsum, int rows, int Np,
+                           cudaStream_t st)
+{
+    rowsum_kernel<<<rows, 256, 0, st>>>(f, absp, w_invE, rowsum, Np);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned glue_slot_mask, double g2, double m_D,
+                      cudaStream_t st)
+{
+    m2_kernel<<<(Nx + 127) / 128, 128, 0, st>>>(rowsum, m2, Nx, S, glue_slot_mask, g2, m_D);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
+                           double d3p_over_2pi3, double d3x, cudaStream_t st)
+{
+    int blocks = (Nx * S + 255) / 256;
+    if (blocks > 148) blocks = 148;
+    moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, deg[0], deg[1], deg[2], deg[3], deg[4],
+                                           deg[5], deg[6]);
+    return cudaGetLastError();
+}
+
+}  // namespace bz

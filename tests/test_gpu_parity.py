@@ -1,0 +1,260 @@
+"""GPU parity: the CUDA path (through the C ABI of include/bz.h) against the CPU oracle, element by element, on the
+same seeded inputs (workloads.py).  Targets (BASELINE.json north_star):
+  - sampled cell indices and (s, t, u): bit exact;
+  - dF and f after N steps: |gpu - cpu| <= 1e-11 * max(|cpu|, G) per value, G = the gross sum of |A| deposited into
+    that value (reading S16 of SURVEY.md 8c: a net dF that cancels to ~0 is compared on the scale of what was
+    summed);
+  - moments within 1e-12 relative; particle number conserved to 1e-13 of the gross deposit per step.
+"""
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+from oracle import bzo
+from paper_1912_04457_b200 import bz
+
+pytestmark = pytest.mark.gpu
+
+TOL_DF = 1e-11
+NDEG = {0: 16.0, 1: 6.0, 2: 6.0, 3: 6.0, 4: 6.0, 5: 6.0, 6: 6.0}
+
+
+def _pair(cfg, threads=0):
+    kw = dict(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species,
+              alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
+    import os
+    o = bzo.Oracle(threads=threads or min(16, os.cpu_count() or 1), **kw)
+    g = bz.Boltzmann(**kw)
+    return o, g
+
+
+def _deg(cfg):
+    return np.array([NDEG[s] for s in cfg.species])[None, :, None]
+
+
+def _assert_dF(dF_g, dF_o, gross, what):
+    scale = np.maximum(np.abs(dF_o), gross)
+    err = np.abs(dF_g - dF_o)
+    bad = err > TOL_DF * scale
+    assert not bad.any(), "%s: %d values off, worst %.3e of scale" % (what, bad.sum(), (err / np.maximum(scale, 1e-300)).max())
+    nz = np.abs(dF_o).max()
+    assert err.max() <= TOL_DF * nz
+
+
+def _assert_conserved(cfg, dF, gross):
+    num = (_deg(cfg) * dF).sum()
+    den = (_deg(cfg) * gross).sum()
+    assert abs(num) <= 1e-13 * den
+
+
+SMALL = [
+    wl.CONFIGS[0],                                                     # config 0 at full size: 216 k samples/step
+    wl.scaled(wl.CONFIGS[1], np_=12, samples=40),
+    wl.scaled(wl.CONFIGS[2], np_=13, samples=50),                      # odd grid, ragged sample count
+    wl.scaled(wl.CONFIGS[3], nx=3, np_=10, samples=24),
+    wl.scaled(wl.CONFIGS[4], nx=2, np_=11, samples=33),
+]
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=lambda c: c.name)
+def test_sampled_indices_bit_exact(cfg):
+    o, g = _pair(cfg)
+    for step in (0, 3):
+        for xcell in sorted({0, cfg.Nx - 1, cfg.Nx // 2}):
+            co, so = o.debug_samples(step, xcell, 0, cfg.Np)
+            cg, sg = g.debug_samples(step, xcell, 0, cfg.Np)
+            assert np.array_equal(cg.cpu().numpy(), co)
+            assert np.array_equal(sg.cpu().numpy().view(np.uint64), so.view(np.uint64))
+    assert 0.05 < co[..., 3].mean() < 0.95
+
+
+@pytest.mark.parametrize("k", [0, 1, 2, 3, 4])
+def test_sampled_indices_bit_exact_full_size(k):
+    # the five configs at their BASELINE.json sizes; the oracle checks whole spatial cells one by one
+    cfg = wl.CONFIGS[k]
+    o = bzo.Oracle(np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=(0,), seed=cfg.seed, samples=cfg.samples,
+                   nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx)            # kinematics do not depend on species
+    g = bz.Boltzmann(np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=(0,), seed=cfg.seed, samples=cfg.samples,
+                     nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx)
+    xcells = sorted({0, cfg.Nx - 1, (cfg.Nx * 5) // 7})
+    half = cfg.Np // 2
+    for xcell in xcells:
+        for (b, e) in ((0, half), (half, cfg.Np)):
+            co, so = o.debug_samples(cfg.steps - 1, xcell, b, e)
+            cg, sg = g.debug_samples(cfg.steps - 1, xcell, b, e)
+            assert np.array_equal(cg.cpu().numpy(), co)
+            assert np.array_equal(sg.cpu().numpy().view(np.uint64), so.view(np.uint64))
+
+
+@pytest.mark.parametrize("cfg", SMALL, ids=lambda c: c.name)
+def test_collision_dF_parity_and_conservation(cfg):
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg)
+    o.set_f(f)
+    g.set_f(f)
+    for step in (0, 5):
+        dF_o = o.collision(cfg.dt, step)
+        gross = o.gross()
+        dF_g = g.collision(cfg.dt, step).cpu().numpy()
+        assert np.abs(dF_o).max() > 0
+        _assert_dF(dF_g, dF_o, gross, "%s step %d" % (cfg.name, step))
+        _assert_conserved(cfg, dF_g, gross)
+    # dense random f: every channel and every cell active (shape of the paper's Fig. 2 test)
+    fr = wl.random_f(cfg, seed=7)
+    o.set_f(fr)
+    g.set_f(torch.from_numpy(fr).cuda())                                  # device-to-device path of bz_set_f
+    dF_o = o.collision(cfg.dt, 1)
+    gross = o.gross()
+    dF_g = g.collision(cfg.dt, 1).cpu().numpy()
+    _assert_dF(dF_g, dF_o, gross, cfg.name + " random f")
+    _assert_conserved(cfg, dF_g, gross)
+    assert np.count_nonzero(dF_g) > 0.9 * dF_g.size
+
+
+@pytest.mark.parametrize("k", [1, 2])
+def test_collision_dF_parity_full_size_homogeneous(k):
+    # configs 1 and 2 at full size, one step (1.0 M and 6.9 M samples)
+    cfg = wl.CONFIGS[k]
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg)
+    o.set_f(f)
+    g.set_f(f)
+    dF_o = o.collision(cfg.dt, 0)
+    gross = o.gross()
+    dF_g = g.collision(cfg.dt, 0).cpu().numpy()
+    _assert_dF(dF_g, dF_o, gross, cfg.name)
+    _assert_conserved(cfg, dF_g, gross)
+
+
+@pytest.mark.parametrize("cfg,steps", [(SMALL[0], 10), (SMALL[1], 4), (SMALL[2], 3), (SMALL[3], 5), (SMALL[4], 4)],
+                         ids=lambda c: getattr(c, "name", str(c)))
+def test_f_after_n_steps_and_moments(cfg, steps):
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg)
+    o.set_f(f)
+    g.set_f(f)
+    m0 = g.moments()
+    N0 = float(m0["tot"][:, 0].sum())
+    for _ in range(steps):
+        o.step(cfg.dt)
+        g.step(cfg.dt)
+    f_o = o.get_f()
+    f_g = g.get_f().cpu().numpy()
+    # per-value scale: the value itself or the gross deposit of the last step, whichever is larger
+    gross = o.gross()
+    scale = np.maximum(np.abs(f_o), gross)
+    err = np.abs(f_g - f_o)
+    assert (err <= TOL_DF * np.maximum(scale, np.abs(f_o).max() * 1e-3)).all(), (err / np.maximum(scale, 1e-300)).max()
+    assert err.max() <= TOL_DF * np.abs(f_o).max()
+    # host-buffer path of bz_get_f
+    host = torch.empty(g.shape, dtype=torch.float64)
+    g.get_f(host)
+    assert np.array_equal(host.numpy(), f_g)
+    mo, mg = o.moments(), g.moments()
+    for key in ("ne", "tot", "m2"):
+        a, b = np.asarray(mo[key]), mg[key].numpy()
+        assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(np.abs(a), np.abs(a).max() * 1e-6)), key
+    N1 = float(mg["tot"][:, 0].sum())
+    assert abs(N1 - N0) <= 1e-12 * N0                                      # total particle number
+
+
+@pytest.mark.parametrize("cfg", [SMALL[3], SMALL[4], wl.scaled(wl.CONFIGS[3], nx=4, np_=6, samples=4)],
+                         ids=lambda c: c.name)
+def test_stream_parity(cfg):
+    o, g = _pair(cfg)
+    f = wl.random_f(cfg, seed=3)
+    o.set_f(f)
+    g.set_f(f)
+    for dt in (cfg.dt, cfg.dx):                                            # Courant number 1 on the axes: exact shift
+        d_o = o.stream(dt)
+        d_g = g.stream(dt).cpu().numpy()
+        assert np.all(np.abs(d_g - d_o) <= 1e-13 * np.abs(f).max())
+        assert np.all(np.abs(d_g.sum(axis=0)) <= 1e-12 * np.abs(f).sum(axis=0))   # Eq. 13: flux form conserves
+
+
+def test_config4_full_size_subset_protocol():
+    # config 4 at full size (3.2 GB per copy, 3.6e9 samples per step): the GPU runs whole steps; the oracle is fed
+    # the GPU's f of selected spatial cells at the start of the step ("teacher forcing", the collision term is
+    # local in x) and its dF for those cells is compared; streaming is compared on slabs.
+    cfg = wl.CONFIGS[4]
+    g = bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
+                     species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
+    f0 = torch.from_numpy(wl.initial_f(cfg))
+    g.set_f(f0)
+    o = bzo.Oracle(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
+                   species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
+    deg = _deg(cfg)[0]
+    mom0 = g.moments()
+    g.step(cfg.dt)                                                         # step 0 -> the cells are no longer sparse
+    xcells = [0, 2056, 4095]                                               # a corner, the hot centre (8,8,8), the last
+    for step in (1, 2):
+        f_dev = g.get_f()
+        dF_dev = g.collision(cfg.dt, step)
+        for x in xcells:
+            tile = f_dev[x].cpu().numpy()
+            dN, gross, m2 = o.collision_tile(cfg.dt, step, x, tile, want_gross=True)
+            dF_o, G = dN / deg, gross / deg
+            _assert_dF(dF_dev[x].cpu().numpy(), dF_o, G, "cfg4 xcell %d step %d" % (x, step))
+        # exact conservation over the whole grid, on the device
+        num = float((dF_dev * torch.from_numpy(_deg(cfg)).cuda()).sum())
+        den = float((dF_dev.abs() * torch.from_numpy(_deg(cfg)).cuda()).sum())
+        assert abs(num) <= 1e-12 * den
+        g.step(cfg.dt)
+    mom = g.moments()
+    assert abs(float(mom["tot"][:, 0].sum()) - float(mom0["tot"][:, 0].sum())) <= 1e-12 * float(mom0["tot"][:, 0].sum())
+    # streaming on the full grid: the upwind stencil of three z-slabs against numpy
+    f_dev = g.get_f()
+    dS = g.stream(cfg.dt)
+    f5 = f_dev.view(cfg.nx, cfg.nx, cfg.nx, cfg.S, cfg.Np)
+    d5 = dS.view(cfg.nx, cfg.nx, cfg.nx, cfg.S, cfg.Np)
+    pabs, (px, py, pz) = wl.momentum_centres(cfg)
+    v = [torch.from_numpy(np.where(pabs > 0, c / np.where(pabs > 0, pabs, 1.0), 0.0)).cuda() * (cfg.dt / cfg.dx)
+         for c in (px, py, pz)]
+    acc = torch.zeros_like(f5)
+    for d, axis in ((0, 2), (1, 1), (2, 0)):                               # x is the fastest spatial index
+        c = v[d]
+        acc += torch.clamp(c, min=0) * (f5 - torch.roll(f5, 1, dims=axis)) + torch.clamp(c, max=0) * (torch.roll(f5, -1, dims=axis) - f5)
+    assert float((d5 + acc).abs().max()) <= 1e-13 * float(f5.abs().max())
+
+
+def test_edge_cases():
+    # empty f: nothing is deposited, m^2 = 0 is never divided by because every bracket vanishes first
+    cfg = wl.scaled(wl.CONFIGS[2], np_=6, samples=5)
+    o, g = _pair(cfg)
+    dF = g.collision(cfg.dt, 0).cpu().numpy()
+    assert np.all(dF == 0.0)
+    # ragged sample counts around the warp width, smallest grid, single quark species, generic species subset
+    for species, np_, Ns in (((0,), 2, 1), ((3,), 5, 31), ((0, 1, 2), 7, 33), ((0, 2, 3, 6), 6, 65), ((1, 2, 5), 6, 64)):
+        c = wl.scaled(wl.CONFIGS[2], np_=np_, samples=Ns, species=species)
+        o, g = _pair(c)
+        f = wl.random_f(c, seed=11)
+        o.set_f(f)
+        g.set_f(f)
+        dF_o = o.collision(c.dt, 2)
+        gross = o.gross()
+        dF_g = g.collision(c.dt, 2).cpu().numpy()
+        _assert_dF(dF_g, dF_o, gross, "species %s np %d Ns %d" % (species, np_, Ns))
+        _assert_conserved(c, dF_g, gross)
+    # fixed regulator mass and another seed
+    c = wl.scaled(wl.CONFIGS[1], np_=8, samples=16, m_D=0.6, seed=12345)
+    o, g = _pair(c)
+    f = wl.random_f(c, seed=5)
+    o.set_f(f)
+    g.set_f(f)
+    assert float(g.moments()["m2"][0]) == pytest.approx(0.36, rel=1e-15)
+    _assert_dF(g.collision(c.dt, 0).cpu().numpy(), o.collision(c.dt, 0), o.gross(), "fixed m_D")
+    # non-cubic spatial grid, two streams of calls on a user stream
+    o = bzo.Oracle(nx=4, ny=2, nz=3, dx=0.3, np_=6, species=(0, 1, 2), samples=8, seed=1)
+    g = bz.Boltzmann(nx=4, ny=2, nz=3, dx=0.3, np_=6, species=(0, 1, 2), samples=8, seed=1)
+    s = torch.cuda.Stream()
+    g.set_stream(s)
+    f = np.random.default_rng(0).uniform(0.05, 0.5, size=o.shape)
+    o.set_f(f)
+    g.set_f(f)
+    for _ in range(3):
+        o.step(0.05)
+        g.step(0.05)
+    s.synchronize()
+    f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
+    assert np.abs(f_g - f_o).max() <= TOL_DF * np.abs(f_o).max()

@@ -1,0 +1,88 @@
+"""CPU-side checks of the product: the C-ABI library loads, exports what include/bz.h declares, refuses to run
+without a device, and its factorised channel algebra equals the oracle's channel-by-channel definition."""
+import ctypes as C
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import bzo
+from paper_1912_04457_b200 import bz
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "bz.h")).read()
+    declared = set(re.findall(r"\b(bz_[a-z_0-9]+)\s*\(", header))
+    declared -= {"bz_ctx", "bz_grid"}
+    assert declared == set(bz.EXPORTS)
+    L = bz.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_bad_arguments_are_rejected_without_a_device():
+    L = bz.lib()
+    h = C.c_void_p()
+    g = bz.Grid(1, 1, 1, 1.0, 8, -3.0, 3.0)
+    sp = (C.c_int * 2)(1, 1)                         # not strictly ascending
+    assert L.bz_create(C.byref(g), sp, 2, 0.3, 0.0, C.byref(h)) == -1
+    sp = (C.c_int * 1)(9)
+    assert L.bz_create(C.byref(g), sp, 1, 0.3, 0.0, C.byref(h)) == -1
+    g2 = bz.Grid(1, 1, 1, 1.0, 8, 3.0, -3.0)         # empty box
+    sp = (C.c_int * 1)(0)
+    assert L.bz_create(C.byref(g2), sp, 1, 0.3, 0.0, C.byref(h)) == -1
+    assert L.bz_set_samples(None, 4) == -1
+    assert L.bz_step(None, 0.1) == -1
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="only meaningful on a box without a GPU")
+def test_no_cpu_fallback():
+    with pytest.raises(bz.BzError, match="no CUDA device"):
+        bz.Boltzmann(np_=4, species=(0,))
+    # and the library itself refuses: -2 with a message, no context usable
+    L = bz.lib()
+    h = C.c_void_p()
+    g = bz.Grid(1, 1, 1, 1.0, 4, -3.0, 3.0)
+    assert L.bz_create(C.byref(g), (C.c_int * 1)(0), 1, 0.3, 0.0, C.byref(h)) == -2
+    assert b"no CUDA device" in L.bz_last_error(h)
+    assert L.bz_step(h, 0.01) == -4
+    L.bz_destroy(h)
+
+
+@pytest.mark.parametrize("species", [(0,), (1, 2, 3, 4, 5, 6), (0, 1, 2, 3, 4, 5, 6), (0, 1, 2), (0, 1), (1, 2, 5),
+                                     (0, 3, 4, 5), (2,), (0, 2, 3, 6)])
+def test_factorised_channel_algebra_equals_channel_loop(species):
+    # the kernels never loop over the 127 channels (csrc/bz_channels.cuh); their algebra, run on the host through
+    # bz_debug_deposit_host, must reproduce the oracle's channel-by-channel deposits up to summation order
+    rng = np.random.default_rng(len(species) * 17 + species[0])
+    o = bzo.Oracle(np_=8, species=species, samples=8, seed=3)
+    S = len(species)
+    K = (0.01 / 0.1973269804) * 6.0 ** 3 / (2048 * math.pi ** 4 * 8)
+    done = 0
+    for trial in range(150):
+        sm = o.sample_one(0, 0, int(rng.integers(0, 512)), int(rng.integers(0, 8)))
+        if sm.attempts == 0:
+            continue
+        fvS = rng.uniform(0.0, 0.9, size=(4, S))
+        if trial % 5 == 0:
+            fvS[rng.integers(0, 4), rng.integers(0, S)] = 0.0
+        if trial % 7 == 0:
+            fvS[:, :] = 0.0                                     # empty cells: nothing may be deposited
+        dN, _, gross = o.sample_channels(fvS, sm.s, sm.t, sm.u, sm.E1, sm.E2, 0.37, 0.01)
+        fv = rng.uniform(0.0, 1.0, size=(4, 7))                 # values of inactive species must be ignored
+        fv[:, list(species)] = fvS
+        out = bz.debug_deposit_host(species, 0.3, fv, sm.s, sm.t, sm.u, 0.37, K / (sm.E1 * sm.E2))
+        assert np.all(out[:, [i for i in range(7) if i not in species]] == 0.0)
+        got = out[:, list(species)]
+        if gross == 0.0:
+            assert np.all(got == 0.0)
+        else:
+            assert np.abs(got - dN).max() <= 1e-12 * gross
+            assert abs(got.sum()) <= 1e-12 * gross              # Eq. 23: number units sum to zero
+        done += 1
+    assert done > 100
