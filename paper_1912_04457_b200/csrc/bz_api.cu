@@ -47,7 +47,18 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
 {
     CollideParams P;
     P.g = grid_const(c);
-    P.f = c->f; P.dN = c->dN; P.m2 = c->m2;
+    P.f_aos = c->f_aos; P.dN_aos = c->dN_aos; P.m2 = c->m2;
+    P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x; P.x_per_chunk = c->x_per_chunk;
+    P.region_cap = c->cells_per_region * c->Ns;
+    {   // carve the record buffer: int4 cells first (16-byte aligned), then s, t, w, then the counts
+        const size_t slots = (size_t)c->x_per_chunk * c->regions_per_x * P.region_cap;
+        char* b = (char*)c->rec_buf;
+        P.rec_cells = (int4*)b; b += slots * sizeof(int4);
+        P.rec_s = (double*)b; b += slots * sizeof(double);
+        P.rec_t = (double*)b; b += slots * sizeof(double);
+        P.rec_w = (double*)b; b += slots * sizeof(double);
+        P.rec_count = (int*)b;
+    }
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
     const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
@@ -59,14 +70,34 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     return P;
 }
 
+// (re)allocate the record buffer for the current samples-per-cell: at most ~8 GB, at least one spatial cell
+int ensure_records(bz_ctx* c)
+{
+    if (c->rec_buf && c->rec_Ns == c->Ns) return 0;
+    if (c->rec_buf) { cudaFree(c->rec_buf); c->rec_buf = nullptr; }
+    c->cells_per_region = collide_cells_per_region(c->Np, c->Nx);
+    c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
+    const size_t per_x = (size_t)c->regions_per_x * ((size_t)c->cells_per_region * c->Ns * 40 + sizeof(int));
+    size_t xs = (size_t)8e9 / per_x;
+    if (xs < 1) xs = 1;
+    if (xs > (size_t)c->Nx) xs = c->Nx;
+    c->x_per_chunk = (int)xs;
+    c->rec_bytes = xs * per_x + 256;
+    c->rec_Ns = c->Ns;
+    BZ_CUDA(cudaMalloc(&c->rec_buf, c->rec_bytes), "cudaMalloc record buffer");
+    return 0;
+}
+
 int run_collide(bz_ctx* c, double dt_fm, unsigned step)
 {
+    if (int rc = ensure_records(c)) return rc;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (c->profile) {
         BZ_CUDA(cudaEventCreate(&e0), "event");
         BZ_CUDA(cudaEventCreate(&e1), "event");
         BZ_CUDA(cudaEventRecord(e0, c->stream), "event record");
     }
+    BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
     BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->stream), "collide");
     if (c->profile) {
         BZ_CUDA(cudaEventRecord(e1, c->stream), "event record");
@@ -109,8 +140,9 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
+    c->rec_buf = nullptr; c->rec_bytes = 0; c->rec_Ns = -1; c->cells_per_region = 1; c->regions_per_x = c->Np; c->x_per_chunk = 1;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
-    c->f = c->f_new = c->dN = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = nullptr;
+    c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         c->err = "bz_create: no CUDA device (this library has no CPU path)";
         return -2;
@@ -118,7 +150,10 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     const size_t bytes = c->n_values * sizeof(double);
     BZ_CUDA(cudaMalloc(&c->f, bytes), "cudaMalloc f");
     BZ_CUDA(cudaMalloc(&c->f_new, bytes), "cudaMalloc f_new");
-    BZ_CUDA(cudaMalloc(&c->dN, bytes), "cudaMalloc dN");
+    c->SP = collide_slots_per_cell(c->mask);
+    const size_t aos_bytes = (size_t)c->Nx * c->Np * c->SP * sizeof(double);
+    BZ_CUDA(cudaMalloc(&c->f_aos, aos_bytes), "cudaMalloc f_aos");
+    BZ_CUDA(cudaMalloc(&c->dN_aos, aos_bytes), "cudaMalloc dN_aos");
     BZ_CUDA(cudaMalloc(&c->m2, c->Nx * sizeof(double)), "cudaMalloc m2");
     BZ_CUDA(cudaMalloc(&c->rowsum, (size_t)c->Nx * c->S * 3 * sizeof(double)), "cudaMalloc rowsum");
     BZ_CUDA(cudaMalloc(&c->mom, ((size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx) * sizeof(double)), "cudaMalloc mom");
@@ -126,7 +161,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->w_invE = c->absp + c->Np; c->vx = c->w_invE + c->Np; c->vy = c->vx + c->Np; c->vz = c->vy + c->Np;
     BZ_CUDA(cudaMemset(c->f, 0, bytes), "memset f");
     BZ_CUDA(cudaMemset(c->f_new, 0, bytes), "memset f_new");
-    BZ_CUDA(cudaMemset(c->dN, 0, bytes), "memset dN");
+    BZ_CUDA(cudaMemset(c->dN_aos, 0, aos_bytes), "memset dN_aos");
     // cell-centre tables: |p|, d3p/((2pi)^3 |p|) (0 at p = 0, S10), p/|p| (0 at p = 0)
     {
         const int n = g->np;
@@ -151,7 +186,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
 int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
-    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->dN); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
+    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->rec_buf); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
     delete c;
@@ -192,14 +227,14 @@ int bz_collision(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
     if (int rc = run_collide(c, dt_fm, step)) return rc;
     double deg[7];
     fill_deg(c, deg);
-    BZ_CUDA(launch_finalize(c->dN, dF_dev, c->Nx, c->S, c->Np, deg, c->stream), "finalize");
+    BZ_CUDA(launch_finalize(c->dN_aos, dF_dev, c->Nx, c->S, c->SP, c->Np, deg, c->stream), "finalize");
     return 0;
 }
 
 static TransportParams transport_params(const bz_ctx* c, double dt_fm, double* out)
 {
     TransportParams T;
-    T.f = c->f; T.dN = c->dN; T.out = out; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
+    T.f = c->f; T.dN_aos = c->dN_aos; T.SP = c->SP; T.out = out; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
     T.nx = c->grid.nx; T.ny = c->grid.ny; T.nz = c->grid.nz; T.S = c->S; T.Np = c->Np;
     T.cfl = dt_fm / c->grid.dx;
     fill_deg(c, T.inv_deg);

@@ -16,10 +16,18 @@ constexpr double kPi = 3.14159265358979323846;
 
 struct CollideParams {
     GridConst g;
-    const double* f;      // [Nx][S][Np]
-    double* dN;           // [Nx][S][Np] deposit scratch in number units, zero on entry
+    const double* f_aos;  // [Nx][Np][SP] cell-major staging copy of f (pad slots 0)
+    double* dN_aos;       // [Nx][Np][SP] deposit scratch in number units, zero on entry
     const double* m2;     // [Nx] regulator mass^2
     int S, Np, Nx, Ns;
+    // record buffer written by sample_kernel, read by deposit_kernel (one chunk of spatial cells at a time)
+    int4* rec_cells;      // [regions in chunk][region_cap] (i, j, k, l)
+    double *rec_s, *rec_t, *rec_w;   // [regions in chunk][region_cap]
+    int* rec_count;       // [regions in chunk] accepted samples of the region
+    int cells_per_region; // p1 cells per region (one warp each)
+    int regions_per_x;    // ceil(Np / cells_per_region)
+    int region_cap;       // cells_per_region * Ns record slots per region (worst case: every sample accepted)
+    int x_per_chunk;      // spatial cells per sample/deposit kernel pair
     uint32_t seed, step;
     double K;             // dtG Vp / (2048 pi^4 Ns)                       (S8c step 0)
     double g4;            // (4 pi alpha_s)^2
@@ -29,8 +37,9 @@ struct CollideParams {
 
 struct TransportParams {
     const double* f;      // old f
-    double* dN;           // collision deposits (number units), reset to 0 when consumed
+    double* dN_aos;       // collision deposits [Nx][Np][SP] (number units), reset to 0 when consumed
     double* out;          // f_new or dF
+    int SP;
     const double* vx; const double* vy; const double* vz;   // [Np] p/|p| at the cell centre (0 at p = 0)
     int nx, ny, nz, S, Np;
     double cfl;           // dt / dx
@@ -46,7 +55,12 @@ struct bz_ctx_impl {
     uint32_t seed, step;
     cudaStream_t stream;
     size_t n_values;
-    double *f, *f_new, *dN;          // device, n_values each
+    double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
+    double *f_aos, *dN_aos;          // device, Nx*Np*SP each (cell-major staging for the collision kernel)
+    int SP;                          // doubles per cell in the staging layout
+    // record buffer (see CollideParams), sized for x_per_chunk spatial cells at the current Ns
+    void* rec_buf; size_t rec_bytes; int rec_Ns;
+    int cells_per_region, regions_per_x, x_per_chunk;
     double *m2;                      // device [Nx]
     double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|)
     double *mom;                     // device [2*S*Nx + 2*S + Nx]
@@ -57,11 +71,14 @@ struct bz_ctx_impl {
 };
 
 // launchers (each returns the cudaError_t of the launch)
+int collide_slots_per_cell(unsigned mask);
+int collide_cells_per_region(int Np, int Nx);
 cudaError_t launch_collide(const CollideParams& P, cudaStream_t st);
+cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, int Np, cudaStream_t st);
 cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin, int p_end, int* cells, double* stu,
                                  cudaStream_t st);
-// out = dN / N_a, dN = 0
-cudaError_t launch_finalize(double* dN, double* dF, int Nx, int S, int Np, const double* deg, cudaStream_t st);
+// dF = dN_aos / N_a (transposed to the API layout), dN_aos = 0
+cudaError_t launch_finalize(double* dN_aos, double* dF, int Nx, int S, int SP, int Np, const double* deg, cudaStream_t st);
 // mode 0: out = dF_stream;  mode 1: out = (f + dF_stream) + dN/N_a and dN = 0
 cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st);
 // rowsum[x][a][0..2]

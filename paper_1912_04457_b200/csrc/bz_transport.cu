@@ -6,7 +6,8 @@ namespace bz {
 
 namespace {
 
-// One thread per (xcell, a, pcell) value, pcell fastest.  Upwind flux form of the drift term of Eq. 13:
+// One thread per (xcell, pcell), looping over the species: f is read and written coalesced in pcell for every
+// species, the collision deposits of the cell come from the cell-major scratch (64 contiguous bytes per thread).  Upwind flux form of the drift term of Eq. 13:
 // dF = - sum_d [ max(c_d,0) (f(x) - f(x - e_d)) + min(c_d,0) (f(x + e_d) - f(x)) ],  c_d = v_d dt/dx, periodic.
 template <int kMode>
 __global__ void __launch_bounds__(256) transport_kernel(const TransportParams P)
@@ -17,26 +18,28 @@ __global__ void __launch_bounds__(256) transport_kernel(const TransportParams P)
     const int xm = (ix + P.nx - 1) % P.nx - ix, xp = (ix + 1) % P.nx - ix;
     const int ym = ((iy + P.ny - 1) % P.ny - iy) * P.nx, yp = ((iy + 1) % P.ny - iy) * P.nx;
     const int zm = ((iz + P.nz - 1) % P.nz - iz) * P.nx * P.ny, zp = ((iz + 1) % P.nz - iz) * P.nx * P.ny;
-    const int per_cell = P.S * P.Np;
-    for (int q = blockIdx.x * blockDim.x + threadIdx.x; q < per_cell; q += gridDim.x * blockDim.x) {
-        const int pc = q % P.Np, a = q / P.Np;
-        const size_t idx = (size_t)xcell * row + q;
-        const double f0 = P.f[idx];
+    for (int pc = blockIdx.x * blockDim.x + threadIdx.x; pc < P.Np; pc += gridDim.x * blockDim.x) {
         const double cx = P.vx[pc] * P.cfl, cy = P.vy[pc] * P.cfl, cz = P.vz[pc] * P.cfl;
         // only the upwind neighbour of each axis is read
-        const double fx = P.f[idx + (ptrdiff_t)(cx > 0.0 ? xm : xp) * (ptrdiff_t)row];
-        const double fy = P.f[idx + (ptrdiff_t)(cy > 0.0 ? ym : yp) * (ptrdiff_t)row];
-        const double fz = P.f[idx + (ptrdiff_t)(cz > 0.0 ? zm : zp) * (ptrdiff_t)row];
-        // max(c,0)(f0 - f-) + min(c,0)(f+ - f0) = |c| (f0 - f_upwind)
-        double acc = fabs(cx) * (f0 - fx);
-        acc += fabs(cy) * (f0 - fy);
-        acc += fabs(cz) * (f0 - fz);
-        if (kMode == 0) {
-            P.out[idx] = -acc;
-        } else {
-            const double dFc = P.dN[idx] / P.inv_deg[a];
-            P.dN[idx] = 0.0;
-            P.out[idx] = (f0 - acc) + dFc;
+        const ptrdiff_t ox = (ptrdiff_t)(cx > 0.0 ? xm : xp) * (ptrdiff_t)row;
+        const ptrdiff_t oy = (ptrdiff_t)(cy > 0.0 ? ym : yp) * (ptrdiff_t)row;
+        const ptrdiff_t oz = (ptrdiff_t)(cz > 0.0 ? zm : zp) * (ptrdiff_t)row;
+        const double ax = fabs(cx), ay = fabs(cy), az = fabs(cz);
+        double* dn = kMode == 1 ? P.dN_aos + ((size_t)xcell * P.Np + pc) * P.SP : nullptr;
+        for (int a = 0; a < P.S; ++a) {
+            const size_t idx = (size_t)xcell * row + (size_t)a * P.Np + pc;
+            const double f0 = P.f[idx];
+            // max(c,0)(f0 - f-) + min(c,0)(f+ - f0) = |c| (f0 - f_upwind)
+            double acc = ax * (f0 - P.f[idx + ox]);
+            acc += ay * (f0 - P.f[idx + oy]);
+            acc += az * (f0 - P.f[idx + oz]);
+            if (kMode == 0) {
+                P.out[idx] = -acc;
+            } else {
+                const double dFc = dn[a] / P.inv_deg[a];
+                dn[a] = 0.0;
+                P.out[idx] = (f0 - acc) + dFc;
+            }
         }
     }
 }
@@ -106,8 +109,7 @@ __global__ void moments_kernel(const double* __restrict__ rowsum, const double* 
 
 cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st)
 {
-    const int per_cell = P.S * P.Np;
-    int bx = (per_cell + 255) / 256;
+    int bx = (P.Np + 255) / 256;
     if (bx > 64) bx = 64;
     dim3 grid(bx, P.nx * P.ny * P.nz);
     if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
