@@ -184,6 +184,7 @@ def run_ours(args, cfg):
     g.set_profile(True)
     g.get_profile()
     barrier()
+    launches0 = bz.launch_count()
     ms = 0.0
     if small:
         for _ in range(args.steps):
@@ -203,6 +204,7 @@ def run_ours(args, cfg):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
     barrier()
+    launches = bz.launch_count() - launches0
     coll_ms, coll_n = g.get_profile()
     g.set_profile(False)
     clocks = sampler.stop() if sampler else None
@@ -252,8 +254,8 @@ def run_ours(args, cfg):
         "collision_kernel_share_of_step": coll_ms / ms if ms > 0 else None,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": cfg.n_values * 8,
                 "d2h_bytes_per_step": cfg.n_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
-        "gpu_launches": 7 * args.steps,
-        "roofline": {"bound": "hbm", "kernel": "collide_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
+        "gpu_launches": launches,
+        "roofline": {"bound": "hbm", "kernel": "collision group (pack_kernel + sample_kernel + deposit_kernel; events around the group)", "achieved": ach, "peak": peak, "unit": "GB/s",
                      "frac": ach / peak if ach else None, "traffic": None, "peak_source": peak_src,
                      "bytes_per_sample": bps, "samples_per_launch": samples_step,
                      "ms_per_launch": coll_ms / coll_n if coll_n else None},

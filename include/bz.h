@@ -91,6 +91,10 @@ const char* bz_last_error(const bz_ctx* ctx);
 int bz_set_profile(bz_ctx* ctx, int on);
 int bz_get_profile(bz_ctx* ctx, double* collide_ms_total, int* collide_launches);
 
+/* Number of CUDA kernels this library has launched in this process so far (all contexts); bench.py reports the
+ * difference over its timed region as "gpu_launches". */
+unsigned long long bz_launch_count(void);
+
 /* ---- test-only exports ---------------------------------------------------------------------------------- */
 /* Sampled cells of p1 cells [pcell_begin, pcell_end) of spatial cell xcell, needed for the "bit-exact sampled
  * indices" target of NS: cells_dev[n][Ns][4] = (j, k, l, flag) int32, stu_dev[n][Ns][3] = (s, t, u) or NULL.

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
-           "bz_get_profile", "bz_debug_samples",
+           "bz_get_profile", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
 
 
@@ -48,6 +48,8 @@ def lib():
         L.bz_last_error.restype = C.c_char_p
         L.bz_set_profile.argtypes = [vp, C.c_int]
         L.bz_get_profile.argtypes = [vp, dp, ip]
+        L.bz_launch_count.argtypes = []
+        L.bz_launch_count.restype = C.c_ulonglong
         L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
         L.bz_debug_deposit_host.argtypes = [ip, C.c_int, C.c_double, dp] + [C.c_double] * 5 + [dp]
         _lib = L
@@ -183,6 +185,11 @@ class Boltzmann:
         self._chk(lib().bz_debug_samples(self._h, step, xcell, pbegin, pend, C.c_void_p(cells.data_ptr()),
                                          C.c_void_p(stu.data_ptr()) if want_stu else None), "bz_debug_samples")
         return cells, stu
+
+
+def launch_count():
+    """bz_launch_count: CUDA kernels launched by libbz.so in this process so far."""
+    return int(lib().bz_launch_count())
 
 
 def debug_deposit_host(species, alpha_s, fv, s, t, u, m2, w):

@@ -12,6 +12,10 @@ using namespace bz;
 
 struct bz_ctx : public bz_ctx_impl {};
 
+namespace bz {
+std::atomic<unsigned long long> g_launch_count{0};
+}
+
 namespace {
 
 int fail_cuda(bz_ctx* c, cudaError_t e, const char* where)
@@ -296,6 +300,8 @@ int bz_get_profile(bz_ctx* c, double* ms_total, int* launches)
     c->prof_events.clear();
     return 0;
 }
+
+unsigned long long bz_launch_count(void) { return g_launch_count.load(); }
 
 int bz_debug_samples(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int* cells_dev, double* stu_dev)
 {

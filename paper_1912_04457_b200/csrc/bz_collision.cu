@@ -244,6 +244,7 @@ cudaError_t launch_deposit(const CollideParams& P, int x_begin, int nxc, cudaStr
     }
     dim3 grid((P.regions_per_x + kDepositWarps - 1) / kDepositWarps, nxc), block(kDepositWarps * 32);
     deposit_kernel<kMask><<<grid, block, smem, st>>>(P, x_begin);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -265,6 +266,7 @@ cudaError_t launch_collide(const CollideParams& P, cudaStream_t st)
         const int nxc = P.Nx - x0 < P.x_per_chunk ? P.Nx - x0 : P.x_per_chunk;
         dim3 grid((P.regions_per_x + kSampleWarps - 1) / kSampleWarps, nxc), block(kSampleWarps * 32);
         sample_kernel<<<grid, block, 0, st>>>(P, x0);
+        ++g_launch_count;
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         switch (P.mask) {
@@ -285,6 +287,7 @@ cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin,
     if (total <= 0) return cudaSuccess;
     const int blocks = (int)((total + 127) / 128 < 148 * 16 ? (total + 127) / 128 : 148 * 16);
     debug_samples_kernel<<<blocks, 128, 0, st>>>(P, xcell, p_begin, p_end, cells, stu);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -292,6 +295,7 @@ cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, i
 {
     dim3 grid((Np + 255) / 256, Nx);
     pack_kernel<<<grid, 256, 0, st>>>(f, f_aos, S, SP, Np);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -299,6 +303,7 @@ cudaError_t launch_finalize(double* dN_aos, double* dF, int Nx, int S, int SP, i
 {
     dim3 grid((Np + 255) / 256, Nx);
     finalize_kernel<<<grid, 256, 0, st>>>(dN_aos, dF, S, SP, Np, deg[0], deg[1], deg[2], deg[3], deg[4], deg[5], deg[6]);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <string>
 #include <vector>
@@ -69,6 +70,9 @@ struct bz_ctx_impl {
     bool profile;
     std::vector<cudaEvent_t> prof_events;   // start/stop pairs around collide launches
 };
+
+// kernels launched by this library in this process (bz_launch_count); bumped by every launcher below
+extern std::atomic<unsigned long long> g_launch_count;
 
 // launchers (each returns the cudaError_t of the launch)
 int collide_slots_per_cell(unsigned mask);

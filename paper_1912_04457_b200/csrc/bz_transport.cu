@@ -114,6 +114,7 @@ cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st
     dim3 grid(bx, P.nx * P.ny * P.nz);
     if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
     else transport_kernel<1><<<grid, 256, 0, st>>>(P);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -121,6 +122,7 @@ cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_
                            cudaStream_t st)
 {
     rowsum_kernel<<<rows, 256, 0, st>>>(f, absp, w_invE, rowsum, Np);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -128,6 +130,7 @@ cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned 
                       cudaStream_t st)
 {
     m2_kernel<<<(Nx + 127) / 128, 128, 0, st>>>(rowsum, m2, Nx, S, glue_slot_mask, g2, m_D);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
@@ -138,6 +141,7 @@ cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, 
     if (blocks > 148) blocks = 148;
     moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, deg[0], deg[1], deg[2], deg[3], deg[4],
                                            deg[5], deg[6]);
+    ++g_launch_count;
     return cudaGetLastError();
 }
 
