@@ -52,17 +52,8 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     CollideParams P;
     P.g = grid_const(c);
     P.f_aos = c->f_aos; P.dN_aos = c->dN_aos; P.m2 = c->m2;
-    P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x; P.x_per_chunk = c->x_per_chunk;
-    P.region_cap = c->cells_per_region * c->Ns;
-    {   // carve the record buffer: int4 cells first (16-byte aligned), then s, t, w, then the counts
-        const size_t slots = (size_t)c->x_per_chunk * c->regions_per_x * P.region_cap;
-        char* b = (char*)c->rec_buf;
-        P.rec_cells = (int4*)b; b += slots * sizeof(int4);
-        P.rec_s = (double*)b; b += slots * sizeof(double);
-        P.rec_t = (double*)b; b += slots * sizeof(double);
-        P.rec_w = (double*)b; b += slots * sizeof(double);
-        P.rec_count = (int*)b;
-    }
+    P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
+    P.work_counter = c->work_counter; P.n_items = (unsigned)c->Nx * (unsigned)c->regions_per_x; P.x_begin = 0;
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
     const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
@@ -74,27 +65,8 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     return P;
 }
 
-// (re)allocate the record buffer for the current samples-per-cell: at most ~8 GB, at least one spatial cell
-int ensure_records(bz_ctx* c)
-{
-    if (c->rec_buf && c->rec_Ns == c->Ns) return 0;
-    if (c->rec_buf) { cudaFree(c->rec_buf); c->rec_buf = nullptr; }
-    c->cells_per_region = collide_cells_per_region(c->Np, c->Nx);
-    c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
-    const size_t per_x = (size_t)c->regions_per_x * ((size_t)c->cells_per_region * c->Ns * 40 + sizeof(int));
-    size_t xs = (size_t)8e9 / per_x;
-    if (xs < 1) xs = 1;
-    if (xs > (size_t)c->Nx) xs = c->Nx;
-    c->x_per_chunk = (int)xs;
-    c->rec_bytes = xs * per_x + 256;
-    c->rec_Ns = c->Ns;
-    BZ_CUDA(cudaMalloc(&c->rec_buf, c->rec_bytes), "cudaMalloc record buffer");
-    return 0;
-}
-
 int run_collide(bz_ctx* c, double dt_fm, unsigned step)
 {
-    if (int rc = ensure_records(c)) return rc;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (c->profile) {
         BZ_CUDA(cudaEventCreate(&e0), "event");
@@ -102,7 +74,7 @@ int run_collide(bz_ctx* c, double dt_fm, unsigned step)
         BZ_CUDA(cudaEventRecord(e0, c->stream), "event record");
     }
     BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
-    BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->stream), "collide");
+    BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->sms, c->stream), "collide");
     if (c->profile) {
         BZ_CUDA(cudaEventRecord(e1, c->stream), "event record");
         c->prof_events.push_back(e0);
@@ -144,14 +116,23 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
-    c->rec_buf = nullptr; c->rec_bytes = 0; c->rec_Ns = -1; c->cells_per_region = 1; c->regions_per_x = c->Np; c->x_per_chunk = 1;
+    c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         c->err = "bz_create: no CUDA device (this library has no CPU path)";
         return -2;
     }
+    {
+        int dev = 0;
+        BZ_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+        BZ_CUDA(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev), "SM count");
+        if ((long long)c->Nx * c->Np >= (1LL << 32)) { c->err = "bz_create: more than 2^32 (xcell, pcell) pairs"; return -1; }
+        c->cells_per_region = collide_cells_per_region(c->Np, c->Nx, c->sms);
+        c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
+    }
     const size_t bytes = c->n_values * sizeof(double);
+    BZ_CUDA(cudaMalloc(&c->work_counter, sizeof(unsigned)), "cudaMalloc work counter");
     BZ_CUDA(cudaMalloc(&c->f, bytes), "cudaMalloc f");
     BZ_CUDA(cudaMalloc(&c->f_new, bytes), "cudaMalloc f_new");
     c->SP = collide_slots_per_cell(c->mask);
@@ -190,7 +171,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
 int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
-    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->rec_buf); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
+    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
     delete c;

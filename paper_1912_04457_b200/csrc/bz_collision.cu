@@ -1,24 +1,27 @@
-// bz_collision.cu -- sample -> |M|^2 -> bracket -> symmetric deposit (S8a.2-8a.5), as two kernels per chunk of
-// spatial cells, coupled through a record buffer in HBM:
+// bz_collision.cu -- sample -> |M|^2 -> bracket -> symmetric deposit (S8a.2-8a.5) as ONE persistent, warp-specialised
+// kernel (one CTA of 16 warps per SM):
 //
-//   sample_kernel   one warp per "region" (C consecutive p1 cells of one spatial cell), lanes = samples.  Pure ALU:
-//                   Philox4x32-10, the boost, the binning.  Light on registers, so 4-6x more warps are resident
-//                   than the deposit kernel could afford and the long dependent chains (10 Philox rounds, sqrt,
-//                   div) overlap across warps.  About 46 % of the samples keep both outgoing legs in the box; they
-//                   are compacted (ballot + prefix) into the region's slice of the record buffer:
-//                   (i, j, k, l) cells, s, t and the weight K/(E1 E2) -- 40 bytes per accepted sample.
-//   deposit_kernel  one warp per region, always full batches of 32 accepted samples.
-//       gather   cp.async (LDGSTS) from the cell-major staging copy f_aos[xcell][pcell][SP] (SP = 8 doubles = 64 B per
-//                cell) into shared memory: for one sample the 32 lanes fetch its 4 cells x 8 slots, i.e. 8 sectors per
-//                instruction instead of 32 scattered ones, and the next batch's gather is in flight while the current
-//                batch is computed (double buffer).
-//       compute  each lane takes its own sample: <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh),
-//                4 x S deposits written back to shared memory.
-//       scatter  the same 8-lanes-per-cell mapping issues fp64 reductions (RED.E.ADD.F64, no return value) into the
-//                cell-major deposit scratch dN_aos, which stays in L2 while its spatial cell is being worked on.
+//   producer warps (12, warpgroups 1-3, 88 registers after setmaxnreg.dec)
+//       sample   pull work items (a run of p1 cells of one spatial cell) from a global counter; lanes = samples:
+//                Philox4x32-10, the boost, the binning (bz_sample.cuh).  About 46 % of the samples keep both outgoing
+//                legs in the box; they are compacted (ballot + prefix) straight into the record arrays of one of the
+//                warp's two shared-memory batch slots: (i, j, k, l), s, t and the weight K/(E1 E2).
+//       gather   when a slot holds 32 records: cp.async (LDGSTS) of the 4 x S occupation numbers of every sample from
+//                the cell-major staging copy f_aos[xcell][pcell][SP] (SP = 8 doubles = 64 B per cell) into the slot;
+//                for one sample the 32 lanes fetch its 4 cells x 8 slots, i.e. 8 sectors per instruction instead of 32
+//                scattered ones.  Completion is signalled to the consumer by cp.async.mbarrier.arrive on the slot's
+//                "full" mbarrier: the producer never waits for its own gathers and goes on sampling.
+//       scatter  when the warp needs the slot again and the consumer has signalled "done": the same 8-lanes-per-cell
+//                mapping issues fp64 reductions (RED.E.ADD.F64, no return value) of the slot's 4 x S deposits into
+//                the cell-major scratch dN_aos, which stays in L2 while its spatial cell is being worked on.
+//   consumer warps (4, warpgroup 0, one per SM sub-partition, 232 registers after setmaxnreg.inc)
+//       compute  serve three producers each in rotation: wait "full", every lane takes one sample of the batch:
+//                <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh), the 4 x S deposits overwrite the
+//                gathered f in the slot, arrive on "done".
+// The ALU-bound sampling and the latency-bound gather/scatter overlap on the same SM, the register file is split
+// 232 / 88 between the two roles, and no sample record ever leaves the SM.
 // Measured on B200 (profiles/): a RED (LDG) whose 32 lanes hit 32 different sectors costs 48 (32) cycles of the SM's
 // L1TEX path, the 8-lanes-per-cell form 15.7 (8.5) cycles for the same number of lanes.
-// The record buffer costs 2 x 40 B x 0.46 = 37 B of HBM traffic per sample, ~10 % of a step at the measured rates.
 #include "bz_channels.cuh"
 #include "bz_internal.h"
 
@@ -26,10 +29,14 @@ namespace bz {
 
 namespace {
 
-constexpr int kSampleWarps = 8;                  // warps per CTA, sample_kernel
-constexpr int kDepositWarps = 8;                 // warps per CTA, deposit_kernel
+constexpr int kConsumerWarps = 4;                // warpgroup 0
+constexpr int kProducerWarps = 12;               // warpgroups 1..3
+constexpr int kProducersPerConsumer = kProducerWarps / kConsumerWarps;
+constexpr int kCollideThreads = 32 * (kConsumerWarps + kProducerWarps);
+constexpr int kSlots = 2;                        // batch slots per producer warp
+constexpr int kConsumerRegs = 232, kProducerRegs = 88;   // 128 x 232 + 384 x 88 = 63488 <= 65536
 
-// doubles per cell in the staging layout: 1 for the pure-glue mask, 8 (half a 128-byte line) otherwise
+// doubles per cell in the global staging layout: 1 for the pure-glue mask, 8 (half a 128-byte line) otherwise
 template <int kMask>
 struct MaskTraits {
     static constexpr int SP = kMask == 0x01 ? 1 : 8;
@@ -37,155 +44,260 @@ struct MaskTraits {
 // layout index of species id = number of active ids below it
 __device__ __forceinline__ int slot_of(unsigned mask, int id) { return __popc(mask & ((1u << id) - 1u)); }
 
-// ------------------------------------------------------------------------------------------------ sampling
-__global__ void __launch_bounds__(kSampleWarps * 32) sample_kernel(const CollideParams P, int x_begin)
+// ------------------------------------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, unsigned count)
 {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int region_in_x = blockIdx.x * kSampleWarps + warp;            // region index inside the spatial cell
-    if (region_in_x >= P.regions_per_x) return;
-    const int xcell = x_begin + blockIdx.y;
-    const size_t region = (size_t)blockIdx.y * P.regions_per_x + region_in_x;
-    int4* __restrict__ rc = P.rec_cells + region * P.region_cap;
-    double* __restrict__ rs = P.rec_s + region * P.region_cap;
-    double* __restrict__ rt = P.rec_t + region * P.region_cap;
-    double* __restrict__ rw = P.rec_w + region * P.region_cap;
-    const int n = P.g.n;
-    const int i_begin = region_in_x * P.cells_per_region, i_end = min(i_begin + P.cells_per_region, P.Np);
-    int count = 0;
-    for (int i = i_begin; i < i_end; ++i) {
-        const int ipx = i % n, ipy = (i / n) % n, ipz = i / (n * n);
-        const double p1x = cell_centre(P.g, ipx), p1y = cell_centre(P.g, ipy), p1z = cell_centre(P.g, ipz);
-        const double E1 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p1x, p1x), __dmul_rn(p1y, p1y)), __dmul_rn(p1z, p1z)));
-        for (int base = 0; base < P.Ns; base += 32) {
-            const int smp = base + lane;
-            Sample sa;
-            sa.flag = 0;
-            if (smp < P.Ns)
-                sa = gen_sample(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, p1x, p1y, p1z, E1);
-            const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
-            if (sa.flag) {
-                const int pos = count + __popc(acc & ((1u << lane) - 1u));
-                rc[pos] = make_int4(i, sa.j, sa.k, sa.l);
-                rs[pos] = sa.s; rt[pos] = sa.t; rw[pos] = P.K / sa.E1E2;
-            }
-            count += __popc(acc);
-        }
-    }
-    if (lane == 0) P.rec_count[region] = count;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
 }
-
-// ------------------------------------------------------------------------------------------------ deposits
-template <int kSP>
-struct WarpSmem {
-    int cell[2][32][4];                          // i, j, k, l of the batch's samples
-    double stage[2][32 * (4 * kSP + 1)];         // f in, deposits out; odd stride: conflict-free per-lane access
-};
-
+__device__ __forceinline__ void mbar_arrive(uint64_t* b)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(smem_u32(b)) : "memory");
+}
+// arrive on b when all cp.async issued so far by this thread have landed (does not add to the expected count)
+__device__ __forceinline__ void mbar_arrive_on_cp_async(uint64_t* b)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity)
+{
+    const unsigned a = smem_u32(b);
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    } while (!ok);
+}
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc)
 {
-    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// fp64 reduction without return value (RED.E.ADD.F64), skipped for an exact zero
+__device__ __forceinline__ void red_add_nonzero(double* gdst, double v)
+{
+    asm volatile("{\n .reg .pred p;\n setp.neu.f64 p, %1, 0d0000000000000000;\n @p red.global.add.f64 [%0], %1;\n}"
+                 ::"l"(gdst), "d"(v) : "memory");
+}
 template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
+// ------------------------------------------------------------------------------------------------ batch slot
+// One batch of <= 32 accepted samples in shared memory.  stage holds, per sample, the occupation numbers of its 4 cells
+// (kCS doubles per cell) on the way in and the 4 x S deposits on the way out; the odd stride makes both the per-sample
+// access of the consumer (lane = sample) and the per-cell access of the producer (lanes = slots of a cell) conflict free.
+template <int kSP>
+struct Slot {
+    static constexpr int kCS = kSP == 1 ? 1 : 7;         // doubles per cell
+    static constexpr int kStride = 4 * kCS + 1;          // doubles per sample
+    double stage[32 * kStride];
+    double s[32], t[32], w[32];
+    int cell[32][4];                                     // i, j, k, l
+    double m2;                                           // regulator mass^2 of the batch's spatial cell
+    int nvalid;                                          // samples in the batch; < 0: the producer has finished
+    int xcell;
+    uint64_t full;                                       // producer -> consumer: records + gathered f are in place
+    uint64_t done;                                       // consumer -> producer: deposits are in place
+};
+
+// lane -> element of a sample: kSP slots of each of the 4 cells; 32 / (4 kSP) samples per instruction
+template <int kSP>
+struct LaneMap {
+    static constexpr int kEPS = 4 * kSP;                 // lanes per sample
+    static constexpr int kSPI = 32 / kEPS;               // samples per instruction
+    int sub, cc, sl;
+    __device__ __forceinline__ explicit LaneMap(int lane) : sub(lane / kEPS), cc((lane % kEPS) / kSP), sl(lane % kSP) {}
+};
+
+// ---- producer: issue the gather of the slot's batch and hand the slot to the consumer
+template <int kSP>
+__device__ __forceinline__ void submit_slot(Slot<kSP>& sl, const CollideParams& P, int lane, int nvalid, int xcell, double m2)
+{
+    using S = Slot<kSP>;
+    if (lane == 0) { sl.nvalid = nvalid; sl.xcell = xcell; sl.m2 = m2; }
+    __syncwarp();                                        // the records written by all lanes are visible to all lanes
+    if (nvalid > 0) {
+        const LaneMap<kSP> lm(lane);
+        const double* __restrict__ f_cell = P.f_aos + (size_t)xcell * P.Np * kSP + lm.sl;
+        double* dst = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
+        const int* cp = &sl.cell[lm.sub][lm.cc];
+        const bool on = lm.sl < P.S;
+#pragma unroll 8
+        for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI) {
+            if (m0 < nvalid) {
+                const int c = cp[4 * m0];
+                if (on && m0 + lm.sub < nvalid) cp_async8(dst + m0 * S::kStride, f_cell + (size_t)c * kSP);
+            }
+        }
+    }
+    mbar_arrive_on_cp_async(&sl.full);                   // 32 deferred arrivals: this lane's gathers have landed
+    if (lane == 0) mbar_arrive(&sl.full);                // + 1: header and records (release)
+}
+
+// ---- producer: flush the deposits the consumer left in the slot
+template <int kSP>
+__device__ __forceinline__ void scatter_slot(Slot<kSP>& sl, const CollideParams& P, int lane)
+{
+    using S = Slot<kSP>;
+    const int nvalid = sl.nvalid;
+    const LaneMap<kSP> lm(lane);
+    double* __restrict__ dN_cell = P.dN_aos + (size_t)sl.xcell * P.Np * kSP + lm.sl;
+    const double* src = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
+    const int* cp = &sl.cell[lm.sub][lm.cc];
+    const bool on = lm.sl < P.S;
+#pragma unroll 8
+    for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI) {
+        if (m0 < nvalid) {
+            const int c = cp[4 * m0];
+            double v = src[m0 * S::kStride];
+            if (!(on && m0 + lm.sub < nvalid)) v = 0.0;
+            red_add_nonzero(dN_cell + (size_t)c * kSP, v);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ the kernel
 template <int kMask>
-__global__ void __launch_bounds__(kDepositWarps * 32) deposit_kernel(const CollideParams P, int x_begin)
+__global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const CollideParams P)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
-    constexpr int kStride = 4 * kSP + 1;
+    using S = Slot<kSP>;
     constexpr bool kGlue = kMask < 0 || (kMask & 1);
     constexpr bool kQuark = kMask < 0 || (kMask & 0x7E);
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    S* slots = reinterpret_cast<S*>(smem_raw);           // [kProducerWarps][kSlots]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    WarpSmem<kSP>& sm = reinterpret_cast<WarpSmem<kSP>*>(smem_raw)[warp];
-    const unsigned mask = kMask >= 0 ? (unsigned)kMask : P.mask;
 
-    const int region_in_x = blockIdx.x * kDepositWarps + warp;
-    if (region_in_x >= P.regions_per_x) return;
-    const int xcell = x_begin + blockIdx.y;
-    const size_t region = (size_t)blockIdx.y * P.regions_per_x + region_in_x;
-    const int4* __restrict__ rc = P.rec_cells + region * P.region_cap;
-    const double* __restrict__ rs = P.rec_s + region * P.region_cap;
-    const double* __restrict__ rt = P.rec_t + region * P.region_cap;
-    const double* __restrict__ rw = P.rec_w + region * P.region_cap;
-    const double* __restrict__ f_cell = P.f_aos + (size_t)xcell * P.Np * kSP;
-    double* __restrict__ dN_cell = P.dN_aos + (size_t)xcell * P.Np * kSP;
-    const double m2 = P.m2[xcell];
-    const int count = P.rec_count[region];
-    const int nb = (count + 31) >> 5;
-    if (nb == 0) return;
-
-    // issue the gather of batch b into buffer b & 1; returns this lane's (s, t, w)
-    auto prefetch = [&](int b, double& s, double& t, double& w) {
-        const int e = b * 32 + lane, nvalid = min(32, count - b * 32), buf = b & 1;
-        int4 c = make_int4(0, 0, 0, 0);
-        s = 1.0; t = -0.5; w = 0.0;
-        if (lane < nvalid) { c = rc[e]; s = rs[e]; t = rt[e]; w = rw[e]; }
-        *reinterpret_cast<int4*>(&sm.cell[buf][lane][0]) = c;
-        __syncwarp();
-#pragma unroll 8
-        for (int m = 0; m < 4 * kSP; ++m) {
-            const int q = m * 32 + lane;
-            const int ee = q / (4 * kSP), rem = q % (4 * kSP), cc = rem / kSP, sl = rem % kSP;
-            if (ee < nvalid) cp_async8(&sm.stage[buf][ee * kStride + rem], f_cell + (size_t)sm.cell[buf][ee][cc] * kSP + sl);
-        }
-        cp_async_commit();
-    };
-
-    double s, t, w, s_next = 1.0, t_next = -0.5, w_next = 0.0;
-    prefetch(0, s, t, w);
-    for (int b = 0; b < nb; ++b) {
-        const int buf = b & 1, nvalid = min(32, count - b * 32);
-        if (b + 1 < nb) {
-            prefetch(b + 1, s_next, t_next, w_next);
-            cp_async_wait<1>();
-        } else {
-            cp_async_wait<0>();
-        }
-        __syncwarp();
-
-        // ---- compute: lane e owns sample e of the batch
-        if (lane < nvalid) {
-            double* st = sm.stage[buf] + lane * kStride;
-            double fi[7], fj[7], fk[7], fl[7];
-#pragma unroll
-            for (int id = 0; id < 7; ++id) {
-                if ((mask >> id) & 1u) {
-                    const int sl = slot_of(mask, id);
-                    fi[id] = st[sl]; fj[id] = st[kSP + sl]; fk[id] = st[2 * kSP + sl]; fl[id] = st[3 * kSP + sl];
-                } else {
-                    fi[id] = fj[id] = fk[id] = fl[id] = 0.0;
-                }
-            }
-            const double u = __dsub_rn(-s, t);
-            const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, P.g4 * w);
-            double dI[7], dJ[7], dK[7], dL[7];
-            deposit<kMask>(mask, fi, fj, fk, fl, M, dI, dJ, dK, dL);
-#pragma unroll
-            for (int id = 0; id < 7; ++id) {
-                if ((mask >> id) & 1u) {
-                    const int sl = slot_of(mask, id);
-                    st[sl] = dI[id]; st[kSP + sl] = dJ[id]; st[2 * kSP + sl] = dK[id]; st[3 * kSP + sl] = dL[id];
-                }
-            }
-        }
-        __syncwarp();
-
-        // ---- scatter: 32/kSP cells per instruction, kSP consecutive lanes on the slots of one cell
-#pragma unroll 8
-        for (int m = 0; m < 4 * kSP; ++m) {
-            const int q = m * 32 + lane;
-            const int ee = q / (4 * kSP), rem = q % (4 * kSP), cc = rem / kSP, sl = rem % kSP;
-            if (ee < nvalid && sl < P.S) {
-                const double v = sm.stage[buf][ee * kStride + rem];
-                if (v != 0.0) atomicAdd(dN_cell + (size_t)sm.cell[buf][ee][cc] * kSP + sl, v);   // result unused: RED
-            }
-        }
-        __syncwarp();
-        s = s_next; t = t_next; w = w_next;
+    if (threadIdx.x < kProducerWarps * kSlots) {
+        mbar_init(&slots[threadIdx.x].full, 33);
+        mbar_init(&slots[threadIdx.x].done, 1);
     }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+
+    if (warp < kConsumerWarps) {
+        // ======================================================================================== consumer
+        setmaxnreg_inc<kConsumerRegs>();
+        const unsigned mask = kMask >= 0 ? (unsigned)kMask : P.mask;
+        unsigned alive = (1u << kProducersPerConsumer) - 1u;   // producers of this consumer still running
+        unsigned cur = 0;                                      // bit q: next slot of producer q
+        unsigned par = 0;                                      // bit 2q+slot: parity of the next "full" phase
+        int q = 0;
+        while (alive) {
+            if (!((alive >> q) & 1u)) { q = (q + 1) % kProducersPerConsumer; continue; }
+            const int si = (cur >> q) & 1u;
+            S& sl = slots[(warp + kConsumerWarps * q) * kSlots + si];
+            mbar_wait(&sl.full, (par >> (2 * q + si)) & 1u);
+            par ^= 1u << (2 * q + si);
+            cur ^= 1u << q;
+            const int nvalid = sl.nvalid;
+            if (nvalid < 0) { alive &= ~(1u << q); q = (q + 1) % kProducersPerConsumer; continue; }
+            if (lane < nvalid) {
+                double* st = sl.stage + lane * S::kStride;
+                const double s = sl.s[lane], t = sl.t[lane], w = sl.w[lane], m2 = sl.m2;
+                double fi[7], fj[7], fk[7], fl[7];
+#pragma unroll
+                for (int id = 0; id < 7; ++id) {
+                    if ((mask >> id) & 1u) {
+                        const int a = slot_of(mask, id);
+                        fi[id] = st[a]; fj[id] = st[S::kCS + a]; fk[id] = st[2 * S::kCS + a]; fl[id] = st[3 * S::kCS + a];
+                    } else {
+                        fi[id] = fj[id] = fk[id] = fl[id] = 0.0;
+                    }
+                }
+                const double u = __dsub_rn(-s, t);
+                const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, P.g4 * w);
+                double dI[7], dJ[7], dK[7], dL[7];
+                deposit<kMask>(mask, fi, fj, fk, fl, M, dI, dJ, dK, dL);
+#pragma unroll
+                for (int id = 0; id < 7; ++id) {
+                    if ((mask >> id) & 1u) {
+                        const int a = slot_of(mask, id);
+                        st[a] = dI[id]; st[S::kCS + a] = dJ[id]; st[2 * S::kCS + a] = dK[id]; st[3 * S::kCS + a] = dL[id];
+                    }
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sl.done);
+            q = (q + 1) % kProducersPerConsumer;
+        }
+        return;
+    }
+
+    // ============================================================================================ producer
+    setmaxnreg_dec<kProducerRegs>();
+    const int pw = warp - kConsumerWarps;
+    S* my = slots + pw * kSlots;
+    const int n = P.g.n;
+    int cur = 0;                         // slot being filled
+    int count = 0;                       // records in it
+    unsigned busy = 0;                   // bit s: slot s is with the consumer (submitted, deposits not yet flushed)
+    unsigned dpar = 0;                   // bit s: parity of the next "done" phase of slot s
+    // make slot s writable again: wait for the consumer, flush its deposits
+    auto acquire = [&](int s) {
+        if ((busy >> s) & 1u) {
+            mbar_wait(&my[s].done, (dpar >> s) & 1u);
+            dpar ^= 1u << s;
+            busy &= ~(1u << s);
+            scatter_slot<kSP>(my[s], P, lane);
+            __syncwarp();
+        }
+    };
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(P.work_counter, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= P.n_items) break;
+        const int xi = (int)(item / (unsigned)P.regions_per_x), region = (int)(item % (unsigned)P.regions_per_x);
+        const int xcell = P.x_begin + xi;
+        const double m2 = P.m2[xcell];
+        const int i_begin = region * P.cells_per_region, i_end = min(i_begin + P.cells_per_region, P.Np);
+        for (int i = i_begin; i < i_end; ++i) {
+            const int ipx = i % n, ipy = (i / n) % n, ipz = i / (n * n);
+            const double p1x = cell_centre(P.g, ipx), p1y = cell_centre(P.g, ipy), p1z = cell_centre(P.g, ipz);
+            const double E1 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p1x, p1x), __dmul_rn(p1y, p1y)), __dmul_rn(p1z, p1z)));
+            for (int base = 0; base < P.Ns; base += 32) {
+                const int smp = base + lane;
+                Sample sa;
+                sa.flag = 0;
+                if (smp < P.Ns)
+                    sa = gen_sample(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, p1x, p1y, p1z, E1);
+                const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
+                if (acc == 0u) continue;
+                int pos = count + __popc(acc & ((1u << lane) - 1u));
+                const double w = sa.flag ? P.K / sa.E1E2 : 0.0;
+                if (sa.flag && pos < 32) {
+                    S& sl = my[cur];
+                    *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(i, sa.j, sa.k, sa.l);
+                    sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.w[pos] = w;
+                }
+                count += __popc(acc);
+                if (count >= 32) {
+                    submit_slot<kSP>(my[cur], P, lane, 32, xcell, m2);
+                    busy |= 1u << cur;
+                    cur ^= 1;
+                    acquire(cur);
+                    count -= 32;
+                    pos -= 32;
+                    if (sa.flag && pos >= 0) {
+                        S& sl = my[cur];
+                        *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(i, sa.j, sa.k, sa.l);
+                        sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.w[pos] = w;
+                    }
+                }
+            }
+        }
+        if (count > 0) {                                     // batches never mix spatial cells: flush the partial one
+            submit_slot<kSP>(my[cur], P, lane, count, xcell, m2);
+            busy |= 1u << cur;
+            cur ^= 1;
+            acquire(cur);
+            count = 0;
+        }
+    }
+    submit_slot<kSP>(my[cur], P, lane, -1, 0, 0.0);          // terminator (the current slot is always writable)
+    acquire(cur ^ 1);
 }
 
 __global__ void debug_samples_kernel(const CollideParams P, int xcell, int p_begin, int p_end, int* cells, double* stu)
@@ -232,18 +344,17 @@ __global__ void __launch_bounds__(256) finalize_kernel(double* __restrict__ dN_a
 }
 
 template <int kMask>
-cudaError_t launch_deposit(const CollideParams& P, int x_begin, int nxc, cudaStream_t st)
+cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t st)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
-    const size_t smem = sizeof(WarpSmem<kSP>) * kDepositWarps;
+    const size_t smem = sizeof(Slot<kSP>) * kProducerWarps * kSlots;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(deposit_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    dim3 grid((P.regions_per_x + kDepositWarps - 1) / kDepositWarps, nxc), block(kDepositWarps * 32);
-    deposit_kernel<kMask><<<grid, block, smem, st>>>(P, x_begin);
+    collide_kernel<kMask><<<ctas, kCollideThreads, smem, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }
@@ -252,32 +363,28 @@ cudaError_t launch_deposit(const CollideParams& P, int x_begin, int nxc, cudaStr
 
 int collide_slots_per_cell(unsigned mask) { return mask == 0x01u ? 1 : 8; }
 
-// p1 cells per region: long regions amortise the final partial batch, short ones fill the GPU on small grids
-int collide_cells_per_region(int Np, int Nx)
+// p1 cells per work item: long items amortise the final partial batch, short ones balance the load on small grids
+int collide_cells_per_region(int Np, int Nx, int sms)
 {
     const long long total_cells = (long long)Np * Nx;
-    const long long c = total_cells / (148LL * 8 * 8);
-    return (int)(c < 1 ? 1 : (c > 16 ? 16 : c));
+    const long long c = total_cells / ((long long)sms * kProducerWarps * 8);
+    return (int)(c < 1 ? 1 : (c > 32 ? 32 : c));
 }
 
-cudaError_t launch_collide(const CollideParams& P, cudaStream_t st)
+// one persistent CTA per SM (fewer when there is less work than producer warps)
+cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st)
 {
-    for (int x0 = 0; x0 < P.Nx; x0 += P.x_per_chunk) {
-        const int nxc = P.Nx - x0 < P.x_per_chunk ? P.Nx - x0 : P.x_per_chunk;
-        dim3 grid((P.regions_per_x + kSampleWarps - 1) / kSampleWarps, nxc), block(kSampleWarps * 32);
-        sample_kernel<<<grid, block, 0, st>>>(P, x0);
-        ++g_launch_count;
-        cudaError_t e = cudaGetLastError();
-        if (e != cudaSuccess) return e;
-        switch (P.mask) {
-        case 0x01u: e = launch_deposit<0x01>(P, x0, nxc, st); break;
-        case 0x7Eu: e = launch_deposit<0x7E>(P, x0, nxc, st); break;
-        case 0x7Fu: e = launch_deposit<0x7F>(P, x0, nxc, st); break;
-        default:    e = launch_deposit<-1>(P, x0, nxc, st); break;
-        }
-        if (e != cudaSuccess) return e;
+    cudaError_t e = cudaMemsetAsync(P.work_counter, 0, sizeof(unsigned), st);
+    if (e != cudaSuccess) return e;
+    int ctas = (int)((P.n_items + kProducerWarps - 1) / kProducerWarps);
+    if (ctas > sms) ctas = sms;
+    if (ctas < 1) ctas = 1;
+    switch (P.mask) {
+    case 0x01u: return launch_collide_mask<0x01>(P, ctas, st);
+    case 0x7Eu: return launch_collide_mask<0x7E>(P, ctas, st);
+    case 0x7Fu: return launch_collide_mask<0x7F>(P, ctas, st);
+    default:    return launch_collide_mask<-1>(P, ctas, st);
     }
-    return cudaSuccess;
 }
 
 cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin, int p_end, int* cells, double* stu,

@@ -21,14 +21,11 @@ struct CollideParams {
     double* dN_aos;       // [Nx][Np][SP] deposit scratch in number units, zero on entry
     const double* m2;     // [Nx] regulator mass^2
     int S, Np, Nx, Ns;
-    // record buffer written by sample_kernel, read by deposit_kernel (one chunk of spatial cells at a time)
-    int4* rec_cells;      // [regions in chunk][region_cap] (i, j, k, l)
-    double *rec_s, *rec_t, *rec_w;   // [regions in chunk][region_cap]
-    int* rec_count;       // [regions in chunk] accepted samples of the region
-    int cells_per_region; // p1 cells per region (one warp each)
-    int regions_per_x;    // ceil(Np / cells_per_region)
-    int region_cap;       // cells_per_region * Ns record slots per region (worst case: every sample accepted)
-    int x_per_chunk;      // spatial cells per sample/deposit kernel pair
+    unsigned* work_counter;   // device: next work item of the persistent kernel (zeroed before every launch)
+    unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
+    int x_begin;              // first spatial cell (0; items address xcell = x_begin + item / regions_per_x)
+    int cells_per_region;     // p1 cells per work item (one producer warp each)
+    int regions_per_x;        // ceil(Np / cells_per_region)
     uint32_t seed, step;
     double K;             // dtG Vp / (2048 pi^4 Ns)                       (S8c step 0)
     double g4;            // (4 pi alpha_s)^2
@@ -59,9 +56,9 @@ struct bz_ctx_impl {
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
     double *f_aos, *dN_aos;          // device, Nx*Np*SP each (cell-major staging for the collision kernel)
     int SP;                          // doubles per cell in the staging layout
-    // record buffer (see CollideParams), sized for x_per_chunk spatial cells at the current Ns
-    void* rec_buf; size_t rec_bytes; int rec_Ns;
-    int cells_per_region, regions_per_x, x_per_chunk;
+    unsigned* work_counter;          // device, 1 word
+    int sms;                         // SMs of the device (persistent grid size)
+    int cells_per_region, regions_per_x;
     double *m2;                      // device [Nx]
     double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|)
     double *mom;                     // device [2*S*Nx + 2*S + Nx]
@@ -76,8 +73,8 @@ extern std::atomic<unsigned long long> g_launch_count;
 
 // launchers (each returns the cudaError_t of the launch)
 int collide_slots_per_cell(unsigned mask);
-int collide_cells_per_region(int Np, int Nx);
-cudaError_t launch_collide(const CollideParams& P, cudaStream_t st);
+int collide_cells_per_region(int Np, int Nx, int sms);
+cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st);
 cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, int Np, cudaStream_t st);
 cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin, int p_end, int* cells, double* stu,
                                  cudaStream_t st);
