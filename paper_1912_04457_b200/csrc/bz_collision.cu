@@ -14,12 +14,12 @@
 //       scatter  when the warp needs the slot again and the consumer has signalled "done": the same 8-lanes-per-cell
 //                mapping issues fp64 reductions (RED.E.ADD.F64, no return value) of the slot's 4 x S deposits into
 //                the cell-major scratch dN_aos, which stays in L2 while its spatial cell is being worked on.
-//   consumer warps (4, warpgroup 0, one per SM sub-partition, 232 registers after setmaxnreg.inc)
+//   consumer warps (4, warpgroup 0, one per SM sub-partition, 240 registers after setmaxnreg.inc)
 //       compute  serve three producers each in rotation: wait "full", every lane takes one sample of the batch:
 //                <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh), the 4 x S deposits overwrite the
 //                gathered f in the slot, arrive on "done".
 // The ALU-bound sampling and the latency-bound gather/scatter overlap on the same SM, the register file is split
-// 232 / 88 between the two roles, and no sample record ever leaves the SM.
+// 240 / 88 between the two roles, and no sample record ever leaves the SM.
 // Measured on B200 (profiles/): a RED (LDG) whose 32 lanes hit 32 different sectors costs 48 (32) cycles of the SM's
 // L1TEX path, the 8-lanes-per-cell form 15.7 (8.5) cycles for the same number of lanes.
 #include "bz_channels.cuh"
@@ -34,7 +34,7 @@ constexpr int kProducerWarps = 12;               // warpgroups 1..3
 constexpr int kProducersPerConsumer = kProducerWarps / kConsumerWarps;
 constexpr int kCollideThreads = 32 * (kConsumerWarps + kProducerWarps);
 constexpr int kSlots = 2;                        // batch slots per producer warp
-constexpr int kConsumerRegs = 232, kProducerRegs = 88;   // 128 x 232 + 384 x 88 = 63488 <= 65536
+constexpr int kConsumerRegs = 240, kProducerRegs = 88;   // 128 x 240 + 384 x 88 = 64512 <= 65536
 
 // doubles per cell in the global staging layout: 1 for the pure-glue mask, 8 (half a 128-byte line) otherwise
 template <int kMask>
@@ -59,14 +59,17 @@ __device__ __forceinline__ void mbar_arrive_on_cp_async(uint64_t* b)
 {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(b)) : "memory");
 }
+// one try_wait: the hardware suspends the warp until the phase completes or ~ns nanoseconds have passed
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* b, unsigned parity, unsigned ns)
+{
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity)
 {
-    const unsigned a = smem_u32(b);
-    unsigned ok;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(ok) : "r"(a), "r"(parity) : "memory");
-    } while (!ok);
+    while (!mbar_try_wait(b, parity, 2000u)) {}
 }
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc)
 {
@@ -119,15 +122,17 @@ __device__ __forceinline__ void submit_slot(Slot<kSP>& sl, const CollideParams& 
     __syncwarp();                                        // the records written by all lanes are visible to all lanes
     if (nvalid > 0) {
         const LaneMap<kSP> lm(lane);
-        const double* __restrict__ f_cell = P.f_aos + (size_t)xcell * P.Np * kSP + lm.sl;
-        double* dst = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
-        const int* cp = &sl.cell[lm.sub][lm.cc];
-        const bool on = lm.sl < P.S;
-#pragma unroll 8
-        for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI) {
-            if (m0 < nvalid) {
-                const int c = cp[4 * m0];
-                if (on && m0 + lm.sub < nvalid) cp_async8(dst + m0 * S::kStride, f_cell + (size_t)c * kSP);
+        if (lm.sl < P.S) {                               // pad lanes (slot 7 of a cell) sit the gather out
+            const double* __restrict__ src = P.f_aos + (size_t)xcell * P.Np * kSP + lm.sl;
+            double* dst = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
+            const int* cp = &sl.cell[lm.sub][lm.cc];
+            if (nvalid == 32) {
+#pragma unroll
+                for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI)
+                    cp_async8(dst + m0 * S::kStride, src + (size_t)cp[4 * m0] * kSP);
+            } else {
+                for (int m0 = 0; m0 + lm.sub < nvalid; m0 += LaneMap<kSP>::kSPI)
+                    cp_async8(dst + m0 * S::kStride, src + (size_t)cp[4 * m0] * kSP);
             }
         }
     }
@@ -142,17 +147,17 @@ __device__ __forceinline__ void scatter_slot(Slot<kSP>& sl, const CollideParams&
     using S = Slot<kSP>;
     const int nvalid = sl.nvalid;
     const LaneMap<kSP> lm(lane);
-    double* __restrict__ dN_cell = P.dN_aos + (size_t)sl.xcell * P.Np * kSP + lm.sl;
-    const double* src = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
-    const int* cp = &sl.cell[lm.sub][lm.cc];
-    const bool on = lm.sl < P.S;
-#pragma unroll 8
-    for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI) {
-        if (m0 < nvalid) {
-            const int c = cp[4 * m0];
-            double v = src[m0 * S::kStride];
-            if (!(on && m0 + lm.sub < nvalid)) v = 0.0;
-            red_add_nonzero(dN_cell + (size_t)c * kSP, v);
+    if (lm.sl < P.S) {
+        double* __restrict__ dst = P.dN_aos + (size_t)sl.xcell * P.Np * kSP + lm.sl;
+        const double* src = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
+        const int* cp = &sl.cell[lm.sub][lm.cc];
+        if (nvalid == 32) {
+#pragma unroll
+            for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI)
+                red_add_nonzero(dst + (size_t)cp[4 * m0] * kSP, src[m0 * S::kStride]);
+        } else {
+            for (int m0 = 0; m0 + lm.sub < nvalid; m0 += LaneMap<kSP>::kSPI)
+                red_add_nonzero(dst + (size_t)cp[4 * m0] * kSP, src[m0 * S::kStride]);
         }
     }
 }
@@ -185,10 +190,11 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         unsigned par = 0;                                      // bit 2q+slot: parity of the next "full" phase
         int q = 0;
         while (alive) {
+            // poll the alive producers in rotation; each try suspends the warp for at most ~0.3 us
             if (!((alive >> q) & 1u)) { q = (q + 1) % kProducersPerConsumer; continue; }
             const int si = (cur >> q) & 1u;
             S& sl = slots[(warp + kConsumerWarps * q) * kSlots + si];
-            mbar_wait(&sl.full, (par >> (2 * q + si)) & 1u);
+            if (!mbar_try_wait(&sl.full, (par >> (2 * q + si)) & 1u, 300u)) { q = (q + 1) % kProducersPerConsumer; continue; }
             par ^= 1u << (2 * q + si);
             cur ^= 1u << q;
             const int nvalid = sl.nvalid;
