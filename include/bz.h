@@ -49,7 +49,7 @@ int bz_destroy(bz_ctx* ctx);
 
 int bz_set_stream(bz_ctx* ctx, void* cuda_stream);              /* cudaStream_t; NULL = default stream        */
 int bz_set_seed(bz_ctx* ctx, unsigned long long seed);          /* Philox key word 0 = low 32 bits (S8c step 1) */
-int bz_set_samples(bz_ctx* ctx, int samples_per_cell);          /* kinematic samples per (xcell, pcell) (S3)  */
+int bz_set_samples(bz_ctx* ctx, int samples_per_cell);          /* kinematic samples per (xcell, pcell) (S3), 1..2^24 */
 int bz_set_step(bz_ctx* ctx, unsigned step);                    /* step counter used by bz_step               */
 
 /* Copy S*Nx*Np doubles into / out of the context.  on_device != 0: f is a device pointer (async copy on the

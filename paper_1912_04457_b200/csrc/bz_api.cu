@@ -43,7 +43,19 @@ GridConst grid_const(const bz_ctx* c)
     g.pmin = c->grid.pmin;
     g.L = c->grid.pmax - c->grid.pmin;
     g.dp = g.L / g.n;
-    g.inv_dp = (double)g.n / g.L;
+    // fast path of the binning (bz_sample.cuh): 2^k q with k <= 20 chosen so that 2^k |q| < 2^31 for every reachable
+    // momentum component, |p| <= E1 + E2 <= 2 sqrt(3) max(|pmin|, |pmax|)
+    const double pm = std::fmax(std::fabs(c->grid.pmin), std::fabs(c->grid.pmax));
+    const double qmax = (2.0 * std::sqrt(3.0) * pm + std::fabs(g.pmin)) / g.dp + 2.0;
+    int k = 20;
+    while (k > 0 && std::ldexp(qmax, k) >= 1073741824.0) --k;
+    if (k >= 6) {
+        g.bin_shift = k;
+        g.bin_a = std::ldexp(1.0 / g.dp, k);
+        g.bin_b = -g.pmin * g.bin_a;
+    } else {                        // degenerate box far from the origin: every sample takes the exact binning
+        g.bin_shift = 4; g.bin_a = 0.0; g.bin_b = 0.0;
+    }
     return g;
 }
 
@@ -57,9 +69,9 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
     const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
-    P.K = dtG * Vp / (2048.0 * (kPi * kPi * kPi * kPi) * c->Ns);
+    const double K = dtG * Vp / (2048.0 * (kPi * kPi * kPi * kPi) * c->Ns);
     const double g2 = 4.0 * kPi * c->alpha_s;
-    P.g4 = g2 * g2;
+    P.g4K = (g2 * g2) * K;
     P.mask = c->mask;
     for (int a = 0; a < 7; ++a) P.slot[a] = c->slot[a];
     return P;
@@ -180,7 +192,7 @@ int bz_destroy(bz_ctx* c)
 
 int bz_set_stream(bz_ctx* c, void* s) { if (!c) return -1; c->stream = (cudaStream_t)s; return 0; }
 int bz_set_seed(bz_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
-int bz_set_samples(bz_ctx* c, int n) { if (!c || n < 1) return -1; c->Ns = n; return 0; }
+int bz_set_samples(bz_ctx* c, int n) { if (!c || n < 1 || n > (1 << 24)) return -1; c->Ns = n; return 0; }
 int bz_set_step(bz_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
 const char* bz_last_error(const bz_ctx* c) { return c ? c->err.c_str() : "null context"; }
 

@@ -35,13 +35,29 @@ struct MsqSet {
     double a_t, a_u;      // q1 q2 -> q1 q2 (different flavours), straight / crossed
 };
 
+// 1/x to ~1 ulp without the IEEE division sequence: the 20-bit hardware seed (MUFU.RCP64H) and two Newton steps.
+// Nothing here feeds a sampled index, so correct rounding is not required (S8c step 4: "FMA allowed from here on").
+BZ_HD double rcp_fast(double x)
+{
+#if defined(__CUDA_ARCH__)
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+#else
+    return 1.0 / x;
+#endif
+}
+
 // Table I with the regulated propagators tt = t - m^2, ut = u - m^2; SU(3): 8 dF^2 CF^2/dA = 16,
 // 16 dF CF (CF - CA/2) = -32/3, 8 dF CF^2 = 128/3, 8 dF CF CA = 96, 16 dA CA^2 = 1152.
 template <bool kGlue, bool kQuark>
 BZ_HD MsqSet msq_set(double s, double t, double u, double m2, double g4w)
 {
     MsqSet M = {};
-    const double it = 1.0 / (t - m2), iu = 1.0 / (u - m2), is = 1.0 / s;
+    const double it = rcp_fast(t - m2), iu = rcp_fast(u - m2), is = rcp_fast(s);
     const double s2 = s * s, t2 = t * t, u2 = u * u;
     const double it2 = it * it, iu2 = iu * iu, is2 = is * is;
     const double c16 = 16.0 * g4w, c323 = (32.0 / 3.0) * g4w, c1283 = (128.0 / 3.0) * g4w;

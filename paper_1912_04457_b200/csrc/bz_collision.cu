@@ -95,7 +95,7 @@ struct Slot {
     static constexpr int kCS = kSP == 1 ? 1 : 7;         // doubles per cell
     static constexpr int kStride = 4 * kCS + 1;          // doubles per sample
     double stage[32 * kStride];
-    double s[32], t[32], w[32];
+    double s[32], t[32], e12[32];                        // Mandelstam s, t and E1 E2 of the sample
     int cell[32][4];                                     // i, j, k, l
     double m2;                                           // regulator mass^2 of the batch's spatial cell
     int nvalid;                                          // samples in the batch; < 0: the producer has finished
@@ -103,6 +103,8 @@ struct Slot {
     uint64_t full;                                       // producer -> consumer: records + gathered f are in place
     uint64_t done;                                       // consumer -> producer: deposits are in place
 };
+
+constexpr int kRetryCap = 64;                    // per producer warp: samples whose two Marsaglia attempts both failed
 
 // lane -> element of a sample: kSP slots of each of the 4 cells; 32 / (4 kSP) samples per instruction
 template <int kSP>
@@ -201,7 +203,8 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             if (nvalid < 0) { alive &= ~(1u << q); q = (q + 1) % kProducersPerConsumer; continue; }
             if (lane < nvalid) {
                 double* st = sl.stage + lane * S::kStride;
-                const double s = sl.s[lane], t = sl.t[lane], w = sl.w[lane], m2 = sl.m2;
+                const double s = sl.s[lane], t = sl.t[lane], m2 = sl.m2;
+                const double g4w = P.g4K * rcp_fast(sl.e12[lane]);            // g^4 K / (E1 E2), S8c step 6
                 double fi[7], fj[7], fk[7], fl[7];
 #pragma unroll
                 for (int id = 0; id < 7; ++id) {
@@ -213,7 +216,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                     }
                 }
                 const double u = __dsub_rn(-s, t);
-                const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, P.g4 * w);
+                const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
                 double dI[7], dJ[7], dK[7], dL[7];
                 deposit<kMask>(mask, fi, fj, fk, fl, M, dI, dJ, dK, dL);
 #pragma unroll
@@ -235,21 +238,12 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
     setmaxnreg_dec<kProducerRegs>();
     const int pw = warp - kConsumerWarps;
     S* my = slots + pw * kSlots;
-    const int n = P.g.n;
+    int2* retry = reinterpret_cast<int2*>(slots + kProducerWarps * kSlots) + pw * kRetryCap;
     int cur = 0;                         // slot being filled
     int count = 0;                       // records in it
+    int rcount = 0;                      // entries in the retry list
     unsigned busy = 0;                   // bit s: slot s is with the consumer (submitted, deposits not yet flushed)
     unsigned dpar = 0;                   // bit s: parity of the next "done" phase of slot s
-    // make slot s writable again: wait for the consumer, flush its deposits
-    auto acquire = [&](int s) {
-        if ((busy >> s) & 1u) {
-            mbar_wait(&my[s].done, (dpar >> s) & 1u);
-            dpar ^= 1u << s;
-            busy &= ~(1u << s);
-            scatter_slot<kSP>(my[s], P, lane);
-            __syncwarp();
-        }
-    };
     for (;;) {
         unsigned item = 0;
         if (lane == 0) item = atomicAdd(P.work_counter, 1u);
@@ -258,39 +252,70 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         const int xi = (int)(item / (unsigned)P.regions_per_x), region = (int)(item % (unsigned)P.regions_per_x);
         const int xcell = P.x_begin + xi;
         const double m2 = P.m2[xcell];
-        const int i_begin = region * P.cells_per_region, i_end = min(i_begin + P.cells_per_region, P.Np);
-        for (int i = i_begin; i < i_end; ++i) {
-            const int ipx = i % n, ipy = (i / n) % n, ipz = i / (n * n);
-            const double p1x = cell_centre(P.g, ipx), p1y = cell_centre(P.g, ipy), p1z = cell_centre(P.g, ipz);
-            const double E1 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p1x, p1x), __dmul_rn(p1y, p1y)), __dmul_rn(p1z, p1z)));
-            for (int base = 0; base < P.Ns; base += 32) {
-                const int smp = base + lane;
-                Sample sa;
-                sa.flag = 0;
-                if (smp < P.Ns)
-                    sa = gen_sample(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, p1x, p1y, p1z, E1);
-                const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
-                if (acc == 0u) continue;
-                int pos = count + __popc(acc & ((1u << lane) - 1u));
-                const double w = sa.flag ? P.K / sa.E1E2 : 0.0;
-                if (sa.flag && pos < 32) {
-                    S& sl = my[cur];
-                    *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(i, sa.j, sa.k, sa.l);
-                    sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.w[pos] = w;
+        const int i_end = min((region + 1) * P.cells_per_region, P.Np);
+        int i = region * P.cells_per_region, base = 0;
+        double p1x = 0.0, p1y = 0.0, p1z = 0.0, E1 = 0.0;
+        bool cell_valid = false;
+        for (;;) {
+            // ---- next 32 (cell, sample, first attempt) triples: a full warp of retries if there is one, else fresh samples
+            int ci, smp;
+            unsigned kstart;
+            bool active;
+            if (rcount >= 32 || (i >= i_end && rcount > 0)) {
+                const int nr = min(rcount, 32);
+                rcount -= nr;
+                active = lane < nr;
+                const int2 e = active ? retry[rcount + lane] : make_int2(0, 0);
+                ci = e.x; smp = e.y & 0x1ffffff; kstart = (unsigned)e.y >> 25;
+                cell_kinematics(P.g, ci, p1x, p1y, p1z, E1);              // per lane
+                cell_valid = false;
+            } else if (i < i_end) {
+                if (!cell_valid) { cell_kinematics(P.g, i, p1x, p1y, p1z, E1); cell_valid = true; }
+                ci = i; smp = base + lane; kstart = 0u;
+                active = smp < P.Ns;
+                base += 32;
+                if (base >= P.Ns) { base = 0; ++i; cell_valid = false; }
+            } else {
+                break;
+            }
+            Sample sa;
+            sa.flag = 0; sa.retry = 0;
+            if (active)
+                sa = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+            const unsigned lt = (1u << lane) - 1u;
+            const unsigned rb = __ballot_sync(0xffffffffu, sa.retry);
+            if (rb) {
+                if (sa.retry) retry[rcount + __popc(rb & lt)] = make_int2(ci, smp | (int)((kstart + 2u) << 25));
+                rcount += __popc(rb);
+                __syncwarp();
+            }
+            // ---- compact the accepted samples into the current slot; a full slot goes to the consumer
+            const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
+            if (acc == 0u) continue;
+            int pos = count + __popc(acc & lt);
+            if (sa.flag && pos < 32) {
+                S& sl = my[cur];
+                *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
+                sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.e12[pos] = sa.E1E2;
+            }
+            count += __popc(acc);
+            if (count >= 32) {
+                submit_slot<kSP>(my[cur], P, lane, 32, xcell, m2);
+                busy |= 1u << cur;
+                cur ^= 1;
+                if ((busy >> cur) & 1u) {                    // make the other slot writable: wait for the consumer, flush
+                    mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
+                    dpar ^= 1u << cur;
+                    busy &= ~(1u << cur);
+                    scatter_slot<kSP>(my[cur], P, lane);
+                    __syncwarp();
                 }
-                count += __popc(acc);
-                if (count >= 32) {
-                    submit_slot<kSP>(my[cur], P, lane, 32, xcell, m2);
-                    busy |= 1u << cur;
-                    cur ^= 1;
-                    acquire(cur);
-                    count -= 32;
-                    pos -= 32;
-                    if (sa.flag && pos >= 0) {
-                        S& sl = my[cur];
-                        *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(i, sa.j, sa.k, sa.l);
-                        sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.w[pos] = w;
-                    }
+                count -= 32;
+                pos -= 32;
+                if (sa.flag && pos >= 0) {
+                    S& sl = my[cur];
+                    *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
+                    sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.e12[pos] = sa.E1E2;
                 }
             }
         }
@@ -298,24 +323,37 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             submit_slot<kSP>(my[cur], P, lane, count, xcell, m2);
             busy |= 1u << cur;
             cur ^= 1;
-            acquire(cur);
+            if ((busy >> cur) & 1u) {
+                mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
+                dpar ^= 1u << cur;
+                busy &= ~(1u << cur);
+                scatter_slot<kSP>(my[cur], P, lane);
+                __syncwarp();
+            }
             count = 0;
         }
     }
     submit_slot<kSP>(my[cur], P, lane, -1, 0, 0.0);          // terminator (the current slot is always writable)
-    acquire(cur ^ 1);
+    cur ^= 1;
+    if ((busy >> cur) & 1u) {
+        mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
+        scatter_slot<kSP>(my[cur], P, lane);
+    }
 }
 
 __global__ void debug_samples_kernel(const CollideParams P, int xcell, int p_begin, int p_end, int* cells, double* stu)
 {
     const long long total = (long long)(p_end - p_begin) * P.Ns;
-    const int n = P.g.n;
     for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
         const int i = p_begin + (int)(q / P.Ns), smp = (int)(q % P.Ns);
-        const int ipx = i % n, ipy = (i / n) % n, ipz = i / (n * n);
-        const double p1x = cell_centre(P.g, ipx), p1y = cell_centre(P.g, ipy), p1z = cell_centre(P.g, ipz);
-        const double E1 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p1x, p1x), __dmul_rn(p1y, p1y)), __dmul_rn(p1z, p1z)));
-        const Sample sm = gen_sample(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, p1x, p1y, p1z, E1);
+        double p1x, p1y, p1z, E1;
+        cell_kinematics(P.g, i, p1x, p1y, p1z, E1);
+        Sample sm;
+        unsigned kstart = 0u;
+        do {                                                 // the generator of the collision kernel, attempts two at a time
+            sm = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+            kstart += 2u;
+        } while (sm.retry);
         cells[4 * q + 0] = sm.j; cells[4 * q + 1] = sm.k; cells[4 * q + 2] = sm.l; cells[4 * q + 3] = sm.flag;
         if (stu) { stu[3 * q + 0] = sm.s; stu[3 * q + 1] = sm.t; stu[3 * q + 2] = sm.u; }
     }
@@ -353,7 +391,7 @@ template <int kMask>
 cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t st)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
-    const size_t smem = sizeof(Slot<kSP>) * kProducerWarps * kSlots;
+    const size_t smem = sizeof(Slot<kSP>) * kProducerWarps * kSlots + sizeof(int2) * kRetryCap * kProducerWarps;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

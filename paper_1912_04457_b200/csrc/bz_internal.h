@@ -27,8 +27,7 @@ struct CollideParams {
     int cells_per_region;     // p1 cells per work item (one producer warp each)
     int regions_per_x;        // ceil(Np / cells_per_region)
     uint32_t seed, step;
-    double K;             // dtG Vp / (2048 pi^4 Ns)                       (S8c step 0)
-    double g4;            // (4 pi alpha_s)^2
+    double g4K;           // (4 pi alpha_s)^2 * K,  K = dtG Vp / (2048 pi^4 Ns)    (S8c step 0)
     unsigned mask;        // bit id set <=> species id active
     int slot[7];          // species id -> index a in the layout (or -1)
 };

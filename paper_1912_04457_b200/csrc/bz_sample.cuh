@@ -11,7 +11,9 @@ namespace bz {
 struct GridConst {          // S8c step 0, computed once on the host in fp64
     int n;                  // momentum cells per axis
     double pmin, L, dp;     // box edge, box length pmax - pmin, cell width L/n
-    double inv_dp;          // n / L, only for the guarded fast path of the binning
+    // guarded fast path of the binning: floor(p * bin_a + bin_b) ~ floor(2^bin_shift * (p - pmin) / dp)
+    double bin_a, bin_b;
+    int bin_shift;
 };
 
 // ---- S8c step 1: Philox4x32-10 (Salmon et al. 2011), key = (seed, step), counter = (blk, sample, pcell, xcell)
@@ -37,78 +39,102 @@ __device__ __forceinline__ double uniform52(uint32_t a, uint32_t b)
 }
 
 // ---- S8c step 3: cell index along one axis.  q = (p - pmin)/dp, inside iff 0 <= q < n, idx = floor(q).
-// The division is replaced by a multiplication whenever the product is safely away from an integer (its error
-// is < 1e-13 for |q| < 1e3, the guard is 1e-9), so the result equals the division's bit for bit.
-__device__ __forceinline__ int bin_axis(double p, const GridConst& g, bool& inside)
+// Exact form (the definition): one correctly rounded subtraction and division.
+__device__ __forceinline__ int bin_axis_exact(double p, const GridConst& g, bool& inside)
 {
-    const double x = __dsub_rn(p, g.pmin);
-    double q = __dmul_rn(x, g.inv_dp);
-    double fl = floor(q);
-    const double fr = q - fl;
-    if (!(fr > 1e-9 && fr < 1.0 - 1e-9) || !(fabs(q) < 1e3)) {
-        q = __ddiv_rn(x, g.dp);
-        fl = floor(q);
-    }
+    const double q = __ddiv_rn(__dsub_rn(p, g.pmin), g.dp);
     inside = (q >= 0.0) && (q < (double)g.n);
-    return (int)fl;
+    return (int)floor(q);
 }
-
-__device__ __forceinline__ int bin_cell(double px, double py, double pz, const GridConst& g)
+__device__ __forceinline__ int bin_cell_exact(double px, double py, double pz, const GridConst& g)
 {
     bool ix, iy, iz;
-    const int a = bin_axis(px, g, ix), b = bin_axis(py, g, iy), c = bin_axis(pz, g, iz);
+    const int a = bin_axis_exact(px, g, ix), b = bin_axis_exact(py, g, iy), c = bin_axis_exact(pz, g, iz);
+    return (ix && iy && iz) ? a + g.n * (b + g.n * c) : -1;
+}
+// Fast form: t = floor(2^k q') with q' = fma(p, 2^k/dp, -pmin 2^k/dp), |q' - q| 2^k < 1e-6 (the host picks k <= 20 so that
+// 2^k |q| < 2^31 for every reachable momentum; a saturated conversion lands outside [0, n) like the true q).
+// idx = t >> k and the inside test are those of the exact q unless t is within 2 units of a multiple of 2^k; then
+// `risky` is set and the caller repeats the binning with the exact form.  Cost: 1 DFMA + 1 F2I + 5 integer ops.
+__device__ __forceinline__ int bin_axis_fast(double p, const GridConst& g, bool& inside, bool& risky)
+{
+    const int t = __double2int_rd(fma(p, g.bin_a, g.bin_b));
+    const unsigned mask = (1u << g.bin_shift) - 1u;
+    const int idx = t >> g.bin_shift;
+    risky = risky || (((unsigned)(t - 2) & mask) > mask - 4u);
+    inside = (unsigned)idx < (unsigned)g.n;
+    return idx;
+}
+__device__ __forceinline__ int bin_cell_fast(double px, double py, double pz, const GridConst& g, bool& risky)
+{
+    bool ix, iy, iz;
+    const int a = bin_axis_fast(px, g, ix, risky), b = bin_axis_fast(py, g, iy, risky), c = bin_axis_fast(pz, g, iz, risky);
     return (ix && iy && iz) ? a + g.n * (b + g.n * c) : -1;
 }
 
 struct Sample {
-    int flag, j, k, l;
+    int flag;        // 1: both outgoing legs in the box and s > 0 -> the sample deposits
+    int retry;       // 1: s > 0 but neither Marsaglia attempt of this call was accepted: call again with kstart + 2
+    int j, k, l;     // cells of p2, p3, p4 (k = l = -1 when !(s > 0); k or l = -1 when that leg leaves the box)
     double s, t, u, E1E2;
 };
 
-// One kinematic sample (S8c step 2).  p1 = centre of pcell; E1 passed in (same for all samples of the cell).
-__device__ __forceinline__ Sample gen_sample(const GridConst& g, uint32_t seed, uint32_t step, uint32_t xcell,
-                                             uint32_t pcell, uint32_t smp, double p1x, double p1y, double p1z,
-                                             double E1)
+// momentum and energy of the centre of cell i (S8c step 0 / step 2)
+__device__ __forceinline__ double cell_centre(const GridConst& g, int i)
+{
+    return __dadd_rn(g.pmin, __dmul_rn(__dadd_rn((double)i, 0.5), g.dp));
+}
+__device__ __forceinline__ void cell_kinematics(const GridConst& g, int pcell, double& p1x, double& p1y, double& p1z, double& E1)
+{
+    const int n = g.n, ipx = pcell % n, ipy = (pcell / n) % n, ipz = pcell / (n * n);
+    p1x = cell_centre(g, ipx); p1y = cell_centre(g, ipy); p1z = cell_centre(g, ipz);
+    E1 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p1x, p1x), __dmul_rn(p1y, p1y)), __dmul_rn(p1z, p1z)));
+}
+
+// One kinematic sample (S8c steps 1-3) with Marsaglia attempts kstart and kstart + 1 (kstart even).  All four Philox
+// blocks (0, 1, 2 + kstart, 3 + kstart) are independent and issued together, there is no data-dependent loop: a lane
+// whose two attempts both fail (probability 0.046) reports retry = 1 and is finished by a later call.  The sequence
+// of attempts, and therefore the accepted direction, is exactly that of the one-attempt-at-a-time loop of S8c.
+__device__ __forceinline__ Sample gen_sample_pair(const GridConst& g, uint32_t seed, uint32_t step, uint32_t xcell,
+                                                  uint32_t pcell, uint32_t smp, uint32_t kstart, double p1x, double p1y,
+                                                  double p1z, double E1)
 {
     Sample o;
-    o.flag = 0; o.k = -1; o.l = -1; o.s = 0.0; o.t = 0.0; o.u = 0.0;
-    uint32_t w[4];
-    philox4x32_10(0u, smp, pcell, xcell, seed, step, w);
-    const double u0 = uniform52(w[0], w[1]), u1 = uniform52(w[2], w[3]);
-    philox4x32_10(1u, smp, pcell, xcell, seed, step, w);
-    const double u2 = uniform52(w[0], w[1]);
+    o.flag = 0; o.retry = 0; o.k = -1; o.l = -1; o.s = 0.0; o.t = 0.0; o.u = 0.0;
+    uint32_t w0[4], w1[4], wa[4], wb[4];
+    philox4x32_10(0u, smp, pcell, xcell, seed, step, w0);
+    philox4x32_10(1u, smp, pcell, xcell, seed, step, w1);
+    philox4x32_10(2u + kstart, smp, pcell, xcell, seed, step, wa);
+    philox4x32_10(3u + kstart, smp, pcell, xcell, seed, step, wb);
+    const double u0 = uniform52(w0[0], w0[1]), u1 = uniform52(w0[2], w0[3]), u2 = uniform52(w1[0], w1[1]);
     const double p2x = __dadd_rn(g.pmin, __dmul_rn(u0, g.L));
     const double p2y = __dadd_rn(g.pmin, __dmul_rn(u1, g.L));
     const double p2z = __dadd_rn(g.pmin, __dmul_rn(u2, g.L));
     const double E2 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p2x, p2x), __dmul_rn(p2y, p2y)), __dmul_rn(p2z, p2z)));
     const double d12 = __dadd_rn(__dadd_rn(__dmul_rn(p1x, p2x), __dmul_rn(p1y, p2y)), __dmul_rn(p1z, p2z));
     const double s = __dmul_rn(2.0, __dsub_rn(__dmul_rn(E1, E2), d12));
-    {   // p2 is inside by construction; clamp defensively
-        bool in;
-        int a = bin_axis(p2x, g, in), b = bin_axis(p2y, g, in), c = bin_axis(p2z, g, in);
-        a = min(max(a, 0), g.n - 1); b = min(max(b, 0), g.n - 1); c = min(max(c, 0), g.n - 1);
-        o.j = a + g.n * (b + g.n * c);
-    }
     o.E1E2 = E1 * E2;
-    if (!(s > 0.0)) return o;
 
-    // Marsaglia: first attempt k with q = v1^2 + v2^2 < 1
-    double nx = 0.0, ny = 0.0, nz = 1.0;
-    for (uint32_t k = 0; k < 62u; ++k) {
-        philox4x32_10(2u + k, smp, pcell, xcell, seed, step, w);
-        const double v1 = __dadd_rn(__dmul_rn(2.0, uniform52(w[0], w[1])), -1.0);
-        const double v2 = __dadd_rn(__dmul_rn(2.0, uniform52(w[2], w[3])), -1.0);
-        const double q = __dadd_rn(__dmul_rn(v1, v1), __dmul_rn(v2, v2));
-        if (q < 1.0) {
-            const double r = __dsqrt_rn(__dsub_rn(1.0, q));
-            nx = __dmul_rn(__dmul_rn(2.0, v1), r);
-            ny = __dmul_rn(__dmul_rn(2.0, v2), r);
-            nz = __dsub_rn(1.0, __dmul_rn(2.0, q));
-            break;
-        }
+    // Marsaglia: attempt k is accepted iff q_k = v1^2 + v2^2 < 1; after 62 failures the direction is (0, 0, 1)
+    double v1 = __dadd_rn(__dmul_rn(2.0, uniform52(wa[0], wa[1])), -1.0);
+    double v2 = __dadd_rn(__dmul_rn(2.0, uniform52(wa[2], wa[3])), -1.0);
+    double q = __dadd_rn(__dmul_rn(v1, v1), __dmul_rn(v2, v2));
+    const double v1b = __dadd_rn(__dmul_rn(2.0, uniform52(wb[0], wb[1])), -1.0);
+    const double v2b = __dadd_rn(__dmul_rn(2.0, uniform52(wb[2], wb[3])), -1.0);
+    const double qb = __dadd_rn(__dmul_rn(v1b, v1b), __dmul_rn(v2b, v2b));
+    bool found = q < 1.0;
+    if (!found) { v1 = v1b; v2 = v2b; q = qb; found = qb < 1.0; }
+    double nx, ny, nz;
+    {
+        const double r = __dsqrt_rn(__dsub_rn(1.0, found ? q : 0.0));
+        nx = __dmul_rn(__dmul_rn(2.0, v1), r);
+        ny = __dmul_rn(__dmul_rn(2.0, v2), r);
+        nz = __dsub_rn(1.0, __dmul_rn(2.0, q));
     }
+    if (kstart >= 62u) { nx = 0.0; ny = 0.0; nz = 1.0; found = true; }
+
     const double Px = __dadd_rn(p1x, p2x), Py = __dadd_rn(p1y, p2y), Pz = __dadd_rn(p1z, p2z);
-    const double E = __dadd_rn(E1, E2), M = __dsqrt_rn(s);
+    const double E = __dadd_rn(E1, E2), M = __dsqrt_rn(s > 0.0 ? s : 0.0);
     const double cc = __dadd_rn(__dadd_rn(__dmul_rn(Px, nx), __dmul_rn(Py, ny)), __dmul_rn(Pz, nz));
     const double h = __dadd_rn(1.0, __ddiv_rn(cc, __dadd_rn(E, M)));
     const double p3x = __dmul_rn(0.5, __dadd_rn(__dmul_rn(M, nx), __dmul_rn(Px, h)));
@@ -118,18 +144,29 @@ __device__ __forceinline__ Sample gen_sample(const GridConst& g, uint32_t seed, 
     const double E3 = __dmul_rn(0.5, __dadd_rn(E, cc));
     const double d13 = __dadd_rn(__dadd_rn(__dmul_rn(p1x, p3x), __dmul_rn(p1y, p3y)), __dmul_rn(p1z, p3z));
     const double t = __dmul_rn(-2.0, __dsub_rn(__dmul_rn(E1, E3), d13));
-    const double u = __dsub_rn(-s, t);
-    o.s = s; o.t = t; o.u = u;
-    o.k = bin_cell(p3x, p3y, p3z, g);
-    o.l = bin_cell(p4x, p4y, p4z, g);
-    o.flag = (o.k >= 0) && (o.l >= 0);
-    return o;
-}
 
-// centre of cell i along one axis: pmin + (i + 0.5) * dp, as S8c step 0 writes it
-__device__ __forceinline__ double cell_centre(const GridConst& g, int i)
-{
-    return __dadd_rn(g.pmin, __dmul_rn(__dadd_rn((double)i, 0.5), g.dp));
+    bool risky = false;
+    int j = bin_cell_fast(p2x, p2y, p2z, g, risky);
+    int k = bin_cell_fast(p3x, p3y, p3z, g, risky);
+    int l = bin_cell_fast(p4x, p4y, p4z, g, risky);
+    if (risky) {                                         // ~4e-5 of the samples: repeat with the definition
+        j = bin_cell_exact(p2x, p2y, p2z, g);
+        k = bin_cell_exact(p3x, p3y, p3z, g);
+        l = bin_cell_exact(p4x, p4y, p4z, g);
+    }
+    if (j < 0) {                                         // p2 is inside by construction; clamp defensively (S8c step 3)
+        bool in;
+        int a = bin_axis_exact(p2x, g, in), b = bin_axis_exact(p2y, g, in), c = bin_axis_exact(p2z, g, in);
+        a = min(max(a, 0), g.n - 1); b = min(max(b, 0), g.n - 1); c = min(max(c, 0), g.n - 1);
+        j = a + g.n * (b + g.n * c);
+    }
+    o.j = j;
+    if (!(s > 0.0)) return o;                            // p1 = 0 cell, exact collinearity, rounding: no deposit, no retry
+    if (!found) { o.retry = 1; return o; }
+    o.s = s; o.t = t; o.u = __dsub_rn(-s, t);
+    o.k = k; o.l = l;
+    o.flag = (k >= 0) && (l >= 0);
+    return o;
 }
 
 }  // namespace bz
