@@ -34,6 +34,10 @@ import numpy as np  # noqa: E402
 
 import workloads as wl  # noqa: E402
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one collide_kernel launch, from the ncu --set full capture summarised in
+# profiles/r1_collide_kernel_ncu_full.md (the algorithmic gather/scatter bytes are ~113x larger: the tiles live in L2)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4_inhom16x24": 10.874876e9}
+
 METRIC = "collision_samples_per_sec"
 UNIT = "samples/s"
 
@@ -255,8 +259,10 @@ def run_ours(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": cfg.n_values * 8,
                 "d2h_bytes_per_step": cfg.n_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": "collision group (pack_kernel + sample_kernel + deposit_kernel; events around the group)", "achieved": ach, "peak": peak, "unit": "GB/s",
-                     "frac": ach / peak if ach else None, "traffic": None, "peak_source": peak_src,
+        "roofline": {"bound": "hbm", "kernel": "collide_kernel (+ pack_kernel: CUDA events inside libbz.so around the pair)",
+                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak if ach else None,
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (ncu dram read + write)",
+                     "peak_source": peak_src,
                      "bytes_per_sample": bps, "samples_per_launch": samples_step,
                      "ms_per_launch": coll_ms / coll_n if coll_n else None},
         "clocks": clocks,
