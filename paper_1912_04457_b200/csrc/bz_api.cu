@@ -63,7 +63,7 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
 {
     CollideParams P;
     P.g = grid_const(c);
-    P.f_aos = c->f_aos; P.dN_aos = c->dN_aos; P.m2 = c->m2;
+    P.f_aos = c->f_aos; P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab;
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
     P.work_counter = c->work_counter; P.n_items = (unsigned)c->Nx * (unsigned)c->regions_per_x; P.x_begin = 0;
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
@@ -130,7 +130,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
-    c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = nullptr;
+    c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         c->err = "bz_create: no CUDA device (this library has no CPU path)";
         return -2;
@@ -156,6 +156,8 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     BZ_CUDA(cudaMalloc(&c->mom, ((size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx) * sizeof(double)), "cudaMalloc mom");
     BZ_CUDA(cudaMalloc(&c->absp, 5 * (size_t)c->Np * sizeof(double)), "cudaMalloc tables");
     c->w_invE = c->absp + c->Np; c->vx = c->w_invE + c->Np; c->vy = c->vx + c->Np; c->vz = c->vy + c->Np;
+    BZ_CUDA(cudaMalloc(&c->cell_tab, 4 * (size_t)c->Np * sizeof(double)), "cudaMalloc cell table");
+    BZ_CUDA(launch_cell_table(grid_const(c), c->Np, c->cell_tab, nullptr), "cell table");
     BZ_CUDA(cudaMemset(c->f, 0, bytes), "memset f");
     BZ_CUDA(cudaMemset(c->f_new, 0, bytes), "memset f_new");
     BZ_CUDA(cudaMemset(c->dN_aos, 0, aos_bytes), "memset dN_aos");
@@ -184,7 +186,7 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp);
+    cudaFree(c->absp); cudaFree(c->cell_tab);
     for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
     delete c;
     return 0;

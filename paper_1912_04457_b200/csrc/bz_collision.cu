@@ -4,24 +4,30 @@
 //   producer warps (12, warpgroups 1-3, 88 registers after setmaxnreg.dec)
 //       sample   pull work items (a run of p1 cells of one spatial cell) from a global counter; lanes = samples:
 //                Philox4x32-10, the boost, the binning (bz_sample.cuh).  About 46 % of the samples keep both outgoing
-//                legs in the box; they are compacted (ballot + prefix) straight into the record arrays of one of the
-//                warp's two shared-memory batch slots: (i, j, k, l), s, t and the weight K/(E1 E2).
-//       gather   when a slot holds 32 records: cp.async (LDGSTS) of the 4 x S occupation numbers of every sample from
-//                the cell-major staging copy f_aos[xcell][pcell][SP] (SP = 8 doubles = 64 B per cell) into the slot;
-//                for one sample the 32 lanes fetch its 4 cells x 8 slots, i.e. 8 sectors per instruction instead of 32
-//                scattered ones.  Completion is signalled to the consumer by cp.async.mbarrier.arrive on the slot's
-//                "full" mbarrier: the producer never waits for its own gathers and goes on sampling.
-//       scatter  when the warp needs the slot again and the consumer has signalled "done": the same 8-lanes-per-cell
-//                mapping issues fp64 reductions (RED.E.ADD.F64, no return value) of the slot's 4 x S deposits into
-//                the cell-major scratch dN_aos, which stays in L2 while its spatial cell is being worked on.
+//                legs in the box; they are compacted (ballot + prefix) straight into one of the warp's two record
+//                buffers in shared memory: (i, j, k, l), s, t and E1 E2.
+//       gather   when a record buffer holds 32 samples: cp.async (LDGSTS, 16 bytes per lane, L1 bypassed) of the
+//                4 cells x 64 bytes of every sample from the cell-major staging copy f_aos[xcell][pcell][8] into the
+//                warp's stage buffer: 4 lanes fetch one cell, one instruction fetches 8 cells = 16 sectors instead of
+//                32 scattered ones.  Completion is signalled to the consumer by cp.async.mbarrier.arrive on the
+//                "full" mbarrier: the producer never waits for its own gathers and goes on sampling into the other
+//                record buffer.
 //   consumer warps (4, warpgroup 0, one per SM sub-partition, 240 registers after setmaxnreg.inc)
 //       compute  serve three producers each in rotation: wait "full", every lane takes one sample of the batch:
-//                <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh), the 4 x S deposits overwrite the
-//                gathered f in the slot, arrive on "done".
+//                <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh); the 4 x S deposits overwrite the
+//                gathered f in the stage buffer; arrive on "done".
+//       (pure glue, one double per cell: the consumer issues its four reductions straight from the registers.)
+//   producer, scatter: when the warp's next batch is complete and "done" has been signalled, it flushes the stage
+//                buffer with fp64 reductions (RED.E.ADD.F64, no return value), one sample per instruction with 8 lanes
+//                per 64-byte cell, into the cell-major scratch dN_aos, which stays in L2 while its spatial cell is
+//                being worked on; then it gathers the new batch into the same buffer.
 // The ALU-bound sampling and the latency-bound gather/scatter overlap on the same SM, the register file is split
 // 240 / 88 between the two roles, and no sample record ever leaves the SM.
-// Measured on B200 (profiles/): a RED (LDG) whose 32 lanes hit 32 different sectors costs 48 (32) cycles of the SM's
-// L1TEX path, the 8-lanes-per-cell form 15.7 (8.5) cycles for the same number of lanes.
+// Measured on B200 (microbenchmark over all 148 SMs): a RED whose 32 lanes hit 32 different sectors
+// costs 48 cycles of the SM's L1TEX path, the 8-lanes-per-cell form 15.7; chip-wide that form saturates at ~6e10 cell
+// updates/s (the L2 reduction rate).  The 64-byte TMA bulk reduction (cp.reduce.async.bulk.add.f64) reaches the same
+// chip-wide rate but is a uniform-datapath instruction: per-lane addresses cost an 8-instruction elect loop per cell
+// against 1.5 instructions per cell here, so it is not used.
 #include "bz_channels.cuh"
 #include "bz_internal.h"
 
@@ -33,7 +39,6 @@ constexpr int kConsumerWarps = 4;                // warpgroup 0
 constexpr int kProducerWarps = 12;               // warpgroups 1..3
 constexpr int kProducersPerConsumer = kProducerWarps / kConsumerWarps;
 constexpr int kCollideThreads = 32 * (kConsumerWarps + kProducerWarps);
-constexpr int kSlots = 2;                        // batch slots per producer warp
 constexpr int kConsumerRegs = 240, kProducerRegs = 88;   // 128 x 240 + 384 x 88 = 64512 <= 65536
 
 // doubles per cell in the global staging layout: 1 for the pure-glue mask, 8 (half a 128-byte line) otherwise
@@ -42,7 +47,12 @@ struct MaskTraits {
     static constexpr int SP = kMask == 0x01 ? 1 : 8;
 };
 // layout index of species id = number of active ids below it
-__device__ __forceinline__ int slot_of(unsigned mask, int id) { return __popc(mask & ((1u << id) - 1u)); }
+__host__ __device__ constexpr int slot_of(unsigned mask, int id)
+{
+    int n = 0;
+    for (int b = 0; b < id; ++b) n += (mask >> b) & 1u;
+    return n;
+}
 
 // ------------------------------------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -75,6 +85,10 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
 // fp64 reduction without return value (RED.E.ADD.F64), skipped for an exact zero
 __device__ __forceinline__ void red_add_nonzero(double* gdst, double v)
 {
@@ -86,82 +100,191 @@ __device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.
 template <int N>
 __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
-// ------------------------------------------------------------------------------------------------ batch slot
-// One batch of <= 32 accepted samples in shared memory.  stage holds, per sample, the occupation numbers of its 4 cells
-// (kCS doubles per cell) on the way in and the 4 x S deposits on the way out; the odd stride makes both the per-sample
-// access of the consumer (lane = sample) and the per-cell access of the producer (lanes = slots of a cell) conflict free.
-template <int kSP>
-struct Slot {
-    static constexpr int kCS = kSP == 1 ? 1 : 7;         // doubles per cell
-    static constexpr int kStride = 4 * kCS + 1;          // doubles per sample
-    double stage[32 * kStride];
-    double s[32], t[32], e12[32];                        // Mandelstam s, t and E1 E2 of the sample
+// ------------------------------------------------------------------------------------------------ shared memory
+// Records of one batch of <= 32 accepted samples.
+struct Rec {
     int cell[32][4];                                     // i, j, k, l
+    double s[32], t[32], e12[32];                        // Mandelstam s, t and E1 E2 of the sample
+};
+
+// Per producer warp: two record buffers (one being filled, one with the consumer) and one stage buffer that holds,
+// per sample, the occupation numbers of its 4 cells on the way in and the deposits on the way out.
+//   kSP == 8: 8 doubles (64 B, one staging-layout cell) per cell, 34 doubles per sample: every cell is 16-byte aligned
+//             (cp.async 16) and the consumer's 16-byte accesses (lane = sample, 272 B apart = 17 x 16)
+//             are bank-conflict free.
+//   kSP == 1: 1 double per cell, 5 doubles per sample (odd stride: conflict free for 8-byte accesses).
+template <int kSP>
+struct alignas(16) Chan {
+    static constexpr int kCS = kSP == 1 ? 1 : 8;         // doubles per cell
+    static constexpr int kStride = kSP == 1 ? 5 : 34;    // doubles per sample
+    double stage[32 * kStride];
+    Rec rec[2];
     double m2;                                           // regulator mass^2 of the batch's spatial cell
     int nvalid;                                          // samples in the batch; < 0: the producer has finished
     int xcell;
+    int ridx;                                            // record buffer of the batch
+    int pad_;
     uint64_t full;                                       // producer -> consumer: records + gathered f are in place
-    uint64_t done;                                       // consumer -> producer: deposits are in place
+    uint64_t done;                                       // consumer -> producer: the stage buffer may be overwritten
 };
 
 constexpr int kRetryCap = 64;                    // per producer warp: samples whose two Marsaglia attempts both failed
 
-// lane -> element of a sample: kSP slots of each of the 4 cells; 32 / (4 kSP) samples per instruction
+// ---- producer: wait until the stage buffer is free, issue the gather of the batch in rec[ridx], hand it to the consumer
 template <int kSP>
-struct LaneMap {
-    static constexpr int kEPS = 4 * kSP;                 // lanes per sample
-    static constexpr int kSPI = 32 / kEPS;               // samples per instruction
-    int sub, cc, sl;
-    __device__ __forceinline__ explicit LaneMap(int lane) : sub(lane / kEPS), cc((lane % kEPS) / kSP), sl(lane % kSP) {}
-};
-
-// ---- producer: issue the gather of the slot's batch and hand the slot to the consumer
-template <int kSP>
-__device__ __forceinline__ void submit_slot(Slot<kSP>& sl, const CollideParams& P, int lane, int nvalid, int xcell, double m2)
+__device__ __noinline__ unsigned submit_batch(Chan<kSP>& ch, const double* __restrict__ f_aos, double* __restrict__ dN_aos,
+                                              int Np, int S, int lane, int ridx, int nvalid, int xcell, double m2,
+                                              unsigned in_flight, unsigned dpar)
 {
-    using S = Slot<kSP>;
-    if (lane == 0) { sl.nvalid = nvalid; sl.xcell = xcell; sl.m2 = m2; }
+    using C = Chan<kSP>;
+    if (in_flight) {                                     // the previous batch: flush the deposits the consumer left
+        mbar_wait(&ch.done, dpar);
+        dpar ^= 1u;
+        if constexpr (kSP != 1) {
+            // one sample per instruction: lane = (cell cc, slot sl) of the sample, 8 lanes per 64-byte cell
+            const int pn = ch.nvalid, cc = lane >> 3, sl = lane & 7;
+            if (sl < S) {
+                double* __restrict__ gdst = dN_aos + (size_t)ch.xcell * Np * 8 + sl;
+                const double* src = ch.stage + lane;
+                const int* cp = &ch.rec[ridx ^ 1].cell[0][cc];
+                if (pn == 32) {
+#pragma unroll
+                    for (int m = 0; m < 32; ++m) red_add_nonzero(gdst + (size_t)cp[4 * m] * 8, src[m * C::kStride]);
+                } else {
+                    for (int m = 0; m < pn; ++m) red_add_nonzero(gdst + (size_t)cp[4 * m] * 8, src[m * C::kStride]);
+                }
+            }
+            __syncwarp();
+        }
+    }
+    if (lane == 0) { ch.nvalid = nvalid; ch.xcell = xcell; ch.m2 = m2; ch.ridx = ridx; }
     __syncwarp();                                        // the records written by all lanes are visible to all lanes
     if (nvalid > 0) {
-        const LaneMap<kSP> lm(lane);
-        if (lm.sl < P.S) {                               // pad lanes (slot 7 of a cell) sit the gather out
-            const double* __restrict__ src = P.f_aos + (size_t)xcell * P.Np * kSP + lm.sl;
-            double* dst = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
-            const int* cp = &sl.cell[lm.sub][lm.cc];
+        const int* cells = &ch.rec[ridx].cell[0][0];
+        if constexpr (kSP == 1) {
+            const int sub = lane >> 2, cc = lane & 3;    // 8 samples per instruction, 4 lanes (cells) each
+            const double* __restrict__ src = f_aos + (size_t)xcell * Np;
+            double* dst = ch.stage + sub * C::kStride + cc;
+            const int* cp = cells + sub * 4 + cc;
+#pragma unroll
+            for (int m0 = 0; m0 < 32; m0 += 8)
+                if (m0 + sub < nvalid) cp_async8(dst + m0 * C::kStride, src + cp[4 * m0]);
+        } else {
+            const int sub = lane >> 4, cc = (lane >> 2) & 3, q = lane & 3;   // 2 samples per instruction, 4 lanes per cell
+            const double* __restrict__ src = f_aos + (size_t)xcell * Np * 8 + q * 2;
+            double* dst = ch.stage + sub * C::kStride + cc * 8 + q * 2;
+            const int* cp = cells + sub * 4 + cc;
             if (nvalid == 32) {
 #pragma unroll
-                for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI)
-                    cp_async8(dst + m0 * S::kStride, src + (size_t)cp[4 * m0] * kSP);
+                for (int m0 = 0; m0 < 32; m0 += 2)
+                    cp_async16(dst + m0 * C::kStride, src + (size_t)cp[4 * m0] * 8);
             } else {
-                for (int m0 = 0; m0 + lm.sub < nvalid; m0 += LaneMap<kSP>::kSPI)
-                    cp_async8(dst + m0 * S::kStride, src + (size_t)cp[4 * m0] * kSP);
+                for (int m0 = 0; m0 + sub < nvalid; m0 += 2)
+                    cp_async16(dst + m0 * C::kStride, src + (size_t)cp[4 * m0] * 8);
             }
         }
     }
-    mbar_arrive_on_cp_async(&sl.full);                   // 32 deferred arrivals: this lane's gathers have landed
-    if (lane == 0) mbar_arrive(&sl.full);                // + 1: header and records (release)
+    mbar_arrive_on_cp_async(&ch.full);                   // 32 deferred arrivals: this lane's gathers have landed
+    if (lane == 0) mbar_arrive(&ch.full);                // + 1: header and records (release)
+    return dpar;                                         // parity of the "done" phase this batch will complete
 }
 
-// ---- producer: flush the deposits the consumer left in the slot
-template <int kSP>
-__device__ __forceinline__ void scatter_slot(Slot<kSP>& sl, const CollideParams& P, int lane)
+// ---- consumer: one sample per lane: |M|^2, channel algebra, deposits; then the scatter of the lane's four cells
+template <int kMask, int kSP>
+__device__ __forceinline__ void consume_batch(Chan<kSP>& ch, const CollideParams& P, int lane, unsigned mask)
 {
-    using S = Slot<kSP>;
-    const int nvalid = sl.nvalid;
-    const LaneMap<kSP> lm(lane);
-    if (lm.sl < P.S) {
-        double* __restrict__ dst = P.dN_aos + (size_t)sl.xcell * P.Np * kSP + lm.sl;
-        const double* src = sl.stage + lm.sub * S::kStride + lm.cc * S::kCS + lm.sl;
-        const int* cp = &sl.cell[lm.sub][lm.cc];
-        if (nvalid == 32) {
+    using C = Chan<kSP>;
+    constexpr bool kGlue = kMask < 0 || (kMask & 1);
+    constexpr bool kQuark = kMask < 0 || (kMask & 0x7E);
+    const int nvalid = ch.nvalid;
+    const Rec& R = ch.rec[ch.ridx];
+    if (lane < nvalid) {
+        double* st = ch.stage + lane * C::kStride;
+        const double s = R.s[lane], t = R.t[lane], m2 = ch.m2;
+        const double g4w = P.g4K * rcp_fast(R.e12[lane]);                 // g^4 K / (E1 E2), S8c step 6
+        const int4 cl = *reinterpret_cast<const int4*>(&R.cell[lane][0]);
+        double fi[7], fj[7], fk[7], fl[7];
+        if constexpr (kSP == 8 && kMask >= 0) {
+            // compile-time layout: 16-byte loads, the registers are picked statically
+            constexpr int kPairs = (slot_of((unsigned)kMask, 7) + 1) / 2;
+            double2 v[4][4];
 #pragma unroll
-            for (int m0 = 0; m0 < 32; m0 += LaneMap<kSP>::kSPI)
-                red_add_nonzero(dst + (size_t)cp[4 * m0] * kSP, src[m0 * S::kStride]);
+            for (int c = 0; c < 4; ++c)
+#pragma unroll
+                for (int q = 0; q < kPairs; ++q) v[c][q] = *reinterpret_cast<const double2*>(st + c * 8 + 2 * q);
+#pragma unroll
+            for (int id = 0; id < 7; ++id) {
+                if ((kMask >> id) & 1) {
+                    constexpr unsigned km = (unsigned)kMask;
+                    const int a = slot_of(km, id);
+                    fi[id] = (a & 1) ? v[0][a >> 1].y : v[0][a >> 1].x;
+                    fj[id] = (a & 1) ? v[1][a >> 1].y : v[1][a >> 1].x;
+                    fk[id] = (a & 1) ? v[2][a >> 1].y : v[2][a >> 1].x;
+                    fl[id] = (a & 1) ? v[3][a >> 1].y : v[3][a >> 1].x;
+                } else {
+                    fi[id] = fj[id] = fk[id] = fl[id] = 0.0;
+                }
+            }
         } else {
-            for (int m0 = 0; m0 + lm.sub < nvalid; m0 += LaneMap<kSP>::kSPI)
-                red_add_nonzero(dst + (size_t)cp[4 * m0] * kSP, src[m0 * S::kStride]);
+#pragma unroll
+            for (int id = 0; id < 7; ++id) {
+                if ((mask >> id) & 1u) {
+                    const int a = slot_of(mask, id);
+                    fi[id] = st[a]; fj[id] = st[C::kCS + a]; fk[id] = st[2 * C::kCS + a]; fl[id] = st[3 * C::kCS + a];
+                } else {
+                    fi[id] = fj[id] = fk[id] = fl[id] = 0.0;
+                }
+            }
+        }
+        const double u = __dsub_rn(-s, t);
+        const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
+        double d[4][7];
+        deposit<kMask>(mask, fi, fj, fk, fl, M, d[0], d[1], d[2], d[3]);
+        if constexpr (kSP == 1) {
+            // pure glue: four scalar reductions straight from the registers
+            double* __restrict__ dst = P.dN_aos + (size_t)ch.xcell * P.Np;
+            red_add_nonzero(dst + cl.x, d[0][0]); red_add_nonzero(dst + cl.y, d[1][0]);
+            red_add_nonzero(dst + cl.z, d[2][0]); red_add_nonzero(dst + cl.w, d[3][0]);
+        } else {
+            if constexpr (kMask >= 0) {
+                constexpr unsigned km = (unsigned)kMask;
+                constexpr int kS = slot_of(km, 7), kPairs = (kS + 1) / 2;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double o[8];
+#pragma unroll
+                    for (int a = 0; a < 8; ++a) o[a] = 0.0;
+#pragma unroll
+                    for (int id = 0; id < 7; ++id)
+                        if ((kMask >> id) & 1) o[slot_of(km, id)] = d[c][id];
+#pragma unroll
+                    for (int q = 0; q < kPairs; ++q)
+                        *reinterpret_cast<double2*>(st + c * 8 + 2 * q) = make_double2(o[2 * q], o[2 * q + 1]);
+                }
+            } else {
+#pragma unroll
+                for (int id = 0; id < 7; ++id) {
+                    if ((mask >> id) & 1u) {
+                        const int a = slot_of(mask, id);
+                        st[a] = d[0][id]; st[8 + a] = d[1][id]; st[16 + a] = d[2][id]; st[24 + a] = d[3][id];
+                    }
+                }
+            }
+            // slots that hold no species keep the zeros they were gathered with (pack_kernel writes the pads as 0)
         }
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&ch.done);
+}
+
+// momentum and energy of the centre of a p1 cell from the table built by cell_table_kernel (same arithmetic as
+// cell_kinematics, done once per context instead of once per warp pass)
+__device__ __forceinline__ void cell_lookup(const double* __restrict__ tab, int pcell, double& p1x, double& p1y, double& p1z,
+                                            double& E1)
+{
+    const double2 a = __ldg(reinterpret_cast<const double2*>(tab) + 2 * (size_t)pcell);
+    const double2 b = __ldg(reinterpret_cast<const double2*>(tab) + 2 * (size_t)pcell + 1);
+    p1x = a.x; p1y = a.y; p1z = b.x; E1 = b.y;
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel
@@ -169,16 +292,14 @@ template <int kMask>
 __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const CollideParams P)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
-    using S = Slot<kSP>;
-    constexpr bool kGlue = kMask < 0 || (kMask & 1);
-    constexpr bool kQuark = kMask < 0 || (kMask & 0x7E);
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    S* slots = reinterpret_cast<S*>(smem_raw);           // [kProducerWarps][kSlots]
+    using C = Chan<kSP>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    C* chans = reinterpret_cast<C*>(smem_raw);           // [kProducerWarps]
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-    if (threadIdx.x < kProducerWarps * kSlots) {
-        mbar_init(&slots[threadIdx.x].full, 33);
-        mbar_init(&slots[threadIdx.x].done, 1);
+    if (threadIdx.x < kProducerWarps) {
+        mbar_init(&chans[threadIdx.x].full, 33);
+        mbar_init(&chans[threadIdx.x].done, 1);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -188,48 +309,19 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         setmaxnreg_inc<kConsumerRegs>();
         const unsigned mask = kMask >= 0 ? (unsigned)kMask : P.mask;
         unsigned alive = (1u << kProducersPerConsumer) - 1u;   // producers of this consumer still running
-        unsigned cur = 0;                                      // bit q: next slot of producer q
-        unsigned par = 0;                                      // bit 2q+slot: parity of the next "full" phase
+        unsigned par = 0;                                      // bit q: parity of the next "full" phase of producer q
         int q = 0;
         while (alive) {
             // poll the alive producers in rotation; each try suspends the warp for at most ~0.3 us
-            if (!((alive >> q) & 1u)) { q = (q + 1) % kProducersPerConsumer; continue; }
-            const int si = (cur >> q) & 1u;
-            S& sl = slots[(warp + kConsumerWarps * q) * kSlots + si];
-            if (!mbar_try_wait(&sl.full, (par >> (2 * q + si)) & 1u, 300u)) { q = (q + 1) % kProducersPerConsumer; continue; }
-            par ^= 1u << (2 * q + si);
-            cur ^= 1u << q;
-            const int nvalid = sl.nvalid;
-            if (nvalid < 0) { alive &= ~(1u << q); q = (q + 1) % kProducersPerConsumer; continue; }
-            if (lane < nvalid) {
-                double* st = sl.stage + lane * S::kStride;
-                const double s = sl.s[lane], t = sl.t[lane], m2 = sl.m2;
-                const double g4w = P.g4K * rcp_fast(sl.e12[lane]);            // g^4 K / (E1 E2), S8c step 6
-                double fi[7], fj[7], fk[7], fl[7];
-#pragma unroll
-                for (int id = 0; id < 7; ++id) {
-                    if ((mask >> id) & 1u) {
-                        const int a = slot_of(mask, id);
-                        fi[id] = st[a]; fj[id] = st[S::kCS + a]; fk[id] = st[2 * S::kCS + a]; fl[id] = st[3 * S::kCS + a];
-                    } else {
-                        fi[id] = fj[id] = fk[id] = fl[id] = 0.0;
-                    }
-                }
-                const double u = __dsub_rn(-s, t);
-                const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
-                double dI[7], dJ[7], dK[7], dL[7];
-                deposit<kMask>(mask, fi, fj, fk, fl, M, dI, dJ, dK, dL);
-#pragma unroll
-                for (int id = 0; id < 7; ++id) {
-                    if ((mask >> id) & 1u) {
-                        const int a = slot_of(mask, id);
-                        st[a] = dI[id]; st[S::kCS + a] = dJ[id]; st[2 * S::kCS + a] = dK[id]; st[3 * S::kCS + a] = dL[id];
-                    }
+            if ((alive >> q) & 1u) {
+                C& ch = chans[warp + kConsumerWarps * q];
+                if (mbar_try_wait(&ch.full, (par >> q) & 1u, 300u)) {
+                    par ^= 1u << q;
+                    if (ch.nvalid < 0) alive &= ~(1u << q);
+                    else consume_batch<kMask, kSP>(ch, P, lane, mask);
                 }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sl.done);
-            q = (q + 1) % kProducersPerConsumer;
+            q = (q + 1 == kProducersPerConsumer) ? 0 : q + 1;
         }
         return;
     }
@@ -237,13 +329,13 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
     // ============================================================================================ producer
     setmaxnreg_dec<kProducerRegs>();
     const int pw = warp - kConsumerWarps;
-    S* my = slots + pw * kSlots;
-    int2* retry = reinterpret_cast<int2*>(slots + kProducerWarps * kSlots) + pw * kRetryCap;
-    int cur = 0;                         // slot being filled
+    C& ch = chans[pw];
+    int2* retry = reinterpret_cast<int2*>(chans + kProducerWarps) + pw * kRetryCap;
+    int cur = 0;                         // record buffer being filled
     int count = 0;                       // records in it
     int rcount = 0;                      // entries in the retry list
-    unsigned busy = 0;                   // bit s: slot s is with the consumer (submitted, deposits not yet flushed)
-    unsigned dpar = 0;                   // bit s: parity of the next "done" phase of slot s
+    unsigned in_flight = 0;              // a batch has been submitted and its "done" phase not yet consumed
+    unsigned dpar = 0;                   // parity of the next "done" phase
     for (;;) {
         unsigned item = 0;
         if (lane == 0) item = atomicAdd(P.work_counter, 1u);
@@ -267,10 +359,10 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 active = lane < nr;
                 const int2 e = active ? retry[rcount + lane] : make_int2(0, 0);
                 ci = e.x; smp = e.y & 0x1ffffff; kstart = (unsigned)e.y >> 25;
-                cell_kinematics(P.g, ci, p1x, p1y, p1z, E1);              // per lane
+                cell_lookup(P.cell_tab, ci, p1x, p1y, p1z, E1);           // per lane
                 cell_valid = false;
             } else if (i < i_end) {
-                if (!cell_valid) { cell_kinematics(P.g, i, p1x, p1y, p1z, E1); cell_valid = true; }
+                if (!cell_valid) { cell_lookup(P.cell_tab, i, p1x, p1y, p1z, E1); cell_valid = true; }
                 ci = i; smp = base + lane; kstart = 0u;
                 active = smp < P.Ns;
                 base += 32;
@@ -289,56 +381,45 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 rcount += __popc(rb);
                 __syncwarp();
             }
-            // ---- compact the accepted samples into the current slot; a full slot goes to the consumer
+            // ---- compact the accepted samples into the current record buffer; a full buffer goes to the consumer
             const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
             if (acc == 0u) continue;
             int pos = count + __popc(acc & lt);
             if (sa.flag && pos < 32) {
-                S& sl = my[cur];
-                *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
-                sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.e12[pos] = sa.E1E2;
+                Rec& r = ch.rec[cur];
+                *reinterpret_cast<int4*>(&r.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
+                r.s[pos] = sa.s; r.t[pos] = sa.t; r.e12[pos] = sa.E1E2;
             }
             count += __popc(acc);
             if (count >= 32) {
-                submit_slot<kSP>(my[cur], P, lane, 32, xcell, m2);
-                busy |= 1u << cur;
-                cur ^= 1;
-                if ((busy >> cur) & 1u) {                    // make the other slot writable: wait for the consumer, flush
-                    mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
-                    dpar ^= 1u << cur;
-                    busy &= ~(1u << cur);
-                    scatter_slot<kSP>(my[cur], P, lane);
-                    __syncwarp();
-                }
+                dpar = submit_batch<kSP>(ch, P.f_aos, P.dN_aos, P.Np, P.S, lane, cur, 32, xcell, m2, in_flight, dpar); in_flight = 1u;
+                cur ^= 1;                                    // its previous batch is done: submit_batch has waited for it
                 count -= 32;
                 pos -= 32;
                 if (sa.flag && pos >= 0) {
-                    S& sl = my[cur];
-                    *reinterpret_cast<int4*>(&sl.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
-                    sl.s[pos] = sa.s; sl.t[pos] = sa.t; sl.e12[pos] = sa.E1E2;
+                    Rec& r = ch.rec[cur];
+                    *reinterpret_cast<int4*>(&r.cell[pos][0]) = make_int4(ci, sa.j, sa.k, sa.l);
+                    r.s[pos] = sa.s; r.t[pos] = sa.t; r.e12[pos] = sa.E1E2;
                 }
             }
         }
         if (count > 0) {                                     // batches never mix spatial cells: flush the partial one
-            submit_slot<kSP>(my[cur], P, lane, count, xcell, m2);
-            busy |= 1u << cur;
+            dpar = submit_batch<kSP>(ch, P.f_aos, P.dN_aos, P.Np, P.S, lane, cur, count, xcell, m2, in_flight, dpar); in_flight = 1u;
             cur ^= 1;
-            if ((busy >> cur) & 1u) {
-                mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
-                dpar ^= 1u << cur;
-                busy &= ~(1u << cur);
-                scatter_slot<kSP>(my[cur], P, lane);
-                __syncwarp();
-            }
             count = 0;
         }
     }
-    submit_slot<kSP>(my[cur], P, lane, -1, 0, 0.0);          // terminator (the current slot is always writable)
-    cur ^= 1;
-    if ((busy >> cur) & 1u) {
-        mbar_wait(&my[cur].done, (dpar >> cur) & 1u);
-        scatter_slot<kSP>(my[cur], P, lane);
-    }
+    submit_batch<kSP>(ch, P.f_aos, P.dN_aos, P.Np, P.S, lane, cur, -1, 0, 0.0, in_flight, dpar);   // flush the last batch, then the terminator
+}
+
+// p1-cell table: (p1x, p1y, p1z, E1) of every momentum cell centre, with the arithmetic of S8c steps 0 and 2
+__global__ void cell_table_kernel(const GridConst g, int Np, double* __restrict__ tab)
+{
+    const int pc = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pc >= Np) return;
+    double p1x, p1y, p1z, E1;
+    cell_kinematics(g, pc, p1x, p1y, p1z, E1);
+    tab[4 * (size_t)pc + 0] = p1x; tab[4 * (size_t)pc + 1] = p1y; tab[4 * (size_t)pc + 2] = p1z; tab[4 * (size_t)pc + 3] = E1;
 }
 
 __global__ void debug_samples_kernel(const CollideParams P, int xcell, int p_begin, int p_end, int* cells, double* stu)
@@ -391,7 +472,7 @@ template <int kMask>
 cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t st)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
-    const size_t smem = sizeof(Slot<kSP>) * kProducerWarps * kSlots + sizeof(int2) * kRetryCap * kProducerWarps;
+    const size_t smem = sizeof(Chan<kSP>) * kProducerWarps + sizeof(int2) * kRetryCap * kProducerWarps;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -438,6 +519,13 @@ cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin,
     if (total <= 0) return cudaSuccess;
     const int blocks = (int)((total + 127) / 128 < 148 * 16 ? (total + 127) / 128 : 148 * 16);
     debug_samples_kernel<<<blocks, 128, 0, st>>>(P, xcell, p_begin, p_end, cells, stu);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_cell_table(const GridConst& g, int Np, double* tab, cudaStream_t st)
+{
+    cell_table_kernel<<<(Np + 255) / 256, 256, 0, st>>>(g, Np, tab);
     ++g_launch_count;
     return cudaGetLastError();
 }

@@ -20,6 +20,7 @@ struct CollideParams {
     const double* f_aos;  // [Nx][Np][SP] cell-major staging copy of f (pad slots 0)
     double* dN_aos;       // [Nx][Np][SP] deposit scratch in number units, zero on entry
     const double* m2;     // [Nx] regulator mass^2
+    const double* cell_tab;   // [Np][4] (p1x, p1y, p1z, E1) of the momentum cell centres
     int S, Np, Nx, Ns;
     unsigned* work_counter;   // device: next work item of the persistent kernel (zeroed before every launch)
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
@@ -62,6 +63,7 @@ struct bz_ctx_impl {
     double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|)
     double *mom;                     // device [2*S*Nx + 2*S + Nx]
     double *absp, *w_invE, *vx, *vy, *vz;   // device [Np] tables
+    double *cell_tab;                // device [Np][4]: p1x, p1y, p1z, E1 (built on the device, bit-exact arithmetic)
     std::string err;
     bool profile;
     std::vector<cudaEvent_t> prof_events;   // start/stop pairs around collide launches
@@ -74,6 +76,7 @@ extern std::atomic<unsigned long long> g_launch_count;
 int collide_slots_per_cell(unsigned mask);
 int collide_cells_per_region(int Np, int Nx, int sms);
 cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st);
+cudaError_t launch_cell_table(const GridConst& g, int Np, double* tab, cudaStream_t st);
 cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, int Np, cudaStream_t st);
 cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin, int p_end, int* cells, double* stu,
                                  cudaStream_t st);
