@@ -33,6 +33,9 @@ struct MsqSet {
     double m1b_t, m1b_u;  // q1 q1bar -> q1 q1bar, straight / crossed
     double ann;           // q1 q1bar -> q2 q2bar       (t <-> u symmetric)
     double a_t, a_u;      // q1 q2 -> q1 q2 (different flavours), straight / crossed
+    // differences to the different-flavour value, formed without cancellation from the terms of Table I:
+    double d11;           // m11 - a_t   = M_A(s,u,t) - (32/3) s^2/(tt ut)
+    double d1b_t, d1b_u;  // m1b_t - a_t = M_ann - (32/3) u^2/(tt s);  m1b_u - a_u = M_ann - (32/3) t^2/(ut s)
 };
 
 // 1/x to ~1 ulp without the IEEE division sequence: the 20-bit hardware seed (MUFU.RCP64H) and two Newton steps.
@@ -68,9 +71,12 @@ BZ_HD MsqSet msq_set(double s, double t, double u, double m2, double g4w)
         M.a_t = at;
         M.a_u = au;
         M.ann = ann;
-        M.m11 = (at + au) - c323 * s2 * (it * iu);
-        M.m1b_t = (at + ann) - c323 * u2 * (it * is);
-        M.m1b_u = (au + ann) - c323 * t2 * (iu * is);
+        M.d11 = au - c323 * s2 * (it * iu);
+        M.d1b_t = ann - c323 * u2 * (it * is);
+        M.d1b_u = ann - c323 * t2 * (iu * is);
+        M.m11 = at + M.d11;
+        M.m1b_t = at + M.d1b_t;
+        M.m1b_u = au + M.d1b_u;
     }
     if (kGlue && kQuark) {
         M.qqgg = c1283 * (u * it + t * iu) - 6.0 * ann;
@@ -112,21 +118,25 @@ BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7
             Xf[p] = X[1 + 2 * p] + X[2 + 2 * p]; Yf[p] = Y[1 + 2 * p] + Y[2 + 2 * p];
             Zf[p] = Z[1 + 2 * p] + Z[2 + 2 * p]; Wf[p] = W[1 + 2 * p] + W[2 + 2 * p];
         }
+        const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
+        const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
         if (glue) {
-            const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
-            const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
             const double T = X[0] * (M.gg * Z[0] + M.qg_t * Zq) - Y[0] * (M.gg * W[0] + M.qg_t * Wq);
             const double U = Z[0] * (M.gg * X[0] + M.qg_t * Xq) - W[0] * (M.gg * Y[0] + M.qg_t * Yq);
             dI[0] -= T; dK[0] += T; dJ[0] -= U; dL[0] += U;
         }
+        // partner sum of quark a: qg_t [g] + m11 [a] + m1b_t [abar] + a_t [the other four] = the base over ALL partners
+        // at the different-flavour value plus the two differences (see the bound in DESIGN.md 6)
+        const double bZ = M.qg_t * Z[0] + M.a_t * Zq, bW = M.qg_t * W[0] + M.a_t * Wq;
+        const double bX = M.qg_t * X[0] + M.a_t * Xq, bY = M.qg_t * Y[0] + M.a_t * Yq;
 #pragma unroll
         for (int a = 1; a < 7; ++a) {
             if (!BZ_ON(a)) continue;
-            const int p = (a - 1) >> 1, ab = (a & 1) ? a + 1 : a - 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
-            const double ZM = ((M.qg_t * Z[0] + M.m11 * Z[a]) + M.m1b_t * Z[ab]) + M.a_t * (Zf[p1] + Zf[p2]);
-            const double WM = ((M.qg_t * W[0] + M.m11 * W[a]) + M.m1b_t * W[ab]) + M.a_t * (Wf[p1] + Wf[p2]);
-            const double XM = ((M.qg_t * X[0] + M.m11 * X[a]) + M.m1b_t * X[ab]) + M.a_t * (Xf[p1] + Xf[p2]);
-            const double YM = ((M.qg_t * Y[0] + M.m11 * Y[a]) + M.m1b_t * Y[ab]) + M.a_t * (Yf[p1] + Yf[p2]);
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const double ZM = fma(M.d11, Z[a], fma(M.d1b_t, Z[ab], bZ));
+            const double WM = fma(M.d11, W[a], fma(M.d1b_t, W[ab], bW));
+            const double XM = fma(M.d11, X[a], fma(M.d1b_t, X[ab], bX));
+            const double YM = fma(M.d11, Y[a], fma(M.d1b_t, Y[ab], bY));
             const double T = X[a] * ZM - Y[a] * WM;
             const double U = Z[a] * XM - W[a] * YM;
             dI[a] -= T; dK[a] += T; dJ[a] -= U; dL[a] += U;
@@ -145,21 +155,25 @@ BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7
             Xf[p] = X[1 + 2 * p] + X[2 + 2 * p]; Yf[p] = Y[1 + 2 * p] + Y[2 + 2 * p];
             Zf[p] = Z[1 + 2 * p] + Z[2 + 2 * p]; Wf[p] = W[1 + 2 * p] + W[2 + 2 * p];
         }
+        const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
+        const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
         if (glue) {
-            const double Xq = (Xf[0] + Xf[1]) + Xf[2], Yq = (Yf[0] + Yf[1]) + Yf[2];
-            const double Zq = (Zf[0] + Zf[1]) + Zf[2], Wq = (Wf[0] + Wf[1]) + Wf[2];
             const double T = M.qg_u * (X[0] * Zq - Y[0] * Wq);
             const double U = M.qg_u * (Z[0] * Xq - W[0] * Yq);
             dI[0] -= T; dL[0] += T; dJ[0] -= U; dK[0] += U;
         }
+        // partner sum of quark a: qg_u [g] + m1b_u [abar] + a_u [the other four]; the same-species partner belongs to
+        // the t-family only (M_11 is t <-> u symmetric and listed once), so it is taken out of the base again
+        const double bZ = M.qg_u * Z[0] + M.a_u * Zq, bW = M.qg_u * W[0] + M.a_u * Wq;
+        const double bX = M.qg_u * X[0] + M.a_u * Xq, bY = M.qg_u * Y[0] + M.a_u * Yq;
 #pragma unroll
         for (int a = 1; a < 7; ++a) {
             if (!BZ_ON(a)) continue;
-            const int p = (a - 1) >> 1, ab = (a & 1) ? a + 1 : a - 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
-            const double ZM = (M.qg_u * Z[0] + M.m1b_u * Z[ab]) + M.a_u * (Zf[p1] + Zf[p2]);
-            const double WM = (M.qg_u * W[0] + M.m1b_u * W[ab]) + M.a_u * (Wf[p1] + Wf[p2]);
-            const double XM = (M.qg_u * X[0] + M.m1b_u * X[ab]) + M.a_u * (Xf[p1] + Xf[p2]);
-            const double YM = (M.qg_u * Y[0] + M.m1b_u * Y[ab]) + M.a_u * (Yf[p1] + Yf[p2]);
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const double ZM = fma(-M.a_u, Z[a], fma(M.d1b_u, Z[ab], bZ));
+            const double WM = fma(-M.a_u, W[a], fma(M.d1b_u, W[ab], bW));
+            const double XM = fma(-M.a_u, X[a], fma(M.d1b_u, X[ab], bX));
+            const double YM = fma(-M.a_u, Y[a], fma(M.d1b_u, Y[ab], bY));
             const double T = X[a] * ZM - Y[a] * WM;
             const double U = Z[a] * XM - W[a] * YM;
             dI[a] -= T; dL[a] += T; dJ[a] -= U; dK[a] += U;
@@ -188,15 +202,25 @@ BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7
             const double Rg = M.qqgg * (Outg * ((Inf[0] + Inf[1]) + Inf[2]) - Obg * ((Ibf[0] + Ibf[1]) + Ibf[2]));
             dI[0] -= Sg; dJ[0] -= Sg; dK[0] += Rg; dL[0] += Rg;
         }
+        // partner sum of the quark pair of flavour p: q qbar <-> g g plus annihilation into the OTHER flavours = the
+        // base over all flavours minus its own
+        const double Outq = (Outf[0] + Outf[1]) + Outf[2], Obq = (Obf[0] + Obf[1]) + Obf[2];
+        const double Inq = (Inf[0] + Inf[1]) + Inf[2], Ibq = (Ibf[0] + Ibf[1]) + Ibf[2];
+        const double bOut = M.qqgg * Outg + M.ann * Outq, bOb = M.qqgg * Obg + M.ann * Obq;
+        const double bIn = M.qqgg * Ing + M.ann * Inq, bIb = M.qqgg * Ibg + M.ann * Ibq;
+        double pOut[3], pOb[3], pIn[3], pIb[3];
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            pOut[p] = fma(-M.ann, Outf[p], bOut); pOb[p] = fma(-M.ann, Obf[p], bOb);
+            pIn[p] = fma(-M.ann, Inf[p], bIn);    pIb[p] = fma(-M.ann, Ibf[p], bIb);
+        }
 #pragma unroll
         for (int a = 1; a < 7; ++a) {
             const int ab = (a & 1) ? a + 1 : a - 1;
             if (!(BZ_ON(a) && BZ_ON(ab))) continue;
-            const int p = (a - 1) >> 1, p1 = (p + 1) % 3, p2 = (p + 2) % 3;
-            const double S = In[a] * (M.qqgg * Outg + M.ann * (Outf[p1] + Outf[p2]))
-                           - Ib[a] * (M.qqgg * Obg + M.ann * (Obf[p1] + Obf[p2]));
-            const double R = Out[a] * (M.qqgg * Ing + M.ann * (Inf[p1] + Inf[p2]))
-                           - Ob[a] * (M.qqgg * Ibg + M.ann * (Ibf[p1] + Ibf[p2]));
+            const int p = (a - 1) >> 1;
+            const double S = In[a] * pOut[p] - Ib[a] * pOb[p];
+            const double R = Out[a] * pIn[p] - Ob[a] * pIb[p];
             dI[a] -= S; dJ[ab] -= S; dK[a] += R; dL[ab] += R;
         }
     }

@@ -1,7 +1,7 @@
 // bz_collision.cu -- sample -> |M|^2 -> bracket -> symmetric deposit (S8a.2-8a.5) as ONE persistent, warp-specialised
-// kernel (one CTA of 16 warps per SM):
+// kernel (one CTA of 20 warps per SM):
 //
-//   producer warps (12, warpgroups 1-3, 88 registers after setmaxnreg.dec)
+//   producer warps (16, warpgroups 1-4, 64 registers after setmaxnreg.dec)
 //       sample   pull work items (a run of p1 cells of one spatial cell) from a global counter; lanes = samples:
 //                Philox4x32-10, the boost, the binning (bz_sample.cuh).  About 46 % of the samples keep both outgoing
 //                legs in the box; they are compacted (ballot + prefix) straight into one of the warp's two record
@@ -12,8 +12,8 @@
 //                32 scattered ones.  Completion is signalled to the consumer by cp.async.mbarrier.arrive on the
 //                "full" mbarrier: the producer never waits for its own gathers and goes on sampling into the other
 //                record buffer.
-//   consumer warps (4, warpgroup 0, one per SM sub-partition, 240 registers after setmaxnreg.inc)
-//       compute  serve three producers each in rotation: wait "full", every lane takes one sample of the batch:
+//   consumer warps (4, warpgroup 0, one per SM sub-partition, 224 registers after setmaxnreg.inc)
+//       compute  serve four producers each (non-blocking probes in rotation): every lane takes one sample of the batch:
 //                <= 10 |M|^2 values, factorised channel algebra (bz_channels.cuh); the 4 x S deposits overwrite the
 //                gathered f in the stage buffer; arrive on "done".
 //       (pure glue, one double per cell: the consumer issues its four reductions straight from the registers.)
@@ -22,7 +22,11 @@
 //                per 64-byte cell, into the cell-major scratch dN_aos, which stays in L2 while its spatial cell is
 //                being worked on; then it gathers the new batch into the same buffer.
 // The ALU-bound sampling and the latency-bound gather/scatter overlap on the same SM, the register file is split
-// 240 / 88 between the two roles, and no sample record ever leaves the SM.
+// 224 / 64 between the two roles (640 threads launch with 96 registers each; setmaxnreg only moves registers inside
+// that pool of 61440), and no sample record ever leaves the SM.  Measured on B200, config 4 (ablations, ms per
+// launch of 211): sampling + compaction alone 102, consumer algebra +75, RED flush +43, cp.async gather +27 -- the
+// parts add up, i.e. the kernel is bound by issue slots (FP64 instructions occupy the 16-lane pipe for 2 cycles),
+// not by latency: 12 -> 16 producer warps gave +4 %.
 // Measured on B200 (microbenchmark over all 148 SMs): a RED whose 32 lanes hit 32 different sectors
 // costs 48 cycles of the SM's L1TEX path, the 8-lanes-per-cell form 15.7; chip-wide that form saturates at ~6e10 cell
 // updates/s (the L2 reduction rate).  The 64-byte TMA bulk reduction (cp.reduce.async.bulk.add.f64) reaches the same
@@ -35,11 +39,24 @@ namespace bz {
 
 namespace {
 
+#ifndef BZ_PRODUCER_WARPS
+#define BZ_PRODUCER_WARPS 16
+#endif
+#ifndef BZ_CONSUMER_REGS
+#define BZ_CONSUMER_REGS 224
+#endif
+#ifndef BZ_PRODUCER_REGS
+#define BZ_PRODUCER_REGS 64
+#endif
 constexpr int kConsumerWarps = 4;                // warpgroup 0
-constexpr int kProducerWarps = 12;               // warpgroups 1..3
+constexpr int kProducerWarps = BZ_PRODUCER_WARPS;   // warpgroups 1..
 constexpr int kProducersPerConsumer = kProducerWarps / kConsumerWarps;
 constexpr int kCollideThreads = 32 * (kConsumerWarps + kProducerWarps);
-constexpr int kConsumerRegs = 240, kProducerRegs = 88;   // 128 x 240 + 384 x 88 = 64512 <= 65536
+constexpr int kConsumerRegs = BZ_CONSUMER_REGS, kProducerRegs = BZ_PRODUCER_REGS;
+// setmaxnreg moves registers inside the pool the CTA was launched with (threads x launch registers, the launch count
+// being 64 K / threads rounded down to a multiple of 8): a split that needs more never gets its .inc granted and hangs
+constexpr int kLaunchRegs = (65536 / kCollideThreads) / 8 * 8;
+static_assert(128 * kConsumerRegs + 32 * kProducerWarps * kProducerRegs <= kCollideThreads * kLaunchRegs, "register pool");
 
 // doubles per cell in the global staging layout: 1 for the pure-glue mask, 8 (half a 128-byte line) otherwise
 template <int kMask>
@@ -75,6 +92,14 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* b, unsigned parity, unsi
     unsigned ok;
     asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
+// non-blocking probe of a phase
+__device__ __forceinline__ bool mbar_test_wait(uint64_t* b, unsigned parity)
+{
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
     return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* b, unsigned parity)
@@ -310,15 +335,21 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         const unsigned mask = kMask >= 0 ? (unsigned)kMask : P.mask;
         unsigned alive = (1u << kProducersPerConsumer) - 1u;   // producers of this consumer still running
         unsigned par = 0;                                      // bit q: parity of the next "full" phase of producer q
-        int q = 0;
+        int q = 0, misses = 0;
         while (alive) {
-            // poll the alive producers in rotation; each try suspends the warp for at most ~0.3 us
+            // probe the alive producers in rotation without blocking; only after a whole round of misses suspend
+            // (for at most ~0.2 us) on the next one
             if ((alive >> q) & 1u) {
                 C& ch = chans[warp + kConsumerWarps * q];
-                if (mbar_try_wait(&ch.full, (par >> q) & 1u, 300u)) {
+                const unsigned pq = (par >> q) & 1u;
+                const bool ready = misses < kProducersPerConsumer ? mbar_test_wait(&ch.full, pq) : mbar_try_wait(&ch.full, pq, 200u);
+                if (ready) {
                     par ^= 1u << q;
+                    misses = 0;
                     if (ch.nvalid < 0) alive &= ~(1u << q);
                     else consume_batch<kMask, kSP>(ch, P, lane, mask);
+                } else {
+                    misses = misses < kProducersPerConsumer ? misses + 1 : 0;
                 }
             }
             q = (q + 1 == kProducersPerConsumer) ? 0 : q + 1;
