@@ -47,6 +47,25 @@ def algorithmic_bytes_per_sample(cfg):
     return 48.0 * cfg.S + 16.0 * cfg.S / cfg.samples
 
 
+# fp64 operations per kinematic sample, upper ends of SURVEY.md 8d's table (S = 1, 6, 7 species)
+FP64_FLOP_PER_SAMPLE = {1: 140.0, 6: 1350.0, 7: 1850.0}
+
+
+def transport_roofline(cfg, tr_ms, tr_n, peak):
+    """Stream + Euler kernel (a6 + a7): phase-space cell updates per second against its HBM bytes.  Per value: 8 B f
+    read, 8 B f_new written, 8 B deposit read + 8 B re-zeroed, 8 B cell-major copy of the new f written (padded to 8
+    slots per cell when S > 1), upwind neighbours from L2: DESIGN.md 6."""
+    if not tr_n or tr_ms <= 0:
+        return None
+    pad = 8.0 / cfg.S if cfg.S > 1 else 0.0
+    bytes_per_value = 16.0 + (24.0 * pad if cfg.S > 1 else 16.0)
+    rate = cfg.n_values * tr_n / (tr_ms * 1e-3)
+    ach = rate * bytes_per_value / 1e9
+    return {"bound": "hbm", "kernel": "transport_kernel<1> (upwind stream + Euler + deposit conversion)",
+            "cell_updates_per_sec": rate, "bytes_per_value": bytes_per_value, "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "ms_per_launch": tr_ms / tr_n}
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -186,7 +205,8 @@ def run_ours(args, cfg):
         sampler.start()
         time.sleep(0.3)
     g.set_profile(True)
-    g.get_profile()
+    g.get_profile(0)
+    g.get_profile(1)
     barrier()
     launches0 = bz.launch_count()
     ms = 0.0
@@ -209,8 +229,10 @@ def run_ours(args, cfg):
         ms = e0.elapsed_time(e1)
     barrier()
     launches = bz.launch_count() - launches0
-    coll_ms, coll_n = g.get_profile()
+    coll_ms, coll_n = g.get_profile(0)
+    tr_ms, tr_n = g.get_profile(1)
     g.set_profile(False)
+    fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * cfg.Nx:2 * cfg.S * cfg.Nx + 2 * cfg.S:2].sum())
 
@@ -229,10 +251,10 @@ def run_ours(args, cfg):
     ms_e2e = e0.elapsed_time(e1)
     barrier()
 
-    t = torch.tensor([ms, ms_e2e, coll_ms], dtype=torch.float64, device=dev)
+    t = torch.tensor([ms, ms_e2e, coll_ms, tr_ms], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, ms_e2e, coll_ms = (float(x) for x in t.cpu())
+    ms, ms_e2e, coll_ms, tr_ms = (float(x) for x in t.cpu())
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -259,12 +281,17 @@ def run_ours(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": cfg.n_values * 8,
                 "d2h_bytes_per_step": cfg.n_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": "collide_kernel (+ pack_kernel: CUDA events inside libbz.so around the pair)",
+        "roofline": {"bound": "hbm", "kernel": "collide_kernel (CUDA events inside libbz.so around every launch)",
                      "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak if ach else None,
                      "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (ncu dram read + write)",
                      "peak_source": peak_src,
                      "bytes_per_sample": bps, "samples_per_launch": samples_step,
-                     "ms_per_launch": coll_ms / coll_n if coll_n else None},
+                     "ms_per_launch": coll_ms / coll_n if coll_n else None,
+                     "fp64_peak_tflops_measured": fp64_peak,
+                     "fp64_bound_samples_per_sec": fp64_peak * 1e12 / FP64_FLOP_PER_SAMPLE.get(cfg.S, 1850.0) if fp64_peak else None,
+                     "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; "
+                             "the HBM one is the slower for every config and is the one reported"},
+        "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
         "clocks": clocks,
         "total_particle_number": N1,
     }

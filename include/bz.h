@@ -85,11 +85,18 @@ int bz_moments(bz_ctx* ctx, double* out_host);
 /* Text of the last CUDA error seen by this context ("" if none). */
 const char* bz_last_error(const bz_ctx* ctx);
 
-/* Kernel timing for the roofline report: while profiling is on (on != 0), every launch of the collision kernel is
- * bracketed by CUDA events on the context's stream.  bz_get_profile synchronises the stream, writes the summed
- * duration (milliseconds) and the number of launches since the last call, and clears the record. */
+/* Kernel timing for the roofline report: while profiling is on (on != 0), bz_step / bz_collision bracket two groups
+ * of launches with CUDA events on the context's stream: group 0 = the collision kernel (with the cell-major staging
+ * copy when one is needed), group 1 = the stream + Euler kernel of bz_step.  bz_get_profile synchronises the stream,
+ * writes the summed duration (milliseconds) and the number of bracketed regions of that group since the last call,
+ * and clears the group's record. */
 int bz_set_profile(bz_ctx* ctx, int on);
-int bz_get_profile(bz_ctx* ctx, double* collide_ms_total, int* collide_launches);
+int bz_get_profile(bz_ctx* ctx, int group, double* ms_total, int* launches);
+
+/* FP64 FMA peak of the current device in TFLOP/s, measured with a register-resident DFMA chain kernel on the default
+ * stream (a few milliseconds; synchronises).  This is the FP64 leg of the roofline NS defines for the collision
+ * kernel ("the slower of FP64 FMA peak and gathered/scattered bytes at HBM bandwidth").  Needs no context. */
+int bz_measure_fp64_peak(double* tflops_out_host);
 
 /* Number of CUDA kernels this library has launched in this process so far (all contexts); bench.py reports the
  * difference over its timed region as "gpu_launches". */

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
-           "bz_get_profile", "bz_launch_count", "bz_debug_samples",
+           "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
 
 
@@ -47,7 +47,8 @@ def lib():
         L.bz_last_error.argtypes = [vp]
         L.bz_last_error.restype = C.c_char_p
         L.bz_set_profile.argtypes = [vp, C.c_int]
-        L.bz_get_profile.argtypes = [vp, dp, ip]
+        L.bz_get_profile.argtypes = [vp, C.c_int, dp, ip]
+        L.bz_measure_fp64_peak.argtypes = [dp]
         L.bz_launch_count.argtypes = []
         L.bz_launch_count.restype = C.c_ulonglong
         L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
@@ -173,9 +174,10 @@ class Boltzmann:
     def set_profile(self, on):
         self._chk(lib().bz_set_profile(self._h, int(bool(on))), "bz_set_profile")
 
-    def get_profile(self):
+    def get_profile(self, group=0):
+        """(milliseconds, regions) of group 0 = collision kernel, 1 = stream + Euler kernel since the last call."""
         ms, n = C.c_double(), C.c_int()
-        self._chk(lib().bz_get_profile(self._h, C.byref(ms), C.byref(n)), "bz_get_profile")
+        self._chk(lib().bz_get_profile(self._h, group, C.byref(ms), C.byref(n)), "bz_get_profile")
         return ms.value, n.value
 
     def debug_samples(self, step, xcell, pbegin, pend, want_stu=True):
@@ -185,6 +187,15 @@ class Boltzmann:
         self._chk(lib().bz_debug_samples(self._h, step, xcell, pbegin, pend, C.c_void_p(cells.data_ptr()),
                                          C.c_void_p(stu.data_ptr()) if want_stu else None), "bz_debug_samples")
         return cells, stu
+
+
+def measure_fp64_peak():
+    """bz_measure_fp64_peak: measured FP64 FMA peak of the current device, TFLOP/s."""
+    v = C.c_double()
+    rc = lib().bz_measure_fp64_peak(C.byref(v))
+    if rc != 0:
+        raise BzError("bz_measure_fp64_peak failed (%d)" % rc)
+    return v.value
 
 
 def launch_count():

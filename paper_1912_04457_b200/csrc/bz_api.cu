@@ -63,9 +63,11 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
 {
     CollideParams P;
     P.g = grid_const(c);
-    P.f_aos = c->f_aos; P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab;
+    P.f_aos = c->SP == 1 ? c->f : c->f_aos;    // one species: the API layout is already cell-major
+    P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab;
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
-    P.work_counter = c->work_counter; P.n_items = (unsigned)c->Nx * (unsigned)c->regions_per_x; P.x_begin = 0;
+    P.work_counter = c->work_counter + c->launch_parity; P.next_counter = c->work_counter + (c->launch_parity ^ 1u);
+    P.n_items = (unsigned)c->Nx * (unsigned)c->regions_per_x; P.x_begin = 0;
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
     const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
@@ -77,30 +79,37 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     return P;
 }
 
+// CUDA events around a group of launches while profiling is on
+int prof_mark(bz_ctx* c, int group)
+{
+    if (!c->profile) return 0;
+    cudaEvent_t e = nullptr;
+    BZ_CUDA(cudaEventCreate(&e), "event");
+    BZ_CUDA(cudaEventRecord(e, c->stream), "event record");
+    c->prof_events[group].push_back(e);
+    return 0;
+}
+
 int run_collide(bz_ctx* c, double dt_fm, unsigned step)
 {
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (c->profile) {
-        BZ_CUDA(cudaEventCreate(&e0), "event");
-        BZ_CUDA(cudaEventCreate(&e1), "event");
-        BZ_CUDA(cudaEventRecord(e0, c->stream), "event record");
+    if (int rc = prof_mark(c, 0)) return rc;
+    if (c->SP != 1 && !c->aos_valid) {
+        BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
+        c->aos_valid = true;
     }
-    BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
     BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->sms, c->stream), "collide");
-    if (c->profile) {
-        BZ_CUDA(cudaEventRecord(e1, c->stream), "event record");
-        c->prof_events.push_back(e0);
-        c->prof_events.push_back(e1);
-    }
-    return 0;
+    c->launch_parity ^= 1u;
+    return prof_mark(c, 0);
 }
 
 // regulator mass^2 per spatial cell from the current f (S8a.1)
 int update_m2(bz_ctx* c)
 {
+    if (c->rowsum_valid) return 0;
     BZ_CUDA(launch_rowsums(c->f, c->absp, c->w_invE, c->rowsum, c->Nx * c->S, c->Np, c->stream), "rowsums");
     const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;   // the gluon, if active, is layout index 0
     BZ_CUDA(launch_m2(c->rowsum, c->m2, c->Nx, c->S, glue_slot_mask, 4.0 * kPi * c->alpha_s, c->m_D, c->stream), "m2");
+    c->rowsum_valid = true;
     return 0;
 }
 
@@ -128,6 +137,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
+    c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
@@ -144,7 +154,8 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
         c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
     }
     const size_t bytes = c->n_values * sizeof(double);
-    BZ_CUDA(cudaMalloc(&c->work_counter, sizeof(unsigned)), "cudaMalloc work counter");
+    BZ_CUDA(cudaMalloc(&c->work_counter, 2 * sizeof(unsigned)), "cudaMalloc work counter");
+    BZ_CUDA(cudaMemset(c->work_counter, 0, 2 * sizeof(unsigned)), "memset work counter");
     BZ_CUDA(cudaMalloc(&c->f, bytes), "cudaMalloc f");
     BZ_CUDA(cudaMalloc(&c->f_new, bytes), "cudaMalloc f_new");
     c->SP = collide_slots_per_cell(c->mask);
@@ -187,7 +198,7 @@ int bz_destroy(bz_ctx* c)
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp); cudaFree(c->cell_tab);
-    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
+    for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete c;
     return 0;
 }
@@ -204,6 +215,7 @@ int bz_set_f(bz_ctx* c, const double* f, int on_device)
     if (!c->f) return -4;
     BZ_CUDA(cudaMemcpyAsync(c->f, f, c->n_values * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                             c->stream), "bz_set_f copy");
+    c->aos_valid = false; c->rowsum_valid = false;
     if (!on_device) BZ_CUDA(cudaStreamSynchronize(c->stream), "bz_set_f sync");
     return 0;
 }
@@ -233,7 +245,7 @@ int bz_collision(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
 static TransportParams transport_params(const bz_ctx* c, double dt_fm, double* out)
 {
     TransportParams T;
-    T.f = c->f; T.dN_aos = c->dN_aos; T.SP = c->SP; T.out = out; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
+    T.f = c->f; T.dN_aos = c->dN_aos; T.SP = c->SP; T.out = out; T.f_aos_out = c->f_aos; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
     T.nx = c->grid.nx; T.ny = c->grid.ny; T.nz = c->grid.nz; T.S = c->S; T.Np = c->Np;
     T.cfl = dt_fm / c->grid.dx;
     fill_deg(c, T.inv_deg);
@@ -254,8 +266,11 @@ int bz_step(bz_ctx* c, double dt_fm)
     if (!c->f) return -4;
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, c->step)) return rc;
+    if (int rc = prof_mark(c, 1)) return rc;
     BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 1, c->stream), "stream+euler");
+    if (int rc = prof_mark(c, 1)) return rc;
     double* t = c->f; c->f = c->f_new; c->f_new = t;
+    c->rowsum_valid = false;          // f changed; f_aos was rewritten with the new f by the Euler kernel
     c->step += 1;
     return 0;
 }
@@ -279,20 +294,21 @@ int bz_moments(bz_ctx* c, double* out_host)
 
 int bz_set_profile(bz_ctx* c, int on) { if (!c) return -1; c->profile = on != 0; return 0; }
 
-int bz_get_profile(bz_ctx* c, double* ms_total, int* launches)
+int bz_get_profile(bz_ctx* c, int group, double* ms_total, int* launches)
 {
-    if (!c || !ms_total || !launches) return -1;
+    if (!c || !ms_total || !launches || group < 0 || group > 1) return -1;
     BZ_CUDA(cudaStreamSynchronize(c->stream), "profile sync");
+    std::vector<cudaEvent_t>& ev = c->prof_events[group];
     double tot = 0.0;
-    for (size_t q = 0; q + 1 < c->prof_events.size(); q += 2) {
+    for (size_t q = 0; q + 1 < ev.size(); q += 2) {
         float ms = 0.f;
-        BZ_CUDA(cudaEventElapsedTime(&ms, c->prof_events[q], c->prof_events[q + 1]), "event elapsed");
+        BZ_CUDA(cudaEventElapsedTime(&ms, ev[q], ev[q + 1]), "event elapsed");
         tot += ms;
     }
     *ms_total = tot;
-    *launches = (int)(c->prof_events.size() / 2);
-    for (cudaEvent_t e : c->prof_events) cudaEventDestroy(e);
-    c->prof_events.clear();
+    *launches = (int)(ev.size() / 2);
+    for (cudaEvent_t e : ev) cudaEventDestroy(e);
+    ev.clear();
     return 0;
 }
 

@@ -326,6 +326,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         mbar_init(&chans[threadIdx.x].full, 33);
         mbar_init(&chans[threadIdx.x].done, 1);
     }
+    if (blockIdx.x == 0 && threadIdx.x == 0) *P.next_counter = 0u;   // the other launch parity: idle during this launch
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
 
@@ -530,8 +531,6 @@ int collide_cells_per_region(int Np, int Nx, int sms)
 // one persistent CTA per SM (fewer when there is less work than producer warps)
 cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st)
 {
-    cudaError_t e = cudaMemsetAsync(P.work_counter, 0, sizeof(unsigned), st);
-    if (e != cudaSuccess) return e;
     int ctas = (int)((P.n_items + kProducerWarps - 1) / kProducerWarps);
     if (ctas > sms) ctas = sms;
     if (ctas < 1) ctas = 1;

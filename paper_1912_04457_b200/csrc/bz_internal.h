@@ -22,7 +22,8 @@ struct CollideParams {
     const double* m2;     // [Nx] regulator mass^2
     const double* cell_tab;   // [Np][4] (p1x, p1y, p1z, E1) of the momentum cell centres
     int S, Np, Nx, Ns;
-    unsigned* work_counter;   // device: next work item of the persistent kernel (zeroed before every launch)
+    unsigned* work_counter;   // device: next work item of the persistent kernel (0 on entry)
+    unsigned* next_counter;   // device: the counter of the NEXT launch, zeroed by this one
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
     int x_begin;              // first spatial cell (0; items address xcell = x_begin + item / regions_per_x)
     int cells_per_region;     // p1 cells per work item (one producer warp each)
@@ -37,6 +38,7 @@ struct TransportParams {
     const double* f;      // old f
     double* dN_aos;       // collision deposits [Nx][Np][SP] (number units), reset to 0 when consumed
     double* out;          // f_new or dF
+    double* f_aos_out;    // mode 1: the new f once more, cell-major [Nx][Np][SP] (the next step's gather source); unused if SP == 1
     int SP;
     const double* vx; const double* vy; const double* vz;   // [Np] p/|p| at the cell centre (0 at p = 0)
     int nx, ny, nz, S, Np;
@@ -56,7 +58,10 @@ struct bz_ctx_impl {
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
     double *f_aos, *dN_aos;          // device, Nx*Np*SP each (cell-major staging for the collision kernel)
     int SP;                          // doubles per cell in the staging layout
-    unsigned* work_counter;          // device, 1 word
+    unsigned* work_counter;          // device, 2 words used alternately (each launch zeroes the other one)
+    unsigned launch_parity;          // which of the two the next launch uses
+    bool aos_valid;                  // f_aos holds the current f (written by the Euler kernel; bz_set_f invalidates)
+    bool rowsum_valid;               // rowsum / m2 belong to the current f
     int sms;                         // SMs of the device (persistent grid size)
     int cells_per_region, regions_per_x;
     double *m2;                      // device [Nx]
@@ -66,7 +71,7 @@ struct bz_ctx_impl {
     double *cell_tab;                // device [Np][4]: p1x, p1y, p1z, E1 (built on the device, bit-exact arithmetic)
     std::string err;
     bool profile;
-    std::vector<cudaEvent_t> prof_events;   // start/stop pairs around collide launches
+    std::vector<cudaEvent_t> prof_events[2];   // start/stop pairs: [0] collision (pack + collide), [1] stream + Euler
 };
 
 // kernels launched by this library in this process (bz_launch_count); bumped by every launcher below

@@ -25,20 +25,47 @@ __global__ void __launch_bounds__(256) transport_kernel(const TransportParams P)
         const ptrdiff_t oy = (ptrdiff_t)(cy > 0.0 ? ym : yp) * (ptrdiff_t)row;
         const ptrdiff_t oz = (ptrdiff_t)(cz > 0.0 ? zm : zp) * (ptrdiff_t)row;
         const double ax = fabs(cx), ay = fabs(cy), az = fabs(cz);
-        double* dn = kMode == 1 ? P.dN_aos + ((size_t)xcell * P.Np + pc) * P.SP : nullptr;
-        for (int a = 0; a < P.S; ++a) {
-            const size_t idx = (size_t)xcell * row + (size_t)a * P.Np + pc;
-            const double f0 = P.f[idx];
-            // max(c,0)(f0 - f-) + min(c,0)(f+ - f0) = |c| (f0 - f_upwind)
-            double acc = ax * (f0 - P.f[idx + ox]);
-            acc += ay * (f0 - P.f[idx + oy]);
-            acc += az * (f0 - P.f[idx + oz]);
-            if (kMode == 0) {
+        if (kMode == 0) {
+            for (int a = 0; a < P.S; ++a) {
+                const size_t idx = (size_t)xcell * row + (size_t)a * P.Np + pc;
+                const double f0 = P.f[idx];
+                // max(c,0)(f0 - f-) + min(c,0)(f+ - f0) = |c| (f0 - f_upwind)
+                double acc = ax * (f0 - P.f[idx + ox]);
+                acc += ay * (f0 - P.f[idx + oy]);
+                acc += az * (f0 - P.f[idx + oz]);
                 P.out[idx] = -acc;
+            }
+        } else {
+            // Euler: the cell's collision deposits come from the cell-major scratch (64 contiguous bytes per thread,
+            // reset to 0 here) and the new f also goes out cell-major, as the next step's gather source f_aos
+            double2* dn = reinterpret_cast<double2*>(P.dN_aos + ((size_t)xcell * P.Np + pc) * P.SP);
+            double2* fo = reinterpret_cast<double2*>(P.f_aos_out + ((size_t)xcell * P.Np + pc) * P.SP);
+            double d[8], fn[8];
+            if (P.SP == 8) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) { const double2 v = dn[q]; d[2 * q] = v.x; d[2 * q + 1] = v.y; }
             } else {
-                const double dFc = dn[a] / P.inv_deg[a];
-                dn[a] = 0.0;
-                P.out[idx] = (f0 - acc) + dFc;
+                d[0] = P.dN_aos[(size_t)xcell * P.Np + pc];
+            }
+#pragma unroll
+            for (int a = 0; a < 7; ++a) {
+                fn[a] = 0.0;
+                if (a < P.S) {
+                    const size_t idx = (size_t)xcell * row + (size_t)a * P.Np + pc;
+                    const double f0 = P.f[idx];
+                    double acc = ax * (f0 - P.f[idx + ox]);
+                    acc += ay * (f0 - P.f[idx + oy]);
+                    acc += az * (f0 - P.f[idx + oz]);
+                    fn[a] = (f0 - acc) + d[a] / P.inv_deg[a];
+                    P.out[idx] = fn[a];
+                }
+            }
+            fn[7] = 0.0;
+            if (P.SP == 8) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) { dn[q] = make_double2(0.0, 0.0); fo[q] = make_double2(fn[2 * q], fn[2 * q + 1]); }
+            } else {
+                P.dN_aos[(size_t)xcell * P.Np + pc] = 0.0;      // SP == 1: f itself is the gather source
             }
         }
     }
