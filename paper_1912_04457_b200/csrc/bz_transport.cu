@@ -9,16 +9,22 @@ namespace {
 // One thread per (xcell, pcell), looping over the species: f is read and written coalesced in pcell for every
 // species, the collision deposits of the cell come from the cell-major scratch (64 contiguous bytes per thread).  Upwind flux form of the drift term of Eq. 13:
 // dF = - sum_d [ max(c_d,0) (f(x) - f(x - e_d)) + min(c_d,0) (f(x + e_d) - f(x)) ],  c_d = v_d dt/dx, periodic.
+#ifndef BZ_TR_MINB
+#define BZ_TR_MINB 4
+#endif
 template <int kMode>
-__global__ void __launch_bounds__(256) transport_kernel(const TransportParams P)
+__global__ void __launch_bounds__(256, BZ_TR_MINB) transport_kernel(const TransportParams P)
 {
-    const int xcell = blockIdx.y;
+    // blockIdx.x = spatial cell (fastest), blockIdx.y = chunk of 256 momentum cells: the blocks in flight share one
+    // momentum chunk of ALL spatial cells (Nx x S x 2 KB, 58 MB for config 4), which fits L2, so the three upwind
+    // neighbour reads hit L2 instead of HBM (x-major order: the z neighbour is 256 rows = 198 MB away and misses)
+    const int xcell = blockIdx.x;
     const int ix = xcell % P.nx, iy = (xcell / P.nx) % P.ny, iz = xcell / (P.nx * P.ny);
     const size_t row = (size_t)P.S * P.Np;                    // doubles per spatial cell
     const int xm = (ix + P.nx - 1) % P.nx - ix, xp = (ix + 1) % P.nx - ix;
     const int ym = ((iy + P.ny - 1) % P.ny - iy) * P.nx, yp = ((iy + 1) % P.ny - iy) * P.nx;
     const int zm = ((iz + P.nz - 1) % P.nz - iz) * P.nx * P.ny, zp = ((iz + 1) % P.nz - iz) * P.nx * P.ny;
-    for (int pc = blockIdx.x * blockDim.x + threadIdx.x; pc < P.Np; pc += gridDim.x * blockDim.x) {
+    for (int pc = blockIdx.y * blockDim.x + threadIdx.x; pc < P.Np; pc += gridDim.y * blockDim.x) {
         const double cx = P.vx[pc] * P.cfl, cy = P.vy[pc] * P.cfl, cz = P.vz[pc] * P.cfl;
         // only the upwind neighbour of each axis is read
         const ptrdiff_t ox = (ptrdiff_t)(cx > 0.0 ? xm : xp) * (ptrdiff_t)row;
@@ -136,9 +142,9 @@ __global__ void moments_kernel(const double* __restrict__ rowsum, const double* 
 
 cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st)
 {
-    int bx = (P.Np + 255) / 256;
-    if (bx > 64) bx = 64;
-    dim3 grid(bx, P.nx * P.ny * P.nz);
+    int chunks = (P.Np + 255) / 256;
+    if (chunks > 65535) chunks = 65535;
+    dim3 grid(P.nx * P.ny * P.nz, chunks);
     if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
     else transport_kernel<1><<<grid, 256, 0, st>>>(P);
     ++g_launch_count;
