@@ -14,8 +14,9 @@ north_star quotes the roofline target on; it fits one GPU.  One JSON line is pri
                    algorithmic gather/scatter bytes per sample x samples / duration vs measured HBM GB/s
   cpu_baseline     the oracle as it stands, on this box's host cores, on a bounded sample of the same workload
 
-N > 1 (torchrun): the path is built for one GPU (north_star); ranks run independent replicas ("replicas only", weak
-scaling, no data-path collective) and the max over ranks of the device time is used.
+N > 1 (torchrun): weak scaling by domain decomposition (paper_1912_04457_b200/slab.py): the domain is
+the config repeated N times along z, every rank owns one copy and exchanges one boundary layer with each z neighbour
+per step (the drift stencil's only coupling); collisions are local.  The max over ranks of the device time is used.
 --impl reference: the oracle arm (rank 0 only), each step a bounded sample of the workload.
 """
 import argparse
@@ -36,7 +37,7 @@ import workloads as wl  # noqa: E402
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one collide_kernel launch, from the ncu --set full capture summarised in
 # profiles/r1_collide_kernel_ncu_full.md (the algorithmic gather/scatter bytes are ~113x larger: the tiles live in L2)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4_inhom16x24": 10.874876e9}
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4_inhom16x24": 10.880139e9}
 
 METRIC = "collision_samples_per_sec"
 UNIT = "samples/s"
@@ -178,18 +179,36 @@ def run_ours(args, cfg):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    g = bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
-                     species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples, device=dev)
+    def make(nz):
+        return bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=nz, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
+                            species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples, device=dev)
+
     f0 = wl.initial_f(cfg)
-    host_in = torch.from_numpy(f0).pin_memory()
+    slabs = cfg.Nx > 1 and (world > 1 or args.slab)     # --slab: the N > 1 code path on one GPU (halo layers from itself)
+    if slabs:
+        # weak scaling by domain decomposition: the global domain is the config repeated `world` times
+        # along z (nx x ny x nz*world, periodic); every rank owns one copy plus two halo layers and exchanges one
+        # boundary layer with each z neighbour per step (NCCL send/recv), collisions stay local
+        from paper_1912_04457_b200 import slab
+        dom = slab.SlabDomain(make, cfg.nx, cfg.nx, cfg.nx * world, rank, world)
+        g = dom.engine
+        nl = cfg.nx * cfg.nx
+        f_local = np.zeros(((cfg.nx + 2) * nl, cfg.S, cfg.Np))
+        f_local[nl:-nl] = f0
+        host_in = torch.from_numpy(f_local).pin_memory()
+        step_fn = dom.step
+    else:
+        g = make(cfg.nx)
+        host_in = torch.from_numpy(f0).pin_memory()
+        step_fn = g.step
     host_out = torch.empty_like(host_in).pin_memory()
-    mom_host = torch.empty(2 * cfg.S * cfg.Nx + 2 * cfg.S + cfg.Nx, dtype=torch.float64).pin_memory()
+    mom_host = torch.empty(2 * cfg.S * g.Nx + 2 * cfg.S + g.Nx, dtype=torch.float64).pin_memory()
     g.set_f(host_in)
     small = cfg.n_values * 8 * 3 < 256e6                    # footprint below ~2x L2: flush L2 between steps
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev) if small else None
 
     def one_step():
-        g.step(cfg.dt)
+        step_fn(cfg.dt)
         g.moments(mom_host)
 
     def barrier():
@@ -234,7 +253,7 @@ def run_ours(args, cfg):
     g.set_profile(False)
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     clocks = sampler.stop() if sampler else None
-    N1 = float(mom_host[2 * cfg.S * cfg.Nx:2 * cfg.S * cfg.Nx + 2 * cfg.S:2].sum())
+    N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
     # ---- end to end: host f in, host f and moments out, every step
     e2e_steps = args.steps
@@ -243,7 +262,7 @@ def run_ours(args, cfg):
     e0.record()
     for _ in range(e2e_steps):
         g.set_f(host_in)
-        g.step(cfg.dt)
+        step_fn(cfg.dt)
         g.moments(mom_host)
         g.get_f(host_out)
     e1.record()
@@ -274,12 +293,13 @@ def run_ours(args, cfg):
                    "samples_per_cell": cfg.samples, "dt_fm": cfg.dt, "samples_per_step": samples_step,
                    "phase_space_values": cfg.n_values, "step": "bz_step + bz_moments",
                    "l2": "L2 flushed between steps (256 MB write)" if small else "inputs larger than L2 (3 x %.2f GB)" % (cfg.n_values * 8 / 1e9),
-                   "parallelism": "replicas only (1 GPU path)" if world > 1 else "1 GPU"},
+                   "parallelism": ("z slabs, one halo layer exchanged with each neighbour per step (NCCL send/recv), domain = config x %d along z" % world if slabs
+                                   else "independent replicas (homogeneous config: nothing to exchange)" if world > 1 else "1 GPU")},
         "cell_updates_per_sec": world * cfg.n_values * args.steps / (ms * 1e-3),
         "collision_kernel_samples_per_sec": samples_step * coll_n / (coll_ms * 1e-3) if coll_ms > 0 else None,
         "collision_kernel_share_of_step": coll_ms / ms if ms > 0 else None,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": cfg.n_values * 8,
-                "d2h_bytes_per_step": cfg.n_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": host_in.numel() * 8,
+                "d2h_bytes_per_step": host_out.numel() * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches,
         "roofline": {"bound": "hbm", "kernel": "collide_kernel (CUDA events inside libbz.so around every launch)",
                      "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak if ach else None,
@@ -317,6 +337,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slab", action="store_true", help="run the slab-decomposition path (the N > 1 path) even on one GPU")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

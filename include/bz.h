@@ -52,6 +52,25 @@ int bz_set_seed(bz_ctx* ctx, unsigned long long seed);          /* Philox key wo
 int bz_set_samples(bz_ctx* ctx, int samples_per_cell);          /* kinematic samples per (xcell, pcell) (S3), 1..2^24 */
 int bz_set_step(bz_ctx* ctx, unsigned step);                    /* step counter used by bz_step               */
 
+/* Slab of a larger periodic domain (S8e).  The collision term is local in x (Eq. 5); only the drift stencil of
+ * Eq. 13 couples neighbouring spatial cells, through the upwind neighbour one cell away.  A domain split
+ * along z therefore needs ONE exchange step per Euler step: each slab keeps a copy of its two neighbours' boundary
+ * layers ("halo" layers).  After bz_set_slab the context's z layers [z_begin, z_end) are the slab's own cells and the
+ * layers outside are halo copies that the caller refreshes (bz_copy_layers) before every bz_step / bz_stream:
+ *   - bz_collision / bz_step collide only the own cells (dF_coll = 0 elsewhere) and draw the samples of local cell x
+ *     from the Philox spatial counter x + xcell_offset (mod 2^32), i.e. the cell's index in the undecomposed domain;
+ *   - the totals of bz_moments run over the own cells only (per-cell values are written for every layer);
+ *   - bz_stream / the transport part of bz_step treat the context's grid as periodic as always: the values they
+ *     leave in the halo layers are meaningless and are overwritten by the next refresh.
+ * Default: offset 0, all layers own.  Returns -1 unless 0 <= z_begin <= z_end <= nz. */
+int bz_set_slab(bz_ctx* ctx, unsigned xcell_offset, int z_begin, int z_end);
+
+/* Copy n_layers whole z layers (nx*ny*S*Np doubles each, contiguous in the layout above) starting at layer z0
+ * between the context's f and a DEVICE buffer: to_ctx != 0 writes f, to_ctx == 0 reads it.  Asynchronous on the
+ * context's stream.  This is the pack/unpack of the halo exchange (the transfer itself is the caller's: NCCL
+ * send/recv of the buffer through torch.distributed, paper_1912_04457_b200/slab.py). */
+int bz_copy_layers(bz_ctx* ctx, int z0, int n_layers, double* buf_dev, int to_ctx);
+
 /* Copy S*Nx*Np doubles into / out of the context.  on_device != 0: f is a device pointer (async copy on the
  * context's stream); on_device == 0: f is a host pointer and the call synchronises the stream. */
 int bz_set_f(bz_ctx* ctx, const double* f, int on_device);

@@ -51,6 +51,10 @@ struct bzo_ctx {
     int nch;
     bzo_channel ch[MAXCH];
     double msq_override[BZO_N_KINDS];
+    /* slab of a larger periodic domain (S8e): Philox spatial counter = local xcell + xoff; only the z layers
+     * [zb, ze) collide and count in the totals (the others are halo copies of a neighbour's layers) */
+    unsigned xoff;
+    int zb, ze;
 };
 
 /* ------------------------------------------------------------------ species facts */
@@ -398,10 +402,12 @@ int bzo_collision(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
 
     if (Nx > 1 || nt == 1) {
         /* spatial cells are independent (Eq. 5 is local in x): same result for any thread count */
+        /* only the slab's own z layers collide (bzo_set_slab; all layers by default) */
+        const int layer = c->g.nx * c->g.ny, xb = c->zb * layer, xe = c->ze * layer;
 #pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
-        for (int x = 0; x < Nx; ++x) {
+        for (int x = xb; x < xe; ++x) {
             const double* ft = c->f + (size_t)x * tile;
-            collide_tile(c, dt_fm, step, x, ft, bzo_regulator_m2(c, ft), 0, Np, 0, dF + (size_t)x * tile, c->gross + (size_t)x * tile);
+            collide_tile(c, dt_fm, step, (int)((unsigned)x + c->xoff), ft, bzo_regulator_m2(c, ft), 0, Np, 0, dF + (size_t)x * tile, c->gross + (size_t)x * tile);
         }
     } else {
         /* one spatial cell: strips of p1 cells with private sums, merged in strip order (timed run / long cases) */
@@ -411,7 +417,7 @@ int bzo_collision(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
 #pragma omp parallel for schedule(static, 1) num_threads(nt)
         for (int th = 0; th < nt; ++th) {
             const int b = (int)((long long)Np * th / nt), e = (int)((long long)Np * (th + 1) / nt);
-            collide_tile(c, dt_fm, step, 0, c->f, m2, b, e, 0, priv + (size_t)th * 2 * tile, priv + (size_t)th * 2 * tile + tile);
+            collide_tile(c, dt_fm, step, (int)c->xoff, c->f, m2, b, e, 0, priv + (size_t)th * 2 * tile, priv + (size_t)th * 2 * tile + tile);
         }
         for (int th = 0; th < nt; ++th)
             for (size_t q = 0; q < tile; ++q) {
@@ -510,8 +516,11 @@ int bzo_moments(bzo_ctx* c, double* out)
             const double na = Na * sn * d3p / twopi3, ea = Na * se * d3p / twopi3;
             out[((size_t)x * S + a) * 2 + 0] = na;
             out[((size_t)x * S + a) * 2 + 1] = ea;
-            tot[2 * a + 0] += na * d3x;
-            tot[2 * a + 1] += ea * d3x;
+            const int z = x / (c->g.nx * c->g.ny);
+            if (z >= c->zb && z < c->ze) {                       /* halo layers belong to the neighbour's totals */
+                tot[2 * a + 0] += na * d3x;
+                tot[2 * a + 1] += ea * d3x;
+            }
         }
         m2[x] = bzo_regulator_m2(c, c->f + (size_t)x * S * Np);
     }
@@ -525,7 +534,7 @@ int bzo_debug_samples(bzo_ctx* c, unsigned step, int xcell, int pcell_begin, int
     bzo_sample sm;
     size_t o = 0;
     for (int i = pcell_begin; i < pcell_end; ++i) for (int smp = 0; smp < c->Ns; ++smp, ++o) {
-        gen_sample(c, step, xcell, i, smp, &sm);
+        gen_sample(c, step, (int)((unsigned)xcell + c->xoff), i, smp, &sm);
         cells[4 * o + 0] = sm.j; cells[4 * o + 1] = sm.k; cells[4 * o + 2] = sm.l; cells[4 * o + 3] = sm.flag;
         if (stu) { stu[3 * o + 0] = sm.s; stu[3 * o + 1] = sm.t; stu[3 * o + 2] = sm.u; }
     }
@@ -548,6 +557,7 @@ int bzo_create(const bzo_grid* g, const int* species, int n_species, double alph
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->Ns = 64; c->nthreads = 1; c->step = 0;
     c->Nx = g->nx * g->ny * g->nz; c->Np = g->np * g->np * g->np;
     for (int k = 0; k < BZO_N_KINDS; ++k) c->msq_override[k] = -1.0;
+    c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     const size_t total = (size_t)c->S * c->Np * c->Nx;
     c->f = (double*)calloc(total, sizeof(double));
     c->gross = (double*)calloc(total, sizeof(double));
@@ -562,6 +572,12 @@ int bzo_set_samples(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->Ns = n; 
 int bzo_set_threads(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->nthreads = n; return 0; }
 int bzo_get_threads(const bzo_ctx* c) { return c ? c->nthreads : -1; }
 int bzo_set_step(bzo_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
+int bzo_set_slab(bzo_ctx* c, unsigned xcell_offset, int z_begin, int z_end)
+{
+    if (!c || z_begin < 0 || z_end > c->g.nz || z_begin > z_end) return -1;
+    c->xoff = xcell_offset; c->zb = z_begin; c->ze = z_end;
+    return 0;
+}
 int bzo_set_f(bzo_ctx* c, const double* f)
 {
     if (!c || !f) return -1;

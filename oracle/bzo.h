@@ -58,6 +58,12 @@ int  bzo_get_threads(const bzo_ctx*);
 int  bzo_set_f  (bzo_ctx*, const double* f);
 int  bzo_get_f  (const bzo_ctx*, double* f);
 int  bzo_set_step(bzo_ctx*, unsigned step);                    /* internal step counter of bzo_step   */
+/* Slab of a larger periodic domain (S8e: the collision term is local in x, Eq. 5; only the drift stencil of
+ * Eq. 13 couples neighbouring cells).  The context's z layers [z_begin, z_end) are this slab's own cells, the layers
+ * outside are halo copies the caller refreshes before every step.  Only own cells collide and enter the totals of
+ * bzo_moments; the Philox spatial counter of local cell x is x + xcell_offset, so that a cell draws the same
+ * samples as in the undecomposed domain.  Default: offset 0, all layers. */
+int  bzo_set_slab(bzo_ctx*, unsigned xcell_offset, int z_begin, int z_end);
 
 /* dF = dt * C_a[f] (S8c steps 1-6).  Also fills the per-value gross |A| sum (S16), see bzo_get_gross. */
 int  bzo_collision(bzo_ctx*, double dt_fm, unsigned step, double* dF);

@@ -44,6 +44,7 @@ def lib():
         L.bzo_set_threads.argtypes = [vp, C.c_int]
         L.bzo_get_threads.argtypes = [vp]
         L.bzo_set_step.argtypes = [vp, C.c_uint]
+        L.bzo_set_slab.argtypes = [vp, C.c_uint, C.c_int, C.c_int]
         L.bzo_set_f.argtypes = [vp, dp]
         L.bzo_get_f.argtypes = [vp, dp]
         L.bzo_collision.argtypes = [vp, C.c_double, C.c_uint, dp]
@@ -141,6 +142,9 @@ class Oracle:
 
     def set_step(self, step):
         _chk(lib().bzo_set_step(self._h, step), "bzo_set_step")
+
+    def set_slab(self, xcell_offset, z_begin, z_end):
+        _chk(lib().bzo_set_slab(self._h, xcell_offset & 0xFFFFFFFF, z_begin, z_end), "bzo_set_slab")
 
     def set_f(self, f):
         f = np.ascontiguousarray(f, dtype=np.float64).reshape(self.shape)

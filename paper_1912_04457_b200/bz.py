@@ -19,7 +19,8 @@ class Grid(C.Structure):
                 ("np", C.c_int), ("pmin", C.c_double), ("pmax", C.c_double)]
 
 
-EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_f",
+EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
+           "bz_copy_layers", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
@@ -38,6 +39,8 @@ def lib():
         L.bz_set_seed.argtypes = [vp, C.c_ulonglong]
         L.bz_set_samples.argtypes = [vp, C.c_int]
         L.bz_set_step.argtypes = [vp, C.c_uint]
+        L.bz_set_slab.argtypes = [vp, C.c_uint, C.c_int, C.c_int]
+        L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.bz_set_f.argtypes = [vp, vp, C.c_int]
         L.bz_get_f.argtypes = [vp, vp, C.c_int]
         L.bz_collision.argtypes = [vp, C.c_double, C.c_uint, vp]
@@ -122,6 +125,24 @@ class Boltzmann:
 
     def set_step(self, step):
         self._chk(lib().bz_set_step(self._h, step), "bz_set_step")
+
+    def set_slab(self, xcell_offset, z_begin, z_end):
+        self._chk(lib().bz_set_slab(self._h, xcell_offset & 0xFFFFFFFF, z_begin, z_end), "bz_set_slab")
+
+    def layer_values(self):
+        return self.n_values // self._grid.nz
+
+    def get_layers(self, z0, n_layers, out=None):
+        """n_layers z layers of f starting at z0 as a CUDA tensor (asynchronous device copy)."""
+        n = n_layers * self.layer_values()
+        if out is None:
+            out = torch.empty(n, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_copy_layers(self._h, z0, n_layers, self._dev_ptr(out, n), 0), "bz_copy_layers")
+        return out
+
+    def set_layers(self, z0, n_layers, buf):
+        n = n_layers * self.layer_values()
+        self._chk(lib().bz_copy_layers(self._h, z0, n_layers, self._dev_ptr(buf, n), 1), "bz_copy_layers")
 
     # ---- state
     def set_f(self, f):

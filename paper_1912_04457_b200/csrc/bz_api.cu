@@ -67,7 +67,9 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab;
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
     P.work_counter = c->work_counter + c->launch_parity; P.next_counter = c->work_counter + (c->launch_parity ^ 1u);
-    P.n_items = (unsigned)c->Nx * (unsigned)c->regions_per_x; P.x_begin = 0;
+    const int layer = c->grid.nx * c->grid.ny;              // only the slab's own z layers collide (bz_set_slab)
+    P.n_items = (unsigned)((c->ze - c->zb) * layer) * (unsigned)c->regions_per_x; P.x_begin = c->zb * layer;
+    P.x_rng_offset = c->xoff;
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
     const double Vp = (P.g.L * P.g.L) * P.g.L, dtG = dt_fm / kHbarc;
@@ -137,6 +139,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
+    c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
@@ -207,6 +210,30 @@ int bz_set_stream(bz_ctx* c, void* s) { if (!c) return -1; c->stream = (cudaStre
 int bz_set_seed(bz_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
 int bz_set_samples(bz_ctx* c, int n) { if (!c || n < 1 || n > (1 << 24)) return -1; c->Ns = n; return 0; }
 int bz_set_step(bz_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
+
+int bz_set_slab(bz_ctx* c, unsigned xcell_offset, int z_begin, int z_end)
+{
+    if (!c || z_begin < 0 || z_end > c->grid.nz || z_begin > z_end) return -1;
+    c->xoff = xcell_offset; c->zb = z_begin; c->ze = z_end;
+    return 0;
+}
+
+int bz_copy_layers(bz_ctx* c, int z0, int n_layers, double* buf_dev, int to_ctx)
+{
+    if (!c || !buf_dev || z0 < 0 || n_layers < 0 || z0 + n_layers > c->grid.nz) return -1;
+    if (!c->f) return -4;
+    const size_t layer = (size_t)c->grid.nx * c->grid.ny * c->S * c->Np;      // doubles per z layer, contiguous in f
+    double* p = c->f + (size_t)z0 * layer;
+    if (n_layers == 0) return 0;
+    BZ_CUDA(cudaMemcpyAsync(to_ctx ? p : buf_dev, to_ctx ? buf_dev : p, (size_t)n_layers * layer * sizeof(double),
+                            cudaMemcpyDeviceToDevice, c->stream), "bz_copy_layers");
+    if (to_ctx) {
+        // halo layers never collide: the collision kernel's cell-major copy only has to follow the slab's own layers
+        if (z0 < c->ze && z0 + n_layers > c->zb) c->aos_valid = false;
+        c->rowsum_valid = false;
+    }
+    return 0;
+}
 const char* bz_last_error(const bz_ctx* c) { return c ? c->err.c_str() : "null context"; }
 
 int bz_set_f(bz_ctx* c, const double* f, int on_device)
@@ -285,7 +312,8 @@ int bz_moments(bz_ctx* c, double* out_host)
     const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
     const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
     const double d3x = ((c->grid.dx * c->grid.dx) * c->grid.dx) / ((kHbarc * kHbarc) * kHbarc);
-    BZ_CUDA(launch_moments(c->rowsum, c->m2, c->mom, c->Nx, c->S, deg, d3p / twopi3, d3x, c->stream), "moments");
+    BZ_CUDA(launch_moments(c->rowsum, c->m2, c->mom, c->Nx, c->S, deg, d3p / twopi3, d3x,
+                           c->zb * c->grid.nx * c->grid.ny, c->ze * c->grid.nx * c->grid.ny, c->stream), "moments");
     const size_t cnt = (size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx;
     BZ_CUDA(cudaMemcpyAsync(out_host, c->mom, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "moments copy");
     BZ_CUDA(cudaStreamSynchronize(c->stream), "moments sync");

@@ -405,7 +405,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             Sample sa;
             sa.flag = 0; sa.retry = 0;
             if (active)
-                sa = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+                sa = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell + P.x_rng_offset, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
             const unsigned lt = (1u << lane) - 1u;
             const unsigned rb = __ballot_sync(0xffffffffu, sa.retry);
             if (rb) {
@@ -464,7 +464,7 @@ __global__ void debug_samples_kernel(const CollideParams P, int xcell, int p_beg
         Sample sm;
         unsigned kstart = 0u;
         do {                                                 // the generator of the collision kernel, attempts two at a time
-            sm = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell, (uint32_t)i, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+            sm = gen_sample_pair(P.g, P.seed, P.step, (uint32_t)xcell + P.x_rng_offset, (uint32_t)i, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
             kstart += 2u;
         } while (sm.retry);
         cells[4 * q + 0] = sm.j; cells[4 * q + 1] = sm.k; cells[4 * q + 2] = sm.l; cells[4 * q + 3] = sm.flag;

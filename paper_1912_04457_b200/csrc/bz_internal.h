@@ -25,7 +25,8 @@ struct CollideParams {
     unsigned* work_counter;   // device: next work item of the persistent kernel (0 on entry)
     unsigned* next_counter;   // device: the counter of the NEXT launch, zeroed by this one
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
-    int x_begin;              // first spatial cell (0; items address xcell = x_begin + item / regions_per_x)
+    int x_begin;              // first colliding spatial cell (items address xcell = x_begin + item / regions_per_x)
+    uint32_t x_rng_offset;    // Philox spatial counter = xcell + x_rng_offset (slab of a larger domain, bz_set_slab)
     int cells_per_region;     // p1 cells per work item (one producer warp each)
     int regions_per_x;        // ceil(Np / cells_per_region)
     uint32_t seed, step;
@@ -53,6 +54,8 @@ struct bz_ctx_impl {
     unsigned mask;
     double alpha_s, m_D;
     uint32_t seed, step;
+    uint32_t xoff;                   // bz_set_slab: Philox spatial counter offset
+    int zb, ze;                      // bz_set_slab: own z layers [zb, ze); the others are halo copies
     cudaStream_t stream;
     size_t n_values;
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
@@ -97,6 +100,6 @@ cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned 
                       cudaStream_t st);
 // mom = per-cell (n, e), totals, m2
 cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
-                           double d3p_over_2pi3, double d3x, cudaStream_t st);
+                           double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st);
 
 }  // namespace bz

@@ -118,7 +118,7 @@ __global__ void m2_kernel(const double* __restrict__ rowsum, double* __restrict_
 
 // per-cell (n, e), totals over x in a fixed order (one thread per species), then m2 copied behind them
 __global__ void moments_kernel(const double* __restrict__ rowsum, const double* __restrict__ m2, double* __restrict__ mom,
-                               int Nx, int S, double d3p_over_2pi3, double d3x, const double d0, const double d1,
+                               int Nx, int S, double d3p_over_2pi3, double d3x, int x_begin, int x_end, const double d0, const double d1,
                                const double d2, const double d3, const double d4, const double d5, const double d6)
 {
     const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
@@ -133,7 +133,7 @@ __global__ void moments_kernel(const double* __restrict__ rowsum, const double* 
     if (blockIdx.x == 0 && threadIdx.x < 2 * S) {
         const int a = threadIdx.x >> 1, c = threadIdx.x & 1;
         double t = 0.0;
-        for (int x = 0; x < Nx; ++x) t += (deg[a] * rowsum[3 * ((size_t)x * S + a) + c] * d3p_over_2pi3) * d3x;
+        for (int x = x_begin; x < x_end; ++x) t += (deg[a] * rowsum[3 * ((size_t)x * S + a) + c] * d3p_over_2pi3) * d3x;
         mom[2 * rows + threadIdx.x] = t;
     }
 }
@@ -168,11 +168,11 @@ cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned 
 }
 
 cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
-                           double d3p_over_2pi3, double d3x, cudaStream_t st)
+                           double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st)
 {
     int blocks = (Nx * S + 255) / 256;
     if (blocks > 148) blocks = 148;
-    moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, deg[0], deg[1], deg[2], deg[3], deg[4],
+    moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, x_begin, x_end, deg[0], deg[1], deg[2], deg[3], deg[4],
                                            deg[5], deg[6]);
     ++g_launch_count;
     return cudaGetLastError();

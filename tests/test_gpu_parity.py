@@ -258,3 +258,62 @@ def test_edge_cases():
     s.synchronize()
     f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
     assert np.abs(f_g - f_o).max() <= TOL_DF * np.abs(f_o).max()
+
+
+# ---------------------------------------------------------------------------------------------- slabs
+def _slab_kw(cfg, nz):
+    return dict(nx=cfg.nx, ny=cfg.nx, nz=nz, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species,
+                alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
+
+
+@pytest.mark.parametrize("n_slabs", [1, 2, 3])
+def test_slab_decomposition_matches_undecomposed_domain(n_slabs):
+    """bz_set_slab + bz_copy_layers: the domain cut into z slabs with halo layers (several slabs run back to back on
+    this one GPU, halo refresh in process) reproduces the undecomposed oracle: same sampled cells (the Philox spatial
+    counter is the global cell index), f within the NS tolerance, totals within 1e-12."""
+    from paper_1912_04457_b200 import slab
+    cfg = wl.scaled(wl.CONFIGS[3], nx=4, np_=8, samples=16)
+    nl = cfg.nx * cfg.nx
+    o = bzo.Oracle(threads=8, **_slab_kw(cfg, cfg.nx))
+    f0 = wl.random_f(cfg, seed=5)
+    o.set_f(f0)
+    doms = [slab.SlabDomain(lambda nz: bz.Boltzmann(**_slab_kw(cfg, nz)), cfg.nx, cfg.nx, cfg.nx, r, n_slabs)
+            for r in range(n_slabs)]
+    for d in doms:
+        d.set_own(torch.from_numpy(f0[d.z0 * nl:d.z1 * nl].copy()).cuda())
+    # sampled cells of a cell inside the last slab: local index differs from the global one, the samples must not
+    d = doms[-1]
+    xg = cfg.Nx - 2
+    xl = xg - (d.z0 - 1) * nl
+    co, so = o.debug_samples(2, xg, 0, cfg.Np)
+    cg, sg = d.engine.debug_samples(2, xl, 0, cfg.Np)
+    assert np.array_equal(cg.cpu().numpy(), co)
+    assert np.array_equal(sg.cpu().numpy().view(np.uint64), so.view(np.uint64))
+    steps = 3
+    for _ in range(steps):
+        o.step(cfg.dt)
+        slab.exchange_in_process(doms)
+        for d in doms:
+            d.engine.step(cfg.dt)
+    f_o = o.get_f()
+    f_g = np.concatenate([d.get_own().cpu().numpy() for d in doms]).reshape(f_o.shape)
+    assert np.abs(f_g - f_o).max() <= TOL_DF * np.abs(f_o).max()
+    tot = sum(d.engine.moments()["tot"].numpy() for d in doms)
+    assert np.allclose(tot, o.moments()["tot"], rtol=1e-12, atol=0)
+
+
+def test_slab_halo_layers_do_not_collide():
+    """dF_coll is exactly 0 in the halo layers and unchanged in the own layers."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=3, np_=8, samples=8)
+    kw = _slab_kw(cfg, cfg.nx)
+    a, b = bz.Boltzmann(**kw), bz.Boltzmann(**kw)
+    f0 = wl.random_f(cfg, seed=9)
+    a.set_f(f0)
+    b.set_f(f0)
+    b.set_slab(0, 1, 2)
+    dA, dB = a.collision(cfg.dt, 0).cpu().numpy(), b.collision(cfg.dt, 0).cpu().numpy()
+    nl = cfg.nx * cfg.nx
+    assert not dB[:nl].any() and not dB[2 * nl:].any()
+    assert np.abs(dB[nl:2 * nl] - dA[nl:2 * nl]).max() <= 1e-13 * np.abs(dA).max()
+    with pytest.raises(bz.BzError):
+        b.set_slab(0, 2, 1)
