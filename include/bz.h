@@ -52,6 +52,14 @@ int bz_set_seed(bz_ctx* ctx, unsigned long long seed);          /* Philox key wo
 int bz_set_samples(bz_ctx* ctx, int samples_per_cell);          /* kinematic samples per (xcell, pcell) (S3), 1..2^24 */
 int bz_set_step(bz_ctx* ctx, unsigned step);                    /* step counter used by bz_step               */
 
+/* User-defined matrix elements ("We also provide an application programming interface (API) for users to
+ * define their own matrix elements"): replace one kind of Table I by a constant |M|^2 = value (summed
+ * over colours and helicities like Table I, dimensionless), for the straight and the crossed ordering alike.
+ * kind: 0 = q1 q2 -> q1 q2 (different flavours, all four rows), 1 = q1 q1 -> q1 q1, 2 = q1 q1bar -> q1 q1bar,
+ * 3 = q1 q1bar -> q2 q2bar, 4 = q1 q1bar <-> g g, 5 = q g -> q g, 6 = g g -> g g.  value >= 0 overrides, value < 0
+ * restores Table I.  Takes effect at the next bz_collision / bz_step.  -1 on a bad kind or NaN. */
+int bz_set_msq_override(bz_ctx* ctx, int kind, double value);
+
 /* Slab of a larger periodic domain (S8e).  The collision term is local in x (Eq. 5); only the drift stencil of
  * Eq. 13 couples neighbouring spatial cells, through the upwind neighbour one cell away.  A domain split
  * along z therefore needs ONE exchange step per Euler step: each slab keeps a copy of its two neighbours' boundary

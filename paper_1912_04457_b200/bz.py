@@ -20,10 +20,12 @@ class Grid(C.Structure):
 
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
-           "bz_copy_layers", "bz_set_f",
+           "bz_copy_layers", "bz_set_msq_override", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
+
+KINDS = ("A", "11", "1B", "ANN", "QQGG", "QG", "GG")      # kinds of Table I in the order of bz_set_msq_override
 
 
 def lib():
@@ -40,6 +42,7 @@ def lib():
         L.bz_set_samples.argtypes = [vp, C.c_int]
         L.bz_set_step.argtypes = [vp, C.c_uint]
         L.bz_set_slab.argtypes = [vp, C.c_uint, C.c_int, C.c_int]
+        L.bz_set_msq_override.argtypes = [vp, C.c_int, C.c_double]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.bz_set_f.argtypes = [vp, vp, C.c_int]
         L.bz_get_f.argtypes = [vp, vp, C.c_int]
@@ -125,6 +128,11 @@ class Boltzmann:
 
     def set_step(self, step):
         self._chk(lib().bz_set_step(self._h, step), "bz_set_step")
+
+    def set_msq_override(self, kind, value):
+        """kind: 0..6 or one of KINDS; value >= 0 replaces that kind of Table I by a constant, < 0 restores it."""
+        k = KINDS.index(kind) if isinstance(kind, str) else int(kind)
+        self._chk(lib().bz_set_msq_override(self._h, k, float(value)), "bz_set_msq_override")
 
     def set_slab(self, xcell_offset, z_begin, z_end):
         self._chk(lib().bz_set_slab(self._h, xcell_offset & 0xFFFFFFFF, z_begin, z_end), "bz_set_slab")

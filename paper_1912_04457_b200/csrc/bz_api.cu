@@ -78,6 +78,11 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.g4K = (g2 * g2) * K;
     P.mask = c->mask;
     for (int a = 0; a < 7; ++a) P.slot[a] = c->slot[a];
+    P.has_ovr = 0;
+    for (int k = 0; k < 7; ++k) {
+        P.msq_ovr[k] = c->msq_ovr[k] >= 0.0 ? c->msq_ovr[k] / (g2 * g2) : -1.0;
+        if (c->msq_ovr[k] >= 0.0) P.has_ovr = 1;
+    }
     return P;
 }
 
@@ -140,6 +145,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
+    for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
@@ -210,6 +216,13 @@ int bz_set_stream(bz_ctx* c, void* s) { if (!c) return -1; c->stream = (cudaStre
 int bz_set_seed(bz_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
 int bz_set_samples(bz_ctx* c, int n) { if (!c || n < 1 || n > (1 << 24)) return -1; c->Ns = n; return 0; }
 int bz_set_step(bz_ctx* c, unsigned step) { if (!c) return -1; c->step = step; return 0; }
+
+int bz_set_msq_override(bz_ctx* c, int kind, double value)
+{
+    if (!c || kind < 0 || kind > 6 || value != value) return -1;
+    c->msq_ovr[kind] = value;
+    return 0;
+}
 
 int bz_set_slab(bz_ctx* c, unsigned xcell_offset, int z_begin, int z_end)
 {

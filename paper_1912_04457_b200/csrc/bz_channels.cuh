@@ -87,6 +87,23 @@ BZ_HD MsqSet msq_set(double s, double t, double u, double m2, double g4w)
     return M;
 }
 
+// User-defined matrix elements ("an API for users to define their own matrix elements"): a constant per kind
+// of Table I, in the order A, 11, 1B, ANN, QQGG, QG, GG.  ovr[kind] >= 0 replaces that kind (straight and crossed)
+// by ovr[kind] * g4w (the caller passes value / g^4); the differences the channel algebra uses are re-formed.
+BZ_HD void msq_apply_override(MsqSet& M, const double (&ovr)[7], double g4w)
+{
+    if (ovr[0] >= 0.0) M.a_t = M.a_u = ovr[0] * g4w;
+    if (ovr[1] >= 0.0) M.m11 = ovr[1] * g4w;
+    if (ovr[2] >= 0.0) M.m1b_t = M.m1b_u = ovr[2] * g4w;
+    if (ovr[3] >= 0.0) M.ann = ovr[3] * g4w;
+    if (ovr[4] >= 0.0) M.qqgg = ovr[4] * g4w;
+    if (ovr[5] >= 0.0) M.qg_t = M.qg_u = ovr[5] * g4w;
+    if (ovr[6] >= 0.0) M.gg = ovr[6] * g4w;
+    M.d11 = M.m11 - M.a_t;
+    M.d1b_t = M.m1b_t - M.a_t;
+    M.d1b_u = M.m1b_u - M.a_u;
+}
+
 // Deposits of one sample in number units: dI, dJ, dK, dL for the cells of p1, p2, p3, p4 (Eq. 22, P:201:
 // every channel adds -A, -A, +A, +A).  kMask >= 0: compile-time species mask; kMask < 0: use rt_mask.
 template <int kMask>

@@ -262,7 +262,10 @@ __device__ __forceinline__ void consume_batch(Chan<kSP>& ch, const CollideParams
             }
         }
         const double u = __dsub_rn(-s, t);
-        const MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
+        MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
+        // user-defined matrix elements (bz_set_msq_override) run on the runtime-mask instantiation (and the light
+        // pure-glue one), so that the specialised mixture kernels carry no extra registers for them
+        if constexpr (kMask < 0 || kMask == 0x01) { if (P.has_ovr) msq_apply_override(M, P.msq_ovr, g4w); }
         double d[4][7];
         deposit<kMask>(mask, fi, fj, fk, fl, M, d[0], d[1], d[2], d[3]);
         if constexpr (kSP == 1) {
@@ -534,6 +537,7 @@ cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st)
     int ctas = (int)((P.n_items + kProducerWarps - 1) / kProducerWarps);
     if (ctas > sms) ctas = sms;
     if (ctas < 1) ctas = 1;
+    if (P.has_ovr && P.mask != 0x01u) return launch_collide_mask<-1>(P, ctas, st);
     switch (P.mask) {
     case 0x01u: return launch_collide_mask<0x01>(P, ctas, st);
     case 0x7Eu: return launch_collide_mask<0x7E>(P, ctas, st);

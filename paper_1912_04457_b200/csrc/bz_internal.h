@@ -33,6 +33,8 @@ struct CollideParams {
     double g4K;           // (4 pi alpha_s)^2 * K,  K = dtG Vp / (2048 pi^4 Ns)    (S8c step 0)
     unsigned mask;        // bit id set <=> species id active
     int slot[7];          // species id -> index a in the layout (or -1)
+    int has_ovr;          // bz_set_msq_override: some kind of Table I is replaced by a constant
+    double msq_ovr[7];    // per kind: value / g^4, or -1 (Table I)
 };
 
 struct TransportParams {
@@ -56,6 +58,7 @@ struct bz_ctx_impl {
     uint32_t seed, step;
     uint32_t xoff;                   // bz_set_slab: Philox spatial counter offset
     int zb, ze;                      // bz_set_slab: own z layers [zb, ze); the others are halo copies
+    double msq_ovr[7];               // bz_set_msq_override: constant |M|^2 per kind of Table I, < 0 = Table I
     cudaStream_t stream;
     size_t n_values;
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])

@@ -317,3 +317,35 @@ def test_slab_halo_layers_do_not_collide():
     assert np.abs(dB[nl:2 * nl] - dA[nl:2 * nl]).max() <= 1e-13 * np.abs(dA).max()
     with pytest.raises(bz.BzError):
         b.set_slab(0, 2, 1)
+
+
+# ------------------------------------------------------------------------- user-defined matrix elements
+@pytest.mark.parametrize("species,ovr", [
+    ((0, 1, 2), {"QQGG": 1.0, "A": 0.0, "11": 0.0, "1B": 0.0, "ANN": 0.0, "QG": 0.0, "GG": 0.0}),   # the setting of pin P10
+    ((0, 1, 2, 3, 4, 5, 6), {"GG": 40.0, "QG": 7.5, "ANN": 0.0}),                                  # some kinds, rest Table I
+    ((1, 2, 3, 4, 5, 6), {"A": 3.0, "11": 5.0, "1B": 2.0}),
+    ((0,), {"GG": 9.0}),                                                                           # pure-glue kernel
+], ids=["p10", "mixture", "quarks", "glue"])
+def test_msq_override_parity(species, ovr):
+    """bz_set_msq_override: constant |M|^2 per kind of Table I on the GPU against the oracle's override hook (whose
+    normalisation pin P10 checks against the closed form)."""
+    cfg = wl.scaled(wl.CONFIGS[2], np_=9, samples=20)
+    kw = dict(nx=1, ny=1, nz=1, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=species,
+              alpha_s=cfg.alpha_s, m_D=0.7, seed=3, samples=cfg.samples)
+    o, g = bzo.Oracle(threads=8, **kw), bz.Boltzmann(**kw)
+    rng = np.random.Generator(np.random.Philox(key=11))
+    f = 0.02 + 0.5 * rng.random((1, len(species), cfg.Np))
+    o.set_f(f)
+    g.set_f(f)
+    for kind, v in ovr.items():
+        o.set_msq_override(kind, v)
+        g.set_msq_override(kind, v)
+    dF_o = o.collision(cfg.dt, 1)
+    dF_g = g.collision(cfg.dt, 1).cpu().numpy()
+    _assert_dF(dF_g, dF_o, o.gross(), "override")
+    assert np.abs(dF_o).max() > 0
+    # restoring Table I gives the plain result again
+    for kind in ovr:
+        o.set_msq_override(kind, -1.0)
+        g.set_msq_override(kind, -1.0)
+    _assert_dF(g.collision(cfg.dt, 1).cpu().numpy(), o.collision(cfg.dt, 1), o.gross(), "restored")
