@@ -55,6 +55,7 @@ struct bzo_ctx {
      * [zb, ze) collide and count in the totals (the others are halo copies of a neighbour's layers) */
     unsigned xoff;
     int zb, ze;
+    double* mass2;        /* [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 per spatial cell (Eq. 8-9); 0 at start */
 };
 
 /* ------------------------------------------------------------------ species facts */
@@ -474,6 +475,121 @@ int bzo_stream(bzo_ctx* c, double dt_fm, double* dF)
     return 0;
 }
 
+
+/* ------------------------------------------------------------------ NEXT rank 2 (S8f): thermal masses, Eq. 15 */
+/* mass class of a species: 0 = gluon, 1 + flavour for quarks and antiquarks (m_qbar = m_q, Eq. 9) */
+static int mass_class(int id) { return is_gluon(id) ? 0 : 1 + flavour(id); }
+
+/* E_p^a(x) = sqrt(p^2 + m_a^2(x)) at the centre of momentum cell (ix, iy, iz) */
+static double energy_at(const bzo_ctx* c, int ix, int iy, int iz, double m2)
+{
+    const double px = cell_centre(c, ix), py = cell_centre(c, iy), pz = cell_centre(c, iz);
+    return sqrt(((px * px + py * py) + pz * pz) + m2);
+}
+
+int bzo_set_masses(bzo_ctx* c, const double* mass2)
+{
+    if (!c || !mass2) return -1;
+    memcpy(c->mass2, mass2, (size_t)c->Nx * 4 * sizeof(double));
+    return 0;
+}
+int bzo_get_masses(const bzo_ctx* c, double* mass2)
+{
+    if (!c || !mass2) return -1;
+    memcpy(mass2, c->mass2, (size_t)c->Nx * 4 * sizeof(double));
+    return 0;
+}
+
+/* Eq. 8 and Eq. 9 from the current f.  The energies under the integrals are E_p^a =
+ * sqrt(p^2 + m_a^2(x)) with the masses currently STORED (the previous step's; all 0 before the first call, which is
+ * the paper's first-step prescription E_p = |p|).  A cell with E = 0 (p = 0 and m = 0) is skipped (S10).
+ *   I_a   = sum_cells d3p/((2pi)^3 E_p^a) f_a
+ *   m_g^2 = (2 g^2/d_A) (1/2) [N_g C_A I_g + sum_q N_q C_F I_q] = g^2 [6 I_g + sum_q I_q]     (48/8, 8/8)
+ *   m_qi^2 = 2 C_F g^2 (1/2) [2 I_g + I_qi + I_qbar_i] = (4/3) g^2 [2 I_g + I_qi + I_qbar_i]
+ * The new masses replace the stored ones and are copied to out[Nx][4] (if not NULL). */
+int bzo_thermal_masses(bzo_ctx* c, double* out)
+{
+    if (!c) return -1;
+    const double pi = 3.14159265358979323846;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const double g2 = 4.0 * pi * c->alpha_s;
+    const double dp = cell_width(c), d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * pi) * (2.0 * pi) * (2.0 * pi);
+    for (int x = 0; x < c->Nx; ++x) {
+        double I[MAXS] = { 0 };                      /* by species id */
+        for (int a = 0; a < S; ++a) {
+            const int id = c->species[a];
+            const double m2 = c->mass2[4 * (size_t)x + mass_class(id)];
+            const double* fa = c->f + ((size_t)x * S + a) * Np;
+            double sum = 0.0;
+            for (int pc = 0; pc < Np; ++pc) {
+                const double E = energy_at(c, pc % n, (pc / n) % n, pc / (n * n), m2);
+                if (E > 0.0) sum += d3p / (twopi3 * E) * fa[pc];
+            }
+            I[id] = sum;
+        }
+        double quarks = 0.0;
+        for (int id = 1; id < MAXS; ++id) quarks += I[id];
+        double m2new[4];
+        m2new[0] = g2 * (6.0 * I[0] + quarks);
+        for (int fl = 0; fl < 3; ++fl) m2new[1 + fl] = (4.0 / 3.0) * g2 * ((2.0 * I[0] + I[1 + 2 * fl]) + I[2 + 2 * fl]);
+        for (int k = 0; k < 4; ++k) c->mass2[4 * (size_t)x + k] = m2new[k];
+    }
+    if (out) memcpy(out, c->mass2, (size_t)c->Nx * 4 * sizeof(double));
+    return 0;
+}
+
+/* dF = -dt * { drift + force } of Eq. 15, the central-difference form of the left-hand side of Eq. 13 with
+ * E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses; periodic in x AND in p.  Per axis i:
+ *   drift_i = [ p_i f_p(x+) / E_p(x+) - p_i f_p(x-) / E_p(x-) ] / (2 dx)
+ *   force_i = -[ f_{p+}(x) (E_{p+}(x+) - E_{p+}(x-)) / (2 dx) - f_{p-}(x) (E_{p-}(x+) - E_{p-}(x-)) / (2 dx) ] / (2 dp)
+ * x+- = x +- dx e_i, p+- = p +- dp e_i.  dt, dx in fm; p, E in GeV. */
+int bzo_vlasov(bzo_ctx* c, double dt_fm, double* dF)
+{
+    if (!c || !dF) return -1;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const int dims[3] = { c->g.nx, c->g.ny, c->g.nz };
+    const int strides[3] = { 1, c->g.nx, c->g.nx * c->g.ny };
+    const int pstr[3] = { 1, n, n * n };
+    const double dx = c->g.dx, dp = cell_width(c);
+    const int nt = c->nthreads < 1 ? 1 : c->nthreads;
+#pragma omp parallel for schedule(static) num_threads(nt)
+    for (int x = 0; x < c->Nx; ++x) {
+        const int xi[3] = { x % dims[0], (x / dims[0]) % dims[1], x / (dims[0] * dims[1]) };
+        for (int a = 0; a < S; ++a) {
+            const int mc = mass_class(c->species[a]);
+            for (int pc = 0; pc < Np; ++pc) {
+                const int pi3[3] = { pc % n, (pc / n) % n, pc / (n * n) };
+                double acc = 0.0;
+                for (int d = 0; d < 3; ++d) {
+                    const int xm = x + ((xi[d] + dims[d] - 1) % dims[d] - xi[d]) * strides[d];
+                    const int xp = x + ((xi[d] + 1) % dims[d] - xi[d]) * strides[d];
+                    const double m2m = c->mass2[4 * (size_t)xm + mc], m2p = c->mass2[4 * (size_t)xp + mc];
+                    const double pd = cell_centre(c, pi3[d]);
+                    /* drift */
+                    const double fxp = c->f[((size_t)xp * S + a) * Np + pc], fxm = c->f[((size_t)xm * S + a) * Np + pc];
+                    const double Exp = energy_at(c, pi3[0], pi3[1], pi3[2], m2p), Exm = energy_at(c, pi3[0], pi3[1], pi3[2], m2m);
+                    double drift = 0.0;
+                    if (Exp > 0.0) drift += pd * fxp / Exp;          /* p = 0 and m = 0: p_i / E -> 0 (S10) */
+                    if (Exm > 0.0) drift -= pd * fxm / Exm;
+                    drift = drift / (2.0 * dx);
+                    /* force */
+                    int qp[3] = { pi3[0], pi3[1], pi3[2] }, qm[3] = { pi3[0], pi3[1], pi3[2] };
+                    qp[d] = (pi3[d] + 1) % n; qm[d] = (pi3[d] + n - 1) % n;
+                    const int pcp = pc + (qp[d] - pi3[d]) * pstr[d], pcm = pc + (qm[d] - pi3[d]) * pstr[d];
+                    const double fpp = c->f[((size_t)x * S + a) * Np + pcp], fpm = c->f[((size_t)x * S + a) * Np + pcm];
+                    const double Gp = (energy_at(c, qp[0], qp[1], qp[2], m2p) - energy_at(c, qp[0], qp[1], qp[2], m2m)) / (2.0 * dx);
+                    const double Gm = (energy_at(c, qm[0], qm[1], qm[2], m2p) - energy_at(c, qm[0], qm[1], qm[2], m2m)) / (2.0 * dx);
+                    const double force = -(fpp * Gp - fpm * Gm) / (2.0 * dp);
+                    acc += drift + force;
+                }
+                dF[((size_t)x * S + a) * Np + pc] = -dt_fm * acc;
+            }
+        }
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------ S8a.7: forward Euler, unsplit (Eq. 15) */
 int bzo_step(bzo_ctx* c, double dt_fm)
 {
@@ -561,12 +677,13 @@ int bzo_create(const bzo_grid* g, const int* species, int n_species, double alph
     const size_t total = (size_t)c->S * c->Np * c->Nx;
     c->f = (double*)calloc(total, sizeof(double));
     c->gross = (double*)calloc(total, sizeof(double));
-    if (!c->f || !c->gross) { free(c->f); free(c->gross); free(c); return -3; }
+    c->mass2 = (double*)calloc((size_t)c->Nx * 4, sizeof(double));
+    if (!c->f || !c->gross || !c->mass2) { free(c->f); free(c->gross); free(c->mass2); free(c); return -3; }
     build_channels(c);
     *out = c;
     return 0;
 }
-int bzo_destroy(bzo_ctx* c) { if (!c) return -1; free(c->f); free(c->gross); free(c); return 0; }
+int bzo_destroy(bzo_ctx* c) { if (!c) return -1; free(c->f); free(c->gross); free(c->mass2); free(c); return 0; }
 int bzo_set_seed(bzo_ctx* c, unsigned long long seed) { if (!c) return -1; c->seed = (uint32_t)seed; return 0; }
 int bzo_set_samples(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->Ns = n; return 0; }
 int bzo_set_threads(bzo_ctx* c, int n) { if (!c || n < 1) return -1; c->nthreads = n; return 0; }

@@ -70,6 +70,16 @@ int  bzo_collision(bzo_ctx*, double dt_fm, unsigned step, double* dF);
 int  bzo_get_gross(const bzo_ctx*, double* gross);             /* sum|A| / N_a per value, same layout  */
 /* dF = upwind free-streaming increment (S8a.6; flux form of Eq. 13) */
 int  bzo_stream   (bzo_ctx*, double dt_fm, double* dF);
+/* ---- NEXT rank 2 (S8f): the paper's own left-hand side -------------------------------------------------------
+ * Thermal masses^2 per spatial cell, mass2[x][4] = (m_g^2, m_u^2, m_d^2, m_s^2), m_qbar = m_q (Eq. 8-9).
+ * bzo_thermal_masses evaluates Eq. 8-9 on the current f with E_p^a = sqrt(p^2 + m_a^2) from the masses stored so far
+ * (0 at start = the first-step prescription E_p = |p|) and stores the result; out may be NULL. */
+int  bzo_set_masses(bzo_ctx*, const double* mass2);
+int  bzo_get_masses(const bzo_ctx*, double* mass2);
+int  bzo_thermal_masses(bzo_ctx*, double* out);
+/* dF = -dt { drift + force } of Eq. 15: central differences in x and p, periodic in both,
+ * E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses */
+int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 /* f <- (f + dF_stream) + dF_coll, both from the old f (Eq. 15 unsplit); step counter ++ */
 int  bzo_step     (bzo_ctx*, double dt_fm);
 /* out = [N_x][S][2] (n, e) then [S][2] totals (N, E) then m^2[N_x]  (Eq. 10-11; Eq. 8) */

@@ -51,6 +51,10 @@ def lib():
         L.bzo_get_gross.argtypes = [vp, dp]
         L.bzo_stream.argtypes = [vp, C.c_double, dp]
         L.bzo_step.argtypes = [vp, C.c_double]
+        L.bzo_set_masses.argtypes = [vp, dp]
+        L.bzo_get_masses.argtypes = [vp, dp]
+        L.bzo_thermal_masses.argtypes = [vp, dp]
+        L.bzo_vlasov.argtypes = [vp, C.c_double, dp]
         L.bzo_moments.argtypes = [vp, dp]
         L.bzo_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, ip, dp]
         L.bzo_sample_one.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.POINTER(Sample)]
@@ -173,6 +177,26 @@ class Oracle:
 
     def step(self, dt):
         _chk(lib().bzo_step(self._h, dt), "bzo_step")
+
+    # ---- NEXT rank 2: thermal masses (Eq. 8-9) and the central-difference drift + force of Eq. 15
+    def set_masses(self, mass2):
+        m = np.ascontiguousarray(mass2, dtype=np.float64).reshape(self.Nx, 4)
+        _chk(lib().bzo_set_masses(self._h, _dptr(m)), "bzo_set_masses")
+
+    def get_masses(self):
+        m = np.empty((self.Nx, 4), dtype=np.float64)
+        _chk(lib().bzo_get_masses(self._h, _dptr(m)), "bzo_get_masses")
+        return m
+
+    def thermal_masses(self):
+        m = np.empty((self.Nx, 4), dtype=np.float64)
+        _chk(lib().bzo_thermal_masses(self._h, _dptr(m)), "bzo_thermal_masses")
+        return m
+
+    def vlasov(self, dt):
+        dF = np.empty(self.shape, dtype=np.float64)
+        _chk(lib().bzo_vlasov(self._h, dt, _dptr(dF)), "bzo_vlasov")
+        return dF
 
     def moments(self):
         out = np.empty(self.Nx * self.S * 2 + self.S * 2 + self.Nx, dtype=np.float64)
