@@ -97,6 +97,30 @@ int bz_collision(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
  * centre (flux form of the drift term of Eq. 13; S8a.6).  Asynchronous. */
 int bz_stream(bz_ctx* ctx, double dt_fm, double* dF_dev);
 
+/* ---- NEXT rank 2 of SURVEY.md 8f: the paper's own left-hand side (massive dispersion, drift AND force) ----------
+ * Thermal masses^2 per spatial cell, mass2[x][4] = (m_g^2, m_u^2, m_d^2, m_s^2) in GeV^2, m_qbar = m_q, 0 at start.
+ * bz_thermal_masses evaluates Eq. 8 and Eq. 9 on the current f,
+ *     m_g^2 = g^2 [6 I_g + sum_q I_q],  m_qi^2 = (4/3) g^2 [2 I_g + I_qi + I_qbar_i],  I_a = sum_cells d3p f_a / ((2pi)^3 E_p^a),
+ * with E_p^a = sqrt(p^2 + m_a^2(x)) from the masses stored so far (all 0 before the first call: the first-step
+ * prescription E_p = |p| of P:107; a cell with E = 0 is skipped), stores the result in the context and, if
+ * out_host != NULL, copies the Nx*4 doubles to the host (then it synchronises).  bz_set_masses sets them directly
+ * from HOST memory (e.g. the constant m_g^2 = 0.5 GeV^2 of Fig. 5); synchronises. */
+int bz_thermal_masses(bz_ctx* ctx, double* out_host);
+int bz_set_masses(bz_ctx* ctx, const double* mass2_host);
+
+/* dF = -dt { drift + force } of Eq. 15, the central-difference form of the left-hand side of Eq. 13
+ * (P:133), with E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses; periodic in x and in p.  Per axis i:
+ *   drift_i = [ p_i f_p(x+)/E_p(x+) - p_i f_p(x-)/E_p(x-) ] / (2 dx)
+ *   force_i = -[ f_{p+}(x) (E_{p+}(x+) - E_{p+}(x-))/(2 dx) - f_{p-}(x) (E_{p-}(x+) - E_{p-}(x-))/(2 dx) ] / (2 dp)
+ * dF_dev: device pointer, S*Nx*Np doubles, overwritten.  Asynchronous. */
+int bz_vlasov(bz_ctx* ctx, double dt_fm, double* dF_dev);
+
+/* Transport scheme used by bz_step: 0 (default, NS) = first-order upwind drift with massless velocities (bz_stream);
+ * 1 = Eq. 15 (bz_vlasov) with the thermal masses re-evaluated from the old f at the start of every step;
+ * 2 = Eq. 15 with the masses as stored (bz_set_masses / the last bz_thermal_masses).  The collision term is NS's
+ * massless one in every scheme (the massive collision kinematics of the paper are NEXT rank 1, not built). */
+int bz_set_transport(bz_ctx* ctx, int scheme);
+
 /* One forward-Euler step (Eq. 15 unsplit; S8a.7): f <- (f + dF_stream) + dF_coll with both increments
  * from the old f and the context's step counter as the Philox step; the counter is then incremented.
  * Asynchronous. */

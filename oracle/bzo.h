@@ -80,6 +80,9 @@ int  bzo_thermal_masses(bzo_ctx*, double* out);
 /* dF = -dt { drift + force } of Eq. 15: central differences in x and p, periodic in both,
  * E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses */
 int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
+/* transport used by bzo_step: 0 = upwind massless (default), 1 = Eq. 15 with the masses re-evaluated from the old f
+ * every step, 2 = Eq. 15 with the masses as stored */
+int  bzo_set_transport(bzo_ctx*, int scheme);
 /* f <- (f + dF_stream) + dF_coll, both from the old f (Eq. 15 unsplit); step counter ++ */
 int  bzo_step     (bzo_ctx*, double dt_fm);
 /* out = [N_x][S][2] (n, e) then [S][2] totals (N, E) then m^2[N_x]  (Eq. 10-11; Eq. 8) */

@@ -55,6 +55,7 @@ def lib():
         L.bzo_get_masses.argtypes = [vp, dp]
         L.bzo_thermal_masses.argtypes = [vp, dp]
         L.bzo_vlasov.argtypes = [vp, C.c_double, dp]
+        L.bzo_set_transport.argtypes = [vp, C.c_int]
         L.bzo_moments.argtypes = [vp, dp]
         L.bzo_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, ip, dp]
         L.bzo_sample_one.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.POINTER(Sample)]
@@ -192,6 +193,9 @@ class Oracle:
         m = np.empty((self.Nx, 4), dtype=np.float64)
         _chk(lib().bzo_thermal_masses(self._h, _dptr(m)), "bzo_thermal_masses")
         return m
+
+    def set_transport(self, scheme):
+        _chk(lib().bzo_set_transport(self._h, scheme), "bzo_set_transport")
 
     def vlasov(self, dt):
         dF = np.empty(self.shape, dtype=np.float64)

@@ -20,7 +20,8 @@ class Grid(C.Structure):
 
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
-           "bz_copy_layers", "bz_set_msq_override", "bz_set_f",
+           "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
+           "bz_set_transport", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
@@ -43,6 +44,10 @@ def lib():
         L.bz_set_step.argtypes = [vp, C.c_uint]
         L.bz_set_slab.argtypes = [vp, C.c_uint, C.c_int, C.c_int]
         L.bz_set_msq_override.argtypes = [vp, C.c_int, C.c_double]
+        L.bz_thermal_masses.argtypes = [vp, vp]
+        L.bz_set_masses.argtypes = [vp, vp]
+        L.bz_vlasov.argtypes = [vp, C.c_double, vp]
+        L.bz_set_transport.argtypes = [vp, C.c_int]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.bz_set_f.argtypes = [vp, vp, C.c_int]
         L.bz_get_f.argtypes = [vp, vp, C.c_int]
@@ -187,6 +192,27 @@ class Boltzmann:
             out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
         self._chk(lib().bz_stream(self._h, dt, self._dev_ptr(out, self.n_values)), "bz_stream")
         return out
+
+    # ---- NEXT rank 2: thermal masses (Eq. 8-9) and the central-difference drift + force of Eq. 15
+    def thermal_masses(self):
+        out = torch.empty((self.Nx, 4), dtype=torch.float64)
+        self._chk(lib().bz_thermal_masses(self._h, C.c_void_p(out.data_ptr())), "bz_thermal_masses")
+        return out
+
+    def set_masses(self, mass2):
+        t = torch.as_tensor(mass2, dtype=torch.float64).contiguous()
+        if t.numel() != self.Nx * 4 or t.is_cuda:
+            raise ValueError("mass2: host array of Nx*4 doubles")
+        self._chk(lib().bz_set_masses(self._h, C.c_void_p(t.data_ptr())), "bz_set_masses")
+
+    def vlasov(self, dt, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_vlasov(self._h, dt, self._dev_ptr(out, self.n_values)), "bz_vlasov")
+        return out
+
+    def set_transport(self, scheme):
+        self._chk(lib().bz_set_transport(self._h, scheme), "bz_set_transport")
 
     def step(self, dt):
         self._chk(lib().bz_step(self._h, dt), "bz_step")

@@ -120,6 +120,28 @@ int update_m2(bz_ctx* c)
     return 0;
 }
 
+// species layout index -> mass class (0 = g, 1 + flavour) and species id, 3 bits each
+void class_bits(const bz_ctx* c, unsigned& cls, unsigned& ids)
+{
+    cls = 0; ids = 0;
+    for (int a = 0; a < c->S; ++a) {
+        const int id = c->species[a];
+        cls |= (unsigned)(id == 0 ? 0 : 1 + (id - 1) / 2) << (3 * a);
+        ids |= (unsigned)id << (3 * a);
+    }
+}
+
+int run_thermal_masses(bz_ctx* c)
+{
+    unsigned cls, ids;
+    class_bits(c, cls, ids);
+    const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
+    BZ_CUDA(launch_thermal_masses(c->f, c->cell_tab, c->mass2, c->Nx, c->S, c->Np, cls, ids, 4.0 * kPi * c->alpha_s,
+                                  d3p / twopi3, c->stream), "thermal masses");
+    return 0;
+}
+
 }  // namespace
 
 extern "C" {
@@ -146,6 +168,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
+    c->mass2 = nullptr; c->E_tab = nullptr; c->scheme = 0;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
@@ -172,6 +195,8 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     BZ_CUDA(cudaMalloc(&c->f_aos, aos_bytes), "cudaMalloc f_aos");
     BZ_CUDA(cudaMalloc(&c->dN_aos, aos_bytes), "cudaMalloc dN_aos");
     BZ_CUDA(cudaMalloc(&c->m2, c->Nx * sizeof(double)), "cudaMalloc m2");
+    BZ_CUDA(cudaMalloc(&c->mass2, (size_t)c->Nx * 4 * sizeof(double)), "cudaMalloc mass2");
+    BZ_CUDA(cudaMemset(c->mass2, 0, (size_t)c->Nx * 4 * sizeof(double)), "memset mass2");
     BZ_CUDA(cudaMalloc(&c->rowsum, (size_t)c->Nx * c->S * 3 * sizeof(double)), "cudaMalloc rowsum");
     BZ_CUDA(cudaMalloc(&c->mom, ((size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx) * sizeof(double)), "cudaMalloc mom");
     BZ_CUDA(cudaMalloc(&c->absp, 5 * (size_t)c->Np * sizeof(double)), "cudaMalloc tables");
@@ -206,7 +231,7 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete c;
     return 0;
@@ -300,14 +325,60 @@ int bz_stream(bz_ctx* c, double dt_fm, double* dF_dev)
     return 0;
 }
 
+static int run_vlasov(bz_ctx* c, double dt_fm, double* out)
+{
+    unsigned cls, ids;
+    class_bits(c, cls, ids);
+    const double dp = (c->grid.pmax - c->grid.pmin) / c->grid.np;
+    if (!c->E_tab) BZ_CUDA(cudaMalloc(&c->E_tab, (size_t)c->Nx * 4 * c->Np * sizeof(double)), "cudaMalloc E_tab");
+    BZ_CUDA(launch_vlasov(c->f, out, c->grid.nx, c->grid.ny, c->grid.nz, c->S, c->Np, c->cell_tab, c->mass2, c->E_tab,
+                          c->grid.np, dt_fm, c->grid.dx, dp, cls, c->stream), "vlasov");
+    return 0;
+}
+
+int bz_set_transport(bz_ctx* c, int scheme) { if (!c || scheme < 0 || scheme > 2) return -1; c->scheme = scheme; return 0; }
+
+int bz_set_masses(bz_ctx* c, const double* mass2_host)
+{
+    if (!c || !mass2_host) return -1;
+    if (!c->mass2) return -4;
+    BZ_CUDA(cudaMemcpyAsync(c->mass2, mass2_host, (size_t)c->Nx * 4 * sizeof(double), cudaMemcpyHostToDevice, c->stream), "set masses");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "set masses sync");
+    return 0;
+}
+
+int bz_thermal_masses(bz_ctx* c, double* out_host)
+{
+    if (!c) return -1;
+    if (!c->f) return -4;
+    if (int rc = run_thermal_masses(c)) return rc;
+    if (out_host) {
+        BZ_CUDA(cudaMemcpyAsync(out_host, c->mass2, (size_t)c->Nx * 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "masses copy");
+        BZ_CUDA(cudaStreamSynchronize(c->stream), "masses sync");
+    }
+    return 0;
+}
+
+int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
+{
+    if (!c || !dF_dev) return -1;
+    if (!c->f) return -4;
+    return run_vlasov(c, dt_fm, dF_dev);
+}
+
 int bz_step(bz_ctx* c, double dt_fm)
 {
     if (!c) return -1;
     if (!c->f) return -4;
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, c->step)) return rc;
+    if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f
     if (int rc = prof_mark(c, 1)) return rc;
-    BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 1, c->stream), "stream+euler");
+    if (c->scheme == 0) BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 1, c->stream), "stream+euler");
+    else {
+        if (int rc = run_vlasov(c, dt_fm, c->f_new)) return rc;
+        BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 2, c->stream), "euler");
+    }
     if (int rc = prof_mark(c, 1)) return rc;
     double* t = c->f; c->f = c->f_new; c->f_new = t;
     c->rowsum_valid = false;          // f changed; f_aos was rewritten with the new f by the Euler kernel

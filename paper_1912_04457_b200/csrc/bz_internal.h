@@ -59,6 +59,9 @@ struct bz_ctx_impl {
     uint32_t xoff;                   // bz_set_slab: Philox spatial counter offset
     int zb, ze;                      // bz_set_slab: own z layers [zb, ze); the others are halo copies
     double msq_ovr[7];               // bz_set_msq_override: constant |M|^2 per kind of Table I, < 0 = Table I
+    double* mass2;                   // device [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 (Eq. 8-9); 0 at start
+    double* E_tab;                   // device [Nx][4][Np] energies sqrt(p^2 + m^2), allocated at the first bz_vlasov / scheme >= 1 step
+    int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
@@ -93,7 +96,8 @@ cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin,
                                  cudaStream_t st);
 // dF = dN_aos / N_a (transposed to the API layout), dN_aos = 0
 cudaError_t launch_finalize(double* dN_aos, double* dF, int Nx, int S, int SP, int Np, const double* deg, cudaStream_t st);
-// mode 0: out = dF_stream;  mode 1: out = (f + dF_stream) + dN/N_a and dN = 0
+// mode 0: out = dF_stream;  mode 1: out = (f + dF_stream) + dN/N_a and dN = 0;
+// mode 2: out = (f + out) + dN/N_a and dN = 0 (out holds a transport increment computed elsewhere: bz_vlasov.cu)
 cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st);
 // rowsum[x][a][0..2]
 cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_invE, double* rowsum, int rows, int Np,
@@ -104,5 +108,12 @@ cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned 
 // mom = per-cell (n, e), totals, m2
 cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
                            double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st);
+
+// NEXT rank 2 (bz_vlasov.cu): thermal masses of Eq. 8-9 and the central-difference drift + force of Eq. 15
+cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, double* mass2, int Nx, int S, int Np,
+                                  unsigned cls_bits, unsigned id_bits, double g2, double w, cudaStream_t st);
+cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
+                          const double* mass2, double* E_tab, int n, double dt, double dx, double dp, unsigned cls_bits,
+                          cudaStream_t st);
 
 }  // namespace bz

@@ -59,10 +59,14 @@ __global__ void __launch_bounds__(256, BZ_TR_MINB) transport_kernel(const Transp
                 if (a < P.S) {
                     const size_t idx = (size_t)xcell * row + (size_t)a * P.Np + pc;
                     const double f0 = P.f[idx];
-                    double acc = ax * (f0 - P.f[idx + ox]);
-                    acc += ay * (f0 - P.f[idx + oy]);
-                    acc += az * (f0 - P.f[idx + oz]);
-                    fn[a] = (f0 - acc) + d[a] / P.inv_deg[a];
+                    if (kMode == 2) {
+                        fn[a] = (f0 + P.out[idx]) + d[a] / P.inv_deg[a];      // the increment of Eq. 15 is already in out
+                    } else {
+                        double acc = ax * (f0 - P.f[idx + ox]);
+                        acc += ay * (f0 - P.f[idx + oy]);
+                        acc += az * (f0 - P.f[idx + oz]);
+                        fn[a] = (f0 - acc) + d[a] / P.inv_deg[a];
+                    }
                     P.out[idx] = fn[a];
                 }
             }
@@ -146,7 +150,8 @@ cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st
     if (chunks > 65535) chunks = 65535;
     dim3 grid(P.nx * P.ny * P.nz, chunks);
     if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
-    else transport_kernel<1><<<grid, 256, 0, st>>>(P);
+    else if (mode == 1) transport_kernel<1><<<grid, 256, 0, st>>>(P);
+    else transport_kernel<2><<<grid, 256, 0, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }

@@ -1,0 +1,154 @@
+// bz_vlasov.cu -- NEXT rank 2 of SURVEY.md 8f: the paper's own left-hand side.
+//   mass_kernel    thermal masses^2 per spatial cell, Eq. 8-9, with E_p^a = sqrt(p^2 + m_a^2) from the
+//                  masses of the previous evaluation (0 at start = the first-step prescription E_p = |p|)
+//   vlasov_kernel  dF = -dt { drift + force } of Eq. 15: central differences in x and in p, periodic in both
+//                  (P:139).  In bz_step the increment lands in f_new and transport_kernel<2> adds f and the collision
+//                  deposits (forward Euler, Eq. 15 solved for f(t + dt)).
+//   energy_kernel  E_p^a(x) table for the mass classes present (one square root per entry instead of 18 per value).
+#include "bz_internal.h"
+
+namespace bz {
+
+namespace {
+
+// species layout index a -> mass class (0 = g, 1 + flavour for q and qbar) is passed as 3 bits per slot in cls_bits
+__device__ __forceinline__ int class_of(unsigned cls_bits, int a) { return (int)((cls_bits >> (3 * a)) & 7u); }
+
+__global__ void __launch_bounds__(256) mass_kernel(const double* __restrict__ f, const double* __restrict__ cell_tab,
+                                                   double* __restrict__ mass2, int S, int Np, unsigned cls_bits,
+                                                   unsigned id_bits, double g2, double w /* d3p / (2 pi)^3 */)
+{
+    const int x = blockIdx.x;
+    __shared__ double m_old[4];
+    __shared__ double part[7][8];
+    if (threadIdx.x < 4) m_old[threadIdx.x] = mass2[4 * (size_t)x + threadIdx.x];
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int a = 0; a < S; ++a) {
+        const double m2 = m_old[class_of(cls_bits, a)];
+        const double* fa = f + ((size_t)x * S + a) * Np;
+        double sum = 0.0;
+        for (int pc = threadIdx.x; pc < Np; pc += blockDim.x) {
+            const double2 u = __ldg(reinterpret_cast<const double2*>(cell_tab) + 2 * (size_t)pc);
+            const double pz = __ldg(cell_tab + 4 * (size_t)pc + 2);
+            const double E = sqrt(((u.x * u.x + u.y * u.y) + pz * pz) + m2);
+            if (E > 0.0) sum += w / E * fa[pc];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0) part[a][warp] = sum;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double I[7] = { 0, 0, 0, 0, 0, 0, 0 };                 // by species id
+        for (int a = 0; a < S; ++a) {
+            double t = 0.0;
+            for (int q = 0; q < 8; ++q) t += part[a][q];
+            I[(id_bits >> (3 * a)) & 7u] = t;
+        }
+        double quarks = 0.0;
+        for (int id = 1; id < 7; ++id) quarks += I[id];
+        mass2[4 * (size_t)x + 0] = g2 * (6.0 * I[0] + quarks);                                   // Eq. 8
+        for (int fl = 0; fl < 3; ++fl)
+            mass2[4 * (size_t)x + 1 + fl] = (4.0 / 3.0) * g2 * ((2.0 * I[0] + I[1 + 2 * fl]) + I[2 + 2 * fl]);   // Eq. 9
+    }
+}
+
+// E_tab[(x*4 + cls)*Np + pc] = sqrt(p^2 + m_cls^2(x)) for the mass classes present: one square root per entry, so
+// that the stencil kernel below reads its 18 energies per (cell, class) instead of recomputing them
+__global__ void __launch_bounds__(256) energy_kernel(const double* __restrict__ cell_tab, const double* __restrict__ mass2,
+                                                     double* __restrict__ E_tab, int Np, unsigned cls_present)
+{
+    const int x = blockIdx.x;
+    for (int pc = blockIdx.y * blockDim.x + threadIdx.x; pc < Np; pc += gridDim.y * blockDim.x) {
+        const double a = __ldg(cell_tab + 4 * (size_t)pc), b = __ldg(cell_tab + 4 * (size_t)pc + 1), c = __ldg(cell_tab + 4 * (size_t)pc + 2);
+        const double p2 = (a * a + b * b) + c * c;
+#pragma unroll
+        for (int cls = 0; cls < 4; ++cls)
+            if ((cls_present >> cls) & 1u) E_tab[((size_t)x * 4 + cls) * Np + pc] = sqrt(p2 + __ldg(mass2 + 4 * (size_t)x + cls));
+    }
+}
+
+struct VlasovParams {
+    const double* f;              // [Nx][S][Np]
+    double* out;                  // dF, same layout
+    const double* cell_tab;       // [Np][4] px, py, pz, |p|
+    const double* E_tab;          // [Nx][4][Np] energies of the mass classes present (energy_kernel)
+    int nx, ny, nz, S, Np, n;     // n = momentum cells per axis
+    double dt, inv_2dx, inv_2dp;
+    unsigned cls_bits;
+};
+
+// One thread per phase-space value (x, a, pc): 12 f reads + 18 energy reads + 3 table reads, all independent, ~40
+// registers -> full occupancy; the latency of the scattered neighbour reads is hidden by warps, not by unrolling.
+// blockIdx.x = spatial cell (fastest): the blocks in flight share one (species, 256-cell momentum chunk) slice of all
+// spatial cells (Nx x 2 KB of f and of E), so the six spatial neighbours are L2 hits.
+__global__ void __launch_bounds__(256) vlasov_kernel(const VlasovParams V)
+{
+    const int xcell = blockIdx.x, a = blockIdx.z;
+    const int pc = blockIdx.y * blockDim.x + threadIdx.x;
+    if (pc >= V.Np) return;
+    const int ix = xcell % V.nx, iy = (xcell / V.nx) % V.ny, iz = xcell / (V.nx * V.ny);
+    int xo[3][2];                                            // spatial neighbours (periodic): cell index offsets
+    xo[0][0] = (ix + V.nx - 1) % V.nx - ix;                  xo[0][1] = (ix + 1) % V.nx - ix;
+    xo[1][0] = ((iy + V.ny - 1) % V.ny - iy) * V.nx;         xo[1][1] = ((iy + 1) % V.ny - iy) * V.nx;
+    xo[2][0] = ((iz + V.nz - 1) % V.nz - iz) * V.nx * V.ny;  xo[2][1] = ((iz + 1) % V.nz - iz) * V.nx * V.ny;
+    const int n = V.n;
+    const int pi3[3] = { pc % n, (pc / n) % n, pc / (n * n) };
+    const int pstr[3] = { 1, n, n * n };
+    const int cls = class_of(V.cls_bits, a);
+    const size_t row = (size_t)V.S * V.Np;
+    const double* fx = V.f + (size_t)xcell * row + (size_t)a * V.Np + pc;
+    const double* Ex = V.E_tab + ((size_t)xcell * 4 + cls) * V.Np + pc;
+    double acc = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int pom = ((pi3[d] + n - 1) % n - pi3[d]) * pstr[d];       // momentum neighbours, periodic in p
+        const int pop = ((pi3[d] + 1) % n - pi3[d]) * pstr[d];
+        const double pd = __ldg(V.cell_tab + 4 * (size_t)pc + d);
+        const double* Em = Ex + (ptrdiff_t)xo[d][0] * 4 * V.Np;          // energies at x - dx e_d
+        const double* Ep = Ex + (ptrdiff_t)xo[d][1] * 4 * V.Np;          // energies at x + dx e_d
+        const double Exp = __ldg(Ep), Exm = __ldg(Em);
+        const double cp = Exp > 0.0 ? pd / Exp : 0.0, cm = Exm > 0.0 ? pd / Exm : 0.0;   // p = 0 and m = 0: S10
+        const double Gp = (__ldg(Ep + pop) - __ldg(Em + pop)) * V.inv_2dx;               // dE/dx at p + dp e_d
+        const double Gm = (__ldg(Ep + pom) - __ldg(Em + pom)) * V.inv_2dx;               // dE/dx at p - dp e_d
+        const double fxm = __ldg(fx + (ptrdiff_t)xo[d][0] * (ptrdiff_t)row), fxp = __ldg(fx + (ptrdiff_t)xo[d][1] * (ptrdiff_t)row);
+        const double fpm = __ldg(fx + pom), fpp = __ldg(fx + pop);
+        const double drift = (cp * fxp - cm * fxm) * V.inv_2dx;
+        const double force = -(fpp * Gp - fpm * Gm) * V.inv_2dp;
+        acc += drift + force;
+    }
+    V.out[(size_t)xcell * row + (size_t)a * V.Np + pc] = -V.dt * acc;
+}
+
+}  // namespace
+
+cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, double* mass2, int Nx, int S, int Np,
+                                  unsigned cls_bits, unsigned id_bits, double g2, double w, cudaStream_t st)
+{
+    mass_kernel<<<Nx, 256, 0, st>>>(f, cell_tab, mass2, S, Np, cls_bits, id_bits, g2, w);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
+                          const double* mass2, double* E_tab, int n, double dt, double dx, double dp, unsigned cls_bits,
+                          cudaStream_t st)
+{
+    unsigned present = 0;
+    for (int a = 0; a < S; ++a) present |= 1u << ((cls_bits >> (3 * a)) & 7u);
+    int chunks = (Np + 255) / 256;
+    if (chunks > 65535) return cudaErrorInvalidValue;
+    energy_kernel<<<dim3(nx * ny * nz, chunks), 256, 0, st>>>(cell_tab, mass2, E_tab, Np, present);
+    ++g_launch_count;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    VlasovParams V;
+    V.f = f; V.out = out; V.cell_tab = cell_tab; V.E_tab = E_tab; V.nx = nx; V.ny = ny; V.nz = nz; V.S = S; V.Np = Np; V.n = n;
+    V.dt = dt; V.inv_2dx = 1.0 / (2.0 * dx); V.inv_2dp = 1.0 / (2.0 * dp); V.cls_bits = cls_bits;
+    vlasov_kernel<<<dim3(nx * ny * nz, chunks, S), 256, 0, st>>>(V);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+}  // namespace bz

@@ -349,3 +349,67 @@ def test_msq_override_parity(species, ovr):
         o.set_msq_override(kind, -1.0)
         g.set_msq_override(kind, -1.0)
     _assert_dF(g.collision(cfg.dt, 1).cpu().numpy(), o.collision(cfg.dt, 1), o.gross(), "restored")
+
+
+# ------------------------------------------------- NEXT rank 2: thermal masses (Eq. 8-9) and Eq. 15 (drift + force)
+VLASOV_CASES = [
+    wl.scaled(wl.CONFIGS[3], nx=3, np_=10, samples=8),                 # 7 species, 27 spatial cells
+    wl.scaled(wl.CONFIGS[4], nx=4, np_=7, samples=4),                  # odd momentum grid: the p = 0 cell
+    wl.scaled(wl.CONFIGS[1], np_=6, samples=4),                        # quarks only, one spatial cell (own neighbour)
+]
+
+
+@pytest.mark.parametrize("cfg", VLASOV_CASES, ids=lambda c: c.name)
+def test_thermal_masses_and_vlasov_parity(cfg):
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=21)
+    o.set_f(f0)
+    g.set_f(f0)
+    # first evaluation: E = |p|; second: massive energies of the first
+    for _ in range(3):
+        mo, mg = o.thermal_masses(), g.thermal_masses().numpy()
+        assert np.allclose(mg, mo, rtol=1e-12, atol=0)
+    assert (mo[:, 0] > 0).all()
+    # Eq. 15 with spatially varying masses
+    rng = np.random.Generator(np.random.Philox(key=5))
+    masses = 0.05 + rng.random((cfg.Nx, 4))
+    if cfg.np_ % 2 == 1:
+        masses[::3] = 0.0                                           # m = 0 cells: E = 0 at p = 0 (S10)
+    o.set_masses(masses)
+    g.set_masses(masses)
+    dF_o, dF_g = o.vlasov(cfg.dt), g.vlasov(cfg.dt).cpu().numpy()
+    if cfg.Nx == 1:
+        assert not dF_o.any() and np.abs(dF_g).max() <= 1e-15        # homogeneous: a cell is its own neighbour
+        return
+    assert np.abs(dF_o).max() > 0
+    assert np.abs(dF_g - dF_o).max() <= 1e-13 * np.abs(dF_o).max()
+    for a in range(cfg.S):                                           # Eq. 13: nothing is created
+        assert abs(dF_g[:, a].sum()) <= 1e-12 * np.abs(dF_g[:, a]).sum()
+
+
+@pytest.mark.parametrize("scheme", [1, 2])
+def test_step_with_eq15_transport(scheme):
+    cfg = wl.scaled(wl.CONFIGS[3], nx=3, np_=8, samples=16)
+    o, g = _pair(cfg)
+    f0 = wl.initial_f(cfg) + 0.01
+    for e in (o, g):
+        e.set_f(f0)
+        e.set_transport(scheme)
+        if scheme == 2:
+            e.set_masses(np.full((cfg.Nx, 4), 0.5))                  # constant m^2 = 0.5 GeV^2 as in Fig. 5
+    for _ in range(4):
+        o.step(cfg.dt)
+        g.step(cfg.dt)
+    f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
+    assert np.abs(f_g - f_o).max() <= 1e-11 * np.abs(f_o).max()
+    mo, mg = o.moments(), g.moments()
+    assert np.allclose(mg["tot"].numpy(), mo["tot"], rtol=1e-12, atol=0)
+    if scheme == 1:
+        assert np.allclose(g.thermal_masses().numpy(), o.thermal_masses(), rtol=1e-11, atol=0)
+    # total particle number: conserved by the collision term (Eq. 22) and by Eq. 13's flux form
+    N0 = None
+    o2 = bzo.Oracle(threads=1, nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
+                    species=cfg.species)
+    o2.set_f(f0)
+    N0 = o2.moments()["tot"][:, 0].sum()
+    assert mg["tot"][:, 0].sum().item() == pytest.approx(N0, rel=1e-12)
