@@ -168,7 +168,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
-    c->mass2 = nullptr; c->E_tab = nullptr; c->scheme = 0;
+    c->mass2 = nullptr; c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
@@ -231,7 +231,7 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     delete c;
     return 0;
@@ -330,9 +330,32 @@ static int run_vlasov(bz_ctx* c, double dt_fm, double* out)
     unsigned cls, ids;
     class_bits(c, cls, ids);
     const double dp = (c->grid.pmax - c->grid.pmin) / c->grid.np;
-    if (!c->E_tab) BZ_CUDA(cudaMalloc(&c->E_tab, (size_t)c->Nx * 4 * c->Np * sizeof(double)), "cudaMalloc E_tab");
+    if (!c->E_tab) {
+        // first use: the energy table and the two periodic-wrap tables of the stencil (index bookkeeping only)
+        BZ_CUDA(cudaMalloc(&c->E_tab, (size_t)c->Nx * 4 * c->Np * sizeof(double)), "cudaMalloc E_tab");
+        BZ_CUDA(cudaMalloc(&c->x_nb, (size_t)c->Nx * 6 * sizeof(int)), "cudaMalloc x_nb");
+        BZ_CUDA(cudaMalloc(&c->p_wrap, (size_t)c->Np), "cudaMalloc p_wrap");
+        const int nx = c->grid.nx, ny = c->grid.ny, nz = c->grid.nz, n = c->grid.np;
+        std::vector<int> nb((size_t)c->Nx * 6);
+        for (int x = 0; x < c->Nx; ++x) {
+            const int ix = x % nx, iy = (x / nx) % ny, iz = x / (nx * ny);
+            nb[6 * (size_t)x + 0] = (ix + nx - 1) % nx - ix;               nb[6 * (size_t)x + 1] = (ix + 1) % nx - ix;
+            nb[6 * (size_t)x + 2] = ((iy + ny - 1) % ny - iy) * nx;        nb[6 * (size_t)x + 3] = ((iy + 1) % ny - iy) * nx;
+            nb[6 * (size_t)x + 4] = ((iz + nz - 1) % nz - iz) * nx * ny;   nb[6 * (size_t)x + 5] = ((iz + 1) % nz - iz) * nx * ny;
+        }
+        std::vector<unsigned char> pw((size_t)c->Np);
+        for (int pc = 0; pc < c->Np; ++pc) {
+            const int q[3] = { pc % n, (pc / n) % n, pc / (n * n) };
+            unsigned w = 0;
+            for (int d = 0; d < 3; ++d) w |= (q[d] == 0 ? 1u : 0u) << (2 * d) | (q[d] == n - 1 ? 1u : 0u) << (2 * d + 1);
+            pw[pc] = (unsigned char)w;
+        }
+        BZ_CUDA(cudaMemcpyAsync(c->x_nb, nb.data(), nb.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream), "upload x_nb");
+        BZ_CUDA(cudaMemcpyAsync(c->p_wrap, pw.data(), pw.size(), cudaMemcpyHostToDevice, c->stream), "upload p_wrap");
+        BZ_CUDA(cudaStreamSynchronize(c->stream), "table sync");
+    }
     BZ_CUDA(launch_vlasov(c->f, out, c->grid.nx, c->grid.ny, c->grid.nz, c->S, c->Np, c->cell_tab, c->mass2, c->E_tab,
-                          c->grid.np, dt_fm, c->grid.dx, dp, cls, c->stream), "vlasov");
+                          c->x_nb, c->p_wrap, c->grid.np, dt_fm, c->grid.dx, dp, cls, c->stream), "vlasov");
     return 0;
 }
 

@@ -61,6 +61,8 @@ struct bz_ctx_impl {
     double msq_ovr[7];               // bz_set_msq_override: constant |M|^2 per kind of Table I, < 0 = Table I
     double* mass2;                   // device [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 (Eq. 8-9); 0 at start
     double* E_tab;                   // device [Nx][4][Np] energies sqrt(p^2 + m^2), allocated at the first bz_vlasov / scheme >= 1 step
+    int* x_nb;                       // device [Nx][6] periodic spatial neighbour offsets (built with E_tab)
+    unsigned char* p_wrap;           // device [Np] momentum wrap flags (built with E_tab)
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
@@ -113,7 +115,7 @@ cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, 
 cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, double* mass2, int Nx, int S, int Np,
                                   unsigned cls_bits, unsigned id_bits, double g2, double w, cudaStream_t st);
 cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
-                          const double* mass2, double* E_tab, int n, double dt, double dx, double dp, unsigned cls_bits,
-                          cudaStream_t st);
+                          const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
+                          double dx, double dp, unsigned cls_bits, cudaStream_t st);
 
 }  // namespace bz

@@ -74,51 +74,70 @@ struct VlasovParams {
     double* out;                  // dF, same layout
     const double* cell_tab;       // [Np][4] px, py, pz, |p|
     const double* E_tab;          // [Nx][4][Np] energies of the mass classes present (energy_kernel)
+    const int* x_nb;              // [Nx][6] cell index offsets of the spatial neighbours (-x, +x, -y, +y, -z, +z), periodic
+    const unsigned char* p_wrap;  // [Np] bit 2d: the -e_d momentum neighbour wraps, bit 2d + 1: the +e_d one
     int nx, ny, nz, S, Np, n;     // n = momentum cells per axis
+    int chunks_per_block;
     double dt, inv_2dx, inv_2dp;
     unsigned cls_bits;
 };
 
-// One thread per phase-space value (x, a, pc): 12 f reads + 18 energy reads + 3 table reads, all independent, ~40
-// registers -> full occupancy; the latency of the scattered neighbour reads is hidden by warps, not by unrolling.
-// blockIdx.x = spatial cell (fastest): the blocks in flight share one (species, 256-cell momentum chunk) slice of all
-// spatial cells (Nx x 2 KB of f and of E), so the six spatial neighbours are L2 hits.
+// One thread per phase-space value (x, a, pc): 12 f reads + 18 energy reads, all independent, < 64 registers; the
+// latency of the scattered neighbour reads is hidden by warps, not by unrolling.  blockIdx.x = spatial cell (fastest):
+// the blocks in flight share one (species, 256-cell momentum chunk) slice of all spatial cells, so the six spatial
+// neighbours are L2 hits.  The first version spent 730 instructions per value, most of them integer divisions by the
+// run-time grid sizes and IEEE fp64 divisions (ncu: issue-bound at 74 %); the periodic wrap now comes from two small
+// tables built once per context (x_nb: neighbour cell offsets per spatial cell, p_wrap: one flag byte per momentum
+// cell) and p_i / E from a Newton reciprocal.
+__device__ __forceinline__ double rcp_newton(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 __global__ void __launch_bounds__(256) vlasov_kernel(const VlasovParams V)
 {
     const int xcell = blockIdx.x, a = blockIdx.z;
-    const int pc = blockIdx.y * blockDim.x + threadIdx.x;
+    // a block walks V.chunks_per_block consecutive 256-cell chunks (about 8 p_z planes): the +-n^2 momentum neighbours of
+    // a chunk are then touched again by the same block a few iterations later instead of 2.25 x Nx blocks later, i.e.
+    // they are still in L2 (ncu on the one-chunk version: 3 x the compulsory DRAM reads)
+    for (int ch = 0; ch < V.chunks_per_block; ++ch) {
+    const int pc = (blockIdx.y * V.chunks_per_block + ch) * blockDim.x + threadIdx.x;
     if (pc >= V.Np) return;
-    const int ix = xcell % V.nx, iy = (xcell / V.nx) % V.ny, iz = xcell / (V.nx * V.ny);
-    int xo[3][2];                                            // spatial neighbours (periodic): cell index offsets
-    xo[0][0] = (ix + V.nx - 1) % V.nx - ix;                  xo[0][1] = (ix + 1) % V.nx - ix;
-    xo[1][0] = ((iy + V.ny - 1) % V.ny - iy) * V.nx;         xo[1][1] = ((iy + 1) % V.ny - iy) * V.nx;
-    xo[2][0] = ((iz + V.nz - 1) % V.nz - iz) * V.nx * V.ny;  xo[2][1] = ((iz + 1) % V.nz - iz) * V.nx * V.ny;
     const int n = V.n;
-    const int pi3[3] = { pc % n, (pc / n) % n, pc / (n * n) };
-    const int pstr[3] = { 1, n, n * n };
     const int cls = class_of(V.cls_bits, a);
     const size_t row = (size_t)V.S * V.Np;
     const double* fx = V.f + (size_t)xcell * row + (size_t)a * V.Np + pc;
     const double* Ex = V.E_tab + ((size_t)xcell * 4 + cls) * V.Np + pc;
+    const unsigned wrap = V.p_wrap[pc];                      // bit 2d: p - dp e_d wraps, bit 2d + 1: p + dp e_d wraps
+    const int* xnb = V.x_nb + 6 * (size_t)xcell;             // cell index offsets of x -+ dx e_d (periodic)
+    int pstr = 1;
     double acc = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        const int pom = ((pi3[d] + n - 1) % n - pi3[d]) * pstr[d];       // momentum neighbours, periodic in p
-        const int pop = ((pi3[d] + 1) % n - pi3[d]) * pstr[d];
+        const int pom = ((wrap >> (2 * d)) & 1u) ? (n - 1) * pstr : -pstr;       // periodic in p
+        const int pop = ((wrap >> (2 * d + 1)) & 1u) ? -(n - 1) * pstr : pstr;
+        pstr *= n;
         const double pd = __ldg(V.cell_tab + 4 * (size_t)pc + d);
-        const double* Em = Ex + (ptrdiff_t)xo[d][0] * 4 * V.Np;          // energies at x - dx e_d
-        const double* Ep = Ex + (ptrdiff_t)xo[d][1] * 4 * V.Np;          // energies at x + dx e_d
+        const ptrdiff_t om = __ldg(xnb + 2 * d), op = __ldg(xnb + 2 * d + 1);
+        const double* Em = Ex + om * 4 * V.Np;               // energies at x - dx e_d
+        const double* Ep = Ex + op * 4 * V.Np;               // energies at x + dx e_d
         const double Exp = __ldg(Ep), Exm = __ldg(Em);
-        const double cp = Exp > 0.0 ? pd / Exp : 0.0, cm = Exm > 0.0 ? pd / Exm : 0.0;   // p = 0 and m = 0: S10
-        const double Gp = (__ldg(Ep + pop) - __ldg(Em + pop)) * V.inv_2dx;               // dE/dx at p + dp e_d
-        const double Gm = (__ldg(Ep + pom) - __ldg(Em + pom)) * V.inv_2dx;               // dE/dx at p - dp e_d
-        const double fxm = __ldg(fx + (ptrdiff_t)xo[d][0] * (ptrdiff_t)row), fxp = __ldg(fx + (ptrdiff_t)xo[d][1] * (ptrdiff_t)row);
+        const double cp = Exp > 0.0 ? pd * rcp_newton(Exp) : 0.0, cm = Exm > 0.0 ? pd * rcp_newton(Exm) : 0.0;   // S10
+        const double Gp = (__ldg(Ep + pop) - __ldg(Em + pop)) * V.inv_2dx;       // dE/dx at p + dp e_d
+        const double Gm = (__ldg(Ep + pom) - __ldg(Em + pom)) * V.inv_2dx;       // dE/dx at p - dp e_d
+        const double fxm = __ldg(fx + om * (ptrdiff_t)row), fxp = __ldg(fx + op * (ptrdiff_t)row);
         const double fpm = __ldg(fx + pom), fpp = __ldg(fx + pop);
         const double drift = (cp * fxp - cm * fxm) * V.inv_2dx;
         const double force = -(fpp * Gp - fpm * Gm) * V.inv_2dp;
         acc += drift + force;
     }
     V.out[(size_t)xcell * row + (size_t)a * V.Np + pc] = -V.dt * acc;
+    }
 }
 
 }  // namespace
@@ -132,8 +151,8 @@ cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, doubl
 }
 
 cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
-                          const double* mass2, double* E_tab, int n, double dt, double dx, double dp, unsigned cls_bits,
-                          cudaStream_t st)
+                          const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
+                          double dx, double dp, unsigned cls_bits, cudaStream_t st)
 {
     unsigned present = 0;
     for (int a = 0; a < S; ++a) present |= 1u << ((cls_bits >> (3 * a)) & 7u);
@@ -144,9 +163,12 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     VlasovParams V;
-    V.f = f; V.out = out; V.cell_tab = cell_tab; V.E_tab = E_tab; V.nx = nx; V.ny = ny; V.nz = nz; V.S = S; V.Np = Np; V.n = n;
+    V.f = f; V.out = out; V.cell_tab = cell_tab; V.E_tab = E_tab; V.x_nb = x_nb; V.p_wrap = p_wrap; V.nx = nx; V.ny = ny; V.nz = nz; V.S = S; V.Np = Np; V.n = n;
     V.dt = dt; V.inv_2dx = 1.0 / (2.0 * dx); V.inv_2dp = 1.0 / (2.0 * dp); V.cls_bits = cls_bits;
-    vlasov_kernel<<<dim3(nx * ny * nz, chunks, S), 256, 0, st>>>(V);
+    V.chunks_per_block = (8 * n * n + 255) / 256;
+    if (V.chunks_per_block > chunks) V.chunks_per_block = chunks;
+    const int groups = (chunks + V.chunks_per_block - 1) / V.chunks_per_block;
+    vlasov_kernel<<<dim3(nx * ny * nz, groups, S), 256, 0, st>>>(V);
     ++g_launch_count;
     return cudaGetLastError();
 }
