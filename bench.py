@@ -67,6 +67,36 @@ def transport_roofline(cfg, tr_ms, tr_n, peak):
             "frac": ach / peak, "ms_per_launch": tr_ms / tr_n}
 
 
+def vlasov_probe(g, cfg, dev, reps=5):
+    """NEXT rank 2, outside the timed step: thermal masses (Eq. 8-9) and the central-difference drift +
+    force operator of Eq. 15 on the bench workload's current f, timed with CUDA events on the context's stream."""
+    import torch
+    out = torch.empty(g.shape, dtype=torch.float64, device=dev)
+
+    def timed(fn):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    from paper_1912_04457_b200 import bz
+    L = bz.lib()
+    ms_mass = timed(lambda: L.bz_thermal_masses(g._h, None))
+    ms_vl = timed(lambda: g.vlasov(cfg.dt, out))
+    n_cls = len({0 if s == 0 else 1 + (s - 1) // 2 for s in cfg.species})
+    # per value: 8 B f read + 8 B dF written + the energy table written once and read once, 8 B per (cell, mass class)
+    bytes_per_value = 16.0 + 16.0 * n_cls / cfg.S
+    rate = cfg.n_values / (ms_vl * 1e-3)
+    return {"kernels": "energy_kernel + vlasov_kernel (bz_vlasov), mass_kernel (bz_thermal_masses)", "bound": "hbm",
+            "ms_vlasov": ms_vl, "ms_thermal_masses": ms_mass, "cell_updates_per_sec": rate, "bytes_per_value": bytes_per_value,
+            "achieved": rate * bytes_per_value / 1e9, "unit": "GB/s"}
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -252,6 +282,7 @@ def run_ours(args, cfg):
     tr_ms, tr_n = g.get_profile(1)
     g.set_profile(False)
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
+    rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs) else None
     clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
@@ -312,6 +343,7 @@ def run_ours(args, cfg):
                      "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; "
                              "the HBM one is the slower for every config and is the one reported"},
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
+        "next_rank2_eq15": None if rank2 is None else dict(rank2, peak=peak, frac=rank2["achieved"] / peak),
         "clocks": clocks,
         "total_particle_number": N1,
     }
