@@ -8,8 +8,8 @@ Default workload: BASELINE.json configs[4] (16^3 spatial x 24^3 momentum cells, 
 north_star quotes the roofline target on; it fits one GPU.  One JSON line is printed by rank 0.
 
   value            kinematic collision samples per second over the whole step, inputs resident in HBM
-  e2e              the same, but every step starts from HOST f (bz_set_f from pinned memory) and ends with f and the
-                   moments back on the host (bz_get_f, bz_moments)
+  e2e              the same, but every step starts from HOST f in pinned memory and ends with f and the moments back on
+                   the host (bz_step_host: copies, collision and stream + Euler pipelined by z layers; then bz_moments)
   roofline         the collision kernel alone (CUDA events inside libbz.so around every launch of the timed region):
                    algorithmic gather/scatter bytes per sample x samples / duration vs measured HBM GB/s
   cpu_baseline     the oracle as it stands, on this box's host cores, on a bounded sample of the same workload
@@ -292,10 +292,13 @@ def run_ours(args, cfg):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(e2e_steps):
-        g.set_f(host_in)
-        step_fn(cfg.dt)
+        if slabs:
+            g.set_f(host_in)
+            step_fn(cfg.dt)
+            g.get_f(host_out)
+        else:
+            g.step_host(cfg.dt, host_in, host_out)     # bz_step_host: H2D, collision, stream + Euler, D2H pipelined by z layers
         g.moments(mom_host)
-        g.get_f(host_out)
     e1.record()
     torch.cuda.synchronize()
     ms_e2e = e0.elapsed_time(e1)

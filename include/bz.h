@@ -126,6 +126,15 @@ int bz_set_transport(bz_ctx* ctx, int scheme);
  * Asynchronous. */
 int bz_step(bz_ctx* ctx, double dt_fm);
 
+/* The same step end to end from HOST memory: f_in_host (S*Nx*Np doubles, ideally pinned) replaces the context's f,
+ * one bz_step is taken, and the new f is written to f_out_host; the context keeps the new f and the incremented step
+ * counter exactly as after bz_set_f + bz_step + bz_get_f.  With at least 3 z layers and transport scheme 0 the work
+ * is pipelined in chunks of z layers over three streams -- host-to-device copy of chunk k+1, collision of chunk k (the
+ * collision term needs only the chunk's own cells, Eq. 5), stream + Euler of chunk k-1 (its upwind stencil needs
+ * the old f of both z neighbours) and device-to-host copy of chunk k-2 run concurrently -- otherwise it is that plain
+ * sequence.  Same results as the plain sequence up to the summation order of the deposits.  Synchronises. */
+int bz_step_host(bz_ctx* ctx, double dt_fm, const double* f_in_host, double* f_out_host);
+
 /* Moments of the current f (Eq. 10; T^00 of Eq. 11, massless; S8a.8) written to HOST memory:
  *   out_host[(xcell*S + a)*2 + {0,1}] = n_a(x) in GeV^3, e_a(x) in GeV^4;
  *   then S pairs (N_a, E_a) = sum_x (n, e) dx^3/hbarc^3  (dimensionless, GeV);

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
-           "bz_set_transport", "bz_set_f",
+           "bz_set_transport", "bz_step_host", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
@@ -48,6 +48,7 @@ def lib():
         L.bz_set_masses.argtypes = [vp, vp]
         L.bz_vlasov.argtypes = [vp, C.c_double, vp]
         L.bz_set_transport.argtypes = [vp, C.c_int]
+        L.bz_step_host.argtypes = [vp, C.c_double, vp, vp]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.bz_set_f.argtypes = [vp, vp, C.c_int]
         L.bz_get_f.argtypes = [vp, vp, C.c_int]
@@ -216,6 +217,14 @@ class Boltzmann:
 
     def step(self, dt):
         self._chk(lib().bz_step(self._h, dt), "bz_step")
+
+    def step_host(self, dt, f_in, f_out):
+        """bz_step_host: f_in, f_out are CPU float64 tensors (pinned for full copy speed) of n_values elements."""
+        for t in (f_in, f_out):
+            if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or t.numel() != self.n_values:
+                raise ValueError("expected contiguous CPU float64 tensors with %d elements" % self.n_values)
+        self._chk(lib().bz_step_host(self._h, dt, C.c_void_p(f_in.data_ptr()), C.c_void_p(f_out.data_ptr())), "bz_step_host")
+        return f_out
 
     def moments(self, out=None):
         n = 2 * self.S * self.Nx + 2 * self.S + self.Nx

@@ -1,5 +1,6 @@
 // bz_api.cu -- the C ABI of include/bz.h: context, argument checks, kernel sequencing.  No compute on the host
 // except the O(Np) cell-centre tables built once in bz_create.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -165,7 +166,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->mask = 0;
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
-    c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false;
+    c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false; c->copy_in = nullptr; c->copy_out = nullptr;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
     c->mass2 = nullptr; c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
@@ -233,6 +234,9 @@ int bz_destroy(bz_ctx* c)
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->pipe_events) cudaEventDestroy(e);
+    if (c->copy_in) cudaStreamDestroy(c->copy_in);
+    if (c->copy_out) cudaStreamDestroy(c->copy_out);
     delete c;
     return 0;
 }
@@ -312,6 +316,7 @@ static TransportParams transport_params(const bz_ctx* c, double dt_fm, double* o
     TransportParams T;
     T.f = c->f; T.dN_aos = c->dN_aos; T.SP = c->SP; T.out = out; T.f_aos_out = c->f_aos; T.vx = c->vx; T.vy = c->vy; T.vz = c->vz;
     T.nx = c->grid.nx; T.ny = c->grid.ny; T.nz = c->grid.nz; T.S = c->S; T.Np = c->Np;
+    T.x_begin = 0; T.x_count = c->Nx;
     T.cfl = dt_fm / c->grid.dx;
     fill_deg(c, T.inv_deg);
     return T;
@@ -406,6 +411,89 @@ int bz_step(bz_ctx* c, double dt_fm)
     double* t = c->f; c->f = c->f_new; c->f_new = t;
     c->rowsum_valid = false;          // f changed; f_aos was rewritten with the new f by the Euler kernel
     c->step += 1;
+    return 0;
+}
+
+
+/* Pipelined end-to-end step: see include/bz.h.  Chunks of z layers flow H2D -> (row sums, m^2, cell-major copy,
+ * collision) -> stream + Euler -> D2H on three streams; the collision term of a chunk needs only that chunk's f
+ * (Eq. 5 is local in x), the upwind stencil of chunk k needs the old f of chunks k - 1 and k + 1 as well. */
+int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out_host)
+{
+    if (!c || !f_in_host || !f_out_host) return -1;
+    if (!c->f) return -4;
+    const int nzl = c->grid.nz, layer_cells = c->grid.nx * c->grid.ny;
+    const int lpc = (nzl + 15) / 16;                             // z layers per chunk: at most 16 chunks
+    const int K = (nzl + lpc - 1) / lpc;
+    if (c->scheme != 0 || K < 3) {                               // nothing to overlap (or Eq. 15 transport): the plain sequence
+        if (int rc = bz_set_f(c, f_in_host, 0)) return rc;
+        if (int rc = bz_step(c, dt_fm)) return rc;
+        return bz_get_f(c, f_out_host, 0);
+    }
+    if (!c->copy_in) {
+        BZ_CUDA(cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking), "copy stream");
+        BZ_CUDA(cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking), "copy stream");
+    }
+    while ((int)c->pipe_events.size() < 2 * K + 1) {
+        cudaEvent_t e = nullptr;
+        BZ_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "pipe event");
+        c->pipe_events.push_back(e);
+    }
+    cudaEvent_t* h2d_done = c->pipe_events.data();               // [K]
+    cudaEvent_t* tr_done = c->pipe_events.data() + K;            // [K]
+    cudaEvent_t start = c->pipe_events[2 * K];
+    const size_t cell_vals = (size_t)c->S * c->Np;               // doubles per spatial cell
+    auto x0_of = [&](int k) { return k * lpc * layer_cells; };
+    auto nx_of = [&](int k) { return (std::min(nzl, (k + 1) * lpc) - k * lpc) * layer_cells; };
+    // the copy streams start after whatever the context's stream has queued so far
+    BZ_CUDA(cudaEventRecord(start, c->stream), "record");
+    BZ_CUDA(cudaStreamWaitEvent(c->copy_in, start, 0), "wait");
+    BZ_CUDA(cudaStreamWaitEvent(c->copy_out, start, 0), "wait");
+    for (int k = 0; k < K; ++k) {
+        const size_t off = (size_t)x0_of(k) * cell_vals, cnt = (size_t)nx_of(k) * cell_vals;
+        BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
+        BZ_CUDA(cudaEventRecord(h2d_done[k], c->copy_in), "record");
+    }
+    const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;
+    auto transport_chunk = [&](int k) -> int {
+        TransportParams T = transport_params(c, dt_fm, c->f_new);
+        T.x_begin = x0_of(k); T.x_count = nx_of(k);
+        BZ_CUDA(launch_transport(T, 1, c->stream), "stream+euler");
+        BZ_CUDA(cudaEventRecord(tr_done[k], c->stream), "record");
+        BZ_CUDA(cudaStreamWaitEvent(c->copy_out, tr_done[k], 0), "wait");
+        const size_t off = (size_t)x0_of(k) * cell_vals, cnt = (size_t)nx_of(k) * cell_vals;
+        BZ_CUDA(cudaMemcpyAsync(f_out_host + off, c->f_new + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->copy_out), "d2h");
+        return 0;
+    };
+    for (int k = 0; k < K; ++k) {
+        const int x0 = x0_of(k), nxk = nx_of(k);
+        BZ_CUDA(cudaStreamWaitEvent(c->stream, h2d_done[k], 0), "wait");
+        BZ_CUDA(launch_rowsums(c->f + (size_t)x0 * cell_vals, c->absp, c->w_invE, c->rowsum + (size_t)x0 * c->S * 3, nxk * c->S, c->Np,
+                               c->stream), "rowsums");
+        BZ_CUDA(launch_m2(c->rowsum + (size_t)x0 * c->S * 3, c->m2 + x0, nxk, c->S, glue_slot_mask, 4.0 * kPi * c->alpha_s, c->m_D,
+                          c->stream), "m2");
+        if (c->SP != 1)
+            BZ_CUDA(launch_pack(c->f + (size_t)x0 * cell_vals, c->f_aos + (size_t)x0 * c->Np * c->SP, nxk, c->S, c->SP, c->Np,
+                                c->stream), "pack");
+        // collision of the chunk's own cells (bz_set_slab may exclude halo layers)
+        const int zb = std::max(c->zb, k * lpc), ze = std::min(c->ze, std::min(nzl, (k + 1) * lpc));
+        if (ze > zb) {
+            CollideParams P = collide_params(c, dt_fm, c->step);
+            P.x_begin = zb * layer_cells;
+            P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)c->regions_per_x;
+            BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
+            c->launch_parity ^= 1u;
+        }
+        // chunk k - 1 has both z neighbours on the device now (chunk 0 waits for the last one: periodic)
+        if (k >= 2) { if (int rc = transport_chunk(k - 1)) return rc; }
+    }
+    if (int rc = transport_chunk(K - 1)) return rc;
+    if (int rc = transport_chunk(0)) return rc;
+    double* t = c->f; c->f = c->f_new; c->f_new = t;
+    c->aos_valid = true; c->rowsum_valid = false;
+    c->step += 1;
+    BZ_CUDA(cudaStreamSynchronize(c->copy_out), "d2h sync");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "sync");
     return 0;
 }
 

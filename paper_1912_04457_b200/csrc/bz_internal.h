@@ -45,6 +45,7 @@ struct TransportParams {
     int SP;
     const double* vx; const double* vy; const double* vz;   // [Np] p/|p| at the cell centre (0 at p = 0)
     int nx, ny, nz, S, Np;
+    int x_begin, x_count; // spatial cells [x_begin, x_begin + x_count) are updated (all by default)
     double cfl;           // dt / dx
     double inv_deg[7];    // per layout index a: 1/N_a is NOT used (division kept exact); holds N_a
 };
@@ -82,7 +83,9 @@ struct bz_ctx_impl {
     double *cell_tab;                // device [Np][4]: p1x, p1y, p1z, E1 (built on the device, bit-exact arithmetic)
     std::string err;
     bool profile;
-    std::vector<cudaEvent_t> prof_events[2];   // start/stop pairs: [0] collision (pack + collide), [1] stream + Euler
+    std::vector<cudaEvent_t> prof_events[2];
+    cudaStream_t copy_in, copy_out;  // bz_step_host: H2D / D2H streams (created at first use)
+    std::vector<cudaEvent_t> pipe_events;   // bz_step_host: per chunk h2d-done and transport-done events (created at first use)   // start/stop pairs: [0] collision (pack + collide), [1] stream + Euler
 };
 
 // kernels launched by this library in this process (bz_launch_count); bumped by every launcher below

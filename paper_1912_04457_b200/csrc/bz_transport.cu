@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256, BZ_TR_MINB) transport_kernel(const Transp
     // blockIdx.x = spatial cell (fastest), blockIdx.y = chunk of 256 momentum cells: the blocks in flight share one
     // momentum chunk of ALL spatial cells (Nx x S x 2 KB, 58 MB for config 4), which fits L2, so the three upwind
     // neighbour reads hit L2 instead of HBM (x-major order: the z neighbour is 256 rows = 198 MB away and misses)
-    const int xcell = blockIdx.x;
+    const int xcell = P.x_begin + blockIdx.x;
     const int ix = xcell % P.nx, iy = (xcell / P.nx) % P.ny, iz = xcell / (P.nx * P.ny);
     const size_t row = (size_t)P.S * P.Np;                    // doubles per spatial cell
     const int xm = (ix + P.nx - 1) % P.nx - ix, xp = (ix + 1) % P.nx - ix;
@@ -148,7 +148,7 @@ cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st
 {
     int chunks = (P.Np + 255) / 256;
     if (chunks > 65535) chunks = 65535;
-    dim3 grid(P.nx * P.ny * P.nz, chunks);
+    dim3 grid(P.x_count, chunks);
     if (mode == 0) transport_kernel<0><<<grid, 256, 0, st>>>(P);
     else if (mode == 1) transport_kernel<1><<<grid, 256, 0, st>>>(P);
     else transport_kernel<2><<<grid, 256, 0, st>>>(P);

@@ -413,3 +413,30 @@ def test_step_with_eq15_transport(scheme):
     o2.set_f(f0)
     N0 = o2.moments()["tot"][:, 0].sum()
     assert mg["tot"][:, 0].sum().item() == pytest.approx(N0, rel=1e-12)
+
+
+# ------------------------------------------------------------------------------- bz_step_host (pipelined end to end)
+@pytest.mark.parametrize("cfg", [wl.scaled(wl.CONFIGS[3], nx=5, np_=8, samples=16),      # 5 z layers: 5 chunks
+                                 wl.scaled(wl.CONFIGS[4], nx=3, np_=7, samples=9),       # 3 chunks, odd grid
+                                 wl.scaled(wl.CONFIGS[2], np_=8, samples=16)],           # 1 layer: the plain sequence
+                         ids=lambda c: c.name)
+def test_step_host_matches_oracle(cfg):
+    """bz_step_host (host f in, one step, host f out, chunks of z layers pipelined over three streams) against the oracle,
+    and the context is left as after bz_set_f + bz_step: a following bz_step continues from it."""
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=13)
+    o.set_f(f0)
+    hin = torch.from_numpy(f0.copy()).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    for _ in range(2):
+        o.step(cfg.dt)
+        g.step_host(cfg.dt, hin, hout)
+        f_o = o.get_f()
+        assert np.abs(hout.numpy() - f_o).max() <= TOL_DF * np.abs(f_o).max()
+        hin.copy_(hout)
+    assert np.array_equal(g.get_f().cpu().numpy(), hout.numpy())
+    o.step(cfg.dt)
+    g.step(cfg.dt)
+    f_o = o.get_f()
+    assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= TOL_DF * np.abs(f_o).max()
+    assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
