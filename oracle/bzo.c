@@ -592,6 +592,165 @@ int bzo_vlasov(bzo_ctx* c, double dt_fm, double* dF)
     return 0;
 }
 
+/* ------------------------------------------------------------------ NEXT rank 1 (S8f): the paper's own collision path */
+/* One root of E1 + E2 = E3 + Ep (Eq. 18-19) for one mass tuple; everything a pin may want to look at. */
+/* (struct bzo_proot is declared in bzo.h) */
+
+/* Eq. 17-19 for one sample and one mass tuple (m1^2 .. m4^2 of particles a, b, c, d).  p = grid point (particle d),
+ * k3 and (k1x, k1y) given.  Energy conservation E1(z) + E2(z) = Et, Et = E3 + Ep, with
+ *   E1^2 = A1 + z^2, A1 = k1x^2 + k1y^2 + m1^2;   E2^2 = A2 + (Pz - z)^2, A2 = (Px-k1x)^2 + (Py-k1y)^2 + m2^2, P = k3 + p.
+ * Squaring once: 2 Et E1 = C + 2 Pz z, C = Et^2 + A1 - A2 - Pz^2; squaring again:
+ *   a z^2 - C Pz z + (Et^2 A1 - C^2/4) = 0,  a = Et^2 - Pz^2  =>  z+- = [C Pz +- Et sqrt(D)] / (2 a),  D = C^2 - 4 a A1,
+ * the paper's k1z+- = (A +- sqrt(H))/B.  A root is kept iff C + 2 Pz z >= 0 and E1 <= Et (the two squarings), J != 0,
+ * and k1, k2 lie in the momentum box (S9).  Only + - x / sqrt, association as written (bit-exact on the GPU).
+ * Returns the number of roots written to out[0..1] (order: +, -). */
+static int paper_roots(const bzo_ctx* c, const double p[3], const double k3[3], double k1x, double k1y,
+                       const double msq[4], bzo_proot out[2])
+{
+    const double E3 = sqrt(((k3[0] * k3[0] + k3[1] * k3[1]) + k3[2] * k3[2]) + msq[2]);
+    const double Ep = sqrt(((p[0] * p[0] + p[1] * p[1]) + p[2] * p[2]) + msq[3]);
+    const double Et = E3 + Ep;
+    const double Px = k3[0] + p[0], Py = k3[1] + p[1], Pz = k3[2] + p[2];
+    const double A1 = (k1x * k1x + k1y * k1y) + msq[0];
+    const double qx = Px - k1x, qy = Py - k1y;
+    const double A2 = (qx * qx + qy * qy) + msq[1];
+    const double Et2 = Et * Et;
+    const double C = ((Et2 + A1) - A2) - Pz * Pz;
+    const double a = Et2 - Pz * Pz;
+    if (!(a > 0.0)) return 0;
+    const double D = C * C - (4.0 * a) * A1;
+    if (!(D > 0.0)) return 0;                     /* no root, or a double root with J = 0 */
+    const double sq = Et * sqrt(D), CP = C * Pz, a2 = 2.0 * a;
+    int nr = 0;
+    for (int sign = 0; sign < 2; ++sign) {
+        const double z = (sign == 0 ? CP + sq : CP - sq) / a2;
+        if (!(C + (2.0 * Pz) * z >= 0.0)) continue;
+        const double E1 = sqrt(A1 + z * z);
+        if (!(E1 <= Et)) continue;
+        const double k2z = Pz - z;
+        const double E2 = sqrt(A2 + k2z * k2z);
+        if (!(E1 > 0.0 && E2 > 0.0)) continue;
+        const double J = z / E1 - k2z / E2;       /* Eq. 19 */
+        if (J == 0.0) continue;
+        bzo_proot* r = &out[nr];
+        r->k1[0] = k1x; r->k1[1] = k1y; r->k1[2] = z;
+        r->k2[0] = qx;  r->k2[1] = qy;  r->k2[2] = k2z;
+        r->i1 = bin_cell(c, r->k1);
+        r->i2 = bin_cell(c, r->k2);
+        if (r->i1 < 0 || r->i2 < 0) continue;     /* a leg outside the box: the root contributes nothing (S9) */
+        r->E1 = E1; r->E2 = E2; r->E3 = E3; r->Ep = Ep; r->J = J;
+        r->s = Et2 - ((Px * Px + Py * Py) + Pz * Pz);
+        r->t = (msq[0] + msq[2]) - 2.0 * (E1 * E3 - ((k1x * k3[0] + k1y * k3[1]) + z * k3[2]));
+        r->u = (msq[0] + msq[3]) - 2.0 * (E1 * Ep - ((k1x * p[0] + k1y * p[1]) + z * p[2]));
+        ++nr;
+    }
+    return nr;
+}
+
+/* the five integration variables of Eq. 20 for (step, xcell, pcell, sample): Philox blocks 64, 65, 66 of the same
+ * key/counter layout as S8c step 1 (the CM sampler uses blocks 0..63) */
+static void paper_draw(const bzo_ctx* c, unsigned step, unsigned xcell, int pcell, int sample, double k3[3], double* k1x, double* k1y)
+{
+    const double pmin = c->g.pmin, L = c->g.pmax - c->g.pmin;
+    double u0, u1, u2, u3, u4, unused;
+    draw(c, step, xcell, pcell, sample, 64u, &u0, &u1);
+    draw(c, step, xcell, pcell, sample, 65u, &u2, &u3);
+    draw(c, step, xcell, pcell, sample, 66u, &u4, &unused);
+    k3[0] = pmin + u0 * L; k3[1] = pmin + u1 * L; k3[2] = pmin + u2 * L;
+    *k1x = pmin + u3 * L; *k1y = pmin + u4 * L;
+}
+
+int bzo_paper_sample(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, const double msq[4],
+                     double k3_out[3], int* i3_out, bzo_proot out[2])
+{
+    if (!c || !msq || !out || xcell < 0 || xcell >= c->Nx || pcell < 0 || pcell >= c->Np) return -1;
+    const int n = c->g.np;
+    const double p[3] = { cell_centre(c, pcell % n), cell_centre(c, (pcell / n) % n), cell_centre(c, pcell / (n * n)) };
+    double k3[3], k1x, k1y;
+    paper_draw(c, step, (unsigned)xcell + c->xoff, pcell, sample, k3, &k1x, &k1y);
+    if (k3_out) { k3_out[0] = k3[0]; k3_out[1] = k3[1]; k3_out[2] = k3[2]; }
+    if (i3_out) *i3_out = bin_cell(c, k3);
+    return paper_roots(c, p, k3, k1x, k1y, msq, out);
+}
+
+/* dF = dt C[f] with the paper's own sampler (Eq. 17-21) and massive dispersion E^a = sqrt(p^2 + m_a^2(x))
+ * from the stored thermal masses (Eq. 8-9; all 0 = massless).  Grid point p = centre of cell i = OUTGOING particle d
+ * (Eq. 5); k3 and (k1x, k1y) uniform in the box (Eq. 20, V_domain = L^5); k1z from the roots; k2 = k3 + p - k1.
+ * Every ordered channel (S8c step 5) is evaluated with the roots of its own mass tuple; the sample feeds the four
+ * cells with -A, -A, +A, +A (Eq. 22), A = Kp |M|^2 fwd / (|J| E1 E2 E3 Ep),
+ * Kp = (dt/hbarc) L^5 / (Ns (2 pi)^5 16) * (1/2) * (1/4)   [1/2: Eq. 3-4 over ordered channels, 1/4: four cells, S2].
+ * Table I is evaluated at the massive s, t, u of the root with the regulator m_g^2(x) (the stored gluon mass; m_D^2 if
+ * m_D > 0). */
+int bzo_collision_paper(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
+{
+    if (!c || !dF) return -1;
+    const double pi = 3.14159265358979323846;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const size_t tile = (size_t)S * Np;
+    memset(dF, 0, tile * c->Nx * sizeof(double));
+    memset(c->gross, 0, tile * c->Nx * sizeof(double));
+    const double L = c->g.pmax - c->g.pmin, twopi5 = ((2.0 * pi) * (2.0 * pi)) * ((2.0 * pi) * (2.0 * pi)) * (2.0 * pi);
+    const double Kp = (dt_fm / HBARC) * ((L * L) * (L * L) * L) / ((double)c->Ns * twopi5 * 16.0) * 0.125;
+    const double g2 = 4.0 * pi * c->alpha_s, g4 = g2 * g2;
+    const int layer = c->g.nx * c->g.ny, xb = c->zb * layer, xe = c->ze * layer;
+    const int nt = c->nthreads < 1 ? 1 : c->nthreads;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nt)
+    for (int x = xb; x < xe; ++x) {
+        const double* ft = c->f + (size_t)x * tile;
+        double* dN = dF + (size_t)x * tile;
+        double* gr = c->gross + (size_t)x * tile;
+        const double* mass2 = c->mass2 + 4 * (size_t)x;
+        const double mreg = c->m_D > 0.0 ? c->m_D * c->m_D : mass2[0];
+        for (int i = 0; i < Np; ++i) {
+            const double p[3] = { cell_centre(c, i % n), cell_centre(c, (i / n) % n), cell_centre(c, i / (n * n)) };
+            for (int smp = 0; smp < c->Ns; ++smp) {
+                double k3[3], k1x, k1y;
+                paper_draw(c, step, (unsigned)x + c->xoff, i, smp, k3, &k1x, &k1y);
+                const int i3 = bin_cell(c, k3);
+                if (i3 < 0) continue;                 /* cannot happen: k3 is drawn inside the box */
+                int done[256];                        /* mass tuples already handled for this sample */
+                memset(done, 0, sizeof done);
+                for (int q0 = 0; q0 < c->nch; ++q0) {
+                    const bzo_channel* c0 = &c->ch[q0];
+                    const int key = mass_class(c->species[c0->a]) | mass_class(c->species[c0->b]) << 2 |
+                                    mass_class(c->species[c0->c]) << 4 | mass_class(c->species[c0->d]) << 6;
+                    if (done[key]) continue;
+                    done[key] = 1;
+                    const double msq[4] = { mass2[key & 3], mass2[(key >> 2) & 3], mass2[(key >> 4) & 3], mass2[(key >> 6) & 3] };
+                    bzo_proot rt[2];
+                    const int nr = paper_roots(c, p, k3, k1x, k1y, msq, rt);
+                    for (int r = 0; r < nr; ++r) {
+                        const bzo_proot* R = &rt[r];
+                        const double w = Kp / (fabs(R->J) * (((R->E1 * R->E2) * R->E3) * R->Ep));
+                        for (int q = q0; q < c->nch; ++q) {       /* the channels of this mass tuple */
+                            const bzo_channel* ch = &c->ch[q];
+                            const int ia = c->species[ch->a], ib = c->species[ch->b], ic = c->species[ch->c], id = c->species[ch->d];
+                            if ((mass_class(ia) | mass_class(ib) << 2 | mass_class(ic) << 4 | mass_class(id) << 6) != key) continue;
+                            double M;
+                            if (c->msq_override[ch->kind] >= 0.0) M = c->msq_override[ch->kind];
+                            else M = ch->crossed ? bzo_msq(ch->kind, R->s, R->u, R->t, mreg, g4) : bzo_msq(ch->kind, R->s, R->t, R->u, mreg, g4);
+                            const size_t xa = (size_t)ch->a * Np + R->i1, xbb = (size_t)ch->b * Np + R->i2;
+                            const size_t xc = (size_t)ch->c * Np + i3, xd = (size_t)ch->d * Np + i;
+                            const double fa = ft[xa], fb = ft[xbb], fc = ft[xc], fd = ft[xd];
+                            const double fwd = fa * fb * Fstat(ic, fc) * Fstat(id, fd) - Fstat(ia, fa) * Fstat(ib, fb) * fc * fd;
+                            const double A = w * M * fwd, g = fabs(A);
+                            dN[xa] -= A; dN[xbb] -= A; dN[xc] += A; dN[xd] += A;
+                            gr[xa] += g; gr[xbb] += g; gr[xc] += g; gr[xd] += g;
+                        }
+                    }
+                }
+            }
+        }
+    }
+    for (int x = 0; x < c->Nx; ++x) for (int a = 0; a < S; ++a) {
+        const double Na = degeneracy(c->species[a]);
+        double* d = dF + ((size_t)x * S + a) * Np;
+        double* g = c->gross + ((size_t)x * S + a) * Np;
+        for (int pc = 0; pc < Np; ++pc) { d[pc] = d[pc] / Na; g[pc] = g[pc] / Na; }
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------ S8a.7: forward Euler, unsplit (Eq. 15) */
 int bzo_step(bzo_ctx* c, double dt_fm)
 {

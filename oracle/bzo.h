@@ -83,6 +83,17 @@ int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 /* transport used by bzo_step: 0 = upwind massless (default), 1 = Eq. 15 with the masses re-evaluated from the old f
  * every step, 2 = Eq. 15 with the masses as stored */
 int  bzo_set_transport(bzo_ctx*, int scheme);
+/* ---- NEXT rank 1 (S8f): the paper's own collision path (Eq. 17-21, massive dispersion) ----------------------------
+ * one root of E1 + E2 = E3 + Ep (Eq. 18-19): momenta k1, k2, their cells, the four energies, the Jacobian of Eq. 19 and
+ * the massive Mandelstam variables */
+typedef struct { double k1[3], k2[3]; int i1, i2; double E1, E2, E3, Ep, J, s, t, u; } bzo_proot;
+/* the sample (step, xcell, pcell, sample) of the paper's sampler for one mass tuple msq = (m_a^2, m_b^2, m_c^2, m_d^2):
+ * k3 (drawn), its cell, and the 0..2 roots kept; returns their number */
+int  bzo_paper_sample(const bzo_ctx*, unsigned step, int xcell, int pcell, int sample, const double msq[4],
+                      double k3_out[3], int* i3_out, bzo_proot out[2]);
+/* dF = dt C[f] with the paper's sampler and E^a = sqrt(p^2 + m_a^2(x)) from the stored thermal masses; also fills
+ * the gross sums (bzo_get_gross) */
+int  bzo_collision_paper(bzo_ctx*, double dt_fm, unsigned step, double* dF);
 /* f <- (f + dF_stream) + dF_coll, both from the old f (Eq. 15 unsplit); step counter ++ */
 int  bzo_step     (bzo_ctx*, double dt_fm);
 /* out = [N_x][S][2] (n, e) then [S][2] totals (N, E) then m^2[N_x]  (Eq. 10-11; Eq. 8) */

@@ -24,6 +24,12 @@ class Channel(C.Structure):
     _fields_ = [("a", C.c_int), ("b", C.c_int), ("c", C.c_int), ("d", C.c_int), ("kind", C.c_int), ("crossed", C.c_int)]
 
 
+class PRoot(C.Structure):
+    _fields_ = [("k1", C.c_double * 3), ("k2", C.c_double * 3), ("i1", C.c_int), ("i2", C.c_int), ("E1", C.c_double),
+                ("E2", C.c_double), ("E3", C.c_double), ("Ep", C.c_double), ("J", C.c_double), ("s", C.c_double),
+                ("t", C.c_double), ("u", C.c_double)]
+
+
 class Sample(C.Structure):
     _fields_ = [("flag", C.c_int), ("j", C.c_int), ("k", C.c_int), ("l", C.c_int), ("attempts", C.c_int),
                 ("s", C.c_double), ("t", C.c_double), ("u", C.c_double),
@@ -56,6 +62,8 @@ def lib():
         L.bzo_thermal_masses.argtypes = [vp, dp]
         L.bzo_vlasov.argtypes = [vp, C.c_double, dp]
         L.bzo_set_transport.argtypes = [vp, C.c_int]
+        L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
+        L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_moments.argtypes = [vp, dp]
         L.bzo_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, ip, dp]
         L.bzo_sample_one.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.POINTER(Sample)]
@@ -193,6 +201,22 @@ class Oracle:
         m = np.empty((self.Nx, 4), dtype=np.float64)
         _chk(lib().bzo_thermal_masses(self._h, _dptr(m)), "bzo_thermal_masses")
         return m
+
+    # ---- NEXT rank 1: the paper's sampler (Eq. 17-21) with massive dispersion
+    def paper_sample(self, step, xcell, pcell, sample, msq):
+        m = (C.c_double * 4)(*msq)
+        k3 = (C.c_double * 3)()
+        i3 = C.c_int()
+        roots = (PRoot * 2)()
+        n = lib().bzo_paper_sample(self._h, step, xcell, pcell, sample, m, k3, C.byref(i3), roots)
+        if n < 0:
+            raise RuntimeError("bzo_paper_sample failed")
+        return list(k3), i3.value, [roots[r] for r in range(n)]
+
+    def collision_paper(self, dt, step):
+        dF = np.empty(self.shape, dtype=np.float64)
+        _chk(lib().bzo_collision_paper(self._h, dt, step, _dptr(dF)), "bzo_collision_paper")
+        return dF
 
     def set_transport(self, scheme):
         _chk(lib().bzo_set_transport(self._h, scheme), "bzo_set_transport")
