@@ -115,6 +115,30 @@ int bz_set_masses(bz_ctx* ctx, const double* mass2_host);
  * dF_dev: device pointer, S*Nx*Np doubles, overwritten.  Asynchronous. */
 int bz_vlasov(bz_ctx* ctx, double dt_fm, double* dF_dev);
 
+/* ---- NEXT rank 1 of SURVEY.md 8f: the paper's own collision path ---------------------------------------------
+ * dF = dt * C_a[f] estimated as the paper does (Eq. 17-21): the grid point p (cell centre) is the OUTGOING
+ * particle d of Eq. 5; (k1x, k1y, k3x, k3y, k3z) are uniform in the momentum box (Eq. 20, V_domain = L^5,
+ * Philox blocks 64-66 of the (seed, step) / (block, sample, pcell, xcell) stream); k1z runs over the roots of
+ * E1 + E2 = E3 + Ep with weight 1/|J| (Eq. 18-19); k2 = k3 + p - k1; dispersion E^a = sqrt(p^2 + m_a^2(x)) with the
+ * stored thermal masses (bz_thermal_masses / bz_set_masses; all 0 = massless), so every tuple of mass classes solves its
+ * own roots; Table I is evaluated at the root's massive s, t, u with the regulator m_g^2(x) (m_D^2 if m_D > 0);
+ * symmetrical sampling (Eq. 22): A = Kp |M|^2 [f f F F - F F f f] / (|J| E1 E2 E3 Ep) goes with - to the cells of k1, k2
+ * and with + to those of k3, p; Kp = (dt/hbarc) L^5 / (Ns (2 pi)^5 16) / 8.  A root with k1 or k2 outside the box is
+ * dropped (S9).  dF_dev: device pointer, S*Nx*Np doubles, overwritten.  Asynchronous.  Honours bz_set_slab and
+ * bz_set_msq_override. */
+int bz_collision_paper(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
+
+/* Test-only: the roots of the paper sampler for ONE mass tuple msq_host = (m_a^2, m_b^2, m_c^2, m_d^2), p1 cells
+ * [pcell_begin, pcell_end) of spatial cell xcell: cells_dev[n][Ns][6] = (cell of k3, number of roots kept, cell of k1
+ * and of k2 for root 0, the same for root 1; -1 where there is none), stu_dev[n][Ns][6] = (s, t, u) of root 0 and 1. */
+int bz_debug_paper_samples(bz_ctx* ctx, unsigned step, int xcell, int pcell_begin, int pcell_end, const double* msq_host,
+                           int* cells_dev, double* stu_dev);
+
+/* Test-only, host only (needs no device): the ordered channel table of the paper sampler for a species list (Eq. 3-4,
+ * S8c step 5), 7 ints per channel (a, b, c, d as layout indices, kind, crossed, mass-class key) into out_host (at most
+ * `capacity` channels are written); returns the number of channels. */
+int bz_debug_paper_channels(const int* species, int n_species, int* out_host, int capacity);
+
 /* Transport scheme used by bz_step: 0 (default, NS) = first-order upwind drift with massless velocities (bz_stream);
  * 1 = Eq. 15 (bz_vlasov) with the thermal masses re-evaluated from the old f at the start of every step;
  * 2 = Eq. 15 with the masses as stored (bz_set_masses / the last bz_thermal_masses).  The collision term is NS's

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
-           "bz_set_transport", "bz_step_host", "bz_set_f",
+           "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
@@ -49,6 +49,9 @@ def lib():
         L.bz_vlasov.argtypes = [vp, C.c_double, vp]
         L.bz_set_transport.argtypes = [vp, C.c_int]
         L.bz_step_host.argtypes = [vp, C.c_double, vp, vp]
+        L.bz_collision_paper.argtypes = [vp, C.c_double, C.c_uint, vp]
+        L.bz_debug_paper_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, vp, vp]
+        L.bz_debug_paper_channels.argtypes = [ip, C.c_int, ip, C.c_int]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
         L.bz_set_f.argtypes = [vp, vp, C.c_int]
         L.bz_get_f.argtypes = [vp, vp, C.c_int]
@@ -212,6 +215,22 @@ class Boltzmann:
         self._chk(lib().bz_vlasov(self._h, dt, self._dev_ptr(out, self.n_values)), "bz_vlasov")
         return out
 
+    # ---- NEXT rank 1: the paper's own sampler (Eq. 17-21) with massive dispersion
+    def collision_paper(self, dt, step, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_collision_paper(self._h, dt, step, self._dev_ptr(out, self.n_values)), "bz_collision_paper")
+        return out
+
+    def debug_paper_samples(self, step, xcell, pbegin, pend, msq):
+        n = pend - pbegin
+        cells = torch.empty((n, self.Ns, 6), dtype=torch.int32, device=self.device)
+        stu = torch.empty((n, self.Ns, 6), dtype=torch.float64, device=self.device)
+        m = (C.c_double * 4)(*msq)
+        self._chk(lib().bz_debug_paper_samples(self._h, step, xcell, pbegin, pend, m, C.c_void_p(cells.data_ptr()),
+                                               C.c_void_p(stu.data_ptr())), "bz_debug_paper_samples")
+        return cells, stu
+
     def set_transport(self, scheme):
         self._chk(lib().bz_set_transport(self._h, scheme), "bz_set_transport")
 
@@ -251,6 +270,17 @@ class Boltzmann:
         self._chk(lib().bz_debug_samples(self._h, step, xcell, pbegin, pend, C.c_void_p(cells.data_ptr()),
                                          C.c_void_p(stu.data_ptr()) if want_stu else None), "bz_debug_samples")
         return cells, stu
+
+
+def debug_paper_channels(species):
+    """Host only: the paper sampler's ordered channel table as rows (a, b, c, d, kind, crossed, key)."""
+    import numpy as np
+    sp = (C.c_int * len(species))(*species)
+    out = np.zeros((256, 7), dtype=np.int32)
+    n = lib().bz_debug_paper_channels(sp, len(species), out.ctypes.data_as(C.POINTER(C.c_int)), 256)
+    if n < 0:
+        raise BzError("bz_debug_paper_channels: bad species list")
+    return out[:n]
 
 
 def measure_fp64_peak():

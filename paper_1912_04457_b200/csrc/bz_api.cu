@@ -169,7 +169,8 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false; c->copy_in = nullptr; c->copy_out = nullptr;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
-    c->mass2 = nullptr; c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
+    c->mass2 = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
+    c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
@@ -232,7 +233,7 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->paper_table); cudaFree(c->paper_groups);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     for (cudaEvent_t e : c->pipe_events) cudaEventDestroy(e);
     if (c->copy_in) cudaStreamDestroy(c->copy_in);
@@ -495,6 +496,85 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
     BZ_CUDA(cudaStreamSynchronize(c->copy_out), "d2h sync");
     BZ_CUDA(cudaStreamSynchronize(c->stream), "sync");
     return 0;
+}
+
+/* ---- NEXT rank 1: the paper's own sampler (bz_paper.cu) ---- */
+static int paper_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
+{
+    if (!c->paper_table) {
+        std::vector<PaperChannel> table;
+        std::vector<PaperGroup> groups;
+        build_paper_channels(c->species, c->S, table, groups);
+        BZ_CUDA(cudaMalloc(&c->paper_table, table.size() * sizeof(PaperChannel)), "cudaMalloc channel table");
+        BZ_CUDA(cudaMalloc(&c->paper_groups, groups.size() * sizeof(PaperGroup)), "cudaMalloc channel groups");
+        BZ_CUDA(cudaMemcpy(c->paper_table, table.data(), table.size() * sizeof(PaperChannel), cudaMemcpyHostToDevice), "upload table");
+        BZ_CUDA(cudaMemcpy(c->paper_groups, groups.data(), groups.size() * sizeof(PaperGroup), cudaMemcpyHostToDevice), "upload groups");
+        c->paper_n_groups = (int)groups.size(); c->paper_n_channels = (int)table.size();
+    }
+    P.g = grid_const(c);
+    P.f = c->f; P.dN = nullptr; P.mass2 = c->mass2; P.table = c->paper_table; P.groups = c->paper_groups;
+    P.n_groups = c->paper_n_groups; P.S = c->S; P.Np = c->Np; P.Ns = c->Ns;
+    const int layer = c->grid.nx * c->grid.ny;
+    P.x_begin = c->zb * layer; P.x_count = (c->ze - c->zb) * layer; P.p_begin = 0; P.p_count = c->Np;
+    P.seed = c->seed; P.step = step; P.x_rng_offset = c->xoff;
+    const double L = P.g.L, twopi = 2.0 * kPi, twopi5 = ((twopi * twopi) * (twopi * twopi)) * twopi;
+    P.Kp = (dt_fm / kHbarc) * ((L * L) * (L * L) * L) / ((double)c->Ns * twopi5 * 16.0) * 0.125;
+    const double g2 = 4.0 * kPi * c->alpha_s;
+    P.g4 = g2 * g2;
+    P.mD2 = c->m_D > 0.0 ? c->m_D * c->m_D : 0.0;
+    P.has_ovr = 0;
+    for (int k = 0; k < 7; ++k) {
+        P.msq_ovr[k] = c->msq_ovr[k] >= 0.0 ? c->msq_ovr[k] / P.g4 : -1.0;
+        if (c->msq_ovr[k] >= 0.0) P.has_ovr = 1;
+    }
+    for (int k = 0; k < 4; ++k) P.dbg_msq[k] = 0.0;
+    return 0;
+}
+
+int bz_collision_paper(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
+{
+    if (!c || !dF_dev) return -1;
+    if (!c->f) return -4;
+    PaperParams P;
+    if (int rc = paper_params(c, dt_fm, step, P)) return rc;
+    P.dN = dF_dev;
+    BZ_CUDA(cudaMemsetAsync(dF_dev, 0, c->n_values * sizeof(double), c->stream), "memset dF");
+    BZ_CUDA(launch_paper_collide(P, c->sms, c->stream), "paper collide");
+    double deg[7];
+    fill_deg(c, deg);
+    BZ_CUDA(launch_paper_finalize(dF_dev, c->n_values, c->S, c->Np, deg, c->stream), "paper finalize");
+    return 0;
+}
+
+int bz_debug_paper_samples(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, const double* msq_host,
+                           int* cells_dev, double* stu_dev)
+{
+    if (!c || !msq_host || !cells_dev || !stu_dev || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np ||
+        pcell_begin > pcell_end)
+        return -1;
+    if (!c->f) return -4;
+    PaperParams P;
+    if (int rc = paper_params(c, 1.0, step, P)) return rc;
+    P.x_begin = xcell; P.x_count = 1; P.p_begin = pcell_begin; P.p_count = pcell_end - pcell_begin;
+    for (int k = 0; k < 4; ++k) P.dbg_msq[k] = msq_host[k];
+    BZ_CUDA(launch_paper_debug(P, cells_dev, stu_dev, c->sms, c->stream), "paper debug");
+    return 0;
+}
+
+int bz_debug_paper_channels(const int* species, int n_species, int* out_host, int capacity)
+{
+    if (!species || n_species < 1 || n_species > 7 || (capacity > 0 && !out_host)) return -1;
+    for (int a = 0; a < n_species; ++a)
+        if (species[a] < 0 || species[a] > 6 || (a > 0 && species[a] <= species[a - 1])) return -1;
+    std::vector<PaperChannel> table;
+    std::vector<PaperGroup> groups;
+    build_paper_channels(species, n_species, table, groups);
+    for (size_t q = 0; q < table.size() && (int)q < capacity; ++q) {
+        int* o = out_host + 7 * q;
+        o[0] = table[q].a; o[1] = table[q].b; o[2] = table[q].c; o[3] = table[q].d; o[4] = table[q].kind; o[5] = table[q].crossed;
+        o[6] = table[q].key;
+    }
+    return (int)table.size();
 }
 
 int bz_moments(bz_ctx* c, double* out_host)

@@ -37,6 +37,26 @@ struct CollideParams {
     double msq_ovr[7];    // per kind: value / g^4, or -1 (Table I)
 };
 
+// NEXT rank 1 (bz_paper.cu): ordered channel a(k1) b(k2) -> c(k3) d(p), layout indices; groups share a mass-class tuple
+struct PaperChannel { unsigned char a, b, c, d, kind, crossed, glue /* bit s: leg s is a gluon */, key /* classes, 2 bits per leg */; };
+struct PaperGroup { int key, begin, end; };
+struct PaperParams {
+    GridConst g;
+    const double* f;          // [Nx][S][Np]
+    double* dN;               // [Nx][S][Np] deposits in number units (the caller's dF, zeroed before the launch)
+    const double* mass2;      // [Nx][4] thermal masses^2 (Eq. 8-9)
+    const PaperChannel* table;
+    const PaperGroup* groups;
+    int n_groups;
+    int S, Np, Ns;
+    int x_begin, x_count, p_begin, p_count;
+    uint32_t seed, step, x_rng_offset;
+    double Kp, g4, mD2;       // Kp = (dt/hbarc) L^5 / (Ns (2 pi)^5 16) / 8;  mD2 > 0: fixed regulator, else m_g^2(x)
+    int has_ovr;
+    double msq_ovr[7];
+    double dbg_msq[4];        // debug launch: the mass tuple whose roots are written out
+};
+
 struct TransportParams {
     const double* f;      // old f
     double* dN_aos;       // collision deposits [Nx][Np][SP] (number units), reset to 0 when consumed
@@ -64,6 +84,9 @@ struct bz_ctx_impl {
     double* E_tab;                   // device [Nx][4][Np] energies sqrt(p^2 + m^2), allocated at the first bz_vlasov / scheme >= 1 step
     int* x_nb;                       // device [Nx][6] periodic spatial neighbour offsets (built with E_tab)
     unsigned char* p_wrap;           // device [Np] momentum wrap flags (built with E_tab)
+    PaperChannel* paper_table;       // device: channel table of the paper sampler (built at the first bz_collision_paper)
+    PaperGroup* paper_groups;        // device
+    int paper_n_groups, paper_n_channels;
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
@@ -120,5 +143,11 @@ cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, doubl
 cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
                           const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
                           double dx, double dp, unsigned cls_bits, cudaStream_t st);
+
+// NEXT rank 1 (bz_paper.cu)
+void build_paper_channels(const int* species, int S, std::vector<PaperChannel>& table, std::vector<PaperGroup>& groups);
+cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st);
+cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, int sms, cudaStream_t st);
+cudaError_t launch_paper_finalize(double* dF, size_t n_values, int S, int Np, const double* deg, cudaStream_t st);
 
 }  // namespace bz

@@ -1,0 +1,268 @@
+// bz_paper.cu -- NEXT rank 1 of SURVEY.md 8f: the paper's own collision path.
+//   Grid point p (cell centre) = the OUTGOING particle d of Eq. 5; integration variables (k1x, k1y, k3x, k3y,
+//   k3z) uniform in the momentum box (Eq. 20); k1z from the two roots of E1 + E2 = E3 + Ep with weight 1/|J|
+//   (Eq. 17-19); k2 = k3 + p - k1; massive dispersion E^a = sqrt(p^2 + m_a^2(x)) from the thermal masses of
+//   Eq. 8-9; symmetrical sampling (Eq. 22): the same weight goes to the cells of k1, k2 (-) and k3, p (+).
+// With masses the kinematics depend on the species of the four legs, so a sample is NOT shared by all channels as in
+// the hot path: the ordered channels (S8c step 5) are grouped by their tuple of mass classes (g, u, d, s) and every
+// group solves its own roots.  One thread per (spatial cell, grid point, sample); the deposits of a root are summed
+// per (slot, species) in a small local array and leave as fp64 reductions (RED.E.ADD.F64) into dF, which a second
+// kernel divides by N_a.  Everything that decides a cell index uses single correctly rounded operations in the
+// association order of the oracle (bit-exact sampled cells).
+#include <vector>
+
+#include "bz_channels.cuh"
+#include "bz_internal.h"
+
+namespace bz {
+
+// ---------------------------------------------------------------------------------------------- host: channel table
+// Ordered channels a(k1) b(k2) -> c(k3) d(p) of the active species (Eq. 3-4; S8c step 5), sorted by the mass
+// classes of the four legs.  kind: 0 A, 1 11, 2 1B, 3 ANN, 4 QQGG, 5 QG, 6 GG (Table I); crossed: M(s,u,t).
+namespace {
+
+int cls_of_id(int id) { return id == 0 ? 0 : 1 + (id - 1) / 2; }
+int anti_of_id(int id) { return (id & 1) ? id + 1 : id - 1; }
+
+}  // namespace
+
+void build_paper_channels(const int* species, int S, std::vector<PaperChannel>& table, std::vector<PaperGroup>& groups)
+{
+    int slot[7];
+    for (int id = 0; id < 7; ++id) slot[id] = -1;
+    for (int a = 0; a < S; ++a) slot[species[a]] = a;
+    std::vector<PaperChannel> all;
+    auto emit = [&](int ia, int ib, int ic, int id, int kind, int crossed) {
+        PaperChannel ch;
+        ch.a = (unsigned char)slot[ia]; ch.b = (unsigned char)slot[ib]; ch.c = (unsigned char)slot[ic]; ch.d = (unsigned char)slot[id];
+        ch.kind = (unsigned char)kind; ch.crossed = (unsigned char)crossed;
+        ch.glue = (unsigned char)((ia == 0) | (ib == 0) << 1 | (ic == 0) << 2 | (id == 0) << 3);
+        ch.key = (unsigned char)(cls_of_id(ia) | cls_of_id(ib) << 2 | cls_of_id(ic) << 4 | cls_of_id(id) << 6);
+        all.push_back(ch);
+    };
+    auto pair_active = [&](int fl) { return slot[1 + 2 * fl] >= 0 && slot[2 + 2 * fl] >= 0; };
+    for (int x = 0; x < S; ++x) for (int y = 0; y < S; ++y) {
+        const int ia = species[x], ib = species[y];
+        const bool ga = ia == 0, gb = ib == 0;
+        if (ga && gb) {                                           // g g -> g g; g g -> q qbar in both orders
+            emit(0, 0, 0, 0, 6, 0);
+            for (int fl = 0; fl < 3; ++fl) if (pair_active(fl)) { emit(0, 0, 1 + 2 * fl, 2 + 2 * fl, 4, 0); emit(0, 0, 2 + 2 * fl, 1 + 2 * fl, 4, 0); }
+        } else if (ga != gb) {                                    // q g -> q g, straight and crossed
+            emit(ia, ib, ia, ib, 5, 0); emit(ia, ib, ib, ia, 5, 1);
+        } else if (ia == ib) {                                    // q1 q1 -> q1 q1 (listed once: t <-> u symmetric)
+            emit(ia, ia, ia, ia, 1, 0);
+        } else if (ib == anti_of_id(ia)) {                        // q1 q1bar -> q1 q1bar, -> q2 q2bar, -> g g
+            emit(ia, ib, ia, ib, 2, 0); emit(ia, ib, ib, ia, 2, 1);
+            for (int fl = 0; fl < 3; ++fl) {
+                if (fl == (ia - 1) / 2 || !pair_active(fl)) continue;
+                emit(ia, ib, 1 + 2 * fl, 2 + 2 * fl, 3, 0); emit(ia, ib, 2 + 2 * fl, 1 + 2 * fl, 3, 0);
+            }
+            if (slot[0] >= 0) emit(ia, ib, 0, 0, 4, 0);
+        } else {                                                  // different flavours (or q1 q2bar): straight and crossed
+            emit(ia, ib, ia, ib, 0, 0); emit(ia, ib, ib, ia, 0, 1);
+        }
+    }
+    table.clear(); groups.clear();
+    std::vector<char> used(all.size(), 0);
+    for (size_t q0 = 0; q0 < all.size(); ++q0) {                  // groups in the order of first appearance
+        if (used[q0]) continue;
+        PaperGroup g;
+        g.key = all[q0].key; g.begin = (int)table.size();
+        for (size_t q = q0; q < all.size(); ++q) if (!used[q] && all[q].key == g.key) { table.push_back(all[q]); used[q] = 1; }
+        g.end = (int)table.size();
+        groups.push_back(g);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------ device
+namespace {
+
+struct Root {
+    int i1, i2;
+    double w_inv;          // |J| E1 E2 E3 Ep
+    double s, t, u;
+};
+
+// Eq. 17-19 for one mass tuple: see oracle/bzo.c paper_roots for the algebra (two squarings of E1 + E2 = Et give
+// a z^2 - C Pz z + (Et^2 A1 - C^2/4) = 0).  Single rounded operations, the oracle's association order.
+__device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
+                                           double m1, double m2, double m3, double m4, Root (&out)[2])
+{
+#define MUL __dmul_rn
+#define ADD __dadd_rn
+#define SUB __dsub_rn
+    const double E3 = __dsqrt_rn(ADD(ADD(ADD(MUL(k3[0], k3[0]), MUL(k3[1], k3[1])), MUL(k3[2], k3[2])), m3));
+    const double Ep = __dsqrt_rn(ADD(ADD(ADD(MUL(p[0], p[0]), MUL(p[1], p[1])), MUL(p[2], p[2])), m4));
+    const double Et = ADD(E3, Ep);
+    const double Px = ADD(k3[0], p[0]), Py = ADD(k3[1], p[1]), Pz = ADD(k3[2], p[2]);
+    const double A1 = ADD(ADD(MUL(k1x, k1x), MUL(k1y, k1y)), m1);
+    const double qx = SUB(Px, k1x), qy = SUB(Py, k1y);
+    const double A2 = ADD(ADD(MUL(qx, qx), MUL(qy, qy)), m2);
+    const double Et2 = MUL(Et, Et), Pz2 = MUL(Pz, Pz);
+    const double C = SUB(SUB(ADD(Et2, A1), A2), Pz2);
+    const double a = SUB(Et2, Pz2);
+    if (!(a > 0.0)) return 0;
+    const double D = SUB(MUL(C, C), MUL(MUL(4.0, a), A1));
+    if (!(D > 0.0)) return 0;
+    const double sq = MUL(Et, __dsqrt_rn(D)), CP = MUL(C, Pz), a2 = MUL(2.0, a);
+    int nr = 0;
+#pragma unroll
+    for (int sign = 0; sign < 2; ++sign) {
+        const double z = __ddiv_rn(sign == 0 ? ADD(CP, sq) : SUB(CP, sq), a2);
+        if (!(ADD(C, MUL(MUL(2.0, Pz), z)) >= 0.0)) continue;
+        const double E1 = __dsqrt_rn(ADD(A1, MUL(z, z)));
+        if (!(E1 <= Et)) continue;
+        const double k2z = SUB(Pz, z);
+        const double E2 = __dsqrt_rn(ADD(A2, MUL(k2z, k2z)));
+        if (!(E1 > 0.0 && E2 > 0.0)) continue;
+        const double J = SUB(__ddiv_rn(z, E1), __ddiv_rn(k2z, E2));          // Eq. 19
+        if (J == 0.0) continue;
+        const int i1 = bin_cell_exact(k1x, k1y, z, g), i2 = bin_cell_exact(qx, qy, k2z, g);
+        if (i1 < 0 || i2 < 0) continue;                                       // a leg outside the box (S9)
+        Root& r = out[nr++];
+        r.i1 = i1; r.i2 = i2;
+        r.w_inv = fabs(J) * (((E1 * E2) * E3) * Ep);
+        r.s = SUB(Et2, ADD(ADD(MUL(Px, Px), MUL(Py, Py)), Pz2));
+        r.t = SUB(ADD(m1, m3), MUL(2.0, SUB(MUL(E1, E3), ADD(ADD(MUL(k1x, k3[0]), MUL(k1y, k3[1])), MUL(z, k3[2])))));
+        r.u = SUB(ADD(m1, m4), MUL(2.0, SUB(MUL(E1, Ep), ADD(ADD(MUL(k1x, p[0]), MUL(k1y, p[1])), MUL(z, p[2])))));
+    }
+#undef MUL
+#undef ADD
+#undef SUB
+    return nr;
+}
+
+__device__ __forceinline__ double msq_pick(const MsqSet& M, int kind, int crossed)
+{
+    switch (kind) {
+    case 0: return crossed ? M.a_u : M.a_t;
+    case 1: return M.m11;
+    case 2: return crossed ? M.m1b_u : M.m1b_t;
+    case 3: return M.ann;
+    case 4: return M.qqgg;
+    case 5: return crossed ? M.qg_u : M.qg_t;
+    default: return M.gg;
+    }
+}
+
+__device__ __forceinline__ void red_add(double* dst, double v)
+{
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst), "d"(v) : "memory");
+}
+
+// mode 0: collision; mode 1: debug (writes the roots of one mass tuple instead of depositing)
+template <int kDebug>
+__global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* dbg_cells, double* dbg_stu)
+{
+    const long long total = (long long)P.x_count * P.p_count * P.Ns;
+    for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
+        const int smp = (int)(q % P.Ns);
+        const long long r1 = q / P.Ns;
+        const int i = P.p_begin + (int)(r1 % P.p_count), xcell = P.x_begin + (int)(r1 / P.p_count);
+        double p[3], Emassless;
+        cell_kinematics(P.g, i, p[0], p[1], p[2], Emassless);
+        // the five integration variables of Eq. 20: Philox blocks 64, 65, 66 (the CM sampler owns 0..63)
+        uint32_t w0[4], w1[4], w2[4];
+        const uint32_t xc = (uint32_t)xcell + P.x_rng_offset;
+        philox4x32_10(64u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w0);
+        philox4x32_10(65u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w1);
+        philox4x32_10(66u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w2);
+        double k3[3];
+        k3[0] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[0], w0[1]), P.g.L));
+        k3[1] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[2], w0[3]), P.g.L));
+        k3[2] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[0], w1[1]), P.g.L));
+        const double k1x = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[2], w1[3]), P.g.L));
+        const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
+        const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
+        const double* m = P.mass2 + 4 * (size_t)xcell;
+        if (kDebug) {
+            Root rt[2];
+            const int nr = paper_roots(P.g, p, k3, k1x, k1y, P.dbg_msq[0], P.dbg_msq[1], P.dbg_msq[2], P.dbg_msq[3], rt);
+            int* oc = dbg_cells + 6 * q;
+            double* os = dbg_stu + 6 * q;
+            oc[0] = i3; oc[1] = nr;
+            for (int r = 0; r < 2; ++r) {
+                oc[2 + 2 * r] = r < nr ? rt[r].i1 : -1; oc[3 + 2 * r] = r < nr ? rt[r].i2 : -1;
+                os[3 * r] = r < nr ? rt[r].s : 0.0; os[3 * r + 1] = r < nr ? rt[r].t : 0.0; os[3 * r + 2] = r < nr ? rt[r].u : 0.0;
+            }
+            continue;
+        }
+        if (i3 < 0) continue;
+        const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
+        const double* fx = P.f + (size_t)xcell * P.S * P.Np;
+        double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+        for (int gi = 0; gi < P.n_groups; ++gi) {
+            const PaperGroup G = P.groups[gi];
+            Root rt[2];
+            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[G.key & 3], m[(G.key >> 2) & 3], m[(G.key >> 4) & 3], m[(G.key >> 6) & 3], rt);
+            for (int r = 0; r < nr; ++r) {
+                const Root& R = rt[r];
+                const double w = P.Kp / R.w_inv;
+                MsqSet M = msq_set<true, true>(R.s, R.t, R.u, mreg, P.g4 * w);
+                if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+                const int cell[4] = { R.i1, R.i2, i3, i };
+                double acc[4][7];
+#pragma unroll
+                for (int sl = 0; sl < 4; ++sl)
+#pragma unroll
+                    for (int a = 0; a < 7; ++a) acc[sl][a] = 0.0;
+                for (int c = G.begin; c < G.end; ++c) {
+                    const PaperChannel ch = P.table[c];
+                    const double fa = fx[(size_t)ch.a * P.Np + cell[0]], fb = fx[(size_t)ch.b * P.Np + cell[1]];
+                    const double fc = fx[(size_t)ch.c * P.Np + cell[2]], fd = fx[(size_t)ch.d * P.Np + cell[3]];
+                    const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
+                    const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
+                    const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;                 // Eq. 5 bracket
+                    const double A = msq_pick(M, ch.kind, ch.crossed) * fwd;
+                    acc[0][ch.a] -= A; acc[1][ch.b] -= A; acc[2][ch.c] += A; acc[3][ch.d] += A;     // Eq. 22
+                }
+#pragma unroll
+                for (int sl = 0; sl < 4; ++sl)
+                    for (int a = 0; a < P.S; ++a)
+                        if (acc[sl][a] != 0.0) red_add(dx + (size_t)a * P.Np + cell[sl], acc[sl][a]);
+            }
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) paper_finalize_kernel(double* __restrict__ dF, size_t n_values, int S, int Np, const double d0,
+                                                              const double d1, const double d2, const double d3, const double d4,
+                                                              const double d5, const double d6)
+{
+    const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
+    for (size_t q = blockIdx.x * (size_t)blockDim.x + threadIdx.x; q < n_values; q += (size_t)gridDim.x * blockDim.x)
+        dF[q] = dF[q] / deg[(q / Np) % S];
+}
+
+}  // namespace
+
+cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
+{
+    const long long total = (long long)P.x_count * P.p_count * P.Ns;
+    if (total <= 0) return cudaSuccess;
+    long long blocks = (total + 127) / 128;
+    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    paper_kernel<0><<<(int)blocks, 128, 0, st>>>(P, nullptr, nullptr);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, int sms, cudaStream_t st)
+{
+    const long long total = (long long)P.x_count * P.p_count * P.Ns;
+    if (total <= 0) return cudaSuccess;
+    long long blocks = (total + 127) / 128;
+    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    paper_kernel<1><<<(int)blocks, 128, 0, st>>>(P, cells, stu);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_paper_finalize(double* dF, size_t n_values, int S, int Np, const double* deg, cudaStream_t st)
+{
+    paper_finalize_kernel<<<148 * 8, 256, 0, st>>>(dF, n_values, S, Np, deg[0], deg[1], deg[2], deg[3], deg[4], deg[5], deg[6]);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+}  // namespace bz

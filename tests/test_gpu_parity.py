@@ -440,3 +440,51 @@ def test_step_host_matches_oracle(cfg):
     f_o = o.get_f()
     assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= TOL_DF * np.abs(f_o).max()
     assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
+
+
+# ------------------------------------------------------------------ NEXT rank 1: the paper's own sampler (Eq. 17-21)
+PAPER_TUPLES = [(0.0, 0.0, 0.0, 0.0), (0.5, 0.5, 0.5, 0.5), (0.3, 0.9, 0.3, 0.9), (0.9, 0.3, 0.3, 0.9), (0.0, 0.7, 0.0, 0.7)]
+
+
+@pytest.mark.parametrize("cfg", [wl.scaled(wl.CONFIGS[2], np_=9, samples=40), wl.scaled(wl.CONFIGS[3], nx=2, np_=8, samples=33)],
+                         ids=lambda c: c.name)
+def test_paper_sampler_roots_bit_exact(cfg):
+    """Cells of k1, k2, k3, the number of roots kept and (s, t, u) of every root: bit-exact against the oracle."""
+    o, g = _pair(cfg)
+    xcell = cfg.Nx - 1
+    for msq in PAPER_TUPLES:
+        cells, stu = g.debug_paper_samples(5, xcell, 0, cfg.Np, msq)
+        cells, stu = cells.cpu().numpy(), stu.cpu().numpy()
+        n_roots = 0
+        for pc in range(0, cfg.Np, 7):
+            for smp in range(cfg.samples):
+                _, i3, roots = o.paper_sample(5, xcell, pc, smp, msq)
+                row, srow = cells[pc, smp], stu[pc, smp]
+                assert row[0] == i3 and row[1] == len(roots), (msq, pc, smp)
+                for r, R in enumerate(roots):
+                    assert (row[2 + 2 * r], row[3 + 2 * r]) == (R.i1, R.i2)
+                    assert np.array_equal(srow[3 * r:3 * r + 3].view(np.uint64), np.array([R.s, R.t, R.u]).view(np.uint64))
+                    n_roots += 1
+        assert n_roots > 200
+
+
+@pytest.mark.parametrize("cfg,massive", [(wl.scaled(wl.CONFIGS[0], np_=9, samples=24), False),
+                                         (wl.scaled(wl.CONFIGS[1], np_=8, samples=12), True),
+                                         (wl.scaled(wl.CONFIGS[2], np_=7, samples=10), True),
+                                         (wl.scaled(wl.CONFIGS[3], nx=2, np_=6, samples=6), True)],
+                         ids=["glue_massless", "quarks_massive", "mixture_massive", "inhom_massive"])
+def test_paper_sampler_dF_parity_and_conservation(cfg, massive):
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=31)
+    o.set_f(f0)
+    g.set_f(f0)
+    if massive:
+        mo, mg = o.thermal_masses(), g.thermal_masses().numpy()
+        assert np.allclose(mg, mo, rtol=1e-12, atol=0)
+        g.set_masses(mo)                      # identical bits on both sides: the roots depend on them
+    dF_o = o.collision_paper(cfg.dt, 2)
+    dF_g = g.collision_paper(cfg.dt, 2).cpu().numpy()
+    gross = o.gross()
+    assert np.abs(dF_o).max() > 0
+    _assert_dF(dF_g, dF_o, gross, "paper sampler")
+    _assert_conserved(cfg, dF_g, gross)

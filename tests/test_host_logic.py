@@ -86,3 +86,25 @@ def test_factorised_channel_algebra_equals_channel_loop(species):
             assert abs(got.sum()) <= 1e-12 * gross              # Eq. 23: number units sum to zero
         done += 1
     assert done > 100
+
+
+@pytest.mark.parametrize("species", [(0,), (1, 2, 3, 4, 5, 6), (0, 1, 2, 3, 4, 5, 6), (0, 1, 2), (0, 1), (1, 2, 5), (0, 3, 4, 6)])
+def test_paper_sampler_channel_table_matches_oracle(species):
+    """The channel table of the paper sampler (bz_paper.cu, generated on the host) is the oracle's, as a set; channels of
+    one mass-class tuple are contiguous."""
+    from oracle import bzo
+    rows = bz.debug_paper_channels(species)
+    o = bzo.Oracle(np_=4, species=species)
+    want = sorted(tuple(int(v) for v in c) for c in o.channels())
+    got = sorted(tuple(int(v) for v in r[:6]) for r in rows)
+    assert got == want
+    cls = [0 if s == 0 else 1 + (s - 1) // 2 for s in species]
+    keys = [int(r[6]) for r in rows]
+    for r in rows:
+        assert int(r[6]) == cls[r[0]] | cls[r[1]] << 2 | cls[r[2]] << 4 | cls[r[3]] << 6
+    seen, last = set(), None
+    for k in keys:
+        if k != last:
+            assert k not in seen
+            seen.add(k)
+            last = k
