@@ -191,30 +191,49 @@ __global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* db
         const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
         const double* fx = P.f + (size_t)xcell * P.S * P.Np;
         double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+        // Mass classes with bit-identical masses (e.g. m_u = m_d = m_s for flavour-symmetric f, or all 0) have the same
+        // roots: every class is mapped to the first class with its mass, and all groups with the same mapped tuple share
+        // one root solve, one gather of the 4 x S occupation numbers and one flush of the deposits.
+        int rep[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            rep[c] = c;
+            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rep[c] = c2;
+        }
+        auto canon = [&](int key) { return rep[key & 3] | rep[(key >> 2) & 3] << 2 | rep[(key >> 4) & 3] << 4 | rep[(key >> 6) & 3] << 6; };
+        unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
         for (int gi = 0; gi < P.n_groups; ++gi) {
-            const PaperGroup G = P.groups[gi];
+            const int ck = canon(P.groups[gi].key);
+            if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
+            done[ck >> 5] |= 1u << (ck & 31);
             Root rt[2];
-            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[G.key & 3], m[(G.key >> 2) & 3], m[(G.key >> 4) & 3], m[(G.key >> 6) & 3], rt);
+            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], rt);
             for (int r = 0; r < nr; ++r) {
                 const Root& R = rt[r];
                 const double w = P.Kp / R.w_inv;
                 MsqSet M = msq_set<true, true>(R.s, R.t, R.u, mreg, P.g4 * w);
                 if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
                 const int cell[4] = { R.i1, R.i2, i3, i };
-                double acc[4][7];
+                double fv[4][7], acc[4][7];
 #pragma unroll
                 for (int sl = 0; sl < 4; ++sl)
 #pragma unroll
-                    for (int a = 0; a < 7; ++a) acc[sl][a] = 0.0;
-                for (int c = G.begin; c < G.end; ++c) {
-                    const PaperChannel ch = P.table[c];
-                    const double fa = fx[(size_t)ch.a * P.Np + cell[0]], fb = fx[(size_t)ch.b * P.Np + cell[1]];
-                    const double fc = fx[(size_t)ch.c * P.Np + cell[2]], fd = fx[(size_t)ch.d * P.Np + cell[3]];
-                    const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
-                    const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
-                    const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;                 // Eq. 5 bracket
-                    const double A = msq_pick(M, ch.kind, ch.crossed) * fwd;
-                    acc[0][ch.a] -= A; acc[1][ch.b] -= A; acc[2][ch.c] += A; acc[3][ch.d] += A;     // Eq. 22
+                    for (int a = 0; a < 7; ++a) {
+                        fv[sl][a] = a < P.S ? fx[(size_t)a * P.Np + cell[sl]] : 0.0;
+                        acc[sl][a] = 0.0;
+                    }
+                for (int gj = gi; gj < P.n_groups; ++gj) {
+                    const PaperGroup G = P.groups[gj];
+                    if (canon(G.key) != ck) continue;
+                    for (int c = G.begin; c < G.end; ++c) {
+                        const PaperChannel ch = P.table[c];
+                        const double fa = fv[0][ch.a], fb = fv[1][ch.b], fc = fv[2][ch.c], fd = fv[3][ch.d];
+                        const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
+                        const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
+                        const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
+                        const double A = msq_pick(M, ch.kind, ch.crossed) * fwd;
+                        acc[0][ch.a] -= A; acc[1][ch.b] -= A; acc[2][ch.c] += A; acc[3][ch.d] += A;   // Eq. 22
+                    }
                 }
 #pragma unroll
                 for (int sl = 0; sl < 4; ++sl)
