@@ -97,6 +97,44 @@ def vlasov_probe(g, cfg, dev, reps=5):
             "achieved": rate * bytes_per_value / 1e9, "unit": "GB/s"}
 
 
+def paper_probe(g, cfg, dev, fp64_peak, reps=2):
+    """NEXT rank 1, outside the timed step: the paper's own sampler (Eq. 17-21) with the thermal masses of
+    Eq. 8-9, on a bounded part of the bench workload (one z layer of spatial cells) so that it takes about a second."""
+    import torch
+    out = torch.empty(g.shape, dtype=torch.float64, device=dev)
+    masses = g.thermal_masses().numpy()
+    nz = cfg.nx if cfg.Nx > 1 else 1
+    g.set_slab(0, 0, 1)                                      # collide only the first z layer
+    cells = (cfg.Nx // nz) if cfg.Nx > 1 else 1
+    samples = cells * cfg.Np * cfg.samples
+    g.collision_paper(cfg.dt, 0, out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for r in range(reps):
+        g.collision_paper(cfg.dt, 1 + r, out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    # average number of roots kept per mass tuple, from the debug export on 64 grid points of spatial cell 0
+    m0 = masses[0]
+    cl, _ = g.debug_paper_samples(1, 0, 0, min(64, cfg.Np), (m0[0], m0[0], m0[0], m0[0]))
+    roots = float(cl[..., 1].double().mean())
+    g.set_slab(0, 0, nz)
+    cls = sorted({0 if s == 0 else 1 + (s - 1) // 2 for s in cfg.species})
+    distinct = len({float(m0[c]) for c in cls})               # mass classes with different masses in cell 0
+    n_ch = len(bz.debug_paper_channels(cfg.species))
+    tuples = min(n_ch, {1: 1, 2: 8}.get(distinct, distinct ** 4))
+    # fp64 operations per sample, counted on the oracle's source: root solve 70 per tuple; per kept root Table I 75 +
+    # weight 8; per channel and kept root 13 (bracket 7, x |M|^2, 4 deposits, 1 gross)
+    flop = tuples * 70.0 + roots * tuples * 83.0 + roots * n_ch * 13.0
+    rate = samples / (ms * 1e-3)
+    return {"kernel": "paper_kernel (bz_collision_paper)", "bound": "alu", "sample": "%d of %d spatial cells" % (cells, cfg.Nx),
+            "ms": ms, "samples_per_sec": rate, "mass_tuples": tuples, "roots_per_tuple": roots, "channels": n_ch,
+            "flop_per_sample": flop, "achieved": rate * flop / 1e12, "peak": fp64_peak, "unit": "TFLOP/s",
+            "frac": rate * flop / 1e12 / fp64_peak if fp64_peak else None}
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -194,6 +232,7 @@ def o_threads(o):
 
 
 def run_ours(args, cfg):
+    global bz
     import torch
     import torch.distributed as dist
 
@@ -283,6 +322,7 @@ def run_ours(args, cfg):
     g.set_profile(False)
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs) else None
+    rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs) else None
     clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
@@ -346,6 +386,7 @@ def run_ours(args, cfg):
                      "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; "
                              "the HBM one is the slower for every config and is the one reported"},
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
+        "next_rank1_paper_sampler": rank1,
         "next_rank2_eq15": None if rank2 is None else dict(rank2, peak=peak, frac=rank2["achieved"] / peak),
         "clocks": clocks,
         "total_particle_number": N1,
