@@ -86,7 +86,7 @@ struct Root {
 // Eq. 17-19 for one mass tuple: see oracle/bzo.c paper_roots for the algebra (two squarings of E1 + E2 = Et give
 // a z^2 - C Pz z + (Et^2 A1 - C^2/4) = 0).  Single rounded operations, the oracle's association order.
 __device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
-                                           double m1, double m2, double m3, double m4, Root (&out)[2])
+                                           double m1, double m2, double m3, double m4, int ixy1, int ixy2, Root (&out)[2])
 {
 #define MUL __dmul_rn
 #define ADD __dadd_rn
@@ -110,15 +110,19 @@ __device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)
     for (int sign = 0; sign < 2; ++sign) {
         const double z = __ddiv_rn(sign == 0 ? ADD(CP, sq) : SUB(CP, sq), a2);
         if (!(ADD(C, MUL(MUL(2.0, Pz), z)) >= 0.0)) continue;
+        // the box test of the two z components first (S9): most roots end here, before two square roots and two
+        // divisions; the transverse components of k1 and k2 do not depend on the root and were binned by the caller
+        const double k2z = SUB(Pz, z);
+        bool in1, in2;
+        const int b1 = bin_axis_exact(z, g, in1), b2 = bin_axis_exact(k2z, g, in2);
+        if (!(in1 && in2)) continue;
+        const int i1 = ixy1 + g.n * g.n * b1, i2 = ixy2 + g.n * g.n * b2;
         const double E1 = __dsqrt_rn(ADD(A1, MUL(z, z)));
         if (!(E1 <= Et)) continue;
-        const double k2z = SUB(Pz, z);
         const double E2 = __dsqrt_rn(ADD(A2, MUL(k2z, k2z)));
         if (!(E1 > 0.0 && E2 > 0.0)) continue;
         const double J = SUB(__ddiv_rn(z, E1), __ddiv_rn(k2z, E2));          // Eq. 19
         if (J == 0.0) continue;
-        const int i1 = bin_cell_exact(k1x, k1y, z, g), i2 = bin_cell_exact(qx, qy, k2z, g);
-        if (i1 < 0 || i2 < 0) continue;                                       // a leg outside the box (S9)
         Root& r = out[nr++];
         r.i1 = i1; r.i2 = i2;
         r.w_inv = fabs(J) * (((E1 * E2) * E3) * Ep);
@@ -151,9 +155,12 @@ __device__ __forceinline__ void red_add(double* dst, double v)
 }
 
 // mode 0: collision; mode 1: debug (writes the roots of one mass tuple instead of depositing)
+constexpr int kPaperThreads = 64;
+
 template <int kDebug>
-__global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* dbg_cells, double* dbg_stu)
+__global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams P, int* dbg_cells, double* dbg_stu)
 {
+    __shared__ double sh_fv[28 * kPaperThreads], sh_acc[28 * kPaperThreads];
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
         const int smp = (int)(q % P.Ns);
@@ -175,9 +182,21 @@ __global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* db
         const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
         const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
         const double* m = P.mass2 + 4 * (size_t)xcell;
+        // transverse cells of k1 (inside by construction) and of k2 = k3 + p - k1: the same for every mass tuple and root;
+        // a sample whose k2x or k2y leaves the box deposits nothing whatever the masses are (S9)
+        int ixy1, ixy2;
+        bool k2_in;
+        {
+            bool ia, ib, ic, id;
+            const int a1 = bin_axis_exact(k1x, P.g, ia), b1 = bin_axis_exact(k1y, P.g, ib);
+            const double qx = __dsub_rn(__dadd_rn(k3[0], p[0]), k1x), qy = __dsub_rn(__dadd_rn(k3[1], p[1]), k1y);
+            const int a2 = bin_axis_exact(qx, P.g, ic), b2 = bin_axis_exact(qy, P.g, id);
+            ixy1 = a1 + P.g.n * b1; ixy2 = a2 + P.g.n * b2;
+            k2_in = ia && ib && ic && id;
+        }
         if (kDebug) {
             Root rt[2];
-            const int nr = paper_roots(P.g, p, k3, k1x, k1y, P.dbg_msq[0], P.dbg_msq[1], P.dbg_msq[2], P.dbg_msq[3], rt);
+            const int nr = !k2_in ? 0 : paper_roots(P.g, p, k3, k1x, k1y, P.dbg_msq[0], P.dbg_msq[1], P.dbg_msq[2], P.dbg_msq[3], ixy1, ixy2, rt);
             int* oc = dbg_cells + 6 * q;
             double* os = dbg_stu + 6 * q;
             oc[0] = i3; oc[1] = nr;
@@ -187,7 +206,7 @@ __global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* db
             }
             continue;
         }
-        if (i3 < 0) continue;
+        if (i3 < 0 || !k2_in) continue;
         const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
         const double* fx = P.f + (size_t)xcell * P.S * P.Np;
         double* dx = P.dN + (size_t)xcell * P.S * P.Np;
@@ -201,44 +220,53 @@ __global__ void __launch_bounds__(128) paper_kernel(const PaperParams P, int* db
             for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rep[c] = c2;
         }
         auto canon = [&](int key) { return rep[key & 3] | rep[(key >> 2) & 3] << 2 | rep[(key >> 4) & 3] << 4 | rep[(key >> 6) & 3] << 6; };
+        // The 4 x S occupation numbers and the 4 x S deposit sums of the root being worked on live in shared memory,
+        // [entry][thread]: they are indexed by the channel table (run-time indices), which in registers would mean local
+        // memory; lanes of a warp read the same entry of consecutive threads, i.e. conflict-free.
+        double* fv = sh_fv + threadIdx.x;
+        double* acc = sh_acc + threadIdx.x;
         unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
         for (int gi = 0; gi < P.n_groups; ++gi) {
             const int ck = canon(P.groups[gi].key);
             if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
             done[ck >> 5] |= 1u << (ck & 31);
             Root rt[2];
-            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], rt);
+            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], ixy1, ixy2, rt);
             for (int r = 0; r < nr; ++r) {
                 const Root& R = rt[r];
                 const double w = P.Kp / R.w_inv;
                 MsqSet M = msq_set<true, true>(R.s, R.t, R.u, mreg, P.g4 * w);
                 if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+                const double mv[10] = { M.a_t, M.a_u, M.m11, M.m11, M.m1b_t, M.m1b_u, M.ann, M.ann, M.qqgg, M.qqgg };
                 const int cell[4] = { R.i1, R.i2, i3, i };
-                double fv[4][7], acc[4][7];
 #pragma unroll
                 for (int sl = 0; sl < 4; ++sl)
-#pragma unroll
-                    for (int a = 0; a < 7; ++a) {
-                        fv[sl][a] = a < P.S ? fx[(size_t)a * P.Np + cell[sl]] : 0.0;
-                        acc[sl][a] = 0.0;
+                    for (int a = 0; a < P.S; ++a) {
+                        fv[(sl * 7 + a) * kPaperThreads] = fx[(size_t)a * P.Np + cell[sl]];
+                        acc[(sl * 7 + a) * kPaperThreads] = 0.0;
                     }
                 for (int gj = gi; gj < P.n_groups; ++gj) {
                     const PaperGroup G = P.groups[gj];
                     if (canon(G.key) != ck) continue;
                     for (int c = G.begin; c < G.end; ++c) {
                         const PaperChannel ch = P.table[c];
-                        const double fa = fv[0][ch.a], fb = fv[1][ch.b], fc = fv[2][ch.c], fd = fv[3][ch.d];
+                        const double fa = fv[ch.a * kPaperThreads], fb = fv[(7 + ch.b) * kPaperThreads];
+                        const double fc = fv[(14 + ch.c) * kPaperThreads], fd = fv[(21 + ch.d) * kPaperThreads];
                         const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
                         const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
                         const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-                        const double A = msq_pick(M, ch.kind, ch.crossed) * fwd;
-                        acc[0][ch.a] -= A; acc[1][ch.b] -= A; acc[2][ch.c] += A; acc[3][ch.d] += A;   // Eq. 22
+                        const double Mv = ch.kind == 5 ? (ch.crossed ? M.qg_u : M.qg_t) : ch.kind == 6 ? M.gg : mv[2 * ch.kind + ch.crossed];
+                        const double A = Mv * fwd;
+                        acc[ch.a * kPaperThreads] -= A; acc[(7 + ch.b) * kPaperThreads] -= A;            // Eq. 22
+                        acc[(14 + ch.c) * kPaperThreads] += A; acc[(21 + ch.d) * kPaperThreads] += A;
                     }
                 }
 #pragma unroll
                 for (int sl = 0; sl < 4; ++sl)
-                    for (int a = 0; a < P.S; ++a)
-                        if (acc[sl][a] != 0.0) red_add(dx + (size_t)a * P.Np + cell[sl], acc[sl][a]);
+                    for (int a = 0; a < P.S; ++a) {
+                        const double v = acc[(sl * 7 + a) * kPaperThreads];
+                        if (v != 0.0) red_add(dx + (size_t)a * P.Np + cell[sl], v);
+                    }
             }
         }
     }
@@ -259,9 +287,9 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
-    long long blocks = (total + 127) / 128;
-    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
-    paper_kernel<0><<<(int)blocks, 128, 0, st>>>(P, nullptr, nullptr);
+    long long blocks = (total + kPaperThreads - 1) / kPaperThreads;
+    if (blocks > (long long)sms * 32) blocks = (long long)sms * 32;
+    paper_kernel<0><<<(int)blocks, kPaperThreads, 0, st>>>(P, nullptr, nullptr);
     ++g_launch_count;
     return cudaGetLastError();
 }
@@ -270,9 +298,9 @@ cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, in
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
-    long long blocks = (total + 127) / 128;
-    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
-    paper_kernel<1><<<(int)blocks, 128, 0, st>>>(P, cells, stu);
+    long long blocks = (total + kPaperThreads - 1) / kPaperThreads;
+    if (blocks > (long long)sms * 32) blocks = (long long)sms * 32;
+    paper_kernel<1><<<(int)blocks, kPaperThreads, 0, st>>>(P, cells, stu);
     ++g_launch_count;
     return cudaGetLastError();
 }
