@@ -321,8 +321,8 @@ def run_ours(args, cfg):
     tr_ms, tr_n = g.get_profile(1)
     g.set_profile(False)
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
-    rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs) else None
-    rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs) else None
+    rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs and not args.no_probes) else None
+    rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs and not args.no_probes) else None
     clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
@@ -413,6 +413,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=("ours", "reference"))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-probes", action="store_true", help="skip the NEXT-row probes that run after the timed steps (for profiling the step alone)")
     ap.add_argument("--slab", action="store_true", help="run the slab-decomposition path (the N > 1 path) even on one GPU")
     args = ap.parse_args()
     if args.warmup < 3:
