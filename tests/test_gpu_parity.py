@@ -488,3 +488,39 @@ def test_paper_sampler_dF_parity_and_conservation(cfg, massive):
     assert np.abs(dF_o).max() > 0
     _assert_dF(dF_g, dF_o, gross, "paper sampler")
     _assert_conserved(cfg, dF_g, gross)
+
+
+def test_eq15_and_thermal_masses_full_size_config3():
+    """NEXT rank 2 at the full size of config 3 (8^3 x 20^3 cells, 7 species: 28.7 M values), the launch configuration
+    bench.py probes: thermal masses over two iterations and the Eq. 15 increment, every value against the oracle."""
+    cfg = wl.CONFIGS[3]
+    o, g = _pair(cfg, threads=16)
+    f0 = wl.initial_f(cfg) + 1e-3 * wl.random_f(cfg, seed=2)
+    o.set_f(f0)
+    g.set_f(f0)
+    for _ in range(2):
+        mo, mg = o.thermal_masses(), g.thermal_masses().numpy()
+        assert np.allclose(mg, mo, rtol=1e-12, atol=0)
+    g.set_masses(mo)
+    dF_o, dF_g = o.vlasov(cfg.dt), g.vlasov(cfg.dt).cpu().numpy()
+    assert np.abs(dF_g - dF_o).max() <= 1e-13 * np.abs(dF_o).max()
+
+
+def test_paper_sampler_roots_bit_exact_on_the_config4_momentum_grid():
+    """NEXT rank 1 on config 4's momentum grid (24^3 over [-4, 4] GeV, 64 samples per cell), sampled grid points of a
+    spatial cell with a non-zero Philox offset: cells and (s, t, u) of every root bit-exact."""
+    cfg = wl.scaled(wl.CONFIGS[4], nx=2)
+    o, g = _pair(cfg)
+    o.set_slab(4090, 0, 2)
+    g.set_slab(4090, 0, 2)
+    msq = (0.21, 0.093, 0.21, 0.093)
+    for pb in (0, 6911, 13800):
+        cells, stu = g.debug_paper_samples(9, 5, pb, pb + 8, msq)
+        cells, stu = cells.cpu().numpy(), stu.cpu().numpy()
+        for k in range(8):
+            for smp in range(cfg.samples):
+                _, i3, roots = o.paper_sample(9, 5, pb + k, smp, msq)
+                assert cells[k, smp, 0] == i3 and cells[k, smp, 1] == len(roots)
+                for r, R in enumerate(roots):
+                    assert (cells[k, smp, 2 + 2 * r], cells[k, smp, 3 + 2 * r]) == (R.i1, R.i2)
+                    assert np.array_equal(stu[k, smp, 3 * r:3 * r + 3].view(np.uint64), np.array([R.s, R.t, R.u]).view(np.uint64))
