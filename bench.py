@@ -383,8 +383,10 @@ def run_ours(args, cfg):
                      "ms_per_launch": coll_ms / coll_n if coll_n else None,
                      "fp64_peak_tflops_measured": fp64_peak,
                      "fp64_bound_samples_per_sec": fp64_peak * 1e12 / FP64_FLOP_PER_SAMPLE.get(cfg.S, 1850.0) if fp64_peak else None,
-                     "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; "
-                             "the HBM one is the slower for every config and is the one reported"},
+                     "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; frac is "
+                             "against the HBM leg (measured denominator); the FP64 leg at SURVEY 8d's upper operation count "
+                             "and the measured FP64 peak is printed beside it (fp64_bound_samples_per_sec): the two legs "
+                             "meet within the uncertainty of the operation count (1200-1850 flop per sample)"},
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
         "next_rank1_paper_sampler": rank1,
         "next_rank2_eq15": None if rank2 is None else dict(rank2, peak=peak, frac=rank2["achieved"] / peak),
