@@ -136,19 +136,6 @@ __device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)
     return nr;
 }
 
-__device__ __forceinline__ double msq_pick(const MsqSet& M, int kind, int crossed)
-{
-    switch (kind) {
-    case 0: return crossed ? M.a_u : M.a_t;
-    case 1: return M.m11;
-    case 2: return crossed ? M.m1b_u : M.m1b_t;
-    case 3: return M.ann;
-    case 4: return M.qqgg;
-    case 5: return crossed ? M.qg_u : M.qg_t;
-    default: return M.gg;
-    }
-}
-
 __device__ __forceinline__ void red_add(double* dst, double v)
 {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst), "d"(v) : "memory");
