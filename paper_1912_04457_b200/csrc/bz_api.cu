@@ -513,7 +513,7 @@ static int paper_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
     }
     P.g = grid_const(c);
     P.f = c->f; P.dN = nullptr; P.mass2 = c->mass2; P.table = c->paper_table; P.groups = c->paper_groups;
-    P.n_groups = c->paper_n_groups; P.S = c->S; P.Np = c->Np; P.Ns = c->Ns;
+    P.n_groups = c->paper_n_groups; P.n_channels = c->paper_n_channels; P.S = c->S; P.Np = c->Np; P.Ns = c->Ns;
     const int layer = c->grid.nx * c->grid.ny;
     P.x_begin = c->zb * layer; P.x_count = (c->ze - c->zb) * layer; P.p_begin = 0; P.p_count = c->Np;
     P.seed = c->seed; P.step = step; P.x_rng_offset = c->xoff;

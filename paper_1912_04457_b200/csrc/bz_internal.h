@@ -47,7 +47,7 @@ struct PaperParams {
     const double* mass2;      // [Nx][4] thermal masses^2 (Eq. 8-9)
     const PaperChannel* table;
     const PaperGroup* groups;
-    int n_groups;
+    int n_groups, n_channels;
     int S, Np, Ns;
     int x_begin, x_count, p_begin, p_count;
     uint32_t seed, step, x_rng_offset;

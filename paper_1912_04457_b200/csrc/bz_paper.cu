@@ -259,6 +259,133 @@ __global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams 
     }
 }
 
+// ---- warp-cooperative version (the one bz_collision_paper launches) ------------------------------------------------
+// Only 0.14-0.16 roots per mass tuple survive the box test, so in the thread-per-sample kernel above a warp walks the
+// channel loop of every tuple with 6 of 32 lanes active (ncu).  Here the lanes of a warp still own one sample each for
+// the root solving, but every surviving root is then worked off by the WHOLE warp: the owner publishes the root's
+// |M|^2 values and cells in shared memory, lanes 0..27 gather the 4 x S occupation numbers, the 32 lanes take the
+// channels of the tuple 32 at a time, each adding its deposits to a private column of a [28][33] shared array, and
+// lanes 0..27 sum the rows and issue one RED per non-zero (slot, species).  A warp never spans two spatial cells, so
+// the loop over mass tuples is warp-uniform.
+constexpr int kCoopWarps = 4;
+struct CoopShared {
+    double M[14];              // |M|^2 x weight by 2 * kind + crossed
+    int cells[4];
+    double fv[28];             // f_a at the four cells, [slot * 7 + a]
+    double acc[28][33];        // deposits, one column per lane
+};
+
+__global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const PaperParams P)
+{
+    __shared__ CoopShared sh_all[kCoopWarps];
+    CoopShared& sh = sh_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const unsigned full = 0xffffffffu;
+    const long long per_x = (long long)P.p_count * P.Ns;
+    const long long chunks_per_x = (per_x + 31) / 32;
+    const long long n_items = chunks_per_x * P.x_count;
+    const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long item = warp0; item < n_items; item += n_warps) {
+        const int xcell = P.x_begin + (int)(item / chunks_per_x);
+        const long long local = (item % chunks_per_x) * 32 + lane;
+        const bool valid = local < per_x;
+        const long long lc = valid ? local : per_x - 1;
+        const int smp = (int)(lc % P.Ns), i = P.p_begin + (int)(lc / P.Ns);
+        double p[3], Emassless;
+        cell_kinematics(P.g, i, p[0], p[1], p[2], Emassless);
+        uint32_t w0[4], w1[4], w2[4];
+        const uint32_t xc = (uint32_t)xcell + P.x_rng_offset;
+        philox4x32_10(64u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w0);
+        philox4x32_10(65u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w1);
+        philox4x32_10(66u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w2);
+        double k3[3];
+        k3[0] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[0], w0[1]), P.g.L));
+        k3[1] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[2], w0[3]), P.g.L));
+        k3[2] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[0], w1[1]), P.g.L));
+        const double k1x = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[2], w1[3]), P.g.L));
+        const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
+        const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
+        int ixy1, ixy2;
+        bool live;
+        {
+            bool ia, ib, ic, id;
+            const int a1 = bin_axis_exact(k1x, P.g, ia), b1 = bin_axis_exact(k1y, P.g, ib);
+            const double qx = __dsub_rn(__dadd_rn(k3[0], p[0]), k1x), qy = __dsub_rn(__dadd_rn(k3[1], p[1]), k1y);
+            const int a2 = bin_axis_exact(qx, P.g, ic), b2 = bin_axis_exact(qy, P.g, id);
+            ixy1 = a1 + P.g.n * b1; ixy2 = a2 + P.g.n * b2;
+            live = valid && i3 >= 0 && ia && ib && ic && id;
+        }
+        const double* m = P.mass2 + 4 * (size_t)xcell;
+        const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
+        const double* fx = P.f + (size_t)xcell * P.S * P.Np;
+        double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+        int rep[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            rep[c] = c;
+            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rep[c] = c2;
+        }
+        auto canon = [&](int key) { return rep[key & 3] | rep[(key >> 2) & 3] << 2 | rep[(key >> 4) & 3] << 4 | rep[(key >> 6) & 3] << 6; };
+        unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
+        for (int gi = 0; gi < P.n_groups; ++gi) {                          // warp-uniform: one spatial cell per warp
+            const int ck = canon(P.groups[gi].key);
+            if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
+            done[ck >> 5] |= 1u << (ck & 31);
+            Root rt[2];
+            const int nr = live ? paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], ixy1, ixy2, rt) : 0;
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                unsigned owners = __ballot_sync(full, r < nr);
+                if (!owners) continue;
+                MsqSet M = {};
+                if (r < nr) {                                              // the owners, in parallel
+                    const double w = P.Kp / rt[r].w_inv;
+                    M = msq_set<true, true>(rt[r].s, rt[r].t, rt[r].u, mreg, P.g4 * w);
+                    if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+                }
+                while (owners) {
+                    const int L = __ffs(owners) - 1;
+                    owners &= owners - 1;
+                    if (lane == L) {
+                        sh.M[0] = M.a_t; sh.M[1] = M.a_u; sh.M[2] = M.m11; sh.M[3] = M.m11; sh.M[4] = M.m1b_t; sh.M[5] = M.m1b_u;
+                        sh.M[6] = M.ann; sh.M[7] = M.ann; sh.M[8] = M.qqgg; sh.M[9] = M.qqgg; sh.M[10] = M.qg_t; sh.M[11] = M.qg_u;
+                        sh.M[12] = M.gg; sh.M[13] = M.gg;
+                        sh.cells[0] = rt[r].i1; sh.cells[1] = rt[r].i2; sh.cells[2] = i3; sh.cells[3] = i;
+                    }
+                    __syncwarp();
+                    if (lane < 28) {
+                        const int a = lane % 7;
+                        sh.fv[lane] = a < P.S ? fx[(size_t)a * P.Np + sh.cells[lane / 7]] : 0.0;
+                    }
+#pragma unroll
+                    for (int k = 0; k < 28; ++k) sh.acc[k][lane] = 0.0;
+                    __syncwarp();
+                    for (int c = lane; c < P.n_channels; c += 32) {
+                        const PaperChannel ch = P.table[c];
+                        if (canon(ch.key) != ck) continue;
+                        const double fa = sh.fv[ch.a], fb = sh.fv[7 + ch.b], fc = sh.fv[14 + ch.c], fd = sh.fv[21 + ch.d];
+                        const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
+                        const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
+                        const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
+                        const double A = sh.M[2 * ch.kind + ch.crossed] * fwd;
+                        sh.acc[ch.a][lane] -= A; sh.acc[7 + ch.b][lane] -= A;                 // Eq. 22
+                        sh.acc[14 + ch.c][lane] += A; sh.acc[21 + ch.d][lane] += A;
+                    }
+                    __syncwarp();
+                    if (lane < 28) {
+                        double v = 0.0;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) v += sh.acc[lane][j];
+                        const int a = lane % 7;
+                        if (a < P.S && v != 0.0) red_add(dx + (size_t)a * P.Np + sh.cells[lane / 7], v);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    }
+}
+
 __global__ void __launch_bounds__(256) paper_finalize_kernel(double* __restrict__ dF, size_t n_values, int S, int Np, const double d0,
                                                               const double d1, const double d2, const double d3, const double d4,
                                                               const double d5, const double d6)
@@ -274,9 +401,9 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
-    long long blocks = (total + kPaperThreads - 1) / kPaperThreads;
-    if (blocks > (long long)sms * 32) blocks = (long long)sms * 32;
-    paper_kernel<0><<<(int)blocks, kPaperThreads, 0, st>>>(P, nullptr, nullptr);
+    long long blocks = (total / 32 + kCoopWarps) / kCoopWarps;
+    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    paper_coop_kernel<<<(int)blocks, 32 * kCoopWarps, 0, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }
