@@ -121,10 +121,11 @@ def paper_probe(g, cfg, dev, fp64_peak, reps=2):
     cl, _ = g.debug_paper_samples(1, 0, 0, min(64, cfg.Np), (m0[0], m0[0], m0[0], m0[0]))
     roots = float(cl[..., 1].double().mean())
     g.set_slab(0, 0, nz)
-    cls = sorted({0 if s == 0 else 1 + (s - 1) // 2 for s in cfg.species})
-    distinct = len({float(m0[c]) for c in cls})               # mass classes with different masses in cell 0
-    n_ch = len(bz.debug_paper_channels(cfg.species))
-    tuples = min(n_ch, {1: 1, 2: 8}.get(distinct, distinct ** 4))
+    # distinct mass tuples of spatial cell 0: classes (g, u, d, s) with bit-identical masses share their roots
+    rep = [min(c2 for c2 in range(c + 1) if float(m0[c2]) == float(m0[c])) for c in range(4)]
+    table = bz.debug_paper_channels(cfg.species)
+    n_ch = len(table)
+    tuples = len({tuple(rep[(int(k) >> (2 * leg)) & 3] for leg in range(4)) for k in table[:, 6]})
     # fp64 operations per sample, counted on the oracle's source: root solve 70 per tuple; per kept root Table I 75 +
     # weight 8; per channel and kept root 13 (bracket 7, x |M|^2, 4 deposits, 1 gross)
     flop = tuples * 70.0 + roots * tuples * 83.0 + roots * n_ch * 13.0

@@ -5,9 +5,10 @@
 //   Eq. 8-9; symmetrical sampling (Eq. 22): the same weight goes to the cells of k1, k2 (-) and k3, p (+).
 // With masses the kinematics depend on the species of the four legs, so a sample is NOT shared by all channels as in
 // the hot path: the ordered channels (S8c step 5) are grouped by their tuple of mass classes (g, u, d, s) and every
-// group solves its own roots.  One thread per (spatial cell, grid point, sample); the deposits of a root are summed
-// per (slot, species) in a small local array and leave as fp64 reductions (RED.E.ADD.F64) into dF, which a second
-// kernel divides by N_a.  Everything that decides a cell index uses single correctly rounded operations in the
+// group solves its own roots.  One lane per (spatial cell, grid point, sample) for the root solving; the surviving roots
+// are worked off by the whole warp (paper_coop_kernel), their deposits summed per (slot, species) in shared memory and
+// issued as fp64 reductions (RED.E.ADD.F64) into dF, which a second kernel divides by N_a.  The thread-per-sample
+// kernel (paper_kernel) is kept for the debug export of the roots.  Everything that decides a cell index uses single correctly rounded operations in the
 // association order of the oracle (bit-exact sampled cells).
 #include <vector>
 
