@@ -286,6 +286,9 @@ __global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const Paper
     const long long chunks_per_x = (per_x + 31) / 32;
     const long long n_items = chunks_per_x * P.x_count;
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
+#pragma unroll
+    for (int k = 0; k < 28; ++k) sh.acc[k][lane] = 0.0;       // kept all-zero between roots: a reducer re-zeroes its row
+    __syncwarp();
     for (long long item = warp0; item < n_items; item += n_warps) {
         const int xcell = P.x_begin + (int)(item / chunks_per_x);
         const long long local = (item % chunks_per_x) * 32 + lane;
@@ -320,18 +323,24 @@ __global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const Paper
         const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
         const double* fx = P.f + (size_t)xcell * P.S * P.Np;
         double* dx = P.dN + (size_t)xcell * P.S * P.Np;
-        int rep[4];
+        unsigned rep = 0u;                                 // 2 bits per class: the first class with the same mass
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-            rep[c] = c;
-            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rep[c] = c2;
+            int rc = c;
+            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rc = c2;
+            rep |= (unsigned)rc << (2 * c);
         }
-        auto canon = [&](int key) { return rep[key & 3] | rep[(key >> 2) & 3] << 2 | rep[(key >> 4) & 3] << 4 | rep[(key >> 6) & 3] << 6; };
+        auto rp = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
+        auto canon = [&](int key) { return rp(key & 3) | rp((key >> 2) & 3) << 2 | rp((key >> 4) & 3) << 4 | rp((key >> 6) & 3) << 6; };
         unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
         for (int gi = 0; gi < P.n_groups; ++gi) {                          // warp-uniform: one spatial cell per warp
             const int ck = canon(P.groups[gi].key);
             if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
             done[ck >> 5] |= 1u << (ck & 31);
+            // this lane's channels of the tuple (c = lane + 32 k), found once per tuple, not once per root
+            unsigned mine = 0u;
+            for (int k = 0; lane + 32 * k < P.n_channels && k < 8; ++k)
+                if (canon(P.table[lane + 32 * k].key) == ck) mine |= 1u << k;
             Root rt[2];
             const int nr = live ? paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], ixy1, ixy2, rt) : 0;
 #pragma unroll
@@ -358,12 +367,11 @@ __global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const Paper
                         const int a = lane % 7;
                         sh.fv[lane] = a < P.S ? fx[(size_t)a * P.Np + sh.cells[lane / 7]] : 0.0;
                     }
-#pragma unroll
-                    for (int k = 0; k < 28; ++k) sh.acc[k][lane] = 0.0;
                     __syncwarp();
-                    for (int c = lane; c < P.n_channels; c += 32) {
-                        const PaperChannel ch = P.table[c];
-                        if (canon(ch.key) != ck) continue;
+                    unsigned rows = 0u;                        // rows of sh.acc this lane touches
+                    for (unsigned left = mine; left; left &= left - 1u) {
+                        const PaperChannel ch = P.table[lane + 32 * (__ffs(left) - 1)];
+                        rows |= 1u << ch.a | 1u << (7 + ch.b) | 1u << (14 + ch.c) | 1u << (21 + ch.d);
                         const double fa = sh.fv[ch.a], fb = sh.fv[7 + ch.b], fc = sh.fv[14 + ch.c], fd = sh.fv[21 + ch.d];
                         const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
                         const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
@@ -372,13 +380,13 @@ __global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const Paper
                         sh.acc[ch.a][lane] -= A; sh.acc[7 + ch.b][lane] -= A;                 // Eq. 22
                         sh.acc[14 + ch.c][lane] += A; sh.acc[21 + ch.d][lane] += A;
                     }
+                    rows = __reduce_or_sync(full, rows);
                     __syncwarp();
-                    if (lane < 28) {
+                    if ((rows >> lane) & 1u) {                 // lane < 28: sum the row, re-zero it, one reduction
                         double v = 0.0;
 #pragma unroll
-                        for (int j = 0; j < 32; ++j) v += sh.acc[lane][j];
-                        const int a = lane % 7;
-                        if (a < P.S && v != 0.0) red_add(dx + (size_t)a * P.Np + sh.cells[lane / 7], v);
+                        for (int j = 0; j < 32; ++j) { v += sh.acc[lane][j]; sh.acc[lane][j] = 0.0; }
+                        if (v != 0.0) red_add(dx + (size_t)(lane % 7) * P.Np + sh.cells[lane / 7], v);
                     }
                     __syncwarp();
                 }
