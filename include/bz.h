@@ -128,6 +128,12 @@ int bz_vlasov(bz_ctx* ctx, double dt_fm, double* dF_dev);
  * bz_set_msq_override. */
 int bz_collision_paper(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
 
+/* Collision term used by bz_step: 0 (default, NS) = the massless centre-of-mass sampler of bz_collision; 1 = the
+ * paper's own sampler of bz_collision_paper.  With mode 1 and transport scheme 1, bz_step is the paper's program as a
+ * whole: thermal masses from the old f (Eq. 8-9), collision term by Eq. 17-21 with those masses, Eq. 15 for the
+ * drift and force terms, forward Euler.  -1 on a bad mode. */
+int bz_set_collision(bz_ctx* ctx, int mode);
+
 /* Test-only: the roots of the paper sampler for ONE mass tuple msq_host = (m_a^2, m_b^2, m_c^2, m_d^2), p1 cells
  * [pcell_begin, pcell_end) of spatial cell xcell: cells_dev[n][Ns][6] = (cell of k3, number of roots kept, cell of k1
  * and of k2 for root 0, the same for root 1; -1 where there is none), stu_dev[n][Ns][6] = (s, t, u) of root 0 and 1. */
@@ -141,8 +147,8 @@ int bz_debug_paper_channels(const int* species, int n_species, int* out_host, in
 
 /* Transport scheme used by bz_step: 0 (default, NS) = first-order upwind drift with massless velocities (bz_stream);
  * 1 = Eq. 15 (bz_vlasov) with the thermal masses re-evaluated from the old f at the start of every step;
- * 2 = Eq. 15 with the masses as stored (bz_set_masses / the last bz_thermal_masses).  The collision term is NS's
- * massless one in every scheme (the massive collision kinematics of the paper are NEXT rank 1, not built). */
+ * 2 = Eq. 15 with the masses as stored (bz_set_masses / the last bz_thermal_masses).  The collision term is chosen
+ * independently with bz_set_collision. */
 int bz_set_transport(bz_ctx* ctx, int scheme);
 
 /* One forward-Euler step (Eq. 15 unsplit; S8a.7): f <- (f + dF_stream) + dF_coll with both increments

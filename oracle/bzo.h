@@ -83,6 +83,8 @@ int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 /* transport used by bzo_step: 0 = upwind massless (default), 1 = Eq. 15 with the masses re-evaluated from the old f
  * every step, 2 = Eq. 15 with the masses as stored */
 int  bzo_set_transport(bzo_ctx*, int scheme);
+/* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper */
+int  bzo_set_collision(bzo_ctx*, int mode);
 /* ---- NEXT rank 1 (S8f): the paper's own collision path (Eq. 17-21, massive dispersion) ----------------------------
  * one root of E1 + E2 = E3 + Ep (Eq. 18-19): momenta k1, k2, their cells, the four energies, the Jacobian of Eq. 19 and
  * the massive Mandelstam variables */

@@ -62,6 +62,7 @@ def lib():
         L.bzo_thermal_masses.argtypes = [vp, dp]
         L.bzo_vlasov.argtypes = [vp, C.c_double, dp]
         L.bzo_set_transport.argtypes = [vp, C.c_int]
+        L.bzo_set_collision.argtypes = [vp, C.c_int]
         L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
         L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_moments.argtypes = [vp, dp]
@@ -217,6 +218,9 @@ class Oracle:
         dF = np.empty(self.shape, dtype=np.float64)
         _chk(lib().bzo_collision_paper(self._h, dt, step, _dptr(dF)), "bzo_collision_paper")
         return dF
+
+    def set_collision(self, mode):
+        _chk(lib().bzo_set_collision(self._h, mode), "bzo_set_collision")
 
     def set_transport(self, scheme):
         _chk(lib().bzo_set_transport(self._h, scheme), "bzo_set_transport")

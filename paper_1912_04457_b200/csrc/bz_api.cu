@@ -169,7 +169,7 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false; c->copy_in = nullptr; c->copy_out = nullptr;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
-    c->mass2 = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
+    c->mass2 = nullptr; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
@@ -233,7 +233,7 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->paper_table); cudaFree(c->paper_groups);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     for (cudaEvent_t e : c->pipe_events) cudaEventDestroy(e);
     if (c->copy_in) cudaStreamDestroy(c->copy_in);
@@ -395,10 +395,29 @@ int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
     return run_vlasov(c, dt_fm, dF_dev);
 }
 
+int bz_set_collision(bz_ctx* c, int mode) { if (!c || mode < 0 || mode > 1) return -1; c->coll_mode = mode; return 0; }
+
+// bz_step with the paper's own collision term (rank 1): masses (scheme 1), bz_collision_paper into a scratch, the
+// transport increment of the chosen scheme into f_new, then f_new = (f + dF_transport) + dF_coll
+static int step_paper(bz_ctx* c, double dt_fm)
+{
+    if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f, used by both terms
+    if (!c->dF_scratch) BZ_CUDA(cudaMalloc(&c->dF_scratch, c->n_values * sizeof(double)), "cudaMalloc dF scratch");
+    if (int rc = bz_collision_paper(c, dt_fm, c->step, c->dF_scratch)) return rc;
+    if (c->scheme == 0) BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 0, c->stream), "stream");
+    else if (int rc = run_vlasov(c, dt_fm, c->f_new)) return rc;
+    BZ_CUDA(launch_combine(c->f, c->f_new, c->dF_scratch, c->n_values, c->stream), "combine");
+    double* t = c->f; c->f = c->f_new; c->f_new = t;
+    c->rowsum_valid = false; c->aos_valid = false;
+    c->step += 1;
+    return 0;
+}
+
 int bz_step(bz_ctx* c, double dt_fm)
 {
     if (!c) return -1;
     if (!c->f) return -4;
+    if (c->coll_mode == 1) return step_paper(c, dt_fm);
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, c->step)) return rc;
     if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f
@@ -426,7 +445,7 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
     const int nzl = c->grid.nz, layer_cells = c->grid.nx * c->grid.ny;
     const int lpc = (nzl + 15) / 16;                             // z layers per chunk: at most 16 chunks
     const int K = (nzl + lpc - 1) / lpc;
-    if (c->scheme != 0 || K < 3) {                               // nothing to overlap (or Eq. 15 transport): the plain sequence
+    if (c->scheme != 0 || c->coll_mode != 0 || K < 3) {                               // nothing to overlap (or Eq. 15 transport): the plain sequence
         if (int rc = bz_set_f(c, f_in_host, 0)) return rc;
         if (int rc = bz_step(c, dt_fm)) return rc;
         return bz_get_f(c, f_out_host, 0);

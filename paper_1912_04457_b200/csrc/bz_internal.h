@@ -87,6 +87,8 @@ struct bz_ctx_impl {
     PaperChannel* paper_table;       // device: channel table of the paper sampler (built at the first bz_collision_paper)
     PaperGroup* paper_groups;        // device
     int paper_n_groups, paper_n_channels;
+    int coll_mode;                   // bz_set_collision: 0 CM sampler (hot path), 1 the paper's sampler (bz_collision_paper)
+    double* dF_scratch;              // device n_values, allocated at the first bz_step with coll_mode 1
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
@@ -148,6 +150,8 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
 void build_paper_channels(const int* species, int S, std::vector<PaperChannel>& table, std::vector<PaperGroup>& groups);
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st);
 cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, int sms, cudaStream_t st);
+// out = (f + out) + dFc (forward Euler with both increments given, the oracle's association)
+cudaError_t launch_combine(const double* f, double* out, const double* dFc, size_t n_values, cudaStream_t st);
 cudaError_t launch_paper_finalize(double* dF, size_t n_values, int S, int Np, const double* deg, cudaStream_t st);
 
 }  // namespace bz

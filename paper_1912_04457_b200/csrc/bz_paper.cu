@@ -404,7 +404,21 @@ __global__ void __launch_bounds__(256) paper_finalize_kernel(double* __restrict_
         dF[q] = dF[q] / deg[(q / Np) % S];
 }
 
+__global__ void __launch_bounds__(256) combine_kernel(const double* __restrict__ f, double* __restrict__ out,
+                                                      const double* __restrict__ dFc, size_t n_values)
+{
+    for (size_t q = blockIdx.x * (size_t)blockDim.x + threadIdx.x; q < n_values; q += (size_t)gridDim.x * blockDim.x)
+        out[q] = (f[q] + out[q]) + dFc[q];
+}
+
 }  // namespace
+
+cudaError_t launch_combine(const double* f, double* out, const double* dFc, size_t n_values, cudaStream_t st)
+{
+    combine_kernel<<<148 * 8, 256, 0, st>>>(f, out, dFc, n_values);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {

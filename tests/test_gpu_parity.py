@@ -524,3 +524,34 @@ def test_paper_sampler_roots_bit_exact_on_the_config4_momentum_grid():
                 for r, R in enumerate(roots):
                     assert (cells[k, smp, 2 + 2 * r], cells[k, smp, 3 + 2 * r]) == (R.i1, R.i2)
                     assert np.array_equal(stu[k, smp, 3 * r:3 * r + 3].view(np.uint64), np.array([R.s, R.t, R.u]).view(np.uint64))
+
+
+@pytest.mark.parametrize("scheme", [0, 1, 2])
+def test_step_with_the_papers_collision_term(scheme):
+    """bz_set_collision(1): bz_step with the paper's sampler; with transport scheme 1 this is the paper's program as a
+    whole (masses from the old f, Eq. 17-21, Eq. 15, forward Euler).  f after 3 steps against the oracle."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=6, samples=6)
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=41) * 0.5
+    for e in (o, g):
+        e.set_f(f0)
+        e.set_collision(1)
+        e.set_transport(scheme)
+        if scheme == 2:
+            e.set_masses(np.tile([0.5, 0.2, 0.25, 0.3], (cfg.Nx, 1)))
+    for _ in range(3):
+        o.step(cfg.dt)
+        g.step(cfg.dt)
+    f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
+    assert np.abs(f_o - f0).max() > 0
+    assert np.abs(f_g - f_o).max() <= 1e-11 * np.abs(f_o).max()
+    mo, mg = o.moments(), g.moments()
+    assert np.allclose(mg["tot"].numpy(), mo["tot"], rtol=1e-12, atol=0)
+    # back to the hot path: the cell-major copy is rebuilt and the next step is the CM sampler's again
+    for e in (o, g):
+        e.set_collision(0)
+        e.set_transport(0)
+    o.step(cfg.dt)
+    g.step(cfg.dt)
+    f_o = o.get_f()
+    assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= 1e-11 * np.abs(f_o).max()

@@ -172,3 +172,20 @@ def test_R4b_massless_limit_agrees_with_cm_sampler_number_changing_channels():
     assert c.mean(0)[0] < 0 and np.all(c.mean(0)[1:] > 0)
     assert np.all(ea < 0.03 * np.abs(c.mean(0)))
     assert np.all(np.abs(a.mean(0) - c.mean(0)) < 4 * np.hypot(ea, ec) + 0.03 * np.abs(c.mean(0)))
+
+
+def test_R5_full_program_step_conserves_particle_number():
+    """The paper's program as a whole (bzo_set_collision(1) + bzo_set_transport(1)): masses from the old f, Eq. 17-21,
+    Eq. 15, Euler.  Total particle number is conserved step after step (Eq. 13 + Eq. 22-23); the masses move with f."""
+    o = bzo.Oracle(nx=2, ny=2, nz=1, dx=0.3, np_=5, pmin=-3.0, pmax=3.0, species=(0, 1, 2), samples=20, seed=6)
+    rng = np.random.default_rng(8)
+    o.set_f(rng.uniform(0.05, 0.5, size=o.shape))
+    o.set_collision(1)
+    o.set_transport(1)
+    N0 = o.moments()["tot"][:, 0].sum()
+    masses = []
+    for _ in range(3):
+        o.step(0.01)
+        masses.append(o.get_masses().copy())
+        assert o.moments()["tot"][:, 0].sum() == pytest.approx(N0, rel=1e-13)
+    assert (masses[0] > 0).all() and not np.array_equal(masses[0], masses[2])
