@@ -108,6 +108,13 @@ int bz_stream(bz_ctx* ctx, double dt_fm, double* dF_dev);
 int bz_thermal_masses(bz_ctx* ctx, double* out_host);
 int bz_set_masses(bz_ctx* ctx, const double* mass2_host);
 
+/* Energy balance with dynamical masses (Eq. 11-12; Eq. 26), written to HOST memory, 5 doubles per
+ * spatial cell: out[x][0] = T^00_kin(x) = sum_a N_a sum_cells d3p E_p^a f_a / (2pi)^3 (GeV^4), out[x][1 + c] = Q_c(x) =
+ * sum_{a in mass class c} N_a sum_cells d3p f_a / ((2pi)^3 E_p^a) (GeV^2) for c = g, u, d, s, with E_p^a from the
+ * stored masses.  The source term of Eq. 12 is S_ex^nu = (1/2) sum_c (d^nu m_c^2) Q_c; Eq. 26 compares d_0 T^00_kin with
+ * S_ex^0 (the caller differences T^00 and the masses over steps, as the paper does for Fig. 6).  Synchronises. */
+int bz_energy_diag(bz_ctx* ctx, double* out_host);
+
 /* dF = -dt { drift + force } of Eq. 15, the central-difference form of the left-hand side of Eq. 13
  * (P:133), with E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses; periodic in x and in p.  Per axis i:
  *   drift_i = [ p_i f_p(x+)/E_p(x+) - p_i f_p(x-)/E_p(x-) ] / (2 dx)

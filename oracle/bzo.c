@@ -543,6 +543,38 @@ int bzo_thermal_masses(bzo_ctx* c, double* out)
     return 0;
 }
 
+/* Energy balance with x- and t-dependent masses (Eq. 11-12; Eq. 26): per spatial cell
+ *   out[x][0]     = T^00_kin(x) = sum_a N_a sum_cells d3p/(2pi)^3 E_p^a f_a            (Eq. 11, mu = nu = 0; GeV^4)
+ *   out[x][1 + c] = Q_c(x) = sum_{a in mass class c} N_a sum_cells d3p/((2pi)^3 E_p^a) f_a   (c = g, u, d, s; GeV^2)
+ * with E_p^a = sqrt(p^2 + m_a^2(x)) from the stored masses (a cell with E = 0 is skipped in Q, S10), so that the
+ * source term of Eq. 12 is S_ex^nu = (1/2) sum_c (d^nu m_c^2) Q_c. */
+int bzo_energy_diag(const bzo_ctx* c, double* out)
+{
+    if (!c || !out) return -1;
+    const double pi = 3.14159265358979323846;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const double dp = cell_width(c), d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * pi) * (2.0 * pi) * (2.0 * pi);
+    for (int x = 0; x < c->Nx; ++x) {
+        double* o = out + 5 * (size_t)x;
+        for (int k = 0; k < 5; ++k) o[k] = 0.0;
+        for (int a = 0; a < S; ++a) {
+            const int id = c->species[a], cls = mass_class(id);
+            const double Na = degeneracy(id), m2 = c->mass2[4 * (size_t)x + cls];
+            const double* fa = c->f + ((size_t)x * S + a) * Np;
+            double se = 0.0, sq = 0.0;
+            for (int pc = 0; pc < Np; ++pc) {
+                const double E = energy_at(c, pc % n, (pc / n) % n, pc / (n * n), m2);
+                se += E * fa[pc];
+                if (E > 0.0) sq += fa[pc] / E;
+            }
+            o[0] += Na * se * d3p / twopi3;
+            o[1 + cls] += Na * sq * d3p / twopi3;
+        }
+    }
+    return 0;
+}
+
 /* dF = -dt * { drift + force } of Eq. 15, the central-difference form of the left-hand side of Eq. 13 with
  * E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses; periodic in x AND in p.  Per axis i:
  *   drift_i = [ p_i f_p(x+) / E_p(x+) - p_i f_p(x-) / E_p(x-) ] / (2 dx)

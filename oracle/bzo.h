@@ -77,6 +77,9 @@ int  bzo_stream   (bzo_ctx*, double dt_fm, double* dF);
 int  bzo_set_masses(bzo_ctx*, const double* mass2);
 int  bzo_get_masses(const bzo_ctx*, double* mass2);
 int  bzo_thermal_masses(bzo_ctx*, double* out);
+/* energy balance (Eq. 11-12, 26): out[x][5] = T^00_kin(x), then Q_c(x) = sum_{a in class c} N_a int d3p f_a/((2pi)^3 E^a)
+ * for c = g, u, d, s, with E^a = sqrt(p^2 + m_a^2(x)) from the stored masses; S_ex^nu = (1/2) sum_c (d^nu m_c^2) Q_c */
+int  bzo_energy_diag(const bzo_ctx*, double* out);
 /* dF = -dt { drift + force } of Eq. 15: central differences in x and p, periodic in both,
  * E_p^a(x) = sqrt(p^2 + m_a^2(x)) from the stored masses */
 int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);

@@ -63,6 +63,7 @@ def lib():
         L.bzo_vlasov.argtypes = [vp, C.c_double, dp]
         L.bzo_set_transport.argtypes = [vp, C.c_int]
         L.bzo_set_collision.argtypes = [vp, C.c_int]
+        L.bzo_energy_diag.argtypes = [vp, dp]
         L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
         L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_moments.argtypes = [vp, dp]
@@ -224,6 +225,11 @@ class Oracle:
 
     def set_transport(self, scheme):
         _chk(lib().bzo_set_transport(self._h, scheme), "bzo_set_transport")
+
+    def energy_diag(self):
+        out = np.empty((self.Nx, 5), dtype=np.float64)
+        _chk(lib().bzo_energy_diag(self._h, _dptr(out)), "bzo_energy_diag")
+        return out
 
     def vlasov(self, dt):
         dF = np.empty(self.shape, dtype=np.float64)

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
-           "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
+           "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
            "bz_debug_deposit_host")
@@ -51,6 +51,7 @@ def lib():
         L.bz_step_host.argtypes = [vp, C.c_double, vp, vp]
         L.bz_collision_paper.argtypes = [vp, C.c_double, C.c_uint, vp]
         L.bz_set_collision.argtypes = [vp, C.c_int]
+        L.bz_energy_diag.argtypes = [vp, vp]
         L.bz_debug_paper_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, vp, vp]
         L.bz_debug_paper_channels.argtypes = [ip, C.c_int, ip, C.c_int]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
@@ -209,6 +210,11 @@ class Boltzmann:
         if t.numel() != self.Nx * 4 or t.is_cuda:
             raise ValueError("mass2: host array of Nx*4 doubles")
         self._chk(lib().bz_set_masses(self._h, C.c_void_p(t.data_ptr())), "bz_set_masses")
+
+    def energy_diag(self):
+        out = torch.empty((self.Nx, 5), dtype=torch.float64)
+        self._chk(lib().bz_energy_diag(self._h, C.c_void_p(out.data_ptr())), "bz_energy_diag")
+        return out
 
     def vlasov(self, dt, out=None):
         if out is None:

@@ -388,6 +388,24 @@ int bz_thermal_masses(bz_ctx* c, double* out_host)
     return 0;
 }
 
+int bz_energy_diag(bz_ctx* c, double* out_host)
+{
+    if (!c || !out_host) return -1;
+    if (!c->f) return -4;
+    unsigned cls, ids;
+    class_bits(c, cls, ids);
+    const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
+    const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
+    double* diag = nullptr;                                   // small and rare: allocated per call
+    BZ_CUDA(cudaMalloc(&diag, (size_t)c->Nx * 5 * sizeof(double)), "cudaMalloc diag");
+    cudaError_t e = launch_energy_diag(c->f, c->cell_tab, c->mass2, diag, c->Nx, c->S, c->Np, cls, ids, d3p / twopi3, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, diag, (size_t)c->Nx * 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(diag);
+    if (e != cudaSuccess) return fail_cuda(c, e, "bz_energy_diag");
+    return 0;
+}
+
 int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;

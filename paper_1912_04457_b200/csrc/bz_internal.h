@@ -142,6 +142,8 @@ cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, 
 // NEXT rank 2 (bz_vlasov.cu): thermal masses of Eq. 8-9 and the central-difference drift + force of Eq. 15
 cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, double* mass2, int Nx, int S, int Np,
                                   unsigned cls_bits, unsigned id_bits, double g2, double w, cudaStream_t st);
+cudaError_t launch_energy_diag(const double* f, const double* cell_tab, const double* mass2, double* diag, int Nx, int S, int Np,
+                               unsigned cls_bits, unsigned id_bits, double w, cudaStream_t st);
 cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, int S, int Np, const double* cell_tab,
                           const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
                           double dx, double dp, unsigned cls_bits, cudaStream_t st);

@@ -54,6 +54,43 @@ __global__ void __launch_bounds__(256) mass_kernel(const double* __restrict__ f,
     }
 }
 
+// Energy balance (Eq. 11-12, 26): diag[x][0] = T^00_kin(x), diag[x][1 + c] = Q_c(x) for the mass classes c = g, u, d, s
+__global__ void __launch_bounds__(256) diag_kernel(const double* __restrict__ f, const double* __restrict__ cell_tab,
+                                                   const double* __restrict__ mass2, double* __restrict__ diag, int S, int Np,
+                                                   unsigned cls_bits, unsigned id_bits, double w /* d3p / (2 pi)^3 */)
+{
+    const int x = blockIdx.x;
+    __shared__ double part[2][7][8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int a = 0; a < S; ++a) {
+        const double m2 = mass2[4 * (size_t)x + class_of(cls_bits, a)];
+        const double* fa = f + ((size_t)x * S + a) * Np;
+        double se = 0.0, sq = 0.0;
+        for (int pc = threadIdx.x; pc < Np; pc += blockDim.x) {
+            const double2 u = __ldg(reinterpret_cast<const double2*>(cell_tab) + 2 * (size_t)pc);
+            const double pz = __ldg(cell_tab + 4 * (size_t)pc + 2);
+            const double E = sqrt(((u.x * u.x + u.y * u.y) + pz * pz) + m2), v = fa[pc];
+            se += E * v;
+            if (E > 0.0) sq += v / E;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { se += __shfl_xor_sync(0xffffffffu, se, o); sq += __shfl_xor_sync(0xffffffffu, sq, o); }
+        if (lane == 0) { part[0][a][warp] = se; part[1][a][warp] = sq; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double out[5] = { 0, 0, 0, 0, 0 };
+        for (int a = 0; a < S; ++a) {
+            double te = 0.0, tq = 0.0;
+            for (int q = 0; q < 8; ++q) { te += part[0][a][q]; tq += part[1][a][q]; }
+            const double Na = ((id_bits >> (3 * a)) & 7u) == 0u ? 16.0 : 6.0;      // N_g, N_q
+            out[0] += Na * te * w;
+            out[1 + class_of(cls_bits, a)] += Na * tq * w;
+        }
+        for (int k = 0; k < 5; ++k) diag[5 * (size_t)x + k] = out[k];
+    }
+}
+
 // E_tab[(x*4 + cls)*Np + pc] = sqrt(p^2 + m_cls^2(x)) for the mass classes present: one square root per entry, so
 // that the stencil kernel below reads its 18 energies per (cell, class) instead of recomputing them
 __global__ void __launch_bounds__(256) energy_kernel(const double* __restrict__ cell_tab, const double* __restrict__ mass2,
@@ -146,6 +183,14 @@ cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, doubl
                                   unsigned cls_bits, unsigned id_bits, double g2, double w, cudaStream_t st)
 {
     mass_kernel<<<Nx, 256, 0, st>>>(f, cell_tab, mass2, S, Np, cls_bits, id_bits, g2, w);
+    ++g_launch_count;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_energy_diag(const double* f, const double* cell_tab, const double* mass2, double* diag, int Nx, int S, int Np,
+                               unsigned cls_bits, unsigned id_bits, double w, cudaStream_t st)
+{
+    diag_kernel<<<Nx, 256, 0, st>>>(f, cell_tab, mass2, diag, S, Np, cls_bits, id_bits, w);
     ++g_launch_count;
     return cudaGetLastError();
 }

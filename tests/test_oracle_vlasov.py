@@ -154,3 +154,55 @@ def test_V6_force_term_momentum_balance():
         E0 = np.sqrt(p2 + masses[x0, a])
         assert np.abs(dF[x0 + 1, a] - dt * px / E0 * f[x0, a] / (2 * dx)).max() <= 1e-14
         assert np.abs(dF[x0 - 1, a] + dt * px / E0 * f[x0, a] / (2 * dx)).max() <= 1e-14
+
+
+def test_V7_energy_balance_moments():
+    """Eq. 11-12, 26: T^00_kin and the integrals Q_c of the source term S_ex = (1/2) sum_c (d m_c^2) Q_c.
+    (a) one-cell closed forms with the degeneracies and the mass class of each species; (b) massless: T^00 is the energy
+    density of bz_moments and Q reproduces Eq. 8; (c) Eq. 26 as an identity between the two outputs: at fixed f,
+    d T^00 / d m_c^2 = Q_c / 2."""
+    n, pmin, pmax, alpha_s = 6, -3.0, 3.0, 0.3
+    g2 = 4 * math.pi * alpha_s
+    w = ((pmax - pmin) / n) ** 3 / (2 * math.pi) ** 3
+    px, py, pz = _centres(n, pmin, pmax)
+    p2 = px ** 2 + py ** 2 + pz ** 2
+    o = bzo.Oracle(np_=n, pmin=pmin, pmax=pmax, species=(0, 1, 2, 5), alpha_s=alpha_s)
+    # (a) one cell per species
+    f = np.zeros((1, 4, n ** 3))
+    cells, vals = (17, 100, 101, 200), (0.8, 0.3, 0.2, 0.4)
+    for a, (cc, v) in enumerate(zip(cells, vals)):
+        f[0, a, cc] = v
+    o.set_f(f)
+    masses = np.array([[0.4, 0.25, 0.7, 0.09]])
+    o.set_masses(masses)
+    d = o.energy_diag()[0]
+    E = [math.sqrt(p2[cells[0]] + 0.4), math.sqrt(p2[cells[1]] + 0.25), math.sqrt(p2[cells[2]] + 0.25), math.sqrt(p2[cells[3]] + 0.09)]
+    N = [16.0, 6.0, 6.0, 6.0]
+    assert d[0] == pytest.approx(w * sum(Na * v * e for Na, v, e in zip(N, vals, E)), rel=1e-13)
+    assert d[1] == pytest.approx(w * 16 * 0.8 / E[0], rel=1e-13)
+    assert d[2] == pytest.approx(w * 6 * (0.3 / E[1] + 0.2 / E[2]), rel=1e-13)          # u and ubar share m_u
+    assert d[3] == 0.0                                                                  # no d quarks
+    assert d[4] == pytest.approx(w * 6 * 0.4 / E[3], rel=1e-13)
+    # (b) massless
+    rng = np.random.default_rng(5)
+    f = rng.uniform(0.0, 1.0, size=(1, 4, n ** 3))
+    o.set_f(f)
+    o.set_masses(np.zeros((1, 4)))
+    d = o.energy_diag()[0]
+    mom = o.moments()
+    assert d[0] == pytest.approx(mom["ne"][0, :, 1].sum(), rel=1e-13)
+    assert g2 * (6 * d[1] / 16 + (d[2] + d[3] + d[4]) / 6) == pytest.approx(mom["m2"][0], rel=1e-13)       # Eq. 8
+    # (c) d T00 / d m_c^2 = Q_c / 2 at fixed f (central difference, O(delta^2))
+    base = np.array([0.5, 0.3, 0.2, 0.4])
+    o.set_masses(base[None])
+    Q = o.energy_diag()[0, 1:]
+    for c in (0, 1, 3):
+        delta = 1e-4
+        up, dn = base.copy(), base.copy()
+        up[c] += delta
+        dn[c] -= delta
+        o.set_masses(up[None])
+        Tp = o.energy_diag()[0, 0]
+        o.set_masses(dn[None])
+        Tm = o.energy_diag()[0, 0]
+        assert (Tp - Tm) / (2 * delta) == pytest.approx(0.5 * Q[c], rel=1e-6)
