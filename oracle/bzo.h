@@ -88,6 +88,13 @@ int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 int  bzo_set_transport(bzo_ctx*, int scheme);
 /* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper */
 int  bzo_set_collision(bzo_ctx*, int mode);
+/* ---- NEXT rank 3 (S8f): importance sampling of the t/u-channel peaks of Table I --------------------------------
+ * bzo_collision_is: the estimator of bzo_collision with t drawn from (1/2)[g(t) + g(u)], g ~ 1/(m^2 - t)^2, the azimuth
+ * about the CM direction of p1 uniformly, and every deposit multiplied by the weight (1/s)/p(t): same expectation.
+ * bzo_sample_one_is: one such sample (fields as bzo_sample_one; attempts = azimuth attempts) and its weight. */
+int  bzo_collision_is(bzo_ctx*, double dt_fm, unsigned step, double* dF);
+int  bzo_sample_one_is(const bzo_ctx*, unsigned step, int xcell, int pcell, int sample, double m2, bzo_sample* out, double* weight);
+
 /* ---- NEXT rank 1 (S8f): the paper's own collision path (Eq. 17-21, massive dispersion) ----------------------------
  * one root of E1 + E2 = E3 + Ep (Eq. 18-19): momenta k1, k2, their cells, the four energies, the Jacobian of Eq. 19 and
  * the massive Mandelstam variables */

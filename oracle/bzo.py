@@ -64,6 +64,8 @@ def lib():
         L.bzo_set_transport.argtypes = [vp, C.c_int]
         L.bzo_set_collision.argtypes = [vp, C.c_int]
         L.bzo_energy_diag.argtypes = [vp, dp]
+        L.bzo_collision_is.argtypes = [vp, C.c_double, C.c_uint, dp]
+        L.bzo_sample_one_is.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(Sample), dp]
         L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
         L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_moments.argtypes = [vp, dp]
@@ -219,6 +221,18 @@ class Oracle:
         dF = np.empty(self.shape, dtype=np.float64)
         _chk(lib().bzo_collision_paper(self._h, dt, step, _dptr(dF)), "bzo_collision_paper")
         return dF
+
+    # ---- NEXT rank 3: importance-sampled estimator
+    def collision_is(self, dt, step):
+        dF = np.empty(self.shape, dtype=np.float64)
+        _chk(lib().bzo_collision_is(self._h, dt, step, _dptr(dF)), "bzo_collision_is")
+        return dF
+
+    def sample_one_is(self, step, xcell, pcell, sample, m2):
+        s = Sample()
+        w = C.c_double()
+        _chk(lib().bzo_sample_one_is(self._h, step, xcell, pcell, sample, m2, C.byref(s), C.byref(w)), "bzo_sample_one_is")
+        return s, w.value
 
     def set_collision(self, mode):
         _chk(lib().bzo_set_collision(self._h, mode), "bzo_set_collision")
