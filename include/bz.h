@@ -135,6 +135,21 @@ int bz_vlasov(bz_ctx* ctx, double dt_fm, double* dF_dev);
  * bz_set_msq_override. */
 int bz_collision_paper(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
 
+/* ---- NEXT rank 3 of SURVEY.md 8f: importance sampling of the t/u-channel peaks ------------------------------------
+ * dF = dt * C_a[f] with the estimator of bz_collision, except that the momentum transfer is not uniform on [-s, 0]
+ * (isotropic CM direction) but drawn from p(t) = (1/2)[g(t) + g(-s - t)], g(t) = 1/((m^2 - t)^2 (1/m^2 - 1/(s + m^2))),
+ * where Table I peaks, with the azimuth about the CM direction of p1 uniform, and every deposit is
+ * multiplied by the weight (1/s)/p(t): same expectation, smaller variance for m^2 << s.  p1, p2 and s are those of
+ * bz_collision for the same (seed, step) (Philox blocks 0, 1); t uses block 96, the azimuth blocks 97...  m^2 is the
+ * regulator of the spatial cell (an empty cell, m^2 = 0: uniform t, weight 1).  dF_dev: device pointer, S*Nx*Np
+ * doubles, overwritten.  Asynchronous.  Honours bz_set_slab and bz_set_msq_override. */
+int bz_collision_is(bz_ctx* ctx, double dt_fm, unsigned step, double* dF_dev);
+
+/* Test-only: the samples of bz_collision_is for regulator m2 (GeV^2): cells_dev[n][Ns][4] = (j, k, l, flag),
+ * stu_dev[n][Ns][3] = (s, t, u) of the constructed momenta, w_dev[n][Ns] = the weight (0 where !(s > 0)). */
+int bz_debug_samples_is(bz_ctx* ctx, unsigned step, int xcell, int pcell_begin, int pcell_end, double m2, int* cells_dev,
+                        double* stu_dev, double* w_dev);
+
 /* Collision term used by bz_step: 0 (default, NS) = the massless centre-of-mass sampler of bz_collision; 1 = the
  * paper's own sampler of bz_collision_paper.  With mode 1 and transport scheme 1, bz_step is the paper's program as a
  * whole: thermal masses from the old f (Eq. 8-9), collision term by Eq. 17-21 with those masses, Eq. 15 for the

@@ -565,6 +565,8 @@ static int paper_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
         if (c->msq_ovr[k] >= 0.0) P.has_ovr = 1;
     }
     for (int k = 0; k < 4; ++k) P.dbg_msq[k] = 0.0;
+    P.mask = c->mask;
+    for (int a = 0; a < 7; ++a) P.slot[a] = c->slot[a];
     return 0;
 }
 
@@ -612,6 +614,45 @@ int bz_debug_paper_channels(const int* species, int n_species, int* out_host, in
         o[6] = table[q].key;
     }
     return (int)table.size();
+}
+
+/* ---- NEXT rank 3: importance-sampled estimator (bz_is.cu) ---- */
+static int is_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
+{
+    if (int rc = paper_params(c, dt_fm, step, P)) return rc;
+    const double L = P.g.L, Vp = (L * L) * L, dtG = dt_fm / kHbarc;
+    P.Kp = dtG * Vp / (2048.0 * (kPi * kPi * kPi * kPi) * c->Ns);      // the hot path's K (S8c step 0)
+    return 0;
+}
+
+int bz_collision_is(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
+{
+    if (!c || !dF_dev) return -1;
+    if (!c->f) return -4;
+    if (int rc = update_m2(c)) return rc;
+    PaperParams P;
+    if (int rc = is_params(c, dt_fm, step, P)) return rc;
+    P.dN = dF_dev;
+    BZ_CUDA(cudaMemsetAsync(dF_dev, 0, c->n_values * sizeof(double), c->stream), "memset dF");
+    BZ_CUDA(launch_is_collide(P, c->m2, c->sms, c->stream), "is collide");
+    double deg[7];
+    fill_deg(c, deg);
+    BZ_CUDA(launch_paper_finalize(dF_dev, c->n_values, c->S, c->Np, deg, c->stream), "is finalize");
+    return 0;
+}
+
+int bz_debug_samples_is(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, double m2, int* cells_dev,
+                        double* stu_dev, double* w_dev)
+{
+    if (!c || !cells_dev || !stu_dev || !w_dev || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np ||
+        pcell_begin > pcell_end)
+        return -1;
+    if (!c->f) return -4;
+    PaperParams P;
+    if (int rc = is_params(c, 1.0, step, P)) return rc;
+    P.x_begin = xcell; P.x_count = 1; P.p_begin = pcell_begin; P.p_count = pcell_end - pcell_begin;
+    BZ_CUDA(launch_is_debug(P, m2, cells_dev, stu_dev, w_dev, c->sms, c->stream), "is debug");
+    return 0;
 }
 
 int bz_moments(bz_ctx* c, double* out_host)

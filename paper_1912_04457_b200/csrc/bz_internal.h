@@ -55,6 +55,8 @@ struct PaperParams {
     int has_ovr;
     double msq_ovr[7];
     double dbg_msq[4];        // debug launch: the mass tuple whose roots are written out
+    unsigned mask;            // bz_is.cu: active species ids
+    int slot[7];              // bz_is.cu: species id -> layout index (or -1)
 };
 
 struct TransportParams {
@@ -148,6 +150,9 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
                           const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
                           double dx, double dp, unsigned cls_bits, cudaStream_t st);
 
+// NEXT rank 3 (bz_is.cu): P.Kp holds the hot path's K = dtG Vp / (2048 pi^4 Ns) there
+cudaError_t launch_is_collide(const PaperParams& P, const double* m2_cell, int sms, cudaStream_t st);
+cudaError_t launch_is_debug(const PaperParams& P, double m2, int* cells, double* stu, double* w, int sms, cudaStream_t st);
 // NEXT rank 1 (bz_paper.cu)
 void build_paper_channels(const int* species, int S, std::vector<PaperChannel>& table, std::vector<PaperGroup>& groups);
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st);

@@ -572,3 +572,42 @@ def test_energy_balance_diagnostic_parity():
     g.set_masses(masses)
     d_o, d_g = o.energy_diag(), g.energy_diag().numpy()
     assert np.allclose(d_g, d_o, rtol=1e-12, atol=0) and (d_o > 0).all()
+
+
+# ------------------------------------------------------------ NEXT rank 3: importance sampling of the t/u-channel peaks
+@pytest.mark.parametrize("cfg", [wl.scaled(wl.CONFIGS[2], np_=9, samples=40), wl.scaled(wl.CONFIGS[4], nx=2, np_=24, samples=33)],
+                         ids=lambda c: c.name)
+def test_importance_sampler_cells_bit_exact(cfg):
+    """Cells of p2, p3, p4, the flag, (s, t, u) and the weight of every importance-sampled sample: bit-exact."""
+    o, g = _pair(cfg)
+    xcell = cfg.Nx - 1
+    for m2 in (0.04, 0.7, 0.0):
+        pb, pe = (0, cfg.Np) if cfg.Np < 1000 else (6900, 6930)
+        cells, stu, w = (t.cpu().numpy() for t in g.debug_samples_is(7, xcell, pb, pe, m2))
+        for pc in range(pb, pe, 5):
+            for smp in range(cfg.samples):
+                sm, wt = o.sample_one_is(7, xcell, pc, smp, m2)
+                row = cells[pc - pb, smp]
+                assert tuple(row) == (sm.j, sm.k, sm.l, sm.flag), (m2, pc, smp)
+                if sm.s > 0:
+                    assert np.array_equal(stu[pc - pb, smp].view(np.uint64), np.array([sm.s, sm.t, sm.u]).view(np.uint64))
+                    assert np.array([w[pc - pb, smp]]).view(np.uint64)[0] == np.array([wt]).view(np.uint64)[0]
+
+
+@pytest.mark.parametrize("cfg,m_D", [(wl.scaled(wl.CONFIGS[0], np_=9, samples=40), 0.3),
+                                     (wl.scaled(wl.CONFIGS[2], np_=8, samples=33), 0.0),
+                                     (wl.scaled(wl.CONFIGS[3], nx=2, np_=7, samples=24), 0.5)],
+                         ids=["glue_fixed", "mixture_from_f", "inhom_fixed"])
+def test_importance_sampler_dF_parity_and_conservation(cfg, m_D):
+    import dataclasses
+    cfg = dataclasses.replace(cfg, m_D=m_D)
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=17)
+    o.set_f(f0)
+    g.set_f(f0)
+    dF_o = o.collision_is(cfg.dt, 3)
+    dF_g = g.collision_is(cfg.dt, 3).cpu().numpy()
+    gross = o.gross()
+    assert np.abs(dF_o).max() > 0
+    _assert_dF(dF_g, dF_o, gross, "importance sampler")
+    _assert_conserved(cfg, dF_g, gross)
