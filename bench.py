@@ -136,6 +136,26 @@ def paper_probe(g, cfg, dev, fp64_peak, reps=2):
             "frac": rate * flop / 1e12 / fp64_peak if fp64_peak else None}
 
 
+def is_probe(g, cfg, dev, reps=2):
+    """NEXT rank 3, outside the timed step: the importance-sampled estimator (bz_collision_is) on the whole
+    bench workload; same gathered/scattered bytes per sample as the hot path's kernel, so the same HBM-gather leg."""
+    import torch
+    out = torch.empty(g.shape, dtype=torch.float64, device=dev)
+    g.collision_is(cfg.dt, 0, out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for r in range(reps):
+        g.collision_is(cfg.dt, 1 + r, out)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    rate = cfg.samples_per_step / (ms * 1e-3)
+    bps = algorithmic_bytes_per_sample(cfg)
+    return {"kernel": "is_kernel (bz_collision_is)", "bound": "hbm", "ms": ms, "samples_per_sec": rate, "bytes_per_sample": bps,
+            "achieved": rate * bps / 1e9, "unit": "GB/s"}
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -324,6 +344,7 @@ def run_ours(args, cfg):
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs and not args.no_probes) else None
     rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs and not args.no_probes) else None
+    rank3 = is_probe(g, cfg, dev) if (rank == 0 and not slabs and not args.no_probes) else None
     clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
@@ -390,6 +411,7 @@ def run_ours(args, cfg):
                              "meet within the uncertainty of the operation count (1200-1850 flop per sample)"},
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
         "next_rank1_paper_sampler": rank1,
+        "next_rank3_importance_sampling": None if rank3 is None else dict(rank3, peak=peak, frac=rank3["achieved"] / peak),
         "next_rank2_eq15": None if rank2 is None else dict(rank2, peak=peak, frac=rank2["achieved"] / peak),
         "clocks": clocks,
         "total_particle_number": N1,
