@@ -153,7 +153,7 @@ int bz_debug_samples_is(bz_ctx* ctx, unsigned step, int xcell, int pcell_begin, 
 /* Collision term used by bz_step: 0 (default, NS) = the massless centre-of-mass sampler of bz_collision; 1 = the
  * paper's own sampler of bz_collision_paper.  With mode 1 and transport scheme 1, bz_step is the paper's program as a
  * whole: thermal masses from the old f (Eq. 8-9), collision term by Eq. 17-21 with those masses, Eq. 15 for the
- * drift and force terms, forward Euler.  -1 on a bad mode. */
+ * drift and force terms, forward Euler.  2 = the importance-sampled estimator of bz_collision_is.  -1 on a bad mode. */
 int bz_set_collision(bz_ctx* ctx, int mode);
 
 /* Test-only: the roots of the paper sampler for ONE mass tuple msq_host = (m_a^2, m_b^2, m_c^2, m_d^2), p1 cells

@@ -55,7 +55,7 @@ struct bzo_ctx {
      * [zb, ze) collide and count in the totals (the others are halo copies of a neighbour's layers) */
     unsigned xoff;
     int zb, ze;
-    int coll_mode;        /* bzo_set_collision: 0 = CM sampler, massless (the hot path), 1 = the paper's sampler, massive (rank 1) */
+    int coll_mode;        /* bzo_set_collision: 0 = CM sampler (the hot path), 1 = the paper's sampler, massive (rank 1), 2 = importance-sampled t (rank 3) */
     int scheme;           /* bzo_set_transport: 0 upwind massless, 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set */
     double* mass2;        /* [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 per spatial cell (Eq. 8-9); 0 at start */
 };
@@ -654,7 +654,7 @@ static double energy_at(const bzo_ctx* c, int ix, int iy, int iz, double m2)
     return sqrt(((px * px + py * py) + pz * pz) + m2);
 }
 
-int bzo_set_collision(bzo_ctx* c, int mode) { if (!c || mode < 0 || mode > 1) return -1; c->coll_mode = mode; return 0; }
+int bzo_set_collision(bzo_ctx* c, int mode) { if (!c || mode < 0 || mode > 2) return -1; c->coll_mode = mode; return 0; }
 int bzo_set_transport(bzo_ctx* c, int scheme) { if (!c || scheme < 0 || scheme > 2) return -1; c->scheme = scheme; return 0; }
 int bzo_set_masses(bzo_ctx* c, const double* mass2)
 {
@@ -960,6 +960,7 @@ int bzo_step(bzo_ctx* c, double dt_fm)
     if (!dFc || !dFs) { free(dFc); free(dFs); return -3; }
     if (c->scheme == 1) bzo_thermal_masses(c, NULL);          /* masses from the old f, before anything uses them */
     if (c->coll_mode == 1) bzo_collision_paper(c, dt_fm, c->step, dFc);
+    else if (c->coll_mode == 2) bzo_collision_is(c, dt_fm, c->step, dFc);
     else bzo_collision(c, dt_fm, c->step, dFc);
     if (c->scheme == 0) bzo_stream(c, dt_fm, dFs);
     else bzo_vlasov(c, dt_fm, dFs);

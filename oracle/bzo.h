@@ -86,7 +86,7 @@ int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 /* transport used by bzo_step: 0 = upwind massless (default), 1 = Eq. 15 with the masses re-evaluated from the old f
  * every step, 2 = Eq. 15 with the masses as stored */
 int  bzo_set_transport(bzo_ctx*, int scheme);
-/* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper */
+/* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper, 2 = bzo_collision_is */
 int  bzo_set_collision(bzo_ctx*, int mode);
 /* ---- NEXT rank 3 (S8f): importance sampling of the t/u-channel peaks of Table I --------------------------------
  * bzo_collision_is: the estimator of bzo_collision with t drawn from (1/2)[g(t) + g(u)], g ~ 1/(m^2 - t)^2, the azimuth

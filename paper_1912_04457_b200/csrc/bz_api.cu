@@ -413,7 +413,7 @@ int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
     return run_vlasov(c, dt_fm, dF_dev);
 }
 
-int bz_set_collision(bz_ctx* c, int mode) { if (!c || mode < 0 || mode > 1) return -1; c->coll_mode = mode; return 0; }
+int bz_set_collision(bz_ctx* c, int mode) { if (!c || mode < 0 || mode > 2) return -1; c->coll_mode = mode; return 0; }
 
 // bz_step with the paper's own collision term (rank 1): masses (scheme 1), bz_collision_paper into a scratch, the
 // transport increment of the chosen scheme into f_new, then f_new = (f + dF_transport) + dF_coll
@@ -421,7 +421,8 @@ static int step_paper(bz_ctx* c, double dt_fm)
 {
     if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f, used by both terms
     if (!c->dF_scratch) BZ_CUDA(cudaMalloc(&c->dF_scratch, c->n_values * sizeof(double)), "cudaMalloc dF scratch");
-    if (int rc = bz_collision_paper(c, dt_fm, c->step, c->dF_scratch)) return rc;
+    if (c->coll_mode == 1) { if (int rc = bz_collision_paper(c, dt_fm, c->step, c->dF_scratch)) return rc; }
+    else if (int rc = bz_collision_is(c, dt_fm, c->step, c->dF_scratch)) return rc;
     if (c->scheme == 0) BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 0, c->stream), "stream");
     else if (int rc = run_vlasov(c, dt_fm, c->f_new)) return rc;
     BZ_CUDA(launch_combine(c->f, c->f_new, c->dF_scratch, c->n_values, c->stream), "combine");
@@ -435,7 +436,7 @@ int bz_step(bz_ctx* c, double dt_fm)
 {
     if (!c) return -1;
     if (!c->f) return -4;
-    if (c->coll_mode == 1) return step_paper(c, dt_fm);
+    if (c->coll_mode != 0) return step_paper(c, dt_fm);
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, c->step)) return rc;
     if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f

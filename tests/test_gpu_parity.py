@@ -526,6 +526,22 @@ def test_paper_sampler_roots_bit_exact_on_the_config4_momentum_grid():
                     assert np.array_equal(stu[k, smp, 3 * r:3 * r + 3].view(np.uint64), np.array([R.s, R.t, R.u]).view(np.uint64))
 
 
+def test_step_with_the_importance_sampled_collision_term():
+    """bz_set_collision(2): bz_step with bz_collision_is; f after 3 steps against the oracle."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=7, samples=12)
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=43) * 0.5
+    for e in (o, g):
+        e.set_f(f0)
+        e.set_collision(2)
+    for _ in range(3):
+        o.step(cfg.dt)
+        g.step(cfg.dt)
+    f_o = o.get_f()
+    assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= 1e-11 * np.abs(f_o).max()
+    assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
+
+
 @pytest.mark.parametrize("scheme", [0, 1, 2])
 def test_step_with_the_papers_collision_term(scheme):
     """bz_set_collision(1): bz_step with the paper's sampler; with transport scheme 1 this is the paper's program as a
