@@ -202,8 +202,13 @@ cudaError_t launch_is_collide(const PaperParams& P, const double* m2_cell, int s
 {
     const long long warps = (long long)P.x_count * P.p_count * ((P.Ns + 31) / 32);
     if (warps <= 0) return cudaSuccess;
+    // grid-stride over warp items in order: launch only the CTAs that are resident at once, so that the warps in flight
+    // stay within one or two spatial cells (ncu on a 16-CTAs-per-SM grid: 20 x the compulsory DRAM traffic)
+    int per_sm = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, is_kernel<0>, 128, 0);
+    if (per_sm < 1) per_sm = 1;
     long long blocks = (warps + 3) / 4;
-    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
     is_kernel<0><<<(int)blocks, 128, 0, st>>>(P, m2_cell, 0.0, nullptr, nullptr, nullptr);
     ++g_launch_count;
     return cudaGetLastError();

@@ -424,8 +424,11 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
+    int per_sm = 1;                      // only the CTAs resident at once: the warps in flight stay within a few spatial cells
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_coop_kernel, 32 * kCoopWarps, 0);
+    if (per_sm < 1) per_sm = 1;
     long long blocks = (total / 32 + kCoopWarps) / kCoopWarps;
-    if (blocks > (long long)sms * 16) blocks = (long long)sms * 16;
+    if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
     paper_coop_kernel<<<(int)blocks, 32 * kCoopWarps, 0, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
