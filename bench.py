@@ -341,11 +341,11 @@ def run_ours(args, cfg):
     coll_ms, coll_n = g.get_profile(0)
     tr_ms, tr_n = g.get_profile(1)
     g.set_profile(False)
+    clocks = sampler.stop() if sampler else None          # the clocks of the timed region only, not of the probes below
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs and not args.no_probes) else None
     rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs and not args.no_probes) else None
     rank3 = is_probe(g, cfg, dev) if (rank == 0 and not slabs and not args.no_probes) else None
-    clocks = sampler.stop() if sampler else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
     # ---- end to end: host f in, host f and moments out, every step
