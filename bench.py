@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the whole hot path (bz_step + bz_moments: SURVEY.md 8a rows a1-a8) on synthetic input.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..4] [--impl ours|reference] [--slab] [--graph]
 
 Default workload: BASELINE.json configs[4] (16^3 spatial x 24^3 momentum cells, 7 species, 64 samples per cell:
 3.6e9 kinematic samples and 3.96e8 phase-space values per step, 3.17 GB per copy of f) -- the largest config, the one
@@ -10,18 +10,26 @@ north_star quotes the roofline target on; it fits one GPU.  One JSON line is pri
   value            kinematic collision samples per second over the whole step, inputs resident in HBM
   e2e              the same, but every step starts from HOST f in pinned memory and ends with f and the moments back on
                    the host (bz_step_host: copies, collision and stream + Euler pipelined by z layers; then bz_moments)
-  roofline         the collision kernel alone (CUDA events inside libbz.so around every launch of the timed region):
-                   algorithmic gather/scatter bytes per sample x samples / duration vs measured HBM GB/s
+  roofline         the collision kernel alone (CUDA events inside libbz.so around every launch of the timed region).
+                   `frac` is ACCEPTANCE-WEIGHTED: only samples with both outgoing legs in the box gather and scatter
+                   (reading S9), the kernel counts them (bz_get_sample_counts), so bytes per generated sample =
+                   acceptance x 48 S + 16 S / N_s.  `frac_survey_8d_literal` is SURVEY.md 8d's count as written (every
+                   sample credited with 3 cells x S x 16 B).  `roofline_fp64` is the other leg north_star names: the
+                   operation count of the method as the oracle's source states it (per generated sample, per accepted
+                   sample, per channel) against the measured FP64 peak.  The slower leg is named in `binding_leg`.
   cpu_baseline     the oracle as it stands, on this box's host cores, on a bounded sample of the same workload
 
-N > 1 (torchrun): weak scaling by domain decomposition (paper_1912_04457_b200/slab.py): the domain is
-the config repeated N times along z, every rank owns one copy and exchanges one boundary layer with each z neighbour
-per step (the drift stencil's only coupling); collisions are local.  The max over ranks of the device time is used.
+N > 1: bench.py starts its own ranks (torch.distributed.run, one per GPU, NCCL) unless it already runs under torchrun.
+Weak scaling by domain decomposition (paper_1912_04457_b200/slab.py): the domain is the config repeated N
+times along z, every rank owns one copy and exchanges one boundary layer with each z neighbour per step (the drift
+stencil's only coupling); collisions are local.  The max over ranks of the device time is used.
 --impl reference: the oracle arm (rank 0 only), each step a bounded sample of the workload.
 """
 import argparse
+import csv
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -35,36 +43,70 @@ import numpy as np  # noqa: E402
 
 import workloads as wl  # noqa: E402
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one collide_kernel launch, from the ncu --set full capture summarised in
-# profiles/r1_collide_kernel_ncu_full.md (the algorithmic gather/scatter bytes are ~113x larger: the tiles live in L2)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg4_inhom16x24": 10.880139e9}
-
 METRIC = "collision_samples_per_sec"
 UNIT = "samples/s"
 
+# ---- operation counts of the method, frozen from oracle/bzo.c (each fp64 + - x / sqrt = 1) --------
+# gen_sample, per GENERATED sample: 3 uniforms (add, mul each) 6; p2 6; E2 6; d12 5; s 3; binning of p2 6; Marsaglia
+# 11 per attempt x 4/pi attempts = 14, accepted direction 8; P 3, E 1, M 1; c 5; h 3; p3 12; p4 3; E3 2; d13 5; t 3;
+# u 2; binning of p3, p4 12  (the p1 cell centre and E1 are per cell, 15 / N_s per sample)
+FLOP_PER_GENERATED = 108.0
+# per ACCEPTED sample: w = K/(E1 E2) 2; Table I, the 10 distinct values with shared s^2, t^2, u^2, 1/(t - m^2),
+# 1/(u - m^2): 80 (20 for the pure-glue row alone); F = 1 +- f for 4 cells x S species: 4 S
+# per accepted sample AND ordered channel (collide_tile's inner loop): bracket 7, x w x |M|^2 2, four deposits 4 = 13
+FLOP_PER_CHANNEL = 13.0
+N_CHANNELS = {1: 1, 6: 90, 7: 127}
 
-def algorithmic_bytes_per_sample(cfg):
-    """3 random cells x S species x (8 B gather + 8 B scatter), plus the p1 cell once per N_s samples."""
+
+def flop_per_accepted(cfg):
+    n_ch = N_CHANNELS.get(cfg.S)
+    if n_ch is None:
+        return None
+    return 2.0 + (20.0 if cfg.S == 1 else 80.0) + 4.0 * cfg.S + FLOP_PER_CHANNEL * n_ch
+
+
+def bytes_literal_8d(cfg):
+    """SURVEY.md 8d as written: 3 random cells x S species x (8 B gather + 8 B scatter) for EVERY sample, plus the p1
+    cell once per N_s samples."""
     return 48.0 * cfg.S + 16.0 * cfg.S / cfg.samples
 
 
-# fp64 operations per kinematic sample, upper ends of SURVEY.md 8d's table (S = 1, 6, 7 species)
-FP64_FLOP_PER_SAMPLE = {1: 140.0, 6: 1350.0, 7: 1850.0}
+def bytes_acceptance_weighted(cfg, acceptance):
+    """The method's own bytes: a rejected sample gathers and scatters nothing (S9)."""
+    return acceptance * 48.0 * cfg.S + 16.0 * cfg.S / cfg.samples
+
+
+def ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture (profiles/ncu_traffic.csv:
+    kernel, workload, commit, bytes read, bytes written, source file).  Not measured in this run: returned with its source."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    try:
+        with open(path) as fh:
+            rows = [r for r in csv.DictReader(fh) if r["kernel"] == kernel and r["workload"] == workload]
+        if not rows:
+            return None, None
+        r = rows[-1]
+        return float(r["dram_bytes_read"]) + float(r["dram_bytes_write"]), "%s at commit %s (ncu --set full, one launch; not measured in this run)" % (r["source"], r["commit"])
+    except Exception:
+        return None, None
 
 
 def transport_roofline(cfg, tr_ms, tr_n, peak):
-    """Stream + Euler kernel (a6 + a7): phase-space cell updates per second against its HBM bytes.  Per value: 8 B f
-    read, 8 B f_new written, 8 B deposit read + 8 B re-zeroed, 8 B cell-major copy of the new f written (padded to 8
-    slots per cell when S > 1), upwind neighbours from L2: DESIGN.md 6."""
+    """Stream + Euler kernel (a6 + a7): phase-space cell updates per second.  `frac` is against SURVEY.md 8d's algorithmic
+    24 B per update (f read, deposit read, f_new written); `frac_kernel_bytes` against what this kernel moves by design:
+    also the deposit scratch re-zeroed and the cell-major copy of the new f (the next step's gather source), both padded
+    to 8 slots per cell when S > 1."""
     if not tr_n or tr_ms <= 0:
         return None
     pad = 8.0 / cfg.S if cfg.S > 1 else 0.0
-    bytes_per_value = 16.0 + (24.0 * pad if cfg.S > 1 else 16.0)
+    kernel_bytes = 16.0 + (24.0 * pad if cfg.S > 1 else 16.0)
     rate = cfg.n_values * tr_n / (tr_ms * 1e-3)
-    ach = rate * bytes_per_value / 1e9
+    ach = rate * 24.0 / 1e9
+    traffic, src = ncu_traffic("transport_kernel", cfg.name)
     return {"bound": "hbm", "kernel": "transport_kernel<1> (upwind stream + Euler + deposit conversion)",
-            "cell_updates_per_sec": rate, "bytes_per_value": bytes_per_value, "achieved": ach, "peak": peak, "unit": "GB/s",
-            "frac": ach / peak, "ms_per_launch": tr_ms / tr_n}
+            "cell_updates_per_sec": rate, "bytes_per_value": 24.0, "achieved": ach, "peak": peak, "unit": "GB/s",
+            "frac": ach / peak, "kernel_bytes_per_value": kernel_bytes, "frac_kernel_bytes": rate * kernel_bytes / 1e9 / peak,
+            "ms_per_launch": tr_ms / tr_n, "traffic": traffic, "traffic_source": src}
 
 
 def vlasov_probe(g, cfg, dev, reps=5):
@@ -101,6 +143,7 @@ def paper_probe(g, cfg, dev, fp64_peak, reps=2):
     """NEXT rank 1, outside the timed step: the paper's own sampler (Eq. 17-21) with the thermal masses of
     Eq. 8-9, on a bounded part of the bench workload (one z layer of spatial cells) so that it takes about a second."""
     import torch
+    from paper_1912_04457_b200 import bz
     out = torch.empty(g.shape, dtype=torch.float64, device=dev)
     masses = g.thermal_masses().numpy()
     nz = cfg.nx if cfg.Nx > 1 else 1
@@ -151,9 +194,9 @@ def is_probe(g, cfg, dev, reps=2):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / reps
     rate = cfg.samples_per_step / (ms * 1e-3)
-    bps = algorithmic_bytes_per_sample(cfg)
+    bps = bytes_literal_8d(cfg)
     return {"kernel": "is_kernel (bz_collision_is)", "bound": "hbm", "ms": ms, "samples_per_sec": rate, "bytes_per_sample": bps,
-            "achieved": rate * bps / 1e9, "unit": "GB/s"}
+            "bytes_note": "SURVEY.md 8d's literal count (every sample credited)", "achieved": rate * bps / 1e9, "unit": "GB/s"}
 
 
 def measured_peaks():
@@ -205,10 +248,13 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm)}
 
 
-def oracle_sample(cfg, f0, cores, tiles_per_core=12):
+ORACLE_TILES_PER_CORE = 6        # the ONE bounded oracle sample both cpu_baseline and --impl reference time
+
+
+def oracle_sample(cfg, f0, cores):
     """An oracle context holding M spatial cells of the workload (evenly spaced over the grid) as a bounded sample."""
     from oracle import bzo
-    M = max(1, min(cfg.Nx, cores * tiles_per_core if cfg.Nx > 1 else 1))
+    M = max(1, min(cfg.Nx, cores * ORACLE_TILES_PER_CORE if cfg.Nx > 1 else 1))
     xs = (np.arange(M) * (cfg.Nx // M)).astype(np.int64)
     o = bzo.Oracle(nx=M, ny=1, nz=1, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species,
                    alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples, threads=cores)
@@ -225,7 +271,7 @@ def run_reference(args, cfg):
         return
     cores = os.cpu_count() or 1
     f0 = wl.initial_f(cfg)
-    o, M, desc = oracle_sample(cfg, f0, cores, tiles_per_core=6)
+    o, M, desc = oracle_sample(cfg, f0, cores)
     for _ in range(args.warmup):
         o.step(cfg.dt)
         o.moments()
@@ -250,6 +296,25 @@ def run_reference(args, cfg):
 def o_threads(o):
     from oracle import bzo
     return int(bzo.lib().bzo_get_threads(o._h))
+
+
+def free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(args):
+    """python bench.py --gpus N outside torchrun: start the N ranks ourselves (one process per GPU, NCCL over NVLink)."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit("bench.py: --gpus %d but this box has %d CUDA device(s)" % (args.gpus, have))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    raise SystemExit(subprocess.call(cmd, env=env))
 
 
 def run_ours(args, cfg):
@@ -287,10 +352,12 @@ def run_ours(args, cfg):
         f_local[nl:-nl] = f0
         host_in = torch.from_numpy(f_local).pin_memory()
         step_fn = dom.step
+        own_values = cfg.n_values
     else:
         g = make(cfg.nx)
         host_in = torch.from_numpy(f0).pin_memory()
         step_fn = g.step
+        own_values = cfg.n_values
     host_out = torch.empty_like(host_in).pin_memory()
     mom_host = torch.empty(2 * cfg.S * g.Nx + 2 * cfg.S + g.Nx, dtype=torch.float64).pin_memory()
     g.set_f(host_in)
@@ -316,6 +383,7 @@ def run_ours(args, cfg):
     g.set_profile(True)
     g.get_profile(0)
     g.get_profile(1)
+    g.sample_counts(reset=True)
     barrier()
     launches0 = bz.launch_count()
     ms = 0.0
@@ -340,6 +408,7 @@ def run_ours(args, cfg):
     launches = bz.launch_count() - launches0
     coll_ms, coll_n = g.get_profile(0)
     tr_ms, tr_n = g.get_profile(1)
+    generated, accepted = g.sample_counts(reset=True)
     g.set_profile(False)
     clocks = sampler.stop() if sampler else None          # the clocks of the timed region only, not of the probes below
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
@@ -355,9 +424,7 @@ def run_ours(args, cfg):
     e0.record()
     for _ in range(e2e_steps):
         if slabs:
-            g.set_f(host_in)
-            step_fn(cfg.dt)
-            g.get_f(host_out)
+            dom.step_host(cfg.dt, host_in, host_out)   # boundary layers up, halo exchange, then bz_step_host over the own layers
         else:
             g.step_host(cfg.dt, host_in, host_out)     # bz_step_host: H2D, collision, stream + Euler, D2H pipelined by z layers
         g.moments(mom_host)
@@ -370,6 +437,7 @@ def run_ours(args, cfg):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms, ms_e2e, coll_ms, tr_ms = (float(x) for x in t.cpu())
+    ranks_ran = world
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -379,10 +447,33 @@ def run_ours(args, cfg):
     value = world * samples_step * args.steps / (ms * 1e-3)
     e2e_value = world * samples_step * e2e_steps / (ms_e2e * 1e-3)
     peak, peak_src = measured_peaks()
-    bps = algorithmic_bytes_per_sample(cfg)
-    ach = bps * samples_step * coll_n / (coll_ms * 1e-3) / 1e9 if coll_ms > 0 else None
+    acceptance = accepted / generated if generated else None
+    coll_s = coll_ms * 1e-3
+    kern_rate = samples_step * coll_n / coll_s if coll_s > 0 else None
+    roof = roof64 = None
+    if kern_rate and acceptance is not None:
+        b_aw, b_lit = bytes_acceptance_weighted(cfg, acceptance), bytes_literal_8d(cfg)
+        ach = kern_rate * b_aw / 1e9
+        traffic, tsrc = ncu_traffic("collide_kernel", cfg.name)
+        fpa = flop_per_accepted(cfg)
+        roof = {"bound": "hbm", "kernel": "collide_kernel (CUDA events inside libbz.so around every launch)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
+                "weighting": "acceptance-weighted: bytes per generated sample = acceptance x 48 S + 16 S / N_s (a rejected sample gathers and scatters nothing)",
+                "acceptance": acceptance, "samples_generated": generated, "samples_accepted": accepted,
+                "bytes_per_sample": b_aw, "samples_per_launch": samples_step, "ms_per_launch": coll_ms / coll_n,
+                "bytes_per_sample_survey_8d_literal": b_lit, "frac_survey_8d_literal": kern_rate * b_lit / 1e9 / peak,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read + write)", "traffic_source": tsrc}
+        if fpa and fp64_peak:
+            flop = FLOP_PER_GENERATED + acceptance * fpa
+            a64 = kern_rate * flop / 1e12
+            roof64 = {"bound": "alu", "kernel": "collide_kernel", "achieved": a64, "peak": fp64_peak, "unit": "TFLOP/s",
+                      "frac": a64 / fp64_peak, "peak_source": "measured (bz_measure_fp64_peak, register-resident DFMA chains; an FMA counts 2)",
+                      "flop_per_sample": flop, "flop_per_generated_sample": FLOP_PER_GENERATED, "flop_per_accepted_sample": fpa,
+                      "flop_per_channel": FLOP_PER_CHANNEL, "channels": N_CHANNELS.get(cfg.S),
+                      "count": "the method as oracle/bzo.c states it (channel by channel), each + - x / sqrt = 1; the kernel's factorised channel algebra executes fewer (DESIGN.md 6)"}
+            roof["binding_leg"] = "fp64" if roof64["frac"] > roof["frac"] else "hbm"
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ranks_ran, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "spatial_cells": cfg.Nx, "momentum_cells": cfg.Np, "species": cfg.S,
@@ -392,23 +483,14 @@ def run_ours(args, cfg):
                    "parallelism": ("z slabs, one halo layer exchanged with each neighbour per step (NCCL send/recv), domain = config x %d along z" % world if slabs
                                    else "independent replicas (homogeneous config: nothing to exchange)" if world > 1 else "1 GPU")},
         "cell_updates_per_sec": world * cfg.n_values * args.steps / (ms * 1e-3),
-        "collision_kernel_samples_per_sec": samples_step * coll_n / (coll_ms * 1e-3) if coll_ms > 0 else None,
+        "collision_kernel_samples_per_sec": kern_rate,
+        "collision_kernel_accepted_samples_per_sec": kern_rate * acceptance if (kern_rate and acceptance is not None) else None,
         "collision_kernel_share_of_step": coll_ms / ms if ms > 0 else None,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": host_in.numel() * 8,
-                "d2h_bytes_per_step": host_out.numel() * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": own_values * 8,
+                "d2h_bytes_per_step": own_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches,
-        "roofline": {"bound": "hbm", "kernel": "collide_kernel (CUDA events inside libbz.so around every launch)",
-                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak if ach else None,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.name), "traffic_unit": "bytes per launch (ncu dram read + write)",
-                     "peak_source": peak_src,
-                     "bytes_per_sample": bps, "samples_per_launch": samples_step,
-                     "ms_per_launch": coll_ms / coll_n if coll_n else None,
-                     "fp64_peak_tflops_measured": fp64_peak,
-                     "fp64_bound_samples_per_sec": fp64_peak * 1e12 / FP64_FLOP_PER_SAMPLE.get(cfg.S, 1850.0) if fp64_peak else None,
-                     "note": "north_star's roofline is the slower of the FP64 bound and the HBM gather/scatter bound; frac is "
-                             "against the HBM leg (measured denominator); the FP64 leg at SURVEY 8d's upper operation count "
-                             "and the measured FP64 peak is printed beside it (fp64_bound_samples_per_sec): the two legs "
-                             "meet within the uncertainty of the operation count (1200-1850 flop per sample)"},
+        "roofline": roof,
+        "roofline_fp64": roof64,
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
         "next_rank1_paper_sampler": rank1,
         "next_rank3_importance_sampling": None if rank3 is None else dict(rank3, peak=peak, frac=rank3["achieved"] / peak),
@@ -446,8 +528,10 @@ def main():
     cfg = wl.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg)
-    else:
-        run_ours(args, cfg)
+        return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
+    run_ours(args, cfg)
 
 
 if __name__ == "__main__":

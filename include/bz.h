@@ -39,7 +39,13 @@ typedef struct {
     double pmin, pmax;   /* momentum box edges, GeV, same on every axis; uniform cells  */
 } bz_grid;
 
-/* Create a context.  species: n_species ids in 0..6, strictly ascending.  alpha_s > 0.
+/* Create a context on the CUDA device that is current in the calling thread; every later call on the context switches
+ * to that device for its duration, so contexts on several devices can be driven from one thread.
+ * species: n_species ids in 0..6, strictly ascending.  alpha_s > 0.  Limits: 2 <= np <= 1024; nx*ny*nz*np^3 < 2^32
+ * (the Philox counter words and the work items are 32 bits wide).
+ * On failure *out is NULL if no context object was created (bad argument), otherwise a half-built context: it holds
+ * the error text for bz_last_error and whatever device buffers were allocated before the failure, answers every other
+ * call with -4, and the caller MUST bz_destroy it.
  * m_D > 0: fixed regulator mass (GeV) in the t/u propagators of Table I;
  * m_D <= 0: regulator mass^2 = the gluon thermal mass of Eq. 8 evaluated from the current f with
  * E_p = |p|, one value per spatial cell, recomputed at every bz_collision / bz_step (S8a.1, S7).
@@ -184,7 +190,11 @@ int bz_step(bz_ctx* ctx, double dt_fm);
  * is pipelined in chunks of z layers over three streams -- host-to-device copy of chunk k+1, collision of chunk k (the
  * collision term needs only the chunk's own cells, Eq. 5), stream + Euler of chunk k-1 (its upwind stencil needs
  * the old f of both z neighbours) and device-to-host copy of chunk k-2 run concurrently -- otherwise it is that plain
- * sequence.  Same results as the plain sequence up to the summation order of the deposits.  Synchronises. */
+ * sequence.  Same results as the plain sequence up to the summation order of the deposits.  Synchronises.
+ * Slab contexts (bz_set_slab): both host buffers still have the size of the whole context, but only the OWN layers are
+ * read from f_in_host and written to f_out_host; the halo layers must have been refreshed on the device (bz_copy_layers)
+ * before the call, from the neighbours' boundary layers of the same new f (paper_1912_04457_b200/slab.py, step_host);
+ * needs transport scheme 0 and collision mode 0 (-4 otherwise). */
 int bz_step_host(bz_ctx* ctx, double dt_fm, const double* f_in_host, double* f_out_host);
 
 /* Moments of the current f (Eq. 10; T^00 of Eq. 11, massless; S8a.8) written to HOST memory:
@@ -214,19 +224,18 @@ int bz_measure_fp64_peak(double* tflops_out_host);
  * difference over its timed region as "gpu_launches". */
 unsigned long long bz_launch_count(void);
 
+/* Kinematic samples drawn by the hot path's collision kernel (bz_collision, bz_step, bz_step_host) since the last
+ * reset: generated = spatial cells x momentum cells x samples per cell of every launch; accepted = those with s > 0 and
+ * both outgoing legs inside the momentum box (reading S9: the others deposit nothing), counted on the device by the
+ * kernel itself.  bench.py weights the roofline with accepted / generated.  reset != 0 clears both.  Synchronises. */
+int bz_get_sample_counts(bz_ctx* ctx, unsigned long long* generated_out, unsigned long long* accepted_out, int reset);
+
 /* ---- test-only exports ---------------------------------------------------------------------------------- */
 /* Sampled cells of p1 cells [pcell_begin, pcell_end) of spatial cell xcell, needed for the "bit-exact sampled
  * indices" target of NS: cells_dev[n][Ns][4] = (j, k, l, flag) int32, stu_dev[n][Ns][3] = (s, t, u) or NULL.
  * k = l = -1 when !(s > 0); k or l = -1 when that leg leaves the box; flag = 1 iff the sample deposits. */
 int bz_debug_samples(bz_ctx* ctx, unsigned step, int xcell, int pcell_begin, int pcell_end,
                      int* cells_dev, double* stu_dev);
-
-/* The per-sample channel algebra (S8c steps 4-6) run ON THE HOST through the same inline function the kernels
- * use, so that its factorised form can be checked against the per-channel definition without a GPU.
- * fv_host[slot*7 + id], slot 0..3 = cells i, j, k, l, id = species id (inactive ids ignored);
- * out_host[slot*7 + id] = deposit in number units for weight w (= K/(E1 E2)).  Never used by the product path. */
-int bz_debug_deposit_host(const int* species, int n_species, double alpha_s, const double* fv_host,
-                          double s, double t, double u, double m2, double w, double* out_host);
 
 #ifdef __cplusplus
 }

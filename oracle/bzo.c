@@ -950,6 +950,69 @@ int bzo_collision_paper(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
     return 0;
 }
 
+/* The same estimator written channel by channel with NO sharing of root solves: for every sample and every ordered
+ * channel (S8c step 5) the roots of Eq. 18 are solved with that channel's own four masses, and each root deposits
+ * (Eq. 21-22).  This is Eq. 3-4's sum over processes exactly as printed (x -> p -> sample -> channel -> root);
+ * bzo_collision_paper above solves each distinct mass tuple once and is checked against this one
+ * (tests/test_oracle_paper_sampler.py::test_R6).  Sequential, no threads. */
+int bzo_collision_paper_plain(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
+{
+    if (!c || !dF) return -1;
+    const double pi = 3.14159265358979323846;
+    const int S = c->S, Np = c->Np, n = c->g.np;
+    const size_t tile = (size_t)S * Np;
+    memset(dF, 0, tile * c->Nx * sizeof(double));
+    memset(c->gross, 0, tile * c->Nx * sizeof(double));
+    const double L = c->g.pmax - c->g.pmin, twopi5 = ((2.0 * pi) * (2.0 * pi)) * ((2.0 * pi) * (2.0 * pi)) * (2.0 * pi);
+    const double Kp = (dt_fm / HBARC) * ((L * L) * (L * L) * L) / ((double)c->Ns * twopi5 * 16.0) * 0.125;
+    const double g2 = 4.0 * pi * c->alpha_s, g4 = g2 * g2;
+    const int layer = c->g.nx * c->g.ny, xb = c->zb * layer, xe = c->ze * layer;
+    for (int x = xb; x < xe; ++x) {
+        const double* ft = c->f + (size_t)x * tile;
+        double* dN = dF + (size_t)x * tile;
+        double* gr = c->gross + (size_t)x * tile;
+        const double* mass2 = c->mass2 + 4 * (size_t)x;
+        const double mreg = c->m_D > 0.0 ? c->m_D * c->m_D : mass2[0];
+        for (int i = 0; i < Np; ++i) {
+            const double p[3] = { cell_centre(c, i % n), cell_centre(c, (i / n) % n), cell_centre(c, i / (n * n)) };
+            for (int smp = 0; smp < c->Ns; ++smp) {
+                double k3[3], k1x, k1y;
+                paper_draw(c, step, (unsigned)x + c->xoff, i, smp, k3, &k1x, &k1y);
+                const int i3 = bin_cell(c, k3);
+                if (i3 < 0) continue;
+                for (int q = 0; q < c->nch; ++q) {
+                    const bzo_channel* ch = &c->ch[q];
+                    const int ia = c->species[ch->a], ib = c->species[ch->b], ic = c->species[ch->c], id = c->species[ch->d];
+                    const double msq[4] = { mass2[mass_class(ia)], mass2[mass_class(ib)], mass2[mass_class(ic)], mass2[mass_class(id)] };
+                    bzo_proot rt[2];
+                    const int nr = paper_roots(c, p, k3, k1x, k1y, msq, rt);
+                    for (int r = 0; r < nr; ++r) {
+                        const bzo_proot* R = &rt[r];
+                        const double w = Kp / (fabs(R->J) * (((R->E1 * R->E2) * R->E3) * R->Ep));
+                        double M;
+                        if (c->msq_override[ch->kind] >= 0.0) M = c->msq_override[ch->kind];
+                        else M = ch->crossed ? bzo_msq(ch->kind, R->s, R->u, R->t, mreg, g4) : bzo_msq(ch->kind, R->s, R->t, R->u, mreg, g4);
+                        const size_t xa = (size_t)ch->a * Np + R->i1, xbb = (size_t)ch->b * Np + R->i2;
+                        const size_t xc = (size_t)ch->c * Np + i3, xd = (size_t)ch->d * Np + i;
+                        const double fa = ft[xa], fb = ft[xbb], fc = ft[xc], fd = ft[xd];
+                        const double fwd = fa * fb * Fstat(ic, fc) * Fstat(id, fd) - Fstat(ia, fa) * Fstat(ib, fb) * fc * fd;
+                        const double A = w * M * fwd, g = fabs(A);
+                        dN[xa] -= A; dN[xbb] -= A; dN[xc] += A; dN[xd] += A;
+                        gr[xa] += g; gr[xbb] += g; gr[xc] += g; gr[xd] += g;
+                    }
+                }
+            }
+        }
+    }
+    for (int x = 0; x < c->Nx; ++x) for (int a = 0; a < S; ++a) {
+        const double Na = degeneracy(c->species[a]);
+        double* d = dF + ((size_t)x * S + a) * Np;
+        double* g = c->gross + ((size_t)x * S + a) * Np;
+        for (int pc = 0; pc < Np; ++pc) { d[pc] = d[pc] / Na; g[pc] = g[pc] / Na; }
+    }
+    return 0;
+}
+
 /* ------------------------------------------------------------------ S8a.7: forward Euler, unsplit (Eq. 15) */
 int bzo_step(bzo_ctx* c, double dt_fm)
 {

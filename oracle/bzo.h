@@ -106,6 +106,9 @@ int  bzo_paper_sample(const bzo_ctx*, unsigned step, int xcell, int pcell, int s
 /* dF = dt C[f] with the paper's sampler and E^a = sqrt(p^2 + m_a^2(x)) from the stored thermal masses; also fills
  * the gross sums (bzo_get_gross) */
 int  bzo_collision_paper(bzo_ctx*, double dt_fm, unsigned step, double* dF);
+/* the same, channel by channel: every ordered channel solves its own roots, nothing is shared between channels
+ * (Eq. 3-4 as printed); the check of bzo_collision_paper's grouping by mass tuple.  Sequential. */
+int  bzo_collision_paper_plain(bzo_ctx*, double dt_fm, unsigned step, double* dF);
 /* f <- (f + dF_stream) + dF_coll, both from the old f (Eq. 15 unsplit); step counter ++ */
 int  bzo_step     (bzo_ctx*, double dt_fm);
 /* out = [N_x][S][2] (n, e) then [S][2] totals (N, E) then m^2[N_x]  (Eq. 10-11; Eq. 8) */

@@ -68,6 +68,7 @@ def lib():
         L.bzo_sample_one_is.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(Sample), dp]
         L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
         L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
+        L.bzo_collision_paper_plain.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_moments.argtypes = [vp, dp]
         L.bzo_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, ip, dp]
         L.bzo_sample_one.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.POINTER(Sample)]
@@ -220,6 +221,11 @@ class Oracle:
     def collision_paper(self, dt, step):
         dF = np.empty(self.shape, dtype=np.float64)
         _chk(lib().bzo_collision_paper(self._h, dt, step, _dptr(dF)), "bzo_collision_paper")
+        return dF
+
+    def collision_paper_plain(self, dt, step):
+        dF = np.empty(self.shape, dtype=np.float64)
+        _chk(lib().bzo_collision_paper_plain(self._h, dt, step, _dptr(dF)), "bzo_collision_paper_plain")
         return dF
 
     # ---- NEXT rank 3: importance-sampled estimator

@@ -23,8 +23,8 @@ EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_sa
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
            "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
-           "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_debug_samples",
-           "bz_debug_deposit_host")
+           "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_get_sample_counts",
+           "bz_debug_samples")
 
 KINDS = ("A", "11", "1B", "ANN", "QQGG", "QG", "GG")      # kinds of Table I in the order of bz_set_msq_override
 
@@ -68,10 +68,10 @@ def lib():
         L.bz_set_profile.argtypes = [vp, C.c_int]
         L.bz_get_profile.argtypes = [vp, C.c_int, dp, ip]
         L.bz_measure_fp64_peak.argtypes = [dp]
+        L.bz_get_sample_counts.argtypes = [vp, C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong), C.c_int]
         L.bz_launch_count.argtypes = []
         L.bz_launch_count.restype = C.c_ulonglong
         L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
-        L.bz_debug_deposit_host.argtypes = [ip, C.c_int, C.c_double, dp] + [C.c_double] * 5 + [dp]
         _lib = L
     return _lib
 
@@ -81,7 +81,13 @@ class BzError(RuntimeError):
 
 
 class Boltzmann:
-    """One bz_ctx.  Methods carry the names of the C entry points without the prefix."""
+    """One bz_ctx.  Methods carry the names of the C entry points without the prefix.
+
+    Stream semantics: every call enqueues its work on the context's stream (the torch stream that was current when the
+    object was made, or the one given to set_stream).  CUDA tensors returned by get_f / collision / stream / vlasov /
+    get_layers are therefore ordered on THAT stream only: a consumer on another stream (torch streams are non-blocking
+    with respect to each other) must synchronise it or wait on it first, e.g.
+    torch.cuda.current_stream().wait_stream(s).  Calls that copy to host memory synchronise the stream themselves."""
 
     def __init__(self, nx=1, ny=1, nz=1, dx=1.0, np_=15, pmin=-3.0, pmax=3.0, species=(0,), alpha_s=0.3, m_D=0.0,
                  seed=0, samples=64, device="cuda:0"):
@@ -130,6 +136,7 @@ class Boltzmann:
         return C.c_void_p(t.data_ptr())
 
     def set_stream(self, stream):
+        self.stream = stream
         self._chk(lib().bz_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "bz_set_stream")
 
     def set_seed(self, seed):
@@ -291,6 +298,12 @@ class Boltzmann:
         self._chk(lib().bz_get_profile(self._h, group, C.byref(ms), C.byref(n)), "bz_get_profile")
         return ms.value, n.value
 
+    def sample_counts(self, reset=False):
+        """(generated, accepted) kinematic samples of the hot path's collision kernel since the last reset."""
+        g, a = C.c_ulonglong(), C.c_ulonglong()
+        self._chk(lib().bz_get_sample_counts(self._h, C.byref(g), C.byref(a), int(bool(reset))), "bz_get_sample_counts")
+        return g.value, a.value
+
     def debug_samples(self, step, xcell, pbegin, pend, want_stu=True):
         n = pend - pbegin
         cells = torch.empty((n, self.Ns, 4), dtype=torch.int32, device=self.device)
@@ -323,16 +336,3 @@ def measure_fp64_peak():
 def launch_count():
     """bz_launch_count: CUDA kernels launched by libbz.so in this process so far."""
     return int(lib().bz_launch_count())
-
-
-def debug_deposit_host(species, alpha_s, fv, s, t, u, m2, w):
-    """bz_debug_deposit_host: the kernels' channel algebra evaluated on the host (test aid, not a compute path)."""
-    import numpy as np
-    fv = np.ascontiguousarray(fv, dtype=np.float64).reshape(4, 7)
-    out = np.empty((4, 7), dtype=np.float64)
-    sp = (C.c_int * len(species))(*species)
-    rc = lib().bz_debug_deposit_host(sp, len(species), alpha_s, fv.ctypes.data_as(C.POINTER(C.c_double)), s, t, u, m2, w,
-                                     out.ctypes.data_as(C.POINTER(C.c_double)))
-    if rc != 0:
-        raise BzError("bz_debug_deposit_host failed (%d)" % rc)
-    return out

@@ -30,6 +30,21 @@ int fail_cuda(bz_ctx* c, cudaError_t e, const char* where)
         if (e_ != cudaSuccess) return fail_cuda(c, e_, where); \
     } while (0)
 
+// Every entry point runs on the device the context was created on, whatever device is current in the calling thread
+// (the previous one is restored on return).  A failing cudaSetDevice leaves a sticky error the next CUDA call reports.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev)
+    {
+        int cur = -1;
+        if (dev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != dev && cudaSetDevice(dev) == cudaSuccess) prev = cur;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define BZ_ON_DEVICE(c) DeviceGuard device_guard_((c)->device)
+
 double degeneracy(int id) { return id == 0 ? 16.0 : 6.0; }   // N_g = 2 x 8, N_q = 2 x 3
 
 void fill_deg(const bz_ctx* c, double (&deg)[7])
@@ -65,7 +80,7 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     CollideParams P;
     P.g = grid_const(c);
     P.f_aos = c->SP == 1 ? c->f : c->f_aos;    // one species: the API layout is already cell-major
-    P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab;
+    P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab; P.counters = c->counters;
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
     P.work_counter = c->work_counter + c->launch_parity; P.next_counter = c->work_counter + (c->launch_parity ^ 1u);
     const int layer = c->grid.nx * c->grid.ny;              // only the slab's own z layers collide (bz_set_slab)
@@ -105,7 +120,9 @@ int run_collide(bz_ctx* c, double dt_fm, unsigned step)
         BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
         c->aos_valid = true;
     }
-    BZ_CUDA(launch_collide(collide_params(c, dt_fm, step), c->sms, c->stream), "collide");
+    const CollideParams P = collide_params(c, dt_fm, step);
+    BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
+    c->generated += (unsigned long long)(P.n_items / (unsigned)P.regions_per_x) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
     c->launch_parity ^= 1u;
     return prof_mark(c, 0);
 }
@@ -147,13 +164,13 @@ int run_thermal_masses(bz_ctx* c)
 
 extern "C" {
 
-int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_s, double m_D, bz_ctx** out)
+static int create_impl(const bz_grid* g, const int* species, int n_species, double alpha_s, double m_D, bz_ctx** out)
 {
+    if (out) *out = nullptr;
     if (!g || !species || !out || n_species < 1 || n_species > 7) return -1;
     if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->np < 2 || g->np > 1024 || !(g->pmax > g->pmin) || !(g->dx > 0.0) ||
         !(alpha_s > 0.0))
         return -1;
-    if ((long long)g->nx * g->ny * g->nz > 65535) return -1;
     for (int a = 0; a < n_species; ++a) {
         if (species[a] < 0 || species[a] > 6) return -1;
         if (a > 0 && species[a] <= species[a - 1]) return -1;
@@ -166,13 +183,14 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     c->mask = 0;
     for (int a = 0; a < 7; ++a) c->slot[a] = -1;
     for (int a = 0; a < n_species; ++a) { c->species[a] = species[a]; c->slot[species[a]] = a; c->mask |= 1u << species[a]; }
+    c->device = -1;
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false; c->copy_in = nullptr; c->copy_out = nullptr;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
     c->mass2 = nullptr; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
-    c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0;
+    c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
     c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
-    c->work_counter = nullptr; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
+    c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -182,12 +200,15 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     {
         int dev = 0;
         BZ_CUDA(cudaGetDevice(&dev), "cudaGetDevice");
+        c->device = dev;                            // the context lives on the device that is current now
         BZ_CUDA(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev), "SM count");
         if ((long long)c->Nx * c->Np >= (1LL << 32)) { c->err = "bz_create: more than 2^32 (xcell, pcell) pairs"; return -1; }
         c->cells_per_region = collide_cells_per_region(c->Np, c->Nx, c->sms);
         c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
     }
     const size_t bytes = c->n_values * sizeof(double);
+    BZ_CUDA(cudaMalloc(&c->counters, sizeof(unsigned long long)), "cudaMalloc sample counter");
+    BZ_CUDA(cudaMemset(c->counters, 0, sizeof(unsigned long long)), "memset sample counter");
     BZ_CUDA(cudaMalloc(&c->work_counter, 2 * sizeof(unsigned)), "cudaMalloc work counter");
     BZ_CUDA(cudaMemset(c->work_counter, 0, 2 * sizeof(unsigned)), "memset work counter");
     BZ_CUDA(cudaMalloc(&c->f, bytes), "cudaMalloc f");
@@ -229,11 +250,22 @@ int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_
     return 0;
 }
 
+int bz_create(const bz_grid* g, const int* species, int n_species, double alpha_s, double m_D, bz_ctx** out)
+{
+    const int rc = create_impl(g, species, n_species, alpha_s, m_D, out);
+    if (rc != 0 && out && *out && (*out)->f) {       // half-built: every entry point but bz_last_error / bz_destroy answers -4
+        cudaFree((*out)->f);
+        (*out)->f = nullptr;
+    }
+    return rc;
+}
+
 int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
-    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups);
+    BZ_ON_DEVICE(c);
+    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->counters); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups); cudaFree(c->diag);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     for (cudaEvent_t e : c->pipe_events) cudaEventDestroy(e);
     if (c->copy_in) cudaStreamDestroy(c->copy_in);
@@ -257,6 +289,8 @@ int bz_set_msq_override(bz_ctx* c, int kind, double value)
 int bz_set_slab(bz_ctx* c, unsigned xcell_offset, int z_begin, int z_end)
 {
     if (!c || z_begin < 0 || z_end > c->grid.nz || z_begin > z_end) return -1;
+    // the cell-major copy of f is only kept up to date for the own layers (bz_copy_layers): a new range starts afresh
+    if (z_begin != c->zb || z_end != c->ze) c->aos_valid = false;
     c->xoff = xcell_offset; c->zb = z_begin; c->ze = z_end;
     return 0;
 }
@@ -265,6 +299,7 @@ int bz_copy_layers(bz_ctx* c, int z0, int n_layers, double* buf_dev, int to_ctx)
 {
     if (!c || !buf_dev || z0 < 0 || n_layers < 0 || z0 + n_layers > c->grid.nz) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     const size_t layer = (size_t)c->grid.nx * c->grid.ny * c->S * c->Np;      // doubles per z layer, contiguous in f
     double* p = c->f + (size_t)z0 * layer;
     if (n_layers == 0) return 0;
@@ -283,6 +318,7 @@ int bz_set_f(bz_ctx* c, const double* f, int on_device)
 {
     if (!c || !f) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     BZ_CUDA(cudaMemcpyAsync(c->f, f, c->n_values * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                             c->stream), "bz_set_f copy");
     c->aos_valid = false; c->rowsum_valid = false;
@@ -294,6 +330,7 @@ int bz_get_f(bz_ctx* c, double* f, int on_device)
 {
     if (!c || !f) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     BZ_CUDA(cudaMemcpyAsync(f, c->f, c->n_values * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
                             c->stream), "bz_get_f copy");
     if (!on_device) BZ_CUDA(cudaStreamSynchronize(c->stream), "bz_get_f sync");
@@ -304,6 +341,7 @@ int bz_collision(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, step)) return rc;
     double deg[7];
@@ -327,6 +365,7 @@ int bz_stream(bz_ctx* c, double dt_fm, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     BZ_CUDA(launch_transport(transport_params(c, dt_fm, dF_dev), 0, c->stream), "stream");
     return 0;
 }
@@ -380,6 +419,7 @@ int bz_thermal_masses(bz_ctx* c, double* out_host)
 {
     if (!c) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     if (int rc = run_thermal_masses(c)) return rc;
     if (out_host) {
         BZ_CUDA(cudaMemcpyAsync(out_host, c->mass2, (size_t)c->Nx * 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "masses copy");
@@ -392,17 +432,15 @@ int bz_energy_diag(bz_ctx* c, double* out_host)
 {
     if (!c || !out_host) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     unsigned cls, ids;
     class_bits(c, cls, ids);
     const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
     const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
-    double* diag = nullptr;                                   // small and rare: allocated per call
-    BZ_CUDA(cudaMalloc(&diag, (size_t)c->Nx * 5 * sizeof(double)), "cudaMalloc diag");
-    cudaError_t e = launch_energy_diag(c->f, c->cell_tab, c->mass2, diag, c->Nx, c->S, c->Np, cls, ids, d3p / twopi3, c->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out_host, diag, (size_t)c->Nx * 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    cudaFree(diag);
-    if (e != cudaSuccess) return fail_cuda(c, e, "bz_energy_diag");
+    if (!c->diag) BZ_CUDA(cudaMalloc(&c->diag, (size_t)c->Nx * 5 * sizeof(double)), "cudaMalloc diag");   // kept with the context
+    BZ_CUDA(launch_energy_diag(c->f, c->cell_tab, c->mass2, c->diag, c->Nx, c->S, c->Np, cls, ids, d3p / twopi3, c->stream), "energy diag");
+    BZ_CUDA(cudaMemcpyAsync(out_host, c->diag, (size_t)c->Nx * 5 * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "diag copy");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "diag sync");
     return 0;
 }
 
@@ -410,6 +448,7 @@ int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     return run_vlasov(c, dt_fm, dF_dev);
 }
 
@@ -436,6 +475,7 @@ int bz_step(bz_ctx* c, double dt_fm)
 {
     if (!c) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     if (c->coll_mode != 0) return step_paper(c, dt_fm);
     if (int rc = update_m2(c)) return rc;
     if (int rc = run_collide(c, dt_fm, c->step)) return rc;
@@ -461,10 +501,13 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
 {
     if (!c || !f_in_host || !f_out_host) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     const int nzl = c->grid.nz, layer_cells = c->grid.nx * c->grid.ny;
     const int lpc = (nzl + 15) / 16;                             // z layers per chunk: at most 16 chunks
     const int K = (nzl + lpc - 1) / lpc;
-    if (c->scheme != 0 || c->coll_mode != 0 || K < 3) {                               // nothing to overlap (or Eq. 15 transport): the plain sequence
+    const bool slab = c->zb != 0 || c->ze != nzl;
+    if (slab && (c->scheme != 0 || c->coll_mode != 0)) { c->err = "bz_step_host: a slab context needs transport scheme 0 and collision mode 0"; return -4; }
+    if (!slab && (c->scheme != 0 || c->coll_mode != 0 || K < 3)) {                    // nothing to overlap (or Eq. 15 transport): the plain sequence
         if (int rc = bz_set_f(c, f_in_host, 0)) return rc;
         if (int rc = bz_step(c, dt_fm)) return rc;
         return bz_get_f(c, f_out_host, 0);
@@ -488,9 +531,13 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
     BZ_CUDA(cudaEventRecord(start, c->stream), "record");
     BZ_CUDA(cudaStreamWaitEvent(c->copy_in, start, 0), "wait");
     BZ_CUDA(cudaStreamWaitEvent(c->copy_out, start, 0), "wait");
+    // own layers of chunk k as a range of spatial cells (bz_set_slab: halo layers are refreshed on the device by the
+    // caller, they are neither read from nor written to the host buffers)
+    auto own_x0 = [&](int k) { return std::max(c->zb, k * lpc) * layer_cells; };
+    auto own_nx = [&](int k) { return std::max(0, std::min(c->ze, std::min(nzl, (k + 1) * lpc)) - std::max(c->zb, k * lpc)) * layer_cells; };
     for (int k = 0; k < K; ++k) {
-        const size_t off = (size_t)x0_of(k) * cell_vals, cnt = (size_t)nx_of(k) * cell_vals;
-        BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
+        const size_t off = (size_t)own_x0(k) * cell_vals, cnt = (size_t)own_nx(k) * cell_vals;
+        if (cnt) BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
         BZ_CUDA(cudaEventRecord(h2d_done[k], c->copy_in), "record");
     }
     const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;
@@ -500,8 +547,8 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
         BZ_CUDA(launch_transport(T, 1, c->stream), "stream+euler");
         BZ_CUDA(cudaEventRecord(tr_done[k], c->stream), "record");
         BZ_CUDA(cudaStreamWaitEvent(c->copy_out, tr_done[k], 0), "wait");
-        const size_t off = (size_t)x0_of(k) * cell_vals, cnt = (size_t)nx_of(k) * cell_vals;
-        BZ_CUDA(cudaMemcpyAsync(f_out_host + off, c->f_new + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->copy_out), "d2h");
+        const size_t off = (size_t)own_x0(k) * cell_vals, cnt = (size_t)own_nx(k) * cell_vals;
+        if (cnt) BZ_CUDA(cudaMemcpyAsync(f_out_host + off, c->f_new + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->copy_out), "d2h");
         return 0;
     };
     for (int k = 0; k < K; ++k) {
@@ -521,6 +568,7 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
             P.x_begin = zb * layer_cells;
             P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)c->regions_per_x;
             BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
+            c->generated += (unsigned long long)((ze - zb) * layer_cells) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
             c->launch_parity ^= 1u;
         }
         // chunk k - 1 has both z neighbours on the device now (chunk 0 waits for the last one: periodic)
@@ -575,6 +623,7 @@ int bz_collision_paper(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     PaperParams P;
     if (int rc = paper_params(c, dt_fm, step, P)) return rc;
     P.dN = dF_dev;
@@ -593,6 +642,7 @@ int bz_debug_paper_samples(bz_ctx* c, unsigned step, int xcell, int pcell_begin,
         pcell_begin > pcell_end)
         return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     PaperParams P;
     if (int rc = paper_params(c, 1.0, step, P)) return rc;
     P.x_begin = xcell; P.x_count = 1; P.p_begin = pcell_begin; P.p_count = pcell_end - pcell_begin;
@@ -630,6 +680,7 @@ int bz_collision_is(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     if (int rc = update_m2(c)) return rc;
     PaperParams P;
     if (int rc = is_params(c, dt_fm, step, P)) return rc;
@@ -649,6 +700,7 @@ int bz_debug_samples_is(bz_ctx* c, unsigned step, int xcell, int pcell_begin, in
         pcell_begin > pcell_end)
         return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     PaperParams P;
     if (int rc = is_params(c, 1.0, step, P)) return rc;
     P.x_begin = xcell; P.x_count = 1; P.p_begin = pcell_begin; P.p_count = pcell_end - pcell_begin;
@@ -660,6 +712,7 @@ int bz_moments(bz_ctx* c, double* out_host)
 {
     if (!c || !out_host) return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     if (int rc = update_m2(c)) return rc;
     double deg[7];
     fill_deg(c, deg);
@@ -679,6 +732,7 @@ int bz_set_profile(bz_ctx* c, int on) { if (!c) return -1; c->profile = on != 0;
 int bz_get_profile(bz_ctx* c, int group, double* ms_total, int* launches)
 {
     if (!c || !ms_total || !launches || group < 0 || group > 1) return -1;
+    BZ_ON_DEVICE(c);
     BZ_CUDA(cudaStreamSynchronize(c->stream), "profile sync");
     std::vector<cudaEvent_t>& ev = c->prof_events[group];
     double tot = 0.0;
@@ -696,33 +750,30 @@ int bz_get_profile(bz_ctx* c, int group, double* ms_total, int* launches)
 
 unsigned long long bz_launch_count(void) { return g_launch_count.load(); }
 
+int bz_get_sample_counts(bz_ctx* c, unsigned long long* generated_out, unsigned long long* accepted_out, int reset)
+{
+    if (!c || !generated_out || !accepted_out) return -1;
+    if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
+    unsigned long long acc = 0ull;
+    BZ_CUDA(cudaMemcpyAsync(&acc, c->counters, sizeof acc, cudaMemcpyDeviceToHost, c->stream), "sample counter copy");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "sample counter sync");
+    *generated_out = c->generated; *accepted_out = acc;
+    if (reset) {
+        BZ_CUDA(cudaMemsetAsync(c->counters, 0, sizeof acc, c->stream), "sample counter reset");
+        c->generated = 0ull;
+    }
+    return 0;
+}
+
 int bz_debug_samples(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int* cells_dev, double* stu_dev)
 {
     if (!c || !cells_dev || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np || pcell_begin > pcell_end)
         return -1;
     if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
     BZ_CUDA(launch_debug_samples(collide_params(c, 1.0, step), xcell, pcell_begin, pcell_end, cells_dev, stu_dev, c->stream),
             "debug_samples");
-    return 0;
-}
-
-int bz_debug_deposit_host(const int* species, int n_species, double alpha_s, const double* fv, double s, double t, double u,
-                          double m2, double w, double* out)
-{
-    if (!species || !fv || !out || n_species < 1 || n_species > 7) return -1;
-    unsigned mask = 0;
-    for (int a = 0; a < n_species; ++a) {
-        if (species[a] < 0 || species[a] > 6) return -1;
-        mask |= 1u << species[a];
-    }
-    double f[4][7], d[4][7];
-    for (int sl = 0; sl < 4; ++sl)
-        for (int id = 0; id < 7; ++id) f[sl][id] = ((mask >> id) & 1u) ? fv[sl * 7 + id] : 0.0;
-    const double g2 = 4.0 * kPi * alpha_s;
-    const MsqSet M = msq_set<true, true>(s, t, u, m2, g2 * g2 * w);
-    deposit<-1>(mask, f[0], f[1], f[2], f[3], M, d[0], d[1], d[2], d[3]);
-    for (int sl = 0; sl < 4; ++sl)
-        for (int id = 0; id < 7; ++id) out[sl * 7 + id] = d[sl][id];
     return 0;
 }
 

@@ -244,4 +244,108 @@ BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7
 #undef BZ_ON
 }
 
+// ---- the same algebra split into its gain and its loss half ------------------------------------------------------------
+// Every channel's bracket is  f_a(i) f_b(j) F_c(k) F_d(l)  -  F_a(i) F_b(j) f_c(k) f_d(l)  (Eq. 5): a "gain" product
+// and a "loss" product of the same shape with f and F = 1 +- f exchanged.  deposit_half evaluates ONE of the two for all
+// channels: P holds the incoming-side factors at the cells i, j (f for the gain half, F for the loss half), Q the
+// outgoing-side factors at k, l (F for the gain half, f for the loss half), and the caller passes the |M|^2 set with its
+// sign (+ gain, - loss), so that the half's deposits are -H, -H, +H, +H like the whole bracket's (Eq. 22).  The collision
+// kernel gives the two halves of a sample to two neighbouring lanes (half the registers per lane, the same instruction
+// stream for both) and adds the two sets of deposits when it flushes them; each half's deposits cancel exactly by
+// themselves, so particle number is conserved as before.  Entries of inactive species must be 0 in P and in Q.
+template <int kMask>
+BZ_HD void deposit_half(unsigned rt_mask, const double (&Pi)[7], const double (&Pj)[7], const double (&Qk)[7],
+                        const double (&Ql)[7], const MsqSet& M, double (&dI)[7], double (&dJ)[7], double (&dK)[7],
+                        double (&dL)[7])
+{
+    const unsigned mask = kMask >= 0 ? (unsigned)kMask : rt_mask;
+#define BZ_ON(a) (((mask) >> (a)) & 1u)
+    const bool glue = BZ_ON(0);
+#pragma unroll
+    for (int a = 0; a < 7; ++a) dI[a] = dJ[a] = dK[a] = dL[a] = 0.0;
+    // ------------------------------------------------------------------ t-family: a i->k, b j->l
+    {
+        double X[7], Z[7];
+#pragma unroll
+        for (int a = 0; a < 7; ++a) { X[a] = Pi[a] * Qk[a]; Z[a] = Pj[a] * Ql[a]; }
+        const double Xq = ((X[1] + X[2]) + (X[3] + X[4])) + (X[5] + X[6]);
+        const double Zq = ((Z[1] + Z[2]) + (Z[3] + Z[4])) + (Z[5] + Z[6]);
+        if (glue) {
+            const double T = X[0] * (M.gg * Z[0] + M.qg_t * Zq);
+            const double U = Z[0] * (M.gg * X[0] + M.qg_t * Xq);
+            dI[0] -= T; dK[0] += T; dJ[0] -= U; dL[0] += U;
+        }
+        const double bZ = M.qg_t * Z[0] + M.a_t * Zq, bX = M.qg_t * X[0] + M.a_t * Xq;
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            if (!BZ_ON(a)) continue;
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const double T = X[a] * fma(M.d11, Z[a], fma(M.d1b_t, Z[ab], bZ));
+            const double U = Z[a] * fma(M.d11, X[a], fma(M.d1b_t, X[ab], bX));
+            dI[a] -= T; dK[a] += T; dJ[a] -= U; dL[a] += U;
+        }
+    }
+    // ------------------------------------------------------------------ u-family: a i->l, b j->k
+    {
+        double X[7], Z[7];
+#pragma unroll
+        for (int a = 0; a < 7; ++a) { X[a] = Pi[a] * Ql[a]; Z[a] = Pj[a] * Qk[a]; }
+        const double Xq = ((X[1] + X[2]) + (X[3] + X[4])) + (X[5] + X[6]);
+        const double Zq = ((Z[1] + Z[2]) + (Z[3] + Z[4])) + (Z[5] + Z[6]);
+        if (glue) {
+            const double T = M.qg_u * (X[0] * Zq);
+            const double U = M.qg_u * (Z[0] * Xq);
+            dI[0] -= T; dL[0] += T; dJ[0] -= U; dK[0] += U;
+        }
+        const double bZ = M.qg_u * Z[0] + M.a_u * Zq, bX = M.qg_u * X[0] + M.a_u * Xq;
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            if (!BZ_ON(a)) continue;
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const double T = X[a] * fma(-M.a_u, Z[a], fma(M.d1b_u, Z[ab], bZ));
+            const double U = Z[a] * fma(-M.a_u, X[a], fma(M.d1b_u, X[ab], bX));
+            dI[a] -= T; dL[a] += T; dJ[a] -= U; dK[a] += U;
+        }
+    }
+    // ------------------------------------------------------------------ s-family: pairs at (i,j) -> pairs at (k,l)
+    {
+        double In[7], Out[7], Inf[3], Outf[3];
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            const bool ok = BZ_ON(a) && BZ_ON(ab);
+            In[a] = ok ? Pi[a] * Pj[ab] : 0.0;
+            Out[a] = ok ? Qk[a] * Ql[ab] : 0.0;
+        }
+#pragma unroll
+        for (int p = 0; p < 3; ++p) { Inf[p] = In[1 + 2 * p] + In[2 + 2 * p]; Outf[p] = Out[1 + 2 * p] + Out[2 + 2 * p]; }
+        const double Inq = (Inf[0] + Inf[1]) + Inf[2], Outq = (Outf[0] + Outf[1]) + Outf[2];
+        const double Ing = glue ? Pi[0] * Pj[0] : 0.0, Outg = glue ? Qk[0] * Ql[0] : 0.0;
+        if (glue) {
+            const double Sg = M.qqgg * (Ing * Outq), Rg = M.qqgg * (Outg * Inq);
+            dI[0] -= Sg; dJ[0] -= Sg; dK[0] += Rg; dL[0] += Rg;
+        }
+        const double bOut = M.qqgg * Outg + M.ann * Outq, bIn = M.qqgg * Ing + M.ann * Inq;
+#pragma unroll
+        for (int a = 1; a < 7; ++a) {
+            const int ab = (a & 1) ? a + 1 : a - 1;
+            if (!(BZ_ON(a) && BZ_ON(ab))) continue;
+            const int p = (a - 1) >> 1;
+            const double S = In[a] * fma(-M.ann, Outf[p], bOut);
+            const double R = Out[a] * fma(-M.ann, Inf[p], bIn);
+            dI[a] -= S; dJ[ab] -= S; dK[a] += R; dL[ab] += R;
+        }
+    }
+#undef BZ_ON
+}
+
+// the |M|^2 set with every value negated: the loss half's sign
+BZ_HD MsqSet msq_negated(const MsqSet& M)
+{
+    MsqSet N;
+    N.gg = -M.gg; N.qqgg = -M.qqgg; N.qg_t = -M.qg_t; N.qg_u = -M.qg_u; N.m11 = -M.m11; N.m1b_t = -M.m1b_t; N.m1b_u = -M.m1b_u;
+    N.ann = -M.ann; N.a_t = -M.a_t; N.a_u = -M.a_u; N.d11 = -M.d11; N.d1b_t = -M.d1b_t; N.d1b_u = -M.d1b_u;
+    return N;
+}
+
 }  // namespace bz

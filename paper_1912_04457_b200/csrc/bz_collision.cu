@@ -153,6 +153,7 @@ struct alignas(16) Chan {
     uint64_t done;                                       // consumer -> producer: the stage buffer may be overwritten
 };
 
+constexpr int kMaxDevices = 64;
 constexpr int kRetryCap = 64;                    // per producer warp: samples whose two Marsaglia attempts both failed
 
 // ---- producer: wait until the stage buffer is free, issue the gather of the batch in rec[ridx], hand it to the consumer
@@ -370,6 +371,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
     int count = 0;                       // records in it
     int rcount = 0;                      // entries in the retry list
     unsigned in_flight = 0;              // a batch has been submitted and its "done" phase not yet consumed
+    unsigned long long n_acc = 0ull;     // samples accepted by this warp (bz_get_sample_counts)
     unsigned dpar = 0;                   // parity of the next "done" phase
     for (;;) {
         unsigned item = 0;
@@ -418,6 +420,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             }
             // ---- compact the accepted samples into the current record buffer; a full buffer goes to the consumer
             const unsigned acc = __ballot_sync(0xffffffffu, sa.flag);
+            n_acc += (unsigned)__popc(acc);
             if (acc == 0u) continue;
             int pos = count + __popc(acc & lt);
             if (sa.flag && pos < 32) {
@@ -445,6 +448,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         }
     }
     submit_batch<kSP>(ch, P.f_aos, P.dN_aos, P.Np, P.S, lane, cur, -1, 0, 0.0, in_flight, dpar);   // flush the last batch, then the terminator
+    if (lane == 0 && P.counters) atomicAdd(P.counters, n_acc);
 }
 
 // p1-cell table: (p1x, p1y, p1z, E1) of every momentum cell centre, with the arithmetic of S8c steps 0 and 2
@@ -478,12 +482,12 @@ __global__ void debug_samples_kernel(const CollideParams P, int xcell, int p_beg
 // f (species-major, the API layout) -> cell-major staging copy f_aos[x][p][SP]; pad slots are written as 0
 __global__ void __launch_bounds__(256) pack_kernel(const double* __restrict__ f, double* __restrict__ f_aos, int S, int SP, int Np)
 {
-    const int xcell = blockIdx.y;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= Np) return;
+    const int xcell = blockIdx.x;
     const double* fx = f + (size_t)xcell * S * Np;
-    double* o = f_aos + ((size_t)xcell * Np + p) * SP;
-    for (int a = 0; a < SP; ++a) o[a] = a < S ? fx[(size_t)a * Np + p] : 0.0;
+    for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < Np; p += gridDim.y * blockDim.x) {
+        double* o = f_aos + ((size_t)xcell * Np + p) * SP;
+        for (int a = 0; a < SP; ++a) o[a] = a < S ? fx[(size_t)a * Np + p] : 0.0;
+    }
 }
 
 // dF[x][a][p] = dN_aos[x][p][a] / N_a, and the scratch is reset to 0
@@ -492,14 +496,14 @@ __global__ void __launch_bounds__(256) finalize_kernel(double* __restrict__ dN_a
                                                         const double d4, const double d5, const double d6)
 {
     const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
-    const int xcell = blockIdx.y;
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= Np) return;
-    double* src = dN_aos + ((size_t)xcell * Np + p) * SP;
+    const int xcell = blockIdx.x;
     double* dx = dF + (size_t)xcell * S * Np;
-    for (int a = 0; a < S; ++a) {
-        dx[(size_t)a * Np + p] = src[a] / deg[a];
-        src[a] = 0.0;
+    for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < Np; p += gridDim.y * blockDim.x) {
+        double* src = dN_aos + ((size_t)xcell * Np + p) * SP;
+        for (int a = 0; a < S; ++a) {
+            dx[(size_t)a * Np + p] = src[a] / deg[a];
+            src[a] = 0.0;
+        }
     }
 }
 
@@ -508,11 +512,15 @@ cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t s
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
     const size_t smem = sizeof(Chan<kSP>) * kProducerWarps + sizeof(int2) * kRetryCap * kProducerWarps;
-    static bool configured = false;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the attribute belongs to the (function, device) pair: one flag per device, not per process
+    static bool configured[kMaxDevices] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices || !configured[dev]) {
+        e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < kMaxDevices) configured[dev] = true;
     }
     collide_kernel<kMask><<<ctas, kCollideThreads, smem, st>>>(P);
     ++g_launch_count;
@@ -566,7 +574,7 @@ cudaError_t launch_cell_table(const GridConst& g, int Np, double* tab, cudaStrea
 
 cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, int Np, cudaStream_t st)
 {
-    dim3 grid((Np + 255) / 256, Nx);
+    dim3 grid(Nx, min((Np + 255) / 256, 65535));
     pack_kernel<<<grid, 256, 0, st>>>(f, f_aos, S, SP, Np);
     ++g_launch_count;
     return cudaGetLastError();
@@ -574,7 +582,7 @@ cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, i
 
 cudaError_t launch_finalize(double* dN_aos, double* dF, int Nx, int S, int SP, int Np, const double* deg, cudaStream_t st)
 {
-    dim3 grid((Np + 255) / 256, Nx);
+    dim3 grid(Nx, min((Np + 255) / 256, 65535));
     finalize_kernel<<<grid, 256, 0, st>>>(dN_aos, dF, S, SP, Np, deg[0], deg[1], deg[2], deg[3], deg[4], deg[5], deg[6]);
     ++g_launch_count;
     return cudaGetLastError();

@@ -22,6 +22,7 @@ struct CollideParams {
     const double* m2;     // [Nx] regulator mass^2
     const double* cell_tab;   // [Np][4] (p1x, p1y, p1z, E1) of the momentum cell centres
     int S, Np, Nx, Ns;
+    unsigned long long* counters;   // device [1]: kinematic samples accepted (both outgoing legs in the box), accumulated over launches
     unsigned* work_counter;   // device: next work item of the persistent kernel (0 on entry)
     unsigned* next_counter;   // device: the counter of the NEXT launch, zeroed by this one
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
@@ -74,6 +75,7 @@ struct TransportParams {
 
 struct bz_ctx_impl {
     bz_grid grid;
+    int device;                      // the CUDA device the context was created on; every entry point switches to it
     int S, Nx, Np, Ns;
     int species[7], slot[7];
     unsigned mask;
@@ -91,12 +93,15 @@ struct bz_ctx_impl {
     int paper_n_groups, paper_n_channels;
     int coll_mode;                   // bz_set_collision: 0 CM sampler (hot path), 1 the paper's sampler (bz_collision_paper)
     double* dF_scratch;              // device n_values, allocated at the first bz_step with coll_mode 1
+    double* diag;                    // device [Nx][5], allocated at the first bz_energy_diag
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
     double *f, *f_new;               // device, n_values each (API layout [Nx][S][Np])
     double *f_aos, *dN_aos;          // device, Nx*Np*SP each (cell-major staging for the collision kernel)
     int SP;                          // doubles per cell in the staging layout
+    unsigned long long* counters;    // device [1]: samples accepted by the collision kernels since the last reset
+    unsigned long long generated;    // host: samples generated by the collision kernels since the last reset
     unsigned* work_counter;          // device, 2 words used alternately (each launch zeroes the other one)
     unsigned launch_parity;          // which of the two the next launch uses
     bool aos_valid;                  // f_aos holds the current f (written by the Euler kernel; bz_set_f invalidates)

@@ -120,8 +120,10 @@ __global__ void m2_kernel(const double* __restrict__ rowsum, double* __restrict_
     m2[x] = g2 * acc;
 }
 
-// per-cell (n, e), totals over x in a fixed order (one thread per species), then m2 copied behind them
-__global__ void moments_kernel(const double* __restrict__ rowsum, const double* __restrict__ m2, double* __restrict__ mom,
+// per-cell (n, e) and m2 copied behind them (all blocks); totals over the own cells x_begin..x_end: block b < 2 S sums
+// total b = (species b / 2, n or e) with all its threads (strided partial sums, then a fixed-order tree: the result
+// does not depend on the launch)
+__global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__ rowsum, const double* __restrict__ m2, double* __restrict__ mom,
                                int Nx, int S, double d3p_over_2pi3, double d3x, int x_begin, int x_end, const double d0, const double d1,
                                const double d2, const double d3, const double d4, const double d5, const double d6)
 {
@@ -134,11 +136,19 @@ __global__ void moments_kernel(const double* __restrict__ rowsum, const double* 
     }
     for (size_t x = blockIdx.x * (size_t)blockDim.x + threadIdx.x; x < (size_t)Nx; x += (size_t)gridDim.x * blockDim.x)
         mom[2 * rows + 2 * S + x] = m2[x];
-    if (blockIdx.x == 0 && threadIdx.x < 2 * S) {
-        const int a = threadIdx.x >> 1, c = threadIdx.x & 1;
+    if (blockIdx.x < 2 * S) {
+        const int a = blockIdx.x >> 1, c = blockIdx.x & 1;
         double t = 0.0;
-        for (int x = x_begin; x < x_end; ++x) t += (deg[a] * rowsum[3 * ((size_t)x * S + a) + c] * d3p_over_2pi3) * d3x;
-        mom[2 * rows + threadIdx.x] = t;
+        for (int x = x_begin + threadIdx.x; x < x_end; x += blockDim.x)
+            t += (deg[a] * rowsum[3 * ((size_t)x * S + a) + c] * d3p_over_2pi3) * d3x;
+        __shared__ double sh[256];
+        sh[threadIdx.x] = t;
+        __syncthreads();
+        for (int o = 128; o > 0; o >>= 1) {
+            if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) mom[2 * rows + blockIdx.x] = sh[0];
     }
 }
 
@@ -177,6 +187,7 @@ cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, 
 {
     int blocks = (Nx * S + 255) / 256;
     if (blocks > 148) blocks = 148;
+    if (blocks < 2 * S) blocks = 2 * S;          // one block per total
     moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, x_begin, x_end, deg[0], deg[1], deg[2], deg[3], deg[4],
                                            deg[5], deg[6]);
     ++g_launch_count;

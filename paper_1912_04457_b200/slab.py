@@ -45,6 +45,7 @@ class SlabDomain:
         self.down = (rank - 1) % world
         self.up = (rank + 1) % world
         self._recv_lo = self._recv_hi = None
+        self._stage_lo = self._stage_hi = None
 
     # ---- state
     def set_own(self, f_own):
@@ -60,6 +61,12 @@ class SlabDomain:
         e = self.engine
         lo = e.get_layers(1, 1)                     # lowest own layer  -> the lower neighbour's upper halo
         hi = e.get_layers(self.nz_local, 1)         # highest own layer -> the upper neighbour's lower halo
+        self._exchange(lo, hi)
+
+    def _exchange(self, lo, hi):
+        """lo / hi: this rank's lowest / highest own layer as flat tensors on the engine's device, produced on the
+        engine's stream.  They go to the lower / upper neighbour; what comes back fills the two halo layers."""
+        e = self.engine
         if self.world == 1:
             e.set_layers(self.nz_local + 1, 1, lo)
             e.set_layers(0, 1, hi)
@@ -67,7 +74,12 @@ class SlabDomain:
         if self._recv_lo is None:
             self._recv_lo, self._recv_hi = torch.empty_like(lo), torch.empty_like(hi)
         if lo.is_cuda:
-            torch.cuda.current_stream(lo.device).synchronize()      # the pack copies ran on the engine's stream
+            # NCCL's send/recv kernels run on the process group's own stream, which waits for the CURRENT torch stream;
+            # the engine works on the stream that was current when it was made: the two are the same unless the caller
+            # changed streams, in which case the current one is made to wait for the engine's here.
+            cur = torch.cuda.current_stream(lo.device)
+            if getattr(e, "stream", None) is not None and e.stream != cur:
+                cur.wait_stream(e.stream)
         # Message order between a pair of ranks is the same on both sides (down-going first, tag 0; up-going second,
         # tag 1), which is what NCCL matches by (it ignores tags) and gloo matches by tag; with two ranks both
         # neighbours are the same peer.
@@ -76,7 +88,7 @@ class SlabDomain:
                dist.P2POp(dist.irecv, self._recv_hi, self.up, self.group, 0),
                dist.P2POp(dist.irecv, self._recv_lo, self.down, self.group, 1)]
         for req in dist.batch_isend_irecv(ops):
-            req.wait()
+            req.wait()                              # CUDA: the current stream waits for the transfer, the host does not block
         e.set_layers(self.nz_local + 1, 1, self._recv_hi)
         e.set_layers(0, 1, self._recv_lo)
 
@@ -85,6 +97,22 @@ class SlabDomain:
         """One Euler step of the whole domain's share on this rank: halo exchange, then bz_step."""
         self.exchange_halos()
         self.engine.step(dt)
+
+    def step_host(self, dt, f_in_host, f_out_host):
+        """The same step end to end from HOST memory (pinned): f_in_host / f_out_host have the size of the whole local
+        context (nz_local + 2 layers), of which only the own layers 1 .. nz_local are read / written.  The two boundary
+        layers go to the device first and are exchanged with the neighbours while bz_step_host pipelines the own layers
+        (host-to-device copy, collision, stream + Euler, device-to-host copy by chunks of z layers)."""
+        e = self.engine
+        lv = e.layer_values()
+        flat = f_in_host.reshape(-1)
+        if self._stage_lo is None:
+            self._stage_lo = torch.empty(lv, dtype=torch.float64, device=e.device)
+            self._stage_hi = torch.empty(lv, dtype=torch.float64, device=e.device)
+        self._stage_lo.copy_(flat[lv:2 * lv], non_blocking=True)
+        self._stage_hi.copy_(flat[self.nz_local * lv:(self.nz_local + 1) * lv], non_blocking=True)
+        self._exchange(self._stage_lo, self._stage_hi)
+        e.step_host(dt, f_in_host, f_out_host)
 
     def moments_totals(self):
         """[S, 2] totals (N_a, E_a) over the WHOLE domain: the local totals (own layers only) all-reduced."""

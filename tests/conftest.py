@@ -11,6 +11,16 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: long oracle runs (still part of the default CPU suite unless deselected)")
+    config.addinivalue_line("markers", "long: opt-in runs of several minutes (set BZ_LONG=1), e.g. config 3 for all of its 20 steps")
+
+
+def pytest_collection_modifyitems(config, items):
+    if os.environ.get("BZ_LONG") == "1":
+        return
+    skip = pytest.mark.skip(reason="opt-in: set BZ_LONG=1")
+    for item in items:
+        if item.get_closest_marker("long"):
+            item.add_marker(skip)
 
 
 @pytest.fixture(scope="session")

@@ -189,3 +189,23 @@ def test_R5_full_program_step_conserves_particle_number():
         masses.append(o.get_masses().copy())
         assert o.moments()["tot"][:, 0].sum() == pytest.approx(N0, rel=1e-13)
     assert (masses[0] > 0).all() and not np.array_equal(masses[0], masses[2])
+
+
+@pytest.mark.parametrize("masses", [None, (0.41, 0.13, 0.13, 0.13), (0.5, 0.2, 0.25, 0.3)], ids=["massless", "equal_quarks", "four_masses"])
+def test_R6_grouping_by_mass_tuple_equals_the_channel_by_channel_sum(masses):
+    """bzo_collision_paper solves the roots once per distinct tuple of mass classes; bzo_collision_paper_plain walks
+    Eq. 3-4 as printed (sample -> channel -> that channel's own root solve -> deposit).  Same roots, same terms, another
+    summation order: they agree to rounding on the scale of the gross deposit (S16), massless, with degenerate quark
+    masses and with four distinct masses, on two spatial cells with different masses."""
+    o = bzo.Oracle(nx=2, ny=1, nz=1, dx=0.3, np_=5, pmin=-3.0, pmax=3.0, species=SP7, samples=12, seed=9, threads=2)
+    rng = np.random.Generator(np.random.Philox(key=19))
+    o.set_f(0.02 + 0.5 * rng.random(o.shape))
+    if masses is not None:
+        o.set_masses(np.array([masses, [1.3 * m for m in masses]]))
+    a = o.collision_paper(0.01, 4)
+    ga = o.gross()
+    b = o.collision_paper_plain(0.01, 4)
+    gb = o.gross()
+    assert np.abs(a).max() > 0 and np.count_nonzero(a) > 0.5 * a.size
+    assert np.all(np.abs(a - b) <= 1e-13 * np.maximum(ga, np.abs(a)))
+    assert np.all(np.abs(ga - gb) <= 1e-13 * ga)
