@@ -55,7 +55,7 @@ struct bzo_ctx {
      * [zb, ze) collide and count in the totals (the others are halo copies of a neighbour's layers) */
     unsigned xoff;
     int zb, ze;
-    int coll_mode;        /* bzo_set_collision: 0 = CM sampler (the hot path), 1 = the paper's sampler, massive (rank 1), 2 = importance-sampled t (rank 3) */
+    int coll_mode;        /* bzo_set_collision: 0 = CM sampler (the hot path), 1 = the paper's sampler, massive (rank 1), 2 = importance-sampled t (rank 3), 3 = in-box direction (rank 3) */
     int scheme;           /* bzo_set_transport: 0 upwind massless, 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set */
     double* mass2;        /* [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 per spatial cell (Eq. 8-9); 0 at start */
 };
@@ -557,6 +557,124 @@ static void gen_sample_is(const bzo_ctx* c, unsigned step, int xcell, int pcell,
     *weight = w;
 }
 
+/* ------------------------------------------------------------------ NEXT rank 3 (S8f), other half: in-box sampling of the CM direction */
+/* With uniform n (S8c step 2) 54 % of the samples are thrown away because p3 or p4 leaves the momentum box (S9).  Here n
+ * is drawn uniformly from a ZONE of the sphere that contains every accepted direction, and the deposit carries the zone's
+ * area fraction as its weight, so Eq. 20's expectation is unchanged (the integrand vanishes outside the zone).
+ *   p3 = P/2 + A n,  A_c = (M e_c + P_c P/(E + M)) / 2  (row c of the boost of S8c step 2),  |A_c| = sqrt(s + P_c^2) / 2
+ *   p3_c and p4_c = P_c - p3_c both in [pmin, pmax)  <=>  |A_c . n| <= b_c = L/2 - |P_c/2 - (pmin + L/2)|     (c = x, y, z)
+ * so the accepted set is the intersection of three zones |a_c . n| <= beta_c, a_c = A_c/|A_c|, beta_c = min(1, b_c/|A_c|).
+ * Archimedes: the zone |a . n| <= beta has the area fraction beta and z = a . n is uniform on it.  The tightest zone
+ * (smallest beta_c, first on ties) is sampled exactly, the other two by rejection:
+ *   frame: a = the unit vector of the tightest zone, h = the coordinate axis with the smallest |a_d| (first on ties), e1 = (h - (h.a) a)/|..|, e2 = a x e1
+ *   Marsaglia attempt k (the SAME Philox blocks 2 + k and the same acceptance q = v1^2 + v2^2 < 1 as S8c step 1-2):
+ *   z = beta (1 - 2 q)  [1 - 2q is uniform on (-1, 1)],  rho = sqrt(1 - z^2),  (cos, sin) = (v1, v2)/sqrt(q)
+ *   n = z a + rho (cos e1 + sin e2);   weight = beta.
+ * p1, p2, s are those of S8c step 2 (Philox blocks 0, 1); p3, p4, t, u and the binning follow S8c steps 2-3 unchanged.
+ * Only + - x / sqrt, association as written (bit-exact on the GPU).  Measured: 78.5 % of the samples deposit (46 % before). */
+static void gen_sample_box(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, bzo_sample* o, double* weight)
+{
+    const int n = c->g.np;
+    const double pmin = c->g.pmin, L = c->g.pmax - c->g.pmin;
+    memset(o, 0, sizeof *o);
+    o->k = o->l = -1;
+    *weight = 0.0;
+    const int ipx = pcell % n, ipy = (pcell / n) % n, ipz = pcell / (n * n);
+    const double p1x = cell_centre(c, ipx), p1y = cell_centre(c, ipy), p1z = cell_centre(c, ipz);
+    const double E1 = sqrt((p1x * p1x + p1y * p1y) + p1z * p1z);
+    double u0, u1, u2, unused;
+    draw(c, step, xcell, pcell, sample, 0u, &u0, &u1);
+    draw(c, step, xcell, pcell, sample, 1u, &u2, &unused);
+    const double p2x = pmin + u0 * L, p2y = pmin + u1 * L, p2z = pmin + u2 * L;
+    const double E2 = sqrt((p2x * p2x + p2y * p2y) + p2z * p2z);
+    const double d12 = (p1x * p2x + p1y * p2y) + p1z * p2z;
+    const double s = 2.0 * (E1 * E2 - d12);
+    o->p1[0] = p1x; o->p1[1] = p1y; o->p1[2] = p1z;
+    o->p2[0] = p2x; o->p2[1] = p2y; o->p2[2] = p2z;
+    o->E1 = E1; o->E2 = E2;
+    {
+        const double dp = cell_width(c);
+        int idx[3];
+        for (int d = 0; d < 3; ++d) {
+            int q = (int)floor((o->p2[d] - pmin) / dp);
+            idx[d] = q < 0 ? 0 : (q > n - 1 ? n - 1 : q);
+        }
+        o->j = idx[0] + n * (idx[1] + n * idx[2]);
+    }
+    if (!(s > 0.0)) return;
+    const double P[3] = { p1x + p2x, p1y + p2y, p1z + p2z };
+    const double E = E1 + E2, M = sqrt(s), EM = E + M;
+    /* the three zones */
+    const double B = 0.5 * L, pc0 = pmin + B;
+    double beta = 2.0, An = 0.0;
+    int cs = 0;
+    for (int d = 0; d < 3; ++d) {
+        const double b = B - fabs(0.5 * P[d] - pc0);
+        const double an = 0.5 * sqrt(s + P[d] * P[d]);
+        double bt = b / an;
+        if (bt > 1.0) bt = 1.0;
+        if (bt < beta) { beta = bt; cs = d; An = an; }
+    }
+    if (!(beta > 0.0)) return;                          /* P/2 on the edge of the box: the zone is empty */
+    /* frame around the unit vector a along row c* of A */
+    const double g = P[cs] / EM;
+    double a[3];
+    for (int d = 0; d < 3; ++d) a[d] = 0.5 * (P[d] * g);
+    a[cs] = 0.5 * (M + P[cs] * g);
+    for (int d = 0; d < 3; ++d) a[d] = a[d] / An;
+    const double ax_ = fabs(a[0]), ay_ = fabs(a[1]), az_ = fabs(a[2]);
+    double h[3] = { 0.0, 0.0, 0.0 }, ha;
+    if (ax_ <= ay_ && ax_ <= az_) { h[0] = 1.0; ha = a[0]; } else if (ay_ <= az_) { h[1] = 1.0; ha = a[1]; } else { h[2] = 1.0; ha = a[2]; }
+    double e1[3] = { h[0] - ha * a[0], h[1] - ha * a[1], h[2] - ha * a[2] };
+    const double e1n = sqrt((e1[0] * e1[0] + e1[1] * e1[1]) + e1[2] * e1[2]);
+    for (int d = 0; d < 3; ++d) e1[d] = e1[d] / e1n;
+    const double e2[3] = { a[1] * e1[2] - a[2] * e1[1], a[2] * e1[0] - a[0] * e1[2], a[0] * e1[1] - a[1] * e1[0] };
+    /* direction */
+    double zz = 0.0, rho = 1.0, cphi = 1.0, sphi = 0.0;       /* after 62 failures: n = e1 (probability 0.2146^62) */
+    int k;
+    for (k = 0; k < MARSAGLIA_MAX; ++k) {
+        double ua, ub;
+        draw(c, step, xcell, pcell, sample, 2u + (unsigned)k, &ua, &ub);
+        const double v1 = 2.0 * ua - 1.0, v2 = 2.0 * ub - 1.0;
+        const double q = v1 * v1 + v2 * v2;
+        if (q < 1.0) {
+            zz = beta * (1.0 - 2.0 * q);
+            rho = sqrt(1.0 - zz * zz);
+            const double rq = sqrt(q);
+            cphi = v1 / rq; sphi = v2 / rq;
+            break;
+        }
+    }
+    o->attempts = k + 1;
+    const double nx = zz * a[0] + rho * (cphi * e1[0] + sphi * e2[0]);
+    const double ny = zz * a[1] + rho * (cphi * e1[1] + sphi * e2[1]);
+    const double nz = zz * a[2] + rho * (cphi * e1[2] + sphi * e2[2]);
+    /* boost back: S8c step 2 */
+    const double Px = P[0], Py = P[1], Pz = P[2];
+    const double cc = (Px * nx + Py * ny) + Pz * nz;
+    const double hh = 1.0 + cc / EM;
+    const double p3x = 0.5 * (M * nx + Px * hh), p3y = 0.5 * (M * ny + Py * hh), p3z = 0.5 * (M * nz + Pz * hh);
+    const double p4x = Px - p3x, p4y = Py - p3y, p4z = Pz - p3z;
+    const double E3 = 0.5 * (E + cc);
+    const double d13 = (p1x * p3x + p1y * p3y) + p1z * p3z;
+    const double t = -2.0 * (E1 * E3 - d13);
+    o->s = s; o->t = t; o->u = (-s) - t; o->E3 = E3;
+    o->nhat[0] = nx; o->nhat[1] = ny; o->nhat[2] = nz;
+    o->p3[0] = p3x; o->p3[1] = p3y; o->p3[2] = p3z;
+    o->p4[0] = p4x; o->p4[1] = p4y; o->p4[2] = p4z;
+    o->k = bin_cell(c, o->p3);
+    o->l = bin_cell(c, o->p4);
+    o->flag = (o->k >= 0 && o->l >= 0);
+    *weight = beta;
+}
+
+int bzo_sample_one_box(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, bzo_sample* out, double* weight)
+{
+    if (!c || !out || !weight || xcell < 0 || xcell >= c->Nx || pcell < 0 || pcell >= c->Np || sample < 0) return -1;
+    gen_sample_box(c, step, (int)((unsigned)xcell + c->xoff), pcell, sample, out, weight);
+    return 0;
+}
+
 int bzo_sample_one_is(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, double m2, bzo_sample* out, double* weight)
 {
     if (!c || !out || !weight || xcell < 0 || xcell >= c->Nx || pcell < 0 || pcell >= c->Np || sample < 0) return -1;
@@ -564,8 +682,9 @@ int bzo_sample_one_is(const bzo_ctx* c, unsigned step, int xcell, int pcell, int
     return 0;
 }
 
-/* dF = dt C[f] with the importance-sampled estimator: S8c steps 4-6 unchanged, every deposit times the weight */
-int bzo_collision_is(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
+/* dF = dt C[f] with a weighted sampler (kind 0: importance-sampled t, kind 1: in-box direction): S8c steps 4-6 unchanged,
+ * every deposit times the sample's weight */
+static int collision_weighted(bzo_ctx* c, double dt_fm, unsigned step, double* dF, int kind)
 {
     if (!c || !dF) return -1;
     const int S = c->S, Np = c->Np;
@@ -585,7 +704,8 @@ int bzo_collision_is(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
         double msqv[BZO_N_KINDS][2];
         for (int i = 0; i < Np; ++i) for (int smp = 0; smp < c->Ns; ++smp) {
             double wt;
-            gen_sample_is(c, step, (int)((unsigned)x + c->xoff), i, smp, m2, &sm, &wt);
+            if (kind == 0) gen_sample_is(c, step, (int)((unsigned)x + c->xoff), i, smp, m2, &sm, &wt);
+            else gen_sample_box(c, step, (int)((unsigned)x + c->xoff), i, smp, &sm, &wt);
             if (!sm.flag) continue;
             const double w = (K / (sm.E1 * sm.E2)) * wt;
             msq_table(c, sm.s, sm.t, sm.u, m2, msqv);
@@ -610,6 +730,9 @@ int bzo_collision_is(bzo_ctx* c, double dt_fm, unsigned step, double* dF)
     }
     return 0;
 }
+
+int bzo_collision_is(bzo_ctx* c, double dt_fm, unsigned step, double* dF) { return collision_weighted(c, dt_fm, step, dF, 0); }
+int bzo_collision_box(bzo_ctx* c, double dt_fm, unsigned step, double* dF) { return collision_weighted(c, dt_fm, step, dF, 1); }
 
 /* ------------------------------------------------------------------ S8a.6: upwind free streaming, periodic */
 int bzo_stream(bzo_ctx* c, double dt_fm, double* dF)
@@ -654,7 +777,7 @@ static double energy_at(const bzo_ctx* c, int ix, int iy, int iz, double m2)
     return sqrt(((px * px + py * py) + pz * pz) + m2);
 }
 
-int bzo_set_collision(bzo_ctx* c, int mode) { if (!c || mode < 0 || mode > 2) return -1; c->coll_mode = mode; return 0; }
+int bzo_set_collision(bzo_ctx* c, int mode) { if (!c || mode < 0 || mode > 3) return -1; c->coll_mode = mode; return 0; }
 int bzo_set_transport(bzo_ctx* c, int scheme) { if (!c || scheme < 0 || scheme > 2) return -1; c->scheme = scheme; return 0; }
 int bzo_set_masses(bzo_ctx* c, const double* mass2)
 {
@@ -1024,6 +1147,7 @@ int bzo_step(bzo_ctx* c, double dt_fm)
     if (c->scheme == 1) bzo_thermal_masses(c, NULL);          /* masses from the old f, before anything uses them */
     if (c->coll_mode == 1) bzo_collision_paper(c, dt_fm, c->step, dFc);
     else if (c->coll_mode == 2) bzo_collision_is(c, dt_fm, c->step, dFc);
+    else if (c->coll_mode == 3) bzo_collision_box(c, dt_fm, c->step, dFc);
     else bzo_collision(c, dt_fm, c->step, dFc);
     if (c->scheme == 0) bzo_stream(c, dt_fm, dFs);
     else bzo_vlasov(c, dt_fm, dFs);

@@ -86,7 +86,7 @@ int  bzo_vlasov   (bzo_ctx*, double dt_fm, double* dF);
 /* transport used by bzo_step: 0 = upwind massless (default), 1 = Eq. 15 with the masses re-evaluated from the old f
  * every step, 2 = Eq. 15 with the masses as stored */
 int  bzo_set_transport(bzo_ctx*, int scheme);
-/* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper, 2 = bzo_collision_is */
+/* collision term used by bzo_step: 0 = bzo_collision (default), 1 = bzo_collision_paper, 2 = bzo_collision_is, 3 = bzo_collision_box */
 int  bzo_set_collision(bzo_ctx*, int mode);
 /* ---- NEXT rank 3 (S8f): importance sampling of the t/u-channel peaks of Table I --------------------------------
  * bzo_collision_is: the estimator of bzo_collision with t drawn from (1/2)[g(t) + g(u)], g ~ 1/(m^2 - t)^2, the azimuth
@@ -94,6 +94,12 @@ int  bzo_set_collision(bzo_ctx*, int mode);
  * bzo_sample_one_is: one such sample (fields as bzo_sample_one; attempts = azimuth attempts) and its weight. */
 int  bzo_collision_is(bzo_ctx*, double dt_fm, unsigned step, double* dF);
 int  bzo_sample_one_is(const bzo_ctx*, unsigned step, int xcell, int pcell, int sample, double m2, bzo_sample* out, double* weight);
+/* ---- NEXT rank 3 (S8f), the other half: the CM direction is drawn uniformly from the tightest of the three zones
+ * |a_c . n| <= beta_c of the sphere outside which p3 or p4 leaves the momentum box (Archimedes: area fraction beta_c, z
+ * uniform), weight beta: same expectation as bzo_collision (Eq. 20), 78 % instead of 46 % of the samples deposit.
+ * Same Philox blocks and Marsaglia acceptance as bzo_collision.  bzo_sample_one_box: one such sample and its weight. */
+int  bzo_collision_box(bzo_ctx*, double dt_fm, unsigned step, double* dF);
+int  bzo_sample_one_box(const bzo_ctx*, unsigned step, int xcell, int pcell, int sample, bzo_sample* out, double* weight);
 
 /* ---- NEXT rank 1 (S8f): the paper's own collision path (Eq. 17-21, massive dispersion) ----------------------------
  * one root of E1 + E2 = E3 + Ep (Eq. 18-19): momenta k1, k2, their cells, the four energies, the Jacobian of Eq. 19 and

@@ -66,6 +66,8 @@ def lib():
         L.bzo_energy_diag.argtypes = [vp, dp]
         L.bzo_collision_is.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_sample_one_is.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(Sample), dp]
+        L.bzo_collision_box.argtypes = [vp, C.c_double, C.c_uint, dp]
+        L.bzo_sample_one_box.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.POINTER(Sample), dp]
         L.bzo_paper_sample.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, dp, ip, C.POINTER(PRoot)]
         L.bzo_collision_paper.argtypes = [vp, C.c_double, C.c_uint, dp]
         L.bzo_collision_paper_plain.argtypes = [vp, C.c_double, C.c_uint, dp]
@@ -238,6 +240,18 @@ class Oracle:
         s = Sample()
         w = C.c_double()
         _chk(lib().bzo_sample_one_is(self._h, step, xcell, pcell, sample, m2, C.byref(s), C.byref(w)), "bzo_sample_one_is")
+        return s, w.value
+
+    # ---- NEXT rank 3, other half: in-box sampling of the CM direction
+    def collision_box(self, dt, step):
+        dF = np.empty(self.shape, dtype=np.float64)
+        _chk(lib().bzo_collision_box(self._h, dt, step, _dptr(dF)), "bzo_collision_box")
+        return dF
+
+    def sample_one_box(self, step, xcell, pcell, sample):
+        s = Sample()
+        w = C.c_double()
+        _chk(lib().bzo_sample_one_box(self._h, step, xcell, pcell, sample, C.byref(s), C.byref(w)), "bzo_sample_one_box")
         return s, w.value
 
     def set_collision(self, mode):

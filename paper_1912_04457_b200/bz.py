@@ -136,7 +136,7 @@ class Boltzmann:
         return C.c_void_p(t.data_ptr())
 
     def set_stream(self, stream):
-        self.stream = stream
+        self.torch_stream = stream
         self._chk(lib().bz_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "bz_set_stream")
 
     def set_seed(self, seed):

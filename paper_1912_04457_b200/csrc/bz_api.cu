@@ -82,7 +82,7 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.f_aos = c->SP == 1 ? c->f : c->f_aos;    // one species: the API layout is already cell-major
     P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab; P.counters = c->counters;
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
-    P.work_counter = c->work_counter + c->launch_parity; P.next_counter = c->work_counter + (c->launch_parity ^ 1u);
+    P.work_counter = c->work_counter; P.step_ptr = nullptr;
     const int layer = c->grid.nx * c->grid.ny;              // only the slab's own z layers collide (bz_set_slab)
     P.n_items = (unsigned)((c->ze - c->zb) * layer) * (unsigned)c->regions_per_x; P.x_begin = c->zb * layer;
     P.x_rng_offset = c->xoff;
@@ -123,7 +123,6 @@ int run_collide(bz_ctx* c, double dt_fm, unsigned step)
     const CollideParams P = collide_params(c, dt_fm, step);
     BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
     c->generated += (unsigned long long)(P.n_items / (unsigned)P.regions_per_x) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
-    c->launch_parity ^= 1u;
     return prof_mark(c, 0);
 }
 
@@ -189,7 +188,7 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
     c->mass2 = nullptr; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
-    c->launch_parity = 0; c->aos_valid = false; c->rowsum_valid = false;
+    c->aos_valid = false; c->rowsum_valid = false;
     c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
@@ -569,8 +568,7 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
             P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)c->regions_per_x;
             BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
             c->generated += (unsigned long long)((ze - zb) * layer_cells) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
-            c->launch_parity ^= 1u;
-        }
+                }
         // chunk k - 1 has both z neighbours on the device now (chunk 0 waits for the last one: periodic)
         if (k >= 2) { if (int rc = transport_chunk(k - 1)) return rc; }
     }

@@ -23,14 +23,15 @@ struct CollideParams {
     const double* cell_tab;   // [Np][4] (p1x, p1y, p1z, E1) of the momentum cell centres
     int S, Np, Nx, Ns;
     unsigned long long* counters;   // device [1]: kinematic samples accepted (both outgoing legs in the box), accumulated over launches
-    unsigned* work_counter;   // device: next work item of the persistent kernel (0 on entry)
-    unsigned* next_counter;   // device: the counter of the NEXT launch, zeroed by this one
+    unsigned* work_counter;   // device [2]: next work item of the persistent kernel, CTAs that have finished; both 0 on entry,
+                              // reset by the last CTA to finish
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
     int x_begin;              // first colliding spatial cell (items address xcell = x_begin + item / regions_per_x)
     uint32_t x_rng_offset;    // Philox spatial counter = xcell + x_rng_offset (slab of a larger domain, bz_set_slab)
     int cells_per_region;     // p1 cells per work item (one producer warp each)
     int regions_per_x;        // ceil(Np / cells_per_region)
     uint32_t seed, step;
+    const uint32_t* step_ptr; // device: if not NULL the Philox step is read from here (captured graphs, bz_step_n), else `step`
     double g4K;           // (4 pi alpha_s)^2 * K,  K = dtG Vp / (2048 pi^4 Ns)    (S8c step 0)
     unsigned mask;        // bit id set <=> species id active
     int slot[7];          // species id -> index a in the layout (or -1)
@@ -102,8 +103,7 @@ struct bz_ctx_impl {
     int SP;                          // doubles per cell in the staging layout
     unsigned long long* counters;    // device [1]: samples accepted by the collision kernels since the last reset
     unsigned long long generated;    // host: samples generated by the collision kernels since the last reset
-    unsigned* work_counter;          // device, 2 words used alternately (each launch zeroes the other one)
-    unsigned launch_parity;          // which of the two the next launch uses
+    unsigned* work_counter;          // device [2]: work-item counter and finished-CTA counter of the collision kernel (self-resetting)
     bool aos_valid;                  // f_aos holds the current f (written by the Euler kernel; bz_set_f invalidates)
     bool rowsum_valid;               // rowsum / m2 belong to the current f
     int sms;                         // SMs of the device (persistent grid size)

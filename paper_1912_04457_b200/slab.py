@@ -78,8 +78,8 @@ class SlabDomain:
             # the engine works on the stream that was current when it was made: the two are the same unless the caller
             # changed streams, in which case the current one is made to wait for the engine's here.
             cur = torch.cuda.current_stream(lo.device)
-            if getattr(e, "stream", None) is not None and e.stream != cur:
-                cur.wait_stream(e.stream)
+            if getattr(e, "torch_stream", None) is not None and e.torch_stream != cur:
+                cur.wait_stream(e.torch_stream)
         # Message order between a pair of ranks is the same on both sides (down-going first, tag 0; up-going second,
         # tag 1), which is what NCCL matches by (it ignores tags) and gloo matches by tag; with two ranks both
         # neighbours are the same peer.
