@@ -9,11 +9,11 @@
 //            bytes of each from the cell-major staging copy f_aos[xcell][pcell][8] into the warp's stage buffer: 4 lanes
 //            fetch one cell, one instruction fetches 8 cells.  The warp then runs its next sampling pass; the gather
 //            lands underneath it.
-//   algebra  TWO lanes per sample: the gain half and the loss half of every channel's bracket are the same expression with
-//            f and F = 1 +- f exchanged (deposit_half, bz_channels.cuh), so the even lane evaluates all gain terms and the
-//            odd lane all loss terms (with -|M|^2), each with half the registers the whole bracket needs -- which is what
-//            lets all 16 warps be identical instead of a few fat "consumer" warps that everything else waits for.  Each
-//            lane writes its 4 x S deposits back to the stage buffer.
+//   algebra  TWO lanes per sample: the loss half of every channel's bracket is the gain half of the time-reversed channel
+//            (deposit_half, bz_channels.cuh), so lane m evaluates all gain terms of sample m on the cells (i, j | k, l) and
+//            lane m + 16 the same code on (k, l | i, j), each with half the registers the whole bracket needs -- which is
+//            what lets all 16 warps be identical instead of a few fat "consumer" warps that everything else waits for.
+//            Each lane writes its 4 x S deposits back to the stage buffer.
 //   scatter  one sample per instruction: lane = (cell, slot), 8 lanes per 64-byte cell add the two halves and issue one
 //            fp64 reduction (RED.E.ADD.F64, no return value) into the cell-major scratch dN_aos, which stays in L2 while
 //            its spatial cell is being worked on.
@@ -69,17 +69,18 @@ __device__ __forceinline__ void red_add(double* gdst, double v)
 
 // ------------------------------------------------------------------------------------------------ shared memory
 // Per warp.  kSP == 8: the stage buffer holds, per sample of the batch in flight, the occupation numbers of its 4 cells
-// on the way in ([0, 32): 4 cells x 8 doubles, overwritten by the gain half's deposits) and the loss half's deposits
-// ([40, 72)); 74 doubles per sample.  Every cell is 16-byte aligned (cp.async 16).  In units of 16 bytes a sample starts
-// at 37 m and its loss area at 37 m + 20: within a quarter warp (4 samples x 2 halves) the eight 16-byte accesses fall
-// into eight different bank groups (m mod 8 and m + 4 mod 8), so the lane pairs' loads and stores are conflict free.
+// on the way in ([0, 32): 4 cells x 8 doubles, overwritten by the forward half's deposits) and the reversed half's
+// deposits ([32, 64)); 66 doubles per sample.  Every cell is 16-byte aligned (cp.async 16).  The two halves of a sample
+// sit in different half warps (lane and lane + 16), so a quarter warp's eight 16-byte accesses go to eight consecutive
+// samples, 33 x 16 bytes apart: eight different bank groups, no conflicts.
 template <int kSP>
 struct alignas(16) WarpMem {
     static constexpr int kBatch = kSP == 1 ? 32 : 16;    // samples per algebra pass
-    static constexpr int kStride = 74, kLoss = 40;
+    static constexpr int kStride = 66, kLoss = 32;
     double stage[kSP == 1 ? 2 : 16 * kStride];
     double p1tab[32][4];                                 // (p1x, p1y, p1z, E1) of the p1 cells of the current work item
-    unsigned cell[kRing][4];                             // i, j, k, l as indices into the whole grid: xcell * Np + pcell
+    unsigned cell[4][kRing + 4];                         // [slot i, j, k, l][record]: indices into the whole grid, xcell * Np + pcell
+                                                         // (rows 272 bytes apart: the four slots' 16-byte reads hit different banks)
     double s[kRing], t[kRing], e12[kRing];               // Mandelstam s, t and E1 E2 of the sample
     double m2x;                                          // regulator mass^2 of the current spatial cell
     int2 retry[kRetryCap];
@@ -95,23 +96,23 @@ __device__ __forceinline__ void cell_lookup(const double* __restrict__ tab, int 
     p1x = a.x; p1y = a.y; p1z = b.x; E1 = b.y;
 }
 
-// ---- gather: the 4 x 64 bytes of records [head, head + nb) into the stage buffer (kSP == 8)
+// ---- gather: the 4 x 64 bytes of records [head, head + nb) into the stage buffer (kSP == 8).  head is a multiple of 16
+// (a batch never wraps around the ring), so the cell indices of a lane's eight samples are two 16-byte loads.
 template <int kSP>
 __device__ __forceinline__ void issue_gather(WarpMem<kSP>& wm, const double* __restrict__ f_aos, int lane, int head, int nb)
 {
     using W = WarpMem<kSP>;
-    const int sub = lane >> 4, cc = (lane >> 2) & 3, q = lane & 3;     // 2 samples per instruction, 4 lanes per cell
+    const int sub = lane >> 4, cc = (lane >> 2) & 3, q = lane & 3;     // lanes 0-15: samples 0-7, lanes 16-31: samples 8-15; 4 lanes per cell
     const double* __restrict__ src = f_aos + q * 2;
-    double* dst = wm.stage + sub * W::kStride + cc * 8 + q * 2;
+    double* dst = wm.stage + sub * 8 * W::kStride + cc * 8 + q * 2;
+    const unsigned* cp = &wm.cell[cc][head + sub * 8];
     if (nb == W::kBatch) {
-        unsigned ci[W::kBatch / 2];
+        const uint4 c0 = *reinterpret_cast<const uint4*>(cp), c1 = *reinterpret_cast<const uint4*>(cp + 4);
+        const unsigned ci[8] = { c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w };
 #pragma unroll
-        for (int k = 0; k < W::kBatch / 2; ++k) ci[k] = wm.cell[(head + 2 * k + sub) & (kRing - 1)][cc];
-#pragma unroll
-        for (int k = 0; k < W::kBatch / 2; ++k) cp_async16(dst + 2 * k * W::kStride, src + (size_t)ci[k] * 8);
+        for (int k = 0; k < 8; ++k) cp_async16(dst + k * W::kStride, src + (size_t)ci[k] * 8);
     } else {
-        for (int m0 = 0; m0 + sub < nb; m0 += 2)
-            cp_async16(dst + m0 * W::kStride, src + (size_t)wm.cell[(head + m0 + sub) & (kRing - 1)][cc] * 8);
+        for (int k = 0; k < 8 && sub * 8 + k < nb; ++k) cp_async16(dst + k * W::kStride, src + (size_t)cp[k] * 8);
     }
     cp_async_commit();
 }
@@ -126,36 +127,39 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
     constexpr bool kQuark = kMask < 0 || (kMask & 0x7E);
     cp_async_wait_all();
     __syncwarp();                                        // every lane's gathers have landed
-    const int m = lane >> 1;
-    const bool loss = lane & 1;
+    // The loss half of a channel a b -> c d at the cells (i, j | k, l) is the GAIN half of the time-reversed channel
+    // c d -> a b at the cells (k, l | i, j): same s, t, u, same |M|^2 (the table is closed under time reversal, S8c step 5),
+    // and its deposits -H at (k, l), +H at (i, j) are exactly the loss term's.  So both lanes of a sample run the same gain
+    // algebra; the second one just takes the four cells in the order k, l, i, j, on the way in and on the way out.
+    const int m = lane & 15;                             // lanes 0-15: the forward halves of samples 0-15, lanes 16-31: the reversed ones
+    const int rev = (lane >> 4) * 16;                    // doubles: offset of the lane's "incoming" pair of cells
     double* st = wm.stage + m * W::kStride;
+    const double* sin_ = st + rev;                       // incoming legs: cells (i, j) or, reversed, (k, l)
+    const double* sout = st + (16 - rev);                // outgoing legs
     double d[4][7];
     const bool work = m < nb;
     if (work) {
-        const int r = (head + m) & (kRing - 1);
+        const int r = head + m;
         const double s = wm.s[r], t = wm.t[r];
         const double g4w = P.g4K * rcp_fast(wm.e12[r]);                   // g^4 K / (E1 E2), S8c step 6
-        // factors of this half: gain  P = f,           Q = F = 1 +- f   (incoming legs i, j / outgoing legs k, l)
-        //                       loss  P = F = 1 +- f,  Q = f            -- both as c + sigma f, no selects
-        const double cP = loss ? 1.0 : 0.0, cQ = loss ? 0.0 : 1.0;
-        const double sPq = loss ? -1.0 : 1.0, sQq = loss ? 1.0 : -1.0;   // quark sign of F = 1 - f; gluon: +
+        // gain factors: P = f at the incoming cells, Q = F = 1 + f (gluon), 1 - f (quark) at the outgoing ones
         double Pi[7], Pj[7], Qk[7], Ql[7];
         if constexpr (kMask >= 0) {
             constexpr unsigned km = (unsigned)kMask;
             constexpr int kPairs = (slot_of(km, 7) + 1) / 2;
             double2 v[4][4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c)
-#pragma unroll
-                for (int q = 0; q < kPairs; ++q) v[c][q] = *reinterpret_cast<const double2*>(st + c * 8 + 2 * q);
+            for (int q = 0; q < kPairs; ++q) {
+                v[0][q] = *reinterpret_cast<const double2*>(sin_ + 2 * q); v[1][q] = *reinterpret_cast<const double2*>(sin_ + 8 + 2 * q);
+                v[2][q] = *reinterpret_cast<const double2*>(sout + 2 * q); v[3][q] = *reinterpret_cast<const double2*>(sout + 8 + 2 * q);
+            }
 #pragma unroll
             for (int id = 0; id < 7; ++id) {
                 if ((kMask >> id) & 1) {
                     const int a = slot_of(km, id);
-                    const double fi = (a & 1) ? v[0][a >> 1].y : v[0][a >> 1].x, fj = (a & 1) ? v[1][a >> 1].y : v[1][a >> 1].x;
+                    Pi[id] = (a & 1) ? v[0][a >> 1].y : v[0][a >> 1].x; Pj[id] = (a & 1) ? v[1][a >> 1].y : v[1][a >> 1].x;
                     const double fk = (a & 1) ? v[2][a >> 1].y : v[2][a >> 1].x, fl = (a & 1) ? v[3][a >> 1].y : v[3][a >> 1].x;
-                    if (id == 0) { Pi[0] = fi + cP; Pj[0] = fj + cP; Qk[0] = fk + cQ; Ql[0] = fl + cQ; }
-                    else { Pi[id] = fma(sPq, fi, cP); Pj[id] = fma(sPq, fj, cP); Qk[id] = fma(sQq, fk, cQ); Ql[id] = fma(sQq, fl, cQ); }
+                    Qk[id] = id == 0 ? 1.0 + fk : 1.0 - fk; Ql[id] = id == 0 ? 1.0 + fl : 1.0 - fl;
                 } else {
                     Pi[id] = Pj[id] = Qk[id] = Ql[id] = 0.0;
                 }
@@ -165,25 +169,26 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
             for (int id = 0; id < 7; ++id) {
                 if ((mask >> id) & 1u) {
                     const int a = slot_of(mask, id);
-                    const double fi = st[a], fj = st[8 + a], fk = st[16 + a], fl = st[24 + a];
-                    if (id == 0) { Pi[0] = fi + cP; Pj[0] = fj + cP; Qk[0] = fk + cQ; Ql[0] = fl + cQ; }
-                    else { Pi[id] = fma(sPq, fi, cP); Pj[id] = fma(sPq, fj, cP); Qk[id] = fma(sQq, fk, cQ); Ql[id] = fma(sQq, fl, cQ); }
+                    Pi[id] = sin_[a]; Pj[id] = sin_[8 + a];
+                    const double fk = sout[a], fl = sout[8 + a];
+                    Qk[id] = id == 0 ? 1.0 + fk : 1.0 - fk; Ql[id] = id == 0 ? 1.0 + fl : 1.0 - fl;
                 } else {
                     Pi[id] = Pj[id] = Qk[id] = Ql[id] = 0.0;
                 }
             }
         }
         const double u = __dsub_rn(-s, t);
-        const double g4ws = loss ? -g4w : g4w;                            // the loss half carries the minus sign of the bracket
-        MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4ws);
+        MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
         // user-defined matrix elements (bz_set_msq_override) run on the runtime-mask instantiation, so that the
         // specialised mixture kernels carry no extra registers for them
-        if constexpr (kMask < 0) { if (P.has_ovr) msq_apply_override(M, P.msq_ovr, g4ws); }
+        if constexpr (kMask < 0) { if (P.has_ovr) msq_apply_override(M, P.msq_ovr, g4w); }
         deposit_half<kMask>(mask, Pi, Pj, Qk, Ql, M, d[0], d[1], d[2], d[3]);
     }
     __syncwarp();                                        // both lanes of every pair have read the gathered f
     if (work) {
-        double* out = st + (loss ? W::kLoss : 0);
+        // d[0], d[1] belong to the lane's incoming cells, d[2], d[3] to its outgoing ones: back in the order i, j, k, l
+        double* oin = st + (lane >> 4) * W::kLoss + rev;
+        double* oout = st + (lane >> 4) * W::kLoss + (16 - rev);
         if constexpr (kMask >= 0) {
             constexpr unsigned km = (unsigned)kMask;
             constexpr int kS = slot_of(km, 7), kPairs = (kS + 1) / 2;
@@ -195,45 +200,46 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
 #pragma unroll
                 for (int id = 0; id < 7; ++id)
                     if ((kMask >> id) & 1) o[slot_of(km, id)] = d[c][id];
+                double* dst = (c < 2 ? oin : oout) + (c & 1) * 8;
 #pragma unroll
                 for (int q = 0; q < kPairs; ++q)
-                    *reinterpret_cast<double2*>(out + c * 8 + 2 * q) = make_double2(o[2 * q], o[2 * q + 1]);
+                    *reinterpret_cast<double2*>(dst + 2 * q) = make_double2(o[2 * q], o[2 * q + 1]);
             }
         } else {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
+                double* dst = (c < 2 ? oin : oout) + (c & 1) * 8;
 #pragma unroll
-                for (int a = 0; a < 8; ++a) out[c * 8 + a] = 0.0;
+                for (int a = 0; a < 8; ++a) dst[a] = 0.0;
 #pragma unroll
                 for (int id = 0; id < 7; ++id)
-                    if ((mask >> id) & 1u) out[c * 8 + slot_of(mask, id)] = d[c][id];
+                    if ((mask >> id) & 1u) dst[slot_of(mask, id)] = d[c][id];
             }
         }
     }
     __syncwarp();
     // scatter: one sample per instruction, lane = (cell cc, slot sl) of the sample, 8 lanes per 64-byte cell; the cell
-    // indices and the sums of the two halves are collected first, eight samples at a time, then the reductions go out
+    // indices (four 16-byte loads: a batch never wraps around the ring) and the sums of the two halves are collected
+    // first, then the reductions go out
     {
         const int cc = lane >> 3, sl = lane & 7;
         if (sl < P.S) {
             double* __restrict__ gdst = P.dN_aos + sl;
             const double* src = wm.stage + lane;
+            const unsigned* cp = &wm.cell[cc][head];
             if (nb == W::kBatch) {
 #pragma unroll
                 for (int q0 = 0; q0 < W::kBatch; q0 += 8) {
-                    unsigned ci[8];
+                    const uint4 c0 = *reinterpret_cast<const uint4*>(cp + q0), c1 = *reinterpret_cast<const uint4*>(cp + q0 + 4);
+                    const unsigned ci[8] = { c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w };
                     double v[8];
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) {
-                        ci[q] = wm.cell[(head + q0 + q) & (kRing - 1)][cc];
-                        v[q] = src[(q0 + q) * W::kStride] + src[(q0 + q) * W::kStride + W::kLoss];
-                    }
+                    for (int q = 0; q < 8; ++q) v[q] = src[(q0 + q) * W::kStride] + src[(q0 + q) * W::kStride + W::kLoss];
 #pragma unroll
                     for (int q = 0; q < 8; ++q) red_add(gdst + (size_t)ci[q] * 8, v[q]);
                 }
             } else {
-                for (int q = 0; q < nb; ++q)
-                    red_add(gdst + (size_t)wm.cell[(head + q) & (kRing - 1)][cc] * 8, src[q * W::kStride] + src[q * W::kStride + W::kLoss]);
+                for (int q = 0; q < nb; ++q) red_add(gdst + (size_t)cp[q] * 8, src[q * W::kStride] + src[q * W::kStride + W::kLoss]);
             }
         }
     }
@@ -244,8 +250,8 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
 __device__ __forceinline__ void consume_batch_glue(WarpMem<1>& wm, const CollideParams& P, int lane, int head, int nb, double m2)
 {
     if (lane < nb) {
-        const int r = (head + lane) & (kRing - 1);
-        const uint4 cl = *reinterpret_cast<const uint4*>(&wm.cell[r][0]);
+        const int r = head + lane;
+        const uint4 cl = make_uint4(wm.cell[0][r], wm.cell[1][r], wm.cell[2][r], wm.cell[3][r]);
         const double s = wm.s[r], t = wm.t[r];
         const double g4w = P.g4K * rcp_fast(wm.e12[r]);
         const double fi = __ldg(P.f_aos + cl.x), fj = __ldg(P.f_aos + cl.y), fk = __ldg(P.f_aos + cl.z), fl = __ldg(P.f_aos + cl.w);
@@ -290,7 +296,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         bool fresh = i < i_end;
         if (!fresh && !exhausted) {
             if (next_item == 0xffffffffu) {
-                next_item = __shfl_sync(0xffffffffu, pref_item, 0);
+                next_item = __reduce_max_sync(0xffffffffu, lane == 0 ? pref_item : 0u);   // REDUX: the result is provably warp-uniform
                 if (next_item >= P.n_items) { exhausted = true; next_item = 0xffffffffu; }
             }
             if (next_item != 0xffffffffu) {
@@ -355,7 +361,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             if (sa.flag) {
                 const int r = (head + count + __popc(acc & lt)) & (kRing - 1);
                 const unsigned xb = (unsigned)xcell * (unsigned)P.Np;
-                *reinterpret_cast<uint4*>(&wm.cell[r][0]) = make_uint4(xb + (unsigned)ci, xb + (unsigned)sa.j, xb + (unsigned)sa.k, xb + (unsigned)sa.l);
+                wm.cell[0][r] = xb + (unsigned)ci; wm.cell[1][r] = xb + (unsigned)sa.j; wm.cell[2][r] = xb + (unsigned)sa.k; wm.cell[3][r] = xb + (unsigned)sa.l;
                 wm.s[r] = sa.s; wm.t[r] = sa.t; wm.e12[r] = sa.E1E2;
             }
             const int na = __popc(acc);
@@ -367,8 +373,8 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         if (nb > 0) {
             if constexpr (kSP == 1) consume_batch_glue(wm, P, lane, head, nb, wm.m2x);
             else consume_batch<kMask, kSP>(wm, P, lane, mask, head, nb, wm.m2x);
-            head = (head + nb) & (kRing - 1);
             count -= nb;
+            head = count == 0 ? 0 : (head + nb) & (kRing - 1);   // only the last batch before a drain is partial: head stays a multiple of kBatch
             nb = 0;
         } else if (!can_sample && exhausted && count == 0) {
             break;

@@ -37,6 +37,20 @@ __device__ __forceinline__ double uniform52(uint32_t a, uint32_t b)
     const double d = __hiloint2double((int)(0x43300000u | (a >> 12)), (int)(((a >> 6) << 26) | (b >> 6)));
     return __dmul_rn(__dadd_rn(d, -4503599627370495.5), 2.220446049250313e-16);
 }
+// The same uniform times 2^52, i.e. m + 1/2 (exact): a product u * c equals fl((m + 1/2) * (c 2^-52)) bit for bit, because
+// scaling by 2^-52 is exact on either side of the single rounding.
+__device__ __forceinline__ double uniform52_scaled(uint32_t a, uint32_t b)
+{
+    const double d = __hiloint2double((int)(0x43300000u | (a >> 12)), (int)(((a >> 6) << 26) | (b >> 6)));
+    return __dadd_rn(d, -4503599627370495.5);
+}
+// v = 2 U - 1 = (m + 1/2) 2^-51 - 1 = (2 m + 1 - 2^52) 2^-52: an odd multiple of 2^-52 below 1 in magnitude, exactly
+// representable, so S8c's two rounded steps "2 * u" and "- 1" are both exact and this single fused one gives the same bits
+__device__ __forceinline__ double symmetric52(uint32_t a, uint32_t b)
+{
+    const double d = __hiloint2double((int)(0x43300000u | (a >> 12)), (int)(((a >> 6) << 26) | (b >> 6)));
+    return fma(__dadd_rn(d, -4503599627370495.5), 4.440892098500626e-16, -1.0);
+}
 
 // ---- S8c step 3: cell index along one axis.  q = (p - pmin)/dp, inside iff 0 <= q < n, idx = floor(q).
 // Exact form (the definition): one correctly rounded subtraction and division.
@@ -106,21 +120,22 @@ __device__ __forceinline__ Sample gen_sample_pair(const GridConst& g, uint32_t s
     philox4x32_10(1u, smp, pcell, xcell, seed, step, w1);
     philox4x32_10(2u + kstart, smp, pcell, xcell, seed, step, wa);
     philox4x32_10(3u + kstart, smp, pcell, xcell, seed, step, wb);
-    const double u0 = uniform52(w0[0], w0[1]), u1 = uniform52(w0[2], w0[3]), u2 = uniform52(w1[0], w1[1]);
-    const double p2x = __dadd_rn(g.pmin, __dmul_rn(u0, g.L));
-    const double p2y = __dadd_rn(g.pmin, __dmul_rn(u1, g.L));
-    const double p2z = __dadd_rn(g.pmin, __dmul_rn(u2, g.L));
+    const double L52 = g.L * 2.220446049250313e-16;       // L 2^-52, exact
+    const double p2x = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[0], w0[1]), L52));
+    const double p2y = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[2], w0[3]), L52));
+    const double p2z = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w1[0], w1[1]), L52));
     const double E2 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(p2x, p2x), __dmul_rn(p2y, p2y)), __dmul_rn(p2z, p2z)));
     const double d12 = __dadd_rn(__dadd_rn(__dmul_rn(p1x, p2x), __dmul_rn(p1y, p2y)), __dmul_rn(p1z, p2z));
-    const double s = __dmul_rn(2.0, __dsub_rn(__dmul_rn(E1, E2), d12));
-    o.E1E2 = E1 * E2;
+    const double e12 = __dmul_rn(E1, E2);
+    const double s = __dmul_rn(2.0, __dsub_rn(e12, d12));
+    o.E1E2 = e12;
 
     // Marsaglia: attempt k is accepted iff q_k = v1^2 + v2^2 < 1; after 62 failures the direction is (0, 0, 1)
-    double v1 = __dadd_rn(__dmul_rn(2.0, uniform52(wa[0], wa[1])), -1.0);
-    double v2 = __dadd_rn(__dmul_rn(2.0, uniform52(wa[2], wa[3])), -1.0);
+    double v1 = symmetric52(wa[0], wa[1]);
+    double v2 = symmetric52(wa[2], wa[3]);
     double q = __dadd_rn(__dmul_rn(v1, v1), __dmul_rn(v2, v2));
-    const double v1b = __dadd_rn(__dmul_rn(2.0, uniform52(wb[0], wb[1])), -1.0);
-    const double v2b = __dadd_rn(__dmul_rn(2.0, uniform52(wb[2], wb[3])), -1.0);
+    const double v1b = symmetric52(wb[0], wb[1]);
+    const double v2b = symmetric52(wb[2], wb[3]);
     const double qb = __dadd_rn(__dmul_rn(v1b, v1b), __dmul_rn(v2b, v2b));
     bool found = q < 1.0;
     if (!found) { v1 = v1b; v2 = v2b; q = qb; found = qb < 1.0; }

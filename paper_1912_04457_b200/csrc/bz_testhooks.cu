@@ -26,21 +26,23 @@ extern "C" int bz_debug_deposit_host(const int* species, int n_species, double a
             for (int id = 0; id < 7; ++id) out[sl * 7 + id] = d[sl][id];
         return 0;
     }
-    // the collision kernel's form: gain half (P = f, Q = F, +M) and loss half (P = F, Q = f, -M) evaluated separately and
-    // added, with the factors built as the kernel builds them (c + sigma f; inactive species 0 on both sides)
+    // the collision kernel's form: the gain half on the cells (i, j | k, l) and, for the loss half, the gain half of the
+    // time-reversed channels on (k, l | i, j), evaluated separately and added (P = f at the incoming cells, Q = 1 +- f at
+    // the outgoing ones; inactive species 0 on both sides)
     double h[2][4][7];
     for (int half = 0; half < 2; ++half) {
-        double P[2][7], Q[2][7];
+        double P[2][7], Q[2][7], dd[4][7];
+        const int in0 = half == 0 ? 0 : 2, out0 = half == 0 ? 2 : 0;
         for (int id = 0; id < 7; ++id) {
             const bool on = (mask >> id) & 1u;
-            const double sg = id == 0 ? 1.0 : -1.0;              // F = 1 + f (gluon), 1 - f (quark)
             for (int c = 0; c < 2; ++c) {
-                P[c][id] = !on ? 0.0 : (half == 0 ? fma(1.0, f[c][id], 0.0) : fma(sg, f[c][id], 1.0));
-                Q[c][id] = !on ? 0.0 : (half == 0 ? fma(sg, f[2 + c][id], 1.0) : fma(1.0, f[2 + c][id], 0.0));
+                P[c][id] = on ? f[in0 + c][id] : 0.0;
+                Q[c][id] = !on ? 0.0 : (id == 0 ? 1.0 + f[out0 + c][id] : 1.0 - f[out0 + c][id]);     // F = 1 + f (gluon), 1 - f (quark)
             }
         }
-        const MsqSet Ms = half == 0 ? M : msq_negated(M);
-        deposit_half<-1>(mask, P[0], P[1], Q[0], Q[1], Ms, h[half][0], h[half][1], h[half][2], h[half][3]);
+        deposit_half<-1>(mask, P[0], P[1], Q[0], Q[1], M, dd[0], dd[1], dd[2], dd[3]);
+        for (int c = 0; c < 2; ++c)
+            for (int id = 0; id < 7; ++id) { h[half][in0 + c][id] = dd[c][id]; h[half][out0 + c][id] = dd[2 + c][id]; }
     }
     for (int sl = 0; sl < 4; ++sl)
         for (int id = 0; id < 7; ++id) out[sl * 7 + id] = h[0][sl][id] + h[1][sl][id];
