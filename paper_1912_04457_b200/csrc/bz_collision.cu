@@ -30,7 +30,10 @@ namespace bz {
 
 namespace {
 
-constexpr int kWarps = 16;
+#ifndef BZ_WARPS
+#define BZ_WARPS 16
+#endif
+constexpr int kWarps = BZ_WARPS;
 constexpr int kCollideThreads = 32 * kWarps;
 constexpr int kRing = 64;                        // records per warp (a sampling pass adds at most 32)
 constexpr int kRetryCap = 64;                    // per warp: samples whose two Marsaglia attempts both failed
