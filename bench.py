@@ -180,24 +180,31 @@ def paper_probe(g, cfg, dev, fp64_peak, reps=2):
             "frac": rate * flop / 1e12 / fp64_peak if fp64_peak else None}
 
 
-def is_probe(g, cfg, dev, reps=2):
-    """NEXT rank 3, outside the timed step: the importance-sampled estimator (bz_collision_is) on the whole
-    bench workload; same gathered/scattered bytes per sample as the hot path's kernel, so the same HBM-gather leg."""
+def weighted_probe(g, cfg, dev, which, reps=2):
+    """NEXT rank 3, outside the timed step: the weighted estimators on the whole bench workload --
+    "is": importance-sampled t (bz_collision_is), "box": in-box CM direction (bz_collision_box).  Both run in
+    collide_kernel with another sampler; the HBM leg is acceptance-weighted like the hot path's."""
     import torch
+    fn = g.collision_is if which == "is" else g.collision_box
     out = torch.empty(g.shape, dtype=torch.float64, device=dev)
-    g.collision_is(cfg.dt, 0, out)
+    fn(cfg.dt, 0, out)
     torch.cuda.synchronize()
+    g.sample_counts(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for r in range(reps):
-        g.collision_is(cfg.dt, 1 + r, out)
+        fn(cfg.dt, 1 + r, out)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / reps
+    gen, acc = g.sample_counts(reset=True)
     rate = cfg.samples_per_step / (ms * 1e-3)
-    bps = bytes_literal_8d(cfg)
-    return {"kernel": "is_kernel (bz_collision_is)", "bound": "hbm", "ms": ms, "samples_per_sec": rate, "bytes_per_sample": bps,
-            "bytes_note": "SURVEY.md 8d's literal count (every sample credited)", "achieved": rate * bps / 1e9, "unit": "GB/s"}
+    acceptance = acc / gen if gen else None
+    bps = bytes_acceptance_weighted(cfg, acceptance or 0.0)
+    return {"kernel": "collide_kernel<mask, sampler %d> + finalize_kernel (bz_collision_%s)" % (1 if which == "is" else 2, which), "bound": "hbm",
+            "ms": ms, "samples_per_sec": rate, "acceptance": acceptance, "accepted_samples_per_sec": rate * (acceptance or 0.0),
+            "bytes_per_sample": bps, "achieved": rate * bps / 1e9, "unit": "GB/s",
+            "bytes_per_sample_survey_8d_literal": bytes_literal_8d(cfg)}
 
 
 def measured_peaks():
@@ -415,7 +422,8 @@ def run_ours(args, cfg):
     fp64_peak = bz.measure_fp64_peak() if rank == 0 else 0.0
     rank2 = vlasov_probe(g, cfg, dev) if (rank == 0 and cfg.Nx > 1 and not slabs and not args.no_probes) else None
     rank1 = paper_probe(g, cfg, dev, fp64_peak) if (rank == 0 and not slabs and not args.no_probes) else None
-    rank3 = is_probe(g, cfg, dev) if (rank == 0 and not slabs and not args.no_probes) else None
+    rank3 = weighted_probe(g, cfg, dev, "is") if (rank == 0 and not slabs and not args.no_probes) else None
+    rank3b = weighted_probe(g, cfg, dev, "box") if (rank == 0 and not slabs and not args.no_probes) else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
     # ---- end to end: host f in, host f and moments out, every step
@@ -499,6 +507,7 @@ def run_ours(args, cfg):
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),
         "next_rank1_paper_sampler": rank1,
         "next_rank3_importance_sampling": None if rank3 is None else dict(rank3, peak=peak, frac=rank3["achieved"] / peak),
+        "next_rank3_inbox_sampling": None if rank3b is None else dict(rank3b, peak=peak, frac=rank3b["achieved"] / peak),
         "next_rank2_eq15": None if rank2 is None else dict(rank2, peak=peak, frac=rank2["achieved"] / peak),
         "clocks": clocks,
         "total_particle_number": N1,

@@ -21,7 +21,7 @@ class Grid(C.Structure):
 
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
-           "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
+           "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_collision_box", "bz_debug_samples_box", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_get_sample_counts",
            "bz_debug_samples")
@@ -54,6 +54,8 @@ def lib():
         L.bz_energy_diag.argtypes = [vp, vp]
         L.bz_collision_is.argtypes = [vp, C.c_double, C.c_uint, vp]
         L.bz_debug_samples_is.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, C.c_double, vp, vp, vp]
+        L.bz_collision_box.argtypes = [vp, C.c_double, C.c_uint, vp]
+        L.bz_debug_samples_box.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp, vp]
         L.bz_debug_paper_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, dp, vp, vp]
         L.bz_debug_paper_channels.argtypes = [ip, C.c_int, ip, C.c_int]
         L.bz_copy_layers.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int]
@@ -252,6 +254,22 @@ class Boltzmann:
         w = torch.empty((n, self.Ns), dtype=torch.float64, device=self.device)
         self._chk(lib().bz_debug_samples_is(self._h, step, xcell, pbegin, pend, m2, C.c_void_p(cells.data_ptr()),
                                             C.c_void_p(stu.data_ptr()), C.c_void_p(w.data_ptr())), "bz_debug_samples_is")
+        return cells, stu, w
+
+    # ---- NEXT rank 3, other half: in-box sampling of the CM direction
+    def collision_box(self, dt, step, out=None):
+        if out is None:
+            out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_collision_box(self._h, dt, step, self._dev_ptr(out, self.n_values)), "bz_collision_box")
+        return out
+
+    def debug_samples_box(self, step, xcell, pbegin, pend):
+        n = pend - pbegin
+        cells = torch.empty((n, self.Ns, 4), dtype=torch.int32, device=self.device)
+        stu = torch.empty((n, self.Ns, 3), dtype=torch.float64, device=self.device)
+        w = torch.empty((n, self.Ns), dtype=torch.float64, device=self.device)
+        self._chk(lib().bz_debug_samples_box(self._h, step, xcell, pbegin, pend, C.c_void_p(cells.data_ptr()),
+                                             C.c_void_p(stu.data_ptr()), C.c_void_p(w.data_ptr())), "bz_debug_samples_box")
         return cells, stu, w
 
     def set_collision(self, mode):

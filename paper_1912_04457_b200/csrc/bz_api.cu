@@ -94,6 +94,7 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.g4K = (g2 * g2) * K;
     P.mask = c->mask;
     for (int a = 0; a < 7; ++a) P.slot[a] = c->slot[a];
+    P.sampler = 0;
     P.has_ovr = 0;
     for (int k = 0; k < 7; ++k) {
         P.msq_ovr[k] = c->msq_ovr[k] >= 0.0 ? c->msq_ovr[k] / (g2 * g2) : -1.0;
@@ -113,14 +114,16 @@ int prof_mark(bz_ctx* c, int group)
     return 0;
 }
 
-int run_collide(bz_ctx* c, double dt_fm, unsigned step)
+// sampler: 0 the hot path's isotropic CM direction, 1 importance-sampled t, 2 in-box direction (collide_kernel's template)
+int run_collide(bz_ctx* c, double dt_fm, unsigned step, int sampler = 0)
 {
     if (int rc = prof_mark(c, 0)) return rc;
     if (c->SP != 1 && !c->aos_valid) {
         BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
         c->aos_valid = true;
     }
-    const CollideParams P = collide_params(c, dt_fm, step);
+    CollideParams P = collide_params(c, dt_fm, step);
+    P.sampler = sampler;
     BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
     c->generated += (unsigned long long)(P.n_items / (unsigned)P.regions_per_x) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
     return prof_mark(c, 0);
@@ -451,7 +454,7 @@ int bz_vlasov(bz_ctx* c, double dt_fm, double* dF_dev)
     return run_vlasov(c, dt_fm, dF_dev);
 }
 
-int bz_set_collision(bz_ctx* c, int mode) { if (!c || mode < 0 || mode > 2) return -1; c->coll_mode = mode; return 0; }
+int bz_set_collision(bz_ctx* c, int mode) { if (!c || mode < 0 || mode > 3) return -1; c->coll_mode = mode; return 0; }
 
 // bz_step with the paper's own collision term (rank 1): masses (scheme 1), bz_collision_paper into a scratch, the
 // transport increment of the chosen scheme into f_new, then f_new = (f + dF_transport) + dF_coll
@@ -459,8 +462,7 @@ static int step_paper(bz_ctx* c, double dt_fm)
 {
     if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f, used by both terms
     if (!c->dF_scratch) BZ_CUDA(cudaMalloc(&c->dF_scratch, c->n_values * sizeof(double)), "cudaMalloc dF scratch");
-    if (c->coll_mode == 1) { if (int rc = bz_collision_paper(c, dt_fm, c->step, c->dF_scratch)) return rc; }
-    else if (int rc = bz_collision_is(c, dt_fm, c->step, c->dF_scratch)) return rc;
+    if (int rc = bz_collision_paper(c, dt_fm, c->step, c->dF_scratch)) return rc;
     if (c->scheme == 0) BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 0, c->stream), "stream");
     else if (int rc = run_vlasov(c, dt_fm, c->f_new)) return rc;
     BZ_CUDA(launch_combine(c->f, c->f_new, c->dF_scratch, c->n_values, c->stream), "combine");
@@ -475,9 +477,9 @@ int bz_step(bz_ctx* c, double dt_fm)
     if (!c) return -1;
     if (!c->f) return -4;
     BZ_ON_DEVICE(c);
-    if (c->coll_mode != 0) return step_paper(c, dt_fm);
+    if (c->coll_mode == 1) return step_paper(c, dt_fm);
     if (int rc = update_m2(c)) return rc;
-    if (int rc = run_collide(c, dt_fm, c->step)) return rc;
+    if (int rc = run_collide(c, dt_fm, c->step, c->coll_mode == 0 ? 0 : c->coll_mode - 1)) return rc;   // modes 2, 3: the weighted samplers
     if (c->scheme == 1) { if (int rc = run_thermal_masses(c)) return rc; }     // masses from the old f
     if (int rc = prof_mark(c, 1)) return rc;
     if (c->scheme == 0) BZ_CUDA(launch_transport(transport_params(c, dt_fm, c->f_new), 1, c->stream), "stream+euler");
@@ -665,34 +667,25 @@ int bz_debug_paper_channels(const int* species, int n_species, int* out_host, in
     return (int)table.size();
 }
 
-/* ---- NEXT rank 3: importance-sampled estimator (bz_is.cu) ---- */
-static int is_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
-{
-    if (int rc = paper_params(c, dt_fm, step, P)) return rc;
-    const double L = P.g.L, Vp = (L * L) * L, dtG = dt_fm / kHbarc;
-    P.Kp = dtG * Vp / (2048.0 * (kPi * kPi * kPi * kPi) * c->Ns);      // the hot path's K (S8c step 0)
-    return 0;
-}
-
-int bz_collision_is(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
+/* ---- NEXT rank 3: the weighted samplers (importance-sampled t, in-box direction) run in collide_kernel ---- */
+static int collision_weighted(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev, int sampler)
 {
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
     BZ_ON_DEVICE(c);
     if (int rc = update_m2(c)) return rc;
-    PaperParams P;
-    if (int rc = is_params(c, dt_fm, step, P)) return rc;
-    P.dN = dF_dev;
-    BZ_CUDA(cudaMemsetAsync(dF_dev, 0, c->n_values * sizeof(double), c->stream), "memset dF");
-    BZ_CUDA(launch_is_collide(P, c->m2, c->sms, c->stream), "is collide");
+    if (int rc = run_collide(c, dt_fm, step, sampler)) return rc;
     double deg[7];
     fill_deg(c, deg);
-    BZ_CUDA(launch_paper_finalize(dF_dev, c->n_values, c->S, c->Np, deg, c->stream), "is finalize");
+    BZ_CUDA(launch_finalize(c->dN_aos, dF_dev, c->Nx, c->S, c->SP, c->Np, deg, c->stream), "finalize");
     return 0;
 }
 
-int bz_debug_samples_is(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, double m2, int* cells_dev,
-                        double* stu_dev, double* w_dev)
+int bz_collision_is(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev) { return collision_weighted(c, dt_fm, step, dF_dev, 1); }
+int bz_collision_box(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev) { return collision_weighted(c, dt_fm, step, dF_dev, 2); }
+
+static int debug_weighted(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int sampler, double m2, int* cells_dev,
+                          double* stu_dev, double* w_dev)
 {
     if (!c || !cells_dev || !stu_dev || !w_dev || xcell < 0 || xcell >= c->Nx || pcell_begin < 0 || pcell_end > c->Np ||
         pcell_begin > pcell_end)
@@ -700,10 +693,22 @@ int bz_debug_samples_is(bz_ctx* c, unsigned step, int xcell, int pcell_begin, in
     if (!c->f) return -4;
     BZ_ON_DEVICE(c);
     PaperParams P;
-    if (int rc = is_params(c, 1.0, step, P)) return rc;
+    if (int rc = paper_params(c, 1.0, step, P)) return rc;
     P.x_begin = xcell; P.x_count = 1; P.p_begin = pcell_begin; P.p_count = pcell_end - pcell_begin;
-    BZ_CUDA(launch_is_debug(P, m2, cells_dev, stu_dev, w_dev, c->sms, c->stream), "is debug");
+    BZ_CUDA(launch_weighted_debug(P, sampler, m2, cells_dev, stu_dev, w_dev, c->sms, c->stream), "weighted sampler debug");
     return 0;
+}
+
+int bz_debug_samples_is(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, double m2, int* cells_dev,
+                        double* stu_dev, double* w_dev)
+{
+    return debug_weighted(c, step, xcell, pcell_begin, pcell_end, 1, m2, cells_dev, stu_dev, w_dev);
+}
+
+int bz_debug_samples_box(bz_ctx* c, unsigned step, int xcell, int pcell_begin, int pcell_end, int* cells_dev, double* stu_dev,
+                         double* w_dev)
+{
+    return debug_weighted(c, step, xcell, pcell_begin, pcell_end, 2, 0.0, cells_dev, stu_dev, w_dev);
 }
 
 int bz_moments(bz_ctx* c, double* out_host)

@@ -85,6 +85,7 @@ struct alignas(16) WarpMem {
     unsigned cell[4][kRing + 4];                         // [slot i, j, k, l][record]: indices into the whole grid, xcell * Np + pcell
                                                          // (rows 272 bytes apart: the four slots' 16-byte reads hit different banks)
     double s[kRing], t[kRing], e12[kRing];               // Mandelstam s, t and E1 E2 of the sample
+    double w[kRing];                                     // weight of the sample (weighted samplers only)
     double m2x;                                          // regulator mass^2 of the current spatial cell
     int2 retry[kRetryCap];
 };
@@ -121,7 +122,7 @@ __device__ __forceinline__ void issue_gather(WarpMem<kSP>& wm, const double* __r
 }
 
 // ---- algebra + scatter of records [head, head + nb), kSP == 8: two lanes per sample
-template <int kMask, int kSP>
+template <int kMask, int kSP, int kSampler>
 __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollideParams& P, int lane, unsigned mask, int head, int nb,
                                               double m2)
 {
@@ -144,7 +145,8 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
     if (work) {
         const int r = head + m;
         const double s = wm.s[r], t = wm.t[r];
-        const double g4w = P.g4K * rcp_fast(wm.e12[r]);                   // g^4 K / (E1 E2), S8c step 6
+        double g4w = P.g4K * rcp_fast(wm.e12[r]);                         // g^4 K / (E1 E2), S8c step 6
+        if constexpr (kSampler != 0) g4w *= wm.w[r];                      // x the sampler's weight
         // gain factors: P = f at the incoming cells, Q = F = 1 + f (gluon), 1 - f (quark) at the outgoing ones
         double Pi[7], Pj[7], Qk[7], Ql[7];
         if constexpr (kMask >= 0) {
@@ -250,13 +252,15 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
 }
 
 // ---- pure glue: lane = sample, plain loads, the whole bracket in one lane, four reductions from the registers
+template <int kSampler>
 __device__ __forceinline__ void consume_batch_glue(WarpMem<1>& wm, const CollideParams& P, int lane, int head, int nb, double m2)
 {
     if (lane < nb) {
         const int r = head + lane;
         const uint4 cl = make_uint4(wm.cell[0][r], wm.cell[1][r], wm.cell[2][r], wm.cell[3][r]);
         const double s = wm.s[r], t = wm.t[r];
-        const double g4w = P.g4K * rcp_fast(wm.e12[r]);
+        double g4w = P.g4K * rcp_fast(wm.e12[r]);
+        if constexpr (kSampler != 0) g4w *= wm.w[r];
         const double fi = __ldg(P.f_aos + cl.x), fj = __ldg(P.f_aos + cl.y), fk = __ldg(P.f_aos + cl.z), fl = __ldg(P.f_aos + cl.w);
         const double u = __dsub_rn(-s, t);
         MsqSet M = msq_set<true, false>(s, t, u, m2, g4w);
@@ -270,7 +274,8 @@ __device__ __forceinline__ void consume_batch_glue(WarpMem<1>& wm, const Collide
 }
 
 // ------------------------------------------------------------------------------------------------ the kernel
-template <int kMask>
+// kSampler: 0 = isotropic CM direction (the hot path, NS), 1 = importance-sampled t, 2 = in-box direction (bz_sample.cuh)
+template <int kMask, int kSampler>
 __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const CollideParams P)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
@@ -351,8 +356,12 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             }
             Sample sa;
             sa.flag = 0; sa.retry = 0;
-            if (active)
-                sa = gen_sample_pair(P.g, P.seed, step, (uint32_t)xcell + P.x_rng_offset, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+            if (active) {
+                const uint32_t xr = (uint32_t)xcell + P.x_rng_offset;
+                if constexpr (kSampler == 0) sa = gen_sample_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+                else if constexpr (kSampler == 1) sa = gen_sample_is_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1, wm.m2x);
+                else sa = gen_sample_box_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+            }
             const unsigned lt = (1u << lane) - 1u;
             const unsigned rb = __ballot_sync(0xffffffffu, sa.retry);
             if (rb) {
@@ -366,6 +375,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 const unsigned xb = (unsigned)xcell * (unsigned)P.Np;
                 wm.cell[0][r] = xb + (unsigned)ci; wm.cell[1][r] = xb + (unsigned)sa.j; wm.cell[2][r] = xb + (unsigned)sa.k; wm.cell[3][r] = xb + (unsigned)sa.l;
                 wm.s[r] = sa.s; wm.t[r] = sa.t; wm.e12[r] = sa.E1E2;
+                if constexpr (kSampler != 0) wm.w[r] = sa.w;
             }
             const int na = __popc(acc);
             count += na;
@@ -374,8 +384,8 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
         }
         // ---- D: the batch in flight: algebra and scatter
         if (nb > 0) {
-            if constexpr (kSP == 1) consume_batch_glue(wm, P, lane, head, nb, wm.m2x);
-            else consume_batch<kMask, kSP>(wm, P, lane, mask, head, nb, wm.m2x);
+            if constexpr (kSP == 1) consume_batch_glue<kSampler>(wm, P, lane, head, nb, wm.m2x);
+            else consume_batch<kMask, kSP, kSampler>(wm, P, lane, mask, head, nb, wm.m2x);
             count -= nb;
             head = count == 0 ? 0 : (head + nb) & (kRing - 1);   // only the last batch before a drain is partial: head stays a multiple of kBatch
             nb = 0;
@@ -449,7 +459,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(double* __restrict__ dN_a
     }
 }
 
-template <int kMask>
+template <int kMask, int kSampler>
 cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t st)
 {
     constexpr int kSP = MaskTraits<kMask>::SP;
@@ -460,13 +470,22 @@ cudaError_t launch_collide_mask(const CollideParams& P, int ctas, cudaStream_t s
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= kMaxDevices || !configured[dev]) {
-        e = cudaFuncSetAttribute(collide_kernel<kMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        e = cudaFuncSetAttribute(collide_kernel<kMask, kSampler>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < kMaxDevices) configured[dev] = true;
     }
-    collide_kernel<kMask><<<ctas, kCollideThreads, smem, st>>>(P);
+    collide_kernel<kMask, kSampler><<<ctas, kCollideThreads, smem, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
+}
+
+// the weighted samplers (NEXT rank 3) are instantiated for the pure-glue mask, the full mixture and the run-time mask
+template <int kSampler>
+cudaError_t launch_collide_weighted(const CollideParams& P, int ctas, cudaStream_t st)
+{
+    if (P.mask == 0x01u) return launch_collide_mask<0x01, kSampler>(P, ctas, st);
+    if (P.mask == 0x7Fu && !P.has_ovr) return launch_collide_mask<0x7F, kSampler>(P, ctas, st);
+    return launch_collide_mask<-1, kSampler>(P, ctas, st);
 }
 
 }  // namespace
@@ -487,12 +506,14 @@ cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st)
     int ctas = (int)((P.n_items + kWarps - 1) / kWarps);
     if (ctas > sms) ctas = sms;
     if (ctas < 1) ctas = 1;
-    if (P.has_ovr && P.mask != 0x01u) return launch_collide_mask<-1>(P, ctas, st);
+    if (P.sampler == 1) return launch_collide_weighted<1>(P, ctas, st);
+    if (P.sampler == 2) return launch_collide_weighted<2>(P, ctas, st);
+    if (P.has_ovr && P.mask != 0x01u) return launch_collide_mask<-1, 0>(P, ctas, st);
     switch (P.mask) {
-    case 0x01u: return launch_collide_mask<0x01>(P, ctas, st);
-    case 0x7Eu: return launch_collide_mask<0x7E>(P, ctas, st);
-    case 0x7Fu: return launch_collide_mask<0x7F>(P, ctas, st);
-    default:    return launch_collide_mask<-1>(P, ctas, st);
+    case 0x01u: return launch_collide_mask<0x01, 0>(P, ctas, st);
+    case 0x7Eu: return launch_collide_mask<0x7E, 0>(P, ctas, st);
+    case 0x7Fu: return launch_collide_mask<0x7F, 0>(P, ctas, st);
+    default:    return launch_collide_mask<-1, 0>(P, ctas, st);
     }
 }
 

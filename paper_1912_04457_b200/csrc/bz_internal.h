@@ -37,6 +37,7 @@ struct CollideParams {
     int slot[7];          // species id -> index a in the layout (or -1)
     int has_ovr;          // bz_set_msq_override: some kind of Table I is replaced by a constant
     double msq_ovr[7];    // per kind: value / g^4, or -1 (Table I)
+    int sampler;          // 0 isotropic CM direction (hot path), 1 importance-sampled t, 2 in-box direction (NEXT rank 3)
 };
 
 // NEXT rank 1 (bz_paper.cu): ordered channel a(k1) b(k2) -> c(k3) d(p), layout indices; groups share a mass-class tuple
@@ -92,7 +93,7 @@ struct bz_ctx_impl {
     PaperChannel* paper_table;       // device: channel table of the paper sampler (built at the first bz_collision_paper)
     PaperGroup* paper_groups;        // device
     int paper_n_groups, paper_n_channels;
-    int coll_mode;                   // bz_set_collision: 0 CM sampler (hot path), 1 the paper's sampler (bz_collision_paper)
+    int coll_mode;                   // bz_set_collision: 0 CM sampler (hot path), 1 the paper's sampler, 2 importance-sampled t, 3 in-box direction
     double* dF_scratch;              // device n_values, allocated at the first bz_step with coll_mode 1
     double* diag;                    // device [Nx][5], allocated at the first bz_energy_diag
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
@@ -155,9 +156,8 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
                           const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
                           double dx, double dp, unsigned cls_bits, cudaStream_t st);
 
-// NEXT rank 3 (bz_is.cu): P.Kp holds the hot path's K = dtG Vp / (2048 pi^4 Ns) there
-cudaError_t launch_is_collide(const PaperParams& P, const double* m2_cell, int sms, cudaStream_t st);
-cudaError_t launch_is_debug(const PaperParams& P, double m2, int* cells, double* stu, double* w, int sms, cudaStream_t st);
+// NEXT rank 3 (bz_is.cu): what the weighted samplers draw (sampler 1: importance-sampled t with regulator m2, 2: in-box)
+cudaError_t launch_weighted_debug(const PaperParams& P, int sampler, double m2, int* cells, double* stu, double* w, int sms, cudaStream_t st);
 // NEXT rank 1 (bz_paper.cu)
 void build_paper_channels(const int* species, int S, std::vector<PaperChannel>& table, std::vector<PaperGroup>& groups);
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st);

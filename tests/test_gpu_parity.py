@@ -726,3 +726,62 @@ def test_importance_sampler_dF_parity_and_conservation(cfg, m_D):
     assert np.abs(dF_o).max() > 0
     _assert_dF(dF_g, dF_o, gross, "importance sampler")
     _assert_conserved(cfg, dF_g, gross)
+
+
+# ------------------------------------------------------------ NEXT rank 3, other half: in-box sampling of the CM direction
+@pytest.mark.parametrize("cfg", [wl.scaled(wl.CONFIGS[2], np_=9, samples=40), wl.scaled(wl.CONFIGS[4], nx=2, np_=24, samples=33),
+                                 wl.scaled(wl.CONFIGS[0], np_=15, samples=64, pmin=-1.0, pmax=4.0)],
+                         ids=["mix9", "cfg4_grid", "off_centre_box"])
+def test_inbox_sampler_cells_bit_exact(cfg):
+    """Cells of p2, p3, p4, the flag, (s, t, u) and the weight beta of every in-box sample: bit-exact."""
+    o, g = _pair(cfg)
+    xcell = cfg.Nx - 1
+    pb, pe = (0, cfg.Np) if cfg.Np < 1000 else (cfg.Np // 2 - 12, cfg.Np // 2 + 48)
+    cells, stu, w = (t.cpu().numpy() for t in g.debug_samples_box(7, xcell, pb, pe))
+    n_acc = n_all = 0
+    for pc in range(pb, pe, 3):
+        for smp in range(cfg.samples):
+            sm, wt = o.sample_one_box(7, xcell, pc, smp)
+            row = cells[pc - pb, smp]
+            assert tuple(row) == (sm.j, sm.k, sm.l, sm.flag), (pc, smp)
+            assert np.array_equal(stu[pc - pb, smp].view(np.uint64), np.array([sm.s, sm.t, sm.u]).view(np.uint64))
+            assert np.array([w[pc - pb, smp]]).view(np.uint64)[0] == np.array([wt]).view(np.uint64)[0]
+            n_acc += sm.flag
+            n_all += 1
+    assert n_all > 600 and n_acc > 0.6 * n_all
+
+
+@pytest.mark.parametrize("cfg", [wl.scaled(wl.CONFIGS[0], np_=9, samples=40),
+                                 wl.scaled(wl.CONFIGS[2], np_=8, samples=33),
+                                 wl.scaled(wl.CONFIGS[3], nx=2, np_=7, samples=24),
+                                 wl.scaled(wl.CONFIGS[1], np_=8, samples=20)],
+                         ids=["glue", "mixture", "inhom", "quarks"])
+def test_inbox_sampler_dF_parity_and_conservation(cfg):
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=19)
+    o.set_f(f0)
+    g.set_f(f0)
+    dF_o = o.collision_box(cfg.dt, 3)
+    dF_g = g.collision_box(cfg.dt, 3).cpu().numpy()
+    gross = o.gross()
+    assert np.abs(dF_o).max() > 0
+    _assert_dF(dF_g, dF_o, gross, "in-box sampler")
+    _assert_conserved(cfg, dF_g, gross)
+    # the hot path right after it: the sampler is a per-call choice, nothing sticks to the context
+    _assert_dF(g.collision(cfg.dt, 3).cpu().numpy(), o.collision(cfg.dt, 3), o.gross(), "hot path after in-box")
+
+
+def test_step_with_the_inbox_collision_term():
+    """bz_set_collision(3): bz_step with the in-box estimator; f after 3 steps against the oracle."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=7, samples=12)
+    o, g = _pair(cfg)
+    f0 = wl.random_f(cfg, seed=47) * 0.5
+    for e in (o, g):
+        e.set_f(f0)
+        e.set_collision(3)
+    for _ in range(3):
+        o.step(cfg.dt)
+        g.step(cfg.dt)
+    f_o = o.get_f()
+    assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= 1e-11 * np.abs(f_o).max()
+    assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
