@@ -207,6 +207,10 @@ def weighted_probe(g, cfg, dev, which, reps=2):
             "bytes_per_sample_survey_8d_literal": bytes_literal_8d(cfg)}
 
 
+def samples_rate(cfg, steps, ms):
+    return cfg.samples_per_step * steps / (ms * 1e-3)
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -426,6 +430,22 @@ def run_ours(args, cfg):
     rank3b = weighted_probe(g, cfg, dev, "box") if (rank == 0 and not slabs and not args.no_probes) else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
 
+    # ---- bz_step_n: the same steps without returning to the host in between (captured CUDA graph), moments once at the end
+    stepn = None
+    if rank == 0 and not slabs:
+        nn = max(args.steps, 200 if small else args.steps)
+        g.step_n(cfg.dt, 4)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.step_n(cfg.dt, nn)
+        g.moments(mom_host)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_n = e0.elapsed_time(e1)
+        stepn = {"steps": nn, "ms_per_step": ms_n / nn, "samples_per_sec": samples_rate(cfg, nn, ms_n),
+                 "what": "bz_step_n(%d) + one bz_moments: two steps per replay of a captured CUDA graph, Philox step word on the device" % nn}
+
     # ---- end to end: host f in, host f and moments out, every step
     e2e_steps = args.steps
     barrier()
@@ -502,6 +522,7 @@ def run_ours(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": own_values * 8,
                 "d2h_bytes_per_step": own_values * 8 + mom_host.numel() * 8, "ms_per_step": ms_e2e / e2e_steps},
         "gpu_launches": launches,
+        "step_n": stepn,
         "roofline": roof64 if (roof64 and roof64["frac"] > roof["frac"]) else roof,
         "roofline_other_leg": roof if (roof64 and roof64["frac"] > roof["frac"]) else roof64,
         "roofline_transport": transport_roofline(cfg, tr_ms, tr_n, peak),

@@ -203,6 +203,16 @@ int bz_set_transport(bz_ctx* ctx, int scheme);
  * Asynchronous. */
 int bz_step(bz_ctx* ctx, double dt_fm);
 
+/* n forward-Euler steps, equivalent to n calls of bz_step.  The paper's runs are 10^4 - 10^6 steps of a 30^3 grid (P:330,
+ * P:348), i.e. steps of a few hundred microseconds, where the time between kernels counts: with transport scheme 0 and
+ * collision mode 0, 2 or 3 two consecutive steps (f -> f_new -> f: row sums, collision kernel, stream + Euler kernel,
+ * twice) are captured once as a CUDA graph on a stream of the library's own and replayed; the Philox step word lives on
+ * the device, is read by the collision kernel and advanced by the Euler kernel, so nothing returns to the host between
+ * steps.  Other settings run the plain loop.  Same results as n x bz_step up to the summation order of the deposits.
+ * Asynchronous with respect to the host like bz_step (the context's stream waits for the replays); the step copied to
+ * the device word is read from host memory at the call.  n = 0 is a no-op; n < 0: -1. */
+int bz_step_n(bz_ctx* ctx, double dt_fm, int n);
+
 /* The same step end to end from HOST memory: f_in_host (S*Nx*Np doubles, ideally pinned) replaces the context's f,
  * one bz_step is taken, and the new f is written to f_out_host; the context keeps the new f and the incremented step
  * counter exactly as after bz_set_f + bz_step + bz_get_f.  With at least 3 z layers and transport scheme 0 the work

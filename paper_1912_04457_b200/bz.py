@@ -22,7 +22,7 @@ class Grid(C.Structure):
 EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_samples", "bz_set_step", "bz_set_slab",
            "bz_copy_layers", "bz_set_msq_override", "bz_thermal_masses", "bz_set_masses", "bz_vlasov",
            "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_collision_box", "bz_debug_samples_box", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
-           "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_moments", "bz_last_error", "bz_set_profile",
+           "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_step_n", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_get_sample_counts",
            "bz_debug_samples")
 
@@ -64,6 +64,7 @@ def lib():
         L.bz_collision.argtypes = [vp, C.c_double, C.c_uint, vp]
         L.bz_stream.argtypes = [vp, C.c_double, vp]
         L.bz_step.argtypes = [vp, C.c_double]
+        L.bz_step_n.argtypes = [vp, C.c_double, C.c_int]
         L.bz_moments.argtypes = [vp, vp]
         L.bz_last_error.argtypes = [vp]
         L.bz_last_error.restype = C.c_char_p
@@ -289,6 +290,10 @@ class Boltzmann:
 
     def step(self, dt):
         self._chk(lib().bz_step(self._h, dt), "bz_step")
+
+    def step_n(self, dt, n):
+        """bz_step_n: n steps without returning to the host in between (two steps per replay of a captured CUDA graph)."""
+        self._chk(lib().bz_step_n(self._h, dt, int(n)), "bz_step_n")
 
     def step_host(self, dt, f_in, f_out):
         """bz_step_host: f_in, f_out are CPU float64 tensors (pinned for full copy speed) of n_values elements."""

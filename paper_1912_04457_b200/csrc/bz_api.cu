@@ -80,7 +80,8 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     CollideParams P;
     P.g = grid_const(c);
     P.f_aos = c->SP == 1 ? c->f : c->f_aos;    // one species: the API layout is already cell-major
-    P.dN_aos = c->dN_aos; P.m2 = c->m2; P.cell_tab = c->cell_tab; P.counters = c->counters;
+    P.dN_aos = c->dN_aos; P.rowsum = c->rowsum; P.cell_tab = c->cell_tab; P.counters = c->counters;
+    P.g2 = 4.0 * kPi * c->alpha_s; P.mD2 = c->m_D > 0.0 ? c->m_D * c->m_D : 0.0; P.glue_slot_mask = (c->mask & 1u) ? 1u : 0u;   // the gluon, if active, is layout index 0
     P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
     P.work_counter = c->work_counter; P.step_ptr = nullptr;
     const int layer = c->grid.nx * c->grid.ny;              // only the slab's own z layers collide (bz_set_slab)
@@ -129,13 +130,11 @@ int run_collide(bz_ctx* c, double dt_fm, unsigned step, int sampler = 0)
     return prof_mark(c, 0);
 }
 
-// regulator mass^2 per spatial cell from the current f (S8a.1)
+// row sums of the current f: the regulator mass^2 of S8a.1 and the moments of S8a.8 are functions of them (regulator_m2)
 int update_m2(bz_ctx* c)
 {
     if (c->rowsum_valid) return 0;
     BZ_CUDA(launch_rowsums(c->f, c->absp, c->w_invE, c->rowsum, c->Nx * c->S, c->Np, c->stream), "rowsums");
-    const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;   // the gluon, if active, is layout index 0
-    BZ_CUDA(launch_m2(c->rowsum, c->m2, c->Nx, c->S, glue_slot_mask, 4.0 * kPi * c->alpha_s, c->m_D, c->stream), "m2");
     c->rowsum_valid = true;
     return 0;
 }
@@ -192,9 +191,10 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     c->mass2 = nullptr; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
     c->aos_valid = false; c->rowsum_valid = false;
+    c->gstream = nullptr; c->gexec = nullptr; c->step_dev = nullptr; std::memset(&c->gkey, 0, sizeof c->gkey);
     c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
-    c->f = c->f_new = c->f_aos = c->dN_aos = c->m2 = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
+    c->f = c->f_new = c->f_aos = c->dN_aos = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         c->err = "bz_create: no CUDA device (this library has no CPU path)";
         return -2;
@@ -219,7 +219,6 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     const size_t aos_bytes = (size_t)c->Nx * c->Np * c->SP * sizeof(double);
     BZ_CUDA(cudaMalloc(&c->f_aos, aos_bytes), "cudaMalloc f_aos");
     BZ_CUDA(cudaMalloc(&c->dN_aos, aos_bytes), "cudaMalloc dN_aos");
-    BZ_CUDA(cudaMalloc(&c->m2, c->Nx * sizeof(double)), "cudaMalloc m2");
     BZ_CUDA(cudaMalloc(&c->mass2, (size_t)c->Nx * 4 * sizeof(double)), "cudaMalloc mass2");
     BZ_CUDA(cudaMemset(c->mass2, 0, (size_t)c->Nx * 4 * sizeof(double)), "memset mass2");
     BZ_CUDA(cudaMalloc(&c->rowsum, (size_t)c->Nx * c->S * 3 * sizeof(double)), "cudaMalloc rowsum");
@@ -266,8 +265,11 @@ int bz_destroy(bz_ctx* c)
 {
     if (!c) return -1;
     BZ_ON_DEVICE(c);
-    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->counters); cudaFree(c->m2); cudaFree(c->rowsum); cudaFree(c->mom);
+    cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->counters); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups); cudaFree(c->diag);
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
+    cudaFree(c->step_dev);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
     for (cudaEvent_t e : c->pipe_events) cudaEventDestroy(e);
     if (c->copy_in) cudaStreamDestroy(c->copy_in);
@@ -359,6 +361,7 @@ static TransportParams transport_params(const bz_ctx* c, double dt_fm, double* o
     T.nx = c->grid.nx; T.ny = c->grid.ny; T.nz = c->grid.nz; T.S = c->S; T.Np = c->Np;
     T.x_begin = 0; T.x_count = c->Nx;
     T.cfl = dt_fm / c->grid.dx;
+    T.step_ptr = nullptr;
     fill_deg(c, T.inv_deg);
     return T;
 }
@@ -495,6 +498,78 @@ int bz_step(bz_ctx* c, double dt_fm)
 }
 
 
+/* n steps without returning to the host in between: see include/bz.h */
+int bz_step_n(bz_ctx* c, double dt_fm, int n)
+{
+    if (!c || n < 0) return -1;
+    if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
+    // Eq. 15 transport and the paper's sampler keep per-step host logic (mass updates, scratch buffers): plain loop
+    const bool graphable = c->scheme == 0 && c->coll_mode != 1 && !c->profile;
+    int done = 0;
+    // the first step (and one more if an odd number is left) goes the ordinary way: it also configures the kernels and
+    // brings the cell-major copy and the row-sum bookkeeping into the state the captured steps start from
+    while (done < n && (!graphable || done == 0 || ((n - done) & 1))) {
+        if (int rc = bz_step(c, dt_fm)) return rc;
+        ++done;
+    }
+    if (done == n) return 0;
+    const int pairs = (n - done) / 2;
+    if (!c->gstream) BZ_CUDA(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking), "graph stream");
+    if (!c->step_dev) BZ_CUDA(cudaMalloc(&c->step_dev, sizeof(uint32_t)), "cudaMalloc step word");
+    bz_ctx::GraphKey key;
+    std::memset(&key, 0, sizeof key);
+    key.dt = dt_fm; key.Ns = c->Ns; key.coll_mode = c->coll_mode; key.zb = c->zb; key.ze = c->ze; key.seed = c->seed; key.xoff = c->xoff;
+    for (int k = 0; k < 7; ++k) key.ovr[k] = c->msq_ovr[k];
+    key.f = c->f;
+    if (!c->gexec || std::memcmp(&key, &c->gkey, sizeof key) != 0) {
+        if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+        cudaGraph_t graph = nullptr;
+        BZ_CUDA(cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal), "begin capture");
+        cudaError_t e = cudaSuccess;
+        double* fa = c->f;
+        double* fb = c->f_new;
+        for (int half = 0; half < 2 && e == cudaSuccess; ++half) {
+            e = launch_rowsums(fa, c->absp, c->w_invE, c->rowsum, c->Nx * c->S, c->Np, c->gstream);
+            if (e != cudaSuccess) break;
+            CollideParams P = collide_params(c, dt_fm, 0u);
+            P.step_ptr = c->step_dev;
+            P.sampler = c->coll_mode == 0 ? 0 : c->coll_mode - 1;
+            if (c->SP == 1) P.f_aos = fa;                      // one species: f itself is the gather source
+            e = launch_collide(P, c->sms, c->gstream);
+            if (e != cudaSuccess) break;
+            TransportParams T = transport_params(c, dt_fm, fb);
+            T.f = fa; T.step_ptr = c->step_dev;
+            e = launch_transport(T, 1, c->gstream);
+            std::swap(fa, fb);
+        }
+        cudaError_t e2 = cudaStreamEndCapture(c->gstream, &graph);
+        if (e == cudaSuccess) e = e2;
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { c->gexec = nullptr; return fail_cuda(c, e, "bz_step_n: graph capture"); }
+        c->gkey = key;
+    }
+    // order: whatever the context's stream has queued -> the graph launches -> the context's stream again
+    cudaEvent_t ev = nullptr;
+    BZ_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event");
+    cudaError_t e = cudaEventRecord(ev, c->stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->gstream, ev, 0);
+    const uint32_t step0 = c->step;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->step_dev, &step0, sizeof step0, cudaMemcpyHostToDevice, c->gstream);
+    for (int q = 0; q < pairs && e == cudaSuccess; ++q) e = cudaGraphLaunch(c->gexec, c->gstream);
+    if (e == cudaSuccess) e = cudaEventRecord(ev, c->gstream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, ev, 0);
+    cudaEventDestroy(ev);
+    if (e != cudaSuccess) return fail_cuda(c, e, "bz_step_n: graph launch");
+    c->step += 2u * (unsigned)pairs;
+    g_launch_count += 6ull * (unsigned long long)pairs;
+    c->generated += 2ull * (unsigned long long)pairs * (unsigned long long)((c->ze - c->zb) * c->grid.nx * c->grid.ny) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
+    c->rowsum_valid = false;          // the row sums on the device belong to the f before the last step
+    c->aos_valid = true;
+    return 0;
+}
+
 /* Pipelined end-to-end step: see include/bz.h.  Chunks of z layers flow H2D -> (row sums, m^2, cell-major copy,
  * collision) -> stream + Euler -> D2H on three streams; the collision term of a chunk needs only that chunk's f
  * (Eq. 5 is local in x), the upwind stencil of chunk k needs the old f of chunks k - 1 and k + 1 as well. */
@@ -541,7 +616,6 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
         if (cnt) BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
         BZ_CUDA(cudaEventRecord(h2d_done[k], c->copy_in), "record");
     }
-    const unsigned glue_slot_mask = (c->mask & 1u) ? 1u : 0u;
     auto transport_chunk = [&](int k) -> int {
         TransportParams T = transport_params(c, dt_fm, c->f_new);
         T.x_begin = x0_of(k); T.x_count = nx_of(k);
@@ -557,8 +631,6 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
         BZ_CUDA(cudaStreamWaitEvent(c->stream, h2d_done[k], 0), "wait");
         BZ_CUDA(launch_rowsums(c->f + (size_t)x0 * cell_vals, c->absp, c->w_invE, c->rowsum + (size_t)x0 * c->S * 3, nxk * c->S, c->Np,
                                c->stream), "rowsums");
-        BZ_CUDA(launch_m2(c->rowsum + (size_t)x0 * c->S * 3, c->m2 + x0, nxk, c->S, glue_slot_mask, 4.0 * kPi * c->alpha_s, c->m_D,
-                          c->stream), "m2");
         if (c->SP != 1)
             BZ_CUDA(launch_pack(c->f + (size_t)x0 * cell_vals, c->f_aos + (size_t)x0 * c->Np * c->SP, nxk, c->S, c->SP, c->Np,
                                 c->stream), "pack");
@@ -722,7 +794,8 @@ int bz_moments(bz_ctx* c, double* out_host)
     const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
     const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
     const double d3x = ((c->grid.dx * c->grid.dx) * c->grid.dx) / ((kHbarc * kHbarc) * kHbarc);
-    BZ_CUDA(launch_moments(c->rowsum, c->m2, c->mom, c->Nx, c->S, deg, d3p / twopi3, d3x,
+    BZ_CUDA(launch_moments(c->rowsum, c->mom, c->Nx, c->S, deg, (c->mask & 1u) ? 1u : 0u, 4.0 * kPi * c->alpha_s,
+                           c->m_D > 0.0 ? c->m_D * c->m_D : 0.0, d3p / twopi3, d3x,
                            c->zb * c->grid.nx * c->grid.ny, c->ze * c->grid.nx * c->grid.ny, c->stream), "moments");
     const size_t cnt = (size_t)2 * c->S * c->Nx + 2 * c->S + c->Nx;
     BZ_CUDA(cudaMemcpyAsync(out_host, c->mom, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "moments copy");

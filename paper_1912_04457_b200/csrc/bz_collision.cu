@@ -311,7 +311,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 const int nxt_x = P.x_begin + (int)(next_item / (unsigned)P.regions_per_x);
                 if (nxt_x == xcell || (count == 0 && rcount == 0)) {
                     const int region = (int)(next_item % (unsigned)P.regions_per_x);
-                    if (nxt_x != xcell) { xcell = nxt_x; if (lane == 0) wm.m2x = P.m2[xcell]; }
+                    if (nxt_x != xcell) { xcell = nxt_x; if (lane == 0) wm.m2x = regulator_m2(P.rowsum, xcell, P.S, P.glue_slot_mask, P.g2, P.mD2); }
                     i = i0 = region * P.cells_per_region; i_end = min(i + P.cells_per_region, P.Np); base = 0;
                     next_item = 0xffffffffu;
                     fresh = i < i_end;

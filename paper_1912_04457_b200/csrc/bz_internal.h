@@ -19,7 +19,9 @@ struct CollideParams {
     GridConst g;
     const double* f_aos;  // [Nx][Np][SP] cell-major staging copy of f (pad slots 0)
     double* dN_aos;       // [Nx][Np][SP] deposit scratch in number units, zero on entry
-    const double* m2;     // [Nx] regulator mass^2
+    const double* rowsum; // [Nx][S][3] row sums of the current f (rowsum_kernel): [2] = sum f d3p/((2pi)^3 |p|)
+    double g2, mD2;       // 4 pi alpha_s; m_D^2 if m_D > 0 (fixed regulator), else 0: m^2(x) from the row sums (Eq. 8, S8a.1)
+    unsigned glue_slot_mask;   // bit a: layout index a is the gluon
     const double* cell_tab;   // [Np][4] (p1x, p1y, p1z, E1) of the momentum cell centres
     int S, Np, Nx, Ns;
     unsigned long long* counters;   // device [1]: kinematic samples accepted (both outgoing legs in the box), accumulated over launches
@@ -67,6 +69,7 @@ struct TransportParams {
     double* dN_aos;       // collision deposits [Nx][Np][SP] (number units), reset to 0 when consumed
     double* out;          // f_new or dF
     double* f_aos_out;    // mode 1: the new f once more, cell-major [Nx][Np][SP] (the next step's gather source); unused if SP == 1
+    uint32_t* step_ptr;   // modes 1, 2: if not NULL the device step counter is incremented (captured graphs, bz_step_n)
     int SP;
     const double* vx; const double* vy; const double* vz;   // [Np] p/|p| at the cell centre (0 at p = 0)
     int nx, ny, nz, S, Np;
@@ -109,17 +112,34 @@ struct bz_ctx_impl {
     bool rowsum_valid;               // rowsum / m2 belong to the current f
     int sms;                         // SMs of the device (persistent grid size)
     int cells_per_region, regions_per_x;
-    double *m2;                      // device [Nx]
-    double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|)
+    double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|) of the current f
     double *mom;                     // device [2*S*Nx + 2*S + Nx]
     double *absp, *w_invE, *vx, *vy, *vz;   // device [Np] tables
     double *cell_tab;                // device [Np][4]: p1x, p1y, p1z, E1 (built on the device, bit-exact arithmetic)
+    // bz_step_n: two consecutive steps (f -> f_new -> f) captured as one CUDA graph on a stream of the library's own
+    cudaStream_t gstream;
+    cudaGraphExec_t gexec;
+    uint32_t* step_dev;              // device: the Philox step word the captured kernels read and advance
+    struct GraphKey { double dt; int Ns, coll_mode, zb, ze; uint32_t seed, xoff; double ovr[7]; const double* f; } gkey;
     std::string err;
     bool profile;
     std::vector<cudaEvent_t> prof_events[2];
     cudaStream_t copy_in, copy_out;  // bz_step_host: H2D / D2H streams (created at first use)
     std::vector<cudaEvent_t> pipe_events;   // bz_step_host: per chunk h2d-done and transport-done events (created at first use)   // start/stop pairs: [0] collision (pack + collide), [1] stream + Euler
 };
+
+#ifdef __CUDACC__
+// regulator mass^2 of spatial cell x (S8a.1): m_D^2 if fixed, else Eq. 8 with E_p = |p| from the row sums,
+// g^2 sum_a c_a rowsum[x][a][2], c = 6 for the gluon row, 1 for quark rows.  One definition for the collision kernel and
+// for bz_moments, so that the m^2 reported is bit for bit the one used.
+__device__ __forceinline__ double regulator_m2(const double* __restrict__ rowsum, int x, int S, unsigned glue_slot_mask, double g2, double mD2)
+{
+    if (mD2 > 0.0) return mD2;
+    double acc = 0.0;
+    for (int a = 0; a < S; ++a) acc += (((glue_slot_mask >> a) & 1u) ? 6.0 : 1.0) * rowsum[((size_t)x * S + a) * 3 + 2];
+    return g2 * acc;
+}
+#endif
 
 // kernels launched by this library in this process (bz_launch_count); bumped by every launcher below
 extern std::atomic<unsigned long long> g_launch_count;
@@ -140,12 +160,9 @@ cudaError_t launch_transport(const TransportParams& P, int mode, cudaStream_t st
 // rowsum[x][a][0..2]
 cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_invE, double* rowsum, int rows, int Np,
                            cudaStream_t st);
-// m2[x] = g2 * sum_a c_a rowsum[x][a][2]  (or m_D^2)
-cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned glue_slot_mask, double g2, double m_D,
-                      cudaStream_t st);
-// mom = per-cell (n, e), totals, m2
-cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
-                           double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st);
+// mom = per-cell (n, e), totals, m2(x) = regulator_m2
+cudaError_t launch_moments(const double* rowsum, double* mom, int Nx, int S, const double* deg, unsigned glue_slot_mask, double g2,
+                           double mD2, double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st);
 
 // NEXT rank 2 (bz_vlasov.cu): thermal masses of Eq. 8-9 and the central-difference drift + force of Eq. 15
 cudaError_t launch_thermal_masses(const double* f, const double* cell_tab, double* mass2, int Nx, int S, int Np,

@@ -79,6 +79,10 @@ __global__ void __launch_bounds__(256, BZ_TR_MINB) transport_kernel(const Transp
             }
         }
     }
+    if (kMode != 0) {
+        // bz_step_n: the device step counter (the next step's Philox key word) moves on once per launch
+        if (P.step_ptr && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) *P.step_ptr += 1u;
+    }
 }
 
 // One CTA per (xcell, a) row: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|) over the Np momentum cells.
@@ -108,23 +112,11 @@ __global__ void __launch_bounds__(256) rowsum_kernel(const double* __restrict__ 
     }
 }
 
-// m2[x] = g^2 sum_a c_a rowsum[x][a][2], c = 6 for the gluon row, 1 for quark rows (Eq. 8 with E_p = |p|, S8a.1)
-__global__ void m2_kernel(const double* __restrict__ rowsum, double* __restrict__ m2, int Nx, int S, unsigned glue_slot_mask,
-                          double g2, double m_D)
-{
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    if (x >= Nx) return;
-    if (m_D > 0.0) { m2[x] = m_D * m_D; return; }
-    double acc = 0.0;
-    for (int a = 0; a < S; ++a) acc += (((glue_slot_mask >> a) & 1u) ? 6.0 : 1.0) * rowsum[((size_t)x * S + a) * 3 + 2];
-    m2[x] = g2 * acc;
-}
-
 // per-cell (n, e) and m2 copied behind them (all blocks); totals over the own cells x_begin..x_end: block b < 2 S sums
 // total b = (species b / 2, n or e) with all its threads (strided partial sums, then a fixed-order tree: the result
 // does not depend on the launch)
-__global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__ rowsum, const double* __restrict__ m2, double* __restrict__ mom,
-                               int Nx, int S, double d3p_over_2pi3, double d3x, int x_begin, int x_end, const double d0, const double d1,
+__global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__ rowsum, double* __restrict__ mom, int Nx, int S,
+                               unsigned glue_slot_mask, double g2, double mD2, double d3p_over_2pi3, double d3x, int x_begin, int x_end, const double d0, const double d1,
                                const double d2, const double d3, const double d4, const double d5, const double d6)
 {
     const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
@@ -135,7 +127,7 @@ __global__ void __launch_bounds__(256) moments_kernel(const double* __restrict__
         mom[2 * r + 1] = deg[a] * rowsum[3 * r + 1] * d3p_over_2pi3;
     }
     for (size_t x = blockIdx.x * (size_t)blockDim.x + threadIdx.x; x < (size_t)Nx; x += (size_t)gridDim.x * blockDim.x)
-        mom[2 * rows + 2 * S + x] = m2[x];
+        mom[2 * rows + 2 * S + x] = regulator_m2(rowsum, (int)x, S, glue_slot_mask, g2, mD2);
     if (blockIdx.x < 2 * S) {
         const int a = blockIdx.x >> 1, c = blockIdx.x & 1;
         double t = 0.0;
@@ -174,21 +166,13 @@ cudaError_t launch_rowsums(const double* f, const double* absp, const double* w_
     return cudaGetLastError();
 }
 
-cudaError_t launch_m2(const double* rowsum, double* m2, int Nx, int S, unsigned glue_slot_mask, double g2, double m_D,
-                      cudaStream_t st)
-{
-    m2_kernel<<<(Nx + 127) / 128, 128, 0, st>>>(rowsum, m2, Nx, S, glue_slot_mask, g2, m_D);
-    ++g_launch_count;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_moments(const double* rowsum, const double* m2, double* mom, int Nx, int S, const double* deg,
-                           double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st)
+cudaError_t launch_moments(const double* rowsum, double* mom, int Nx, int S, const double* deg, unsigned glue_slot_mask, double g2,
+                           double mD2, double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st)
 {
     int blocks = (Nx * S + 255) / 256;
     if (blocks > 148) blocks = 148;
     if (blocks < 2 * S) blocks = 2 * S;          // one block per total
-    moments_kernel<<<blocks, 256, 0, st>>>(rowsum, m2, mom, Nx, S, d3p_over_2pi3, d3x, x_begin, x_end, deg[0], deg[1], deg[2], deg[3], deg[4],
+    moments_kernel<<<blocks, 256, 0, st>>>(rowsum, mom, Nx, S, glue_slot_mask, g2, mD2, d3p_over_2pi3, d3x, x_begin, x_end, deg[0], deg[1], deg[2], deg[3], deg[4],
                                            deg[5], deg[6]);
     ++g_launch_count;
     return cudaGetLastError();

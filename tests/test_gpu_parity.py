@@ -785,3 +785,32 @@ def test_step_with_the_inbox_collision_term():
     f_o = o.get_f()
     assert np.abs(g.get_f().cpu().numpy() - f_o).max() <= 1e-11 * np.abs(f_o).max()
     assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
+
+
+# --------------------------------------------------------------------------------- bz_step_n (captured CUDA graph)
+@pytest.mark.parametrize("cfg,n", [(wl.CONFIGS[0], 10), (wl.scaled(wl.CONFIGS[2], np_=12, samples=40), 7),
+                                   (wl.scaled(wl.CONFIGS[3], nx=3, np_=8, samples=16), 6), (wl.scaled(wl.CONFIGS[1], np_=10, samples=33), 1)],
+                         ids=["cfg0_full", "mix12", "inhom3", "quarks_one_step"])
+def test_step_n_matches_oracle_and_step_loop(cfg, n):
+    """bz_step_n(n): n Euler steps replayed from a captured CUDA graph (device-resident Philox step word) against the
+    oracle's n steps; then bz_step continues from the same state and step counter, and a second bz_step_n reuses the graph."""
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg) + 0.01 * wl.random_f(cfg, seed=23)
+    o.set_f(f)
+    g.set_f(f)
+    g.step_n(cfg.dt, n)
+    for _ in range(n):
+        o.step(cfg.dt)
+    _f_after_steps_check(g.get_f().cpu().numpy(), o.get_f(), o.gross(), "step_n(%d)" % n)
+    o.step(cfg.dt)
+    g.step(cfg.dt)                                                         # the host step counter moved with the device's
+    _f_after_steps_check(g.get_f().cpu().numpy(), o.get_f(), o.gross(), "step after step_n")
+    g.step_n(cfg.dt, 4)
+    for _ in range(4):
+        o.step(cfg.dt)
+    f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
+    _f_after_steps_check(f_g, f_o, o.gross(), "second step_n")
+    mo, mg = o.moments(), g.moments()
+    for key in ("ne", "tot", "m2"):
+        a, b = np.asarray(mo[key]), mg[key].numpy()
+        assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(np.abs(a), np.abs(a).max() * 1e-6)), key
