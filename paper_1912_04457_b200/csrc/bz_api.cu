@@ -82,10 +82,10 @@ CollideParams collide_params(const bz_ctx* c, double dt_fm, unsigned step)
     P.f_aos = c->SP == 1 ? c->f : c->f_aos;    // one species: the API layout is already cell-major
     P.dN_aos = c->dN_aos; P.rowsum = c->rowsum; P.cell_tab = c->cell_tab; P.counters = c->counters;
     P.g2 = 4.0 * kPi * c->alpha_s; P.mD2 = c->m_D > 0.0 ? c->m_D * c->m_D : 0.0; P.glue_slot_mask = (c->mask & 1u) ? 1u : 0u;   // the gluon, if active, is layout index 0
-    P.cells_per_region = c->cells_per_region; P.regions_per_x = c->regions_per_x;
+    collide_item_geometry(c->Np, c->Nx, c->Ns, c->sms, &P.units_per_item, &P.ppc, &P.regions_per_x);
     P.work_counter = c->work_counter; P.step_ptr = nullptr;
     const int layer = c->grid.nx * c->grid.ny;              // only the slab's own z layers collide (bz_set_slab)
-    P.n_items = (unsigned)((c->ze - c->zb) * layer) * (unsigned)c->regions_per_x; P.x_begin = c->zb * layer;
+    P.n_items = (unsigned)((c->ze - c->zb) * layer) * (unsigned)P.regions_per_x; P.x_begin = c->zb * layer;
     P.x_rng_offset = c->xoff;
     P.S = c->S; P.Np = c->Np; P.Nx = c->Nx; P.Ns = c->Ns;
     P.seed = c->seed; P.step = step;
@@ -192,7 +192,7 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
     c->aos_valid = false; c->rowsum_valid = false;
     c->gstream = nullptr; c->gexec = nullptr; c->step_dev = nullptr; std::memset(&c->gkey, 0, sizeof c->gkey);
-    c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1; c->cells_per_region = 1; c->regions_per_x = c->Np;
+    c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -205,8 +205,6 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
         c->device = dev;                            // the context lives on the device that is current now
         BZ_CUDA(cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev), "SM count");
         if ((long long)c->Nx * c->Np >= (1LL << 32)) { c->err = "bz_create: more than 2^32 (xcell, pcell) pairs"; return -1; }
-        c->cells_per_region = collide_cells_per_region(c->Np, c->Nx, c->sms);
-        c->regions_per_x = (c->Np + c->cells_per_region - 1) / c->cells_per_region;
     }
     const size_t bytes = c->n_values * sizeof(double);
     BZ_CUDA(cudaMalloc(&c->counters, sizeof(unsigned long long)), "cudaMalloc sample counter");
@@ -639,7 +637,7 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
         if (ze > zb) {
             CollideParams P = collide_params(c, dt_fm, c->step);
             P.x_begin = zb * layer_cells;
-            P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)c->regions_per_x;
+            P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)P.regions_per_x;
             BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
             c->generated += (unsigned long long)((ze - zb) * layer_cells) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
                 }

@@ -292,7 +292,8 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
     int head = 0, count = 0;             // ring: records [head, head + count)
     int nb = 0;                          // > 0: the gather of records [head, head + nb) is in flight
     int rcount = 0;                      // entries in the retry list
-    int xcell = -1, i = 0, i_end = 0, i0 = 0, base = 0;   // current item: p1 cells [i, i_end) of xcell (i0 = its first), next sample
+    int xcell = -1, i = 0, i0 = 0, base = 0, units_left = 0;   // current item: units_left passes of 32 samples left, the next one
+                                                                // starts at sample `base` of p1 cell i of xcell (i0 = the item's first cell)
     unsigned next_item = 0xffffffffu;    // decoded later; 0xffffffff: none fetched yet
     bool exhausted = false;
     unsigned n_acc = 0u;                 // samples accepted by this warp (bz_get_sample_counts)
@@ -301,7 +302,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
 
     for (;;) {
         // ---- A: fresh work?  An item of ANOTHER spatial cell is only adopted once ring and retry list are empty
-        bool fresh = i < i_end;
+        bool fresh = units_left > 0;
         if (!fresh && !exhausted) {
             if (next_item == 0xffffffffu) {
                 next_item = __reduce_max_sync(0xffffffffu, lane == 0 ? pref_item : 0u);   // REDUX: the result is provably warp-uniform
@@ -312,12 +313,14 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 if (nxt_x == xcell || (count == 0 && rcount == 0)) {
                     const int region = (int)(next_item % (unsigned)P.regions_per_x);
                     if (nxt_x != xcell) { xcell = nxt_x; if (lane == 0) wm.m2x = regulator_m2(P.rowsum, xcell, P.S, P.glue_slot_mask, P.g2, P.mD2); }
-                    i = i0 = region * P.cells_per_region; i_end = min(i + P.cells_per_region, P.Np); base = 0;
+                    // an item is a run of units_per_item passes (32 samples each) through the p1 cells, ppc passes per cell
+                    const int u0 = region * P.units_per_item, u1 = min(u0 + P.units_per_item, P.Np * P.ppc);
+                    i = i0 = u0 / P.ppc; base = (u0 - i0 * P.ppc) * 32; units_left = u1 - u0;
                     next_item = 0xffffffffu;
-                    fresh = i < i_end;
+                    fresh = units_left > 0;
                     if (lane == 0) pref_item = atomicAdd(P.work_counter, 1u);
                     // the item's p1 cells (at most 32): one coalesced read of the cell table into shared memory
-                    if (i0 + lane < i_end) {
+                    if (i0 + lane <= (u1 - 1) / P.ppc) {
                         const double2* src = reinterpret_cast<const double2*>(P.cell_tab) + 2 * (size_t)(i0 + lane);
                         double2* dst = reinterpret_cast<double2*>(&wm.p1tab[lane][0]);
                         dst[0] = __ldg(src); dst[1] = __ldg(src + 1);
@@ -351,7 +354,7 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 p1x = a.x; p1y = a.y; p1z = b.x; E1 = b.y;
                 ci = i; smp = base + lane; kstart = 0u;
                 active = smp < P.Ns;
-                base += 32;
+                base += 32; --units_left;
                 if (base >= P.Ns) { base = 0; ++i; }
             }
             Sample sa;
@@ -492,12 +495,19 @@ cudaError_t launch_collide_weighted(const CollideParams& P, int ctas, cudaStream
 
 int collide_slots_per_cell(unsigned mask) { return mask == 0x01u ? 1 : 8; }
 
-// p1 cells per work item: long items amortise the hand-over between items, short ones balance the load on small grids
-int collide_cells_per_region(int Np, int Nx, int sms)
+// Work items: a run of `units` passes of 32 samples (ppc = ceil(Ns / 32) passes per p1 cell).  About 8 items per warp:
+// long items amortise the hand-over between items, short ones balance the load on small grids (config 0 has 2.9 passes
+// per warp in all).  Items of a cell or more are whole cells, at most 32 (the warp's p1 table).
+void collide_item_geometry(int Np, int Nx, int Ns, int sms, int* units_per_item, int* ppc_out, int* regions_per_x)
 {
-    const long long total_cells = (long long)Np * Nx;
-    const long long c = total_cells / ((long long)sms * kWarps * 8);
-    return (int)(c < 1 ? 1 : (c > 32 ? 32 : c));
+    const int ppc = (Ns + 31) / 32;
+    const long long total = (long long)Np * Nx * ppc;
+    const long long slots = (long long)sms * kWarps * 8;
+    long long u = (total + slots - 1) / slots;
+    if (u < 1) u = 1;
+    if (u >= ppc) { u = (u / ppc) * ppc; if (u > 32LL * ppc) u = 32LL * ppc; }
+    *units_per_item = (int)u; *ppc_out = ppc;
+    *regions_per_x = (int)(((long long)Np * ppc + u - 1) / u);
 }
 
 // one persistent CTA per SM (fewer when there is less work than warps)

@@ -30,8 +30,8 @@ struct CollideParams {
     unsigned n_items;         // Nx * regions_per_x work items, item = xcell * regions_per_x + region
     int x_begin;              // first colliding spatial cell (items address xcell = x_begin + item / regions_per_x)
     uint32_t x_rng_offset;    // Philox spatial counter = xcell + x_rng_offset (slab of a larger domain, bz_set_slab)
-    int cells_per_region;     // p1 cells per work item (one producer warp each)
-    int regions_per_x;        // ceil(Np / cells_per_region)
+    int units_per_item, ppc;  // passes of 32 samples per work item; passes per p1 cell = ceil(Ns / 32)
+    int regions_per_x;        // work items per spatial cell = ceil(Np * ppc / units_per_item)
     uint32_t seed, step;
     const uint32_t* step_ptr; // device: if not NULL the Philox step is read from here (captured graphs, bz_step_n), else `step`
     double g4K;           // (4 pi alpha_s)^2 * K,  K = dtG Vp / (2048 pi^4 Ns)    (S8c step 0)
@@ -111,7 +111,6 @@ struct bz_ctx_impl {
     bool aos_valid;                  // f_aos holds the current f (written by the Euler kernel; bz_set_f invalidates)
     bool rowsum_valid;               // rowsum / m2 belong to the current f
     int sms;                         // SMs of the device (persistent grid size)
-    int cells_per_region, regions_per_x;
     double *rowsum;                  // device [Nx][S][3]: sum f, sum |p| f, sum f d3p/((2pi)^3 |p|) of the current f
     double *mom;                     // device [2*S*Nx + 2*S + Nx]
     double *absp, *w_invE, *vx, *vy, *vz;   // device [Np] tables
@@ -146,7 +145,7 @@ extern std::atomic<unsigned long long> g_launch_count;
 
 // launchers (each returns the cudaError_t of the launch)
 int collide_slots_per_cell(unsigned mask);
-int collide_cells_per_region(int Np, int Nx, int sms);
+void collide_item_geometry(int Np, int Nx, int Ns, int sms, int* units_per_item, int* ppc, int* regions_per_x);
 cudaError_t launch_collide(const CollideParams& P, int sms, cudaStream_t st);
 cudaError_t launch_cell_table(const GridConst& g, int Np, double* tab, cudaStream_t st);
 cudaError_t launch_pack(const double* f, double* f_aos, int Nx, int S, int SP, int Np, cudaStream_t st);
