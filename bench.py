@@ -174,7 +174,7 @@ def paper_probe(g, cfg, dev, fp64_peak, reps=2):
     # weight 8; per channel and kept root 13 (bracket 7, x |M|^2, 4 deposits, 1 gross)
     flop = tuples * 70.0 + roots * tuples * 83.0 + roots * n_ch * 13.0
     rate = samples / (ms * 1e-3)
-    return {"kernel": "paper_kernel (bz_collision_paper)", "bound": "alu", "sample": "%d of %d spatial cells" % (cells, cfg.Nx),
+    return {"kernel": "paper_queue_kernel (bz_collision_paper)", "bound": "alu", "sample": "%d of %d spatial cells" % (cells, cfg.Nx),
             "ms": ms, "samples_per_sec": rate, "mass_tuples": tuples, "roots_per_tuple": roots, "channels": n_ch,
             "flop_per_sample": flop, "achieved": rate * flop / 1e12, "peak": fp64_peak, "unit": "TFLOP/s",
             "frac": rate * flop / 1e12 / fp64_peak if fp64_peak else None}

@@ -156,6 +156,7 @@ int run_thermal_masses(bz_ctx* c)
     class_bits(c, cls, ids);
     const double L = c->grid.pmax - c->grid.pmin, dp = L / c->grid.np, d3p = (dp * dp) * dp;
     const double twopi3 = (2.0 * kPi) * (2.0 * kPi) * (2.0 * kPi);
+    c->masses_zero = false;
     BZ_CUDA(launch_thermal_masses(c->f, c->cell_tab, c->mass2, c->Nx, c->S, c->Np, cls, ids, 4.0 * kPi * c->alpha_s,
                                   d3p / twopi3, c->stream), "thermal masses");
     return 0;
@@ -188,7 +189,7 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     c->alpha_s = alpha_s; c->m_D = m_D; c->seed = 0; c->step = 0; c->stream = nullptr; c->profile = false; c->copy_in = nullptr; c->copy_out = nullptr;
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
-    c->mass2 = nullptr; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
+    c->mass2 = nullptr; c->masses_zero = true; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
     c->aos_valid = false; c->rowsum_valid = false;
     c->gstream = nullptr; c->gexec = nullptr; c->step_dev = nullptr; std::memset(&c->gkey, 0, sizeof c->gkey);
@@ -413,6 +414,7 @@ int bz_set_masses(bz_ctx* c, const double* mass2_host)
 {
     if (!c || !mass2_host) return -1;
     if (!c->mass2) return -4;
+    c->masses_zero = false;
     BZ_CUDA(cudaMemcpyAsync(c->mass2, mass2_host, (size_t)c->Nx * 4 * sizeof(double), cudaMemcpyHostToDevice, c->stream), "set masses");
     BZ_CUDA(cudaStreamSynchronize(c->stream), "set masses sync");
     return 0;
@@ -678,6 +680,7 @@ static int paper_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
     const double g2 = 4.0 * kPi * c->alpha_s;
     P.g4 = g2 * g2;
     P.mD2 = c->m_D > 0.0 ? c->m_D * c->m_D : 0.0;
+    P.all_massless = c->masses_zero ? 1 : 0;
     P.has_ovr = 0;
     for (int k = 0; k < 7; ++k) {
         P.msq_ovr[k] = c->msq_ovr[k] >= 0.0 ? c->msq_ovr[k] / P.g4 : -1.0;

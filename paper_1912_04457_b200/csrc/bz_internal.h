@@ -58,6 +58,7 @@ struct PaperParams {
     uint32_t seed, step, x_rng_offset;
     double Kp, g4, mD2;       // Kp = (dt/hbarc) L^5 / (Ns (2 pi)^5 16) / 8;  mD2 > 0: fixed regulator, else m_g^2(x)
     int has_ovr;
+    int all_massless;         // the host knows every stored thermal mass is 0 (never set): one tuple, factorised channel algebra
     double msq_ovr[7];
     double dbg_msq[4];        // debug launch: the mass tuple whose roots are written out
     unsigned mask;            // bz_is.cu: active species ids
@@ -90,6 +91,7 @@ struct bz_ctx_impl {
     int zb, ze;                      // bz_set_slab: own z layers [zb, ze); the others are halo copies
     double msq_ovr[7];               // bz_set_msq_override: constant |M|^2 per kind of Table I, < 0 = Table I
     double* mass2;                   // device [Nx][4]: thermal masses^2 m_g^2, m_u^2, m_d^2, m_s^2 (Eq. 8-9); 0 at start
+    bool masses_zero;                // no bz_thermal_masses / bz_set_masses call yet: mass2 is all 0
     double* E_tab;                   // device [Nx][4][Np] energies sqrt(p^2 + m^2), allocated at the first bz_vlasov / scheme >= 1 step
     int* x_nb;                       // device [Nx][6] periodic spatial neighbour offsets (built with E_tab)
     unsigned char* p_wrap;           // device [Np] momentum wrap flags (built with E_tab)

@@ -86,14 +86,28 @@ struct Root {
 
 // Eq. 17-19 for one mass tuple: see oracle/bzo.c paper_roots for the algebra (two squarings of E1 + E2 = Et give
 // a z^2 - C Pz z + (Et^2 A1 - C^2/4) = 0).  Single rounded operations, the oracle's association order.
-__device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
-                                           double m1, double m2, double m3, double m4, int ixy1, int ixy2, Root (&out)[2])
+// energies of the two outgoing legs for the four mass classes: E3[c] = sqrt(k3^2 + m_c^2), Ep[c] = sqrt(p^2 + m_c^2), with
+// the association of paper_roots; the roots of a tuple take E3 of its third and Ep of its fourth class
+struct PaperLegs {
+    double E3[4], Ep[4];
+    __device__ __forceinline__ PaperLegs(const double (&p)[3], const double (&k3)[3], const double* m)
+    {
+        const double k2 = __dadd_rn(__dadd_rn(__dmul_rn(k3[0], k3[0]), __dmul_rn(k3[1], k3[1])), __dmul_rn(k3[2], k3[2]));
+        const double p2 = __dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2]));
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { E3[c] = __dsqrt_rn(__dadd_rn(k2, m[c])); Ep[c] = __dsqrt_rn(__dadd_rn(p2, m[c])); }
+    }
+    __device__ __forceinline__ double e3(int c) const { return c == 0 ? E3[0] : (c == 1 ? E3[1] : (c == 2 ? E3[2] : E3[3])); }
+    __device__ __forceinline__ double ep(int c) const { return c == 0 ? Ep[0] : (c == 1 ? Ep[1] : (c == 2 ? Ep[2] : Ep[3])); }
+};
+
+__device__ __forceinline__ int paper_roots_core(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
+                                                double m1, double m2, double m3, double m4, double E3, double Ep, int ixy1, int ixy2,
+                                                Root (&out)[2])
 {
 #define MUL __dmul_rn
 #define ADD __dadd_rn
 #define SUB __dsub_rn
-    const double E3 = __dsqrt_rn(ADD(ADD(ADD(MUL(k3[0], k3[0]), MUL(k3[1], k3[1])), MUL(k3[2], k3[2])), m3));
-    const double Ep = __dsqrt_rn(ADD(ADD(ADD(MUL(p[0], p[0]), MUL(p[1], p[1])), MUL(p[2], p[2])), m4));
     const double Et = ADD(E3, Ep);
     const double Px = ADD(k3[0], p[0]), Py = ADD(k3[1], p[1]), Pz = ADD(k3[2], p[2]);
     const double A1 = ADD(ADD(MUL(k1x, k1x), MUL(k1y, k1y)), m1);
@@ -135,6 +149,14 @@ __device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)
 #undef ADD
 #undef SUB
     return nr;
+}
+
+__device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
+                                           double m1, double m2, double m3, double m4, int ixy1, int ixy2, Root (&out)[2])
+{
+    const double E3 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(k3[0], k3[0]), __dmul_rn(k3[1], k3[1])), __dmul_rn(k3[2], k3[2])), m3));
+    const double Ep = __dsqrt_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2])), m4));
+    return paper_roots_core(g, p, k3, k1x, k1y, m1, m2, m3, m4, E3, Ep, ixy1, ixy2, out);
 }
 
 __device__ __forceinline__ void red_add(double* dst, double v)
@@ -260,37 +282,127 @@ __global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams 
     }
 }
 
-// ---- warp-cooperative version (the one bz_collision_paper launches) ------------------------------------------------
-// Only 0.14-0.16 roots per mass tuple survive the box test, so in the thread-per-sample kernel above a warp walks the
-// channel loop of every tuple with 6 of 32 lanes active (ncu).  Here the lanes of a warp still own one sample each for
-// the root solving, but every surviving root is then worked off by the WHOLE warp: the owner publishes the root's
-// |M|^2 values and cells in shared memory, lanes 0..27 gather the 4 x S occupation numbers, the 32 lanes take the
-// channels of the tuple 32 at a time, each adding its deposits to a private column of a [28][33] shared array, and
-// lanes 0..27 sum the rows and issue one RED per non-zero (slot, species).  A warp never spans two spatial cells, so
-// the loop over mass tuples is warp-uniform.
-constexpr int kCoopWarps = 4;
-struct CoopShared {
-    double M[14];              // |M|^2 x weight by 2 * kind + crossed
-    int cells[4];
-    double fv[28];             // f_a at the four cells, [slot * 7 + a]
-    double acc[28][33];        // deposits, one column per lane
+// ---- the kernel bz_collision_paper launches ------------------------------------------------------------------------
+// Only 0.14-0.16 roots per mass tuple survive the box test.  History: a thread-per-sample kernel walked the channel loop of
+// every tuple with 6 of 32 lanes active; a warp-cooperative version (the owner of a surviving root publishes it, the
+// whole warp works its channels off) fixed that for the massless case (one tuple, 127 channels) but with four distinct
+// masses a tuple has ~3 channels, so 29 lanes idled and every root cost a shared-memory column reduction: 0.010 of the
+// FP64 peak on config 4 (ncu: 16 of 32 lanes active, 23 % occupancy).  Here the two phases are decoupled through a queue:
+//   solve    lanes = samples, warp-uniform loop over the distinct mass tuples of the spatial cell; E3 and Ep are computed
+//            once per mass class (4 + 4 square roots per sample instead of 2 per tuple); every surviving root is appended
+//            to the warp's ring of 64 records in shared memory (ballot + prefix): cells of k1, k2, k3, p, (s, t, u),
+//            |J| E1 E2 E3 Ep and the bit mask of the channel groups that share the tuple.
+//   deposit  whenever the ring holds 32 records: lanes = roots; Table I at the root's massive s, t, u, then the lane
+//            walks the channels of its tuple: 4 loads, the bracket of Eq. 5, 4 reductions (RED.E.ADD.F64) per channel.
+constexpr int kQWarps = 8, kQRing = 64;
+struct QWarp {
+    unsigned cell[4][kQRing];          // k1, k2, k3, p
+    double s[kQRing], t[kQRing], u[kQRing], w_inv[kQRing];
+    unsigned long long groups[kQRing]; // bit g: channel group g belongs to the record's (canonical) mass tuple
+    unsigned long long gmask[64];      // per channel group of the current spatial cell: the groups with the same canonical tuple
 };
 
-__global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const PaperParams P)
+template <bool kAllMassless>
+__device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
 {
-    __shared__ CoopShared sh_all[kCoopWarps];
-    CoopShared& sh = sh_all[threadIdx.x >> 5];
+    if (lane >= nb) return;
+    const int r = (head + lane) & (kQRing - 1);
+    const double w = P.Kp / q.w_inv[r];
+    MsqSet M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
+    if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+    const double mv[14] = { M.a_t, M.a_u, M.m11, M.m11, M.m1b_t, M.m1b_u, M.ann, M.ann, M.qqgg, M.qqgg, M.qg_t, M.qg_u, M.gg, M.gg };
+    const unsigned c1 = q.cell[0][r], c2 = q.cell[1][r], c3 = q.cell[2][r], c4 = q.cell[3][r];
+    const double* fx = P.f + (size_t)xcell * P.S * P.Np;
+    double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+    if constexpr (kAllMassless) {
+        // every mass is zero (no bz_thermal_masses / bz_set_masses call yet): one tuple, the root serves ALL channels, and their sum
+        // is the hot path's factorised algebra (bz_channels.cuh) on the four cells -- 4 x S loads and reductions per root
+        // instead of 4 per channel.  (A separate instantiation: inlined into the general kernel it cost that one 40 %.)
+        double fv[4][7], d[4][7];
+#pragma unroll
+        for (int id = 0; id < 7; ++id) {
+            const int a = P.slot[id];
+            fv[0][id] = a >= 0 ? fx[(size_t)a * P.Np + c1] : 0.0; fv[1][id] = a >= 0 ? fx[(size_t)a * P.Np + c2] : 0.0;
+            fv[2][id] = a >= 0 ? fx[(size_t)a * P.Np + c3] : 0.0; fv[3][id] = a >= 0 ? fx[(size_t)a * P.Np + c4] : 0.0;
+        }
+        deposit<-1>(P.mask, fv[0], fv[1], fv[2], fv[3], M, d[0], d[1], d[2], d[3]);
+#pragma unroll
+        for (int id = 0; id < 7; ++id) {
+            const int a = P.slot[id];
+            if (a < 0) continue;
+            if (d[0][id] != 0.0) red_add(dx + (size_t)a * P.Np + c1, d[0][id]);
+            if (d[1][id] != 0.0) red_add(dx + (size_t)a * P.Np + c2, d[1][id]);
+            if (d[2][id] != 0.0) red_add(dx + (size_t)a * P.Np + c3, d[2][id]);
+            if (d[3][id] != 0.0) red_add(dx + (size_t)a * P.Np + c4, d[3][id]);
+        }
+        return;
+    }
+    for (unsigned long long left = q.groups[r]; left; left &= left - 1ull) {
+        const PaperGroup G = P.groups[__ffsll((long long)left) - 1];
+        for (int c = G.begin; c < G.end; ++c) {
+            const PaperChannel ch = P.table[c];
+            const double fa = fx[(size_t)ch.a * P.Np + c1], fb = fx[(size_t)ch.b * P.Np + c2];
+            const double fc = fx[(size_t)ch.c * P.Np + c3], fd = fx[(size_t)ch.d * P.Np + c4];
+            const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
+            const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
+            const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
+            // mv is indexed at run time: a 14-way select keeps it in registers
+            double Mv = mv[0];
+            const int mi = 2 * ch.kind + ch.crossed;
+#pragma unroll
+            for (int k = 1; k < 14; ++k) Mv = mi == k ? mv[k] : Mv;
+            const double A = Mv * fwd;
+            if (A != 0.0) {
+                red_add(dx + (size_t)ch.a * P.Np + c1, -A); red_add(dx + (size_t)ch.b * P.Np + c2, -A);   // Eq. 22
+                red_add(dx + (size_t)ch.c * P.Np + c3, A);  red_add(dx + (size_t)ch.d * P.Np + c4, A);
+            }
+        }
+    }
+}
+
+template <bool kAllMassless>
+__global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperParams P)
+{
+    __shared__ QWarp sh_all[kQWarps];
+    QWarp& q = sh_all[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
-    const unsigned full = 0xffffffffu;
+    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
     const long long per_x = (long long)P.p_count * P.Ns;
     const long long chunks_per_x = (per_x + 31) / 32;
     const long long n_items = chunks_per_x * P.x_count;
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
-#pragma unroll
-    for (int k = 0; k < 28; ++k) sh.acc[k][lane] = 0.0;       // kept all-zero between roots: a reducer re-zeroes its row
-    __syncwarp();
+    int head = 0, count = 0, cur_x = -1;
+    unsigned rep = 0u;
+    double mreg = 0.0;
     for (long long item = warp0; item < n_items; item += n_warps) {
         const int xcell = P.x_begin + (int)(item / chunks_per_x);
+        const double* m = P.mass2 + 4 * (size_t)xcell;
+        if (xcell != cur_x) {                              // warp-uniform: a warp's items are consecutive
+            // records never mix spatial cells: flush what the previous cell left
+            while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
+            __syncwarp();
+            cur_x = xcell;
+            mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
+            // classes with bit-identical masses share their roots: every class is mapped to the first class with its mass
+            rep = 0u;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                int rc = c;
+                for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rc = c2;
+                rep |= (unsigned)rc << (2 * c);
+            }
+            auto rp0 = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
+            auto canon0 = [&](int key) { return rp0(key & 3) | rp0((key >> 2) & 3) << 2 | rp0((key >> 4) & 3) << 4 | rp0((key >> 6) & 3) << 6; };
+            for (int g0 = lane; g0 < P.n_groups; g0 += 32) {
+                const int ck = canon0(P.groups[g0].key);
+                unsigned long long mk = 0ull;
+                for (int g1 = 0; g1 < P.n_groups; ++g1) if (canon0(P.groups[g1].key) == ck) mk |= 1ull << g1;
+                q.gmask[g0] = mk;
+            }
+            __syncwarp();
+        }
+        auto rp = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
+        auto canon = [&](int key) { return rp(key & 3) | rp((key >> 2) & 3) << 2 | rp((key >> 4) & 3) << 4 | rp((key >> 6) & 3) << 6; };
         const long long local = (item % chunks_per_x) * 32 + lane;
         const bool valid = local < per_x;
         const long long lc = valid ? local : per_x - 1;
@@ -319,80 +431,40 @@ __global__ void __launch_bounds__(32 * kCoopWarps) paper_coop_kernel(const Paper
             ixy1 = a1 + P.g.n * b1; ixy2 = a2 + P.g.n * b2;
             live = valid && i3 >= 0 && ia && ib && ic && id;
         }
-        const double* m = P.mass2 + 4 * (size_t)xcell;
-        const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
-        const double* fx = P.f + (size_t)xcell * P.S * P.Np;
-        double* dx = P.dN + (size_t)xcell * P.S * P.Np;
-        unsigned rep = 0u;                                 // 2 bits per class: the first class with the same mass
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            int rc = c;
-            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rc = c2;
-            rep |= (unsigned)rc << (2 * c);
-        }
-        auto rp = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
-        auto canon = [&](int key) { return rp(key & 3) | rp((key >> 2) & 3) << 2 | rp((key >> 4) & 3) << 4 | rp((key >> 6) & 3) << 6; };
-        unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
+        if (!__any_sync(full, live)) continue;
+        // energies of the outgoing legs, once per mass class (the roots of a tuple take E3 of its third, Ep of its fourth class)
+        const PaperLegs L(p, k3, m);
+        unsigned long long done_lo = 0ull, done_hi = 0ull, done_2 = 0ull, done_3 = 0ull;   // canonical keys already solved (256 bits)
         for (int gi = 0; gi < P.n_groups; ++gi) {                          // warp-uniform: one spatial cell per warp
             const int ck = canon(P.groups[gi].key);
-            if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
-            done[ck >> 5] |= 1u << (ck & 31);
-            // this lane's channels of the tuple (c = lane + 32 k), found once per tuple, not once per root
-            unsigned mine = 0u;
-            for (int k = 0; lane + 32 * k < P.n_channels && k < 8; ++k)
-                if (canon(P.table[lane + 32 * k].key) == ck) mine |= 1u << k;
+            unsigned long long& dw = ck < 64 ? done_lo : (ck < 128 ? done_hi : (ck < 192 ? done_2 : done_3));
+            if ((dw >> (ck & 63)) & 1ull) continue;
+            dw |= 1ull << (ck & 63);
             Root rt[2];
-            const int nr = live ? paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], ixy1, ixy2, rt) : 0;
+            const int nr = live ? paper_roots_core(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), ixy1, ixy2, rt) : 0;
+            const unsigned long long gm = q.gmask[gi];
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
-                unsigned owners = __ballot_sync(full, r < nr);
-                if (!owners) continue;
-                MsqSet M = {};
-                if (r < nr) {                                              // the owners, in parallel
-                    const double w = P.Kp / rt[r].w_inv;
-                    M = msq_set<true, true>(rt[r].s, rt[r].t, rt[r].u, mreg, P.g4 * w);
-                    if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+                const unsigned has = __ballot_sync(full, r < nr);
+                if (!has) continue;
+                if (r < nr) {
+                    const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
+                    q.cell[0][w] = (unsigned)rt[r].i1; q.cell[1][w] = (unsigned)rt[r].i2; q.cell[2][w] = (unsigned)i3; q.cell[3][w] = (unsigned)i;
+                    q.s[w] = rt[r].s; q.t[w] = rt[r].t; q.u[w] = rt[r].u; q.w_inv[w] = rt[r].w_inv;
+                    q.groups[w] = gm;
                 }
-                while (owners) {
-                    const int L = __ffs(owners) - 1;
-                    owners &= owners - 1;
-                    if (lane == L) {
-                        sh.M[0] = M.a_t; sh.M[1] = M.a_u; sh.M[2] = M.m11; sh.M[3] = M.m11; sh.M[4] = M.m1b_t; sh.M[5] = M.m1b_u;
-                        sh.M[6] = M.ann; sh.M[7] = M.ann; sh.M[8] = M.qqgg; sh.M[9] = M.qqgg; sh.M[10] = M.qg_t; sh.M[11] = M.qg_u;
-                        sh.M[12] = M.gg; sh.M[13] = M.gg;
-                        sh.cells[0] = rt[r].i1; sh.cells[1] = rt[r].i2; sh.cells[2] = i3; sh.cells[3] = i;
-                    }
-                    __syncwarp();
-                    if (lane < 28) {
-                        const int a = lane % 7;
-                        sh.fv[lane] = a < P.S ? fx[(size_t)a * P.Np + sh.cells[lane / 7]] : 0.0;
-                    }
-                    __syncwarp();
-                    unsigned rows = 0u;                        // rows of sh.acc this lane touches
-                    for (unsigned left = mine; left; left &= left - 1u) {
-                        const PaperChannel ch = P.table[lane + 32 * (__ffs(left) - 1)];
-                        rows |= 1u << ch.a | 1u << (7 + ch.b) | 1u << (14 + ch.c) | 1u << (21 + ch.d);
-                        const double fa = sh.fv[ch.a], fb = sh.fv[7 + ch.b], fc = sh.fv[14 + ch.c], fd = sh.fv[21 + ch.d];
-                        const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
-                        const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
-                        const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-                        const double A = sh.M[2 * ch.kind + ch.crossed] * fwd;
-                        sh.acc[ch.a][lane] -= A; sh.acc[7 + ch.b][lane] -= A;                 // Eq. 22
-                        sh.acc[14 + ch.c][lane] += A; sh.acc[21 + ch.d][lane] += A;
-                    }
-                    rows = __reduce_or_sync(full, rows);
-                    __syncwarp();
-                    if ((rows >> lane) & 1u) {                 // lane < 28: sum the row, re-zero it, one reduction
-                        double v = 0.0;
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) { v += sh.acc[lane][j]; sh.acc[lane][j] = 0.0; }
-                        if (v != 0.0) red_add(dx + (size_t)(lane % 7) * P.Np + sh.cells[lane / 7], v);
-                    }
+                count += __popc(has);
+                __syncwarp();
+                if (count >= 32) {
+                    paper_deposit_batch<kAllMassless>(P, q, lane, head, 32, xcell, mreg);
+                    head = (head + 32) & (kQRing - 1);
+                    count -= 32;
                     __syncwarp();
                 }
             }
         }
     }
+    while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
 }
 
 __global__ void __launch_bounds__(256) paper_finalize_kernel(double* __restrict__ dF, size_t n_values, int S, int Np, const double d0,
@@ -424,12 +496,15 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
+    if (P.n_groups > 64) return cudaErrorInvalidValue;       // the records carry a 64-bit mask of channel groups (7 species: 40)
     int per_sm = 1;                      // only the CTAs resident at once: the warps in flight stay within a few spatial cells
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_coop_kernel, 32 * kCoopWarps, 0);
+    if (P.all_massless) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<true>, 32 * kQWarps, 0);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<false>, 32 * kQWarps, 0);
     if (per_sm < 1) per_sm = 1;
-    long long blocks = (total / 32 + kCoopWarps) / kCoopWarps;
+    long long blocks = (total / 32 + kQWarps) / kQWarps;
     if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
-    paper_coop_kernel<<<(int)blocks, 32 * kCoopWarps, 0, st>>>(P);
+    if (P.all_massless) paper_queue_kernel<true><<<(int)blocks, 32 * kQWarps, 0, st>>>(P);
+    else paper_queue_kernel<false><<<(int)blocks, 32 * kQWarps, 0, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }
