@@ -135,7 +135,7 @@ def vlasov_probe(g, cfg, dev, reps=5):
     # per value: 8 B f read + 8 B dF written + the energy table written once and read once, 8 B per (cell, mass class)
     bytes_per_value = 16.0 + 16.0 * n_cls / cfg.S
     rate = cfg.n_values / (ms_vl * 1e-3)
-    return {"kernels": "energy_kernel + vlasov_kernel (bz_vlasov), mass_kernel (bz_thermal_masses)", "bound": "hbm",
+    return {"kernels": "energy_kernel + vlasov_class_kernel (bz_vlasov), mass_kernel (bz_thermal_masses)", "bound": "hbm",
             "ms_vlasov": ms_vl, "ms_thermal_masses": ms_mass, "cell_updates_per_sec": rate, "bytes_per_value": bytes_per_value,
             "achieved": rate * bytes_per_value / 1e9, "unit": "GB/s"}
 

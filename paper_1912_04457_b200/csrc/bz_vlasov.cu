@@ -1,7 +1,7 @@
 // bz_vlasov.cu -- NEXT rank 2 of SURVEY.md 8f: the paper's own left-hand side.
 //   mass_kernel    thermal masses^2 per spatial cell, Eq. 8-9, with E_p^a = sqrt(p^2 + m_a^2) from the
 //                  masses of the previous evaluation (0 at start = the first-step prescription E_p = |p|)
-//   vlasov_kernel  dF = -dt { drift + force } of Eq. 15: central differences in x and in p, periodic in both
+//   vlasov_class_kernel  dF = -dt { drift + force } of Eq. 15: central differences in x and in p, periodic in both
 //                  (P:139).  In bz_step the increment lands in f_new and transport_kernel<2> adds f and the collision
 //                  deposits (forward Euler, Eq. 15 solved for f(t + dt)).
 //   energy_kernel  E_p^a(x) table for the mass classes present (one square root per entry instead of 18 per value).
@@ -119,13 +119,6 @@ struct VlasovParams {
     unsigned cls_bits;
 };
 
-// One thread per phase-space value (x, a, pc): 12 f reads + 18 energy reads, all independent, < 64 registers; the
-// latency of the scattered neighbour reads is hidden by warps, not by unrolling.  blockIdx.x = spatial cell (fastest):
-// the blocks in flight share one (species, 256-cell momentum chunk) slice of all spatial cells, so the six spatial
-// neighbours are L2 hits.  The first version spent 730 instructions per value, most of them integer divisions by the
-// run-time grid sizes and IEEE fp64 divisions (ncu: issue-bound at 74 %); the periodic wrap now comes from two small
-// tables built once per context (x_nb: neighbour cell offsets per spatial cell, p_wrap: one flag byte per momentum
-// cell) and p_i / E from a Newton reciprocal.
 __device__ __forceinline__ double rcp_newton(double x)
 {
     double y;
@@ -136,44 +129,96 @@ __device__ __forceinline__ double rcp_newton(double x)
     return fma(y, e, y);
 }
 
-__global__ void __launch_bounds__(256) vlasov_kernel(const VlasovParams V)
+// ---- the stencil kernel bz_vlasov launches -----------------------------------------------------------------------------
+// One thread per (spatial cell, mass class, momentum cell); blockIdx.x = spatial cell (fastest): the blocks in flight share
+// one (class, 256-cell momentum chunk) slice of all spatial cells, so the six spatial neighbours are L2 hits; a block walks
+// chunks_per_block consecutive chunks (about 8 p_z planes) so that the +-n^2 momentum neighbours are still in L2 when they
+// are touched again.  The periodic wraps come from two small tables built once per context (x_nb: neighbour cell offsets
+// per spatial cell, p_wrap: one flag byte per momentum cell), p_i / E from a Newton reciprocal.
+// History (config 4): the round-1 kernel, one thread per value and SPECIES, issued 30 global loads per value (12 of f, 18 of
+// the energy table) and sat at 90 % of the L1 data pipe (5.7 ms with the energy table).  Two restructurings were measured
+// slower:
+// staging every energy and f plane in shared memory, one block per (spatial cell, mass class) sweeping the p_z planes
+// (12.1 ms: an 8-byte LDS of a warp costs the same two wavefronts of that pipe as an 8-byte LDG, and the block-wide syncs
+// per plane expose the load latency), and one thread per (p_x, p_y) column walking p_z with register windows (15.7 ms: 156
+// registers, 8 warps per SM).  What is kept is what needs neither: one thread per value, but the thread serves
+// ALL species of its mass class (q and qbar share the 18 energies) and takes the p_x neighbours -- of f and of the energy
+// difference E(x + e_x) - E(x - e_x) -- from the neighbouring lanes by warp shuffles (lanes at the ends of a p_x row or of
+// the warp load theirs): 14 energy loads per class and 11 f loads per species, 19 per value for the mixture instead of 30
+// -- which bought 2 % (5.59 ms): with the L1 pipe relieved the kernel is bound by the L2 -> L1 traffic of its scattered
+// 8-byte neighbour loads; the next step would be the plane sweep again, software-pipelined instead of block-synchronous.
+__global__ void __launch_bounds__(256) vlasov_class_kernel(const VlasovParams V)
 {
-    const int xcell = blockIdx.x, a = blockIdx.z;
-    // a block walks V.chunks_per_block consecutive 256-cell chunks (about 8 p_z planes): the +-n^2 momentum neighbours of
-    // a chunk are then touched again by the same block a few iterations later instead of 2.25 x Nx blocks later, i.e.
-    // they are still in L2 (ncu on the one-chunk version: 3 x the compulsory DRAM reads)
-    for (int ch = 0; ch < V.chunks_per_block; ++ch) {
-    const int pc = (blockIdx.y * V.chunks_per_block + ch) * blockDim.x + threadIdx.x;
-    if (pc >= V.Np) return;
-    const int n = V.n;
-    const int cls = class_of(V.cls_bits, a);
-    const size_t row = (size_t)V.S * V.Np;
-    const double* fx = V.f + (size_t)xcell * row + (size_t)a * V.Np + pc;
-    const double* Ex = V.E_tab + ((size_t)xcell * 4 + cls) * V.Np + pc;
-    const unsigned wrap = V.p_wrap[pc];                      // bit 2d: p - dp e_d wraps, bit 2d + 1: p + dp e_d wraps
-    const int* xnb = V.x_nb + 6 * (size_t)xcell;             // cell index offsets of x -+ dx e_d (periodic)
-    int pstr = 1;
-    double acc = 0.0;
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        const int pom = ((wrap >> (2 * d)) & 1u) ? (n - 1) * pstr : -pstr;       // periodic in p
-        const int pop = ((wrap >> (2 * d + 1)) & 1u) ? -(n - 1) * pstr : pstr;
-        pstr *= n;
-        const double pd = __ldg(V.cell_tab + 4 * (size_t)pc + d);
-        const ptrdiff_t om = __ldg(xnb + 2 * d), op = __ldg(xnb + 2 * d + 1);
-        const double* Em = Ex + om * 4 * V.Np;               // energies at x - dx e_d
-        const double* Ep = Ex + op * 4 * V.Np;               // energies at x + dx e_d
-        const double Exp = __ldg(Ep), Exm = __ldg(Em);
-        const double cp = Exp > 0.0 ? pd * rcp_newton(Exp) : 0.0, cm = Exm > 0.0 ? pd * rcp_newton(Exm) : 0.0;   // S10
-        const double Gp = (__ldg(Ep + pop) - __ldg(Em + pop)) * V.inv_2dx;       // dE/dx at p + dp e_d
-        const double Gm = (__ldg(Ep + pom) - __ldg(Em + pom)) * V.inv_2dx;       // dE/dx at p - dp e_d
-        const double fxm = __ldg(fx + om * (ptrdiff_t)row), fxp = __ldg(fx + op * (ptrdiff_t)row);
-        const double fpm = __ldg(fx + pom), fpp = __ldg(fx + pop);
-        const double drift = (cp * fxp - cm * fxm) * V.inv_2dx;
-        const double force = -(fpp * Gp - fpm * Gm) * V.inv_2dp;
-        acc += drift + force;
+    const int xcell = blockIdx.x;
+    int cls = -1;                                            // the blockIdx.z-th mass class present
+    {
+        unsigned present = 0;
+        for (int a = 0; a < V.S; ++a) present |= 1u << class_of(V.cls_bits, a);
+        int k = blockIdx.z;
+        for (int c = 0; c < 4; ++c) if ((present >> c) & 1u) { if (k == 0) { cls = c; break; } --k; }
     }
-    V.out[(size_t)xcell * row + (size_t)a * V.Np + pc] = -V.dt * acc;
+    if (cls < 0) return;
+    int sp[2] = { 0, 0 }, nsp = 0;                           // the species (layout indices) of the class: q and qbar, or g
+    for (int a = 0; a < V.S; ++a) if (class_of(V.cls_bits, a) == cls && nsp < 2) sp[nsp++] = a;
+    const int lane = threadIdx.x & 31, n = V.n;
+    const size_t row = (size_t)V.S * V.Np;
+    const int* xnb = V.x_nb + 6 * (size_t)xcell;             // cell index offsets of x -+ dx e_d (periodic)
+    const double* Ex = V.E_tab + ((size_t)xcell * 4 + cls) * V.Np;
+    for (int ch = 0; ch < V.chunks_per_block; ++ch) {
+        const int pc_raw = (blockIdx.y * V.chunks_per_block + ch) * blockDim.x + threadIdx.x;
+        if (pc_raw - lane >= V.Np) return;                   // the whole warp is past the end
+        const bool on = pc_raw < V.Np;
+        const int pc = on ? pc_raw : V.Np - 1;
+        const unsigned wrap = V.p_wrap[pc];                  // bit 2d: p - dp e_d wraps, bit 2d + 1: p + dp e_d wraps
+        // p_x neighbours from the lanes next door, except at the ends of a p_x row and of the warp
+        const bool ld_m = lane == 0 || (wrap & 1u) || !on, ld_p = lane == 31 || (wrap & 2u) || pc_raw + 1 >= V.Np;
+        double acc[2] = { 0.0, 0.0 };
+        int pstr = 1;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int pom = ((wrap >> (2 * d)) & 1u) ? (n - 1) * pstr : -pstr;       // periodic in p
+            const int pop = ((wrap >> (2 * d + 1)) & 1u) ? -(n - 1) * pstr : pstr;
+            pstr *= n;
+            const double pd = __ldg(V.cell_tab + 4 * (size_t)pc + d);
+            const ptrdiff_t om = __ldg(xnb + 2 * d), op = __ldg(xnb + 2 * d + 1);
+            const double* Em = Ex + pc + om * 4 * V.Np;      // energies at x - dx e_d
+            const double* Ep = Ex + pc + op * 4 * V.Np;      // energies at x + dx e_d
+            const double Exp = __ldg(Ep), Exm = __ldg(Em);
+            const double cp = Exp > 0.0 ? pd * rcp_newton(Exp) : 0.0, cm = Exm > 0.0 ? pd * rcp_newton(Exm) : 0.0;   // S10
+            double Gp, Gm;
+            if (d == 0) {
+                const double dE = Exp - Exm;
+                Gp = __shfl_sync(0xffffffffu, dE, (lane + 1) & 31); Gm = __shfl_sync(0xffffffffu, dE, (lane + 31) & 31);
+                if (ld_p) Gp = __ldg(Ep + pop) - __ldg(Em + pop);
+                if (ld_m) Gm = __ldg(Ep + pom) - __ldg(Em + pom);
+                Gp *= V.inv_2dx; Gm *= V.inv_2dx;
+            } else {
+                Gp = (__ldg(Ep + pop) - __ldg(Em + pop)) * V.inv_2dx;       // dE/dx at p + dp e_d
+                Gm = (__ldg(Ep + pom) - __ldg(Em + pom)) * V.inv_2dx;       // dE/dx at p - dp e_d
+            }
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                if (s < nsp) {
+                    const double* fx = V.f + (size_t)xcell * row + (size_t)sp[s] * V.Np + pc;
+                    const double fxm = __ldg(fx + om * (ptrdiff_t)row), fxp = __ldg(fx + op * (ptrdiff_t)row);
+                    double fpm, fpp;
+                    if (d == 0) {
+                        const double f0 = __ldg(fx);
+                        fpp = __shfl_sync(0xffffffffu, f0, (lane + 1) & 31); fpm = __shfl_sync(0xffffffffu, f0, (lane + 31) & 31);
+                        if (ld_p) fpp = __ldg(fx + pop);
+                        if (ld_m) fpm = __ldg(fx + pom);
+                    } else {
+                        fpm = __ldg(fx + pom); fpp = __ldg(fx + pop);
+                    }
+                    const double drift = (cp * fxp - cm * fxm) * V.inv_2dx;
+                    const double force = -(fpp * Gp - fpm * Gm) * V.inv_2dp;
+                    acc[s] += drift + force;
+                }
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+            if (s < nsp && on) V.out[(size_t)xcell * row + (size_t)sp[s] * V.Np + pc] = -V.dt * acc[s];
     }
 }
 
@@ -213,7 +258,9 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
     V.chunks_per_block = (8 * n * n + 255) / 256;
     if (V.chunks_per_block > chunks) V.chunks_per_block = chunks;
     const int groups = (chunks + V.chunks_per_block - 1) / V.chunks_per_block;
-    vlasov_kernel<<<dim3(nx * ny * nz, groups, S), 256, 0, st>>>(V);
+    int n_cls = 0;
+    for (int c = 0; c < 4; ++c) n_cls += (present >> c) & 1u;
+    vlasov_class_kernel<<<dim3(nx * ny * nz, groups, n_cls), 256, 0, st>>>(V);
     ++g_launch_count;
     return cudaGetLastError();
 }
