@@ -23,7 +23,7 @@ def _nvcc():
 def _deps():
     out = [os.path.join(HERE, "..", "include", "bz.h")]
     for name in os.listdir(CSRC):
-        if not name.startswith("bz_testhooks"):
+        if not name.startswith("bz_testhooks") and not name.startswith("bz_scatter_probe"):
             out.append(os.path.join(CSRC, name))
     return out
 
@@ -50,5 +50,17 @@ def build_testhooks(force=False):
     return TESTHOOKS_LIB
 
 
+def build_scatter_probe():
+    """The scatter-design measurement tool (csrc/bz_scatter_probe.cu -> bz_scatter_probe, a stand-alone executable; not part
+    of libbz.so): profiles/r2_scatter_variants.md keeps its output."""
+    out = os.path.join(HERE, "bz_scatter_probe")
+    subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+                    os.path.join(CSRC, "bz_scatter_probe.cu"), "-o", out], check=True, cwd=CSRC)
+    return out
+
+
 if __name__ == "__main__":
+    if "scatter_probe" in sys.argv:
+        print(build_scatter_probe())
+        sys.exit(0)
     print(build(force=True, verbose="-v" in sys.argv))
