@@ -101,6 +101,8 @@ struct PaperLegs {
     __device__ __forceinline__ double ep(int c) const { return c == 0 ? Ep[0] : (c == 1 ? Ep[1] : (c == 2 ? Ep[2] : Ep[3])); }
 };
 
+// Returns a bit mask: bit 0 = the + root is kept (out[0]), bit 1 = the - root (out[1]): no run-time index into out, so the two
+// roots stay in registers.
 __device__ __forceinline__ int paper_roots_core(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
                                                 double m1, double m2, double m3, double m4, double E3, double Ep, int ixy1, int ixy2,
                                                 Root (&out)[2])
@@ -138,7 +140,8 @@ __device__ __forceinline__ int paper_roots_core(const GridConst& g, const double
         if (!(E1 > 0.0 && E2 > 0.0)) continue;
         const double J = SUB(__ddiv_rn(z, E1), __ddiv_rn(k2z, E2));          // Eq. 19
         if (J == 0.0) continue;
-        Root& r = out[nr++];
+        Root& r = out[sign];
+        nr |= 1 << sign;
         r.i1 = i1; r.i2 = i2;
         r.w_inv = fabs(J) * (((E1 * E2) * E3) * Ep);
         r.s = SUB(Et2, ADD(ADD(MUL(Px, Px), MUL(Py, Py)), Pz2));
@@ -156,7 +159,9 @@ __device__ __forceinline__ int paper_roots(const GridConst& g, const double (&p)
 {
     const double E3 = __dsqrt_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(k3[0], k3[0]), __dmul_rn(k3[1], k3[1])), __dmul_rn(k3[2], k3[2])), m3));
     const double Ep = __dsqrt_rn(__dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(p[0], p[0]), __dmul_rn(p[1], p[1])), __dmul_rn(p[2], p[2])), m4));
-    return paper_roots_core(g, p, k3, k1x, k1y, m1, m2, m3, m4, E3, Ep, ixy1, ixy2, out);
+    const int kept = paper_roots_core(g, p, k3, k1x, k1y, m1, m2, m3, m4, E3, Ep, ixy1, ixy2, out);
+    if (kept == 2) out[0] = out[1];                       // the oracle's order: +, then -
+    return kept == 3 ? 2 : (kept ? 1 : 0);
 }
 
 __device__ __forceinline__ void red_add(double* dst, double v)
@@ -437,17 +442,20 @@ __global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperPa
         unsigned long long done_lo = 0ull, done_hi = 0ull, done_2 = 0ull, done_3 = 0ull;   // canonical keys already solved (256 bits)
         for (int gi = 0; gi < P.n_groups; ++gi) {                          // warp-uniform: one spatial cell per warp
             const int ck = canon(P.groups[gi].key);
-            unsigned long long& dw = ck < 64 ? done_lo : (ck < 128 ? done_hi : (ck < 192 ? done_2 : done_3));
-            if ((dw >> (ck & 63)) & 1ull) continue;
-            dw |= 1ull << (ck & 63);
+            const unsigned long long bit = 1ull << (ck & 63);
+            const int wsel = ck >> 6;
+            const unsigned long long dw = wsel == 0 ? done_lo : (wsel == 1 ? done_hi : (wsel == 2 ? done_2 : done_3));
+            if (dw & bit) continue;
+            if (wsel == 0) done_lo |= bit; else if (wsel == 1) done_hi |= bit; else if (wsel == 2) done_2 |= bit; else done_3 |= bit;
             Root rt[2];
-            const int nr = live ? paper_roots_core(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), ixy1, ixy2, rt) : 0;
+            const int kept = live ? paper_roots_core(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), ixy1, ixy2, rt) : 0;
             const unsigned long long gm = q.gmask[gi];
 #pragma unroll
             for (int r = 0; r < 2; ++r) {
-                const unsigned has = __ballot_sync(full, r < nr);
+                const bool mine = (kept >> r) & 1;
+                const unsigned has = __ballot_sync(full, mine);
                 if (!has) continue;
-                if (r < nr) {
+                if (mine) {
                     const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
                     q.cell[0][w] = (unsigned)rt[r].i1; q.cell[1][w] = (unsigned)rt[r].i2; q.cell[2][w] = (unsigned)i3; q.cell[3][w] = (unsigned)i;
                     q.s[w] = rt[r].s; q.t[w] = rt[r].t; q.u[w] = rt[r].u; q.w_inv[w] = rt[r].w_inv;
