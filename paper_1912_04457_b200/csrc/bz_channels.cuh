@@ -244,15 +244,16 @@ BZ_HD void deposit(unsigned rt_mask, const double (&fi)[7], const double (&fj)[7
 #undef BZ_ON
 }
 
-// ---- the same algebra split into its gain and its loss half ------------------------------------------------------------
-// Every channel's bracket is  f_a(i) f_b(j) F_c(k) F_d(l)  -  F_a(i) F_b(j) f_c(k) f_d(l)  (Eq. 5): a "gain" product
-// and a "loss" product of the same shape with f and F = 1 +- f exchanged.  deposit_half evaluates ONE of the two for all
-// channels: P holds the incoming-side factors at the cells i, j (f for the gain half, F for the loss half), Q the
-// outgoing-side factors at k, l (F for the gain half, f for the loss half), and the caller passes the |M|^2 set with its
-// sign (+ gain, - loss), so that the half's deposits are -H, -H, +H, +H like the whole bracket's (Eq. 22).  The collision
-// kernel gives the two halves of a sample to two neighbouring lanes (half the registers per lane, the same instruction
-// stream for both) and adds the two sets of deposits when it flushes them; each half's deposits cancel exactly by
-// themselves, so particle number is conserved as before.  Entries of inactive species must be 0 in P and in Q.
+// ---- the same algebra, one half of the bracket at a time ---------------------------------------------------------------
+// Every channel's bracket is  f_a(i) f_b(j) F_c(k) F_d(l)  -  F_a(i) F_b(j) f_c(k) f_d(l)  (Eq. 5).  deposit_half
+// evaluates the GAIN product of all channels: P holds the incoming-side factors f at the cells (i, j), Q the outgoing-side
+// factors F = 1 +- f at (k, l); its deposits are -H, -H at (i, j) and +H, +H at (k, l) (Eq. 22).  The LOSS product of a
+// channel a b -> c d is the gain product of the time-reversed channel c d -> a b on the cells (k, l | i, j) -- same s, t,
+// u, same |M|^2, and the channel table is closed under time reversal (S8c step 5) -- so the loss half of all channels is
+// deposit_half called with the two pairs of cells exchanged.  The collision kernel gives the two halves of a sample to two
+// lanes (half the registers per lane, the same instruction stream for both) and adds the two sets of deposits when it
+// flushes them; each half's deposits cancel exactly by themselves, so particle number is conserved as before.  Entries
+// of inactive species must be 0 in P and in Q.
 template <int kMask>
 BZ_HD void deposit_half(unsigned rt_mask, const double (&Pi)[7], const double (&Pj)[7], const double (&Qk)[7],
                         const double (&Ql)[7], const MsqSet& M, double (&dI)[7], double (&dJ)[7], double (&dK)[7],
@@ -337,15 +338,6 @@ BZ_HD void deposit_half(unsigned rt_mask, const double (&Pi)[7], const double (&
         }
     }
 #undef BZ_ON
-}
-
-// the |M|^2 set with every value negated: the loss half's sign
-BZ_HD MsqSet msq_negated(const MsqSet& M)
-{
-    MsqSet N;
-    N.gg = -M.gg; N.qqgg = -M.qqgg; N.qg_t = -M.qg_t; N.qg_u = -M.qg_u; N.m11 = -M.m11; N.m1b_t = -M.m1b_t; N.m1b_u = -M.m1b_u;
-    N.ann = -M.ann; N.a_t = -M.a_t; N.a_u = -M.a_u; N.d11 = -M.d11; N.d1b_t = -M.d1b_t; N.d1b_u = -M.d1b_u;
-    return N;
 }
 
 }  // namespace bz

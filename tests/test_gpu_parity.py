@@ -814,3 +814,28 @@ def test_step_n_matches_oracle_and_step_loop(cfg, n):
     for key in ("ne", "tot", "m2"):
         a, b = np.asarray(mo[key]), mg[key].numpy()
         assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(np.abs(a), np.abs(a).max() * 1e-6)), key
+
+
+def test_slab_step_host_on_one_gpu():
+    """SlabDomain.step_host (the end-to-end leg of the slab path: boundary layers up, halo exchange, bz_step_host over the
+    own layers of a slab context) with world = 1 against the oracle on the undecomposed periodic domain."""
+    from paper_1912_04457_b200 import slab
+    cfg = wl.scaled(wl.CONFIGS[3], nx=4, np_=8, samples=16)
+    nl = cfg.nx * cfg.nx
+    o = bzo.Oracle(threads=8, **_slab_kw(cfg, cfg.nx))
+    f0 = wl.random_f(cfg, seed=29)
+    o.set_f(f0)
+    dom = slab.SlabDomain(lambda nz: bz.Boltzmann(**_slab_kw(cfg, nz)), cfg.nx, cfg.nx, cfg.nx, 0, 1)
+    f_local = np.zeros(((cfg.nx + 2) * nl, cfg.S, cfg.Np))
+    f_local[nl:-nl] = f0
+    hin = torch.from_numpy(f_local).pin_memory()
+    hout = torch.zeros_like(hin).pin_memory()
+    for _ in range(3):
+        o.step(cfg.dt)
+        dom.step_host(cfg.dt, hin, hout)
+        f_o = o.get_f()
+        got = hout.numpy()[nl:-nl]
+        assert np.abs(got - f_o).max() <= TOL_DF * np.abs(f_o).max()
+        assert not hout.numpy()[:nl].any() and not hout.numpy()[-nl:].any()      # halo layers of the host buffer are not written
+        hin.copy_(hout)
+    assert np.allclose(dom.moments_totals().numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
