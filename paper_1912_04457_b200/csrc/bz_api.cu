@@ -123,6 +123,7 @@ int run_collide(bz_ctx* c, double dt_fm, unsigned step, int sampler = 0)
         BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
         c->aos_valid = true;
     }
+    if ((long long)c->Np * ((c->Ns + 31) / 32) >= (1LL << 31)) { c->err = "collision: momentum cells x ceil(samples / 32) must stay below 2^31"; return -1; }
     CollideParams P = collide_params(c, dt_fm, step);
     P.sampler = sampler;
     BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");

@@ -281,8 +281,12 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
     constexpr int kSP = MaskTraits<kMask>::SP;
     using W = WarpMem<kSP>;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31;
-    W& wm = reinterpret_cast<W*>(smem_raw)[threadIdx.x >> 5];
+    // lane and warp through volatile asm: ptxas otherwise re-derives them from S2R SR_TID.X a dozen times per loop iteration
+    // (the special-register read is slow and sat on the critical path of gather and scatter)
+    int lane, warp;
+    asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
+    asm volatile("{\n .reg .u32 t;\n mov.u32 t, %%tid.x;\n shr.u32 %0, t, 5;\n}" : "=r"(warp));
+    W& wm = reinterpret_cast<W*>(smem_raw)[warp];
     const unsigned mask = kMask >= 0 ? (unsigned)kMask : P.mask;
     const uint32_t step = P.step_ptr ? *P.step_ptr : P.step;
 

@@ -6,10 +6,9 @@
 // With masses the kinematics depend on the species of the four legs, so a sample is NOT shared by all channels as in
 // the hot path: the ordered channels (S8c step 5) are grouped by their tuple of mass classes (g, u, d, s) and every
 // group solves its own roots.  One lane per (spatial cell, grid point, sample) for the root solving; the surviving roots
-// are worked off by the whole warp (paper_coop_kernel), their deposits summed per (slot, species) in shared memory and
-// issued as fp64 reductions (RED.E.ADD.F64) into dF, which a second kernel divides by N_a.  The thread-per-sample
-// kernel (paper_kernel) is kept for the debug export of the roots.  Everything that decides a cell index uses single correctly rounded operations in the
-// association order of the oracle (bit-exact sampled cells).
+// go through a per-warp queue to a second phase with one lane per root (paper_queue_kernel), whose deposits are issued as
+// fp64 reductions (RED.E.ADD.F64) into dF, which a second kernel divides by N_a.  Everything that decides a cell index
+// uses single correctly rounded operations in the association order of the oracle (bit-exact sampled cells).
 #include <vector>
 
 #include "bz_channels.cuh"
@@ -169,13 +168,12 @@ __device__ __forceinline__ void red_add(double* dst, double v)
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(dst), "d"(v) : "memory");
 }
 
-// mode 0: collision; mode 1: debug (writes the roots of one mass tuple instead of depositing)
+// test export: the roots of ONE mass tuple (P.dbg_msq) for every sample of cells [p_begin, p_begin + p_count) of x_begin,
+// thread per sample, the same draw and root solving as paper_queue_kernel
 constexpr int kPaperThreads = 64;
 
-template <int kDebug>
-__global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams P, int* dbg_cells, double* dbg_stu)
+__global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperParams P, int* dbg_cells, double* dbg_stu)
 {
-    __shared__ double sh_fv[28 * kPaperThreads], sh_acc[28 * kPaperThreads];
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < total; q += (long long)gridDim.x * blockDim.x) {
         const int smp = (int)(q % P.Ns);
@@ -209,7 +207,7 @@ __global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams 
             ixy1 = a1 + P.g.n * b1; ixy2 = a2 + P.g.n * b2;
             k2_in = ia && ib && ic && id;
         }
-        if (kDebug) {
+        {
             Root rt[2];
             const int nr = !k2_in ? 0 : paper_roots(P.g, p, k3, k1x, k1y, P.dbg_msq[0], P.dbg_msq[1], P.dbg_msq[2], P.dbg_msq[3], ixy1, ixy2, rt);
             int* oc = dbg_cells + 6 * q;
@@ -218,70 +216,6 @@ __global__ void __launch_bounds__(kPaperThreads) paper_kernel(const PaperParams 
             for (int r = 0; r < 2; ++r) {
                 oc[2 + 2 * r] = r < nr ? rt[r].i1 : -1; oc[3 + 2 * r] = r < nr ? rt[r].i2 : -1;
                 os[3 * r] = r < nr ? rt[r].s : 0.0; os[3 * r + 1] = r < nr ? rt[r].t : 0.0; os[3 * r + 2] = r < nr ? rt[r].u : 0.0;
-            }
-            continue;
-        }
-        if (i3 < 0 || !k2_in) continue;
-        const double mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
-        const double* fx = P.f + (size_t)xcell * P.S * P.Np;
-        double* dx = P.dN + (size_t)xcell * P.S * P.Np;
-        // Mass classes with bit-identical masses (e.g. m_u = m_d = m_s for flavour-symmetric f, or all 0) have the same
-        // roots: every class is mapped to the first class with its mass, and all groups with the same mapped tuple share
-        // one root solve, one gather of the 4 x S occupation numbers and one flush of the deposits.
-        int rep[4];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            rep[c] = c;
-            for (int c2 = c - 1; c2 >= 0; --c2) if (m[c2] == m[c]) rep[c] = c2;
-        }
-        auto canon = [&](int key) { return rep[key & 3] | rep[(key >> 2) & 3] << 2 | rep[(key >> 4) & 3] << 4 | rep[(key >> 6) & 3] << 6; };
-        // The 4 x S occupation numbers and the 4 x S deposit sums of the root being worked on live in shared memory,
-        // [entry][thread]: they are indexed by the channel table (run-time indices), which in registers would mean local
-        // memory; lanes of a warp read the same entry of consecutive threads, i.e. conflict-free.
-        double* fv = sh_fv + threadIdx.x;
-        double* acc = sh_acc + threadIdx.x;
-        unsigned done[8] = { 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u };
-        for (int gi = 0; gi < P.n_groups; ++gi) {
-            const int ck = canon(P.groups[gi].key);
-            if ((done[ck >> 5] >> (ck & 31)) & 1u) continue;
-            done[ck >> 5] |= 1u << (ck & 31);
-            Root rt[2];
-            const int nr = paper_roots(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], ixy1, ixy2, rt);
-            for (int r = 0; r < nr; ++r) {
-                const Root& R = rt[r];
-                const double w = P.Kp / R.w_inv;
-                MsqSet M = msq_set<true, true>(R.s, R.t, R.u, mreg, P.g4 * w);
-                if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
-                const double mv[10] = { M.a_t, M.a_u, M.m11, M.m11, M.m1b_t, M.m1b_u, M.ann, M.ann, M.qqgg, M.qqgg };
-                const int cell[4] = { R.i1, R.i2, i3, i };
-#pragma unroll
-                for (int sl = 0; sl < 4; ++sl)
-                    for (int a = 0; a < P.S; ++a) {
-                        fv[(sl * 7 + a) * kPaperThreads] = fx[(size_t)a * P.Np + cell[sl]];
-                        acc[(sl * 7 + a) * kPaperThreads] = 0.0;
-                    }
-                for (int gj = gi; gj < P.n_groups; ++gj) {
-                    const PaperGroup G = P.groups[gj];
-                    if (canon(G.key) != ck) continue;
-                    for (int c = G.begin; c < G.end; ++c) {
-                        const PaperChannel ch = P.table[c];
-                        const double fa = fv[ch.a * kPaperThreads], fb = fv[(7 + ch.b) * kPaperThreads];
-                        const double fc = fv[(14 + ch.c) * kPaperThreads], fd = fv[(21 + ch.d) * kPaperThreads];
-                        const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
-                        const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
-                        const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-                        const double Mv = ch.kind == 5 ? (ch.crossed ? M.qg_u : M.qg_t) : ch.kind == 6 ? M.gg : mv[2 * ch.kind + ch.crossed];
-                        const double A = Mv * fwd;
-                        acc[ch.a * kPaperThreads] -= A; acc[(7 + ch.b) * kPaperThreads] -= A;            // Eq. 22
-                        acc[(14 + ch.c) * kPaperThreads] += A; acc[(21 + ch.d) * kPaperThreads] += A;
-                    }
-                }
-#pragma unroll
-                for (int sl = 0; sl < 4; ++sl)
-                    for (int a = 0; a < P.S; ++a) {
-                        const double v = acc[(sl * 7 + a) * kPaperThreads];
-                        if (v != 0.0) red_add(dx + (size_t)a * P.Np + cell[sl], v);
-                    }
             }
         }
     }
@@ -523,7 +457,7 @@ cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, in
     if (total <= 0) return cudaSuccess;
     long long blocks = (total + kPaperThreads - 1) / kPaperThreads;
     if (blocks > (long long)sms * 32) blocks = (long long)sms * 32;
-    paper_kernel<1><<<(int)blocks, kPaperThreads, 0, st>>>(P, cells, stu);
+    paper_debug_kernel<<<(int)blocks, kPaperThreads, 0, st>>>(P, cells, stu);
     ++g_launch_count;
     return cudaGetLastError();
 }
