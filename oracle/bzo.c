@@ -22,6 +22,13 @@
  * colour/spin-averaged values and crossing relations for Table I.
  * Per-cell values of C[f] are printed nowhere in the paper: they are pinned only through
  * P4/P5/P10 (independent estimators agreeing), not by a published number.
+ * NEXT rows, each pinned in its own test file: thermal masses, Eq. 15 and the
+ * energy balance (V1-V7, test_oracle_vlasov.py); the paper's own sampler, Eq. 17-21 (R1-R5,
+ * and R6: bzo_collision_paper's grouping by mass tuple against the channel-by-channel
+ * bzo_collision_paper_plain; test_oracle_paper_sampler.py); importance-sampled t (I1-I4,
+ * test_oracle_importance.py); in-box sampling of the CM direction (B1-B5: closed-form weight,
+ * brute-force zone containment, weighted isotropy, conservation, same expectation as the
+ * uniform sampler; test_oracle_inbox.py).  No function of this file is "parity unpinned".
  */
 #include "bzo.h"
 #include <math.h>
