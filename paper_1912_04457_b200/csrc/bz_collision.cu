@@ -65,9 +65,16 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 // fp64 reduction without return value (RED.E.ADD.F64)
+#ifndef BZ_ABLATE
+#define BZ_ABLATE 0
+#endif
 __device__ __forceinline__ void red_add(double* gdst, double v)
 {
+#if BZ_ABLATE == 3
+    if (v == 1.2345e300) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gdst), "d"(v));
+#else
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gdst), "d"(v));
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------ shared memory
@@ -114,6 +121,9 @@ __device__ __forceinline__ void issue_gather(WarpMem<kSP>& wm, const double* __r
         const uint4 c0 = *reinterpret_cast<const uint4*>(cp), c1 = *reinterpret_cast<const uint4*>(cp + 4);
         const unsigned ci[8] = { c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w };
 #pragma unroll
+#if BZ_ABLATE == 4
+        if (ci[0] == 0xfffffff0u)
+#endif
         for (int k = 0; k < 8; ++k) cp_async16(dst + k * W::kStride, src + (size_t)ci[k] * 8);
     } else {
         for (int k = 0; k < 8 && sub * 8 + k < nb; ++k) cp_async16(dst + k * W::kStride, src + (size_t)cp[k] * 8);
@@ -183,11 +193,17 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
             }
         }
         const double u = __dsub_rn(-s, t);
+#if BZ_ABLATE == 2
+        MsqSet M = {}; M.gg = s; M.qqgg = t; M.qg_t = u; M.a_t = g4w; M.d11 = m2;
+#pragma unroll
+        for (int a = 0; a < 7; ++a) { d[0][a] = Pi[a] * M.gg; d[1][a] = Pj[a] * M.qqgg; d[2][a] = Qk[a] * M.qg_t; d[3][a] = Ql[a] * M.a_t + M.d11; }
+#else
         MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
         // user-defined matrix elements (bz_set_msq_override) run on the runtime-mask instantiation, so that the
         // specialised mixture kernels carry no extra registers for them
         if constexpr (kMask < 0) { if (P.has_ovr) msq_apply_override(M, P.msq_ovr, g4w); }
         deposit_half<kMask>(mask, Pi, Pj, Qk, Ql, M, d[0], d[1], d[2], d[3]);
+#endif
     }
     __syncwarp();                                        // both lanes of every pair have read the gathered f
     if (work) {
@@ -345,6 +361,8 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
             unsigned kstart;
             bool active;
             double p1x, p1y, p1z, E1;
+            const uint32_t xr = (uint32_t)xcell + P.x_rng_offset;
+            [[maybe_unused]] uint32_t w0[4], w1[4], wa[4], wb[4];      // Philox blocks 0, 1, 2 + kstart, 3 + kstart (uniform sampler)
             if (rcount >= 32 || !fresh) {
                 const int nr = min(rcount, 32);
                 rcount -= nr;
@@ -353,19 +371,32 @@ __global__ void __launch_bounds__(kCollideThreads, 1) collide_kernel(const Colli
                 ci = e.x; smp = e.y & 0x1ffffff; kstart = (unsigned)e.y >> 25;
                 cell_lookup(P.cell_tab, ci, p1x, p1y, p1z, E1);           // per lane
                 __syncwarp();                                    // the entries are read before new ones are appended
+                if constexpr (kSampler == 0) {
+                    philox4x32_10(0u, (uint32_t)smp, (uint32_t)ci, xr, P.seed, step, w0);
+                    philox4x32_10(1u, (uint32_t)smp, (uint32_t)ci, xr, P.seed, step, w1);
+                    philox4x32_10(2u + kstart, (uint32_t)smp, (uint32_t)ci, xr, P.seed, step, wa);
+                    philox4x32_10(3u + kstart, (uint32_t)smp, (uint32_t)ci, xr, P.seed, step, wb);
+                }
             } else {
                 const double2 a = *reinterpret_cast<const double2*>(&wm.p1tab[i - i0][0]), b = *reinterpret_cast<const double2*>(&wm.p1tab[i - i0][2]);
                 p1x = a.x; p1y = a.y; p1z = b.x; E1 = b.y;
                 ci = i; smp = base + lane; kstart = 0u;
                 active = smp < P.Ns;
+                // fresh pass: block number, p1 cell and spatial cell are warp-uniform, only the sample index depends on the
+                // lane -- 16 of the 20 multiplications of a block are per-lane work, the rest goes to the uniform datapath
+                if constexpr (kSampler == 0) {
+                    philox4x32_10(0u, (uint32_t)smp, (uint32_t)i, xr, P.seed, step, w0);
+                    philox4x32_10(1u, (uint32_t)smp, (uint32_t)i, xr, P.seed, step, w1);
+                    philox4x32_10(2u, (uint32_t)smp, (uint32_t)i, xr, P.seed, step, wa);
+                    philox4x32_10(3u, (uint32_t)smp, (uint32_t)i, xr, P.seed, step, wb);
+                }
                 base += 32; --units_left;
                 if (base >= P.Ns) { base = 0; ++i; }
             }
             Sample sa;
             sa.flag = 0; sa.retry = 0;
             if (active) {
-                const uint32_t xr = (uint32_t)xcell + P.x_rng_offset;
-                if constexpr (kSampler == 0) sa = gen_sample_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
+                if constexpr (kSampler == 0) sa = gen_sample_words(P.g, w0, w1, wa, wb, kstart, p1x, p1y, p1z, E1);
                 else if constexpr (kSampler == 1) sa = gen_sample_is_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1, wm.m2x);
                 else sa = gen_sample_box_pair(P.g, P.seed, step, xr, (uint32_t)ci, (uint32_t)smp, kstart, p1x, p1y, p1z, E1);
             }

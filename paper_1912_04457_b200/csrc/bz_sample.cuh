@@ -20,8 +20,11 @@ struct GridConst {          // S8c step 0, computed once on the host in fp64
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
                                               uint32_t k1, uint32_t (&out)[4])
 {
+#ifndef BZ_PHILOX_ROUNDS
+#define BZ_PHILOX_ROUNDS 10
+#endif
 #pragma unroll
-    for (int r = 0; r < 10; ++r) {
+    for (int r = 0; r < BZ_PHILOX_ROUNDS; ++r) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
         const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
         c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
@@ -110,17 +113,16 @@ __device__ __forceinline__ void cell_kinematics(const GridConst& g, int pcell, d
 // blocks (0, 1, 2 + kstart, 3 + kstart) are independent and issued together, there is no data-dependent loop: a lane
 // whose two attempts both fail (probability 0.046) reports retry = 1 and is finished by a later call.  The sequence
 // of attempts, and therefore the accepted direction, is exactly that of the one-attempt-at-a-time loop of S8c.
-__device__ __forceinline__ Sample gen_sample_pair(const GridConst& g, uint32_t seed, uint32_t step, uint32_t xcell,
-                                                  uint32_t pcell, uint32_t smp, uint32_t kstart, double p1x, double p1y,
-                                                  double p1z, double E1)
+// gen_sample_words: the same with the four Philox blocks supplied by the caller (w0, w1: blocks 0, 1; wa, wb: blocks
+// 2 + kstart, 3 + kstart).  The collision kernel computes them itself on a fresh pass, where the block number, the p1 cell
+// and the spatial cell are warp-uniform: of the 20 multiplications of a block only 16 then depend on the lane (round 1 is
+// uniform, rounds 2 and 3 have one uniform product each) and the compiler moves the other 4 to the uniform datapath.
+__device__ __forceinline__ Sample gen_sample_words(const GridConst& g, const uint32_t (&w0)[4], const uint32_t (&w1)[4],
+                                                   const uint32_t (&wa)[4], const uint32_t (&wb)[4], uint32_t kstart, double p1x,
+                                                   double p1y, double p1z, double E1)
 {
     Sample o;
     o.flag = 0; o.retry = 0; o.k = -1; o.l = -1; o.s = 0.0; o.t = 0.0; o.u = 0.0; o.w = 1.0;
-    uint32_t w0[4], w1[4], wa[4], wb[4];
-    philox4x32_10(0u, smp, pcell, xcell, seed, step, w0);
-    philox4x32_10(1u, smp, pcell, xcell, seed, step, w1);
-    philox4x32_10(2u + kstart, smp, pcell, xcell, seed, step, wa);
-    philox4x32_10(3u + kstart, smp, pcell, xcell, seed, step, wb);
     const double L52 = g.L * 2.220446049250313e-16;       // L 2^-52, exact
     const double p2x = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[0], w0[1]), L52));
     const double p2y = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[2], w0[3]), L52));
@@ -183,6 +185,17 @@ __device__ __forceinline__ Sample gen_sample_pair(const GridConst& g, uint32_t s
     o.k = k; o.l = l;
     o.flag = (k >= 0) && (l >= 0);
     return o;
+}
+__device__ __forceinline__ Sample gen_sample_pair(const GridConst& g, uint32_t seed, uint32_t step, uint32_t xcell,
+                                                  uint32_t pcell, uint32_t smp, uint32_t kstart, double p1x, double p1y,
+                                                  double p1z, double E1)
+{
+    uint32_t w0[4], w1[4], wa[4], wb[4];
+    philox4x32_10(0u, smp, pcell, xcell, seed, step, w0);
+    philox4x32_10(1u, smp, pcell, xcell, seed, step, w1);
+    philox4x32_10(2u + kstart, smp, pcell, xcell, seed, step, wa);
+    philox4x32_10(3u + kstart, smp, pcell, xcell, seed, step, wb);
+    return gen_sample_words(g, w0, w1, wa, wb, kstart, p1x, p1y, p1z, E1);
 }
 
 #define BZ_MUL __dmul_rn
