@@ -66,6 +66,11 @@ CONFIGS = (
            noise_seed=1),
 )
 
+# The largest grid the paper's program handles, "on GPU clusters" (n_x,y,z = 20, n_px,py,pz = 40), with the momentum box
+# of its 40^3 runs and all seven species: 3.58e9 phase-space values, 28.7 GB per copy.  Not one of BASELINE.json's
+# configs: the maximum-size case of the parity tests (it fits one B200: f, f_new and the two cell-major copies are 123 GB).
+PAPER_LARGEST = Config("paper_largest_20x40", 20, 0.1, 40, -2.0, 2.0, ALL_SPECIES, 64, 1, 0.0025, init="mix_gauss", Qs=1.0, sigma=0.6)
+
 
 def scaled(cfg, **kw):
     """Same physics, smaller grid / fewer samples: the parity-test cases the oracle finishes in seconds."""
