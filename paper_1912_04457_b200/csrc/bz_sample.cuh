@@ -218,10 +218,16 @@ __device__ __forceinline__ void sample_p2(const GridConst& g, uint32_t seed, uin
     E2 = __dsqrt_rn(BZ_ADD(BZ_ADD(BZ_MUL(p2x, p2x), BZ_MUL(p2y, p2y)), BZ_MUL(p2z, p2z)));
     const double d12 = BZ_ADD(BZ_ADD(BZ_MUL(p1x, p2x), BZ_MUL(p1y, p2y)), BZ_MUL(p1z, p2z));
     s = BZ_MUL(2.0, BZ_SUB(BZ_MUL(E1, E2), d12));
-    bool in;
-    int a = bin_axis_exact(p2x, g, in), b = bin_axis_exact(p2y, g, in), c = bin_axis_exact(p2z, g, in);
-    a = min(max(a, 0), g.n - 1); b = min(max(b, 0), g.n - 1); c = min(max(c, 0), g.n - 1);
-    j = a + g.n * (b + g.n * c);
+    // guarded fast binning (bin_axis_fast), the definition only inside the guard band; p2 is inside by construction, the clamp
+    // is the defensive one of S8c step 3
+    bool risky = false;
+    j = bin_cell_fast(p2x, p2y, p2z, g, risky);
+    if (risky || j < 0) {
+        bool in;
+        int a = bin_axis_exact(p2x, g, in), b = bin_axis_exact(p2y, g, in), c = bin_axis_exact(p2z, g, in);
+        a = min(max(a, 0), g.n - 1); b = min(max(b, 0), g.n - 1); c = min(max(c, 0), g.n - 1);
+        j = a + g.n * (b + g.n * c);
+    }
 }
 
 // boost of the CM pair (M/2)(1, n) back, t, and the cells of p3, p4 (S8c steps 2-3)
@@ -237,8 +243,13 @@ __device__ __forceinline__ void sample_boost(const GridConst& g, double p1x, dou
     const double d13 = BZ_ADD(BZ_ADD(BZ_MUL(p1x, p3x), BZ_MUL(p1y, p3y)), BZ_MUL(p1z, p3z));
     o.t = BZ_MUL(-2.0, BZ_SUB(BZ_MUL(E1, E3), d13));                  // t of the constructed momenta: the one Table I sees
     o.u = BZ_SUB(-o.s, o.t);
-    o.k = bin_cell_exact(p3x, p3y, p3z, g);
-    o.l = bin_cell_exact(p4x, p4y, p4z, g);
+    bool risky = false;
+    o.k = bin_cell_fast(p3x, p3y, p3z, g, risky);
+    o.l = bin_cell_fast(p4x, p4y, p4z, g, risky);
+    if (risky) {                                         // ~4e-5 of the samples: repeat with the definition
+        o.k = bin_cell_exact(p3x, p3y, p3z, g);
+        o.l = bin_cell_exact(p4x, p4y, p4z, g);
+    }
     o.flag = (o.k >= 0) && (o.l >= 0);
 }
 
