@@ -863,7 +863,8 @@ def test_long_run_properties_full_size(k, steps):
     particle number (Eq. 22-23) and, for quarks, the net number of every flavour are conserved to rounding; f stays finite
     and inside the Pauli bound; the entropy of the binned distribution grows (H theorem of Eq. 5's gain - loss bracket).
     Energy is not asserted: deposits at cell centres conserve it only up to the cell size (the paper's Fig. 5, P:262-275:
-    1.5 % at 30^3 after 1 fm/c; on config 0's 15^3 grid it doubles within 10 fm/c, in the oracle as on the GPU)."""
+    1.5 % at 30^3 after 1 fm/c; on config 0's 15^3 grid it doubles within 10 fm/c -- a property of the method: the first
+    10 of these steps agree with the oracle value by value, test_f_after_all_steps_full_size_homogeneous)."""
     cfg = wl.CONFIGS[k]
     _, g = _pair(cfg, threads=1)
     f0 = torch.from_numpy(wl.initial_f(cfg))
