@@ -100,15 +100,18 @@ struct PaperLegs {
     __device__ __forceinline__ double ep(int c) const { return c == 0 ? Ep[0] : (c == 1 ? Ep[1] : (c == 2 ? Ep[2] : Ep[3])); }
 };
 
-// Returns a bit mask: bit 0 = the + root is kept (out[0]), bit 1 = the - root (out[1]): no run-time index into out, so the two
-// roots stay in registers.
-__device__ __forceinline__ int paper_roots_core(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
-                                                double m1, double m2, double m3, double m4, double E3, double Ep, int ixy1, int ixy2,
-                                                Root (&out)[2])
-{
+// The root solving in two stages, so that the kernel can compact the few candidates that pass the cheap first stage
+// before it runs the expensive second one (paper_queue_kernel).  Both use single rounded operations in the oracle's
+// association order; stage 2 recomputes the tuple's constants from the same inputs with the same operations, so the two
+// stages together give the bits of the one-piece form.
 #define MUL __dmul_rn
 #define ADD __dadd_rn
 #define SUB __dsub_rn
+// Stage 1: the quadratic for z = k1z, the sign test of the squarings and the box test of the z components of k1 and k2
+// (S9).  Returns a bit mask: bit 0 = the + root is a candidate, bit 1 = the - root; z and the z cell indices b1, b2 per sign.
+__device__ __forceinline__ int paper_roots_stage1(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
+                                                  double m1, double m2, double E3, double Ep, double (&zr)[2], int (&b1r)[2], int (&b2r)[2])
+{
     const double Et = ADD(E3, Ep);
     const double Px = ADD(k3[0], p[0]), Py = ADD(k3[1], p[1]), Pz = ADD(k3[2], p[2]);
     const double A1 = ADD(ADD(MUL(k1x, k1x), MUL(k1y, k1y)), m1);
@@ -121,38 +124,68 @@ __device__ __forceinline__ int paper_roots_core(const GridConst& g, const double
     const double D = SUB(MUL(C, C), MUL(MUL(4.0, a), A1));
     if (!(D > 0.0)) return 0;
     const double sq = MUL(Et, __dsqrt_rn(D)), CP = MUL(C, Pz), a2 = MUL(2.0, a);
-    int nr = 0;
+    int cand = 0;
 #pragma unroll
     for (int sign = 0; sign < 2; ++sign) {
         const double z = __ddiv_rn(sign == 0 ? ADD(CP, sq) : SUB(CP, sq), a2);
         if (!(ADD(C, MUL(MUL(2.0, Pz), z)) >= 0.0)) continue;
-        // the box test of the two z components first (S9): most roots end here, before two square roots and two
-        // divisions; the transverse components of k1 and k2 do not depend on the root and were binned by the caller
+        // the box test of the two z components (S9): most roots end here.  Guarded fast binning (bin_axis_fast: 1 DFMA +
+        // conversion), the definition's subtraction and division only inside the guard band around a cell edge
         const double k2z = SUB(Pz, z);
-        // guarded fast binning (bin_axis_fast: 1 DFMA + conversion), the definition's subtraction and division only inside the
-        // guard band around a cell edge: same cells and flags, four IEEE divisions fewer per mass tuple
         bool in1, in2, risky = false;
         int b1 = bin_axis_fast(z, g, in1, risky), b2 = bin_axis_fast(k2z, g, in2, risky);
         if (risky) { b1 = bin_axis_exact(z, g, in1); b2 = bin_axis_exact(k2z, g, in2); }
         if (!(in1 && in2)) continue;
-        const int i1 = ixy1 + g.n * g.n * b1, i2 = ixy2 + g.n * g.n * b2;
-        const double E1 = __dsqrt_rn(ADD(A1, MUL(z, z)));
-        if (!(E1 <= Et)) continue;
-        const double E2 = __dsqrt_rn(ADD(A2, MUL(k2z, k2z)));
-        if (!(E1 > 0.0 && E2 > 0.0)) continue;
-        const double J = SUB(__ddiv_rn(z, E1), __ddiv_rn(k2z, E2));          // Eq. 19
-        if (J == 0.0) continue;
-        Root& r = out[sign];
-        nr |= 1 << sign;
-        r.i1 = i1; r.i2 = i2;
-        r.w_inv = fabs(J) * (((E1 * E2) * E3) * Ep);
-        r.s = SUB(Et2, ADD(ADD(MUL(Px, Px), MUL(Py, Py)), Pz2));
-        r.t = SUB(ADD(m1, m3), MUL(2.0, SUB(MUL(E1, E3), ADD(ADD(MUL(k1x, k3[0]), MUL(k1y, k3[1])), MUL(z, k3[2])))));
-        r.u = SUB(ADD(m1, m4), MUL(2.0, SUB(MUL(E1, Ep), ADD(ADD(MUL(k1x, p[0]), MUL(k1y, p[1])), MUL(z, p[2])))));
+        cand |= 1 << sign;
+        zr[sign] = z; b1r[sign] = b1; b2r[sign] = b2;
     }
+    return cand;
+}
+
+// Stage 2 for one candidate z: the energies of the incoming legs, the spurious-root test E1 <= Et, the Jacobian of Eq. 19
+// and (s, t, u) of the constructed momenta.  False: the root is dropped.
+__device__ __forceinline__ bool paper_roots_stage2(const double (&p)[3], const double (&k3)[3], double k1x, double k1y, double m1, double m2,
+                                                   double m3, double m4, double E3, double Ep, double z, Root& r)
+{
+    const double Et = ADD(E3, Ep);
+    const double Px = ADD(k3[0], p[0]), Py = ADD(k3[1], p[1]), Pz = ADD(k3[2], p[2]);
+    const double A1 = ADD(ADD(MUL(k1x, k1x), MUL(k1y, k1y)), m1);
+    const double qx = SUB(Px, k1x), qy = SUB(Py, k1y);
+    const double A2 = ADD(ADD(MUL(qx, qx), MUL(qy, qy)), m2);
+    const double Et2 = MUL(Et, Et), Pz2 = MUL(Pz, Pz);
+    const double k2z = SUB(Pz, z);
+    const double E1 = __dsqrt_rn(ADD(A1, MUL(z, z)));
+    if (!(E1 <= Et)) return false;
+    const double E2 = __dsqrt_rn(ADD(A2, MUL(k2z, k2z)));
+    if (!(E1 > 0.0 && E2 > 0.0)) return false;
+    const double J = SUB(__ddiv_rn(z, E1), __ddiv_rn(k2z, E2));          // Eq. 19
+    if (J == 0.0) return false;
+    r.w_inv = fabs(J) * (((E1 * E2) * E3) * Ep);
+    r.s = SUB(Et2, ADD(ADD(MUL(Px, Px), MUL(Py, Py)), Pz2));
+    r.t = SUB(ADD(m1, m3), MUL(2.0, SUB(MUL(E1, E3), ADD(ADD(MUL(k1x, k3[0]), MUL(k1y, k3[1])), MUL(z, k3[2])))));
+    r.u = SUB(ADD(m1, m4), MUL(2.0, SUB(MUL(E1, Ep), ADD(ADD(MUL(k1x, p[0]), MUL(k1y, p[1])), MUL(z, p[2])))));
+    return true;
+}
 #undef MUL
 #undef ADD
 #undef SUB
+
+// Both stages for one mass tuple (the debug export).  Bit mask: bit 0 = the + root is kept (out[0]), bit 1 = the - root (out[1]).
+__device__ __forceinline__ int paper_roots_core(const GridConst& g, const double (&p)[3], const double (&k3)[3], double k1x, double k1y,
+                                                double m1, double m2, double m3, double m4, double E3, double Ep, int ixy1, int ixy2,
+                                                Root (&out)[2])
+{
+    double z[2];
+    int b1[2], b2[2];
+    const int cand = paper_roots_stage1(g, p, k3, k1x, k1y, m1, m2, E3, Ep, z, b1, b2);
+    int nr = 0;
+#pragma unroll
+    for (int sign = 0; sign < 2; ++sign) {
+        if (!((cand >> sign) & 1)) continue;
+        if (!paper_roots_stage2(p, k3, k1x, k1y, m1, m2, m3, m4, E3, Ep, z[sign], out[sign])) continue;
+        out[sign].i1 = ixy1 + g.n * g.n * b1[sign]; out[sign].i2 = ixy2 + g.n * g.n * b2[sign];
+        nr |= 1 << sign;
+    }
     return nr;
 }
 
@@ -236,16 +269,23 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
 //            |J| E1 E2 E3 Ep and the bit mask of the channel groups that share the tuple.
 //   deposit  whenever the ring holds 32 records: lanes = roots; Table I at the root's massive s, t, u, then the lane
 //            walks the channels of its tuple: 4 loads, the bracket of Eq. 5, 4 reductions (RED.E.ADD.F64) per channel.
-constexpr int kQWarps = 8, kQRing = 64;
+constexpr int kQWarps = 8, kQRing = 64, kQCand = 128;
 struct QWarp {
     unsigned cell[4][kQRing];          // k1, k2, k3, p
     double s[kQRing], t[kQRing], u[kQRing], w_inv[kQRing];
-    unsigned long long groups[kQRing]; // bit g: channel group g belongs to the record's (canonical) mass tuple
+    unsigned char rgi[kQRing];         // the record's channel group (its canonical mass tuple's channels: gmask[rgi])
     unsigned long long gmask[64];      // per channel group of the current spatial cell: the groups with the same canonical tuple
+    unsigned tup[64];                  // the distinct canonical mass tuples of the current spatial cell: key | first group << 16
+    int ntup;
+    double msm[4];                     // the spatial cell's four masses^2
+    // candidates of stage 1 waiting for stage 2 (they refer to the samples the warp's lanes hold at the moment):
+    double cz[kQCand];                 // z component of k1 (a tuple adds at most 64 candidates to fewer than 32 waiting ones)
+    unsigned long long cmeta[kQCand];  // source lane | canonical tuple << 5 | channel group << 13 | z cell of k1 << 19 | z cell of k2 << 30
 };
 
+// not inlined: three call sites, and the kernel's code has to fit the instruction cache (ncu: stall_no_instruction)
 template <bool kAllMassless>
-__device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
+__device__ __noinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
 {
     if (lane >= nb) return;
     const int r = (head + lane) & (kQRing - 1);
@@ -279,7 +319,7 @@ __device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp&
         }
         return;
     }
-    for (unsigned long long left = q.groups[r]; left; left &= left - 1ull) {
+    for (unsigned long long left = q.gmask[q.rgi[r]]; left; left &= left - 1ull) {
         const PaperGroup G = P.groups[__ffsll((long long)left) - 1];
         for (int c = G.begin; c < G.end; ++c) {
             const PaperChannel ch = P.table[c];
@@ -303,7 +343,10 @@ __device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp&
 }
 
 template <bool kAllMassless>
-__global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperParams P)
+#ifndef BZ_PAPER_MINB
+#define BZ_PAPER_MINB 2
+#endif
+__global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB) paper_queue_kernel(const PaperParams P)
 {
     __shared__ QWarp sh_all[kQWarps];
     QWarp& q = sh_all[threadIdx.x >> 5];
@@ -314,6 +357,7 @@ __global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperPa
     const long long n_items = chunks_per_x * P.x_count;
     const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
     int head = 0, count = 0, cur_x = -1;
+    int chead = 0, ccount = 0;          // ring of stage-1 candidates (empty between sampling passes)
     unsigned rep = 0u;
     double mreg = 0.0;
     for (long long item = warp0; item < n_items; item += n_warps) {
@@ -341,6 +385,17 @@ __global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperPa
                 for (int g1 = 0; g1 < P.n_groups; ++g1) if (canon0(P.groups[g1].key) == ck) mk |= 1ull << g1;
                 q.gmask[g0] = mk;
             }
+            if (lane == 0) {                                 // the distinct canonical tuples, in the order of their first group
+                int nt = 0;
+                for (int g0 = 0; g0 < P.n_groups; ++g0) {
+                    const unsigned ck0 = (unsigned)canon0(P.groups[g0].key);
+                    bool seen = false;
+                    for (int t0 = 0; t0 < nt; ++t0) seen = seen || (q.tup[t0] & 0xffffu) == ck0;
+                    if (!seen) q.tup[nt++] = ck0 | (unsigned)g0 << 16;
+                }
+                q.ntup = nt;
+            }
+            if (lane < 4) q.msm[lane] = m[lane];
             __syncwarp();
         }
         auto rp = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
@@ -376,37 +431,77 @@ __global__ void __launch_bounds__(32 * kQWarps) paper_queue_kernel(const PaperPa
         if (!__any_sync(full, live)) continue;
         // energies of the outgoing legs, once per mass class (the roots of a tuple take E3 of its third, Ep of its fourth class)
         const PaperLegs L(p, k3, m);
-        unsigned long long done_lo = 0ull, done_hi = 0ull, done_2 = 0ull, done_3 = 0ull;   // canonical keys already solved (256 bits)
-        for (int gi = 0; gi < P.n_groups; ++gi) {                          // warp-uniform: one spatial cell per warp
-            const int ck = canon(P.groups[gi].key);
-            const unsigned long long bit = 1ull << (ck & 63);
-            const int wsel = ck >> 6;
-            const unsigned long long dw = wsel == 0 ? done_lo : (wsel == 1 ? done_hi : (wsel == 2 ? done_2 : done_3));
-            if (dw & bit) continue;
-            if (wsel == 0) done_lo |= bit; else if (wsel == 1) done_hi |= bit; else if (wsel == 2) done_2 |= bit; else done_3 |= bit;
-            Root rt[2];
-            const int kept = live ? paper_roots_core(P.g, p, k3, k1x, k1y, m[ck & 3], m[(ck >> 2) & 3], m[(ck >> 4) & 3], m[(ck >> 6) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), ixy1, ixy2, rt) : 0;
-            const unsigned long long gm = q.gmask[gi];
+        // stage 2 for candidates [chead, chead + nb): lanes = candidates; the sample a candidate belongs to lives in the registers
+        // of its source lane and comes over by shuffles; E3 and Ep are recomputed with PaperLegs' operations (the same bits)
+        auto stage2_batch = [&](int nb) {
+            const bool on = lane < nb;
+            const int cr = (chead + lane) & (kQCand - 1);
+            const unsigned long long meta = on ? q.cmeta[cr] : (unsigned long long)lane;
+            const double z = on ? q.cz[cr] : 0.0;
+            const int src = (int)(meta & 31ull), ck = (int)((meta >> 5) & 255ull), cgi = (int)((meta >> 13) & 63ull);
+            const int b1 = (int)((meta >> 19) & 2047ull), b2 = (int)((meta >> 30) & 2047ull);
+            double sp[3], sk3[3];
 #pragma unroll
-            for (int r = 0; r < 2; ++r) {
-                const bool mine = (kept >> r) & 1;
-                const unsigned has = __ballot_sync(full, mine);
-                if (!has) continue;
-                if (mine) {
-                    const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
-                    q.cell[0][w] = (unsigned)rt[r].i1; q.cell[1][w] = (unsigned)rt[r].i2; q.cell[2][w] = (unsigned)i3; q.cell[3][w] = (unsigned)i;
-                    q.s[w] = rt[r].s; q.t[w] = rt[r].t; q.u[w] = rt[r].u; q.w_inv[w] = rt[r].w_inv;
-                    q.groups[w] = gm;
-                }
-                count += __popc(has);
-                __syncwarp();
-                if (count >= 32) {
-                    paper_deposit_batch<kAllMassless>(P, q, lane, head, 32, xcell, mreg);
-                    head = (head + 32) & (kQRing - 1);
-                    count -= 32;
-                    __syncwarp();
-                }
+            for (int d = 0; d < 3; ++d) { sp[d] = __shfl_sync(full, p[d], src); sk3[d] = __shfl_sync(full, k3[d], src); }
+            const double sk1x = __shfl_sync(full, k1x, src), sk1y = __shfl_sync(full, k1y, src);
+            const int sxy1 = __shfl_sync(full, ixy1, src), sxy2 = __shfl_sync(full, ixy2, src);
+            const int si3 = __shfl_sync(full, i3, src), si = __shfl_sync(full, i, src);
+            bool kept = false;
+            Root rt;
+            if (on) {
+                const double m1 = q.msm[ck & 3], m2 = q.msm[(ck >> 2) & 3], m3 = q.msm[(ck >> 4) & 3], m4 = q.msm[(ck >> 6) & 3];
+                const double kk = __dadd_rn(__dadd_rn(__dmul_rn(sk3[0], sk3[0]), __dmul_rn(sk3[1], sk3[1])), __dmul_rn(sk3[2], sk3[2]));
+                const double pp = __dadd_rn(__dadd_rn(__dmul_rn(sp[0], sp[0]), __dmul_rn(sp[1], sp[1])), __dmul_rn(sp[2], sp[2]));
+                const double E3 = __dsqrt_rn(__dadd_rn(kk, m3)), Ep = __dsqrt_rn(__dadd_rn(pp, m4));
+                kept = paper_roots_stage2(sp, sk3, sk1x, sk1y, m1, m2, m3, m4, E3, Ep, z, rt);
             }
+            const unsigned has = __ballot_sync(full, kept);
+            if (kept) {
+                const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
+                const int n2 = P.g.n * P.g.n;
+                q.cell[0][w] = (unsigned)(sxy1 + n2 * b1); q.cell[1][w] = (unsigned)(sxy2 + n2 * b2); q.cell[2][w] = (unsigned)si3; q.cell[3][w] = (unsigned)si;
+                q.s[w] = rt.s; q.t[w] = rt.t; q.u[w] = rt.u; q.w_inv[w] = rt.w_inv;
+                q.rgi[w] = (unsigned char)cgi;
+            }
+            count += __popc(has);
+            chead = (chead + nb) & (kQCand - 1);
+            ccount -= nb;
+            __syncwarp();
+            if (count >= 32) {
+                paper_deposit_batch<kAllMassless>(P, q, lane, head, 32, xcell, mreg);
+                head = (head + 32) & (kQRing - 1);
+                count -= 32;
+                __syncwarp();
+            }
+        };
+        // one more trip than there are groups: the last one only drains the candidates (they refer to this pass's samples, none
+        // is carried over).  stage2_batch is expanded at this one place: the kernel's code must stay inside the instruction cache
+        const int ntup = q.ntup;
+        for (int ti = 0; ti <= ntup; ++ti) {                               // warp-uniform: one spatial cell per warp
+            const bool last = ti == ntup;
+            const bool solve = !last;
+            const unsigned tu = q.tup[solve ? ti : 0];
+            const int ck = (int)(tu & 0xffffu), gi = (int)(tu >> 16);
+            if (solve) {
+                // stage 1 for every lane: 0.14-0.16 candidates per lane and tuple pass the box test
+                double zr[2];
+                int b1r[2], b2r[2];
+                const int cand = live ? paper_roots_stage1(P.g, p, k3, k1x, k1y, q.msm[ck & 3], q.msm[(ck >> 2) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), zr, b1r, b2r) : 0;
+#pragma unroll
+                for (int r = 0; r < 2; ++r) {
+                    const bool mine = (cand >> r) & 1;
+                    const unsigned has = __ballot_sync(full, mine);
+                    if (mine) {
+                        const int w = (chead + ccount + __popc(has & lt)) & (kQCand - 1);
+                        q.cz[w] = zr[r];
+                        q.cmeta[w] = (unsigned long long)lane | (unsigned long long)ck << 5 | (unsigned long long)gi << 13 |
+                                     (unsigned long long)b1r[r] << 19 | (unsigned long long)b2r[r] << 30;
+                    }
+                    ccount += __popc(has);
+                }
+                __syncwarp();
+            }
+            while (ccount >= 32 || (last && ccount > 0)) stage2_batch(min(ccount, 32));   // full warps of candidates
         }
     }
     while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
