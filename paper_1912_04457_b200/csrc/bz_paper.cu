@@ -270,36 +270,45 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
 //   deposit  whenever the ring holds 32 records: lanes = roots; Table I at the root's massive s, t, u, then the lane
 //            walks the channels of its tuple: 4 loads, the bracket of Eq. 5, 4 reductions (RED.E.ADD.F64) per channel.
 constexpr int kQWarps = 8, kQRing = 64, kQCand = 128;
-struct QWarp {
-    unsigned cell[4][kQRing];          // k1, k2, k3, p
+struct QWarp {                         // per warp, in dynamic shared memory (9.6 KB)
+    unsigned cell[4][kQRing];          // root records: cells of k1, k2, k3, p
     double s[kQRing], t[kQRing], u[kQRing], w_inv[kQRing];
-    unsigned char rgi[kQRing];         // the record's channel group (its canonical mass tuple's channels: gmask[rgi])
-    unsigned long long gmask[64];      // per channel group of the current spatial cell: the groups with the same canonical tuple
-    unsigned tup[64];                  // the distinct canonical mass tuples of the current spatial cell: key | first group << 16
+    unsigned char rti[kQRing];         // the record's canonical mass tuple (index into tup / choff)
+    // per spatial cell (classes with bit-identical masses are merged: "canonical" tuples)
+    unsigned short ckey[64];           // canonical tuple key of every channel group
+    unsigned tup[64];                  // the distinct canonical tuples: key | first group << 16
+    unsigned short choff[66];          // channels of tuple ti: chlist[choff[ti] .. choff[ti + 1])
+    unsigned char chlist[128];         // indices into the channel table
     int ntup;
     double msm[4];                     // the spatial cell's four masses^2
     // candidates of stage 1 waiting for stage 2 (they refer to the samples the warp's lanes hold at the moment):
     double cz[kQCand];                 // z component of k1 (a tuple adds at most 64 candidates to fewer than 32 waiting ones)
-    unsigned long long cmeta[kQCand];  // source lane | canonical tuple << 5 | channel group << 13 | z cell of k1 << 19 | z cell of k2 << 30
+    unsigned long long cmeta[kQCand];  // source lane | canonical tuple key << 5 | tuple index << 13 | z cell of k1 << 19 | z cell of k2 << 30
+    // deposit scratch: Table I of the 32 roots of a batch, [2 kind + crossed][root], and the running channel counts
+    double mvs[14][32];
+    int pre[33];
 };
 
 // not inlined: three call sites, and the kernel's code has to fit the instruction cache (ncu: stall_no_instruction)
 template <bool kAllMassless>
 __device__ __noinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
 {
-    if (lane >= nb) return;
+    const bool on = lane < nb;
     const int r = (head + lane) & (kQRing - 1);
-    const double w = P.Kp / q.w_inv[r];
-    MsqSet M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
-    if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
-    const double mv[14] = { M.a_t, M.a_u, M.m11, M.m11, M.m1b_t, M.m1b_u, M.ann, M.ann, M.qqgg, M.qqgg, M.qg_t, M.qg_u, M.gg, M.gg };
-    const unsigned c1 = q.cell[0][r], c2 = q.cell[1][r], c3 = q.cell[2][r], c4 = q.cell[3][r];
     const double* fx = P.f + (size_t)xcell * P.S * P.Np;
     double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+    MsqSet M = {};
+    if (on) {
+        const double w = P.Kp / q.w_inv[r];
+        M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
+        if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+    }
     if constexpr (kAllMassless) {
         // every mass is zero (no bz_thermal_masses / bz_set_masses call yet): one tuple, the root serves ALL channels, and their sum
         // is the hot path's factorised algebra (bz_channels.cuh) on the four cells -- 4 x S loads and reductions per root
         // instead of 4 per channel.  (A separate instantiation: inlined into the general kernel it cost that one 40 %.)
+        if (!on) return;
+        const unsigned c1 = q.cell[0][r], c2 = q.cell[1][r], c3 = q.cell[2][r], c4 = q.cell[3][r];
         double fv[4][7], d[4][7];
 #pragma unroll
         for (int id = 0; id < 7; ++id) {
@@ -318,27 +327,50 @@ __device__ __noinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q,
             if (d[3][id] != 0.0) red_add(dx + (size_t)a * P.Np + c4, d[3][id]);
         }
         return;
-    }
-    for (unsigned long long left = q.gmask[q.rgi[r]]; left; left &= left - 1ull) {
-        const PaperGroup G = P.groups[__ffsll((long long)left) - 1];
-        for (int c = G.begin; c < G.end; ++c) {
-            const PaperChannel ch = P.table[c];
-            const double fa = fx[(size_t)ch.a * P.Np + c1], fb = fx[(size_t)ch.b * P.Np + c2];
-            const double fc = fx[(size_t)ch.c * P.Np + c3], fd = fx[(size_t)ch.d * P.Np + c4];
-            const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
-            const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
-            const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-            // mv is indexed at run time: a 14-way select keeps it in registers
-            double Mv = mv[0];
-            const int mi = 2 * ch.kind + ch.crossed;
+    } else {
+        // With masses a root serves only the channels of its own mass tuple (3 on average with four distinct masses, up to 90
+        // when classes coincide).  Lanes = roots for Table I (stored per root in shared memory), then lanes = (root, channel)
+        // pairs of the whole batch, flattened through a prefix sum of the roots' channel counts: every pair costs 4 loads, the
+        // bracket of Eq. 5 and 4 reductions, with no lane waiting for another root's longer channel list.
+        const unsigned full = 0xffffffffu;
+        int cnt = 0;
+        if (on) {
+            const int ti = q.rti[r];
+            cnt = (int)q.choff[ti + 1] - (int)q.choff[ti];
+            q.mvs[0][lane] = M.a_t; q.mvs[1][lane] = M.a_u; q.mvs[2][lane] = M.m11; q.mvs[3][lane] = M.m11;
+            q.mvs[4][lane] = M.m1b_t; q.mvs[5][lane] = M.m1b_u; q.mvs[6][lane] = M.ann; q.mvs[7][lane] = M.ann;
+            q.mvs[8][lane] = M.qqgg; q.mvs[9][lane] = M.qqgg; q.mvs[10][lane] = M.qg_t; q.mvs[11][lane] = M.qg_u;
+            q.mvs[12][lane] = M.gg; q.mvs[13][lane] = M.gg;
+        }
+        int incl = cnt;
 #pragma unroll
-            for (int k = 1; k < 14; ++k) Mv = mi == k ? mv[k] : Mv;
-            const double A = Mv * fwd;
-            if (A != 0.0) {
-                red_add(dx + (size_t)ch.a * P.Np + c1, -A); red_add(dx + (size_t)ch.b * P.Np + c2, -A);   // Eq. 22
-                red_add(dx + (size_t)ch.c * P.Np + c3, A);  red_add(dx + (size_t)ch.d * P.Np + c4, A);
+        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, incl, o); if (lane >= o) incl += v; }
+        q.pre[lane + 1] = incl;
+        if (lane == 0) q.pre[0] = 0;
+        const int total = __shfl_sync(full, incl, 31);
+        __syncwarp();
+        for (int base = 0; base < total; base += 32) {
+            const int fl = base + lane;
+            if (fl < total) {
+                int lo = 0;                                   // the root that owns pair fl: the largest lo with pre[lo] <= fl
+#pragma unroll
+                for (int stp = 16; stp > 0; stp >>= 1) { if (q.pre[lo + stp] <= fl) lo += stp; }
+                const int rr = (head + lo) & (kQRing - 1);
+                const PaperChannel ch = P.table[q.chlist[(int)q.choff[q.rti[rr]] + (fl - q.pre[lo])]];
+                const unsigned c1 = q.cell[0][rr], c2 = q.cell[1][rr], c3 = q.cell[2][rr], c4 = q.cell[3][rr];
+                const size_t oa = (size_t)ch.a * P.Np + c1, ob = (size_t)ch.b * P.Np + c2, oc = (size_t)ch.c * P.Np + c3, od = (size_t)ch.d * P.Np + c4;
+                const double fa = fx[oa], fb = fx[ob], fc = fx[oc], fd = fx[od];
+                const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
+                const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
+                const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
+                const double A = q.mvs[2 * ch.kind + ch.crossed][lo] * fwd;
+                if (A != 0.0) {
+                    red_add(dx + oa, -A); red_add(dx + ob, -A);                        // Eq. 22
+                    red_add(dx + oc, A);  red_add(dx + od, A);
+                }
             }
         }
+        __syncwarp();                                        // the scratch is rewritten by the next batch
     }
 }
 
@@ -348,8 +380,8 @@ template <bool kAllMassless>
 #endif
 __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB) paper_queue_kernel(const PaperParams P)
 {
-    __shared__ QWarp sh_all[kQWarps];
-    QWarp& q = sh_all[threadIdx.x >> 5];
+    extern __shared__ __align__(16) unsigned char paper_smem[];
+    QWarp& q = reinterpret_cast<QWarp*>(paper_smem)[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
     const long long per_x = (long long)P.p_count * P.Ns;
@@ -379,27 +411,38 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
             }
             auto rp0 = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
             auto canon0 = [&](int key) { return rp0(key & 3) | rp0((key >> 2) & 3) << 2 | rp0((key >> 4) & 3) << 4 | rp0((key >> 6) & 3) << 6; };
-            for (int g0 = lane; g0 < P.n_groups; g0 += 32) {
-                const int ck = canon0(P.groups[g0].key);
-                unsigned long long mk = 0ull;
-                for (int g1 = 0; g1 < P.n_groups; ++g1) if (canon0(P.groups[g1].key) == ck) mk |= 1ull << g1;
-                q.gmask[g0] = mk;
+            // canonical key of every channel group; the distinct ones in the order of their first group; their channel lists
+            for (int g0 = lane; g0 < P.n_groups; g0 += 32) q.ckey[g0] = (unsigned short)canon0(P.groups[g0].key);
+            __syncwarp();
+            int nt = 0;
+            for (int g0 = lane; g0 < ((P.n_groups + 31) & ~31); g0 += 32) {
+                bool first = g0 < P.n_groups;
+                for (int g1 = 0; g1 < g0 && first; ++g1) first = q.ckey[g1] != q.ckey[g0];
+                const unsigned fm = __ballot_sync(full, first);
+                if (first) q.tup[nt + __popc(fm & lt)] = (unsigned)q.ckey[g0] | (unsigned)g0 << 16;
+                nt += __popc(fm);
             }
-            if (lane == 0) {                                 // the distinct canonical tuples, in the order of their first group
-                int nt = 0;
-                for (int g0 = 0; g0 < P.n_groups; ++g0) {
-                    const unsigned ck0 = (unsigned)canon0(P.groups[g0].key);
-                    bool seen = false;
-                    for (int t0 = 0; t0 < nt; ++t0) seen = seen || (q.tup[t0] & 0xffffu) == ck0;
-                    if (!seen) q.tup[nt++] = ck0 | (unsigned)g0 << 16;
+            __syncwarp();
+            int run = 0;                                     // channels of the tuples before this trip's
+            for (int t0 = lane; t0 < ((nt + 31) & ~31); t0 += 32) {
+                int cnt = 0;
+                const unsigned key = t0 < nt ? (q.tup[t0] & 0xffffu) : 0xffffffffu;
+                for (int g1 = 0; g1 < P.n_groups; ++g1) if (q.ckey[g1] == key) cnt += P.groups[g1].end - P.groups[g1].begin;
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, incl, o); if (lane >= o) incl += v; }
+                int w = run + incl - cnt;
+                if (t0 < nt) {
+                    q.choff[t0] = (unsigned short)w;
+                    for (int g1 = 0; g1 < P.n_groups; ++g1)
+                        if (q.ckey[g1] == key) for (int c = P.groups[g1].begin; c < P.groups[g1].end; ++c) q.chlist[w++] = (unsigned char)c;
                 }
-                q.ntup = nt;
+                run += __shfl_sync(full, incl, 31);
             }
+            if (lane == 0) { q.choff[nt] = (unsigned short)run; q.ntup = nt; }
             if (lane < 4) q.msm[lane] = m[lane];
             __syncwarp();
         }
-        auto rp = [&](int cls) { return (int)((rep >> (2 * cls)) & 3u); };
-        auto canon = [&](int key) { return rp(key & 3) | rp((key >> 2) & 3) << 2 | rp((key >> 4) & 3) << 4 | rp((key >> 6) & 3) << 6; };
         const long long local = (item % chunks_per_x) * 32 + lane;
         const bool valid = local < per_x;
         const long long lc = valid ? local : per_x - 1;
@@ -438,7 +481,7 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
             const int cr = (chead + lane) & (kQCand - 1);
             const unsigned long long meta = on ? q.cmeta[cr] : (unsigned long long)lane;
             const double z = on ? q.cz[cr] : 0.0;
-            const int src = (int)(meta & 31ull), ck = (int)((meta >> 5) & 255ull), cgi = (int)((meta >> 13) & 63ull);
+            const int src = (int)(meta & 31ull), ck = (int)((meta >> 5) & 255ull), cti = (int)((meta >> 13) & 63ull);
             const int b1 = (int)((meta >> 19) & 2047ull), b2 = (int)((meta >> 30) & 2047ull);
             double sp[3], sk3[3];
 #pragma unroll
@@ -461,7 +504,7 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
                 const int n2 = P.g.n * P.g.n;
                 q.cell[0][w] = (unsigned)(sxy1 + n2 * b1); q.cell[1][w] = (unsigned)(sxy2 + n2 * b2); q.cell[2][w] = (unsigned)si3; q.cell[3][w] = (unsigned)si;
                 q.s[w] = rt.s; q.t[w] = rt.t; q.u[w] = rt.u; q.w_inv[w] = rt.w_inv;
-                q.rgi[w] = (unsigned char)cgi;
+                q.rti[w] = (unsigned char)cti;
             }
             count += __popc(has);
             chead = (chead + nb) & (kQCand - 1);
@@ -481,7 +524,7 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
             const bool last = ti == ntup;
             const bool solve = !last;
             const unsigned tu = q.tup[solve ? ti : 0];
-            const int ck = (int)(tu & 0xffffu), gi = (int)(tu >> 16);
+            const int ck = (int)(tu & 0xffffu);
             if (solve) {
                 // stage 1 for every lane: 0.14-0.16 candidates per lane and tuple pass the box test
                 double zr[2];
@@ -494,7 +537,7 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
                     if (mine) {
                         const int w = (chead + ccount + __popc(has & lt)) & (kQCand - 1);
                         q.cz[w] = zr[r];
-                        q.cmeta[w] = (unsigned long long)lane | (unsigned long long)ck << 5 | (unsigned long long)gi << 13 |
+                        q.cmeta[w] = (unsigned long long)lane | (unsigned long long)ck << 5 | (unsigned long long)ti << 13 |
                                      (unsigned long long)b1r[r] << 19 | (unsigned long long)b2r[r] << 30;
                     }
                     ccount += __popc(has);
@@ -537,14 +580,28 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
     if (total <= 0) return cudaSuccess;
     if (P.n_groups > 64) return cudaErrorInvalidValue;       // the records carry a 64-bit mask of channel groups (7 species: 40)
+    if (P.n_channels > 128) return cudaErrorInvalidValue;    // the per-tuple channel lists hold byte indices into the table
+    const size_t smem = sizeof(QWarp) * kQWarps;
+    // the attribute belongs to the (function, device) pair: one flag per device, not per process
+    static bool configured[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+        e = cudaFuncSetAttribute(paper_queue_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(paper_queue_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
+    }
     int per_sm = 1;                      // only the CTAs resident at once: the warps in flight stay within a few spatial cells
-    if (P.all_massless) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<true>, 32 * kQWarps, 0);
-    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<false>, 32 * kQWarps, 0);
+    if (P.all_massless) cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<true>, 32 * kQWarps, smem);
+    else cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, paper_queue_kernel<false>, 32 * kQWarps, smem);
     if (per_sm < 1) per_sm = 1;
     long long blocks = (total / 32 + kQWarps) / kQWarps;
     if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
-    if (P.all_massless) paper_queue_kernel<true><<<(int)blocks, 32 * kQWarps, 0, st>>>(P);
-    else paper_queue_kernel<false><<<(int)blocks, 32 * kQWarps, 0, st>>>(P);
+    if (P.all_massless) paper_queue_kernel<true><<<(int)blocks, 32 * kQWarps, smem, st>>>(P);
+    else paper_queue_kernel<false><<<(int)blocks, 32 * kQWarps, smem, st>>>(P);
     ++g_launch_count;
     return cudaGetLastError();
 }
