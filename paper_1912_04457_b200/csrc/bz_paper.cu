@@ -289,88 +289,113 @@ struct QWarp {                         // per warp, in dynamic shared memory (9.
     int pre[33];
 };
 
-// not inlined: three call sites, and the kernel's code has to fit the instruction cache (ncu: stall_no_instruction)
-template <bool kAllMassless>
-__device__ __noinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
+// Every mass is zero (no bz_thermal_masses / bz_set_masses call yet): one tuple, the root serves ALL channels, and their sum is
+// the hot path's factorised algebra (bz_channels.cuh) on the four cells -- 4 x S loads and reductions per root instead of 4
+// per channel.  (A separate kernel instantiation: inlined into the general kernel it cost that one 40 %.)
+__device__ __noinline__ void paper_deposit_massless(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
 {
-    const bool on = lane < nb;
+    if (lane >= nb) return;
     const int r = (head + lane) & (kQRing - 1);
     const double* fx = P.f + (size_t)xcell * P.S * P.Np;
     double* dx = P.dN + (size_t)xcell * P.S * P.Np;
-    MsqSet M = {};
-    if (on) {
-        const double w = P.Kp / q.w_inv[r];
-        M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
-        if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+    const double w = P.Kp / q.w_inv[r];
+    MsqSet M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
+    if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
+    const unsigned c1 = q.cell[0][r], c2 = q.cell[1][r], c3 = q.cell[2][r], c4 = q.cell[3][r];
+    double fv[4][7], d[4][7];
+#pragma unroll
+    for (int id = 0; id < 7; ++id) {
+        const int a = P.slot[id];
+        fv[0][id] = a >= 0 ? fx[(size_t)a * P.Np + c1] : 0.0; fv[1][id] = a >= 0 ? fx[(size_t)a * P.Np + c2] : 0.0;
+        fv[2][id] = a >= 0 ? fx[(size_t)a * P.Np + c3] : 0.0; fv[3][id] = a >= 0 ? fx[(size_t)a * P.Np + c4] : 0.0;
     }
-    if constexpr (kAllMassless) {
-        // every mass is zero (no bz_thermal_masses / bz_set_masses call yet): one tuple, the root serves ALL channels, and their sum
-        // is the hot path's factorised algebra (bz_channels.cuh) on the four cells -- 4 x S loads and reductions per root
-        // instead of 4 per channel.  (A separate instantiation: inlined into the general kernel it cost that one 40 %.)
-        if (!on) return;
-        const unsigned c1 = q.cell[0][r], c2 = q.cell[1][r], c3 = q.cell[2][r], c4 = q.cell[3][r];
-        double fv[4][7], d[4][7];
+    deposit<-1>(P.mask, fv[0], fv[1], fv[2], fv[3], M, d[0], d[1], d[2], d[3]);
 #pragma unroll
-        for (int id = 0; id < 7; ++id) {
-            const int a = P.slot[id];
-            fv[0][id] = a >= 0 ? fx[(size_t)a * P.Np + c1] : 0.0; fv[1][id] = a >= 0 ? fx[(size_t)a * P.Np + c2] : 0.0;
-            fv[2][id] = a >= 0 ? fx[(size_t)a * P.Np + c3] : 0.0; fv[3][id] = a >= 0 ? fx[(size_t)a * P.Np + c4] : 0.0;
+    for (int id = 0; id < 7; ++id) {
+        const int a = P.slot[id];
+        if (a < 0) continue;
+        if (d[0][id] != 0.0) red_add(dx + (size_t)a * P.Np + c1, d[0][id]);
+        if (d[1][id] != 0.0) red_add(dx + (size_t)a * P.Np + c2, d[1][id]);
+        if (d[2][id] != 0.0) red_add(dx + (size_t)a * P.Np + c3, d[2][id]);
+        if (d[3][id] != 0.0) red_add(dx + (size_t)a * P.Np + c4, d[3][id]);
+    }
+}
+
+// With masses a root serves only the channels of its own mass tuple (7 on average on config 4, up to 90 when classes
+// coincide).  Lanes = roots for Table I (stored per root in shared memory), then lanes = (root, channel) pairs of the whole
+// batch, flattened through a prefix sum of the roots' channel counts: every pair costs 4 loads, the bracket of Eq. 5 and 4
+// reductions, with no lane waiting for another root's longer channel list.
+// Not inlined (three call sites; the kernel's code has to fit the instruction cache, ncu: stall_no_instruction) and with
+// scalar arguments: a reference to the kernel's parameter struct would make the callee read it back from local memory.
+__device__ __noinline__ void paper_deposit_pairs(QWarp& q, int lane, int head, int nb, const double* __restrict__ fx, double* __restrict__ dx,
+                                                 const unsigned long long* __restrict__ table, size_t Np, double Kp, double g4, double mreg,
+                                                 const double* ovr /* 7 user-defined |M|^2 / g^4, or NULL */)
+{
+    const unsigned full = 0xffffffffu;
+    const bool on = lane < nb;
+    const int r = (head + lane) & (kQRing - 1);
+    int cnt = 0;
+    if (on) {
+        const double w = Kp / q.w_inv[r];
+        MsqSet M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, g4 * w);
+        if (ovr) {
+            double o7[7];
+#pragma unroll
+            for (int k = 0; k < 7; ++k) o7[k] = ovr[k];
+            msq_apply_override(M, o7, g4 * w);
         }
-        deposit<-1>(P.mask, fv[0], fv[1], fv[2], fv[3], M, d[0], d[1], d[2], d[3]);
+        const int ti = q.rti[r];
+        cnt = (int)q.choff[ti + 1] - (int)q.choff[ti];
+        q.mvs[0][lane] = M.a_t; q.mvs[1][lane] = M.a_u; q.mvs[2][lane] = M.m11; q.mvs[3][lane] = M.m11;
+        q.mvs[4][lane] = M.m1b_t; q.mvs[5][lane] = M.m1b_u; q.mvs[6][lane] = M.ann; q.mvs[7][lane] = M.ann;
+        q.mvs[8][lane] = M.qqgg; q.mvs[9][lane] = M.qqgg; q.mvs[10][lane] = M.qg_t; q.mvs[11][lane] = M.qg_u;
+        q.mvs[12][lane] = M.gg; q.mvs[13][lane] = M.gg;
+    }
+    int incl = cnt;
 #pragma unroll
-        for (int id = 0; id < 7; ++id) {
-            const int a = P.slot[id];
-            if (a < 0) continue;
-            if (d[0][id] != 0.0) red_add(dx + (size_t)a * P.Np + c1, d[0][id]);
-            if (d[1][id] != 0.0) red_add(dx + (size_t)a * P.Np + c2, d[1][id]);
-            if (d[2][id] != 0.0) red_add(dx + (size_t)a * P.Np + c3, d[2][id]);
-            if (d[3][id] != 0.0) red_add(dx + (size_t)a * P.Np + c4, d[3][id]);
-        }
-        return;
-    } else {
-        // With masses a root serves only the channels of its own mass tuple (3 on average with four distinct masses, up to 90
-        // when classes coincide).  Lanes = roots for Table I (stored per root in shared memory), then lanes = (root, channel)
-        // pairs of the whole batch, flattened through a prefix sum of the roots' channel counts: every pair costs 4 loads, the
-        // bracket of Eq. 5 and 4 reductions, with no lane waiting for another root's longer channel list.
-        const unsigned full = 0xffffffffu;
-        int cnt = 0;
-        if (on) {
-            const int ti = q.rti[r];
-            cnt = (int)q.choff[ti + 1] - (int)q.choff[ti];
-            q.mvs[0][lane] = M.a_t; q.mvs[1][lane] = M.a_u; q.mvs[2][lane] = M.m11; q.mvs[3][lane] = M.m11;
-            q.mvs[4][lane] = M.m1b_t; q.mvs[5][lane] = M.m1b_u; q.mvs[6][lane] = M.ann; q.mvs[7][lane] = M.ann;
-            q.mvs[8][lane] = M.qqgg; q.mvs[9][lane] = M.qqgg; q.mvs[10][lane] = M.qg_t; q.mvs[11][lane] = M.qg_u;
-            q.mvs[12][lane] = M.gg; q.mvs[13][lane] = M.gg;
-        }
-        int incl = cnt;
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, incl, o); if (lane >= o) incl += v; }
+    q.pre[lane + 1] = incl;
+    if (lane == 0) q.pre[0] = 0;
+    const int total = __shfl_sync(full, incl, 31);
+    __syncwarp();
+    for (int base = 0; base < total; base += 32) {
+        const int fl = base + lane;
+        if (fl < total) {
+            int lo = 0;                                   // the root that owns pair fl: the largest lo with pre[lo] <= fl
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(full, incl, o); if (lane >= o) incl += v; }
-        q.pre[lane + 1] = incl;
-        if (lane == 0) q.pre[0] = 0;
-        const int total = __shfl_sync(full, incl, 31);
-        __syncwarp();
-        for (int base = 0; base < total; base += 32) {
-            const int fl = base + lane;
-            if (fl < total) {
-                int lo = 0;                                   // the root that owns pair fl: the largest lo with pre[lo] <= fl
-#pragma unroll
-                for (int stp = 16; stp > 0; stp >>= 1) { if (q.pre[lo + stp] <= fl) lo += stp; }
-                const int rr = (head + lo) & (kQRing - 1);
-                const PaperChannel ch = P.table[q.chlist[(int)q.choff[q.rti[rr]] + (fl - q.pre[lo])]];
-                const unsigned c1 = q.cell[0][rr], c2 = q.cell[1][rr], c3 = q.cell[2][rr], c4 = q.cell[3][rr];
-                const size_t oa = (size_t)ch.a * P.Np + c1, ob = (size_t)ch.b * P.Np + c2, oc = (size_t)ch.c * P.Np + c3, od = (size_t)ch.d * P.Np + c4;
-                const double fa = fx[oa], fb = fx[ob], fc = fx[oc], fd = fx[od];
-                const double Fa = (ch.glue & 1) ? 1.0 + fa : 1.0 - fa, Fb = (ch.glue & 2) ? 1.0 + fb : 1.0 - fb;
-                const double Fc = (ch.glue & 4) ? 1.0 + fc : 1.0 - fc, Fd = (ch.glue & 8) ? 1.0 + fd : 1.0 - fd;
-                const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-                const double A = q.mvs[2 * ch.kind + ch.crossed][lo] * fwd;
-                if (A != 0.0) {
-                    red_add(dx + oa, -A); red_add(dx + ob, -A);                        // Eq. 22
-                    red_add(dx + oc, A);  red_add(dx + od, A);
-                }
+            for (int stp = 16; stp > 0; stp >>= 1) { if (q.pre[lo + stp] <= fl) lo += stp; }
+            const int rr = (head + lo) & (kQRing - 1);
+            // one 8-byte load of the channel: a | b << 8 | c << 16 | d << 24 | kind << 32 | crossed << 40 | glue << 48 (PaperChannel)
+            const unsigned long long ch = __ldg(table + q.chlist[(int)q.choff[q.rti[rr]] + (fl - q.pre[lo])]);
+            const unsigned lo32 = (unsigned)ch, hi32 = (unsigned)(ch >> 32);
+            const size_t oa = (size_t)(lo32 & 255u) * Np + q.cell[0][rr], ob = (size_t)((lo32 >> 8) & 255u) * Np + q.cell[1][rr];
+            const size_t oc = (size_t)((lo32 >> 16) & 255u) * Np + q.cell[2][rr], od = (size_t)(lo32 >> 24) * Np + q.cell[3][rr];
+            const double fa = fx[oa], fb = fx[ob], fc = fx[oc], fd = fx[od];
+            const unsigned glue = hi32 >> 16;
+            // F = 1 + f (gluon), 1 - f (quark): 1 + sign * f with sign = +-1 is the same rounded sum
+            const double Fa = fma((glue & 1u) ? 1.0 : -1.0, fa, 1.0), Fb = fma((glue & 2u) ? 1.0 : -1.0, fb, 1.0);
+            const double Fc = fma((glue & 4u) ? 1.0 : -1.0, fc, 1.0), Fd = fma((glue & 8u) ? 1.0 : -1.0, fd, 1.0);
+            const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
+            const double A = q.mvs[2 * (hi32 & 255u) + ((hi32 >> 8) & 255u)][lo] * fwd;
+            if (A != 0.0) {
+                red_add(dx + oa, -A); red_add(dx + ob, -A);                        // Eq. 22
+                red_add(dx + oc, A);  red_add(dx + od, A);
             }
         }
-        __syncwarp();                                        // the scratch is rewritten by the next batch
+    }
+    __syncwarp();                                        // the scratch is rewritten by the next batch
+}
+
+template <bool kAllMassless>
+__device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp& q, int lane, int head, int nb, int xcell, double mreg)
+{
+    if constexpr (kAllMassless) {
+        paper_deposit_massless(P, q, lane, head, nb, xcell, mreg);
+    } else {
+        static_assert(sizeof(PaperChannel) == 8, "PaperChannel is read as one 8-byte word");
+        const size_t tile = (size_t)xcell * P.S * P.Np;
+        paper_deposit_pairs(q, lane, head, nb, P.f + tile, P.dN + tile, reinterpret_cast<const unsigned long long*>(P.table), (size_t)P.Np,
+                            P.Kp, P.g4, mreg, P.has_ovr ? P.msq_ovr : nullptr);
     }
 }
 
@@ -378,7 +403,7 @@ template <bool kAllMassless>
 #ifndef BZ_PAPER_MINB
 #define BZ_PAPER_MINB 2
 #endif
-__global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB) paper_queue_kernel(const PaperParams P)
+__global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB) paper_queue_kernel(const __grid_constant__ PaperParams P)
 {
     extern __shared__ __align__(16) unsigned char paper_smem[];
     QWarp& q = reinterpret_cast<QWarp*>(paper_smem)[threadIdx.x >> 5];
