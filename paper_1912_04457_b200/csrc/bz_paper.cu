@@ -5,9 +5,9 @@
 //   Eq. 8-9; symmetrical sampling (Eq. 22): the same weight goes to the cells of k1, k2 (-) and k3, p (+).
 // With masses the kinematics depend on the species of the four legs, so a sample is NOT shared by all channels as in
 // the hot path: the ordered channels (S8c step 5) are grouped by their tuple of mass classes (g, u, d, s) and every
-// group solves its own roots.  One lane per (spatial cell, grid point, sample) for the root solving; the surviving roots
-// go through a per-warp queue to a second phase with one lane per root (paper_queue_kernel), whose deposits are issued as
-// fp64 reductions (RED.E.ADD.F64) into dF, which a second kernel divides by N_a.  Everything that decides a cell index
+// group solves its own roots.  One lane per (spatial cell, grid point, sample) for the first stage of the root solving; its
+// candidates, the kept roots and the (root, channel) pairs go through per-warp rings to later phases that run on full
+// warps (paper_queue_kernel); deposits are fp64 reductions (RED.E.ADD.F64) into dF, which a second kernel divides by N_a.  Everything that decides a cell index
 // uses single correctly rounded operations in the association order of the oracle (bit-exact sampled cells).
 #include <vector>
 
@@ -261,14 +261,22 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
 // Only 0.14-0.16 roots per mass tuple survive the box test.  History: a thread-per-sample kernel walked the channel loop of
 // every tuple with 6 of 32 lanes active; a warp-cooperative version (the owner of a surviving root publishes it, the
 // whole warp works its channels off) fixed that for the massless case (one tuple, 127 channels) but with four distinct
-// masses a tuple has ~3 channels, so 29 lanes idled and every root cost a shared-memory column reduction: 0.010 of the
-// FP64 peak on config 4 (ncu: 16 of 32 lanes active, 23 % occupancy).  Here the two phases are decoupled through a queue:
-//   solve    lanes = samples, warp-uniform loop over the distinct mass tuples of the spatial cell; E3 and Ep are computed
-//            once per mass class (4 + 4 square roots per sample instead of 2 per tuple); every surviving root is appended
-//            to the warp's ring of 64 records in shared memory (ballot + prefix): cells of k1, k2, k3, p, (s, t, u),
-//            |J| E1 E2 E3 Ep and the bit mask of the channel groups that share the tuple.
-//   deposit  whenever the ring holds 32 records: lanes = roots; Table I at the root's massive s, t, u, then the lane
-//            walks the channels of its tuple: 4 loads, the bracket of Eq. 5, 4 reductions (RED.E.ADD.F64) per channel.
+// masses a tuple has few channels, so 29 lanes idled and every root cost a shared-memory column reduction: 0.010 of the
+// FP64 peak on config 4 (ncu: 16 of 32 lanes active, 23 % occupancy).  Here every phase whose survivors are sparse hands
+// them to the next one through a ring in shared memory, so that each phase runs on full warps:
+//   stage 1  lanes = samples, warp-uniform loop over the distinct (canonical) mass tuples of the spatial cell, listed once
+//            per spatial cell; E3 and Ep once per mass class (4 + 4 square roots per sample instead of 2 per tuple); the
+//            quadratic for k1z and the box test of the z components (guarded fast binning).  Candidates (z, source lane,
+//            tuple, z cells) go to the candidate ring.
+//   stage 2  whenever 32 candidates wait (and at the end of the pass: they refer to the pass's samples): lanes =
+//            candidates, the sample comes from the source lane by shuffles; E1, E2, the Jacobian, (s, t, u).  Kept roots go
+//            to the ring of root records: cells of k1, k2, k3, p, (s, t, u), |J| E1 E2 E3 Ep, tuple.
+//   deposit  whenever 32 roots wait: lanes = roots for Table I at the root's massive (s, t, u), stored per root in shared
+//            memory; then lanes = (root, channel) pairs of the whole batch (prefix sum of the roots' channel counts, the
+//            tuples' channel lists built once per spatial cell): 4 loads, the bracket of Eq. 5, 4 reductions per pair.
+// ncu on the first queue version showed stall_no_instruction as large as the memory stalls: the kernel was 63-88 KB of
+// code.  Stage 2 is therefore expanded at one place only and the deposit is a non-inlined function with scalar arguments
+// (kernel parameters are __grid_constant__: no local copy); that alone was worth 15 %.
 constexpr int kQWarps = 8, kQRing = 64, kQCand = 128;
 struct QWarp {                         // per warp, in dynamic shared memory (9.6 KB)
     unsigned cell[4][kQRing];          // root records: cells of k1, k2, k3, p
