@@ -671,7 +671,7 @@ static int paper_params(bz_ctx* c, double dt_fm, unsigned step, PaperParams& P)
         c->paper_n_groups = (int)groups.size(); c->paper_n_channels = (int)table.size();
     }
     P.g = grid_const(c);
-    P.f = c->f; P.dN = nullptr; P.mass2 = c->mass2; P.table = c->paper_table; P.groups = c->paper_groups;
+    P.f = c->SP == 1 ? c->f : c->f_aos; P.dN = c->dN_aos; P.SP = c->SP; P.mass2 = c->mass2; P.table = c->paper_table; P.groups = c->paper_groups;
     P.n_groups = c->paper_n_groups; P.n_channels = c->paper_n_channels; P.S = c->S; P.Np = c->Np; P.Ns = c->Ns;
     const int layer = c->grid.nx * c->grid.ny;
     P.x_begin = c->zb * layer; P.x_count = (c->ze - c->zb) * layer; P.p_begin = 0; P.p_count = c->Np;
@@ -698,14 +698,17 @@ int bz_collision_paper(bz_ctx* c, double dt_fm, unsigned step, double* dF_dev)
     if (!c || !dF_dev) return -1;
     if (!c->f) return -4;
     BZ_ON_DEVICE(c);
+    // gathers from the cell-major copy of f and deposits into the cell-major scratch, like the hot path (run_collide)
+    if (c->SP != 1 && !c->aos_valid) {
+        BZ_CUDA(launch_pack(c->f, c->f_aos, c->Nx, c->S, c->SP, c->Np, c->stream), "pack");
+        c->aos_valid = true;
+    }
     PaperParams P;
     if (int rc = paper_params(c, dt_fm, step, P)) return rc;
-    P.dN = dF_dev;
-    BZ_CUDA(cudaMemsetAsync(dF_dev, 0, c->n_values * sizeof(double), c->stream), "memset dF");
     BZ_CUDA(launch_paper_collide(P, c->sms, c->stream), "paper collide");
     double deg[7];
     fill_deg(c, deg);
-    BZ_CUDA(launch_paper_finalize(dF_dev, c->n_values, c->S, c->Np, deg, c->stream), "paper finalize");
+    BZ_CUDA(launch_finalize(c->dN_aos, dF_dev, c->Nx, c->S, c->SP, c->Np, deg, c->stream), "finalize");   // dF = dN / N_a, scratch back to 0
     return 0;
 }
 

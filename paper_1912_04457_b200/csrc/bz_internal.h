@@ -47,8 +47,9 @@ struct PaperChannel { unsigned char a, b, c, d, kind, crossed, glue /* bit s: le
 struct PaperGroup { int key, begin, end; };
 struct PaperParams {
     GridConst g;
-    const double* f;          // [Nx][S][Np]
-    double* dN;               // [Nx][S][Np] deposits in number units (the caller's dF, zeroed before the launch)
+    const double* f;          // cell-major copy of f, [Nx][Np][SP] (the collision kernel's gather source f_aos; f itself if SP == 1)
+    double* dN;               // cell-major deposit scratch dN_aos [Nx][Np][SP], number units, zero before the launch
+    int SP;                   // doubles per cell in the two: 1 (one species) or 8
     const double* mass2;      // [Nx][4] thermal masses^2 (Eq. 8-9)
     const PaperChannel* table;
     const PaperGroup* groups;
@@ -182,6 +183,5 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, int sms, cudaStream_t st);
 // out = (f + out) + dFc (forward Euler with both increments given, the oracle's association)
 cudaError_t launch_combine(const double* f, double* out, const double* dFc, size_t n_values, cudaStream_t st);
-cudaError_t launch_paper_finalize(double* dF, size_t n_values, int S, int Np, const double* deg, cudaStream_t st);
 
 }  // namespace bz

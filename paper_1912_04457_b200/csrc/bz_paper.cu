@@ -304,8 +304,8 @@ __device__ __noinline__ void paper_deposit_massless(const PaperParams& P, QWarp&
 {
     if (lane >= nb) return;
     const int r = (head + lane) & (kQRing - 1);
-    const double* fx = P.f + (size_t)xcell * P.S * P.Np;
-    double* dx = P.dN + (size_t)xcell * P.S * P.Np;
+    const double* fx = P.f + (size_t)xcell * P.Np * P.SP;                 // cell-major: the S values of a cell are adjacent
+    double* dx = P.dN + (size_t)xcell * P.Np * P.SP;
     const double w = P.Kp / q.w_inv[r];
     MsqSet M = msq_set<true, true>(q.s[r], q.t[r], q.u[r], mreg, P.g4 * w);
     if (P.has_ovr) msq_apply_override(M, P.msq_ovr, P.g4 * w);
@@ -314,18 +314,18 @@ __device__ __noinline__ void paper_deposit_massless(const PaperParams& P, QWarp&
 #pragma unroll
     for (int id = 0; id < 7; ++id) {
         const int a = P.slot[id];
-        fv[0][id] = a >= 0 ? fx[(size_t)a * P.Np + c1] : 0.0; fv[1][id] = a >= 0 ? fx[(size_t)a * P.Np + c2] : 0.0;
-        fv[2][id] = a >= 0 ? fx[(size_t)a * P.Np + c3] : 0.0; fv[3][id] = a >= 0 ? fx[(size_t)a * P.Np + c4] : 0.0;
+        fv[0][id] = a >= 0 ? fx[(size_t)c1 * P.SP + a] : 0.0; fv[1][id] = a >= 0 ? fx[(size_t)c2 * P.SP + a] : 0.0;
+        fv[2][id] = a >= 0 ? fx[(size_t)c3 * P.SP + a] : 0.0; fv[3][id] = a >= 0 ? fx[(size_t)c4 * P.SP + a] : 0.0;
     }
     deposit<-1>(P.mask, fv[0], fv[1], fv[2], fv[3], M, d[0], d[1], d[2], d[3]);
 #pragma unroll
     for (int id = 0; id < 7; ++id) {
         const int a = P.slot[id];
         if (a < 0) continue;
-        if (d[0][id] != 0.0) red_add(dx + (size_t)a * P.Np + c1, d[0][id]);
-        if (d[1][id] != 0.0) red_add(dx + (size_t)a * P.Np + c2, d[1][id]);
-        if (d[2][id] != 0.0) red_add(dx + (size_t)a * P.Np + c3, d[2][id]);
-        if (d[3][id] != 0.0) red_add(dx + (size_t)a * P.Np + c4, d[3][id]);
+        if (d[0][id] != 0.0) red_add(dx + (size_t)c1 * P.SP + a, d[0][id]);
+        if (d[1][id] != 0.0) red_add(dx + (size_t)c2 * P.SP + a, d[1][id]);
+        if (d[2][id] != 0.0) red_add(dx + (size_t)c3 * P.SP + a, d[2][id]);
+        if (d[3][id] != 0.0) red_add(dx + (size_t)c4 * P.SP + a, d[3][id]);
     }
 }
 
@@ -336,7 +336,7 @@ __device__ __noinline__ void paper_deposit_massless(const PaperParams& P, QWarp&
 // Not inlined (three call sites; the kernel's code has to fit the instruction cache, ncu: stall_no_instruction) and with
 // scalar arguments: a reference to the kernel's parameter struct would make the callee read it back from local memory.
 __device__ __noinline__ void paper_deposit_pairs(QWarp& q, int lane, int head, int nb, const double* __restrict__ fx, double* __restrict__ dx,
-                                                 const unsigned long long* __restrict__ table, size_t Np, double Kp, double g4, double mreg,
+                                                 const unsigned long long* __restrict__ table, unsigned SP, double Kp, double g4, double mreg,
                                                  const double* ovr /* 7 user-defined |M|^2 / g^4, or NULL */)
 {
     const unsigned full = 0xffffffffu;
@@ -376,8 +376,10 @@ __device__ __noinline__ void paper_deposit_pairs(QWarp& q, int lane, int head, i
             // one 8-byte load of the channel: a | b << 8 | c << 16 | d << 24 | kind << 32 | crossed << 40 | glue << 48 (PaperChannel)
             const unsigned long long ch = __ldg(table + q.chlist[(int)q.choff[q.rti[rr]] + (fl - q.pre[lo])]);
             const unsigned lo32 = (unsigned)ch, hi32 = (unsigned)(ch >> 32);
-            const size_t oa = (size_t)(lo32 & 255u) * Np + q.cell[0][rr], ob = (size_t)((lo32 >> 8) & 255u) * Np + q.cell[1][rr];
-            const size_t oc = (size_t)((lo32 >> 16) & 255u) * Np + q.cell[2][rr], od = (size_t)(lo32 >> 24) * Np + q.cell[3][rr];
+            // cell-major gather source and deposit scratch (f_aos, dN_aos): the pairs of one root sit in neighbouring lanes and
+            // touch the same four 64-byte cells, so their loads and reductions share sectors
+            const size_t oa = (size_t)q.cell[0][rr] * SP + (lo32 & 255u), ob = (size_t)q.cell[1][rr] * SP + ((lo32 >> 8) & 255u);
+            const size_t oc = (size_t)q.cell[2][rr] * SP + ((lo32 >> 16) & 255u), od = (size_t)q.cell[3][rr] * SP + (lo32 >> 24);
             const double fa = fx[oa], fb = fx[ob], fc = fx[oc], fd = fx[od];
             const unsigned glue = hi32 >> 16;
             // F = 1 + f (gluon), 1 - f (quark): 1 + sign * f with sign = +-1 is the same rounded sum
@@ -401,8 +403,8 @@ __device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp&
         paper_deposit_massless(P, q, lane, head, nb, xcell, mreg);
     } else {
         static_assert(sizeof(PaperChannel) == 8, "PaperChannel is read as one 8-byte word");
-        const size_t tile = (size_t)xcell * P.S * P.Np;
-        paper_deposit_pairs(q, lane, head, nb, P.f + tile, P.dN + tile, reinterpret_cast<const unsigned long long*>(P.table), (size_t)P.Np,
+        const size_t tile = (size_t)xcell * P.Np * P.SP;
+        paper_deposit_pairs(q, lane, head, nb, P.f + tile, P.dN + tile, reinterpret_cast<const unsigned long long*>(P.table), (unsigned)P.SP,
                             P.Kp, P.g4, mreg, P.has_ovr ? P.msq_ovr : nullptr);
     }
 }
@@ -583,15 +585,6 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
     while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
 }
 
-__global__ void __launch_bounds__(256) paper_finalize_kernel(double* __restrict__ dF, size_t n_values, int S, int Np, const double d0,
-                                                              const double d1, const double d2, const double d3, const double d4,
-                                                              const double d5, const double d6)
-{
-    const double deg[7] = { d0, d1, d2, d3, d4, d5, d6 };
-    for (size_t q = blockIdx.x * (size_t)blockDim.x + threadIdx.x; q < n_values; q += (size_t)gridDim.x * blockDim.x)
-        dF[q] = dF[q] / deg[(q / Np) % S];
-}
-
 __global__ void __launch_bounds__(256) combine_kernel(const double* __restrict__ f, double* __restrict__ out,
                                                       const double* __restrict__ dFc, size_t n_values)
 {
@@ -646,13 +639,6 @@ cudaError_t launch_paper_debug(const PaperParams& P, int* cells, double* stu, in
     long long blocks = (total + kPaperThreads - 1) / kPaperThreads;
     if (blocks > (long long)sms * 32) blocks = (long long)sms * 32;
     paper_debug_kernel<<<(int)blocks, kPaperThreads, 0, st>>>(P, cells, stu);
-    ++g_launch_count;
-    return cudaGetLastError();
-}
-
-cudaError_t launch_paper_finalize(double* dF, size_t n_values, int S, int Np, const double* deg, cudaStream_t st)
-{
-    paper_finalize_kernel<<<148 * 8, 256, 0, st>>>(dF, n_values, S, Np, deg[0], deg[1], deg[2], deg[3], deg[4], deg[5], deg[6]);
     ++g_launch_count;
     return cudaGetLastError();
 }
