@@ -230,7 +230,6 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
         const double k1x = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[2], w1[3]), P.g.L));
         const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
         const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
-        const double* m = P.mass2 + 4 * (size_t)xcell;
         // transverse cells of k1 (inside by construction) and of k2 = k3 + p - k1: the same for every mass tuple and root;
         // a sample whose k2x or k2y leaves the box deposits nothing whatever the masses are (S9)
         int ixy1, ixy2;
@@ -264,7 +263,9 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
 // masses a tuple has few channels, so 29 lanes idled and every root cost a shared-memory column reduction: 0.010 of the
 // FP64 peak on config 4 (ncu: 16 of 32 lanes active, 23 % occupancy).  Here every phase whose survivors are sparse hands
 // them to the next one through a ring in shared memory, so that each phase runs on full warps:
-//   stage 1  lanes = samples, warp-uniform loop over the distinct (canonical) mass tuples of the spatial cell, listed once
+//   samples  32 samples per pass (Philox, k3, k1x, k1y, the cells that depend on neither masses nor roots); the ~45 % whose k3,
+//            k2x, k2y are inside the box go to the sample ring.
+//   stage 1  whenever 32 live samples wait: lanes = samples, warp-uniform loop over the distinct (canonical) mass tuples of the spatial cell, listed once
 //            per spatial cell; E3 and Ep once per mass class (4 + 4 square roots per sample instead of 2 per tuple); the
 //            quadratic for k1z and the box test of the z components (guarded fast binning).  Candidates (z, source lane,
 //            tuple, z cells) go to the candidate ring.
@@ -278,7 +279,7 @@ __global__ void __launch_bounds__(kPaperThreads) paper_debug_kernel(const PaperP
 // code.  Stage 2 is therefore expanded at one place only and the deposit is a non-inlined function with scalar arguments
 // (kernel parameters are __grid_constant__: no local copy); that alone was worth 15 %.
 constexpr int kQWarps = 8, kQRing = 64, kQCand = 128;
-struct QWarp {                         // per warp, in dynamic shared memory (9.6 KB)
+struct QWarp {                         // per warp, in dynamic shared memory (13.7 KB)
     unsigned cell[4][kQRing];          // root records: cells of k1, k2, k3, p
     double s[kQRing], t[kQRing], u[kQRing], w_inv[kQRing];
     unsigned char rti[kQRing];         // the record's canonical mass tuple (index into tup / choff)
@@ -292,8 +293,12 @@ struct QWarp {                         // per warp, in dynamic shared memory (9.
     // candidates of stage 1 waiting for stage 2 (they refer to the samples the warp's lanes hold at the moment):
     double cz[kQCand];                 // z component of k1 (a tuple adds at most 64 candidates to fewer than 32 waiting ones)
     unsigned long long cmeta[kQCand];  // source lane | canonical tuple key << 5 | tuple index << 13 | z cell of k1 << 19 | z cell of k2 << 30
+    // samples that can deposit at all (k3 and the transverse components of k1, k2 inside the box: about half), compacted over
+    // the sampling passes so that stage 1 runs on full warps: p, k3, k1x, k1y and the cells
+    double sv[8][kQRing];
+    int si[4][kQRing];                 // transverse cell parts of k1 and k2, cell of k3, cell of p
     // deposit scratch: Table I of the 32 roots of a batch, [2 kind + crossed][root], and the running channel counts
-    double mvs[14][32];
+    double mvs[10][32];                // a_t, a_u, m11, m1b_t, m1b_u, ann, qqgg, qg_t, qg_u, gg
     int pre[33];
 };
 
@@ -354,10 +359,8 @@ __device__ __noinline__ void paper_deposit_pairs(QWarp& q, int lane, int head, i
         }
         const int ti = q.rti[r];
         cnt = (int)q.choff[ti + 1] - (int)q.choff[ti];
-        q.mvs[0][lane] = M.a_t; q.mvs[1][lane] = M.a_u; q.mvs[2][lane] = M.m11; q.mvs[3][lane] = M.m11;
-        q.mvs[4][lane] = M.m1b_t; q.mvs[5][lane] = M.m1b_u; q.mvs[6][lane] = M.ann; q.mvs[7][lane] = M.ann;
-        q.mvs[8][lane] = M.qqgg; q.mvs[9][lane] = M.qqgg; q.mvs[10][lane] = M.qg_t; q.mvs[11][lane] = M.qg_u;
-        q.mvs[12][lane] = M.gg; q.mvs[13][lane] = M.gg;
+        q.mvs[0][lane] = M.a_t; q.mvs[1][lane] = M.a_u; q.mvs[2][lane] = M.m11; q.mvs[3][lane] = M.m1b_t; q.mvs[4][lane] = M.m1b_u;
+        q.mvs[5][lane] = M.ann; q.mvs[6][lane] = M.qqgg; q.mvs[7][lane] = M.qg_t; q.mvs[8][lane] = M.qg_u; q.mvs[9][lane] = M.gg;
     }
     int incl = cnt;
 #pragma unroll
@@ -386,7 +389,8 @@ __device__ __noinline__ void paper_deposit_pairs(QWarp& q, int lane, int head, i
             const double Fa = fma((glue & 1u) ? 1.0 : -1.0, fa, 1.0), Fb = fma((glue & 2u) ? 1.0 : -1.0, fb, 1.0);
             const double Fc = fma((glue & 4u) ? 1.0 : -1.0, fc, 1.0), Fd = fma((glue & 8u) ? 1.0 : -1.0, fd, 1.0);
             const double fwd = fa * fb * Fc * Fd - Fa * Fb * fc * fd;             // Eq. 5 bracket
-            const double A = q.mvs[2 * (hi32 & 255u) + ((hi32 >> 8) & 255u)][lo] * fwd;
+            // row of Table I: first row of the kind (A 0, 11 2, 1B 3, ANN 5, QQGG 6, QG 7, GG 9) + 1 if crossed (kinds A, 1B, QG only)
+            const double A = q.mvs[((0x9765320u >> (4u * (hi32 & 255u))) & 15u) + ((hi32 >> 8) & 255u)][lo] * fwd;
             if (A != 0.0) {
                 red_add(dx + oa, -A); red_add(dx + ob, -A);                        // Eq. 22
                 red_add(dx + oc, A);  red_add(dx + od, A);
@@ -421,23 +425,162 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
     const long long per_x = (long long)P.p_count * P.Ns;
     const long long chunks_per_x = (per_x + 31) / 32;
-    const long long n_items = chunks_per_x * P.x_count;
-    const long long warp0 = (blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5, n_warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    int head = 0, count = 0, cur_x = -1;
-    int chead = 0, ccount = 0;          // ring of stage-1 candidates (empty between sampling passes)
-    unsigned rep = 0u;
+    // Spatial cells go round-robin to up to 8 groups of CTAs, the chunks of a cell are strided over the warps of its group: a
+    // warp stays in one spatial cell for 1/8 of the launch's warps' share of it (its rings are drained only when it leaves),
+    // and the cells in flight (8 x 1.7 MB of f_aos + dN_aos tiles on config 4) stay in L2.
+    const int G = min(min(8, P.x_count), (int)gridDim.x);
+    const int grp = (int)blockIdx.x % G;
+    const long long wg = (long long)(blockIdx.x / G) * kQWarps + (threadIdx.x >> 5);
+    const long long Wg = (long long)((gridDim.x - grp + G - 1) / G) * kQWarps;
+    int head = 0, count = 0;            // ring of root records
+    int chead = 0, ccount = 0;          // ring of stage-1 candidates (empty between solving passes)
+    int shead = 0, scount = 0;          // ring of samples that can deposit
+    int cur_x = -1;
     double mreg = 0.0;
-    for (long long item = warp0; item < n_items; item += n_warps) {
-        const int xcell = P.x_begin + (int)(item / chunks_per_x);
-        const double* m = P.mass2 + 4 * (size_t)xcell;
-        if (xcell != cur_x) {                              // warp-uniform: a warp's items are consecutive
-            // records never mix spatial cells: flush what the previous cell left
+    int xi = grp;                       // the warp's next chunk: chunk cnk of the xi-th spatial cell of the launch
+    long long cnk = wg;
+    // Three things a trip of this loop can do, each written once (the kernel's code has to fit the instruction cache):
+    // generate 32 samples of the current spatial cell and keep the live ones; solve a warp of live samples; move on to the
+    // next spatial cell (the rings never mix spatial cells: they are drained first).
+    for (;;) {
+        const bool have = xi < P.x_count && wg < chunks_per_x;
+        const int xnext = have ? P.x_begin + xi : -2;
+        if (have && xnext == cur_x && scount < 32) {
+            // ---- generate: the five integration variables of Eq. 20 (Philox blocks 64, 65, 66; the CM sampler owns 0..63) and
+            // the cells that depend on neither masses nor roots; a sample whose k3, k2x or k2y leaves the box deposits nothing (S9)
+            const long long local = cnk * 32 + lane;
+            const bool valid = local < per_x;
+            const long long lc = valid ? local : per_x - 1;
+            const int smp = (int)(lc % P.Ns), i = P.p_begin + (int)(lc / P.Ns);
+            double p[3], Emassless;
+            cell_kinematics(P.g, i, p[0], p[1], p[2], Emassless);
+            uint32_t w0[4], w1[4], w2[4];
+            const uint32_t xc = (uint32_t)cur_x + P.x_rng_offset;
+            philox4x32_10(64u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w0);
+            philox4x32_10(65u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w1);
+            philox4x32_10(66u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w2);
+            double k3[3];
+            k3[0] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[0], w0[1]), P.g.L));
+            k3[1] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[2], w0[3]), P.g.L));
+            k3[2] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[0], w1[1]), P.g.L));
+            const double k1x = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[2], w1[3]), P.g.L));
+            const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
+            const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
+            bool ia, ib, ic, id;
+            const int a1 = bin_axis_exact(k1x, P.g, ia), b1 = bin_axis_exact(k1y, P.g, ib);
+            const double qx = __dsub_rn(__dadd_rn(k3[0], p[0]), k1x), qy = __dsub_rn(__dadd_rn(k3[1], p[1]), k1y);
+            const int a2 = bin_axis_exact(qx, P.g, ic), b2 = bin_axis_exact(qy, P.g, id);
+            const bool live = valid && i3 >= 0 && ia && ib && ic && id;
+            const unsigned lm = __ballot_sync(full, live);
+            if (live) {
+                const int w = (shead + scount + __popc(lm & lt)) & (kQRing - 1);
+                q.sv[0][w] = p[0]; q.sv[1][w] = p[1]; q.sv[2][w] = p[2]; q.sv[3][w] = k3[0]; q.sv[4][w] = k3[1]; q.sv[5][w] = k3[2];
+                q.sv[6][w] = k1x; q.sv[7][w] = k1y;
+                q.si[0][w] = a1 + P.g.n * b1; q.si[1][w] = a2 + P.g.n * b2; q.si[2][w] = i3; q.si[3][w] = i;
+            }
+            scount += __popc(lm);
+            cnk += Wg;
+            if (cnk >= chunks_per_x) { cnk = wg; xi += G; }
+            __syncwarp();
+            continue;
+        }
+        if (scount > 0) {
+            // ---- solve: lanes = live samples (a full warp unless the spatial cell or the launch ends)
+            const int ns = min(scount, 32);
+            const bool live = lane < ns;
+            const int sr = (shead + (live ? lane : 0)) & (kQRing - 1);
+            double p[3], k3[3];
+            p[0] = q.sv[0][sr]; p[1] = q.sv[1][sr]; p[2] = q.sv[2][sr]; k3[0] = q.sv[3][sr]; k3[1] = q.sv[4][sr]; k3[2] = q.sv[5][sr];
+            const double k1x = q.sv[6][sr], k1y = q.sv[7][sr];
+            const int ixy1 = q.si[0][sr], ixy2 = q.si[1][sr], i3 = q.si[2][sr], i = q.si[3][sr];
+            shead = (shead + ns) & (kQRing - 1);
+            scount -= ns;
+            // energies of the outgoing legs, once per mass class (the roots of a tuple take E3 of its third, Ep of its fourth class)
+            const PaperLegs L(p, k3, q.msm);
+            // stage 2 for candidates [chead, chead + nb): lanes = candidates; the sample a candidate belongs to lives in the registers
+            // of its source lane and comes over by shuffles; E3 and Ep are recomputed with PaperLegs' operations (the same bits)
+            auto stage2_batch = [&](int nb) {
+                const bool on = lane < nb;
+                const int cr = (chead + lane) & (kQCand - 1);
+                const unsigned long long meta = on ? q.cmeta[cr] : (unsigned long long)lane;
+                const double z = on ? q.cz[cr] : 0.0;
+                const int src = (int)(meta & 31ull), ck = (int)((meta >> 5) & 255ull), cti = (int)((meta >> 13) & 63ull);
+                const int b1 = (int)((meta >> 19) & 2047ull), b2 = (int)((meta >> 30) & 2047ull);
+                double sp[3], sk3[3];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { sp[d] = __shfl_sync(full, p[d], src); sk3[d] = __shfl_sync(full, k3[d], src); }
+                const double sk1x = __shfl_sync(full, k1x, src), sk1y = __shfl_sync(full, k1y, src);
+                const int sxy1 = __shfl_sync(full, ixy1, src), sxy2 = __shfl_sync(full, ixy2, src);
+                const int si3 = __shfl_sync(full, i3, src), si = __shfl_sync(full, i, src);
+                bool kept = false;
+                Root rt;
+                if (on) {
+                    const double m1 = q.msm[ck & 3], m2 = q.msm[(ck >> 2) & 3], m3 = q.msm[(ck >> 4) & 3], m4 = q.msm[(ck >> 6) & 3];
+                    const double kk = __dadd_rn(__dadd_rn(__dmul_rn(sk3[0], sk3[0]), __dmul_rn(sk3[1], sk3[1])), __dmul_rn(sk3[2], sk3[2]));
+                    const double pp = __dadd_rn(__dadd_rn(__dmul_rn(sp[0], sp[0]), __dmul_rn(sp[1], sp[1])), __dmul_rn(sp[2], sp[2]));
+                    const double E3 = __dsqrt_rn(__dadd_rn(kk, m3)), Ep = __dsqrt_rn(__dadd_rn(pp, m4));
+                    kept = paper_roots_stage2(sp, sk3, sk1x, sk1y, m1, m2, m3, m4, E3, Ep, z, rt);
+                }
+                const unsigned has = __ballot_sync(full, kept);
+                if (kept) {
+                    const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
+                    const int n2 = P.g.n * P.g.n;
+                    q.cell[0][w] = (unsigned)(sxy1 + n2 * b1); q.cell[1][w] = (unsigned)(sxy2 + n2 * b2); q.cell[2][w] = (unsigned)si3; q.cell[3][w] = (unsigned)si;
+                    q.s[w] = rt.s; q.t[w] = rt.t; q.u[w] = rt.u; q.w_inv[w] = rt.w_inv;
+                    q.rti[w] = (unsigned char)cti;
+                }
+                count += __popc(has);
+                chead = (chead + nb) & (kQCand - 1);
+                ccount -= nb;
+                __syncwarp();
+                if (count >= 32) {
+                    paper_deposit_batch<kAllMassless>(P, q, lane, head, 32, cur_x, mreg);
+                    head = (head + 32) & (kQRing - 1);
+                    count -= 32;
+                    __syncwarp();
+                }
+            };
+            // one more trip than there are tuples: the last one only drains the candidates (they refer to this pass's samples,
+            // none is carried over).  stage2_batch is expanded at this one place.
+            const int ntup = q.ntup;
+            for (int ti = 0; ti <= ntup; ++ti) {                               // warp-uniform: one spatial cell per warp
+                const bool last = ti == ntup;
+                if (!last) {
+                    // stage 1 for every lane: 0.14-0.16 candidates per lane and tuple pass the box test
+                    const int ck = (int)(q.tup[ti] & 0xffffu);
+                    double zr[2];
+                    int b1r[2], b2r[2];
+                    const int cand = live ? paper_roots_stage1(P.g, p, k3, k1x, k1y, q.msm[ck & 3], q.msm[(ck >> 2) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), zr, b1r, b2r) : 0;
+#pragma unroll
+                    for (int r = 0; r < 2; ++r) {
+                        const bool mine = (cand >> r) & 1;
+                        const unsigned has = __ballot_sync(full, mine);
+                        if (mine) {
+                            const int w = (chead + ccount + __popc(has & lt)) & (kQCand - 1);
+                            q.cz[w] = zr[r];
+                            q.cmeta[w] = (unsigned long long)lane | (unsigned long long)ck << 5 | (unsigned long long)ti << 13 |
+                                         (unsigned long long)b1r[r] << 19 | (unsigned long long)b2r[r] << 30;
+                        }
+                        ccount += __popc(has);
+                    }
+                    __syncwarp();
+                }
+                while (ccount >= 32 || (last && ccount > 0)) stage2_batch(min(ccount, 32));   // full warps of candidates
+            }
+            continue;
+        }
+        // ---- the sample ring is empty: the end, or the next spatial cell
+        if (!have || xnext != cur_x) {
             while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
             __syncwarp();
-            cur_x = xcell;
+        }
+        if (!have) break;
+        {
+            cur_x = xnext;
+            const double* m = P.mass2 + 4 * (size_t)cur_x;
             mreg = P.mD2 > 0.0 ? P.mD2 : m[0];
             // classes with bit-identical masses share their roots: every class is mapped to the first class with its mass
-            rep = 0u;
+            unsigned rep = 0u;
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
                 int rc = c;
@@ -478,111 +621,7 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
             if (lane < 4) q.msm[lane] = m[lane];
             __syncwarp();
         }
-        const long long local = (item % chunks_per_x) * 32 + lane;
-        const bool valid = local < per_x;
-        const long long lc = valid ? local : per_x - 1;
-        const int smp = (int)(lc % P.Ns), i = P.p_begin + (int)(lc / P.Ns);
-        double p[3], Emassless;
-        cell_kinematics(P.g, i, p[0], p[1], p[2], Emassless);
-        uint32_t w0[4], w1[4], w2[4];
-        const uint32_t xc = (uint32_t)xcell + P.x_rng_offset;
-        philox4x32_10(64u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w0);
-        philox4x32_10(65u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w1);
-        philox4x32_10(66u, (uint32_t)smp, (uint32_t)i, xc, P.seed, P.step, w2);
-        double k3[3];
-        k3[0] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[0], w0[1]), P.g.L));
-        k3[1] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w0[2], w0[3]), P.g.L));
-        k3[2] = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[0], w1[1]), P.g.L));
-        const double k1x = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w1[2], w1[3]), P.g.L));
-        const double k1y = __dadd_rn(P.g.pmin, __dmul_rn(uniform52(w2[0], w2[1]), P.g.L));
-        const int i3 = bin_cell_exact(k3[0], k3[1], k3[2], P.g);
-        int ixy1, ixy2;
-        bool live;
-        {
-            bool ia, ib, ic, id;
-            const int a1 = bin_axis_exact(k1x, P.g, ia), b1 = bin_axis_exact(k1y, P.g, ib);
-            const double qx = __dsub_rn(__dadd_rn(k3[0], p[0]), k1x), qy = __dsub_rn(__dadd_rn(k3[1], p[1]), k1y);
-            const int a2 = bin_axis_exact(qx, P.g, ic), b2 = bin_axis_exact(qy, P.g, id);
-            ixy1 = a1 + P.g.n * b1; ixy2 = a2 + P.g.n * b2;
-            live = valid && i3 >= 0 && ia && ib && ic && id;
-        }
-        if (!__any_sync(full, live)) continue;
-        // energies of the outgoing legs, once per mass class (the roots of a tuple take E3 of its third, Ep of its fourth class)
-        const PaperLegs L(p, k3, m);
-        // stage 2 for candidates [chead, chead + nb): lanes = candidates; the sample a candidate belongs to lives in the registers
-        // of its source lane and comes over by shuffles; E3 and Ep are recomputed with PaperLegs' operations (the same bits)
-        auto stage2_batch = [&](int nb) {
-            const bool on = lane < nb;
-            const int cr = (chead + lane) & (kQCand - 1);
-            const unsigned long long meta = on ? q.cmeta[cr] : (unsigned long long)lane;
-            const double z = on ? q.cz[cr] : 0.0;
-            const int src = (int)(meta & 31ull), ck = (int)((meta >> 5) & 255ull), cti = (int)((meta >> 13) & 63ull);
-            const int b1 = (int)((meta >> 19) & 2047ull), b2 = (int)((meta >> 30) & 2047ull);
-            double sp[3], sk3[3];
-#pragma unroll
-            for (int d = 0; d < 3; ++d) { sp[d] = __shfl_sync(full, p[d], src); sk3[d] = __shfl_sync(full, k3[d], src); }
-            const double sk1x = __shfl_sync(full, k1x, src), sk1y = __shfl_sync(full, k1y, src);
-            const int sxy1 = __shfl_sync(full, ixy1, src), sxy2 = __shfl_sync(full, ixy2, src);
-            const int si3 = __shfl_sync(full, i3, src), si = __shfl_sync(full, i, src);
-            bool kept = false;
-            Root rt;
-            if (on) {
-                const double m1 = q.msm[ck & 3], m2 = q.msm[(ck >> 2) & 3], m3 = q.msm[(ck >> 4) & 3], m4 = q.msm[(ck >> 6) & 3];
-                const double kk = __dadd_rn(__dadd_rn(__dmul_rn(sk3[0], sk3[0]), __dmul_rn(sk3[1], sk3[1])), __dmul_rn(sk3[2], sk3[2]));
-                const double pp = __dadd_rn(__dadd_rn(__dmul_rn(sp[0], sp[0]), __dmul_rn(sp[1], sp[1])), __dmul_rn(sp[2], sp[2]));
-                const double E3 = __dsqrt_rn(__dadd_rn(kk, m3)), Ep = __dsqrt_rn(__dadd_rn(pp, m4));
-                kept = paper_roots_stage2(sp, sk3, sk1x, sk1y, m1, m2, m3, m4, E3, Ep, z, rt);
-            }
-            const unsigned has = __ballot_sync(full, kept);
-            if (kept) {
-                const int w = (head + count + __popc(has & lt)) & (kQRing - 1);
-                const int n2 = P.g.n * P.g.n;
-                q.cell[0][w] = (unsigned)(sxy1 + n2 * b1); q.cell[1][w] = (unsigned)(sxy2 + n2 * b2); q.cell[2][w] = (unsigned)si3; q.cell[3][w] = (unsigned)si;
-                q.s[w] = rt.s; q.t[w] = rt.t; q.u[w] = rt.u; q.w_inv[w] = rt.w_inv;
-                q.rti[w] = (unsigned char)cti;
-            }
-            count += __popc(has);
-            chead = (chead + nb) & (kQCand - 1);
-            ccount -= nb;
-            __syncwarp();
-            if (count >= 32) {
-                paper_deposit_batch<kAllMassless>(P, q, lane, head, 32, xcell, mreg);
-                head = (head + 32) & (kQRing - 1);
-                count -= 32;
-                __syncwarp();
-            }
-        };
-        // one more trip than there are groups: the last one only drains the candidates (they refer to this pass's samples, none
-        // is carried over).  stage2_batch is expanded at this one place: the kernel's code must stay inside the instruction cache
-        const int ntup = q.ntup;
-        for (int ti = 0; ti <= ntup; ++ti) {                               // warp-uniform: one spatial cell per warp
-            const bool last = ti == ntup;
-            const bool solve = !last;
-            const unsigned tu = q.tup[solve ? ti : 0];
-            const int ck = (int)(tu & 0xffffu);
-            if (solve) {
-                // stage 1 for every lane: 0.14-0.16 candidates per lane and tuple pass the box test
-                double zr[2];
-                int b1r[2], b2r[2];
-                const int cand = live ? paper_roots_stage1(P.g, p, k3, k1x, k1y, q.msm[ck & 3], q.msm[(ck >> 2) & 3], L.e3((ck >> 4) & 3), L.ep((ck >> 6) & 3), zr, b1r, b2r) : 0;
-#pragma unroll
-                for (int r = 0; r < 2; ++r) {
-                    const bool mine = (cand >> r) & 1;
-                    const unsigned has = __ballot_sync(full, mine);
-                    if (mine) {
-                        const int w = (chead + ccount + __popc(has & lt)) & (kQCand - 1);
-                        q.cz[w] = zr[r];
-                        q.cmeta[w] = (unsigned long long)lane | (unsigned long long)ck << 5 | (unsigned long long)ti << 13 |
-                                     (unsigned long long)b1r[r] << 19 | (unsigned long long)b2r[r] << 30;
-                    }
-                    ccount += __popc(has);
-                }
-                __syncwarp();
-            }
-            while (ccount >= 32 || (last && ccount > 0)) stage2_batch(min(ccount, 32));   // full warps of candidates
-        }
     }
-    while (count > 0) { const int nb = min(count, 32); paper_deposit_batch<kAllMassless>(P, q, lane, head, nb, cur_x, mreg); head = (head + nb) & (kQRing - 1); count -= nb; }
 }
 
 __global__ void __launch_bounds__(256) combine_kernel(const double* __restrict__ f, double* __restrict__ out,
