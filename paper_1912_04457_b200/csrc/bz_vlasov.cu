@@ -14,6 +14,17 @@ namespace {
 // species layout index a -> mass class (0 = g, 1 + flavour for q and qbar) is passed as 3 bits per slot in cls_bits
 __device__ __forceinline__ int class_of(unsigned cls_bits, int a) { return (int)((cls_bits >> (3 * a)) & 7u); }
 
+// 1/x to ~1 ulp: the hardware seed and two Newton steps instead of the IEEE division sequence (nothing here decides an index)
+__device__ __forceinline__ double rcp_newton(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 __global__ void __launch_bounds__(256) mass_kernel(const double* __restrict__ f, const double* __restrict__ cell_tab,
                                                    double* __restrict__ mass2, int S, int Np, unsigned cls_bits,
                                                    unsigned id_bits, double g2, double w /* d3p / (2 pi)^3 */)
@@ -32,7 +43,7 @@ __global__ void __launch_bounds__(256) mass_kernel(const double* __restrict__ f,
             const double2 u = __ldg(reinterpret_cast<const double2*>(cell_tab) + 2 * (size_t)pc);
             const double pz = __ldg(cell_tab + 4 * (size_t)pc + 2);
             const double E = sqrt(((u.x * u.x + u.y * u.y) + pz * pz) + m2);
-            if (E > 0.0) sum += w / E * fa[pc];
+            if (E > 0.0) sum += w * rcp_newton(E) * fa[pc];
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
@@ -71,7 +82,7 @@ __global__ void __launch_bounds__(256) diag_kernel(const double* __restrict__ f,
             const double pz = __ldg(cell_tab + 4 * (size_t)pc + 2);
             const double E = sqrt(((u.x * u.x + u.y * u.y) + pz * pz) + m2), v = fa[pc];
             se += E * v;
-            if (E > 0.0) sq += v / E;
+            if (E > 0.0) sq += v * rcp_newton(E);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) { se += __shfl_xor_sync(0xffffffffu, se, o); sq += __shfl_xor_sync(0xffffffffu, sq, o); }
@@ -118,16 +129,6 @@ struct VlasovParams {
     double dt, inv_2dx, inv_2dp;
     unsigned cls_bits;
 };
-
-__device__ __forceinline__ double rcp_newton(double x)
-{
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    return fma(y, e, y);
-}
 
 // ---- the stencil kernel bz_vlasov launches -----------------------------------------------------------------------------
 // One thread per (spatial cell, mass class, momentum cell); blockIdx.x = spatial cell (fastest): the blocks in flight share
