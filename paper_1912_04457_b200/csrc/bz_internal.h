@@ -50,6 +50,7 @@ struct PaperParams {
     const double* f;          // cell-major copy of f, [Nx][Np][SP] (the collision kernel's gather source f_aos; f itself if SP == 1)
     double* dN;               // cell-major deposit scratch dN_aos [Nx][Np][SP], number units, zero before the launch
     int SP;                   // doubles per cell in the two: 1 (one species) or 8
+    int cta_groups;           // spatial cells are dealt round-robin to this many groups of CTAs (launch_paper_collide)
     const double* mass2;      // [Nx][4] thermal masses^2 (Eq. 8-9)
     const PaperChannel* table;
     const PaperGroup* groups;

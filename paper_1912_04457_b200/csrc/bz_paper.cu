@@ -426,9 +426,9 @@ __global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB
     const long long per_x = (long long)P.p_count * P.Ns;
     const long long chunks_per_x = (per_x + 31) / 32;
     // Spatial cells go round-robin to up to 8 groups of CTAs, the chunks of a cell are strided over the warps of its group: a
-    // warp stays in one spatial cell for 1/8 of the launch's warps' share of it (its rings are drained only when it leaves),
-    // and the cells in flight (8 x 1.7 MB of f_aos + dN_aos tiles on config 4) stay in L2.
-    const int G = min(min(8, P.x_count), (int)gridDim.x);
+    // warp stays in one spatial cell for a long run of passes (its rings are drained only when it leaves), and the cells in
+    // flight (8 x 1.7 MB of f_aos + dN_aos tiles on config 4) stay in L2; 16 and 32 groups measured 4-6 % slower.
+    const int G = P.cta_groups;
     const int grp = (int)blockIdx.x % G;
     const long long wg = (long long)(blockIdx.x / G) * kQWarps + (threadIdx.x >> 5);
     const long long Wg = (long long)((gridDim.x - grp + G - 1) / G) * kQWarps;
@@ -640,6 +640,9 @@ cudaError_t launch_combine(const double* f, double* out, const double* dFc, size
     return cudaGetLastError();
 }
 
+#ifndef BZ_PAPER_GROUPS
+#define BZ_PAPER_GROUPS 8
+#endif
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
@@ -665,8 +668,16 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
     if (per_sm < 1) per_sm = 1;
     long long blocks = (total / 32 + kQWarps) / kQWarps;
     if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
-    if (P.all_massless) paper_queue_kernel<true><<<(int)blocks, 32 * kQWarps, smem, st>>>(P);
-    else paper_queue_kernel<false><<<(int)blocks, 32 * kQWarps, smem, st>>>(P);
+    // groups of CTAs: as many as 8 (BZ_PAPER_GROUPS), but no idle groups in the last round of cells beyond 1/8 of the work
+    PaperParams Q = P;
+    int best = 1;
+    for (int g = 1; g <= BZ_PAPER_GROUPS && g <= P.x_count && g <= (int)blocks; ++g) {
+        const int rounds = (P.x_count + g - 1) / g;
+        if ((long long)rounds * g * 7 <= (long long)P.x_count * 8) best = g;
+    }
+    Q.cta_groups = best;
+    if (P.all_massless) paper_queue_kernel<true><<<(int)blocks, 32 * kQWarps, smem, st>>>(Q);
+    else paper_queue_kernel<false><<<(int)blocks, 32 * kQWarps, smem, st>>>(Q);
     ++g_launch_count;
     return cudaGetLastError();
 }
