@@ -18,8 +18,9 @@
  * isotropy (P2), equilibrium bracket (P3), independent paper-parametrisation Monte Carlo of
  * Eq. 17-21 (P4), labelled-vs-symmetric estimator (P5), exact number conservation (P6),
  * Bose/Fermi closed forms for Eq. 8, 10, 11 (P7), upwind shift / Fourier factor (P8),
- * direction of g -> q qbar conversion (P9), constant-|M|^2 closed form (P10), textbook
- * colour/spin-averaged values and crossing relations for Table I.
+ * direction of g -> q qbar conversion (P9), constant-|M|^2 closed form (P10), entropy growth
+ * (H theorem, P11: the signs of bracket, deposits and F = 1 +- f), textbook colour/spin-averaged
+ * values and crossing relations for Table I.
  * Per-cell values of C[f] are printed nowhere in the paper: they are pinned only through
  * P4/P5/P10 (independent estimators agreeing), not by a published number.
  * NEXT rows, each pinned in its own test file: thermal masses, Eq. 15 and the

@@ -300,3 +300,55 @@ def test_P3b_binned_equilibrium_relaxes_slowly():
     print("P3b equilibrium/step relaxation ratio", ratio)
     assert ratio[10] < 0.2
     assert ratio[16] < 0.75 * ratio[10]
+
+
+def _entropy(f, species):
+    """- sum_a N_a sum_p [ f ln f -+ (1 +- f) ln(1 +- f) ] of the binned distribution (Bose: upper signs, Fermi: lower)"""
+    tot = 0.0
+    for a, sid in enumerate(species):
+        x = np.clip(f[:, a, :], 1e-300, None)
+        if sid == 0:
+            s = -(x * np.log(x) - (1.0 + x) * np.log1p(x))
+        else:
+            y = np.clip(1.0 - f[:, a, :], 1e-300, None)
+            s = -(x * np.log(x) + y * np.log(y))
+        tot += NDEG[sid] * s.sum()
+    return tot
+
+
+@pytest.mark.parametrize("species", [(0,), (1, 2, 3, 4)], ids=["glue", "two_flavours"])
+def test_P11_h_theorem(species):
+    """P11 (an invariant the oracle does not contain): with detailed balance built into Eq. 5's gain - loss bracket the
+    entropy of the distribution cannot fall (H theorem).  Each deposit moves one weight A from two cells to two others; to first
+    order dS = -A [ln(f_k f_l / (F_k F_l)) - ln(f_i f_j / (F_i F_j))] has the sign of -A ln(gain/loss) >= 0 whatever the matrix
+    element, so the entropy of the binned f grows step by step up to O(A^2) and the Monte Carlo noise.  A wrong sign of the
+    bracket, of a deposit or of F = 1 +- f makes it fall."""
+    n = 8
+    o = bzo.Oracle(np_=n, pmin=-3.0, pmax=3.0, species=species, alpha_s=0.3, m_D=0.5, seed=4, samples=48, threads=4)
+    px, py, pz = _centres(n, -3.0, 3.0)
+    pabs = np.sqrt(px ** 2 + py ** 2 + pz ** 2)
+    f = np.zeros(o.shape)
+    for a, sid in enumerate(species):
+        f[0, a] = (0.4 if sid == 0 else 0.6) * (pabs <= 1.6)            # far from equilibrium: a step function
+    o.set_f(f)
+    s = [_entropy(o.get_f(), species)]
+    n0 = (NDEG[list(species)][None, :, None] * o.get_f()).sum()
+    for _ in range(12):
+        o.step(0.05)
+        s.append(_entropy(o.get_f(), species))
+    s = np.array(s)
+    assert np.all(np.diff(s) > 0.0), np.diff(s)
+    assert s[-1] > 1.02 * s[0]
+    n1 = (NDEG[list(species)][None, :, None] * o.get_f()).sum()
+    assert abs(n1 - n0) <= 1e-12 * n0
+    # negative control on a smooth, strictly positive non-equilibrium f (so that f stays positive either way): dt -> -dt flips
+    # every deposit, and the entropy falls
+    g = np.zeros(o.shape)
+    for a, sid in enumerate(species):
+        g[0, a] = 0.02 + 0.3 * np.exp(-(pabs - 1.5) ** 2 / 0.5)
+    for sign in (+1.0, -1.0):
+        o.set_f(g)
+        o.step(sign * 0.01)
+        h = o.get_f()
+        assert h.min() > 0.0
+        assert sign * (_entropy(h, species) - _entropy(g, species)) > 0.0
