@@ -593,62 +593,89 @@ int bz_step_host(bz_ctx* c, double dt_fm, const double* f_in_host, double* f_out
         BZ_CUDA(cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking), "copy stream");
         BZ_CUDA(cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking), "copy stream");
     }
-    while ((int)c->pipe_events.size() < 2 * K + 1) {
+    // Pieces: a chunk is lpc whole z layers; the first and the last chunk are cut into four pieces of cells, so that the first
+    // collision waits for a quarter of a chunk's upload and only a quarter of a chunk's download is left after the last one.
+    struct Piece { int chunk, x0, nx; };
+    std::vector<Piece> pieces;
+    auto x0_of = [&](int k) { return k * lpc * layer_cells; };
+    auto nx_of = [&](int k) { return (std::min(nzl, (k + 1) * lpc) - k * lpc) * layer_cells; };
+    for (int k = 0; k < K; ++k) {
+        // (only where a quarter is still a few milliseconds of collisions: every launch of the persistent kernel has a ramp and a tail)
+        const int n = nx_of(k);
+        const bool big = (double)n * (double)c->Np * (double)c->Ns >= 1e8;
+        const int nsub = ((k == 0 || k == K - 1) && n % 4 == 0 && big) ? 4 : 1;
+        for (int q = 0; q < nsub; ++q) pieces.push_back({ k, x0_of(k) + q * (n / nsub), n / nsub });
+    }
+    const int NP = (int)pieces.size();
+    while ((int)c->pipe_events.size() < 2 * NP + 1) {
         cudaEvent_t e = nullptr;
         BZ_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "pipe event");
         c->pipe_events.push_back(e);
     }
-    cudaEvent_t* h2d_done = c->pipe_events.data();               // [K]
-    cudaEvent_t* tr_done = c->pipe_events.data() + K;            // [K]
-    cudaEvent_t start = c->pipe_events[2 * K];
+    cudaEvent_t* h2d_done = c->pipe_events.data();               // [NP]
+    cudaEvent_t* tr_done = c->pipe_events.data() + NP;           // [NP]
+    cudaEvent_t start = c->pipe_events[2 * NP];
     const size_t cell_vals = (size_t)c->S * c->Np;               // doubles per spatial cell
-    auto x0_of = [&](int k) { return k * lpc * layer_cells; };
-    auto nx_of = [&](int k) { return (std::min(nzl, (k + 1) * lpc) - k * lpc) * layer_cells; };
     // the copy streams start after whatever the context's stream has queued so far
     BZ_CUDA(cudaEventRecord(start, c->stream), "record");
     BZ_CUDA(cudaStreamWaitEvent(c->copy_in, start, 0), "wait");
     BZ_CUDA(cudaStreamWaitEvent(c->copy_out, start, 0), "wait");
-    // own layers of chunk k as a range of spatial cells (bz_set_slab: halo layers are refreshed on the device by the
-    // caller, they are neither read from nor written to the host buffers)
-    auto own_x0 = [&](int k) { return std::max(c->zb, k * lpc) * layer_cells; };
-    auto own_nx = [&](int k) { return std::max(0, std::min(c->ze, std::min(nzl, (k + 1) * lpc)) - std::max(c->zb, k * lpc)) * layer_cells; };
-    for (int k = 0; k < K; ++k) {
-        const size_t off = (size_t)own_x0(k) * cell_vals, cnt = (size_t)own_nx(k) * cell_vals;
-        if (cnt) BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
-        BZ_CUDA(cudaEventRecord(h2d_done[k], c->copy_in), "record");
-    }
-    auto transport_chunk = [&](int k) -> int {
+    // own cells of a piece (bz_set_slab: halo layers are refreshed on the device by the caller, they are neither read from
+    // nor written to the host buffers, and they do not collide)
+    const int own_b = c->zb * layer_cells, own_e = c->ze * layer_cells;
+    auto own_x0 = [&](const Piece& p) { return std::max(own_b, p.x0); };
+    auto own_nx = [&](const Piece& p) { return std::max(0, std::min(own_e, p.x0 + p.nx) - std::max(own_b, p.x0)); };
+    // uploads: chunk 0, then chunk K - 1 (the domain is periodic in z: chunk 0's drift stencil needs it), then 1 ... K - 2
+    for (int pass = 0; pass < 3; ++pass)
+        for (int q = 0; q < NP; ++q) {
+            const Piece& p = pieces[q];
+            const int cls = p.chunk == 0 ? 0 : (p.chunk == K - 1 ? 1 : 2);
+            if (cls != pass) continue;
+            const size_t off = (size_t)own_x0(p) * cell_vals, cnt = (size_t)own_nx(p) * cell_vals;
+            if (cnt) BZ_CUDA(cudaMemcpyAsync(c->f + off, f_in_host + off, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_in), "h2d");
+            BZ_CUDA(cudaEventRecord(h2d_done[q], c->copy_in), "record");
+        }
+    auto transport_piece = [&](int q) -> int {
+        const Piece& p = pieces[q];
+        if (int rc = prof_mark(c, 1)) return rc;
         TransportParams T = transport_params(c, dt_fm, c->f_new);
-        T.x_begin = x0_of(k); T.x_count = nx_of(k);
+        T.x_begin = p.x0; T.x_count = p.nx;
         BZ_CUDA(launch_transport(T, 1, c->stream), "stream+euler");
-        BZ_CUDA(cudaEventRecord(tr_done[k], c->stream), "record");
-        BZ_CUDA(cudaStreamWaitEvent(c->copy_out, tr_done[k], 0), "wait");
-        const size_t off = (size_t)own_x0(k) * cell_vals, cnt = (size_t)own_nx(k) * cell_vals;
+        if (int rc = prof_mark(c, 1)) return rc;
+        BZ_CUDA(cudaEventRecord(tr_done[q], c->stream), "record");
+        BZ_CUDA(cudaStreamWaitEvent(c->copy_out, tr_done[q], 0), "wait");
+        const size_t off = (size_t)own_x0(p) * cell_vals, cnt = (size_t)own_nx(p) * cell_vals;
         if (cnt) BZ_CUDA(cudaMemcpyAsync(f_out_host + off, c->f_new + off, cnt * sizeof(double), cudaMemcpyDeviceToHost, c->copy_out), "d2h");
         return 0;
     };
-    for (int k = 0; k < K; ++k) {
-        const int x0 = x0_of(k), nxk = nx_of(k);
-        BZ_CUDA(cudaStreamWaitEvent(c->stream, h2d_done[k], 0), "wait");
-        BZ_CUDA(launch_rowsums(c->f + (size_t)x0 * cell_vals, c->absp, c->w_invE, c->rowsum + (size_t)x0 * c->S * 3, nxk * c->S, c->Np,
+    for (int q = 0; q < NP; ++q) {
+        const Piece& p = pieces[q];
+        BZ_CUDA(cudaStreamWaitEvent(c->stream, h2d_done[q], 0), "wait");
+        // With the first piece of chunk k here (k >= 1; the uploads are in order and chunk K - 1 came second), every piece of
+        // chunk k - 1 is collided and has both z neighbours' old f on the device: they go out now, under the collisions to come.
+        // (Measured on config 4: the three chunk downloads that used to follow the last collision were 11 of the 17 ms an
+        // end-to-end step lost.)
+        if (p.chunk >= 1 && pieces[q - 1].chunk != p.chunk) {
+            BZ_CUDA(cudaStreamWaitEvent(c->stream, h2d_done[NP - 1], 0), "wait");     // the last piece of chunk K - 1 (k = 1: chunk 0 wraps around)
+            for (int r = 0; r < q; ++r) if (pieces[r].chunk == p.chunk - 1) { if (int rc = transport_piece(r)) return rc; }
+        }
+        BZ_CUDA(launch_rowsums(c->f + (size_t)p.x0 * cell_vals, c->absp, c->w_invE, c->rowsum + (size_t)p.x0 * c->S * 3, p.nx * c->S, c->Np,
                                c->stream), "rowsums");
         if (c->SP != 1)
-            BZ_CUDA(launch_pack(c->f + (size_t)x0 * cell_vals, c->f_aos + (size_t)x0 * c->Np * c->SP, nxk, c->S, c->SP, c->Np,
+            BZ_CUDA(launch_pack(c->f + (size_t)p.x0 * cell_vals, c->f_aos + (size_t)p.x0 * c->Np * c->SP, p.nx, c->S, c->SP, c->Np,
                                 c->stream), "pack");
-        // collision of the chunk's own cells (bz_set_slab may exclude halo layers)
-        const int zb = std::max(c->zb, k * lpc), ze = std::min(c->ze, std::min(nzl, (k + 1) * lpc));
-        if (ze > zb) {
+        if (own_nx(p) > 0) {                                     // collision of the piece's own cells
             CollideParams P = collide_params(c, dt_fm, c->step);
-            P.x_begin = zb * layer_cells;
-            P.n_items = (unsigned)((ze - zb) * layer_cells) * (unsigned)P.regions_per_x;
+            P.x_begin = own_x0(p);
+            P.n_items = (unsigned)own_nx(p) * (unsigned)P.regions_per_x;
+            if (int rc = prof_mark(c, 0)) return rc;
             BZ_CUDA(launch_collide(P, c->sms, c->stream), "collide");
-            c->generated += (unsigned long long)((ze - zb) * layer_cells) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
-                }
-        // chunk k - 1 has both z neighbours on the device now (chunk 0 waits for the last one: periodic)
-        if (k >= 2) { if (int rc = transport_chunk(k - 1)) return rc; }
+            if (int rc = prof_mark(c, 0)) return rc;
+            c->generated += (unsigned long long)own_nx(p) * (unsigned long long)c->Np * (unsigned long long)c->Ns;
+        }
+        // the pieces of the last chunk have had their neighbours (chunks K - 2 and 0) for a long time: out at once
+        if (p.chunk == K - 1) { if (int rc = transport_piece(q)) return rc; }
     }
-    if (int rc = transport_chunk(K - 1)) return rc;
-    if (int rc = transport_chunk(0)) return rc;
     double* t = c->f; c->f = c->f_new; c->f_new = t;
     c->aos_valid = true; c->rowsum_valid = false;
     c->step += 1;
