@@ -216,10 +216,11 @@ int bz_step_n(bz_ctx* ctx, double dt_fm, int n);
 /* The same step end to end from HOST memory: f_in_host (S*Nx*Np doubles, ideally pinned) replaces the context's f,
  * one bz_step is taken, and the new f is written to f_out_host; the context keeps the new f and the incremented step
  * counter exactly as after bz_set_f + bz_step + bz_get_f.  With at least 3 z layers and transport scheme 0 the work
- * is pipelined in chunks of z layers over three streams -- host-to-device copy of chunk k+1, collision of chunk k (the
- * collision term needs only the chunk's own cells, Eq. 5), stream + Euler of chunk k-1 (its upwind stencil needs
- * the old f of both z neighbours) and device-to-host copy of chunk k-2 run concurrently -- otherwise it is that plain
- * sequence.  Same results as the plain sequence up to the summation order of the deposits.  Synchronises.
+ * is pipelined in chunks of z layers over three streams -- host-to-device copies of the chunks to come, collision of
+ * chunk k (the collision term needs only the chunk's own cells, Eq. 5), stream + Euler of chunk k-1 (its upwind
+ * stencil needs the old f of both z neighbours: it is issued as soon as chunk k has arrived) and the device-to-host
+ * copy of its result run concurrently; the first and the last chunk are handled in quarters on large grids --
+ * otherwise it is that plain sequence.  Same results as the plain sequence up to the summation order of the deposits.  Synchronises.
  * Slab contexts (bz_set_slab): both host buffers still have the size of the whole context, but only the OWN layers are
  * read from f_in_host and written to f_out_host; the halo layers must have been refreshed on the device (bz_copy_layers)
  * before the call, from the neighbours' boundary layers of the same new f (paper_1912_04457_b200/slab.py, step_host);
