@@ -950,3 +950,31 @@ def test_papers_largest_grid_on_one_gpu():
     n1 = float(g.moments()["tot"][:, 0].sum())
     assert abs(n1 - n0) <= 1e-12 * n0
     g.close()
+
+
+def test_step_host_pieces_full_size_config4():
+    """bz_step_host at config 4's full size, where its pipeline cuts the first and the last z chunk into quarters (22 pieces):
+    the end-to-end step from pinned host memory against the resident bz_step of a second context on the same input (itself
+    checked against the oracle by the subset protocol above).  The two differ only in the order of the deposits' sums."""
+    cfg = wl.CONFIGS[4]
+    kw = dict(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species,
+              alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
+    f0 = torch.from_numpy(wl.initial_f(cfg))
+    hin = f0.pin_memory()
+    hout = torch.empty_like(f0).pin_memory()
+    a, b = bz.Boltzmann(**kw), bz.Boltzmann(**kw)
+    a.set_f(hin)
+    for _ in range(2):
+        a.step(cfg.dt)
+        b.step_host(cfg.dt, hin, hout)
+        fa = a.get_f()
+        fb = hout.cuda()
+        scale = float(fa.abs().max())
+        assert float((fa - fb).abs().max()) <= TOL_DF * scale
+        assert float((b.get_f() - fb).abs().max()) == 0.0                      # the context keeps what it wrote to the host
+        hin.copy_(hout)
+        del fa, fb
+    ma, mb = a.moments(), b.moments()
+    assert np.allclose(ma["tot"].numpy(), mb["tot"].numpy(), rtol=1e-12, atol=0)
+    a.close()
+    b.close()
