@@ -234,6 +234,34 @@ int bz_step_host(bz_ctx* ctx, double dt_fm, const double* f_in_host, double* f_o
  * Size 2*S*Nx + 2*S + Nx doubles.  Synchronises. */
 int bz_moments(bz_ctx* ctx, double* out_host);
 
+/* The same moments for a caller that keeps f in device memory of its own and cannot allocate any: no context, no
+ * cudaMalloc / cudaFree, no allocating library call, in this call or behind it.  Meant for
+ *   - a solver whose own f already fills most of the card: a context costs about 4.3 x the size of f (f, f_new and two
+ *     cell-major staging copies), which such a caller does not have, just to read n, e and m^2 off its state;
+ *   - a monitor that runs beside a long step on another stream: cudaMalloc and cudaFree synchronise the whole device
+ *     and would stall that step;
+ *   - a process whose device memory belongs in full to a framework's pool, where a raw cudaMalloc fails.
+ * Arguments: grid, species, n_species, alpha_s, m_D as for bz_create (same checks); f_dev: DEVICE pointer, S*Nx*Np
+ * doubles in the layout above, read only; out_dev: DEVICE pointer, 2*S*Nx + 2*S + Nx doubles, overwritten, with the
+ * content bz_moments writes to the host (totals over all cells); cuda_stream: cudaStream_t, NULL = default stream.  The
+ * caller owns both buffers; they must live on the device that is current in the calling thread.  Asynchronous.
+ * Scratch: the row sums between the two kernels (3 doubles per (spatial cell, species)) live in a fixed array inside
+ * the library image, 65536 rows = 1.5 MiB, which every GPU that loads the library holds until the process exits.
+ * Limit: nx*ny*nz * n_species <= 65536 (config 4 has 28672, the paper's 20^3 cells x 7 species 56000); a larger
+ * grid is refused with -5 before anything is launched.
+ * First call on a device: it also looks up the array's device address (cudaGetSymbolAddress, once per device, cached;
+ * the runtime may load the library's kernels onto the device at that moment).  Make that first call before any stream
+ * capture begins.
+ * Sharing: all calls on a device, from every thread and stream, use the one array.  Each call overwrites the rows it
+ * reads before reading them, so what an earlier call left behind never shows; but two calls that overlap on the GPU
+ * (different streams, no ordering between them) race on the array and both results are then undefined.  Order such
+ * calls yourself (same stream, or an event).
+ * Returns 0, -1 bad argument, -2 CUDA error, -5 grid beyond the scratch; bz_noalloc_last_error gives the text of
+ * the calling thread's last failure ("" after a success). */
+int bz_moments_noalloc(const bz_grid* grid, const int* species, int n_species, double alpha_s, double m_D,
+                       const double* f_dev, double* out_dev, void* cuda_stream);
+const char* bz_noalloc_last_error(void);
+
 /* Text of the last CUDA error seen by this context ("" if none). */
 const char* bz_last_error(const bz_ctx* ctx);
 

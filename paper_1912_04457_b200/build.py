@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbz.so")
 TESTHOOKS_LIB = os.path.join(HERE, "libbz_testhooks.so")     # test-only object (csrc/bz_testhooks.cu), never loaded by bz.py
-SOURCES = ["bz_api.cu", "bz_collision.cu", "bz_transport.cu", "bz_vlasov.cu", "bz_paper.cu", "bz_is.cu", "bz_calibrate.cu"]
+SOURCES = ["bz_api.cu", "bz_collision.cu", "bz_transport.cu", "bz_vlasov.cu", "bz_paper.cu", "bz_is.cu", "bz_calibrate.cu", "bz_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-cudart", "shared",
               "-Xlinker", "-rpath=/usr/local/cuda/lib64"]

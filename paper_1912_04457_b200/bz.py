@@ -24,7 +24,7 @@ EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_sa
            "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_collision_box", "bz_debug_samples_box", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_step_n", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_get_sample_counts",
-           "bz_debug_samples")
+           "bz_debug_samples", "bz_moments_noalloc", "bz_noalloc_last_error")
 
 KINDS = ("A", "11", "1B", "ANN", "QQGG", "QG", "GG")      # kinds of Table I in the order of bz_set_msq_override
 
@@ -75,6 +75,9 @@ def lib():
         L.bz_launch_count.argtypes = []
         L.bz_launch_count.restype = C.c_ulonglong
         L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
+        L.bz_moments_noalloc.argtypes = [C.POINTER(Grid), ip, C.c_int, C.c_double, C.c_double, vp, vp, vp]
+        L.bz_noalloc_last_error.argtypes = []
+        L.bz_noalloc_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -345,6 +348,40 @@ def debug_paper_channels(species):
     if n < 0:
         raise BzError("bz_debug_paper_channels: bad species list")
     return out[:n]
+
+
+NOALLOC_MAX_ROWS = 65536      # bz_moments_noalloc: spatial cells x species its fixed scratch holds (include/bz.h)
+
+
+def moments_noalloc(f, out, nx=1, ny=1, nz=1, dx=1.0, np_=15, pmin=-3.0, pmax=3.0, species=(0,), alpha_s=0.3, m_D=0.0,
+                    stream=None):
+    """bz_moments_noalloc: the moments of Boltzmann.moments() for a caller that holds f itself and cannot allocate device
+    memory (its f fills the card, it must not stall other streams with cudaMalloc, or a framework pool owns the memory).
+
+    f: contiguous CUDA float64 tensor, Nx*S*Np values in the library's layout (read only).  out: contiguous CUDA float64
+    tensor of 2*S*Nx + 2*S + Nx values, overwritten.  BOTH come from the caller: nothing is allocated here or in the
+    library, the scratch between the two kernels is a fixed 1.5 MiB array inside libbz.so, which limits the call to
+    Nx*S <= NOALLOC_MAX_ROWS (BzError otherwise) and is shared by all calls: do not let two of them overlap on the GPU.
+    Enqueued on `stream` (default: torch's current stream of f's device); returns views of `out` like moments().
+    The first call on a device also resolves the scratch's address: make it before any stream capture."""
+    S, Nx, Np = len(species), nx * ny * nz, np_ ** 3
+    n_out = 2 * S * Nx + 2 * S + Nx
+    for t, n in ((f, Nx * S * Np), (out, n_out)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n):
+            raise ValueError("expected a contiguous CUDA float64 tensor with %d elements" % n)
+    if out.device != f.device:
+        raise ValueError("f and out must be on the same device")
+    if stream is None:
+        stream = torch.cuda.current_stream(f.device)
+    grid = Grid(nx, ny, nz, dx, np_, pmin, pmax)
+    L = lib()
+    with torch.cuda.device(f.device):
+        rc = L.bz_moments_noalloc(C.byref(grid), (C.c_int * S)(*species), S, alpha_s, m_D, C.c_void_p(f.data_ptr()),
+                                  C.c_void_p(out.data_ptr()), C.c_void_p(stream.cuda_stream))
+    if rc != 0:
+        raise BzError("bz_moments_noalloc failed (%d): %s" % (rc, L.bz_noalloc_last_error().decode()))
+    a = Nx * S * 2
+    return {"ne": out[:a].view(Nx, S, 2), "tot": out[a:a + 2 * S].view(S, 2), "m2": out[a + 2 * S:]}
 
 
 def measure_fp64_peak():
