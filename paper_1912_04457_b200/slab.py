@@ -15,6 +15,8 @@ This module holds only host logic (who sends which layer to whom); every step of
 step, moments, layer_values) so that the exchange logic is covered on CPU by world_size-2 gloo tests that plug the
 oracle in (tests/test_slab_gloo.py); there is no CPU engine in this package.
 """
+import contextlib
+
 import torch
 import torch.distributed as dist
 
@@ -63,6 +65,13 @@ class SlabDomain:
         hi = e.get_layers(self.nz_local, 1)         # highest own layer -> the upper neighbour's lower halo
         self._exchange(lo, hi)
 
+    def _on_engine_stream(self):
+        """Context manager: makes the engine's CUDA stream torch's current stream (a no-op for a host engine).  bz_copy_layers
+        enqueues on the engine's stream, while torch's copies and the process group's send/recv order themselves against the
+        CURRENT stream: with the two made one, every producer and consumer of the boundary layers is on a single stream."""
+        s = getattr(self.engine, "torch_stream", None)
+        return torch.cuda.stream(s) if s is not None else contextlib.nullcontext()
+
     def _exchange(self, lo, hi):
         """lo / hi: this rank's lowest / highest own layer as flat tensors on the engine's device, produced on the
         engine's stream.  They go to the lower / upper neighbour; what comes back fills the two halo layers."""
@@ -73,24 +82,26 @@ class SlabDomain:
             return
         if self._recv_lo is None:
             self._recv_lo, self._recv_hi = torch.empty_like(lo), torch.empty_like(hi)
-        if lo.is_cuda:
-            # NCCL's send/recv kernels run on the process group's own stream, which waits for the CURRENT torch stream;
-            # the engine works on the stream that was current when it was made: the two are the same unless the caller
-            # changed streams, in which case the current one is made to wait for the engine's here.
-            cur = torch.cuda.current_stream(lo.device)
-            if getattr(e, "torch_stream", None) is not None and e.torch_stream != cur:
-                cur.wait_stream(e.torch_stream)
-        # Message order between a pair of ranks is the same on both sides (down-going first, tag 0; up-going second,
-        # tag 1), which is what NCCL matches by (it ignores tags) and gloo matches by tag; with two ranks both
-        # neighbours are the same peer.
-        ops = [dist.P2POp(dist.isend, lo, self.down, self.group, 0),
-               dist.P2POp(dist.isend, hi, self.up, self.group, 1),
-               dist.P2POp(dist.irecv, self._recv_hi, self.up, self.group, 0),
-               dist.P2POp(dist.irecv, self._recv_lo, self.down, self.group, 1)]
-        for req in dist.batch_isend_irecv(ops):
-            req.wait()                              # CUDA: the current stream waits for the transfer, the host does not block
-        e.set_layers(self.nz_local + 1, 1, self._recv_hi)
-        e.set_layers(0, 1, self._recv_lo)
+        with self._on_engine_stream():
+            # NCCL's send/recv kernels run on the process group's own stream, which waits for the current torch stream (here
+            # the engine's: lo and hi are complete before they are sent), and req.wait() makes the current stream (again the
+            # engine's) wait for the transfer, so that the halo copies below, which bz_copy_layers enqueues on the engine's
+            # stream, read the receive buffers after they have landed.
+            # Message order between a pair of ranks is the same on both sides (down-going first, tag 0; up-going second,
+            # tag 1), which is what NCCL matches by (it ignores tags) and gloo matches by tag; with two ranks both
+            # neighbours are the same peer.
+            ops = [dist.P2POp(dist.isend, lo, self.down, self.group, 0),
+                   dist.P2POp(dist.isend, hi, self.up, self.group, 1),
+                   dist.P2POp(dist.irecv, self._recv_hi, self.up, self.group, 0),
+                   dist.P2POp(dist.irecv, self._recv_lo, self.down, self.group, 1)]
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+            if lo.is_cuda:
+                # This branch has not run on two or more GPUs yet (no multi-GPU box in the build): until it has, the host
+                # also waits for the transfer, so that the result does not hang on the stream reasoning above alone.
+                torch.cuda.current_stream(lo.device).synchronize()
+            e.set_layers(self.nz_local + 1, 1, self._recv_hi)
+            e.set_layers(0, 1, self._recv_lo)
 
     # ---- the path
     def step(self, dt):
@@ -101,16 +112,19 @@ class SlabDomain:
     def step_host(self, dt, f_in_host, f_out_host):
         """The same step end to end from HOST memory (pinned): f_in_host / f_out_host have the size of the whole local
         context (nz_local + 2 layers), of which only the own layers 1 .. nz_local are read / written.  The two boundary
-        layers go to the device first and are exchanged with the neighbours while bz_step_host pipelines the own layers
-        (host-to-device copy, collision, stream + Euler, device-to-host copy by chunks of z layers)."""
+        layers go to the device first and are exchanged with the neighbours; bz_step_host then pipelines the own layers
+        (host-to-device copy, collision, stream + Euler, device-to-host copy by chunks of z layers).  The exchange is NOT
+        overlapped with that pipeline: its copy streams start behind the halo copies on the engine's stream (two layers
+        over NVLink, a fraction of a millisecond per step)."""
         e = self.engine
         lv = e.layer_values()
         flat = f_in_host.reshape(-1)
         if self._stage_lo is None:
             self._stage_lo = torch.empty(lv, dtype=torch.float64, device=e.device)
             self._stage_hi = torch.empty(lv, dtype=torch.float64, device=e.device)
-        self._stage_lo.copy_(flat[lv:2 * lv], non_blocking=True)
-        self._stage_hi.copy_(flat[self.nz_local * lv:(self.nz_local + 1) * lv], non_blocking=True)
+        with self._on_engine_stream():              # the staging copies are consumed on the engine's stream (set_layers, send)
+            self._stage_lo.copy_(flat[lv:2 * lv], non_blocking=True)
+            self._stage_hi.copy_(flat[self.nz_local * lv:(self.nz_local + 1) * lv], non_blocking=True)
         self._exchange(self._stage_lo, self._stage_hi)
         e.step_host(dt, f_in_host, f_out_host)
 
