@@ -9,7 +9,8 @@
  *
  * Conventions (S8b)
  *   - every function returns int: 0 = OK, -1 bad argument, -2 CUDA error (text via bz_last_error), -3 out of
- *     memory, -4 wrong state.  No exceptions, no aborts, nothing is printed.
+ *     memory, -4 wrong state (a half-built context, or a call that the context's current settings do not allow).  No
+ *     exceptions, no aborts, nothing is printed.
  *   - bz_ctx is opaque and OWNS its device buffers (f, f_new, the deposit scratch dN, m^2 per spatial cell,
  *     moment partials).  The caller owns every pointer it passes in.
  *   - pointers named *_dev are DEVICE pointers (e.g. torch tensor .data_ptr()); *_host are HOST pointers;

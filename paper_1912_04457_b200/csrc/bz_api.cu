@@ -193,7 +193,7 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     c->mass2 = nullptr; c->masses_zero = true; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
     c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
     c->aos_valid = false; c->rowsum_valid = false;
-    c->gstream = nullptr; c->gexec = nullptr; c->step_dev = nullptr; std::memset(&c->gkey, 0, sizeof c->gkey);
+    c->gstream = nullptr; c->gexec[0] = c->gexec[1] = nullptr; c->step_dev = nullptr; std::memset(c->gkey, 0, sizeof c->gkey);
     c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1;
     c->n_values = (size_t)c->Nx * c->S * c->Np;
     c->f = c->f_new = c->f_aos = c->dN_aos = c->rowsum = c->mom = c->absp = c->w_invE = c->vx = c->vy = c->vz = c->cell_tab = nullptr;
@@ -267,7 +267,7 @@ int bz_destroy(bz_ctx* c)
     BZ_ON_DEVICE(c);
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->counters); cudaFree(c->rowsum); cudaFree(c->mom);
     cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups); cudaFree(c->diag);
-    if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    for (cudaGraphExec_t ge : c->gexec) if (ge) cudaGraphExecDestroy(ge);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     cudaFree(c->step_dev);
     for (auto& v : c->prof_events) for (cudaEvent_t e : v) cudaEventDestroy(e);
@@ -414,7 +414,8 @@ int bz_set_transport(bz_ctx* c, int scheme) { if (!c || scheme < 0 || scheme > 2
 int bz_set_masses(bz_ctx* c, const double* mass2_host)
 {
     if (!c || !mass2_host) return -1;
-    if (!c->mass2) return -4;
+    if (!c->f || !c->mass2) return -4;
+    BZ_ON_DEVICE(c);
     c->masses_zero = false;
     BZ_CUDA(cudaMemcpyAsync(c->mass2, mass2_host, (size_t)c->Nx * 4 * sizeof(double), cudaMemcpyHostToDevice, c->stream), "set masses");
     BZ_CUDA(cudaStreamSynchronize(c->stream), "set masses sync");
@@ -499,6 +500,16 @@ int bz_step(bz_ctx* c, double dt_fm)
 }
 
 
+// field by field: the struct has padding, which an assignment need not copy
+static bool same_graph_key(const bz_ctx::GraphKey& a, const bz_ctx::GraphKey& b)
+{
+    if (!(a.dt == b.dt) || a.Ns != b.Ns || a.coll_mode != b.coll_mode || a.zb != b.zb || a.ze != b.ze || a.seed != b.seed ||
+        a.xoff != b.xoff || a.f != b.f)
+        return false;
+    for (int k = 0; k < 7; ++k) if (!(a.ovr[k] == b.ovr[k])) return false;
+    return true;
+}
+
 /* n steps without returning to the host in between: see include/bz.h */
 int bz_step_n(bz_ctx* c, double dt_fm, int n)
 {
@@ -519,37 +530,43 @@ int bz_step_n(bz_ctx* c, double dt_fm, int n)
     if (!c->gstream) BZ_CUDA(cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking), "graph stream");
     if (!c->step_dev) BZ_CUDA(cudaMalloc(&c->step_dev, sizeof(uint32_t)), "cudaMalloc step word");
     bz_ctx::GraphKey key;
-    std::memset(&key, 0, sizeof key);
     key.dt = dt_fm; key.Ns = c->Ns; key.coll_mode = c->coll_mode; key.zb = c->zb; key.ze = c->ze; key.seed = c->seed; key.xoff = c->xoff;
     for (int k = 0; k < 7; ++k) key.ovr[k] = c->msq_ovr[k];
     key.f = c->f;
-    if (!c->gexec || std::memcmp(&key, &c->gkey, sizeof key) != 0) {
-        if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+    const int slot = c->f < c->f_new ? 0 : 1;             // buffer parity of the pair's first step
+    cudaGraphExec_t& gexec = c->gexec[slot];
+    if (!gexec || !same_graph_key(key, c->gkey[slot])) {
+        if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
         cudaGraph_t graph = nullptr;
+        unsigned long long captured = 0ull;               // the launchers count what they enqueue; nothing runs during capture
         BZ_CUDA(cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeThreadLocal), "begin capture");
         cudaError_t e = cudaSuccess;
         double* fa = c->f;
         double* fb = c->f_new;
         for (int half = 0; half < 2 && e == cudaSuccess; ++half) {
             e = launch_rowsums(fa, c->absp, c->w_invE, c->rowsum, c->Nx * c->S, c->Np, c->gstream);
+            ++captured;
             if (e != cudaSuccess) break;
             CollideParams P = collide_params(c, dt_fm, 0u);
             P.step_ptr = c->step_dev;
             P.sampler = c->coll_mode == 0 ? 0 : c->coll_mode - 1;
             if (c->SP == 1) P.f_aos = fa;                      // one species: f itself is the gather source
             e = launch_collide(P, c->sms, c->gstream);
+            ++captured;
             if (e != cudaSuccess) break;
             TransportParams T = transport_params(c, dt_fm, fb);
             T.f = fa; T.step_ptr = c->step_dev;
             e = launch_transport(T, 1, c->gstream);
+            ++captured;
             std::swap(fa, fb);
         }
         cudaError_t e2 = cudaStreamEndCapture(c->gstream, &graph);
+        g_launch_count -= captured;
         if (e == cudaSuccess) e = e2;
-        if (e == cudaSuccess) e = cudaGraphInstantiate(&c->gexec, graph, 0);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&gexec, graph, 0);
         if (graph) cudaGraphDestroy(graph);
-        if (e != cudaSuccess) { c->gexec = nullptr; return fail_cuda(c, e, "bz_step_n: graph capture"); }
-        c->gkey = key;
+        if (e != cudaSuccess) { gexec = nullptr; return fail_cuda(c, e, "bz_step_n: graph capture"); }
+        c->gkey[slot] = key;
     }
     // order: whatever the context's stream has queued -> the graph launches -> the context's stream again
     cudaEvent_t ev = nullptr;
@@ -558,7 +575,7 @@ int bz_step_n(bz_ctx* c, double dt_fm, int n)
     if (e == cudaSuccess) e = cudaStreamWaitEvent(c->gstream, ev, 0);
     const uint32_t step0 = c->step;
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->step_dev, &step0, sizeof step0, cudaMemcpyHostToDevice, c->gstream);
-    for (int q = 0; q < pairs && e == cudaSuccess; ++q) e = cudaGraphLaunch(c->gexec, c->gstream);
+    for (int q = 0; q < pairs && e == cudaSuccess; ++q) e = cudaGraphLaunch(gexec, c->gstream);
     if (e == cudaSuccess) e = cudaEventRecord(ev, c->gstream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(c->stream, ev, 0);
     cudaEventDestroy(ev);
@@ -840,6 +857,7 @@ int bz_set_profile(bz_ctx* c, int on) { if (!c) return -1; c->profile = on != 0;
 int bz_get_profile(bz_ctx* c, int group, double* ms_total, int* launches)
 {
     if (!c || !ms_total || !launches || group < 0 || group > 1) return -1;
+    if (!c->f) return -4;
     BZ_ON_DEVICE(c);
     BZ_CUDA(cudaStreamSynchronize(c->stream), "profile sync");
     std::vector<cudaEvent_t>& ev = c->prof_events[group];

@@ -121,9 +121,11 @@ struct bz_ctx_impl {
     double *cell_tab;                // device [Np][4]: p1x, p1y, p1z, E1 (built on the device, bit-exact arithmetic)
     // bz_step_n: two consecutive steps (f -> f_new -> f) captured as one CUDA graph on a stream of the library's own
     cudaStream_t gstream;
-    cudaGraphExec_t gexec;
+    // one instantiated graph per buffer parity (slot 0: the pair starts with f in the lower of the two buffers, slot 1: in the
+    // upper one), so that calls with an odd n, which alternate the parity, replay instead of re-capturing
+    cudaGraphExec_t gexec[2];
     uint32_t* step_dev;              // device: the Philox step word the captured kernels read and advance
-    struct GraphKey { double dt; int Ns, coll_mode, zb, ze; uint32_t seed, xoff; double ovr[7]; const double* f; } gkey;
+    struct GraphKey { double dt; int Ns, coll_mode, zb, ze; uint32_t seed, xoff; double ovr[7]; const double* f; } gkey[2];
     std::string err;
     bool profile;
     std::vector<cudaEvent_t> prof_events[2];
