@@ -11,7 +11,7 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
     config.addinivalue_line("markers", "slow: long oracle runs (still part of the default CPU suite unless deselected)")
-    config.addinivalue_line("markers", "long: opt-in runs of several minutes (set BZ_LONG=1), e.g. config 3 for all of its 20 steps")
+    config.addinivalue_line("markers", "long: opt-in runs of many minutes (set BZ_LONG=1); no test carries it at present")
 
 
 def pytest_collection_modifyitems(config, items):

@@ -233,9 +233,9 @@ def test_config3_full_size_dF_and_f_after_steps():
     _config3_run(3, (0, 1))
 
 
-@pytest.mark.long
 def test_config3_full_size_all_20_steps():
-    """Config 3 for its own 20 steps (5.2e9 samples; the oracle needs ~5 min on 16 cores): opt-in, BZ_LONG=1."""
+    """Config 3 for its own 20 steps (5.2e9 samples; the oracle needs ~3-5 min on 16 cores): f after the last step on every
+    value, dF of the first and the last step."""
     _config3_run(wl.CONFIGS[3].steps, (0, 19))
 
 
@@ -257,7 +257,8 @@ def test_config4_full_size_subset_protocol():
     steps; (1) sampled indices and (s, t, u) of EVERY sample of the 64-cell block and of every 64th cell are bit-exact;
     (2) on every step of a 3-step run the oracle is fed the GPU's f of the 64 block cells at the start of the step
     ("teacher forcing": the collision term is local in x) and its dF for those cells is compared value by value,
-    with exact conservation per cell at 1e-13 of the gross deposit; (3) streaming is compared on the full grid."""
+    with exact conservation per cell at 1e-13 of the gross deposit.  (The whole grid, streaming included, against the oracle:
+    test_config4_full_size_whole_grid_one_step.)"""
     cfg = wl.CONFIGS[4]
     g = bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax,
                      species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D, seed=cfg.seed, samples=cfg.samples)
@@ -301,19 +302,40 @@ def test_config4_full_size_subset_protocol():
         g.step(cfg.dt)
     mom = g.moments()
     assert abs(float(mom["tot"][:, 0].sum()) - float(mom0["tot"][:, 0].sum())) <= 1e-12 * float(mom0["tot"][:, 0].sum())
-    # (3) streaming on the full grid: the upwind stencil against torch.roll
-    f_dev = g.get_f()
-    dS = g.stream(cfg.dt)
-    f5 = f_dev.view(cfg.nx, cfg.nx, cfg.nx, cfg.S, cfg.Np)
-    d5 = dS.view(cfg.nx, cfg.nx, cfg.nx, cfg.S, cfg.Np)
-    pabs, (px, py, pz) = wl.momentum_centres(cfg)
-    v = [torch.from_numpy(np.where(pabs > 0, c / np.where(pabs > 0, pabs, 1.0), 0.0)).cuda() * (cfg.dt / cfg.dx)
-         for c in (px, py, pz)]
-    acc = torch.zeros_like(f5)
-    for d, axis in ((0, 2), (1, 1), (2, 0)):                               # x is the fastest spatial index
-        c = v[d]
-        acc += torch.clamp(c, min=0) * (f5 - torch.roll(f5, 1, dims=axis)) + torch.clamp(c, max=0) * (torch.roll(f5, -1, dims=axis) - f5)
-    assert float((d5 + acc).abs().max()) <= 1e-13 * float(f5.abs().max())
+
+
+def test_config4_full_size_whole_grid_one_step():
+    """Config 4 at full size, ALL 4096 spatial cells (NS "f after N steps ... within 1e-11"): the
+    streaming increment of the whole grid against bzo_stream, then one whole step (3.6e9 kinematic samples, upwind streaming,
+    Euler) against bzo_step: every value of f at 1e-11 (S16), the moments at 1e-12.  The oracle's step takes 3-4 minutes on
+    16 host cores."""
+    cfg = wl.CONFIGS[4]
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg)
+    o.set_f(f)
+    g.set_f(torch.from_numpy(f))
+    fmax = np.abs(f).max()
+    d_o = o.stream(cfg.dt)
+    d_g = g.stream(cfg.dt).cpu().numpy()
+    assert np.abs(d_o).max() > 1e-6 * fmax
+    d_g -= d_o
+    assert np.abs(d_g).max() <= 1e-13 * fmax
+    del d_o, d_g
+    N0 = float(g.moments()["tot"][:, 0].sum())
+    o.step(cfg.dt)
+    g.step(cfg.dt)
+    f_o, f_g = o.get_f(), g.get_f().cpu().numpy()
+    assert np.abs(f_o - f).max() > 1e-6 * fmax
+    del f
+    _f_after_steps_check(f_g, f_o, o.gross(), "cfg4 whole grid, one step")
+    del f_o, f_g
+    mo, mg = o.moments(), g.moments()
+    for key in ("ne", "tot", "m2"):
+        a, b = np.asarray(mo[key]), mg[key].numpy()
+        assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(np.abs(a), np.abs(a).max() * 1e-6)), key
+    assert abs(float(mg["tot"][:, 0].sum()) - N0) <= 1e-12 * N0
+    g.close()
+    o.close()
 
 
 def test_edge_cases():
@@ -625,6 +647,46 @@ def test_paper_sampler_roots_bit_exact_on_the_config4_momentum_grid():
                     assert np.array_equal(stu[k, smp, 3 * r:3 * r + 3].view(np.uint64), np.array([R.s, R.t, R.u]).view(np.uint64))
 
 
+@pytest.mark.parametrize("which", ["paper", "is", "box"])
+def test_next_kernels_dF_parity_on_the_config4_momentum_grid(which):
+    """The NEXT-row collision kernels in the launch geometry bench.py probes -- config 4's momentum grid (24^3 cells over
+    [-4, 4] GeV, 64 samples per cell) and 64 spatial cells in one launch, so that the paper kernel runs its 8 CTA groups with
+    rings that wrap thousands of times and the weighted samplers their full persistent grid: dF of four spatial cells against
+    the oracle, value by value at 1e-11 (S16), with conservation per cell at 1e-13 of the gross deposit (Eq. 22).  The oracle
+    runs one spatial cell at a time with that cell's f, global index and, for the paper's sampler (Eq. 17-21), its four
+    distinct thermal masses: the collision term is local in x."""
+    import os
+    cfg = wl.scaled(wl.CONFIGS[4], nx=4)
+    kw = dict(dx=cfg.dx, np_=cfg.np_, pmin=cfg.pmin, pmax=cfg.pmax, species=cfg.species, alpha_s=cfg.alpha_s, m_D=cfg.m_D,
+              seed=cfg.seed, samples=cfg.samples)
+    g = bz.Boltzmann(nx=cfg.nx, ny=cfg.nx, nz=cfg.nx, **kw)
+    o = bzo.Oracle(nx=1, ny=1, nz=1, threads=min(16, os.cpu_count() or 1), **kw)
+    f0 = wl.initial_f(cfg) + 0.05 * wl.random_f(cfg, seed=47)
+    g.set_f(f0)
+    rng = np.random.Generator(np.random.Philox(key=53))
+    masses = 0.05 + 0.5 * rng.random((cfg.Nx, 4))                          # m_g^2, m_u^2, m_d^2, m_s^2: all different, per cell
+    step = 2
+    if which == "paper":
+        g.set_masses(masses)
+        dF = g.collision_paper(cfg.dt, step)
+    else:
+        dF = (g.collision_is if which == "is" else g.collision_box)(cfg.dt, step)
+    deg = _deg(cfg)[0]
+    for x in (0, 21, 42, 63):
+        o.set_slab(x, 0, 1)                                               # the cell draws the samples of its global index
+        o.set_f(f0[x][None])
+        if which == "paper":
+            o.set_masses(masses[x:x + 1])
+        dF_o = {"paper": o.collision_paper, "is": o.collision_is, "box": o.collision_box}[which](cfg.dt, step)[0]
+        G = o.gross()[0]
+        dF_g = dF[x].cpu().numpy()
+        assert np.abs(dF_o).max() > 0
+        _assert_dF(dF_g, dF_o, G, "%s, xcell %d" % (which, x))
+        assert abs((deg * dF_g).sum()) <= 1e-13 * (deg * G).sum()
+    degd = torch.from_numpy(_deg(cfg)).cuda()
+    assert abs(float((dF * degd).sum())) <= 1e-13 * float((dF.abs() * degd).sum())      # the whole launch
+
+
 def test_step_with_the_importance_sampled_collision_term():
     """bz_set_collision(2): bz_step with bz_collision_is; f after 3 steps against the oracle."""
     cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=7, samples=12)
@@ -814,6 +876,63 @@ def test_step_n_matches_oracle_and_step_loop(cfg, n):
     for key in ("ne", "tot", "m2"):
         a, b = np.asarray(mo[key]), mg[key].numpy()
         assert np.all(np.abs(a - b) <= 1e-12 * np.maximum(np.abs(a), np.abs(a).max() * 1e-6)), key
+
+
+def test_step_n_with_odd_n_keeps_one_graph_per_buffer_parity():
+    """Calls of bz_step_n with an odd n start from alternating buffers (the single ordinary step in front swaps f and f_new):
+    each parity has its own instantiated graph, so the third and fourth call replay what the first two captured.  The launch
+    counter sees 3 kernels for the ordinary step and 6 per replayed pair -- a capture enqueues nothing and counts nothing --
+    and the state after 4 x 5 steps is the oracle's after 20."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=8, samples=16)
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg) + 0.01 * wl.random_f(cfg, seed=31)
+    o.set_f(f)
+    g.set_f(f)
+    g.step(cfg.dt)                                                         # the cell-major copy exists from here on (no pack launch below)
+    o.step(cfg.dt)
+    for call in range(4):
+        before = bz.launch_count()
+        g.step_n(cfg.dt, 5)
+        assert bz.launch_count() - before == 3 + 2 * 6, call
+        for _ in range(5):
+            o.step(cfg.dt)
+    _f_after_steps_check(g.get_f().cpu().numpy(), o.get_f(), o.gross(), "4 x step_n(5)")
+    assert np.allclose(g.moments()["tot"].numpy(), o.moments()["tot"], rtol=1e-12, atol=0)
+
+
+def test_checkpoint_restart_continues_the_run():
+    """bz_get_f + (seed, step) is a complete checkpoint.  A run of 6 steps against one that is stopped after 3,
+    read out to the host, and continued in a NEW context from bz_set_f + bz_set_step: same f (the two differ only in the
+    order of the deposits' sums), same moments, and both equal to the oracle's uninterrupted 6 steps."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=3, np_=8, samples=16)
+    o, a = _pair(cfg)
+    f = wl.initial_f(cfg) + 0.01 * wl.random_f(cfg, seed=37)
+    o.set_f(f)
+    a.set_f(f)
+    for _ in range(6):
+        o.step(cfg.dt)
+        a.step(cfg.dt)
+    _, b = _pair(cfg, threads=1)
+    b.set_f(f)
+    for _ in range(3):
+        b.step(cfg.dt)
+    saved = torch.empty(b.shape, dtype=torch.float64)
+    b.get_f(saved)                                                         # the checkpoint: f on the host; seed and step are the caller's
+    b.close()
+    _, c = _pair(cfg, threads=1)                                           # a fresh context: seed from the config, step counter 0
+    c.set_f(saved)
+    c.set_step(3)
+    for _ in range(3):
+        c.step(cfg.dt)
+    f_a, f_c, f_o = a.get_f().cpu().numpy(), c.get_f().cpu().numpy(), o.get_f()
+    _f_after_steps_check(f_c, f_o, o.gross(), "restarted run")
+    assert np.abs(f_c - f_a).max() <= TOL_DF * np.abs(f_a).max()
+    assert np.allclose(c.moments()["tot"].numpy(), a.moments()["tot"].numpy(), rtol=1e-12, atol=0)
+    c.set_step(0)                                                          # the wrong step word draws other samples: the checkpoint needs it
+    c.set_f(saved)
+    for _ in range(3):
+        c.step(cfg.dt)
+    assert np.abs(c.get_f().cpu().numpy() - f_a).max() > 1e3 * TOL_DF * np.abs(f_a).max()
 
 
 def test_slab_step_host_on_one_gpu():
