@@ -56,14 +56,36 @@ FLOP_PER_GENERATED = 108.0
 # 1/(u - m^2): 80 (20 for the pure-glue row alone); F = 1 +- f for 4 cells x S species: 4 S
 # per accepted sample AND ordered channel (collide_tile's inner loop): bracket 7, x w x |M|^2 2, four deposits 4 = 13
 FLOP_PER_CHANNEL = 13.0
+FLOP_PER_CHANNEL_LOW = 8.0          # the lower end of SURVEY.md 8d's "8-13 flop per channel"
+FP64_NOMINAL_TFLOPS = 37.2          # 148 SMs x 64 FP64 lanes x 2 x 1.965 GHz
 N_CHANNELS = {1: 1, 6: 90, 7: 127}
 
 
-def flop_per_accepted(cfg):
+def flop_per_accepted(cfg, per_channel=FLOP_PER_CHANNEL):
     n_ch = N_CHANNELS.get(cfg.S)
     if n_ch is None:
         return None
-    return 2.0 + (20.0 if cfg.S == 1 else 80.0) + 4.0 * cfg.S + FLOP_PER_CHANNEL * n_ch
+    return 2.0 + (20.0 if cfg.S == 1 else 80.0) + 4.0 * cfg.S + per_channel * n_ch
+
+
+def negative_msq_report(g, cfg, step):
+    """Reading S8: the fraction of (sample, channel) pairs whose regulated Table I value is negative, over
+    the samples bz_collision draws at `step` in a bounded block of spatial cells, for the f the context holds now.  Counted
+    on the device (bz_msq_sign_counts); the ordered-channel multiplicity of every (kind, ordering) is the library's table."""
+    from paper_1912_04457_b200 import bz
+    cells = min(cfg.Nx, 64)
+    x0 = (cfg.Nx - cells) // 2
+    accepted, neg = g.msq_sign_counts(step, x0, x0 + cells)
+    mult = [[0, 0] for _ in range(7)]
+    for row in bz.debug_paper_channels(cfg.species):
+        mult[int(row[4])][int(row[5])] += 1
+    n_ch = sum(a + b for a, b in mult)
+    pairs = sum(mult[k][c] * neg[k][c] for k in range(7) for c in range(2))
+    return {"fraction_of_sample_channel_pairs": pairs / (accepted * n_ch) if accepted else None,
+            "samples_accepted": accepted, "ordered_channels": n_ch, "negative_pairs": pairs,
+            "negative_samples_by_kind": {k: neg[i] for i, k in enumerate(bz.KINDS)},
+            "sample": "spatial cells %d..%d of %d, every momentum cell and sample, Philox step %d" % (x0, x0 + cells - 1, cfg.Nx, step),
+            "what": "regulated Table I evaluated literally, no clamp (reading S8); [straight, crossed] counts per kind"}
 
 
 def bytes_literal_8d(cfg):
@@ -325,7 +347,8 @@ def spawn_ranks(args):
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
            "--master-addr", "127.0.0.1", "--master-port", str(free_port()), os.path.abspath(__file__)] + sys.argv[1:]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")           # the communicator's init lines (ranks, transport) are what a scaling run is checked by
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     raise SystemExit(subprocess.call(cmd, env=env))
 
 
@@ -429,6 +452,7 @@ def run_ours(args, cfg):
     rank3 = weighted_probe(g, cfg, dev, "is") if (rank == 0 and not slabs and not args.no_probes) else None
     rank3b = weighted_probe(g, cfg, dev, "box") if (rank == 0 and not slabs and not args.no_probes) else None
     N1 = float(mom_host[2 * cfg.S * g.Nx:2 * cfg.S * g.Nx + 2 * cfg.S:2].sum())
+    neg_msq = negative_msq_report(g, cfg, args.warmup + args.steps) if (rank == 0 and not slabs) else None
 
     # ---- bz_step_n: the same steps without returning to the host in between (captured CUDA graph), moments once at the end
     stepn = None
@@ -495,8 +519,15 @@ def run_ours(args, cfg):
         if fpa and fp64_peak:
             flop = FLOP_PER_GENERATED + acceptance * fpa
             a64 = kern_rate * flop / 1e12
+            fpa_low = flop_per_accepted(cfg, FLOP_PER_CHANNEL_LOW)
+            a64_low = kern_rate * (FLOP_PER_GENERATED + acceptance * fpa_low) / 1e12
             roof64 = {"bound": "alu", "kernel": "collide_kernel", "achieved": a64, "peak": fp64_peak, "unit": "TFLOP/s",
                       "frac": a64 / fp64_peak, "peak_source": "measured (bz_measure_fp64_peak, register-resident DFMA chains; an FMA counts 2)",
+                      "kind": "ALGORITHMIC flop rate: the method's operations per sample x samples/s, not executed instructions -- a factorised kernel is credited with the channel-by-channel count and could exceed 1.0; it is north_star's FP64 leg, not a pipe utilisation",
+                      "frac_nominal_peak": a64 / FP64_NOMINAL_TFLOPS, "nominal_peak": FP64_NOMINAL_TFLOPS,
+                      "nominal_peak_source": "SURVEY.md 8d: 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz",
+                      "frac_at_8_flop_per_channel": a64_low / fp64_peak, "frac_nominal_peak_at_8_flop_per_channel": a64_low / FP64_NOMINAL_TFLOPS,
+                      "executed": "ncu at round 2 (profiles/r2_collide_kernel_ncu_full.md): about 300 FP64 instructions per accepted sample, FP64 pipe 46.5 % busy, issue port about 95 % of what the instruction mix allows",
                       "flop_per_sample": flop, "flop_per_generated_sample": FLOP_PER_GENERATED, "flop_per_accepted_sample": fpa,
                       "flop_per_channel": FLOP_PER_CHANNEL, "channels": N_CHANNELS.get(cfg.S),
                       "count": "the method as oracle/bzo.c states it (channel by channel), each + - x / sqrt = 1; the kernel's factorised channel algebra executes fewer (DESIGN.md 6)",
@@ -519,6 +550,8 @@ def run_ours(args, cfg):
                    "parallelism": ("z slabs, one halo layer exchanged with each neighbour per step (NCCL send/recv), domain = config x %d along z" % world if slabs
                                    else "independent replicas (homogeneous config: nothing to exchange)" if world > 1 else "1 GPU")},
         "cell_updates_per_sec": world * cfg.n_values * args.steps / (ms * 1e-3),
+        "samples_x_channels_per_sec": value * N_CHANNELS[cfg.S] if cfg.S in N_CHANNELS else None,     # SURVEY.md 8d "Metric" (i)
+        "negative_msq": neg_msq,                                                                       # reading S8
         "collision_kernel_samples_per_sec": kern_rate,
         "collision_kernel_accepted_samples_per_sec": kern_rate * acceptance if (kern_rate and acceptance is not None) else None,
         "collision_kernel_share_of_step": coll_ms / ms if ms > 0 else None,

@@ -289,6 +289,17 @@ unsigned long long bz_launch_count(void);
  * kernel itself.  bench.py weights the roofline with accepted / generated.  reset != 0 clears both.  Synchronises. */
 int bz_get_sample_counts(bz_ctx* ctx, unsigned long long* generated_out, unsigned long long* accepted_out, int reset);
 
+/* Reading S8 of SURVEY.md 8c: Table I with the regulator in the t and u propagators is evaluated literally
+ * and can turn negative (e.g. q qbar <-> g g, where -96 (t^2 + u^2)/s^2 stays while the regulated part shrinks); nothing
+ * is clamped.  This call reports how often: it regenerates the kinematic samples that bz_collision draws for `step` in
+ * spatial cells [xcell_begin, xcell_end), evaluates the |M|^2 of every kind and ordering with each cell's regulator for
+ * the current f (honouring bz_set_msq_override) and writes 15 counters to HOST memory: out_host[0] = samples that
+ * deposit; out_host[1 + 2*kind + crossed] = those of them with |M|^2(kind, ordering) < 0, kind as in
+ * bz_set_msq_override, crossed = 1 for the t <-> u exchanged ordering (the same number for the symmetric kinds).
+ * Weighted with the number of ordered channels of each (kind, ordering) this is the fraction of negative
+ * (sample, channel) pairs.  Not part of the timed path.  Synchronises. */
+int bz_msq_sign_counts(bz_ctx* ctx, unsigned step, int xcell_begin, int xcell_end, unsigned long long* out_host);
+
 /* ---- test-only exports ---------------------------------------------------------------------------------- */
 /* Sampled cells of p1 cells [pcell_begin, pcell_end) of spatial cell xcell, needed for the "bit-exact sampled
  * indices" target of NS: cells_dev[n][Ns][4] = (j, k, l, flag) int32, stu_dev[n][Ns][3] = (s, t, u) or NULL.

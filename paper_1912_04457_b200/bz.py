@@ -24,7 +24,7 @@ EXPORTS = ("bz_create", "bz_destroy", "bz_set_stream", "bz_set_seed", "bz_set_sa
            "bz_set_transport", "bz_step_host", "bz_collision_paper", "bz_set_collision", "bz_energy_diag", "bz_collision_is", "bz_debug_samples_is", "bz_collision_box", "bz_debug_samples_box", "bz_debug_paper_samples", "bz_debug_paper_channels", "bz_set_f",
            "bz_get_f", "bz_collision", "bz_stream", "bz_step", "bz_step_n", "bz_moments", "bz_last_error", "bz_set_profile",
            "bz_get_profile", "bz_measure_fp64_peak", "bz_launch_count", "bz_get_sample_counts",
-           "bz_debug_samples", "bz_moments_noalloc", "bz_noalloc_last_error")
+           "bz_debug_samples", "bz_moments_noalloc", "bz_noalloc_last_error", "bz_msq_sign_counts")
 
 KINDS = ("A", "11", "1B", "ANN", "QQGG", "QG", "GG")      # kinds of Table I in the order of bz_set_msq_override
 
@@ -75,6 +75,7 @@ def lib():
         L.bz_launch_count.argtypes = []
         L.bz_launch_count.restype = C.c_ulonglong
         L.bz_debug_samples.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.c_int, vp, vp]
+        L.bz_msq_sign_counts.argtypes = [vp, C.c_uint, C.c_int, C.c_int, C.POINTER(C.c_ulonglong)]
         L.bz_moments_noalloc.argtypes = [C.POINTER(Grid), ip, C.c_int, C.c_double, C.c_double, vp, vp, vp]
         L.bz_noalloc_last_error.argtypes = []
         L.bz_noalloc_last_error.restype = C.c_char_p
@@ -329,6 +330,13 @@ class Boltzmann:
         g, a = C.c_ulonglong(), C.c_ulonglong()
         self._chk(lib().bz_get_sample_counts(self._h, C.byref(g), C.byref(a), int(bool(reset))), "bz_get_sample_counts")
         return g.value, a.value
+
+    def msq_sign_counts(self, step, xbegin, xend):
+        """bz_msq_sign_counts (reading S8): (accepted samples, counts[kind][crossed] of negative |M|^2 among them) for the
+        samples bz_collision draws at `step` in spatial cells [xbegin, xend)."""
+        out = (C.c_ulonglong * 15)()
+        self._chk(lib().bz_msq_sign_counts(self._h, step, xbegin, xend, out), "bz_msq_sign_counts")
+        return int(out[0]), [[int(out[1 + 2 * k]), int(out[2 + 2 * k])] for k in range(7)]
 
     def debug_samples(self, step, xcell, pbegin, pend, want_stu=True):
         n = pend - pbegin

@@ -15,6 +15,18 @@ struct bz_ctx : public bz_ctx_impl {};
 
 namespace bz {
 std::atomic<unsigned long long> g_launch_count{0};
+
+int device_sms()
+{
+    static std::atomic<int> cache[64];
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    n = cache[dev].load(std::memory_order_relaxed);
+    if (n > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) return 148;
+    cache[dev].store(n, std::memory_order_relaxed);
+    return n;
+}
 }
 
 namespace {
@@ -191,7 +203,7 @@ static int create_impl(const bz_grid* g, const int* species, int n_species, doub
     c->xoff = 0u; c->zb = 0; c->ze = g->nz;
     for (int k = 0; k < 7; ++k) c->msq_ovr[k] = -1.0;
     c->mass2 = nullptr; c->masses_zero = true; c->coll_mode = 0; c->dF_scratch = nullptr; c->paper_table = nullptr; c->paper_groups = nullptr; c->paper_n_groups = 0; c->paper_n_channels = 0;
-    c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr;
+    c->E_tab = nullptr; c->x_nb = nullptr; c->p_wrap = nullptr; c->scheme = 0; c->diag = nullptr; c->sign_counts = nullptr;
     c->aos_valid = false; c->rowsum_valid = false;
     c->gstream = nullptr; c->gexec[0] = c->gexec[1] = nullptr; c->step_dev = nullptr; std::memset(c->gkey, 0, sizeof c->gkey);
     c->work_counter = nullptr; c->counters = nullptr; c->generated = 0ull; c->sms = 1;
@@ -266,7 +278,7 @@ int bz_destroy(bz_ctx* c)
     if (!c) return -1;
     BZ_ON_DEVICE(c);
     cudaFree(c->f); cudaFree(c->f_new); cudaFree(c->f_aos); cudaFree(c->dN_aos); cudaFree(c->work_counter); cudaFree(c->counters); cudaFree(c->rowsum); cudaFree(c->mom);
-    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups); cudaFree(c->diag);
+    cudaFree(c->absp); cudaFree(c->cell_tab); cudaFree(c->mass2); cudaFree(c->E_tab); cudaFree(c->x_nb); cudaFree(c->p_wrap); cudaFree(c->dF_scratch); cudaFree(c->paper_table); cudaFree(c->paper_groups); cudaFree(c->diag); cudaFree(c->sign_counts);
     for (cudaGraphExec_t ge : c->gexec) if (ge) cudaGraphExecDestroy(ge);
     if (c->gstream) cudaStreamDestroy(c->gstream);
     cudaFree(c->step_dev);
@@ -889,6 +901,20 @@ int bz_get_sample_counts(bz_ctx* c, unsigned long long* generated_out, unsigned 
         BZ_CUDA(cudaMemsetAsync(c->counters, 0, sizeof acc, c->stream), "sample counter reset");
         c->generated = 0ull;
     }
+    return 0;
+}
+
+int bz_msq_sign_counts(bz_ctx* c, unsigned step, int xcell_begin, int xcell_end, unsigned long long* out_host)
+{
+    if (!c || !out_host || xcell_begin < 0 || xcell_end > c->Nx || xcell_begin > xcell_end) return -1;
+    if (!c->f) return -4;
+    BZ_ON_DEVICE(c);
+    if (int rc = update_m2(c)) return rc;                // the regulator of every spatial cell for the current f
+    if (!c->sign_counts) BZ_CUDA(cudaMalloc(&c->sign_counts, 15 * sizeof(unsigned long long)), "cudaMalloc sign counters");   // kept with the context
+    BZ_CUDA(cudaMemsetAsync(c->sign_counts, 0, 15 * sizeof(unsigned long long), c->stream), "sign counters reset");
+    BZ_CUDA(launch_msq_signs(collide_params(c, 1.0, step), xcell_begin, xcell_end, c->sign_counts, c->sms, c->stream), "msq signs");
+    BZ_CUDA(cudaMemcpyAsync(out_host, c->sign_counts, 15 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream), "sign counters copy");
+    BZ_CUDA(cudaStreamSynchronize(c->stream), "sign counters sync");
     return 0;
 }
 

@@ -30,10 +30,7 @@ namespace bz {
 
 namespace {
 
-#ifndef BZ_WARPS
-#define BZ_WARPS 16
-#endif
-constexpr int kWarps = BZ_WARPS;
+constexpr int kWarps = 16;
 constexpr int kCollideThreads = 32 * kWarps;
 constexpr int kRing = 64;                        // records per warp (a sampling pass adds at most 32)
 constexpr int kRetryCap = 64;                    // per warp: samples whose two Marsaglia attempts both failed
@@ -65,16 +62,9 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 // fp64 reduction without return value (RED.E.ADD.F64)
-#ifndef BZ_ABLATE
-#define BZ_ABLATE 0
-#endif
 __device__ __forceinline__ void red_add(double* gdst, double v)
 {
-#if BZ_ABLATE == 3
-    if (v == 1.2345e300) asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gdst), "d"(v));
-#else
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(gdst), "d"(v));
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------ shared memory
@@ -121,9 +111,6 @@ __device__ __forceinline__ void issue_gather(WarpMem<kSP>& wm, const double* __r
         const uint4 c0 = *reinterpret_cast<const uint4*>(cp), c1 = *reinterpret_cast<const uint4*>(cp + 4);
         const unsigned ci[8] = { c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w };
 #pragma unroll
-#if BZ_ABLATE == 4
-        if (ci[0] == 0xfffffff0u)
-#endif
         for (int k = 0; k < 8; ++k) cp_async16(dst + k * W::kStride, src + (size_t)ci[k] * 8);
     } else {
         for (int k = 0; k < 8 && sub * 8 + k < nb; ++k) cp_async16(dst + k * W::kStride, src + (size_t)cp[k] * 8);
@@ -193,17 +180,11 @@ __device__ __forceinline__ void consume_batch(WarpMem<kSP>& wm, const CollidePar
             }
         }
         const double u = __dsub_rn(-s, t);
-#if BZ_ABLATE == 2
-        MsqSet M = {}; M.gg = s; M.qqgg = t; M.qg_t = u; M.a_t = g4w; M.d11 = m2;
-#pragma unroll
-        for (int a = 0; a < 7; ++a) { d[0][a] = Pi[a] * M.gg; d[1][a] = Pj[a] * M.qqgg; d[2][a] = Qk[a] * M.qg_t; d[3][a] = Ql[a] * M.a_t + M.d11; }
-#else
         MsqSet M = msq_set<kGlue, kQuark>(s, t, u, m2, g4w);
         // user-defined matrix elements (bz_set_msq_override) run on the runtime-mask instantiation, so that the
         // specialised mixture kernels carry no extra registers for them
         if constexpr (kMask < 0) { if (P.has_ovr) msq_apply_override(M, P.msq_ovr, g4w); }
         deposit_half<kMask>(mask, Pi, Pj, Qk, Ql, M, d[0], d[1], d[2], d[3]);
-#endif
     }
     __syncwarp();                                        // both lanes of every pair have read the gathered f
     if (work) {
@@ -567,7 +548,8 @@ cudaError_t launch_debug_samples(const CollideParams& P, int xcell, int p_begin,
 {
     const long long total = (long long)(p_end - p_begin) * P.Ns;
     if (total <= 0) return cudaSuccess;
-    const int blocks = (int)((total + 127) / 128 < 148 * 16 ? (total + 127) / 128 : 148 * 16);
+    const long long cap = (long long)device_sms() * 16;
+    const int blocks = (int)((total + 127) / 128 < cap ? (total + 127) / 128 : cap);
     debug_samples_kernel<<<blocks, 128, 0, st>>>(P, xcell, p_begin, p_end, cells, stu);
     ++g_launch_count;
     return cudaGetLastError();

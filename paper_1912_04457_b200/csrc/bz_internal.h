@@ -103,6 +103,7 @@ struct bz_ctx_impl {
     int coll_mode;                   // bz_set_collision: 0 CM sampler (hot path), 1 the paper's sampler, 2 importance-sampled t, 3 in-box direction
     double* dF_scratch;              // device n_values, allocated at the first bz_step with coll_mode 1
     double* diag;                    // device [Nx][5], allocated at the first bz_energy_diag
+    unsigned long long* sign_counts; // device [15], allocated at the first bz_msq_sign_counts
     int scheme;                      // bz_set_transport: 0 upwind massless (NS), 1 Eq. 15 + masses per step, 2 Eq. 15, masses as set
     cudaStream_t stream;
     size_t n_values;
@@ -149,6 +150,10 @@ __device__ __forceinline__ double regulator_m2(const double* __restrict__ rowsum
 // kernels launched by this library in this process (bz_launch_count); bumped by every launcher below
 extern std::atomic<unsigned long long> g_launch_count;
 
+// SMs of the device that is current in the calling thread (cached per device; 148 if the query fails): the grid cap of the
+// grid-stride launchers that do not get the context's SM count
+int device_sms();
+
 // launchers (each returns the cudaError_t of the launch)
 int collide_slots_per_cell(unsigned mask);
 void collide_item_geometry(int Np, int Nx, int Ns, int sms, int* units_per_item, int* ppc, int* regions_per_x);
@@ -178,6 +183,9 @@ cudaError_t launch_vlasov(const double* f, double* out, int nx, int ny, int nz, 
                           const double* mass2, double* E_tab, const int* x_nb, const unsigned char* p_wrap, int n, double dt,
                           double dx, double dp, unsigned cls_bits, cudaStream_t st);
 
+// reading S8 (bz_diag.cu): counts[0] += accepted samples of spatial cells [x_begin, x_end), counts[1 + 2 kind + crossed] += those
+// whose |M|^2 of that kind and ordering is negative
+cudaError_t launch_msq_signs(const CollideParams& P, int x_begin, int x_end, unsigned long long* counts, int sms, cudaStream_t st);
 // NEXT rank 3 (bz_is.cu): what the weighted samplers draw (sampler 1: importance-sampled t with regulator m2, 2: in-box)
 cudaError_t launch_weighted_debug(const PaperParams& P, int sampler, double m2, int* cells, double* stu, double* w, int sms, cudaStream_t st);
 // NEXT rank 1 (bz_paper.cu)

@@ -414,10 +414,7 @@ __device__ __forceinline__ void paper_deposit_batch(const PaperParams& P, QWarp&
 }
 
 template <bool kAllMassless>
-#ifndef BZ_PAPER_MINB
-#define BZ_PAPER_MINB 2
-#endif
-__global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : BZ_PAPER_MINB) paper_queue_kernel(const __grid_constant__ PaperParams P)
+__global__ void __launch_bounds__(32 * kQWarps, kAllMassless ? 1 : 2) paper_queue_kernel(const __grid_constant__ PaperParams P)
 {
     extern __shared__ __align__(16) unsigned char paper_smem[];
     QWarp& q = reinterpret_cast<QWarp*>(paper_smem)[threadIdx.x >> 5];
@@ -635,14 +632,12 @@ __global__ void __launch_bounds__(256) combine_kernel(const double* __restrict__
 
 cudaError_t launch_combine(const double* f, double* out, const double* dFc, size_t n_values, cudaStream_t st)
 {
-    combine_kernel<<<148 * 8, 256, 0, st>>>(f, out, dFc, n_values);
+    combine_kernel<<<device_sms() * 8, 256, 0, st>>>(f, out, dFc, n_values);
     ++g_launch_count;
     return cudaGetLastError();
 }
 
-#ifndef BZ_PAPER_GROUPS
-#define BZ_PAPER_GROUPS 8
-#endif
+constexpr int kPaperGroupsMax = 8;       // groups of CTAs at most (16 and 32 measured slower)
 cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
 {
     const long long total = (long long)P.x_count * P.p_count * P.Ns;
@@ -668,10 +663,10 @@ cudaError_t launch_paper_collide(const PaperParams& P, int sms, cudaStream_t st)
     if (per_sm < 1) per_sm = 1;
     long long blocks = (total / 32 + kQWarps) / kQWarps;
     if (blocks > (long long)sms * per_sm) blocks = (long long)sms * per_sm;
-    // groups of CTAs: as many as 8 (BZ_PAPER_GROUPS), but no idle groups in the last round of cells beyond 1/8 of the work
+    // groups of CTAs: as many as kPaperGroupsMax, but no idle groups in the last round of cells beyond 1/8 of the work
     PaperParams Q = P;
     int best = 1;
-    for (int g = 1; g <= BZ_PAPER_GROUPS && g <= P.x_count && g <= (int)blocks; ++g) {
+    for (int g = 1; g <= kPaperGroupsMax && g <= P.x_count && g <= (int)blocks; ++g) {
         const int rounds = (P.x_count + g - 1) / g;
         if ((long long)rounds * g * 7 <= (long long)P.x_count * 8) best = g;
     }

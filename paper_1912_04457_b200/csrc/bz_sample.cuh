@@ -20,11 +20,8 @@ struct GridConst {          // S8c step 0, computed once on the host in fp64
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
                                               uint32_t k1, uint32_t (&out)[4])
 {
-#ifndef BZ_PHILOX_ROUNDS
-#define BZ_PHILOX_ROUNDS 10
-#endif
 #pragma unroll
-    for (int r = 0; r < BZ_PHILOX_ROUNDS; ++r) {
+    for (int r = 0; r < 10; ++r) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
         const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
         c1 = (uint32_t)p1; c3 = (uint32_t)p0; c0 = n0; c2 = n2;
@@ -123,17 +120,6 @@ __device__ __forceinline__ Sample gen_sample_words(const GridConst& g, const uin
 {
     Sample o;
     o.flag = 0; o.retry = 0; o.k = -1; o.l = -1; o.s = 0.0; o.t = 0.0; o.u = 0.0; o.w = 1.0;
-#if defined(BZ_ABLATE) && BZ_ABLATE == 5
-    {   // measurement build (profiles/r2_collide_ablation.md): no sampling arithmetic, the same acceptance and retry rates
-        const unsigned n3 = (unsigned)(g.n * g.n * g.n);
-        o.j = (int)(w0[0] % n3); o.k = (int)(w0[1] % n3); o.l = (int)(w0[2] % n3);
-        o.retry = wa[0] < 197568495u && kstart < 60u;         // 0.046
-        o.flag = !o.retry && w1[0] < 1971389988u;             // 0.459
-        o.s = 1.0 + (double)(w1[1] >> 8) * 1e-7; o.t = -0.5 * o.s; o.u = -0.5 * o.s; o.E1E2 = 1.0 + p1x * p1y + p1z + E1;
-        if (!o.flag) o.k = -1;
-        return o;
-    }
-#endif
     const double L52 = g.L * 2.220446049250313e-16;       // L 2^-52, exact
     const double p2x = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[0], w0[1]), L52));
     const double p2y = __dadd_rn(g.pmin, __dmul_rn(uniform52_scaled(w0[2], w0[3]), L52));

@@ -9,11 +9,8 @@ namespace {
 // One thread per (xcell, pcell), looping over the species: f is read and written coalesced in pcell for every
 // species, the collision deposits of the cell come from the cell-major scratch (64 contiguous bytes per thread).  Upwind flux form of the drift term of Eq. 13:
 // dF = - sum_d [ max(c_d,0) (f(x) - f(x - e_d)) + min(c_d,0) (f(x + e_d) - f(x)) ],  c_d = v_d dt/dx, periodic.
-#ifndef BZ_TR_MINB
-#define BZ_TR_MINB 4
-#endif
 template <int kMode>
-__global__ void __launch_bounds__(256, BZ_TR_MINB) transport_kernel(const TransportParams P)
+__global__ void __launch_bounds__(256, 4) transport_kernel(const TransportParams P)
 {
     // blockIdx.x = spatial cell (fastest), blockIdx.y = chunk of 256 momentum cells: the blocks in flight share one
     // momentum chunk of ALL spatial cells (Nx x S x 2 KB, 58 MB for config 4), which fits L2, so the three upwind
@@ -170,7 +167,8 @@ cudaError_t launch_moments(const double* rowsum, double* mom, int Nx, int S, con
                            double mD2, double d3p_over_2pi3, double d3x, int x_begin, int x_end, cudaStream_t st)
 {
     int blocks = (Nx * S + 255) / 256;
-    if (blocks > 148) blocks = 148;
+    const int sms = device_sms();
+    if (blocks > sms) blocks = sms;
     if (blocks < 2 * S) blocks = 2 * S;          // one block per total
     moments_kernel<<<blocks, 256, 0, st>>>(rowsum, mom, Nx, S, glue_slot_mask, g2, mD2, d3p_over_2pi3, d3x, x_begin, x_end, deg[0], deg[1], deg[2], deg[3], deg[4],
                                            deg[5], deg[6]);

@@ -472,6 +472,39 @@ def test_msq_override_parity(species, ovr):
     _assert_dF(g.collision(cfg.dt, 1).cpu().numpy(), o.collision(cfg.dt, 1), o.gross(), "restored")
 
 
+def test_msq_sign_counts_against_the_oracle_channel_by_channel():
+    """bz_msq_sign_counts (reading S8: the regulated Table I is evaluated literally and can be negative): the counters of
+    every (kind, ordering) against the oracle, which evaluates bzo_msq for every depositing sample of the cells, and the
+    (sample, channel) pair fraction that bench.py reports against a plain loop over the oracle's 127 ordered channels."""
+    cfg = wl.scaled(wl.CONFIGS[3], nx=2, np_=8, samples=12)
+    o, g = _pair(cfg)
+    f = wl.initial_f(cfg) + 0.05 * wl.random_f(cfg, seed=59)
+    o.set_f(f)
+    g.set_f(f)
+    m2 = np.asarray(o.moments()["m2"])
+    g4 = (4.0 * np.pi * cfg.alpha_s) ** 2
+    step, xb, xe = 4, 1, 7
+    acc_o, neg_o = 0, np.zeros((7, 2), dtype=np.int64)
+    for x in range(xb, xe):
+        cells, stu = o.debug_samples(step, x, 0, cfg.Np)
+        for (s_, t_, u_) in stu[cells[..., 3] == 1]:
+            acc_o += 1
+            for kind in range(7):
+                neg_o[kind, 0] += bzo.msq(kind, s_, t_, u_, m2[x], g4) < 0.0
+                neg_o[kind, 1] += bzo.msq(kind, s_, u_, t_, m2[x], g4) < 0.0
+    acc_g, neg_g = g.msq_sign_counts(step, xb, xe)
+    assert acc_g == acc_o and acc_o > 1000
+    assert np.array_equal(np.asarray(neg_g), neg_o)
+    assert neg_o[4].min() > 0                                             # q qbar <-> g g does go negative (S8's example)
+    # pair fraction: channel multiplicities from the product's table against the oracle's channel list, one by one
+    mult = np.zeros((7, 2), dtype=np.int64)
+    for row in bz.debug_paper_channels(cfg.species):
+        mult[row[4], row[5]] += 1
+    pairs_o = sum(neg_o[ch[4], ch[5]] for ch in o.channels())
+    assert len(o.channels()) == mult.sum() == 127
+    assert int((mult * np.asarray(neg_g)).sum()) == int(pairs_o)
+
+
 # ------------------------------------------------- NEXT rank 2: thermal masses (Eq. 8-9) and Eq. 15 (drift + force)
 VLASOV_CASES = [
     wl.scaled(wl.CONFIGS[3], nx=3, np_=10, samples=8),                 # 7 species, 27 spatial cells
