@@ -201,7 +201,8 @@ static void gen_sample(const bzo_ctx* c, unsigned step, int xcell, int pcell, in
 int bzo_sample_one(const bzo_ctx* c, unsigned step, int xcell, int pcell, int sample, bzo_sample* out)
 {
     if (!c || !out || xcell < 0 || xcell >= c->Nx || pcell < 0 || pcell >= c->Np || sample < 0) return -1;
-    gen_sample(c, step, xcell, pcell, sample, out);
+    /* the Philox spatial counter of local cell x is x + the slab offset (bzo_set_slab), as in bzo_collision / bzo_debug_samples */
+    gen_sample(c, step, (int)((unsigned)xcell + c->xoff), pcell, sample, out);
     return 0;
 }
 

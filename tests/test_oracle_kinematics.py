@@ -79,3 +79,22 @@ def test_acceptance_fraction_uniform_box():
     cells, _ = o.debug_samples(0, 0, 0, o.Np)
     frac = cells[..., 3].mean()
     assert 0.40 < frac < 0.52
+
+
+def test_sample_one_honours_the_slab_offset_like_debug_samples():
+    """bzo_set_slab: local cell x draws the samples of global cell x + offset in every entry point that samples (S8e: the Philox
+    spatial counter is the cell's index in the undecomposed domain) -- bzo_sample_one included."""
+    kw = dict(np_=8, pmin=-3.0, pmax=3.0, species=(0,), seed=5, samples=6)
+    whole = bzo.Oracle(nx=1, ny=1, nz=4, **kw)
+    part = bzo.Oracle(nx=1, ny=1, nz=2, **kw)
+    part.set_slab(2, 0, 2)                                   # local cells 0, 1 = global cells 2, 3
+    cells_w, stu_w = whole.debug_samples(3, 3, 100, 104)
+    cells_p, stu_p = part.debug_samples(3, 1, 100, 104)
+    assert np.array_equal(cells_w, cells_p) and np.array_equal(stu_w.view(np.uint64), stu_p.view(np.uint64))
+    for k, pc in enumerate(range(100, 104)):
+        for smp in range(6):
+            a, b = whole.sample_one(3, 3, pc, smp), part.sample_one(3, 1, pc, smp)
+            assert (a.j, a.k, a.l, a.flag) == (b.j, b.k, b.l, b.flag) == tuple(cells_w[k, smp])
+            assert (a.s, a.t, a.u) == (b.s, b.t, b.u)
+    c = whole.sample_one(3, 1, 100, 0)
+    assert (c.s, c.t, c.u) != (part.sample_one(3, 1, 100, 0).s, part.sample_one(3, 1, 100, 0).t, part.sample_one(3, 1, 100, 0).u)
