@@ -41,6 +41,26 @@ def test_library_exports_every_declared_symbol():
     assert not hasattr(L, "bz_debug_deposit_host")      # the host evaluation of the channel algebra is a test-only object
 
 
+def test_moments_noalloc_checks_its_arguments_before_touching_the_device():
+    """bz_moments_noalloc (include/bz.h): bad arguments (-1) and grids beyond the fixed scratch (-5, with a message that names
+    both numbers) are refused on the host, before any CUDA call -- so this runs without a GPU."""
+    L = bz.lib()
+    buf = (C.c_double * 8)()
+    ptr = C.cast(buf, C.c_void_p)
+    sp7 = (C.c_int * 7)(0, 1, 2, 3, 4, 5, 6)
+    big = bz.Grid(22, 22, 22, 0.1, 4, -2.0, 2.0)                      # 10648 cells x 7 species = 74536 rows > 65536
+    assert L.bz_moments_noalloc(C.byref(big), sp7, 7, 0.3, 0.0, ptr, ptr, None) == -5
+    msg = L.bz_noalloc_last_error().decode()
+    assert "74536" in msg and str(bz.NOALLOC_MAX_ROWS) in msg
+    ok = bz.Grid(2, 2, 2, 0.1, 4, -2.0, 2.0)
+    assert L.bz_moments_noalloc(C.byref(ok), sp7, 7, 0.3, 0.0, None, ptr, None) == -1          # no input
+    assert L.bz_moments_noalloc(C.byref(ok), sp7, 7, 0.3, 0.0, ptr, None, None) == -1          # no output
+    assert L.bz_moments_noalloc(C.byref(ok), sp7, 7, -0.3, 0.0, ptr, ptr, None) == -1          # alpha_s <= 0
+    assert L.bz_moments_noalloc(C.byref(ok), (C.c_int * 2)(3, 3), 2, 0.3, 0.0, ptr, ptr, None) == -1   # not ascending
+    assert L.bz_moments_noalloc(C.byref(bz.Grid(2, 2, 2, 0.1, 1, -2.0, 2.0)), sp7, 7, 0.3, 0.0, ptr, ptr, None) == -1   # np < 2
+    assert L.bz_noalloc_last_error().decode() != ""
+
+
 def test_bad_arguments_are_rejected_without_a_device():
     L = bz.lib()
     h = C.c_void_p()
